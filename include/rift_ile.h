@@ -1,0 +1,141 @@
+/*
+ * rift_ile.h -- C ABI of the ILE extrinsic-marginalised factored likelihood on one B200 (sm_100a).
+ *
+ * The operation is the inner evaluation of RIFT's ILE worker (arXiv 2210.07912; citations below are
+ * line numbers of /root/reference/PAPER.md, readings "A#/G#" are listed in DESIGN.md section 3):
+ *
+ *   L(lambda) = int L_full(lambda, theta) p(theta) dtheta                         Eq. (1), :37
+ *            ~= (1/N) sum_i L_full(lambda, theta_i) p(theta_i)/p_s(theta_i)        Eq. (3), :55
+ *   ln L_full = (D_ref/D) Re sum_k sum_lm (F_k Y_lm)^* Q_{k,lm}(t_k)               Eq. (D2), :763
+ *             - (D_ref/D)^2/4 sum_k sum_{lm,l'm'} [ |F_k|^2 Y_lm^* Y_l'm' U_{k,lm,l'm'}
+ *                                                   + Re(F_k^2 Y_lm Y_l'm' V_{k,lm,l'm'}) ]   Eq. (D3), :766
+ *   with Q, U, V the mode/data inner products of Eq. (D4a-c), :771-776, held fixed per intrinsic
+ *   point lambda; Y_lm = -2Y_lm(iota, -phi_ref); F_k = F+ + i Fx; t_k = t_ref + dt_k + tau with dt_k
+ *   the geocentre-to-detector delay rounded to the nearest Q sample; the time tau is marginalised
+ *   over the window with a logsumexp (App. D.2, :801); n_eff etc. are Eq. (B1)-(B3), :637-646; the
+ *   per-parameter sampling weights are the weighted histograms behind Eq. (22), :348.
+ *
+ * Every step runs in hand-written CUDA kernels; there is no CPU fallback.  All functions return
+ * RIFT_OK (0) or a negative error code and never throw.  On error, outputs are untouched.
+ * Units: radians, seconds, metres, Mpc.  A handle is bound to the CUDA device that is current when
+ * it is created and is not thread-safe; distinct handles are independent.
+ */
+#ifndef RIFT_ILE_H
+#define RIFT_ILE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rift_ile rift_ile_t;   /* opaque */
+
+enum {
+  RIFT_OK = 0,
+  RIFT_EINVAL = -1,   /* bad argument (null pointer, size out of range, duplicate mode, ...) */
+  RIFT_ENOMEM = -2,   /* host or device allocation failed */
+  RIFT_ECUDA = -3,    /* a CUDA runtime call or kernel launch failed; see rift_ile_last_error */
+  RIFT_EWINDOW = -4,  /* n_tau < n_t but n_tau + 2*S_max > n_t (the guard band would wrap) */
+  RIFT_ERANGE = -5,   /* intrinsic id outside [0, n_points) */
+  RIFT_ESTATE = -6    /* reduce(merge=1) with a different n_seg / n_bins than the stored state */
+};
+
+enum { RIFT_PREC_FP64 = 0, RIFT_PREC_MIXED = 1 };   /* arithmetic of the window term (reading A17) */
+enum { RIFT_Q_C128 = 0, RIFT_Q_C64 = 1 };           /* storage of Q on the device */
+enum { RIFT_MEM_HOST = 0, RIFT_MEM_DEVICE = 1 };    /* where the Q/U/V arrays passed to create live */
+enum { RIFT_KERNEL_AUTO = 0, RIFT_KERNEL_DIRECT = 1, RIFT_KERNEL_TILED = 2 };   /* rift_ile_set_kernel */
+
+#define RIFT_MAX_DET 8
+#define RIFT_MAX_MODES 80
+#define RIFT_N_PARAMS 6   /* ra, dec, psi, iota, phi_ref, dist_mpc -- the extrinsic sample */
+
+typedef struct {
+  int32_t n_det;                  /* K, 1..RIFT_MAX_DET */
+  const double *det_location_m;   /* host [n_det][3]: Earth-fixed position, metres */
+  const double *det_response;     /* host [n_det][3][3]: response tensor D_k = (x x^T - y y^T)/2 */
+  double gmst_rad;                /* Greenwich mean sidereal time, one value per handle (reading A16) */
+  int32_t n_modes;                /* M, 1..RIFT_MAX_MODES */
+  const int32_t *mode_l;          /* host [n_modes], 2 <= l <= 8 */
+  const int32_t *mode_m;          /* host [n_modes], |m| <= l, no duplicate (l,m) */
+  int32_t n_points;               /* P >= 1 intrinsic points */
+  int32_t n_t;                    /* stored Q samples per (point, detector, mode); centre sample (n_t-1)/2 = t_ref */
+  double delta_t;                 /* Q sample spacing, seconds (> 0) */
+  int32_t n_tau;                  /* marginalisation samples, 1..n_t, n_t - n_tau even; n_tau == n_t: circular (A4) */
+  double d_ref_mpc;               /* reference distance D_ref of Eq. (D2)-(D3), > 0 */
+  const void *Q;                  /* [P][K][M][n_t] complex128 interleaved; host or device per input_mem */
+  const void *U;                  /* [P][K][M][M]   complex128, Hermitian in the mode indices */
+  const void *V;                  /* [P][K][M][M]   complex128, symmetric in the mode indices */
+  int32_t input_mem;              /* RIFT_MEM_HOST | RIFT_MEM_DEVICE (applies to Q, U, V) */
+  int32_t precision;              /* RIFT_PREC_FP64 | RIFT_PREC_MIXED */
+  int32_t q_storage;              /* RIFT_Q_C128 | RIFT_Q_C64; FP64 precision requires C128 */
+} rift_ile_config;
+
+/* Create a handle: validates cfg, builds the per-mode harmonic tables, copies (and for C64 storage
+ * converts) Q/U/V to device memory owned by the handle.  Nothing in cfg is referenced afterwards.
+ * Synchronous.  *out is written only on success. */
+int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out);
+
+/* Time-marginalised lnL of every extrinsic sample (steps a1-a7 of DESIGN.md section 1).
+ *   n_seg, intrinsic_ids : HOST [n_seg]; segment s uses Q/U/V of point intrinsic_ids[s].
+ *   n_per_seg            : samples per segment (>= 0).
+ *   params               : HOST array of 6 DEVICE pointers (ra, dec, psi, iota, phi_ref, dist_mpc), each
+ *                          fp64 [n_seg*n_per_seg], segment-major.
+ *   lnL_out              : DEVICE fp64 [n_seg*n_per_seg]:
+ *                            ln[(1/n_tau) sum_j exp(lnL(tau_j))],  tau_j over the window (readings A4, A5).
+ *                          dist <= 0 or a NaN parameter gives NaN for that sample only.
+ *   shift_out            : DEVICE int32 [n_seg*n_per_seg][n_det] or NULL: s_k = floor(dt_k/delta_t + 1/2) (G4).
+ *   cuda_stream          : a cudaStream_t (NULL = legacy default stream).  Asynchronous on that stream. */
+int rift_ile_eval_batch(rift_ile_t *h, int32_t n_seg, const int32_t *intrinsic_ids, int64_t n_per_seg,
+                        const double *const params[RIFT_N_PARAMS], double *lnL_out, int32_t *shift_out,
+                        void *cuda_stream);
+
+/* Sample-axis reduce (step a8): per segment, with ln omega_i = lnL_i + ln_weight_i,
+ *   lnZ = ln[(1/N) sum omega_i]  (Eq. (3));  n_eff = sum omega / max omega  (B1);
+ *   n_ess = (sum omega)^2 / sum omega^2  (B2);  rel_err^2 = (N/n_ess - 1)/(N - 1)  (B3, reading A20);
+ *   hist[s][d][b] = sum_{i in bin b of parameter d} omega_i / sum omega, b = floor(n_bins (x-lo)/(hi-lo))
+ *   clamped to [0, n_bins-1]  (Eq. (22), reading A13).
+ *   lnL, ln_weight (NULL = 0), params (NULL or 6 device pointers; needed only for hist) : DEVICE.
+ *   lo, hi : HOST [6].  merge = 0 resets the handle's per-segment state, 1 pools this call with the state
+ *   left by earlier calls (Eq. (20)-(21)); outputs always describe the pooled state.
+ *   lnZ, rel_err, n_eff, n_ess : HOST [n_seg];  hist : HOST [n_seg][6][n_bins] or NULL.
+ * Synchronises cuda_stream before returning (host outputs). */
+int rift_ile_reduce(rift_ile_t *h, int32_t n_seg, int64_t n_per_seg, const double *lnL, const double *ln_weight,
+                    const double *const params[RIFT_N_PARAMS], const double lo[RIFT_N_PARAMS],
+                    const double hi[RIFT_N_PARAMS], int32_t n_bins, int32_t merge, double *lnZ, double *rel_err,
+                    double *n_eff, double *n_ess, double *hist, void *cuda_stream);
+
+/* Inspection of the geometry kernel (steps a1-a5) in fp64 for n samples of ONE intrinsic point.
+ * All outputs DEVICE, any may be NULL: F [n][n_det] complex128 (F+ + i Fx); Y [n][n_modes] complex128
+ * (-2Y_lm(iota,-phi_ref)); shift [n][n_det] int32; quad [n] fp64 (the U/V term of Eq. (D3) including
+ * (D_ref/D)^2/4).  Asynchronous on cuda_stream. */
+int rift_ile_geometry(rift_ile_t *h, int32_t intrinsic_id, int64_t n, const double *const params[RIFT_N_PARAMS],
+                      void *F, void *Y, int32_t *shift, double *quad, void *cuda_stream);
+
+/* Choose the fused-lnL kernel variant (RIFT_KERNEL_*); AUTO picks per configuration. */
+int rift_ile_set_kernel(rift_ile_t *h, int32_t variant);
+
+/* Number of kernels launched by this handle since creation (bench.py's gpu_launches), and the name of
+ * the fused kernel variant the last eval_batch used. */
+int64_t rift_ile_launch_count(const rift_ile_t *h);
+const char *rift_ile_kernel_name(const rift_ile_t *h);
+
+/* Per-kernel device timing for bench.py's roofline: while enabled, every geometry / fused-lnL / reduce launch is
+ * bracketed by CUDA events on its stream.  rift_ile_profile_read synchronises those events, returns the summed
+ * milliseconds and launch counts per kernel family since the last read ([0] geometry, [1] fused lnL, [2] reduce),
+ * and clears them. */
+int rift_ile_profile(rift_ile_t *h, int32_t enable);
+int rift_ile_profile_read(rift_ile_t *h, double ms[3], int64_t launches[3]);
+
+/* Dense FMA-pipe microbenchmark (hard part H7): runs `iters` dependent-free FMA per thread over a grid
+ * filling the device and returns achieved TFLOP/s in *tflops (fp64 != 0 selects DFMA). */
+int rift_ile_fma_peak(int32_t fp64, int32_t iters, double *tflops, void *cuda_stream);
+
+int rift_ile_destroy(rift_ile_t *h);
+const char *rift_ile_strerror(int code);
+const char *rift_ile_last_error(const rift_ile_t *h);   /* never NULL; "" when no error was recorded */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RIFT_ILE_H */

@@ -1,0 +1,217 @@
+"""Thin ctypes binding of librift_ile.so (include/rift_ile.h).  Argument marshalling only: every step of
+the hot path runs in the CUDA kernels behind the C ABI.  PyTorch (if the caller uses it) only owns device
+memory and streams; this module accepts anything with ``data_ptr()`` or a raw integer address.
+
+There is no CPU fallback: if the shared library is missing or cannot be loaded, importing the functions
+raises.  Build it with ``python -m paper_2210_07912_b200.build``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "librift_ile.so")
+
+RIFT_OK, RIFT_EINVAL, RIFT_ENOMEM, RIFT_ECUDA, RIFT_EWINDOW, RIFT_ERANGE, RIFT_ESTATE = 0, -1, -2, -3, -4, -5, -6
+RIFT_PREC_FP64, RIFT_PREC_MIXED = 0, 1
+RIFT_Q_C128, RIFT_Q_C64 = 0, 1
+RIFT_MEM_HOST, RIFT_MEM_DEVICE = 0, 1
+RIFT_KERNEL_AUTO, RIFT_KERNEL_DIRECT, RIFT_KERNEL_TILED = 0, 1, 2
+RIFT_N_PARAMS = 6
+
+EXPORTS = ("rift_ile_create", "rift_ile_eval_batch", "rift_ile_reduce", "rift_ile_geometry", "rift_ile_set_kernel",
+           "rift_ile_launch_count", "rift_ile_kernel_name", "rift_ile_profile", "rift_ile_profile_read",
+           "rift_ile_fma_peak", "rift_ile_destroy",
+           "rift_ile_strerror", "rift_ile_last_error")
+
+
+class RiftError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"rift_ile error {code}: {msg}")
+        self.code = code
+
+
+class _Config(C.Structure):
+    _fields_ = [("n_det", C.c_int32), ("det_location_m", C.c_void_p), ("det_response", C.c_void_p),
+                ("gmst_rad", C.c_double), ("n_modes", C.c_int32), ("mode_l", C.c_void_p), ("mode_m", C.c_void_p),
+                ("n_points", C.c_int32), ("n_t", C.c_int32), ("delta_t", C.c_double), ("n_tau", C.c_int32),
+                ("d_ref_mpc", C.c_double), ("Q", C.c_void_p), ("U", C.c_void_p), ("V", C.c_void_p),
+                ("input_mem", C.c_int32), ("precision", C.c_int32), ("q_storage", C.c_int32)]
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load librift_ile.so; raises if it is missing (no fallback of any kind)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} not found: run `python -m paper_2210_07912_b200.build` (needs nvcc); "
+                              "there is no CPU fallback")
+        L = C.CDLL(LIB_PATH)
+        vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+        L.rift_ile_create.argtypes = [C.POINTER(_Config), C.POINTER(vp)]
+        L.rift_ile_create.restype = C.c_int
+        L.rift_ile_eval_batch.argtypes = [vp, i32, vp, i64, C.POINTER(vp), vp, vp, vp]
+        L.rift_ile_eval_batch.restype = C.c_int
+        L.rift_ile_reduce.argtypes = [vp, i32, i64, vp, vp, C.POINTER(vp), vp, vp, i32, i32, vp, vp, vp, vp, vp, vp]
+        L.rift_ile_reduce.restype = C.c_int
+        L.rift_ile_geometry.argtypes = [vp, i32, i64, C.POINTER(vp), vp, vp, vp, vp, vp]
+        L.rift_ile_geometry.restype = C.c_int
+        L.rift_ile_set_kernel.argtypes = [vp, i32]
+        L.rift_ile_set_kernel.restype = C.c_int
+        L.rift_ile_launch_count.argtypes = [vp]
+        L.rift_ile_launch_count.restype = i64
+        L.rift_ile_kernel_name.argtypes = [vp]
+        L.rift_ile_kernel_name.restype = C.c_char_p
+        L.rift_ile_profile.argtypes = [vp, i32]
+        L.rift_ile_profile.restype = C.c_int
+        L.rift_ile_profile_read.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
+        L.rift_ile_profile_read.restype = C.c_int
+        L.rift_ile_fma_peak.argtypes = [i32, i32, C.POINTER(dbl), vp]
+        L.rift_ile_fma_peak.restype = C.c_int
+        L.rift_ile_destroy.argtypes = [vp]
+        L.rift_ile_destroy.restype = C.c_int
+        L.rift_ile_strerror.argtypes = [C.c_int]
+        L.rift_ile_strerror.restype = C.c_char_p
+        L.rift_ile_last_error.argtypes = [vp]
+        L.rift_ile_last_error.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def _ptr(x) -> Optional[int]:
+    """Address of a device tensor / numpy array / raw int; None stays NULL."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return int(x.data_ptr())
+    if isinstance(x, np.ndarray):
+        return int(x.ctypes.data)
+    raise TypeError(type(x))
+
+
+def _check(rc: int, h=None):
+    if rc != RIFT_OK:
+        msg = lib().rift_ile_strerror(rc).decode()
+        if h:
+            detail = lib().rift_ile_last_error(h).decode()
+            if detail:
+                msg = f"{msg} ({detail})"
+        raise RiftError(rc, msg)
+
+
+def _params6(params) -> "C.Array":
+    """params: a [6][N] device tensor or a sequence of six device arrays (fp64, contiguous)."""
+    ptrs = []
+    if hasattr(params, "data_ptr") and not isinstance(params, (list, tuple)):
+        if params.shape[0] != 6:
+            raise ValueError("params must be [6][N]")
+        for d in range(6):
+            row = params[d]
+            if hasattr(row, "is_contiguous") and not row.is_contiguous():
+                raise ValueError("params rows must be contiguous")
+            ptrs.append(_ptr(row))
+    else:
+        if len(params) != 6:
+            raise ValueError("params must have six entries")
+        ptrs = [_ptr(p) for p in params]
+    return (C.c_void_p * 6)(*ptrs)
+
+
+def rift_ile_strerror(code: int) -> str:
+    return lib().rift_ile_strerror(int(code)).decode()
+
+
+def rift_ile_last_error(h) -> str:
+    return lib().rift_ile_last_error(h).decode()
+
+
+def rift_ile_create(det_location_m, det_response, gmst_rad: float, mode_l, mode_m, n_points: int, n_t: int,
+                    delta_t: float, n_tau: int, d_ref_mpc: float, Q, U, V, input_mem: int = RIFT_MEM_HOST,
+                    precision: int = RIFT_PREC_FP64, q_storage: Optional[int] = None):
+    """Returns an opaque handle (ctypes.c_void_p).  Q/U/V: numpy complex128 (host) or device tensors."""
+    loc = np.ascontiguousarray(det_location_m, dtype=np.float64)
+    resp = np.ascontiguousarray(det_response, dtype=np.float64)
+    ml = np.ascontiguousarray(mode_l, dtype=np.int32)
+    mm = np.ascontiguousarray(mode_m, dtype=np.int32)
+    keep = []
+    if input_mem == RIFT_MEM_HOST:
+        Q, U, V = (np.ascontiguousarray(a, dtype=np.complex128) for a in (Q, U, V))
+        keep = [Q, U, V]
+    if q_storage is None:
+        q_storage = RIFT_Q_C64 if precision == RIFT_PREC_MIXED else RIFT_Q_C128
+    cfg = _Config(int(loc.shape[0]), loc.ctypes.data, resp.ctypes.data, float(gmst_rad), int(ml.size), ml.ctypes.data,
+                  mm.ctypes.data, int(n_points), int(n_t), float(delta_t), int(n_tau), float(d_ref_mpc), _ptr(Q),
+                  _ptr(U), _ptr(V), int(input_mem), int(precision), int(q_storage))
+    h = C.c_void_p()
+    _check(lib().rift_ile_create(C.byref(cfg), C.byref(h)))
+    del keep
+    return h
+
+
+def rift_ile_destroy(h) -> None:
+    _check(lib().rift_ile_destroy(h))
+
+
+def rift_ile_eval_batch(h, intrinsic_ids: Sequence[int], n_per_seg: int, params, lnL_out, shift_out=None,
+                        cuda_stream: int = 0) -> None:
+    ids = np.ascontiguousarray(intrinsic_ids, dtype=np.int32)
+    _check(lib().rift_ile_eval_batch(h, int(ids.size), ids.ctypes.data, int(n_per_seg), _params6(params), _ptr(lnL_out),
+                                     _ptr(shift_out), int(cuda_stream) or None), h)
+
+
+def rift_ile_geometry(h, intrinsic_id: int, n: int, params, F=None, Y=None, shift=None, quad=None,
+                      cuda_stream: int = 0) -> None:
+    _check(lib().rift_ile_geometry(h, int(intrinsic_id), int(n), _params6(params), _ptr(F), _ptr(Y), _ptr(shift),
+                                   _ptr(quad), int(cuda_stream) or None), h)
+
+
+def rift_ile_reduce(h, n_seg: int, n_per_seg: int, lnL, ln_weight=None, params=None, lo=None, hi=None,
+                    n_bins: int = 0, merge: int = 0, want_hist: bool = False, cuda_stream: int = 0) -> dict:
+    """Returns dict(lnZ, rel_err, n_eff, n_ess [n_seg] numpy fp64, hist [n_seg][6][n_bins] or None)."""
+    out = [np.empty(n_seg, dtype=np.float64) for _ in range(4)]
+    hist = np.empty((n_seg, 6, n_bins), dtype=np.float64) if want_hist else None
+    lo_ = None if lo is None else np.ascontiguousarray(lo, dtype=np.float64)
+    hi_ = None if hi is None else np.ascontiguousarray(hi, dtype=np.float64)
+    _check(lib().rift_ile_reduce(h, int(n_seg), int(n_per_seg), _ptr(lnL), _ptr(ln_weight),
+                                 None if params is None else _params6(params), _ptr(lo_), _ptr(hi_), int(n_bins),
+                                 int(merge), *[o.ctypes.data for o in out], _ptr(hist), int(cuda_stream) or None), h)
+    return dict(lnZ=out[0], rel_err=out[1], n_eff=out[2], n_ess=out[3], hist=hist)
+
+
+def rift_ile_set_kernel(h, variant: int) -> None:
+    _check(lib().rift_ile_set_kernel(h, int(variant)), h)
+
+
+def rift_ile_launch_count(h) -> int:
+    return int(lib().rift_ile_launch_count(h))
+
+
+def rift_ile_kernel_name(h) -> str:
+    return lib().rift_ile_kernel_name(h).decode()
+
+
+def rift_ile_profile(h, enable: bool) -> None:
+    _check(lib().rift_ile_profile(h, int(bool(enable))), h)
+
+
+def rift_ile_profile_read(h) -> dict:
+    """dict(ms=[geometry, lnl, reduce], launches=[...]) summed since the last read."""
+    ms = (C.c_double * 3)()
+    nl = (C.c_int64 * 3)()
+    _check(lib().rift_ile_profile_read(h, ms, nl), h)
+    return dict(ms=[float(x) for x in ms], launches=[int(x) for x in nl])
+
+
+def rift_ile_fma_peak(fp64: bool, iters: int = 4096, cuda_stream: int = 0) -> float:
+    v = C.c_double()
+    _check(lib().rift_ile_fma_peak(int(bool(fp64)), int(iters), C.byref(v), int(cuda_stream) or None))
+    return float(v.value)

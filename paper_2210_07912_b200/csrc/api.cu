@@ -1,0 +1,523 @@
+// C ABI of librift_ile.so (include/rift_ile.h): handle management, argument validation, chunking, launches.
+// Host logic only -- every step of the hot path runs in the kernels of geometry.cu, lnl_*.cu and reduce.cu.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "rift_internal.h"
+
+struct rift_ile {
+  int device = 0, n_sm = 0;
+  int P = 0, K = 0, M = 0, n_t = 0, n_tp = 0, n_tau = 0;
+  int precision = 0, q_storage = 0;
+  DetGeom geom{};
+  ModeEntry *d_modes = nullptr;
+  void *d_Q = nullptr;
+  double *d_U = nullptr, *d_V = nullptr;
+  QStore qs{};
+  // per-chunk workspace
+  int64_t ws_cap = 0;
+  Workspace ws{};
+  int32_t *d_ids = nullptr;
+  int64_t ids_cap = 0;
+  // reduce state
+  ReduceState *d_state = nullptr;
+  double *d_state_hist = nullptr;
+  int state_nseg = 0, state_nbins = -1;
+  double *d_partial = nullptr;
+  size_t partial_cap = 0;
+  double *d_out = nullptr, *h_out = nullptr;
+  size_t out_cap = 0;
+  // bookkeeping
+  int kernel_variant = RIFT_KERNEL_AUTO;
+  const char *kernel_name = "none";
+  int64_t launches = 0;
+  char err[512] = {0};
+  // optional per-kernel event timing (rift_ile_profile)
+  bool profiling = false;
+  struct Span { cudaEvent_t a, b; int kind; };
+  std::vector<Span> spans;
+};
+
+namespace {
+
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = (cudaSetDevice(dev) == cudaSuccess);
+  }
+  ~DeviceGuard() {
+    if (switched) cudaSetDevice(prev);
+  }
+};
+
+int fail(rift_ile *h, int code, const char *what, cudaError_t ce = cudaSuccess) {
+  if (h) {
+    if (ce != cudaSuccess)
+      snprintf(h->err, sizeof(h->err), "%s: %s", what, cudaGetErrorString(ce));
+    else
+      snprintf(h->err, sizeof(h->err), "%s", what);
+  }
+  return code;
+}
+
+#define CU(h, call)                                                   \
+  do {                                                                \
+    cudaError_t e__ = (call);                                         \
+    if (e__ != cudaSuccess) {                                         \
+      cudaGetLastError();                                             \
+      return fail(h, e__ == cudaErrorMemoryAllocation ? RIFT_ENOMEM : RIFT_ECUDA, #call, e__); \
+    }                                                                 \
+  } while (0)
+
+// RAII-less helper: record an event pair around a launch when profiling is on
+struct ProfSpan {
+  rift_ile *h;
+  cudaStream_t s;
+  rift_ile::Span sp{};
+  bool on = false;
+  ProfSpan(rift_ile *h_, int kind, cudaStream_t s_) : h(h_), s(s_) {
+    if (h->profiling && cudaEventCreate(&sp.a) == cudaSuccess) {
+      if (cudaEventCreate(&sp.b) == cudaSuccess) {
+        sp.kind = kind;
+        on = true;
+        cudaEventRecord(sp.a, s);
+      } else {
+        cudaEventDestroy(sp.a);
+      }
+    }
+  }
+  void end() {
+    if (on) {
+      cudaEventRecord(sp.b, s);
+      h->spans.push_back(sp);
+      on = false;
+    }
+  }
+};
+
+double factorial(int n) {
+  double f = 1.0;
+  for (int i = 2; i <= n; ++i) f *= i;
+  return f;
+}
+
+// Term table of -2Y_lm (reading G3): coefficient, power of cos(theta/2), power of sin(theta/2).
+void build_mode(int l, int m, ModeEntry &e) {
+  memset(&e, 0, sizeof(e));
+  e.l = l;
+  e.m = m;
+  const int k0 = (m - 2 > 0) ? m - 2 : 0;
+  const int k1 = (l + m < l - 2) ? l + m : l - 2;
+  const long double pref = sqrtl((long double)factorial(l + m) * factorial(l - m) * factorial(l + 2) * factorial(l - 2)) *
+                           sqrtl((2.0L * l + 1.0L) / (4.0L * 3.14159265358979323846264338327950288L));
+  int n = 0;
+  for (int k = k0; k <= k1; ++k, ++n) {
+    const long double den = (long double)factorial(l + m - k) * factorial(l - 2 - k) * factorial(k) * factorial(k - m + 2);
+    e.coef[n] = (double)(((k & 1) ? -1.0L : 1.0L) * pref / den);
+    e.pc[n] = 2 * l + m - 2 - 2 * k;
+    e.ps[n] = 2 * k - m + 2;
+  }
+  e.n_terms = n;
+}
+
+void free_handle(rift_ile *h) {
+  if (!h) return;
+  for (auto &sp : h->spans) {
+    cudaEventDestroy(sp.a);
+    cudaEventDestroy(sp.b);
+  }
+  cudaFree(h->d_modes);
+  cudaFree(h->d_Q);
+  cudaFree(h->d_U);
+  cudaFree(h->d_V);
+  cudaFree(h->ws.coef);
+  cudaFree(h->ws.scale_c);
+  cudaFree(h->ws.quad);
+  cudaFree(h->ws.shift);
+  cudaFree(h->d_ids);
+  cudaFree(h->d_state);
+  cudaFree(h->d_state_hist);
+  cudaFree(h->d_partial);
+  cudaFree(h->d_out);
+  if (h->h_out) cudaFreeHost(h->h_out);
+  delete h;
+}
+
+size_t coef_bytes(const rift_ile *h) { return (size_t)h->K * h->M * (h->precision == RIFT_PREC_MIXED ? 8 : 16); }
+
+int ensure_workspace(rift_ile *h, int64_t n) {
+  if (n <= h->ws_cap) return RIFT_OK;
+  cudaFree(h->ws.coef);
+  cudaFree(h->ws.scale_c);
+  cudaFree(h->ws.quad);
+  cudaFree(h->ws.shift);
+  h->ws = Workspace{};
+  h->ws_cap = 0;
+  CU(h, cudaMalloc(&h->ws.coef, (size_t)n * coef_bytes(h)));
+  CU(h, cudaMalloc(&h->ws.scale_c, (size_t)n * sizeof(double)));
+  CU(h, cudaMalloc(&h->ws.quad, (size_t)n * sizeof(double)));
+  CU(h, cudaMalloc(&h->ws.shift, (size_t)n * h->K * sizeof(int32_t)));
+  h->ws_cap = n;
+  return RIFT_OK;
+}
+
+int upload_ids(rift_ile *h, int32_t n_seg, const int32_t *ids, cudaStream_t s) {
+  for (int32_t i = 0; i < n_seg; ++i)
+    if (ids[i] < 0 || ids[i] >= h->P) return fail(h, RIFT_ERANGE, "intrinsic id outside [0, n_points)");
+  if (n_seg > h->ids_cap) {
+    cudaFree(h->d_ids);
+    h->d_ids = nullptr;
+    h->ids_cap = 0;
+    CU(h, cudaMalloc(&h->d_ids, (size_t)n_seg * sizeof(int32_t)));
+    h->ids_cap = n_seg;
+  }
+  CU(h, cudaMemcpyAsync(h->d_ids, ids, (size_t)n_seg * sizeof(int32_t), cudaMemcpyHostToDevice, s));
+  return RIFT_OK;
+}
+
+// chunk size in samples: keep the per-chunk workspace near 64 MiB so that it lives in the 126 MB L2
+int64_t chunk_samples(const rift_ile *h) {
+  const size_t per = coef_bytes(h) + 16 + 4 * (size_t)h->K;
+  int64_t n = (int64_t)((64u << 20) / per);
+  if (n < 65536) n = 65536;
+  return n;
+}
+
+bool q_fits_smem(const rift_ile *h) {
+  const bool fp32 = h->precision == RIFT_PREC_MIXED;
+  return lnl_direct_smem_bytes(h->qs, fp32, true) <= 227u * 1024u;
+}
+
+int run_chunks(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *const params[6], double *lnL_out,
+               int32_t *shift_out, double *dbg_F, double *dbg_Y, double *dbg_quad, cudaStream_t s) {
+  const int64_t total = (int64_t)n_seg * n_per_seg;
+  if (total == 0) return RIFT_OK;
+  const int64_t cap = chunk_samples(h);
+  int rc = ensure_workspace(h, total < cap ? total : cap);
+  if (rc != RIFT_OK) return rc;
+  const bool fp32 = h->precision == RIFT_PREC_MIXED;
+  const bool in_smem = q_fits_smem(h);
+  for (int64_t g0 = 0; g0 < total; g0 += cap) {
+    Batch b;
+    b.n_per_seg = n_per_seg;
+    b.g0 = g0;
+    b.n = (total - g0 < cap) ? total - g0 : cap;
+    b.ids = h->d_ids;
+    {
+      ProfSpan ps(h, 0, s);
+      CU(h, launch_geometry(h->geom, h->d_modes, b, params, h->d_U, h->d_V, fp32, h->ws, shift_out, dbg_F, dbg_Y, s));
+      ps.end();
+    }
+    ++h->launches;
+    if (dbg_quad) CU(h, cudaMemcpyAsync(dbg_quad + g0, h->ws.quad, (size_t)b.n * sizeof(double), cudaMemcpyDeviceToDevice, s));
+    if (lnL_out) {
+      int nl = 0;
+      ProfSpan ps(h, 1, s);
+      CU(h, launch_lnl_direct(h->qs, fp32, in_smem, b, h->ws, h->K, lnL_out, h->n_sm, s, &nl));
+      ps.end();
+      h->launches += nl;
+      h->kernel_name = fp32 ? (in_smem ? "lnl_direct<f32,smem>" : "lnl_direct<f32,global>")
+                            : (in_smem ? "lnl_direct<f64,smem>" : "lnl_direct<f64,global>");
+    }
+  }
+  return RIFT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *rift_ile_strerror(int code) {
+  switch (code) {
+    case RIFT_OK: return "ok";
+    case RIFT_EINVAL: return "invalid argument";
+    case RIFT_ENOMEM: return "out of memory";
+    case RIFT_ECUDA: return "CUDA error";
+    case RIFT_EWINDOW: return "marginalisation window plus delay guard band exceeds the stored Q window";
+    case RIFT_ERANGE: return "intrinsic id out of range";
+    case RIFT_ESTATE: return "reduce state does not match (n_seg / n_bins changed under merge=1)";
+    default: return "unknown error";
+  }
+}
+
+const char *rift_ile_last_error(const rift_ile_t *h) { return h ? h->err : ""; }
+int64_t rift_ile_launch_count(const rift_ile_t *h) { return h ? h->launches : 0; }
+const char *rift_ile_kernel_name(const rift_ile_t *h) { return h ? h->kernel_name : "none"; }
+
+int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
+  if (!cfg || !out) return RIFT_EINVAL;
+  if (cfg->n_det < 1 || cfg->n_det > RIFT_MAX_DET || !cfg->det_location_m || !cfg->det_response) return RIFT_EINVAL;
+  if (cfg->n_modes < 1 || cfg->n_modes > RIFT_MAX_MODES || !cfg->mode_l || !cfg->mode_m) return RIFT_EINVAL;
+  if (cfg->n_points < 1 || cfg->n_t < 1 || !(cfg->delta_t > 0.0) || !(cfg->d_ref_mpc > 0.0)) return RIFT_EINVAL;
+  if (cfg->n_tau < 1 || cfg->n_tau > cfg->n_t || ((cfg->n_t - cfg->n_tau) & 1)) return RIFT_EINVAL;
+  if (!cfg->Q || !cfg->U || !cfg->V) return RIFT_EINVAL;
+  if (cfg->input_mem != RIFT_MEM_HOST && cfg->input_mem != RIFT_MEM_DEVICE) return RIFT_EINVAL;
+  if (cfg->precision != RIFT_PREC_FP64 && cfg->precision != RIFT_PREC_MIXED) return RIFT_EINVAL;
+  if (cfg->q_storage != RIFT_Q_C128 && cfg->q_storage != RIFT_Q_C64) return RIFT_EINVAL;
+  if (cfg->precision == RIFT_PREC_FP64 && cfg->q_storage != RIFT_Q_C128) return RIFT_EINVAL;
+  if (cfg->precision == RIFT_PREC_MIXED && cfg->q_storage != RIFT_Q_C64) return RIFT_EINVAL;
+  if (!std::isfinite(cfg->gmst_rad)) return RIFT_EINVAL;
+  int l_max = 0;
+  for (int a = 0; a < cfg->n_modes; ++a) {
+    const int l = cfg->mode_l[a], m = cfg->mode_m[a];
+    if (l < 2 || l > 8 || m < -l || m > l) return RIFT_EINVAL;
+    for (int b = 0; b < a; ++b)
+      if (cfg->mode_l[b] == l && cfg->mode_m[b] == m) return RIFT_EINVAL;
+    if (l > l_max) l_max = l;
+  }
+  // guard band: S_max = max_k ceil(|r_k| / (c delta_t))
+  if (cfg->n_tau < cfg->n_t) {
+    int s_max = 0;
+    for (int k = 0; k < cfg->n_det; ++k) {
+      const double *r = cfg->det_location_m + 3 * k;
+      const double d = std::sqrt(r[0] * r[0] + r[1] * r[1] + r[2] * r[2]) / (RIFT_C_LIGHT * cfg->delta_t);
+      const int s = (int)std::ceil(d);
+      if (s > s_max) s_max = s;
+    }
+    if ((int64_t)cfg->n_tau + 2 * (int64_t)s_max > cfg->n_t) return RIFT_EWINDOW;
+  }
+
+  rift_ile *h = new (std::nothrow) rift_ile();
+  if (!h) return RIFT_ENOMEM;
+  int rc = RIFT_OK;
+  auto bail = [&](int code) {
+    free_handle(h);
+    return code;
+  };
+#define CUC(call)                                                              \
+  do {                                                                         \
+    cudaError_t e__ = (call);                                                  \
+    if (e__ != cudaSuccess) {                                                  \
+      cudaGetLastError();                                                      \
+      return bail(e__ == cudaErrorMemoryAllocation ? RIFT_ENOMEM : RIFT_ECUDA); \
+    }                                                                          \
+  } while (0)
+
+  CUC(cudaGetDevice(&h->device));
+  CUC(cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device));
+  h->P = cfg->n_points;
+  h->K = cfg->n_det;
+  h->M = cfg->n_modes;
+  h->n_t = cfg->n_t;
+  h->n_tp = (cfg->n_t + 1) & ~1;
+  h->n_tau = cfg->n_tau;
+  h->precision = cfg->precision;
+  h->q_storage = cfg->q_storage;
+  h->geom.n_det = h->K;
+  h->geom.n_modes = h->M;
+  h->geom.l_max = l_max;
+  h->geom.gmst = cfg->gmst_rad;
+  h->geom.delta_t = cfg->delta_t;
+  h->geom.d_ref = cfg->d_ref_mpc;
+  for (int k = 0; k < h->K; ++k) {
+    for (int i = 0; i < 3; ++i) h->geom.loc[k][i] = cfg->det_location_m[3 * k + i];
+    for (int i = 0; i < 9; ++i) h->geom.resp[k][i] = cfg->det_response[9 * k + i];
+  }
+  {
+    std::vector<ModeEntry> modes(h->M);
+    for (int a = 0; a < h->M; ++a) build_mode(cfg->mode_l[a], cfg->mode_m[a], modes[a]);
+    CUC(cudaMalloc(&h->d_modes, sizeof(ModeEntry) * h->M));
+    CUC(cudaMemcpy(h->d_modes, modes.data(), sizeof(ModeEntry) * h->M, cudaMemcpyHostToDevice));
+  }
+  const cudaMemcpyKind kind = cfg->input_mem == RIFT_MEM_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+  const size_t uv_bytes = (size_t)h->P * h->K * h->M * h->M * 16;
+  CUC(cudaMalloc(&h->d_U, uv_bytes));
+  CUC(cudaMalloc(&h->d_V, uv_bytes));
+  CUC(cudaMemcpy(h->d_U, cfg->U, uv_bytes, kind));
+  CUC(cudaMemcpy(h->d_V, cfg->V, uv_bytes, kind));
+  {
+    const bool fp32 = cfg->q_storage == RIFT_Q_C64;
+    const int64_t rows = (int64_t)h->P * h->K * h->M;
+    const size_t csz = fp32 ? 8 : 16;
+    const size_t src_bytes = (size_t)rows * h->n_t * 16;
+    CUC(cudaMalloc(&h->d_Q, (size_t)rows * h->n_tp * csz));
+    const double *src = reinterpret_cast<const double *>(cfg->Q);
+    void *tmp = nullptr;
+    if (cfg->input_mem == RIFT_MEM_HOST) {
+      CUC(cudaMalloc(&tmp, src_bytes));
+      cudaError_t e = cudaMemcpy(tmp, cfg->Q, src_bytes, cudaMemcpyHostToDevice);
+      if (e != cudaSuccess) {
+        cudaFree(tmp);
+        return bail(RIFT_ECUDA);
+      }
+      src = reinterpret_cast<const double *>(tmp);
+    }
+    cudaError_t e = launch_convert_q(src, h->d_Q, rows, h->n_t, h->n_tp, fp32, 0);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    cudaFree(tmp);
+    if (e != cudaSuccess) return bail(RIFT_ECUDA);
+    ++h->launches;
+    h->qs.data = h->d_Q;
+    h->qs.n_t = h->n_t;
+    h->qs.n_tp = h->n_tp;
+    h->qs.n_tau = h->n_tau;
+    h->qs.km = h->K * h->M;
+    h->qs.point_stride_bytes = (int64_t)h->K * h->M * h->n_tp * csz;
+  }
+#undef CUC
+  (void)rc;
+  *out = h;
+  return RIFT_OK;
+}
+
+int rift_ile_destroy(rift_ile_t *h) {
+  if (!h) return RIFT_EINVAL;
+  DeviceGuard g(h->device);
+  free_handle(h);
+  return RIFT_OK;
+}
+
+int rift_ile_set_kernel(rift_ile_t *h, int32_t variant) {
+  if (!h) return RIFT_EINVAL;
+  if (variant != RIFT_KERNEL_AUTO && variant != RIFT_KERNEL_DIRECT && variant != RIFT_KERNEL_TILED)
+    return fail(h, RIFT_EINVAL, "unknown kernel variant");
+  h->kernel_variant = variant;
+  return RIFT_OK;
+}
+
+int rift_ile_eval_batch(rift_ile_t *h, int32_t n_seg, const int32_t *intrinsic_ids, int64_t n_per_seg,
+                        const double *const params[RIFT_N_PARAMS], double *lnL_out, int32_t *shift_out,
+                        void *cuda_stream) {
+  if (!h) return RIFT_EINVAL;
+  if (n_seg < 0 || n_per_seg < 0) return fail(h, RIFT_EINVAL, "negative size");
+  if (n_seg == 0 || n_per_seg == 0) return RIFT_OK;
+  if (!intrinsic_ids || !params || !lnL_out) return fail(h, RIFT_EINVAL, "null pointer");
+  for (int d = 0; d < RIFT_N_PARAMS; ++d)
+    if (!params[d]) return fail(h, RIFT_EINVAL, "null parameter array");
+  DeviceGuard g(h->device);
+  cudaStream_t s = reinterpret_cast<cudaStream_t>(cuda_stream);
+  int rc = upload_ids(h, n_seg, intrinsic_ids, s);
+  if (rc != RIFT_OK) return rc;
+  return run_chunks(h, n_seg, n_per_seg, params, lnL_out, shift_out, nullptr, nullptr, nullptr, s);
+}
+
+int rift_ile_geometry(rift_ile_t *h, int32_t intrinsic_id, int64_t n, const double *const params[RIFT_N_PARAMS],
+                      void *F, void *Y, int32_t *shift, double *quad, void *cuda_stream) {
+  if (!h) return RIFT_EINVAL;
+  if (n < 0) return fail(h, RIFT_EINVAL, "negative size");
+  if (n == 0) return RIFT_OK;
+  if (!params) return fail(h, RIFT_EINVAL, "null pointer");
+  for (int d = 0; d < RIFT_N_PARAMS; ++d)
+    if (!params[d]) return fail(h, RIFT_EINVAL, "null parameter array");
+  DeviceGuard g(h->device);
+  cudaStream_t s = reinterpret_cast<cudaStream_t>(cuda_stream);
+  int rc = upload_ids(h, 1, &intrinsic_id, s);
+  if (rc != RIFT_OK) return rc;
+  return run_chunks(h, 1, n, params, nullptr, shift, reinterpret_cast<double *>(F), reinterpret_cast<double *>(Y), quad,
+                    s);
+}
+
+int rift_ile_reduce(rift_ile_t *h, int32_t n_seg, int64_t n_per_seg, const double *lnL, const double *ln_weight,
+                    const double *const params[RIFT_N_PARAMS], const double lo[RIFT_N_PARAMS],
+                    const double hi[RIFT_N_PARAMS], int32_t n_bins, int32_t merge, double *lnZ, double *rel_err,
+                    double *n_eff, double *n_ess, double *hist, void *cuda_stream) {
+  if (!h) return RIFT_EINVAL;
+  if (n_seg < 1 || n_seg > 65535 || n_per_seg < 0) return fail(h, RIFT_EINVAL, "bad n_seg / n_per_seg");
+  if ((n_per_seg > 0 && !lnL) || !lnZ || !rel_err || !n_eff || !n_ess) return fail(h, RIFT_EINVAL, "null pointer");
+  const bool want_hist = hist != nullptr;
+  if (want_hist) {
+    if (!params || !lo || !hi || n_bins < 1 || n_bins > 1024) return fail(h, RIFT_EINVAL, "histogram arguments");
+    for (int d = 0; d < RIFT_N_PARAMS; ++d)
+      if (!params[d] || !(hi[d] > lo[d])) return fail(h, RIFT_EINVAL, "histogram range / parameter array");
+  }
+  const int nb = want_hist ? n_bins : 0;
+  if (merge && h->state_nseg == 0) merge = 0;      // nothing stored yet: the first accumulate is a reset
+  if (merge && (h->state_nseg != n_seg || h->state_nbins != nb))
+    return fail(h, RIFT_ESTATE, "merge=1 with a different n_seg / n_bins than the stored state");
+  DeviceGuard g(h->device);
+  cudaStream_t s = reinterpret_cast<cudaStream_t>(cuda_stream);
+
+  if (!merge && (h->state_nseg != n_seg || h->state_nbins != nb)) {
+    cudaFree(h->d_state);
+    cudaFree(h->d_state_hist);
+    h->d_state = nullptr;
+    h->d_state_hist = nullptr;
+    h->state_nseg = 0;
+    h->state_nbins = -1;
+    CU(h, cudaMalloc(&h->d_state, sizeof(ReduceState) * n_seg));
+    if (nb > 0) CU(h, cudaMalloc(&h->d_state_hist, sizeof(double) * (size_t)n_seg * 6 * nb));
+    h->state_nseg = n_seg;
+    h->state_nbins = nb;
+  }
+  const int32_t bps = reduce_blocks_per_seg(n_per_seg);
+  const size_t need_partial = reduce_partial_doubles(n_seg, bps, nb);
+  if (need_partial > h->partial_cap) {
+    cudaFree(h->d_partial);
+    h->d_partial = nullptr;
+    h->partial_cap = 0;
+    CU(h, cudaMalloc(&h->d_partial, need_partial * sizeof(double)));
+    h->partial_cap = need_partial;
+  }
+  const size_t need_out = (size_t)n_seg * (4 + 6 * (size_t)nb);
+  if (need_out > h->out_cap) {
+    cudaFree(h->d_out);
+    if (h->h_out) cudaFreeHost(h->h_out);
+    h->d_out = nullptr;
+    h->h_out = nullptr;
+    h->out_cap = 0;
+    CU(h, cudaMalloc(&h->d_out, need_out * sizeof(double)));
+    CU(h, cudaMallocHost(&h->h_out, need_out * sizeof(double)));
+    h->out_cap = need_out;
+  }
+  double *d_scalars = h->d_out, *d_hist = h->d_out + 4 * (size_t)n_seg;
+  int nl = 0;
+  {
+    ProfSpan ps(h, 2, s);
+    CU(h, launch_reduce(n_seg, n_per_seg, lnL, ln_weight, want_hist ? params : nullptr, lo, hi, nb, merge ? 1 : 0,
+                        h->d_state, h->d_state_hist, h->d_partial, bps, d_scalars, d_hist, s, &nl));
+    ps.end();
+  }
+  h->launches += nl;
+  CU(h, cudaMemcpyAsync(h->h_out, h->d_out, need_out * sizeof(double), cudaMemcpyDeviceToHost, s));
+  CU(h, cudaStreamSynchronize(s));
+  memcpy(lnZ, h->h_out, sizeof(double) * n_seg);
+  memcpy(rel_err, h->h_out + n_seg, sizeof(double) * n_seg);
+  memcpy(n_eff, h->h_out + 2 * (size_t)n_seg, sizeof(double) * n_seg);
+  memcpy(n_ess, h->h_out + 3 * (size_t)n_seg, sizeof(double) * n_seg);
+  if (want_hist) memcpy(hist, h->h_out + 4 * (size_t)n_seg, sizeof(double) * (size_t)n_seg * 6 * nb);
+  return RIFT_OK;
+}
+
+int rift_ile_profile(rift_ile_t *h, int32_t enable) {
+  if (!h) return RIFT_EINVAL;
+  h->profiling = enable != 0;
+  return RIFT_OK;
+}
+
+int rift_ile_profile_read(rift_ile_t *h, double ms[3], int64_t launches[3]) {
+  if (!h || !ms || !launches) return RIFT_EINVAL;
+  DeviceGuard g(h->device);
+  for (int i = 0; i < 3; ++i) {
+    ms[i] = 0.0;
+    launches[i] = 0;
+  }
+  int rc = RIFT_OK;
+  for (auto &sp : h->spans) {
+    float t = 0.f;
+    cudaError_t e = cudaEventSynchronize(sp.b);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&t, sp.a, sp.b);
+    if (e == cudaSuccess) {
+      ms[sp.kind] += t;
+      launches[sp.kind] += (sp.kind == 2) ? 2 : 1;
+    } else {
+      rc = fail(h, RIFT_ECUDA, "profile event", e);
+    }
+    cudaEventDestroy(sp.a);
+    cudaEventDestroy(sp.b);
+  }
+  h->spans.clear();
+  return rc;
+}
+
+int rift_ile_fma_peak(int32_t fp64, int32_t iters, double *tflops, void *cuda_stream) {
+  if (!tflops || iters < 1) return RIFT_EINVAL;
+  cudaError_t e = run_fma_peak(fp64 != 0, iters, tflops, reinterpret_cast<cudaStream_t>(cuda_stream));
+  return e == cudaSuccess ? RIFT_OK : RIFT_ECUDA;
+}
+
+}  // extern "C"

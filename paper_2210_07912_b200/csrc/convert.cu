@@ -1,0 +1,89 @@
+// Create-time layout conversion of Q, and the FMA-pipe microbenchmark used as the roofline denominator (H7).
+#include "rift_internal.h"
+
+namespace {
+
+// Q rows: [rows][n_t] complex128  ->  [rows][n_tp] complex<float|double>, padding zero-filled.
+template <typename CT>
+__global__ void convert_q_kernel(const double2 *__restrict__ src, CT *__restrict__ dst, int64_t rows, int n_t, int n_tp) {
+  const int64_t total = rows * n_tp;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t r = i / n_tp;
+    const int t = (int)(i % n_tp);
+    CT v;
+    v.x = 0;
+    v.y = 0;
+    if (t < n_t) {
+      const double2 s = src[r * n_t + t];
+      v.x = s.x;
+      v.y = s.y;
+    }
+    dst[i] = v;
+  }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) fma_peak_kernel(int iters, T seed, T *sink) {
+  T a[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) a[i] = seed + (T)(threadIdx.x + i);
+  const T m = (T)0.999999, c = (T)1e-6;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) a[i] = fma(a[i], m, c);
+  }
+  T s = 0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) s += a[i];
+  if (s == (T)123.456) sink[0] = s;   // never true; keeps the chain alive
+}
+
+}  // namespace
+
+cudaError_t launch_convert_q(const double *Q_c128, void *dst, int64_t rows, int32_t n_t, int32_t n_tp, bool to_fp32,
+                             cudaStream_t s) {
+  const int64_t total = rows * n_tp;
+  int grid = (int)((total + 255) / 256);
+  if (grid > 148 * 16) grid = 148 * 16;
+  if (grid < 1) grid = 1;
+  if (to_fp32)
+    convert_q_kernel<float2><<<grid, 256, 0, s>>>(reinterpret_cast<const double2 *>(Q_c128),
+                                                  reinterpret_cast<float2 *>(dst), rows, n_t, n_tp);
+  else
+    convert_q_kernel<double2><<<grid, 256, 0, s>>>(reinterpret_cast<const double2 *>(Q_c128),
+                                                   reinterpret_cast<double2 *>(dst), rows, n_t, n_tp);
+  return cudaGetLastError();
+}
+
+cudaError_t run_fma_peak(bool fp64, int iters, double *tflops, cudaStream_t s) {
+  int dev = 0, n_sm = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+  void *sink = nullptr;
+  cudaError_t e = cudaMalloc(&sink, 64);
+  if (e != cudaSuccess) return e;
+  cudaEvent_t t0, t1;
+  cudaEventCreate(&t0);
+  cudaEventCreate(&t1);
+  const int grid = n_sm * 8, threads = 256;
+  float best = 1e30f;
+  for (int rep = 0; rep < 4; ++rep) {
+    cudaEventRecord(t0, s);
+    if (fp64)
+      fma_peak_kernel<double><<<grid, threads, 0, s>>>(iters, 1.0, reinterpret_cast<double *>(sink));
+    else
+      fma_peak_kernel<float><<<grid, threads, 0, s>>>(iters, 1.0f, reinterpret_cast<float *>(sink));
+    cudaEventRecord(t1, s);
+    e = cudaEventSynchronize(t1);
+    if (e != cudaSuccess) break;
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, t0, t1);
+    if (rep > 0 && ms < best) best = ms;
+  }
+  cudaEventDestroy(t0);
+  cudaEventDestroy(t1);
+  cudaFree(sink);
+  if (e != cudaSuccess) return e;
+  *tflops = 2.0 * 8.0 * (double)iters * grid * threads / (best * 1e-3) / 1e12;
+  return cudaGetLastError();
+}

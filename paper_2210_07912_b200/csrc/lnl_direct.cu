@@ -1,0 +1,231 @@
+// Fused lnL kernel, "direct" variant: steps a6-a7 of DESIGN.md section 1.
+//   a6  x_j = sum_k sum_lm ( B.re Q.re + B.im Q.im ),  B = F_k Y_lm,  Q = Q_{k,lm}[(j0 + s_k + j) mod N_t]   (Eq. (D2))
+//   a7  lnL_tm = c x_max + ln sum_j exp(c (x_j - x_max)) - ln N_tau - q                                   (App. D.2)
+// One warp per extrinsic sample, lanes over tau (j = lane + 32 i): the per-detector shift s_k is a warp-uniform
+// address offset, so shared-memory reads of the staged Q window are contiguous across lanes and conflict-free.
+// Each intrinsic point's Q block ([K*M][n_tp] complex) is staged in shared memory with cp.async.bulk (TMA 1-D)
+// completing on an mbarrier; the time-axis max / sum are warp-shuffle reductions.  fp32 variant = reading A17.
+#include "rift_internal.h"
+
+namespace {
+
+constexpr int LNL_WARPS = 8;
+constexpr int LNL_THREADS = LNL_WARPS * 32;
+constexpr int SLOTS = 13;                       // 13 * 32 = 416 >= 411 tau samples per block
+constexpr int BLOCK_T = SLOTS * 32;
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t phase) {
+  uint32_t ok = 0;
+  while (!ok) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(phase)
+        : "memory");
+  }
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+
+template <typename Real> struct CplxOf;
+template <> struct CplxOf<float> { typedef float2 type; };
+template <> struct CplxOf<double> { typedef double2 type; };
+
+__device__ __forceinline__ float fast_exp2(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
+template <typename Real>
+__device__ __forceinline__ Real warp_max(Real v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+template <typename Real, bool QSMEM>
+__global__ void __launch_bounds__(LNL_THREADS)
+lnl_direct_kernel(QStore q, Batch b, Workspace ws, int K, double *__restrict__ lnL_out) {
+  typedef typename CplxOf<Real>::type CT;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
+  CT *Qs = reinterpret_cast<CT *>(smem_raw + 128);
+  const size_t q_bytes = QSMEM ? (size_t)q.point_stride_bytes : 0;
+  CT *coef_s = reinterpret_cast<CT *>(smem_raw + 128 + q_bytes);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int km = q.km, M = km / K;
+  CT *wcoef = coef_s + warp * km;
+
+  // contiguous sample range of this CTA, processed as runs of equal segment
+  const int64_t w_begin = (b.n * blockIdx.x) / gridDim.x;
+  const int64_t w_end = (b.n * (blockIdx.x + 1)) / gridDim.x;
+
+  if (QSMEM && threadIdx.x == 0) mbar_init(bar, 1);
+  __syncthreads();
+
+  uint32_t phase = 0;
+  int staged_point = -1;
+  const int j0 = (q.n_t - q.n_tau) / 2;
+  const double ln_ntau = log((double)q.n_tau);
+
+  for (int64_t w0 = w_begin; w0 < w_end;) {
+    const int64_t seg = (b.g0 + w0) / b.n_per_seg;
+    const int64_t run_end = min(w_end, (seg + 1) * b.n_per_seg - b.g0);
+    const int point = b.ids[seg];
+    const CT *Qp;
+    if (QSMEM) {
+      if (point != staged_point) {
+        __syncthreads();                                  // every warp is done with the previous window
+        if (threadIdx.x == 0) {
+          const uint32_t total = (uint32_t)q.point_stride_bytes;
+          mbar_expect_tx(bar, total);
+          const unsigned char *src = reinterpret_cast<const unsigned char *>(q.data) + (int64_t)point * q.point_stride_bytes;
+          for (uint32_t off = 0; off < total; off += 32768u) {
+            const uint32_t nb = min(32768u, total - off);
+            bulk_g2s(reinterpret_cast<unsigned char *>(Qs) + off, src + off, nb, bar);
+          }
+        }
+        mbar_wait(bar, phase);
+        phase ^= 1u;
+        staged_point = point;
+      }
+      Qp = Qs;
+    } else {
+      Qp = reinterpret_cast<const CT *>(reinterpret_cast<const unsigned char *>(q.data) +
+                                        (int64_t)point * q.point_stride_bytes);
+    }
+
+    for (int64_t w = w0 + warp; w < run_end; w += LNL_WARPS) {   // w = workspace slot
+      const double c = ws.scale_c[w];
+      const double quad = ws.quad[w];
+      __syncwarp();
+      {
+        const CT *src = reinterpret_cast<const CT *>(ws.coef) + w * km;
+        for (int i = lane; i < km; i += 32) wcoef[i] = src[i];
+      }
+      __syncwarp();
+
+      Real run_max = -INFINITY;
+      double run_sum = 0.0;
+      for (int jb = 0; jb < q.n_tau; jb += BLOCK_T) {
+        Real x[SLOTS];
+#pragma unroll
+        for (int i = 0; i < SLOTS; ++i) x[i] = (Real)0;
+        for (int k = 0; k < K; ++k) {
+          int base = (j0 + ws.shift[w * K + k] + jb) % q.n_t;
+          if (base < 0) base += q.n_t;
+          int idx[SLOTS];
+#pragma unroll
+          for (int i = 0; i < SLOTS; ++i) {
+            int t = base + lane + 32 * i;
+            if (t >= q.n_t) t -= q.n_t;
+            if (jb + lane + 32 * i >= q.n_tau) t = 0;       // masked slot, keep the address in range
+            idx[i] = t;
+          }
+          for (int m = 0; m < M; ++m) {
+            const CT a = wcoef[k * M + m];
+            const CT *row = Qp + (size_t)(k * M + m) * q.n_tp;
+#pragma unroll
+            for (int i = 0; i < SLOTS; ++i) {
+              const CT v = QSMEM ? row[idx[i]] : __ldg(row + idx[i]);
+              x[i] = fma(a.x, v.x, x[i]);
+              x[i] = fma(a.y, v.y, x[i]);
+            }
+          }
+        }
+        Real bmax = -INFINITY;
+#pragma unroll
+        for (int i = 0; i < SLOTS; ++i) {
+          if (jb + lane + 32 * i >= q.n_tau) x[i] = -INFINITY;
+          bmax = fmax(bmax, x[i]);
+        }
+        bmax = warp_max(bmax);
+        double bsum;
+        if (sizeof(Real) == 4) {
+          const float cl2 = (float)c * 1.4426950408889634f;
+          float s = 0.f;
+#pragma unroll
+          for (int i = 0; i < SLOTS; ++i) s += fast_exp2(((float)x[i] - (float)bmax) * cl2);
+          bsum = (double)s;
+        } else {
+          double s = 0.0;
+#pragma unroll
+          for (int i = 0; i < SLOTS; ++i) s += exp(c * ((double)x[i] - (double)bmax));
+          bsum = s;
+        }
+        bsum = warp_sum(bsum);
+        if (bmax > run_max) {
+          run_sum = run_sum * exp(c * ((double)run_max - (double)bmax)) + bsum;   // exp(-inf) = 0 on the first block
+          run_max = bmax;
+        } else {
+          run_sum += bsum * exp(c * ((double)bmax - (double)run_max));
+        }
+      }
+      if (lane == 0) lnL_out[b.g0 + w] = c * (double)run_max + log(run_sum) - ln_ntau - quad;
+    }
+    w0 = run_end;
+  }
+}
+
+template <typename Real, bool QSMEM>
+cudaError_t launch_t(const QStore &q, const Batch &b, const Workspace &ws, int K, double *lnL_out, int n_sm,
+                     size_t smem, cudaStream_t s) {
+  auto kern = lnl_direct_kernel<Real, QSMEM>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  int occ = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, LNL_THREADS, smem);
+  if (e != cudaSuccess) return e;
+  if (occ < 1) occ = 1;
+  int64_t grid = (int64_t)n_sm * occ;
+  const int64_t max_grid = (b.n + LNL_WARPS - 1) / LNL_WARPS;
+  if (grid > max_grid) grid = max_grid;
+  kern<<<(unsigned)grid, LNL_THREADS, smem, s>>>(q, b, ws, K, lnL_out);
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+size_t lnl_direct_smem_bytes(const QStore &q, bool fp32, bool q_in_smem) {
+  const size_t csz = fp32 ? 8 : 16;
+  return 128 + (q_in_smem ? (size_t)q.point_stride_bytes : 0) + (size_t)LNL_WARPS * q.km * csz;
+}
+
+cudaError_t launch_lnl_direct(const QStore &q, bool fp32, bool q_in_smem, const Batch &b, const Workspace &ws,
+                              int n_det, double *lnL_out, int n_sm, cudaStream_t s, int *n_launch) {
+  if (b.n <= 0) return cudaSuccess;
+  const size_t smem = lnl_direct_smem_bytes(q, fp32, q_in_smem);
+  if (n_launch) ++*n_launch;
+  if (fp32)
+    return q_in_smem ? launch_t<float, true>(q, b, ws, n_det, lnL_out, n_sm, smem, s)
+                     : launch_t<float, false>(q, b, ws, n_det, lnL_out, n_sm, smem, s);
+  return q_in_smem ? launch_t<double, true>(q, b, ws, n_det, lnL_out, n_sm, smem, s)
+                   : launch_t<double, false>(q, b, ws, n_det, lnL_out, n_sm, smem, s);
+}

@@ -1,0 +1,216 @@
+// Sample-axis reduce, step a8 of DESIGN.md section 1 (fp64 throughout, HBM-bound).
+//   ln omega_i = lnL_i + ln w_i;  lnZ = ln[(1/N) sum omega]  (Eq. (3));  n_eff = sum omega / max omega (B1);
+//   n_ess = (sum omega)^2 / sum omega^2 (B2);  rel_err^2 = (N/n_ess - 1)/(N-1) (B3, reading A20);
+//   weighted 1-D histograms per parameter (Eq. (22), reading A13).
+// Two kernels: per-block partial states (block max, sums and histograms relative to the block max; warp-shuffle
+// reductions), then one block per segment merges the partials with the stored state (Eq. (20)-(21): pooled sums).
+#include "rift_internal.h"
+
+namespace {
+
+constexpr int RED_THREADS = 256;
+constexpr int PARTIAL_HDR = 4;   // m, s1, s2, nan flag
+
+__device__ __forceinline__ double block_reduce(double v, double *scratch, bool is_max) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const double u = __shfl_xor_sync(0xffffffffu, v, o);
+    v = is_max ? fmax(v, u) : v + u;
+  }
+  __syncthreads();
+  if (lane == 0) scratch[warp] = v;
+  __syncthreads();
+  double r = scratch[0];
+  for (int i = 1; i < RED_THREADS / 32; ++i) r = is_max ? fmax(r, scratch[i]) : r + scratch[i];
+  return r;
+}
+
+struct HistArgs {
+  const double *p[6];
+  double lo[6], hi[6];
+};
+
+__global__ void __launch_bounds__(RED_THREADS)
+reduce_partial_kernel(int64_t n_per_seg, const double *__restrict__ lnL, const double *__restrict__ ln_w, HistArgs ha,
+                      int has_params, int n_bins, double *__restrict__ partial) {
+  extern __shared__ double sh[];
+  double *scratch = sh;                 // [8]
+  double *hist = sh + 8;                // [6][n_bins]
+  const int seg = blockIdx.y, bx = blockIdx.x, nbx = gridDim.x;
+  const int64_t chunk = (n_per_seg + nbx - 1) / nbx;
+  const int64_t i0 = (int64_t)bx * chunk, i1 = min(n_per_seg, i0 + chunk);
+  const int64_t base = (int64_t)seg * n_per_seg;
+  const int pstride = PARTIAL_HDR + 6 * n_bins;
+  double *out = partial + ((int64_t)seg * nbx + bx) * pstride;
+
+  for (int i = threadIdx.x; i < 6 * n_bins; i += RED_THREADS) hist[i] = 0.0;
+
+  double mx = -INFINITY;
+  int nan_seen = 0;
+  for (int64_t i = i0 + threadIdx.x; i < i1; i += RED_THREADS) {
+    const double v = lnL[base + i] + (ln_w ? ln_w[base + i] : 0.0);
+    if (isnan(v)) nan_seen = 1;
+    mx = fmax(mx, v);
+  }
+  mx = block_reduce(mx, scratch, true);
+  const double nanf = block_reduce((double)nan_seen, scratch, false);
+  __syncthreads();
+
+  double s1 = 0.0, s2 = 0.0;
+  if (mx > -INFINITY && nanf == 0.0) {
+    for (int64_t i = i0 + threadIdx.x; i < i1; i += RED_THREADS) {
+      const double v = lnL[base + i] + (ln_w ? ln_w[base + i] : 0.0);
+      const double w = exp(v - mx);
+      s1 += w;
+      s2 += w * w;
+      if (has_params) {
+#pragma unroll
+        for (int d = 0; d < 6; ++d) {
+          const double x = ha.p[d][base + i];
+          int bin = (int)floor(((double)n_bins * (x - ha.lo[d])) / (ha.hi[d] - ha.lo[d]));
+          if (!(bin >= 0)) bin = 0;
+          if (bin > n_bins - 1) bin = n_bins - 1;
+          atomicAdd(&hist[d * n_bins + bin], w);
+        }
+      }
+    }
+  }
+  s1 = block_reduce(s1, scratch, false);
+  s2 = block_reduce(s2, scratch, false);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    out[0] = mx;
+    out[1] = s1;
+    out[2] = s2;
+    out[3] = nanf;
+  }
+  for (int i = threadIdx.x; i < 6 * n_bins; i += RED_THREADS) out[PARTIAL_HDR + i] = hist[i];
+}
+
+__global__ void __launch_bounds__(128)
+reduce_merge_kernel(int64_t n_per_seg, int n_seg, int nbx, int n_bins, int merge, const double *__restrict__ partial,
+                    ReduceState *__restrict__ state, double *__restrict__ state_hist, double *__restrict__ out_scalars,
+                    double *__restrict__ out_hist) {
+  const int seg = blockIdx.x;
+  const int pstride = PARTIAL_HDR + 6 * n_bins;
+  const double *P = partial + (int64_t)seg * nbx * pstride;
+  __shared__ double s_m, s_s1;
+  __shared__ int s_nan;
+  ReduceState old;
+  old.m = -INFINITY;
+  old.s1 = old.s2 = 0.0;
+  old.n = 0;
+  if (merge) old = state[seg];
+
+  if (threadIdx.x == 0) {
+    double m = old.m;
+    int nan_seen = isnan(old.m) ? 1 : 0;
+    for (int b = 0; b < nbx; ++b) {
+      if (P[b * pstride + 3] != 0.0) nan_seen = 1;
+      m = fmax(m, P[b * pstride]);
+    }
+    double s1 = 0.0, s2 = 0.0;
+    if (!nan_seen && m > -INFINITY) {
+      if (old.m > -INFINITY) {
+        const double f = exp(old.m - m);
+        s1 = old.s1 * f;
+        s2 = old.s2 * f * f;
+      }
+      for (int b = 0; b < nbx; ++b) {
+        const double mb = P[b * pstride];
+        if (mb > -INFINITY) {
+          const double f = exp(mb - m);
+          s1 += P[b * pstride + 1] * f;
+          s2 += P[b * pstride + 2] * f * f;
+        }
+      }
+    }
+    const int64_t n = old.n + n_per_seg;
+    ReduceState st;
+    st.m = nan_seen ? __longlong_as_double(0x7ff8000000000000LL) : m;
+    st.s1 = s1;
+    st.s2 = s2;
+    st.n = n;
+    state[seg] = st;
+    const double N = (double)n;
+    double lnZ, rel, neff, ness;
+    const double qnan = __longlong_as_double(0x7ff8000000000000LL);
+    if (nan_seen) {
+      lnZ = rel = neff = ness = qnan;
+    } else if (n == 0 || !(m > -INFINITY)) {
+      lnZ = (n == 0) ? qnan : m;
+      rel = qnan;
+      neff = ness = 0.0;
+    } else {
+      lnZ = m + log(s1) - log(N);
+      neff = s1;
+      ness = s1 * s1 / s2;
+      if (n > 1) {
+        const double r2 = (N / ness - 1.0) / (N - 1.0);
+        rel = sqrt(r2 > 0.0 ? r2 : 0.0);
+      } else {
+        rel = 0.0;
+      }
+    }
+    out_scalars[0 * n_seg + seg] = lnZ;
+    out_scalars[1 * n_seg + seg] = rel;
+    out_scalars[2 * n_seg + seg] = neff;
+    out_scalars[3 * n_seg + seg] = ness;
+    s_m = m;
+    s_s1 = s1;
+    s_nan = nan_seen;
+  }
+  __syncthreads();
+  if (state_hist == nullptr) return;
+  const double m = s_m, s1 = s_s1;
+  const bool live = !s_nan && m > -INFINITY;
+  for (int i = threadIdx.x; i < 6 * n_bins; i += blockDim.x) {
+    double h = 0.0;
+    if (live) {
+      if (merge && old.m > -INFINITY) h = state_hist[(int64_t)seg * 6 * n_bins + i] * exp(old.m - m);
+      for (int b = 0; b < nbx; ++b) {
+        const double mb = P[b * pstride];
+        if (mb > -INFINITY) h += P[b * pstride + PARTIAL_HDR + i] * exp(mb - m);
+      }
+    }
+    state_hist[(int64_t)seg * 6 * n_bins + i] = h;
+    if (out_hist) out_hist[(int64_t)seg * 6 * n_bins + i] = (live && s1 > 0.0) ? h / s1 : 0.0;
+  }
+}
+
+}  // namespace
+
+int32_t reduce_blocks_per_seg(int64_t n_per_seg) {
+  int64_t b = (n_per_seg + 16383) / 16384;
+  if (b < 1) b = 1;
+  if (b > 64) b = 64;
+  return (int32_t)b;
+}
+
+size_t reduce_partial_doubles(int32_t n_seg, int32_t blocks_per_seg, int32_t n_bins) {
+  return (size_t)n_seg * blocks_per_seg * (PARTIAL_HDR + 6 * (size_t)n_bins);
+}
+
+cudaError_t launch_reduce(int32_t n_seg, int64_t n_per_seg, const double *lnL, const double *ln_w,
+                          const double *const params[6], const double lo[6], const double hi[6], int32_t n_bins,
+                          int merge, ReduceState *state, double *state_hist, double *partial, int32_t blocks_per_seg,
+                          double *out_scalars, double *out_hist, cudaStream_t s, int *n_launch) {
+  HistArgs ha;
+  const bool hp = params != nullptr && n_bins > 0;
+  for (int d = 0; d < 6; ++d) {
+    ha.p[d] = hp ? params[d] : nullptr;
+    ha.lo[d] = hp ? lo[d] : 0.0;
+    ha.hi[d] = hp ? hi[d] : 1.0;
+  }
+  const int nb = hp ? n_bins : 0;
+  const size_t smem = (8 + 6 * (size_t)nb) * sizeof(double);
+  dim3 grid(blocks_per_seg, n_seg);
+  reduce_partial_kernel<<<grid, RED_THREADS, smem, s>>>(n_per_seg, lnL, ln_w, ha, hp ? 1 : 0, nb, partial);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  reduce_merge_kernel<<<n_seg, 128, 0, s>>>(n_per_seg, n_seg, blocks_per_seg, nb, merge, partial, state,
+                                            hp ? state_hist : nullptr, out_scalars, hp ? out_hist : nullptr);
+  if (n_launch) *n_launch += 2;
+  return cudaGetLastError();
+}

@@ -1,0 +1,69 @@
+// Internal declarations shared by the CUDA translation units of librift_ile.so (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "rift_ile.h"
+
+#define RIFT_MAX_TERMS 8         // terms of the Wigner-d sum of one mode (l <= 8  =>  <= l-1 = 7)
+#define RIFT_C_LIGHT 299792458.0
+
+struct ModeEntry {               // one (l,m): -2Y_lm(th,ph) = e^{i m ph} sum_t coef[t] cos(th/2)^pc[t] sin(th/2)^ps[t]
+  int32_t l, m, n_terms, pad;
+  double coef[RIFT_MAX_TERMS];
+  int32_t pc[RIFT_MAX_TERMS];
+  int32_t ps[RIFT_MAX_TERMS];
+};
+
+struct DetGeom {                 // passed by value to the geometry kernel
+  int32_t n_det, n_modes, l_max, pad;
+  double gmst, delta_t, d_ref;
+  double loc[RIFT_MAX_DET][3];
+  double resp[RIFT_MAX_DET][9];
+};
+
+// A chunk = contiguous range [g0, g0 + n) of the caller's flattened sample index g = seg * n_per_seg + i.
+struct Batch {
+  int64_t n_per_seg;
+  int64_t g0;
+  int64_t n;
+  const int32_t *ids;            // device [n_seg]: intrinsic point of each segment
+};
+
+// Per-sample workspace written by the geometry kernel for one chunk (slot = g - g0)
+struct Workspace {
+  void *coef;                    // [n][K*M] complex<float|double>: B_{k,lm} = F_k * Y_lm   (step a5)
+  double *scale_c;               // [n] c = D_ref / D (NaN marks an invalid sample)
+  double *quad;                  // [n] q, the U/V term of Eq. (D3)
+  int32_t *shift;                // [n][K]
+};
+
+struct QStore {                  // device copy of Q: [P][K*M][n_tp] complex<float|double>, n_tp = n_t rounded up to even
+  const void *data;
+  int32_t n_t, n_tp, n_tau, km;
+  int64_t point_stride_bytes;
+};
+
+// geometry.cu
+cudaError_t launch_geometry(const DetGeom &g, const ModeEntry *modes, const Batch &b, const double *const params[6],
+                            const double *U, const double *V, bool coef_fp32, const Workspace &ws,
+                            int32_t *shift_out, double *dbg_F, double *dbg_Y, cudaStream_t s);
+// lnl_direct.cu
+size_t lnl_direct_smem_bytes(const QStore &q, bool fp32, bool q_in_smem);
+cudaError_t launch_lnl_direct(const QStore &q, bool fp32, bool q_in_smem, const Batch &b, const Workspace &ws,
+                              int n_det, double *lnL_out, int n_sm, cudaStream_t s, int *n_launch);
+// reduce.cu
+struct ReduceState {             // device, per segment
+  double m, s1, s2;
+  int64_t n;
+};
+cudaError_t launch_reduce(int32_t n_seg, int64_t n_per_seg, const double *lnL, const double *ln_w,
+                          const double *const params[6], const double lo[6], const double hi[6], int32_t n_bins,
+                          int merge, ReduceState *state, double *state_hist, double *partial, int32_t blocks_per_seg,
+                          double *out_scalars /*[4][n_seg]*/, double *out_hist, cudaStream_t s, int *n_launch);
+size_t reduce_partial_doubles(int32_t n_seg, int32_t blocks_per_seg, int32_t n_bins);
+int32_t reduce_blocks_per_seg(int64_t n_per_seg);
+// convert.cu
+cudaError_t launch_convert_q(const double *Q_c128, void *dst, int64_t rows, int32_t n_t, int32_t n_tp, bool to_fp32,
+                             cudaStream_t s);
+cudaError_t run_fma_peak(bool fp64, int iters, double *tflops, cudaStream_t s);

@@ -197,6 +197,20 @@ def true_point(cfg: Config, point: int) -> np.ndarray:
     return prior_draw(point_rng(cfg, point, stream=250), 1)[:, 0].copy()
 
 
+_DFT_CACHE: Dict[Tuple[int, float], np.ndarray] = {}
+
+
+def _dft_matrix(n_t: int, f_s: float) -> np.ndarray:
+    """exp(2 pi i f_n t_j), t_j = (j - (N_t-1)/2)/f_s; cached per (N_t, f_s)."""
+    key = (n_t, f_s)
+    if key not in _DFT_CACHE:
+        f, _df = freq_grid()
+        t = (np.arange(n_t, dtype=np.float64) - (n_t - 1) / 2.0) / f_s
+        _DFT_CACHE.clear()
+        _DFT_CACHE[key] = np.exp(2j * math.pi * np.outer(t, f))
+    return _DFT_CACHE[key]
+
+
 @dataclass
 class PointData:
     Q: np.ndarray        # [K][M][N_t] complex128, centre sample = t_ref
@@ -250,8 +264,7 @@ def make_point(cfg: Config, point: int, coeff_true: np.ndarray, shift_true: np.n
     V = 0.5 * (V + np.swapaxes(V, 1, 2))
 
     # Q(t_j) = 4 df sum_n exp(2 pi i f_n t_j) h*(f_n) d(f_n) / S(f_n), t_j = (j - (N_t-1)/2)/f_s (A9)
-    t = (np.arange(n_t, dtype=np.float64) - (n_t - 1) / 2.0) / cfg.f_s
-    E = np.exp(2j * math.pi * np.outer(t, f))              # [N_t][N_FREQ]
+    E = _dft_matrix(n_t, cfg.f_s)                          # [N_t][N_FREQ]
     W = (np.conj(h) * (d / S)[:, None, :]).reshape(K * M, N_FREQ)
     Q = (4.0 * df) * (W @ E.T)                             # [K*M][N_t]
     return PointData(np.ascontiguousarray(Q.reshape(K, M, n_t)), np.ascontiguousarray(U),

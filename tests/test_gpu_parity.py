@@ -1,0 +1,346 @@
+"""GPU parity: the CUDA path (through the C ABI binding) against the CPU oracle, element by element on the same
+seeded inputs.  Tolerances (BASELINE.json north_star): shifts bit-exact; fp64 mode lnL relative 1e-10 (relative to
+max(1,|lnL|)); mixed mode |dlnL| <= 2e-3 and |dlnZ| <= 1e-3."""
+import math
+
+import numpy as np
+import pytest
+
+import paper_2210_07912_b200 as rift
+from paper_2210_07912_b200 import synth
+
+from helpers import build, create, oracle_eval, rel_err
+
+pytestmark = pytest.mark.gpu
+
+TOL_FP64_REL = 1e-10
+TOL_MIXED_LNL = 2e-3
+TOL_MIXED_LNZ = 1e-3
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    assert t.cuda.is_available(), "GPU tests need a CUDA device"
+    rift.lib()                       # fail loudly if the extension is missing
+    return t
+
+
+def dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def gpu_eval(torch, h, ids, n_per_seg, params, want_shifts=True, K=None):
+    p = dev(torch, params)
+    n = p.shape[1]
+    lnL = torch.full((n,), float("nan"), dtype=torch.float64, device="cuda")
+    sh = torch.zeros((n, K), dtype=torch.int32, device="cuda") if want_shifts else None
+    rift.rift_ile_eval_batch(h, ids, n_per_seg, p, lnL, sh, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    return lnL, sh, p
+
+
+# ------------------------------------------------------------------------------------------------ geometry
+def test_geometry_kernel_matches_oracle(torch, oracle):
+    cfg = synth.with_overrides(synth.CONFIGS[2], n_points=1)          # 21 modes, l = 2..4
+    inp = build(oracle, cfg, n_points=1)
+    h = create(rift, inp, rift.RIFT_PREC_FP64)
+    n = 3001
+    params = synth.prior_draw(np.random.default_rng(5), n)
+    p = dev(torch, params)
+    K, M = cfg.n_det, cfg.n_modes
+    F = torch.zeros((n, K, 2), dtype=torch.float64, device="cuda")
+    Y = torch.zeros((n, M, 2), dtype=torch.float64, device="cuda")
+    sh = torch.zeros((n, K), dtype=torch.int32, device="cuda")
+    quad = torch.zeros(n, dtype=torch.float64, device="cuda")
+    rift.rift_ile_geometry(h, 0, n, p, F, Y, sh, quad, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    F = F.cpu().numpy().view(np.complex128)[..., 0]
+    Y = Y.cpu().numpy().view(np.complex128)[..., 0]
+    Fo = oracle.antenna(params[0], params[1], params[2], cfg.gmst, inp.det_response)
+    Yo = oracle.harmonics(params[3], params[4], inp.mode_l, inp.mode_m)
+    _dt, so, fr = oracle.delays(params[0], params[1], cfg.gmst, inp.det_location, cfg.delta_t)
+    assert np.max(np.abs(F - Fo)) < 1e-14
+    assert np.max(np.abs(Y - Yo)) < 1e-14
+    ok = fr.sum(axis=1) == 0
+    assert np.array_equal(sh.cpu().numpy()[ok], so[ok])
+    for i in range(0, n, 97):
+        c = synth.D_REF_MPC / params[5, i]
+        q = oracle.lnl_core(Fo[i], Yo[i], c, so[i], inp.Q[0], inp.U[0], inp.V[0])[2]
+        assert abs(quad[i].item() - q) < 1e-12 * max(1.0, abs(q))
+    rift.rift_ile_destroy(h)
+
+
+def test_higher_l_harmonics(torch, oracle):
+    modes = tuple((l, m) for l in (5, 6, 7, 8) for m in (-l, -3, 0, 2, l))
+    cfg = synth.with_overrides(synth.CONFIGS[0], modes=modes, f_s=512.0, t_window=0.02)
+    inp = build(oracle, cfg)
+    h = create(rift, inp, rift.RIFT_PREC_FP64)
+    n = 500
+    params = synth.prior_draw(np.random.default_rng(6), n)
+    Y = torch.zeros((n, len(modes), 2), dtype=torch.float64, device="cuda")
+    rift.rift_ile_geometry(h, 0, n, dev(torch, params), None, Y, None, None)
+    torch.cuda.synchronize()
+    Yo = oracle.harmonics(params[3], params[4], inp.mode_l, inp.mode_m)
+    assert np.max(np.abs(Y.cpu().numpy().view(np.complex128)[..., 0] - Yo)) < 2e-14
+    rift.rift_ile_destroy(h)
+
+
+# ------------------------------------------------------------------------------------------------ C0, whole config
+@pytest.mark.parametrize("rho", [12.0, 30.0])
+def test_c0_all_samples_both_precisions(torch, oracle, rho):
+    cfg = synth.with_overrides(synth.CONFIGS[0], rho=rho)
+    inp = build(oracle, cfg)
+    params, ln_w = synth.draw_samples(cfg, 0)
+    ref, sh_ref, fr = oracle_eval(oracle, inp, 0, params)
+    red_ref = oracle.reduce(ref, ln_w, params, synth.HIST_LO, synth.HIST_HI, 100)
+    for prec, name in ((rift.RIFT_PREC_FP64, "fp64"), (rift.RIFT_PREC_MIXED, "mixed")):
+        h = create(rift, inp, prec)
+        lnL, sh, p = gpu_eval(torch, h, [0], cfg.n_samples, params, K=cfg.n_det)
+        got = lnL.cpu().numpy()
+        assert np.array_equal(sh.cpu().numpy()[fr == 0], sh_ref[fr == 0])
+        if prec == rift.RIFT_PREC_FP64:
+            assert np.max(rel_err(got, ref)) < TOL_FP64_REL, name
+        else:
+            assert np.max(np.abs(got - ref)) < TOL_MIXED_LNL, name
+        red = rift.rift_ile_reduce(h, 1, cfg.n_samples, lnL, dev(torch, ln_w), p, synth.HIST_LO, synth.HIST_HI, 100,
+                                   merge=0, want_hist=True)
+        tol = 1e-10 * max(1.0, abs(red_ref["lnZ"])) if prec == rift.RIFT_PREC_FP64 else TOL_MIXED_LNZ
+        assert abs(red["lnZ"][0] - red_ref["lnZ"]) < tol
+        rtol = 1e-9 if prec == rift.RIFT_PREC_FP64 else 5e-3
+        assert abs(red["n_eff"][0] - red_ref["n_eff"]) < rtol * red_ref["n_eff"]
+        assert abs(red["n_ess"][0] - red_ref["n_ess"]) < rtol * red_ref["n_ess"]
+        assert abs(red["rel_err"][0] - red_ref["rel_err"]) < rtol
+        assert np.max(np.abs(red["hist"][0] - red_ref["hist"])) < rtol
+        assert "lnl_" in rift.rift_ile_kernel_name(h)
+        assert rift.rift_ile_launch_count(h) >= 4
+        rift.rift_ile_destroy(h)
+
+
+# ------------------------------------------------------------------------------------------------ C1 reduced + ragged
+def test_c1_multi_point_ragged_segments(torch, oracle):
+    cfg = synth.CONFIGS[1]
+    inp = build(oracle, cfg, n_points=3)
+    n_per = 2 * 256 + 37                                    # several warps' worth and a ragged tail
+    ids = [2, 0, 1, 0]                                      # repeated and permuted intrinsic ids
+    params = np.concatenate([synth.draw_samples(cfg, 10 + s, n_per)[0] for s in range(len(ids))], axis=1)
+    ref = np.concatenate([oracle_eval(oracle, inp, ids[s], params[:, s * n_per:(s + 1) * n_per])[0]
+                          for s in range(len(ids))])
+    for prec in (rift.RIFT_PREC_FP64, rift.RIFT_PREC_MIXED):
+        h = create(rift, inp, prec)
+        lnL, _sh, _p = gpu_eval(torch, h, ids, n_per, params, K=cfg.n_det)
+        got = lnL.cpu().numpy()
+        if prec == rift.RIFT_PREC_FP64:
+            assert np.max(rel_err(got, ref)) < TOL_FP64_REL
+        else:
+            assert np.max(np.abs(got - ref)) < TOL_MIXED_LNL
+        rift.rift_ile_destroy(h)
+
+
+def test_edge_sizes_and_invalid_samples(torch, oracle):
+    cfg = synth.CONFIGS[0]
+    inp = build(oracle, cfg)
+    h = create(rift, inp, rift.RIFT_PREC_FP64)
+    # empty batches are a no-op
+    lnL = torch.zeros(4, dtype=torch.float64, device="cuda")
+    p4 = dev(torch, synth.prior_draw(np.random.default_rng(1), 4))
+    rift.rift_ile_eval_batch(h, [], 0, p4, lnL)
+    rift.rift_ile_eval_batch(h, [0], 0, p4, lnL)
+    for n in (1, 7, 33):
+        params = synth.prior_draw(np.random.default_rng(n), n)
+        got, _, _ = gpu_eval(torch, h, [0], n, params, K=cfg.n_det)
+        ref = oracle_eval(oracle, inp, 0, params)[0]
+        assert np.max(rel_err(got.cpu().numpy(), ref)) < TOL_FP64_REL
+    # dist <= 0 and NaN parameters: NaN for that sample only
+    params = synth.prior_draw(np.random.default_rng(9), 64)
+    params[5, 3] = -10.0
+    params[5, 4] = 0.0
+    params[0, 5] = np.nan
+    params[3, 40] = np.nan
+    got = gpu_eval(torch, h, [0], 64, params, K=cfg.n_det)[0].cpu().numpy()
+    ref = oracle_eval(oracle, inp, 0, params)[0]
+    assert np.array_equal(np.isnan(got), np.isnan(ref)) and np.isnan(got).sum() == 4
+    ok = ~np.isnan(ref)
+    assert np.max(rel_err(got[ok], ref[ok])) < TOL_FP64_REL
+    # error codes
+    with pytest.raises(rift.RiftError) as e:
+        rift.rift_ile_eval_batch(h, [1], 4, p4, lnL)
+    assert e.value.code == rift.RIFT_ERANGE
+    with pytest.raises(rift.RiftError) as e:
+        rift.rift_ile_eval_batch(h, [0], 4, p4, None)
+    assert e.value.code == rift.RIFT_EINVAL
+    rift.rift_ile_destroy(h)
+
+
+def test_guard_band_window(torch, oracle):
+    """n_tau < n_t (reading A4): the physical mode in which the circular wrap never triggers."""
+    cfg = synth.CONFIGS[1]
+    inp = build(oracle, cfg, n_points=1)
+    n_tau = cfg.n_t - 2 * 88 - 2                              # S_max = 88 at 4096 Hz
+    params = synth.draw_samples(cfg, 0, 1500)[0]
+    ref = oracle_eval(oracle, inp, 0, params, n_tau=n_tau)[0]
+    for prec, tol in ((rift.RIFT_PREC_FP64, None), (rift.RIFT_PREC_MIXED, TOL_MIXED_LNL)):
+        h = create(rift, inp, prec, n_tau=n_tau)
+        got = gpu_eval(torch, h, [0], 1500, params, K=cfg.n_det)[0].cpu().numpy()
+        if tol is None:
+            assert np.max(rel_err(got, ref)) < TOL_FP64_REL
+        else:
+            assert np.max(np.abs(got - ref)) < tol
+        rift.rift_ile_destroy(h)
+    with pytest.raises(rift.RiftError) as e:
+        create(rift, inp, rift.RIFT_PREC_FP64, n_tau=cfg.n_t - 100)
+    assert e.value.code == rift.RIFT_EWINDOW
+
+
+# ------------------------------------------------------------------------------------------------ C2 / C4 shapes, reduced
+def test_c2_shape_21_modes(torch, oracle):
+    cfg = synth.CONFIGS[2]
+    inp = build(oracle, cfg, n_points=2)
+    n = 1200
+    params, ln_w = synth.draw_samples(cfg, 1, n, theta_true=inp.theta_true[1])
+    ref = oracle_eval(oracle, inp, 1, params)[0]
+    zref = oracle.reduce(ref, ln_w)
+    for prec in (rift.RIFT_PREC_FP64, rift.RIFT_PREC_MIXED):
+        h = create(rift, inp, prec)
+        lnL, _, _ = gpu_eval(torch, h, [1], n, params, K=cfg.n_det)
+        got = lnL.cpu().numpy()
+        red = rift.rift_ile_reduce(h, 1, n, lnL, dev(torch, ln_w))
+        if prec == rift.RIFT_PREC_FP64:
+            assert np.max(rel_err(got, ref)) < TOL_FP64_REL
+            assert abs(red["lnZ"][0] - zref["lnZ"]) < 1e-10 * max(1.0, abs(zref["lnZ"]))
+        else:
+            assert np.max(np.abs(got - ref)) < TOL_MIXED_LNL
+            assert abs(red["lnZ"][0] - zref["lnZ"]) < TOL_MIXED_LNZ
+        rift.rift_ile_destroy(h)
+
+
+def test_c4_shape_long_window(torch, oracle):
+    cfg = synth.CONFIGS[4]
+    inp = build(oracle, cfg, n_points=1)
+    n = 600
+    params, _ = synth.draw_samples(cfg, 0, n)
+    ref, sh_ref, fr = oracle_eval(oracle, inp, 0, params)
+    for prec in (rift.RIFT_PREC_FP64, rift.RIFT_PREC_MIXED):
+        h = create(rift, inp, prec)
+        lnL, sh, _ = gpu_eval(torch, h, [0], n, params, K=cfg.n_det)
+        got = lnL.cpu().numpy()
+        assert np.array_equal(sh.cpu().numpy()[fr == 0], sh_ref[fr == 0])
+        if prec == rift.RIFT_PREC_FP64:
+            assert np.max(rel_err(got, ref)) < TOL_FP64_REL
+        else:
+            assert np.max(np.abs(got - ref)) < TOL_MIXED_LNL
+        rift.rift_ile_destroy(h)
+
+
+# ------------------------------------------------------------------------------------------------ reduce
+def test_reduce_merge_and_degenerate(torch, oracle):
+    cfg = synth.CONFIGS[0]
+    inp = build(oracle, cfg)
+    h = create(rift, inp, rift.RIFT_PREC_FP64)
+    rng = np.random.default_rng(3)
+    n_seg, n = 3, 40_000
+    lnL = 6.0 * rng.standard_normal(n_seg * n)
+    lw = 0.4 * rng.standard_normal(n_seg * n)
+    params = synth.prior_draw(rng, n_seg * n)
+    one = rift.rift_ile_reduce(h, n_seg, n, dev(torch, lnL), dev(torch, lw), dev(torch, params), synth.HIST_LO,
+                               synth.HIST_HI, 50, merge=0, want_hist=True)
+    for s in range(n_seg):
+        sl = slice(s * n, (s + 1) * n)
+        ref = oracle.reduce(lnL[sl], lw[sl], params[:, sl], synth.HIST_LO, synth.HIST_HI, 50)
+        for key in ("lnZ", "rel_err", "n_eff", "n_ess"):
+            assert abs(one[key][s] - ref[key]) < 1e-10 * max(1.0, abs(ref[key])), (s, key)
+        assert np.max(np.abs(one["hist"][s] - ref["hist"])) < 1e-12
+    # two halves merged == one pass (Eq. (20)-(21)); segments are interleaved halves of the same data
+    half = n // 2
+    a = np.concatenate([lnL[s * n:s * n + half] for s in range(n_seg)])
+    b = np.concatenate([lnL[s * n + half:(s + 1) * n] for s in range(n_seg)])
+    wa = np.concatenate([lw[s * n:s * n + half] for s in range(n_seg)])
+    wb = np.concatenate([lw[s * n + half:(s + 1) * n] for s in range(n_seg)])
+    pa = np.concatenate([params[:, s * n:s * n + half] for s in range(n_seg)], axis=1)
+    pb = np.concatenate([params[:, s * n + half:(s + 1) * n] for s in range(n_seg)], axis=1)
+    rift.rift_ile_reduce(h, n_seg, half, dev(torch, a), dev(torch, wa), dev(torch, pa), synth.HIST_LO, synth.HIST_HI, 50,
+                         merge=0, want_hist=True)
+    two = rift.rift_ile_reduce(h, n_seg, half, dev(torch, b), dev(torch, wb), dev(torch, pb), synth.HIST_LO,
+                               synth.HIST_HI, 50, merge=1, want_hist=True)
+    for key in ("lnZ", "rel_err", "n_eff", "n_ess"):
+        assert np.max(np.abs(one[key] - two[key])) < 1e-10 * max(1.0, np.max(np.abs(one[key]))), key
+    assert np.max(np.abs(one["hist"] - two["hist"])) < 1e-12
+    with pytest.raises(rift.RiftError) as e:
+        rift.rift_ile_reduce(h, n_seg + 1, half, dev(torch, np.zeros((n_seg + 1) * half)), merge=1)
+    assert e.value.code == rift.RIFT_ESTATE
+    # degenerate inputs
+    r = rift.rift_ile_reduce(h, 1, 1, dev(torch, np.array([2.5])), dev(torch, np.array([-0.5])))
+    assert abs(r["lnZ"][0] - 2.0) < 1e-15 and r["n_eff"][0] == 1.0 and r["rel_err"][0] == 0.0
+    r = rift.rift_ile_reduce(h, 1, 4, dev(torch, np.full(4, -np.inf)))
+    assert r["lnZ"][0] == -np.inf and r["n_eff"][0] == 0.0
+    r = rift.rift_ile_reduce(h, 1, 4, dev(torch, np.array([0.0, np.nan, 1.0, 2.0])))
+    assert math.isnan(r["lnZ"][0])
+    x = np.array([800.0, 799.0, -800.0, -np.inf])
+    r = rift.rift_ile_reduce(h, 1, 4, dev(torch, x))
+    assert abs(r["lnZ"][0] - oracle.reduce(x)["lnZ"]) < 1e-12
+    rift.rift_ile_destroy(h)
+
+
+# ------------------------------------------------------------------------------------------------ full sizes, sampled
+def _full_size_sampled(torch, oracle, cfg, precisions, n_check_points, stride, lnz_points=0):
+    """Run a whole config on the GPU (the launch configuration bench.py times: all segments in one eval_batch
+    where memory allows) and compare a strided subsample of outputs, plus lnZ of whole points, with the oracle."""
+    P = cfg.n_points
+    inp = build(oracle, cfg)
+    n = cfg.n_samples
+    pts = sorted(set(np.linspace(0, P - 1, n_check_points).astype(int).tolist()))
+    results = {}
+    for prec in precisions:
+        h = create(rift, inp, prec)
+        seg_per_call = max(1, min(P, int(2.5e7 // n)))
+        for p0 in range(0, P, seg_per_call):
+            ids = list(range(p0, min(P, p0 + seg_per_call)))
+            ps, ws = zip(*[synth.draw_samples(cfg, p, theta_true=inp.theta_true[p]) for p in ids])
+            params = np.concatenate(ps, axis=1)
+            lnL, sh, pdev = gpu_eval(torch, h, ids, n, params, K=cfg.n_det)
+            red = rift.rift_ile_reduce(h, len(ids), n, lnL, dev(torch, np.concatenate(ws)))
+            got = lnL.cpu().numpy()
+            shg = sh.cpu().numpy()
+            assert not np.isnan(got).any()
+            for p in ids:
+                if p not in pts:
+                    continue
+                o = (p - p0) * n
+                sel = np.arange(0, n, stride)
+                full = lnz_points > 0 and p in pts[:lnz_points]
+                if full:
+                    sel = np.arange(n)
+                ref, sh_ref, fr = oracle_eval(oracle, inp, p, params[:, o:o + n][:, sel])
+                ok = fr == 0
+                assert np.array_equal(shg[o:o + n][sel][ok], sh_ref[ok])
+                if prec == rift.RIFT_PREC_FP64:
+                    assert np.max(rel_err(got[o:o + n][sel], ref)) < TOL_FP64_REL, (cfg.name, p)
+                else:
+                    assert np.max(np.abs(got[o:o + n][sel] - ref)) < TOL_MIXED_LNL, (cfg.name, p)
+                if full:
+                    zr = oracle.reduce(ref, ws[p - p0])
+                    tol = 1e-10 * max(1.0, abs(zr["lnZ"])) if prec == rift.RIFT_PREC_FP64 else TOL_MIXED_LNZ
+                    assert abs(red["lnZ"][p - p0] - zr["lnZ"]) < tol, (cfg.name, p)
+            results[prec] = True
+        rift.rift_ile_destroy(h)
+    return results
+
+
+def test_c1_full_size(torch, oracle):
+    # 16 points x 1e5 samples in ONE eval_batch (bench.py's launch); two whole points and a 1/50 subsample elsewhere
+    _full_size_sampled(torch, oracle, synth.CONFIGS[1], (rift.RIFT_PREC_MIXED, rift.RIFT_PREC_FP64), 4, 50, lnz_points=2)
+
+
+@pytest.mark.slow
+def test_c2_full_size(torch, oracle):
+    _full_size_sampled(torch, oracle, synth.CONFIGS[2], (rift.RIFT_PREC_MIXED,), 3, 500, lnz_points=0)
+
+
+@pytest.mark.slow
+def test_c3_full_size(torch, oracle):
+    _full_size_sampled(torch, oracle, synth.CONFIGS[3], (rift.RIFT_PREC_MIXED,), 5, 100, lnz_points=1)
+
+
+@pytest.mark.slow
+def test_c4_full_size(torch, oracle):
+    _full_size_sampled(torch, oracle, synth.CONFIGS[4], (rift.RIFT_PREC_MIXED,), 2, 4000, lnz_points=0)
