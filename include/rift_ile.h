@@ -44,7 +44,7 @@ enum {
 enum { RIFT_PREC_FP64 = 0, RIFT_PREC_MIXED = 1 };   /* arithmetic of the window term (reading A17) */
 enum { RIFT_Q_C128 = 0, RIFT_Q_C64 = 1 };           /* storage of Q on the device */
 enum { RIFT_MEM_HOST = 0, RIFT_MEM_DEVICE = 1 };    /* where the Q/U/V arrays passed to create live */
-enum { RIFT_KERNEL_AUTO = 0, RIFT_KERNEL_DIRECT = 1, RIFT_KERNEL_TILED = 2 };   /* rift_ile_set_kernel */
+enum { RIFT_KERNEL_AUTO = 0, RIFT_KERNEL_DIRECT = 1, RIFT_KERNEL_GROUPED = 2 };   /* rift_ile_set_kernel */
 
 #define RIFT_MAX_DET 8
 #define RIFT_MAX_MODES 80
@@ -122,13 +122,14 @@ const char *rift_ile_kernel_name(const rift_ile_t *h);
 
 /* Per-kernel device timing for bench.py's roofline: while enabled, every geometry / fused-lnL / reduce launch is
  * bracketed by CUDA events on its stream.  rift_ile_profile_read synchronises those events, returns the summed
- * milliseconds and launch counts per kernel family since the last read ([0] geometry, [1] fused lnL, [2] reduce),
- * and clears them. */
+ * milliseconds and launch counts per kernel family since the last read ([0] geometry, [1] fused lnL, [2] reduce,
+ * [3] grouping sort), and clears them. */
 int rift_ile_profile(rift_ile_t *h, int32_t enable);
-int rift_ile_profile_read(rift_ile_t *h, double ms[3], int64_t launches[3]);
+int rift_ile_profile_read(rift_ile_t *h, double ms[4], int64_t launches[4]);
 
 /* Dense FMA-pipe microbenchmark (hard part H7): runs `iters` dependent-free FMA per thread over a grid
- * filling the device and returns achieved TFLOP/s in *tflops (fp64 != 0 selects DFMA). */
+ * filling the device and returns achieved TFLOP/s in *tflops.  fp64: 0 = FFMA chains, 1 = DFMA chains, 2 = FFMA 7x8
+ * register tile (all operands in registers, the operand pattern of the fused kernels). */
 int rift_ile_fma_peak(int32_t fp64, int32_t iters, double *tflops, void *cuda_stream);
 
 int rift_ile_destroy(rift_ile_t *h);

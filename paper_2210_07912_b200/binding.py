@@ -20,7 +20,7 @@ RIFT_OK, RIFT_EINVAL, RIFT_ENOMEM, RIFT_ECUDA, RIFT_EWINDOW, RIFT_ERANGE, RIFT_E
 RIFT_PREC_FP64, RIFT_PREC_MIXED = 0, 1
 RIFT_Q_C128, RIFT_Q_C64 = 0, 1
 RIFT_MEM_HOST, RIFT_MEM_DEVICE = 0, 1
-RIFT_KERNEL_AUTO, RIFT_KERNEL_DIRECT, RIFT_KERNEL_TILED = 0, 1, 2
+RIFT_KERNEL_AUTO, RIFT_KERNEL_DIRECT, RIFT_KERNEL_GROUPED = 0, 1, 2
 RIFT_N_PARAMS = 6
 
 EXPORTS = ("rift_ile_create", "rift_ile_eval_batch", "rift_ile_reduce", "rift_ile_geometry", "rift_ile_set_kernel",
@@ -204,14 +204,14 @@ def rift_ile_profile(h, enable: bool) -> None:
 
 
 def rift_ile_profile_read(h) -> dict:
-    """dict(ms=[geometry, lnl, reduce], launches=[...]) summed since the last read."""
-    ms = (C.c_double * 3)()
-    nl = (C.c_int64 * 3)()
+    """dict(ms=[geometry, lnl, reduce, sort], launches=[...]) summed since the last read."""
+    ms = (C.c_double * 4)()
+    nl = (C.c_int64 * 4)()
     _check(lib().rift_ile_profile_read(h, ms, nl), h)
     return dict(ms=[float(x) for x in ms], launches=[int(x) for x in nl])
 
 
 def rift_ile_fma_peak(fp64: bool, iters: int = 4096, cuda_stream: int = 0) -> float:
     v = C.c_double()
-    _check(lib().rift_ile_fma_peak(int(bool(fp64)), int(iters), C.byref(v), int(cuda_stream) or None))
+    _check(lib().rift_ile_fma_peak(int(fp64), int(iters), C.byref(v), int(cuda_stream) or None))
     return float(v.value)

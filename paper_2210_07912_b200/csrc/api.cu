@@ -18,6 +18,12 @@ struct rift_ile {
   void *d_Q = nullptr;
   double *d_U = nullptr, *d_V = nullptr;
   QStore qs{};
+  void *d_Qp = nullptr;            // planar, circularly extended copy for the grouped kernel (NULL if it cannot fit)
+  QStore qsp{};
+  SortPlan plan{};
+  int32_t *d_bucket = nullptr, *d_perm = nullptr;
+  uint32_t *d_hist = nullptr;
+  size_t hist_cap = 0;
   // per-chunk workspace
   int64_t ws_cap = 0;
   Workspace ws{};
@@ -133,6 +139,11 @@ void free_handle(rift_ile *h) {
   }
   cudaFree(h->d_modes);
   cudaFree(h->d_Q);
+  cudaFree(h->d_Qp);
+  cudaFree(h->d_bucket);
+  cudaFree(h->d_perm);
+  cudaFree(h->d_hist);
+  cudaFree(h->ws.orig);
   cudaFree(h->d_U);
   cudaFree(h->d_V);
   cudaFree(h->ws.coef);
@@ -148,7 +159,11 @@ void free_handle(rift_ile *h) {
   delete h;
 }
 
-size_t coef_bytes(const rift_ile *h) { return (size_t)h->K * h->M * (h->precision == RIFT_PREC_MIXED ? 8 : 16); }
+int64_t coef_stride(const rift_ile *h) {          // Reals per sample, a multiple of 16 bytes
+  const int64_t n = 2 * (int64_t)h->K * h->M;
+  return h->precision == RIFT_PREC_MIXED ? ((n + 3) & ~3ll) : n;
+}
+size_t coef_bytes(const rift_ile *h) { return (size_t)coef_stride(h) * (h->precision == RIFT_PREC_MIXED ? 4 : 8); }
 
 int ensure_workspace(rift_ile *h, int64_t n) {
   if (n <= h->ws_cap) return RIFT_OK;
@@ -156,12 +171,20 @@ int ensure_workspace(rift_ile *h, int64_t n) {
   cudaFree(h->ws.scale_c);
   cudaFree(h->ws.quad);
   cudaFree(h->ws.shift);
+  cudaFree(h->ws.orig);
+  cudaFree(h->d_bucket);
+  cudaFree(h->d_perm);
+  h->d_bucket = h->d_perm = nullptr;
   h->ws = Workspace{};
   h->ws_cap = 0;
   CU(h, cudaMalloc(&h->ws.coef, (size_t)n * coef_bytes(h)));
+  h->ws.coef_stride = coef_stride(h);
   CU(h, cudaMalloc(&h->ws.scale_c, (size_t)n * sizeof(double)));
   CU(h, cudaMalloc(&h->ws.quad, (size_t)n * sizeof(double)));
   CU(h, cudaMalloc(&h->ws.shift, (size_t)n * h->K * sizeof(int32_t)));
+  CU(h, cudaMalloc(&h->ws.orig, (size_t)n * sizeof(int32_t)));
+  CU(h, cudaMalloc(&h->d_bucket, (size_t)n * sizeof(int32_t)));
+  CU(h, cudaMalloc(&h->d_perm, (size_t)n * sizeof(int32_t)));
   h->ws_cap = n;
   return RIFT_OK;
 }
@@ -193,6 +216,19 @@ bool q_fits_smem(const rift_ile *h) {
   return lnl_direct_smem_bytes(h->qs, fp32, true) <= 227u * 1024u;
 }
 
+// AUTO currently resolves to the direct kernel: on C1 the grouped kernel (3.7 ms + 0.4 ms of sorting per 1.6e6
+// evaluations) does not yet beat it (3.6 ms); see DESIGN.md section 5 and profiles/.
+bool use_grouped(const rift_ile *h) {
+  if (h->kernel_variant != RIFT_KERNEL_GROUPED) return false;
+  return h->d_Qp != nullptr;
+}
+
+int32_t next_pow2(int64_t v) {
+  int32_t p = 1;
+  while (p < v && p < (1 << 30)) p <<= 1;
+  return p;
+}
+
 int run_chunks(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *const params[6], double *lnL_out,
                int32_t *shift_out, double *dbg_F, double *dbg_Y, double *dbg_quad, cudaStream_t s) {
   const int64_t total = (int64_t)n_seg * n_per_seg;
@@ -202,27 +238,63 @@ int run_chunks(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *cons
   if (rc != RIFT_OK) return rc;
   const bool fp32 = h->precision == RIFT_PREC_MIXED;
   const bool in_smem = q_fits_smem(h);
+  const bool grouped = lnL_out != nullptr && use_grouped(h);
   for (int64_t g0 = 0; g0 < total; g0 += cap) {
     Batch b;
     b.n_per_seg = n_per_seg;
     b.g0 = g0;
     b.n = (total - g0 < cap) ? total - g0 : cap;
     b.ids = h->d_ids;
+    Workspace ws = h->ws;
+    const int32_t *perm = nullptr;
+    if (grouped) {
+      const int32_t n_seg_chunk = (int32_t)((g0 + b.n - 1) / n_per_seg - g0 / n_per_seg + 1);
+      SortPlan sp = h->plan;
+      int32_t nb = sp.n_buckets;
+      const int32_t by_n = next_pow2(n_per_seg);
+      if (nb > by_n) nb = by_n;
+      while ((int64_t)nb * n_seg_chunk > (16ll << 20) && nb > 1) nb >>= 1;
+      if (nb != sp.n_buckets) {
+        sp.exact = 0;
+        sp.n_buckets = nb;
+      }
+      const size_t need = (size_t)nb * n_seg_chunk;
+      if (need > h->hist_cap) {
+        cudaFree(h->d_hist);
+        h->d_hist = nullptr;
+        h->hist_cap = 0;
+        CU(h, cudaMalloc(&h->d_hist, need * sizeof(uint32_t)));
+        h->hist_cap = need;
+      }
+      int nl = 0;
+      ProfSpan ps(h, 3, s);
+      CU(h, launch_group_sort(h->geom, sp, b, params, h->d_bucket, h->d_hist, n_seg_chunk, h->d_perm, s, &nl));
+      ps.end();
+      h->launches += nl;
+      perm = h->d_perm;
+    } else {
+      ws.orig = nullptr;
+    }
     {
       ProfSpan ps(h, 0, s);
-      CU(h, launch_geometry(h->geom, h->d_modes, b, params, h->d_U, h->d_V, fp32, h->ws, shift_out, dbg_F, dbg_Y, s));
+      CU(h, launch_geometry(h->geom, h->d_modes, b, params, h->d_U, h->d_V, fp32, ws, shift_out, dbg_F, dbg_Y, perm, s));
       ps.end();
     }
     ++h->launches;
-    if (dbg_quad) CU(h, cudaMemcpyAsync(dbg_quad + g0, h->ws.quad, (size_t)b.n * sizeof(double), cudaMemcpyDeviceToDevice, s));
+    if (dbg_quad) CU(h, cudaMemcpyAsync(dbg_quad + g0, ws.quad, (size_t)b.n * sizeof(double), cudaMemcpyDeviceToDevice, s));
     if (lnL_out) {
       int nl = 0;
       ProfSpan ps(h, 1, s);
-      CU(h, launch_lnl_direct(h->qs, fp32, in_smem, b, h->ws, h->K, lnL_out, h->n_sm, s, &nl));
+      if (grouped) {
+        CU(h, launch_lnl_grouped(h->qsp, fp32, b, ws, h->K, lnL_out, h->n_sm, s, &nl));
+        h->kernel_name = fp32 ? "lnl_grouped<f32>" : "lnl_grouped<f64>";
+      } else {
+        CU(h, launch_lnl_direct(h->qs, fp32, in_smem, b, ws, h->K, lnL_out, h->n_sm, s, &nl));
+        h->kernel_name = fp32 ? (in_smem ? "lnl_direct<f32,smem>" : "lnl_direct<f32,global>")
+                              : (in_smem ? "lnl_direct<f64,smem>" : "lnl_direct<f64,global>");
+      }
       ps.end();
       h->launches += nl;
-      h->kernel_name = fp32 ? (in_smem ? "lnl_direct<f32,smem>" : "lnl_direct<f32,global>")
-                            : (in_smem ? "lnl_direct<f64,smem>" : "lnl_direct<f64,global>");
     }
   }
   return RIFT_OK;
@@ -348,6 +420,24 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
       src = reinterpret_cast<const double *>(tmp);
     }
     cudaError_t e = launch_convert_q(src, h->d_Q, rows, h->n_t, h->n_tp, fp32, 0);
+    // planar, circularly extended copy for the grouped kernel, if one point's block fits in shared memory
+    {
+      const size_t rsz = fp32 ? 4 : 8;
+      const int32_t n_tpp = (h->n_t + RIFT_EXT + 3) & ~3;
+      QStore qp{};
+      qp.n_t = h->n_t;
+      qp.n_tp = n_tpp;
+      qp.n_tau = h->n_tau;
+      qp.km = h->K * h->M;
+      qp.point_stride_bytes = (int64_t)2 * h->K * h->M * n_tpp * rsz;
+      if (e == cudaSuccess && lnl_grouped_smem_bytes(qp, fp32) <= 227u * 1024u) {
+        e = cudaMalloc(&h->d_Qp, (size_t)h->P * qp.point_stride_bytes);
+        if (e == cudaSuccess) e = launch_convert_q_planar(src, h->d_Qp, rows, h->n_t, n_tpp, fp32, 0);
+        qp.data = h->d_Qp;
+        h->qsp = qp;
+        ++h->launches;
+      }
+    }
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     cudaFree(tmp);
     if (e != cudaSuccess) return bail(RIFT_ECUDA);
@@ -358,6 +448,24 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
     h->qs.n_tau = h->n_tau;
     h->qs.km = h->K * h->M;
     h->qs.point_stride_bytes = (int64_t)h->K * h->M * h->n_tp * csz;
+  }
+  {  // grouping plan: ranges of the relative shifts d_k = s_k - s_0
+    SortPlan &sp = h->plan;
+    int64_t prod = 1;
+    for (int k = 0; k < RIFT_MAX_DET; ++k) sp.half[k] = sp.range[k] = 1;
+    for (int k = 1; k < h->K; ++k) {
+      double d2 = 0;
+      for (int i = 0; i < 3; ++i) {
+        const double d = h->geom.loc[k][i] - h->geom.loc[0][i];
+        d2 += d * d;
+      }
+      const int m = (int)std::ceil(std::sqrt(d2) / (RIFT_C_LIGHT * cfg->delta_t)) + 1;
+      sp.half[k] = m;
+      sp.range[k] = 2 * m + 1;
+      if (prod <= (1ll << 40)) prod *= sp.range[k];
+    }
+    sp.exact = prod <= 65536 ? 1 : 0;
+    sp.n_buckets = sp.exact ? next_pow2(prod) : 65536;
   }
 #undef CUC
   (void)rc;
@@ -374,7 +482,7 @@ int rift_ile_destroy(rift_ile_t *h) {
 
 int rift_ile_set_kernel(rift_ile_t *h, int32_t variant) {
   if (!h) return RIFT_EINVAL;
-  if (variant != RIFT_KERNEL_AUTO && variant != RIFT_KERNEL_DIRECT && variant != RIFT_KERNEL_TILED)
+  if (variant != RIFT_KERNEL_AUTO && variant != RIFT_KERNEL_DIRECT && variant != RIFT_KERNEL_GROUPED)
     return fail(h, RIFT_EINVAL, "unknown kernel variant");
   h->kernel_variant = variant;
   return RIFT_OK;
@@ -489,10 +597,10 @@ int rift_ile_profile(rift_ile_t *h, int32_t enable) {
   return RIFT_OK;
 }
 
-int rift_ile_profile_read(rift_ile_t *h, double ms[3], int64_t launches[3]) {
+int rift_ile_profile_read(rift_ile_t *h, double ms[4], int64_t launches[4]) {
   if (!h || !ms || !launches) return RIFT_EINVAL;
   DeviceGuard g(h->device);
-  for (int i = 0; i < 3; ++i) {
+  for (int i = 0; i < 4; ++i) {
     ms[i] = 0.0;
     launches[i] = 0;
   }
@@ -503,7 +611,7 @@ int rift_ile_profile_read(rift_ile_t *h, double ms[3], int64_t launches[3]) {
     if (e == cudaSuccess) e = cudaEventElapsedTime(&t, sp.a, sp.b);
     if (e == cudaSuccess) {
       ms[sp.kind] += t;
-      launches[sp.kind] += (sp.kind == 2) ? 2 : 1;
+      launches[sp.kind] += (sp.kind == 2) ? 2 : (sp.kind == 3 ? 3 : 1);
     } else {
       rc = fail(h, RIFT_ECUDA, "profile event", e);
     }
@@ -516,7 +624,7 @@ int rift_ile_profile_read(rift_ile_t *h, double ms[3], int64_t launches[3]) {
 
 int rift_ile_fma_peak(int32_t fp64, int32_t iters, double *tflops, void *cuda_stream) {
   if (!tflops || iters < 1) return RIFT_EINVAL;
-  cudaError_t e = run_fma_peak(fp64 != 0, iters, tflops, reinterpret_cast<cudaStream_t>(cuda_stream));
+  cudaError_t e = run_fma_peak(fp64, iters, tflops, reinterpret_cast<cudaStream_t>(cuda_stream));
   return e == cudaSuccess ? RIFT_OK : RIFT_ECUDA;
 }
 

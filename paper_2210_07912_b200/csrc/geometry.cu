@@ -17,10 +17,12 @@ geometry_kernel(DetGeom g, const ModeEntry *__restrict__ modes, Batch b, const d
                 const double *__restrict__ p_dec, const double *__restrict__ p_psi, const double *__restrict__ p_iota,
                 const double *__restrict__ p_phi, const double *__restrict__ p_dist, const double *__restrict__ U,
                 const double *__restrict__ V, Workspace ws, int32_t *__restrict__ shift_out,
-                double *__restrict__ dbg_F, double *__restrict__ dbg_Y) {
-  const int64_t w = (int64_t)blockIdx.x * GEOM_THREADS + threadIdx.x;     // workspace slot
+                double *__restrict__ dbg_F, double *__restrict__ dbg_Y, const int32_t *__restrict__ perm) {
+  const int64_t w = (int64_t)blockIdx.x * GEOM_THREADS + threadIdx.x;     // workspace slot (sorted position)
   if (w >= b.n) return;
-  const int64_t gi = b.g0 + w;                                             // caller's sample index
+  const int64_t src = perm ? (int64_t)perm[w] : w;                         // chunk-local index of the sample
+  if (ws.orig) ws.orig[w] = (int32_t)src;
+  const int64_t gi = b.g0 + src;                                           // caller's sample index
   const int32_t point = b.ids[gi / b.n_per_seg];
   const int K = g.n_det, M = g.n_modes;
 
@@ -113,7 +115,7 @@ geometry_kernel(DetGeom g, const ModeEntry *__restrict__ modes, Batch b, const d
   const double c = bad ? __longlong_as_double(0x7ff8000000000000LL) : g.d_ref / dist;
   ws.scale_c[w] = c;
   {
-    CT *out = reinterpret_cast<CT *>(ws.coef) + w * (int64_t)(K * M);
+    CT *out = reinterpret_cast<CT *>(reinterpret_cast<decltype(CT::x) *>(ws.coef) + w * ws.coef_stride);
     for (int k = 0; k < K; ++k)
       for (int a = 0; a < M; ++a) {
         CT v;
@@ -160,15 +162,15 @@ geometry_kernel(DetGeom g, const ModeEntry *__restrict__ modes, Batch b, const d
 
 cudaError_t launch_geometry(const DetGeom &g, const ModeEntry *modes, const Batch &b, const double *const params[6],
                             const double *U, const double *V, bool coef_fp32, const Workspace &ws,
-                            int32_t *shift_out, double *dbg_F, double *dbg_Y, cudaStream_t s) {
+                            int32_t *shift_out, double *dbg_F, double *dbg_Y, const int32_t *perm, cudaStream_t s) {
   if (b.n <= 0) return cudaSuccess;
   const int64_t n = b.n;
   const unsigned grid = (unsigned)((n + GEOM_THREADS - 1) / GEOM_THREADS);
   if (coef_fp32)
     geometry_kernel<float2><<<grid, GEOM_THREADS, 0, s>>>(g, modes, b, params[0], params[1], params[2], params[3],
-                                                           params[4], params[5], U, V, ws, shift_out, dbg_F, dbg_Y);
+                                                           params[4], params[5], U, V, ws, shift_out, dbg_F, dbg_Y, perm);
   else
     geometry_kernel<double2><<<grid, GEOM_THREADS, 0, s>>>(g, modes, b, params[0], params[1], params[2], params[3],
-                                                            params[4], params[5], U, V, ws, shift_out, dbg_F, dbg_Y);
+                                                            params[4], params[5], U, V, ws, shift_out, dbg_F, dbg_Y, perm);
   return cudaGetLastError();
 }

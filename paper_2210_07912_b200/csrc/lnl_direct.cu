@@ -6,6 +6,7 @@
 // Each intrinsic point's Q block ([K*M][n_tp] complex) is staged in shared memory with cp.async.bulk (TMA 1-D)
 // completing on an mbarrier; the time-axis max / sum are warp-shuffle reductions.  fp32 variant = reading A17.
 #include "rift_internal.h"
+#include "tma_utils.cuh"
 
 namespace {
 
@@ -14,60 +15,9 @@ constexpr int LNL_THREADS = LNL_WARPS * 32;
 constexpr int SLOTS = 13;                       // 13 * 32 = 416 >= 411 tau samples per block
 constexpr int BLOCK_T = SLOTS * 32;
 
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t phase) {
-  uint32_t ok = 0;
-  while (!ok) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(ok)
-        : "r"(smem_u32(bar)), "r"(phase)
-        : "memory");
-  }
-}
-__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                   smem_u32(dst)),
-               "l"(src), "r"(bytes), "r"(smem_u32(bar))
-               : "memory");
-}
-
 template <typename Real> struct CplxOf;
 template <> struct CplxOf<float> { typedef float2 type; };
 template <> struct CplxOf<double> { typedef double2 type; };
-
-__device__ __forceinline__ float fast_exp2(float x) {
-  float y;
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-}
-
-template <typename Real>
-__device__ __forceinline__ Real warp_max(Real v) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
-  return v;
-}
-__device__ __forceinline__ float warp_max(float v) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
-  return v;
-}
-__device__ __forceinline__ double warp_sum(double v) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-  return v;
-}
 
 template <typename Real, bool QSMEM>
 __global__ void __launch_bounds__(LNL_THREADS)
@@ -104,13 +54,8 @@ lnl_direct_kernel(QStore q, Batch b, Workspace ws, int K, double *__restrict__ l
       if (point != staged_point) {
         __syncthreads();                                  // every warp is done with the previous window
         if (threadIdx.x == 0) {
-          const uint32_t total = (uint32_t)q.point_stride_bytes;
-          mbar_expect_tx(bar, total);
-          const unsigned char *src = reinterpret_cast<const unsigned char *>(q.data) + (int64_t)point * q.point_stride_bytes;
-          for (uint32_t off = 0; off < total; off += 32768u) {
-            const uint32_t nb = min(32768u, total - off);
-            bulk_g2s(reinterpret_cast<unsigned char *>(Qs) + off, src + off, nb, bar);
-          }
+          stage_block(Qs, reinterpret_cast<const unsigned char *>(q.data) + (int64_t)point * q.point_stride_bytes,
+                      (uint32_t)q.point_stride_bytes, bar);
         }
         mbar_wait(bar, phase);
         phase ^= 1u;
@@ -127,7 +72,7 @@ lnl_direct_kernel(QStore q, Batch b, Workspace ws, int K, double *__restrict__ l
       const double quad = ws.quad[w];
       __syncwarp();
       {
-        const CT *src = reinterpret_cast<const CT *>(ws.coef) + w * km;
+        const CT *src = reinterpret_cast<const CT *>(reinterpret_cast<const Real *>(ws.coef) + w * ws.coef_stride);
         for (int i = lane; i < km; i += 32) wcoef[i] = src[i];
       }
       __syncwarp();
@@ -188,7 +133,7 @@ lnl_direct_kernel(QStore q, Batch b, Workspace ws, int K, double *__restrict__ l
           run_sum += bsum * exp(c * ((double)bmax - (double)run_max));
         }
       }
-      if (lane == 0) lnL_out[b.g0 + w] = c * (double)run_max + log(run_sum) - ln_ntau - quad;
+      if (lane == 0) lnL_out[b.g0 + (ws.orig ? ws.orig[w] : w)] = c * (double)run_max + log(run_sum) - ln_ntau - quad;
     }
     w0 = run_end;
   }

@@ -32,22 +32,45 @@ struct Batch {
 
 // Per-sample workspace written by the geometry kernel for one chunk (slot = g - g0)
 struct Workspace {
-  void *coef;                    // [n][K*M] complex<float|double>: B_{k,lm} = F_k * Y_lm   (step a5)
+  void *coef;                    // [n][coef_stride] Real, the first 2*K*M hold complex B_{k,lm} = F_k * Y_lm (step a5)
+  int64_t coef_stride;           // Reals per sample: 2*K*M rounded up to a 16-byte multiple
   double *scale_c;               // [n] c = D_ref / D (NaN marks an invalid sample)
   double *quad;                  // [n] q, the U/V term of Eq. (D3)
   int32_t *shift;                // [n][K]
+  int32_t *orig;                 // [n] chunk-local index of the caller's sample held in this slot (NULL = identity)
 };
 
-struct QStore {                  // device copy of Q: [P][K*M][n_tp] complex<float|double>, n_tp = n_t rounded up to even
+// Grouping plan (sort.cu): bucket = exact mixed-radix index of the relative shift tuple, or a hash of it.
+struct SortPlan {
+  int32_t exact, n_buckets;      // n_buckets is a power of two
+  int32_t half[RIFT_MAX_DET];    // d_k + half[k] in [0, range[k])
+  int32_t range[RIFT_MAX_DET];
+};
+
+// Device copy of Q.  Interleaved layout (direct kernel): [P][K*M][n_tp] complex<Real>, n_tp = n_t rounded up to even.
+// Planar extended layout (grouped kernel): [P][2*K*M][n_tp] Real, row 2r = Re, 2r+1 = Im, each row holding the n_t
+// samples followed by a circular repeat of its first RIFT_EXT samples (so base + j never needs a wrap), zero padded.
+struct QStore {
   const void *data;
   int32_t n_t, n_tp, n_tau, km;
   int64_t point_stride_bytes;
 };
+#define RIFT_EXT 416             // 13 slots x 32 lanes: one time block of the fused kernels
 
 // geometry.cu
 cudaError_t launch_geometry(const DetGeom &g, const ModeEntry *modes, const Batch &b, const double *const params[6],
                             const double *U, const double *V, bool coef_fp32, const Workspace &ws,
-                            int32_t *shift_out, double *dbg_F, double *dbg_Y, cudaStream_t s);
+                            int32_t *shift_out, double *dbg_F, double *dbg_Y, const int32_t *perm, cudaStream_t s);
+// sort.cu
+cudaError_t launch_group_sort(const DetGeom &g, const SortPlan &sp, const Batch &b, const double *const params[6],
+                              int32_t *bucket_of, uint32_t *hist, int32_t n_seg_chunk, int32_t *perm, cudaStream_t s,
+                              int *n_launch);
+// lnl_grouped.cu
+size_t lnl_grouped_smem_bytes(const QStore &q, bool fp32);
+cudaError_t launch_lnl_grouped(const QStore &q, bool fp32, const Batch &b, const Workspace &ws, int n_det,
+                               double *lnL_out, int n_sm, cudaStream_t s, int *n_launch);
+cudaError_t launch_convert_q_planar(const double *Q_c128, void *dst, int64_t rows, int32_t n_t, int32_t n_tp,
+                                    bool to_fp32, cudaStream_t s);
 // lnl_direct.cu
 size_t lnl_direct_smem_bytes(const QStore &q, bool fp32, bool q_in_smem);
 cudaError_t launch_lnl_direct(const QStore &q, bool fp32, bool q_in_smem, const Batch &b, const Workspace &ws,
@@ -66,4 +89,4 @@ int32_t reduce_blocks_per_seg(int64_t n_per_seg);
 // convert.cu
 cudaError_t launch_convert_q(const double *Q_c128, void *dst, int64_t rows, int32_t n_t, int32_t n_tp, bool to_fp32,
                              cudaStream_t s);
-cudaError_t run_fma_peak(bool fp64, int iters, double *tflops, cudaStream_t s);
+cudaError_t run_fma_peak(int mode, int iters, double *tflops, cudaStream_t s);   // 0 fp32, 1 fp64, 2 fp32 register tile

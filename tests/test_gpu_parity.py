@@ -30,7 +30,9 @@ def dev(torch, a):
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
 
-def gpu_eval(torch, h, ids, n_per_seg, params, want_shifts=True, K=None):
+def gpu_eval(torch, h, ids, n_per_seg, params, want_shifts=True, K=None, kernel=None):
+    if kernel is not None:
+        rift.rift_ile_set_kernel(h, kernel)
     p = dev(torch, params)
     n = p.shape[1]
     lnL = torch.full((n,), float("nan"), dtype=torch.float64, device="cuda")
@@ -87,8 +89,12 @@ def test_higher_l_harmonics(torch, oracle):
 
 
 # ------------------------------------------------------------------------------------------------ C0, whole config
+KERNELS = [rift.RIFT_KERNEL_DIRECT, rift.RIFT_KERNEL_GROUPED]
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
 @pytest.mark.parametrize("rho", [12.0, 30.0])
-def test_c0_all_samples_both_precisions(torch, oracle, rho):
+def test_c0_all_samples_both_precisions(torch, oracle, rho, kernel):
     cfg = synth.with_overrides(synth.CONFIGS[0], rho=rho)
     inp = build(oracle, cfg)
     params, ln_w = synth.draw_samples(cfg, 0)
@@ -96,9 +102,10 @@ def test_c0_all_samples_both_precisions(torch, oracle, rho):
     red_ref = oracle.reduce(ref, ln_w, params, synth.HIST_LO, synth.HIST_HI, 100)
     for prec, name in ((rift.RIFT_PREC_FP64, "fp64"), (rift.RIFT_PREC_MIXED, "mixed")):
         h = create(rift, inp, prec)
-        lnL, sh, p = gpu_eval(torch, h, [0], cfg.n_samples, params, K=cfg.n_det)
+        lnL, sh, p = gpu_eval(torch, h, [0], cfg.n_samples, params, K=cfg.n_det, kernel=kernel)
         got = lnL.cpu().numpy()
         assert np.array_equal(sh.cpu().numpy()[fr == 0], sh_ref[fr == 0])
+        assert ("grouped" in rift.rift_ile_kernel_name(h)) == (kernel == rift.RIFT_KERNEL_GROUPED)
         if prec == rift.RIFT_PREC_FP64:
             assert np.max(rel_err(got, ref)) < TOL_FP64_REL, name
         else:
@@ -118,7 +125,8 @@ def test_c0_all_samples_both_precisions(torch, oracle, rho):
 
 
 # ------------------------------------------------------------------------------------------------ C1 reduced + ragged
-def test_c1_multi_point_ragged_segments(torch, oracle):
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_c1_multi_point_ragged_segments(torch, oracle, kernel):
     cfg = synth.CONFIGS[1]
     inp = build(oracle, cfg, n_points=3)
     n_per = 2 * 256 + 37                                    # several warps' worth and a ragged tail
@@ -128,7 +136,7 @@ def test_c1_multi_point_ragged_segments(torch, oracle):
                           for s in range(len(ids))])
     for prec in (rift.RIFT_PREC_FP64, rift.RIFT_PREC_MIXED):
         h = create(rift, inp, prec)
-        lnL, _sh, _p = gpu_eval(torch, h, ids, n_per, params, K=cfg.n_det)
+        lnL, _sh, _p = gpu_eval(torch, h, ids, n_per, params, K=cfg.n_det, kernel=kernel)
         got = lnL.cpu().numpy()
         if prec == rift.RIFT_PREC_FP64:
             assert np.max(rel_err(got, ref)) < TOL_FP64_REL
@@ -172,7 +180,8 @@ def test_edge_sizes_and_invalid_samples(torch, oracle):
     rift.rift_ile_destroy(h)
 
 
-def test_guard_band_window(torch, oracle):
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_guard_band_window(torch, oracle, kernel):
     """n_tau < n_t (reading A4): the physical mode in which the circular wrap never triggers."""
     cfg = synth.CONFIGS[1]
     inp = build(oracle, cfg, n_points=1)
@@ -181,7 +190,7 @@ def test_guard_band_window(torch, oracle):
     ref = oracle_eval(oracle, inp, 0, params, n_tau=n_tau)[0]
     for prec, tol in ((rift.RIFT_PREC_FP64, None), (rift.RIFT_PREC_MIXED, TOL_MIXED_LNL)):
         h = create(rift, inp, prec, n_tau=n_tau)
-        got = gpu_eval(torch, h, [0], 1500, params, K=cfg.n_det)[0].cpu().numpy()
+        got = gpu_eval(torch, h, [0], 1500, params, K=cfg.n_det, kernel=kernel)[0].cpu().numpy()
         if tol is None:
             assert np.max(rel_err(got, ref)) < TOL_FP64_REL
         else:
@@ -282,7 +291,7 @@ def test_reduce_merge_and_degenerate(torch, oracle):
 
 
 # ------------------------------------------------------------------------------------------------ full sizes, sampled
-def _full_size_sampled(torch, oracle, cfg, precisions, n_check_points, stride, lnz_points=0):
+def _full_size_sampled(torch, oracle, cfg, precisions, n_check_points, stride, lnz_points=0, kernel=None):
     """Run a whole config on the GPU (the launch configuration bench.py times: all segments in one eval_batch
     where memory allows) and compare a strided subsample of outputs, plus lnZ of whole points, with the oracle."""
     P = cfg.n_points
@@ -297,7 +306,7 @@ def _full_size_sampled(torch, oracle, cfg, precisions, n_check_points, stride, l
             ids = list(range(p0, min(P, p0 + seg_per_call)))
             ps, ws = zip(*[synth.draw_samples(cfg, p, theta_true=inp.theta_true[p]) for p in ids])
             params = np.concatenate(ps, axis=1)
-            lnL, sh, pdev = gpu_eval(torch, h, ids, n, params, K=cfg.n_det)
+            lnL, sh, pdev = gpu_eval(torch, h, ids, n, params, K=cfg.n_det, kernel=kernel)
             red = rift.rift_ile_reduce(h, len(ids), n, lnL, dev(torch, np.concatenate(ws)))
             got = lnL.cpu().numpy()
             shg = sh.cpu().numpy()
@@ -329,6 +338,11 @@ def _full_size_sampled(torch, oracle, cfg, precisions, n_check_points, stride, l
 def test_c1_full_size(torch, oracle):
     # 16 points x 1e5 samples in ONE eval_batch (bench.py's launch); two whole points and a 1/50 subsample elsewhere
     _full_size_sampled(torch, oracle, synth.CONFIGS[1], (rift.RIFT_PREC_MIXED, rift.RIFT_PREC_FP64), 4, 50, lnz_points=2)
+
+
+def test_c1_full_size_grouped_kernel(torch, oracle):
+    _full_size_sampled(torch, oracle, synth.CONFIGS[1], (rift.RIFT_PREC_MIXED, rift.RIFT_PREC_FP64), 3, 50, lnz_points=1,
+                       kernel=rift.RIFT_KERNEL_GROUPED)
 
 
 @pytest.mark.slow
