@@ -18,6 +18,8 @@ struct rift_ile {
   void *d_Q = nullptr;
   double *d_U = nullptr, *d_V = nullptr;
   QStore qs{};
+  void *d_Qe = nullptr;            // interleaved, circularly extended copy for the direct_ext kernel (NULL if too big)
+  QStore qse{};
   void *d_Qp = nullptr;            // planar, circularly extended copy for the grouped kernel (NULL if it cannot fit)
   QStore qsp{};
   SortPlan plan{};
@@ -140,6 +142,7 @@ void free_handle(rift_ile *h) {
   cudaFree(h->d_modes);
   cudaFree(h->d_Q);
   cudaFree(h->d_Qp);
+  cudaFree(h->d_Qe);
   cudaFree(h->d_bucket);
   cudaFree(h->d_perm);
   cudaFree(h->d_hist);
@@ -216,8 +219,8 @@ bool q_fits_smem(const rift_ile *h) {
   return lnl_direct_smem_bytes(h->qs, fp32, true) <= 227u * 1024u;
 }
 
-// AUTO currently resolves to the direct kernel: on C1 the grouped kernel (3.7 ms + 0.4 ms of sorting per 1.6e6
-// evaluations) does not yet beat it (3.6 ms); see DESIGN.md section 5 and profiles/.
+// AUTO resolves to direct_ext when one point's extended Q block fits in shared memory, else to direct.  The grouped
+// kernel is opt-in (RIFT_KERNEL_GROUPED): on C1 it does not yet beat the direct kernels, profiles/.
 bool use_grouped(const rift_ile *h) {
   if (h->kernel_variant != RIFT_KERNEL_GROUPED) return false;
   return h->d_Qp != nullptr;
@@ -288,6 +291,10 @@ int run_chunks(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *cons
       if (grouped) {
         CU(h, launch_lnl_grouped(h->qsp, fp32, b, ws, h->K, lnL_out, h->n_sm, s, &nl));
         h->kernel_name = fp32 ? "lnl_grouped<f32>" : "lnl_grouped<f64>";
+      } else if (h->d_Qe != nullptr && fp32 && h->kernel_variant != RIFT_KERNEL_DIRECT) {
+        // (fp64: the extended block leaves room for one CTA per SM only and measures slower than direct)
+        CU(h, launch_lnl_direct_ext(h->qse, fp32, b, ws, h->K, lnL_out, h->n_sm, s, &nl));
+        h->kernel_name = fp32 ? "lnl_direct_ext<f32>" : "lnl_direct_ext<f64>";
       } else {
         CU(h, launch_lnl_direct(h->qs, fp32, in_smem, b, ws, h->K, lnL_out, h->n_sm, s, &nl));
         h->kernel_name = fp32 ? (in_smem ? "lnl_direct<f32,smem>" : "lnl_direct<f32,global>")
@@ -420,6 +427,23 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
       src = reinterpret_cast<const double *>(tmp);
     }
     cudaError_t e = launch_convert_q(src, h->d_Q, rows, h->n_t, h->n_tp, fp32, 0);
+    // interleaved, circularly extended copy for the direct_ext kernel, if one point's block fits in shared memory
+    {
+      const int32_t n_te = (h->n_t + RIFT_EXT + 1) & ~1;
+      QStore qe{};
+      qe.n_t = h->n_t;
+      qe.n_tp = n_te;
+      qe.n_tau = h->n_tau;
+      qe.km = h->K * h->M;
+      qe.point_stride_bytes = (int64_t)h->K * h->M * n_te * csz;
+      if (e == cudaSuccess && lnl_direct_ext_smem_bytes(qe, fp32) <= 227u * 1024u) {
+        e = cudaMalloc(&h->d_Qe, (size_t)h->P * qe.point_stride_bytes);
+        if (e == cudaSuccess) e = launch_convert_q_ext(src, h->d_Qe, rows, h->n_t, n_te, fp32, 0);
+        qe.data = h->d_Qe;
+        h->qse = qe;
+        ++h->launches;
+      }
+    }
     // planar, circularly extended copy for the grouped kernel, if one point's block fits in shared memory
     {
       const size_t rsz = fp32 ? 4 : 8;
@@ -552,7 +576,7 @@ int rift_ile_reduce(rift_ile_t *h, int32_t n_seg, int64_t n_per_seg, const doubl
     h->state_nseg = n_seg;
     h->state_nbins = nb;
   }
-  const int32_t bps = reduce_blocks_per_seg(n_per_seg);
+  const int32_t bps = reduce_blocks_per_seg(n_per_seg, n_seg);
   const size_t need_partial = reduce_partial_doubles(n_seg, bps, nb);
   if (need_partial > h->partial_cap) {
     cudaFree(h->d_partial);

@@ -22,6 +22,27 @@ __global__ void convert_q_kernel(const double2 *__restrict__ src, CT *__restrict
   }
 }
 
+// Q rows: [rows][n_t] complex128 -> [rows][n_te] complex<float|double>; columns n_t..n_t+RIFT_EXT-1 repeat columns
+// 0..RIFT_EXT-1 circularly, the rest is zero.
+template <typename CT>
+__global__ void convert_q_ext_kernel(const double2 *__restrict__ src, CT *__restrict__ dst, int64_t rows, int n_t,
+                                     int n_te) {
+  const int64_t total = rows * n_te;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t r = i / n_te;
+    const int t = (int)(i % n_te);
+    CT v;
+    v.x = 0;
+    v.y = 0;
+    if (t < n_t + RIFT_EXT) {
+      const double2 s = src[r * n_t + (t % n_t)];
+      v.x = s.x;
+      v.y = s.y;
+    }
+    dst[i] = v;
+  }
+}
+
 // Q rows: [rows][n_t] complex128 -> planar rows [2*rows][n_tp] Real (2r = Re, 2r+1 = Im); columns n_t..n_t+RIFT_EXT-1
 // repeat columns 0..RIFT_EXT-1 circularly, the rest is zero.
 template <typename T>
@@ -96,6 +117,21 @@ cudaError_t launch_convert_q(const double *Q_c128, void *dst, int64_t rows, int3
   else
     convert_q_kernel<double2><<<grid, 256, 0, s>>>(reinterpret_cast<const double2 *>(Q_c128),
                                                    reinterpret_cast<double2 *>(dst), rows, n_t, n_tp);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_convert_q_ext(const double *Q_c128, void *dst, int64_t rows, int32_t n_t, int32_t n_te, bool to_fp32,
+                                 cudaStream_t s) {
+  const int64_t total = rows * n_te;
+  int grid = (int)((total + 255) / 256);
+  if (grid > 148 * 16) grid = 148 * 16;
+  if (grid < 1) grid = 1;
+  if (to_fp32)
+    convert_q_ext_kernel<float2><<<grid, 256, 0, s>>>(reinterpret_cast<const double2 *>(Q_c128),
+                                                      reinterpret_cast<float2 *>(dst), rows, n_t, n_te);
+  else
+    convert_q_ext_kernel<double2><<<grid, 256, 0, s>>>(reinterpret_cast<const double2 *>(Q_c128),
+                                                       reinterpret_cast<double2 *>(dst), rows, n_t, n_te);
   return cudaGetLastError();
 }
 

@@ -64,7 +64,7 @@ reduce_partial_kernel(int64_t n_per_seg, const double *__restrict__ lnL, const d
       const double w = exp(v - mx);
       s1 += w;
       s2 += w * w;
-      if (has_params) {
+      if (has_params && w > 1e-25) {       // smaller weights cannot move a normalised bin by 1e-25 (the block max has w = 1)
 #pragma unroll
         for (int d = 0; d < 6; ++d) {
           const double x = ha.p[d][base + i];
@@ -181,10 +181,12 @@ reduce_merge_kernel(int64_t n_per_seg, int n_seg, int nbx, int n_bins, int merge
 
 }  // namespace
 
-int32_t reduce_blocks_per_seg(int64_t n_per_seg) {
-  int64_t b = (n_per_seg + 16383) / 16384;
+// ~2048 samples per block, at most ~4096 blocks over all segments (the partial buffer is n_seg * blocks * (4 + 6 n_bins))
+int32_t reduce_blocks_per_seg(int64_t n_per_seg, int32_t n_seg) {
+  int64_t b = (n_per_seg + 2047) / 2048;
+  const int64_t cap = 4096 / (n_seg > 0 ? n_seg : 1);
+  if (b > cap) b = cap;
   if (b < 1) b = 1;
-  if (b > 64) b = 64;
   return (int32_t)b;
 }
 

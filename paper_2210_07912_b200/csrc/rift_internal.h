@@ -75,6 +75,12 @@ cudaError_t launch_convert_q_planar(const double *Q_c128, void *dst, int64_t row
 size_t lnl_direct_smem_bytes(const QStore &q, bool fp32, bool q_in_smem);
 cudaError_t launch_lnl_direct(const QStore &q, bool fp32, bool q_in_smem, const Batch &b, const Workspace &ws,
                               int n_det, double *lnL_out, int n_sm, cudaStream_t s, int *n_launch);
+// lnl_direct_ext.cu (interleaved layout with a circular extension of RIFT_EXT samples per row)
+size_t lnl_direct_ext_smem_bytes(const QStore &q, bool fp32);
+cudaError_t launch_lnl_direct_ext(const QStore &q, bool fp32, const Batch &b, const Workspace &ws, int n_det,
+                                  double *lnL_out, int n_sm, cudaStream_t s, int *n_launch);
+cudaError_t launch_convert_q_ext(const double *Q_c128, void *dst, int64_t rows, int32_t n_t, int32_t n_te, bool to_fp32,
+                                 cudaStream_t s);
 // reduce.cu
 struct ReduceState {             // device, per segment
   double m, s1, s2;
@@ -85,7 +91,7 @@ cudaError_t launch_reduce(int32_t n_seg, int64_t n_per_seg, const double *lnL, c
                           int merge, ReduceState *state, double *state_hist, double *partial, int32_t blocks_per_seg,
                           double *out_scalars /*[4][n_seg]*/, double *out_hist, cudaStream_t s, int *n_launch);
 size_t reduce_partial_doubles(int32_t n_seg, int32_t blocks_per_seg, int32_t n_bins);
-int32_t reduce_blocks_per_seg(int64_t n_per_seg);
+int32_t reduce_blocks_per_seg(int64_t n_per_seg, int32_t n_seg);
 // convert.cu
 cudaError_t launch_convert_q(const double *Q_c128, void *dst, int64_t rows, int32_t n_t, int32_t n_tp, bool to_fp32,
                              cudaStream_t s);

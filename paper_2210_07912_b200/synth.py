@@ -338,8 +338,12 @@ class ConfigInputs:
 
 
 def build_inputs(cfg: Config, geometry_fn: GeometryFn, n_points: Optional[int] = None,
-                 noise: bool = True) -> ConfigInputs:
+                 noise: bool = True, point_ids: Optional[Sequence[int]] = None) -> ConfigInputs:
+    """point_ids: the seeds' point indices (default 0..P-1); a multi-GPU run gives every rank its own ids."""
     P = cfg.n_points if n_points is None else int(n_points)
+    if point_ids is None:
+        point_ids = list(range(P))
+    P = len(point_ids)
     loc, resp = detector_arrays(cfg)
     ml, mm = mode_arrays(cfg)
     K, M, n_t = cfg.n_det, cfg.n_modes, cfg.n_t
@@ -348,11 +352,11 @@ def build_inputs(cfg: Config, geometry_fn: GeometryFn, n_points: Optional[int] =
     V = np.empty((P, K, M, M), dtype=np.complex128)
     th = np.empty((P, 6), dtype=np.float64)
     pts = []
-    for p in range(P):
-        th[p] = true_point(cfg, p)
+    for p, pid in enumerate(point_ids):
+        th[p] = true_point(cfg, pid)
         F, Y, shift = geometry_fn(th[p])
         coeff = np.asarray(F).reshape(K, 1) * np.asarray(Y).reshape(1, M)
-        pd = make_point(cfg, p, coeff, shift, D_REF_MPC / th[p, 5], noise=noise)
+        pd = make_point(cfg, pid, coeff, shift, D_REF_MPC / th[p, 5], noise=noise)
         Q[p], U[p], V[p] = pd.Q, pd.U, pd.V
         pts.append(PointData(None, None, None, pd.rho, pd.scale))
     return ConfigInputs(cfg, loc, resp, ml, mm, Q, U, V, th, pts)

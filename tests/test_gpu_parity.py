@@ -89,7 +89,7 @@ def test_higher_l_harmonics(torch, oracle):
 
 
 # ------------------------------------------------------------------------------------------------ C0, whole config
-KERNELS = [rift.RIFT_KERNEL_DIRECT, rift.RIFT_KERNEL_GROUPED]
+KERNELS = [rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_DIRECT, rift.RIFT_KERNEL_GROUPED]
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
