@@ -225,6 +225,11 @@ bool use_grouped(const rift_ile *h) {
   if (h->kernel_variant != RIFT_KERNEL_GROUPED) return false;
   return h->d_Qp != nullptr;
 }
+bool use_quad(const rift_ile *h) {
+  if (h->kernel_variant != RIFT_KERNEL_QUAD) return false;
+  const bool fp32 = h->precision == RIFT_PREC_MIXED;
+  return h->d_Qe != nullptr && lnl_quad_smem_bytes(h->qse, fp32) <= 227u * 1024u;
+}
 
 int32_t next_pow2(int64_t v) {
   int32_t p = 1;
@@ -241,7 +246,8 @@ int run_chunks(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *cons
   if (rc != RIFT_OK) return rc;
   const bool fp32 = h->precision == RIFT_PREC_MIXED;
   const bool in_smem = q_fits_smem(h);
-  const bool grouped = lnL_out != nullptr && use_grouped(h);
+  const bool quad = lnL_out != nullptr && use_quad(h);
+  const bool grouped = lnL_out != nullptr && (use_grouped(h) || quad);      // "grouped": sort the chunk first
   for (int64_t g0 = 0; g0 < total; g0 += cap) {
     Batch b;
     b.n_per_seg = n_per_seg;
@@ -288,7 +294,10 @@ int run_chunks(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *cons
     if (lnL_out) {
       int nl = 0;
       ProfSpan ps(h, 1, s);
-      if (grouped) {
+      if (quad) {
+        CU(h, launch_lnl_quad(h->qse, fp32, b, ws, h->K, lnL_out, h->n_sm, s, &nl));
+        h->kernel_name = fp32 ? "lnl_quad<f32>" : "lnl_quad<f64>";
+      } else if (grouped) {
         CU(h, launch_lnl_grouped(h->qsp, fp32, b, ws, h->K, lnL_out, h->n_sm, s, &nl));
         h->kernel_name = fp32 ? "lnl_grouped<f32>" : "lnl_grouped<f64>";
       } else if (h->d_Qe != nullptr && fp32 && h->kernel_variant != RIFT_KERNEL_DIRECT) {
@@ -506,7 +515,7 @@ int rift_ile_destroy(rift_ile_t *h) {
 
 int rift_ile_set_kernel(rift_ile_t *h, int32_t variant) {
   if (!h) return RIFT_EINVAL;
-  if (variant != RIFT_KERNEL_AUTO && variant != RIFT_KERNEL_DIRECT && variant != RIFT_KERNEL_GROUPED)
+  if (variant != RIFT_KERNEL_AUTO && variant != RIFT_KERNEL_DIRECT && variant != RIFT_KERNEL_GROUPED && variant != RIFT_KERNEL_QUAD)
     return fail(h, RIFT_EINVAL, "unknown kernel variant");
   h->kernel_variant = variant;
   return RIFT_OK;

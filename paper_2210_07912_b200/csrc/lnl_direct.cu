@@ -126,8 +126,11 @@ lnl_direct_kernel(QStore q, Batch b, Workspace ws, int K, double *__restrict__ l
           bsum = s;
         }
         bsum = warp_sum(bsum);
-        if (bmax > run_max) {
-          run_sum = run_sum * exp(c * ((double)run_max - (double)bmax)) + bsum;   // exp(-inf) = 0 on the first block
+        if (jb == 0) {                         // first block (the only one when N_tau <= 416)
+          run_sum = bsum;
+          run_max = bmax;
+        } else if (bmax > run_max) {
+          run_sum = run_sum * exp(c * ((double)run_max - (double)bmax)) + bsum;
           run_max = bmax;
         } else {
           run_sum += bsum * exp(c * ((double)bmax - (double)run_max));

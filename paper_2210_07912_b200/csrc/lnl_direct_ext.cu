@@ -53,7 +53,7 @@ lnl_direct_ext_kernel(QStore q, Batch b, Workspace ws, int K, double *__restrict
   CT *coef_s = reinterpret_cast<CT *>(smem_raw + 128 + q.point_stride_bytes);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int km = q.km, M = km / K;
-  CT *wcoef = coef_s + warp * km;
+  CT *wcoef = coef_s + warp * (2 * km);           // [2][km], double-buffered
   const uint32_t wcoef_addr = smem_u32(wcoef);
   const uint32_t q_addr = smem_u32(Qs);
   uint32_t row_bytes = (uint32_t)(q.n_tp * sizeof(CT));
@@ -82,16 +82,42 @@ lnl_direct_ext_kernel(QStore q, Batch b, Workspace ws, int K, double *__restrict
       staged_point = point;
     }
 
-    for (int64_t w = w0 + warp; w < run_end; w += E_WARPS) {     // w = workspace slot
-      const double c = ws.scale_c[w];
-      const double quad = ws.quad[w];
-      int my_shift = (lane < K) ? ws.shift[w * K + lane] : 0;
-      __syncwarp();
-      {
-        const CT *src = reinterpret_cast<const CT *>(reinterpret_cast<const Real *>(ws.coef) + w * ws.coef_stride);
-        for (int i = lane; i < km; i += 32) wcoef[i] = src[i];
+    // The NEXT sample's scalars are prefetched into registers and its coefficient vector into the other half of the
+    // per-warp shared buffer (cp.async) while the current sample is evaluated.
+    auto fetch_coef = [&](int64_t w, int buf) {
+      const CT *src = reinterpret_cast<const CT *>(reinterpret_cast<const Real *>(ws.coef) + w * ws.coef_stride);
+      for (int i = lane; i < km; i += 32) {
+        const uint32_t dst = wcoef_addr + (uint32_t)((buf * km + i) * sizeof(CT));
+        if (sizeof(CT) == 8)
+          asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src + i) : "memory");
+        else
+          asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src + i) : "memory");
       }
+      asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    int buf = 0;
+    int64_t w = w0 + warp;
+    double n_c = 0.0, n_quad = 0.0;
+    int n_shift = 0;
+    if (w < run_end) {
+      n_c = ws.scale_c[w];
+      n_quad = ws.quad[w];
+      n_shift = (lane < K) ? ws.shift[w * K + lane] : 0;
+      fetch_coef(w, buf);
+    }
+    for (; w < run_end; w += E_WARPS, buf ^= 1) {                // w = workspace slot
+      const double c = n_c, quad = n_quad;
+      const int my_shift = n_shift;
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
       __syncwarp();
+      const int64_t wn = w + E_WARPS;
+      if (wn < run_end) {
+        n_c = ws.scale_c[wn];
+        n_quad = ws.quad[wn];
+        n_shift = (lane < K) ? ws.shift[wn * K + lane] : 0;
+        fetch_coef(wn, buf ^ 1);
+      }
+      const uint32_t wc_addr = wcoef_addr + (uint32_t)(buf * km * sizeof(CT));
 
       Real run_max = -INFINITY;
       double run_sum = 0.0;
@@ -104,7 +130,7 @@ lnl_direct_ext_kernel(QStore q, Batch b, Workspace ws, int K, double *__restrict
           int base = (j0 + __shfl_sync(0xffffffffu, my_shift, k) + jb) % q.n_t;
           if (base < 0) base += q.n_t;
           uint32_t addr = q_addr + (uint32_t)((k * M) * q.n_tp + base + lane) * (uint32_t)sizeof(CT);
-          uint32_t caddr = wcoef_addr + (uint32_t)(k * M * sizeof(CT));
+          uint32_t caddr = wc_addr + (uint32_t)(k * M * sizeof(CT));
           CT va[SLOTS], vb[SLOTS];
           load_row<Real>(va, addr);
 #pragma unroll 1
@@ -146,15 +172,21 @@ lnl_direct_ext_kernel(QStore q, Batch b, Workspace ws, int K, double *__restrict
           bsum = s;
         }
         bsum = warp_sum(bsum);
-        if (bmax > run_max) {
-          run_sum = run_sum * exp(c * ((double)run_max - (double)bmax)) + bsum;   // exp(-inf) = 0 on the first block
+        if (jb == 0) {                         // first block (the only one when N_tau <= 416)
+          run_sum = bsum;
+          run_max = bmax;
+        } else if (bmax > run_max) {
+          run_sum = run_sum * exp(c * ((double)run_max - (double)bmax)) + bsum;
           run_max = bmax;
         } else {
           run_sum += bsum * exp(c * ((double)bmax - (double)run_max));
         }
       }
-      if (lane == 0)
-        lnL_out[b.g0 + (ws.orig ? ws.orig[w] : w)] = c * (double)run_max + log(run_sum) - ln_ntau - quad;
+      if (lane == 0) {
+        // ln of the sum of exponentials (1 <= sum <= N_tau): logf is accurate to ~1e-6 absolute here (reading B5)
+        const double ls = (sizeof(Real) == 4) ? (double)logf((float)run_sum) : log(run_sum);
+        lnL_out[b.g0 + (ws.orig ? ws.orig[w] : w)] = c * (double)run_max + ls - ln_ntau - quad;
+      }
     }
     w0 = run_end;
   }
@@ -181,7 +213,7 @@ cudaError_t launch_t(const QStore &q, const Batch &b, const Workspace &ws, int K
 
 size_t lnl_direct_ext_smem_bytes(const QStore &q, bool fp32) {
   const size_t csz = fp32 ? 8 : 16;
-  return 128 + (size_t)q.point_stride_bytes + (size_t)E_WARPS * q.km * csz;
+  return 128 + (size_t)q.point_stride_bytes + (size_t)E_WARPS * 2 * q.km * csz;
 }
 
 cudaError_t launch_lnl_direct_ext(const QStore &q, bool fp32, const Batch &b, const Workspace &ws, int n_det,

@@ -81,6 +81,10 @@ cudaError_t launch_lnl_direct_ext(const QStore &q, bool fp32, const Batch &b, co
                                   double *lnL_out, int n_sm, cudaStream_t s, int *n_launch);
 cudaError_t launch_convert_q_ext(const double *Q_c128, void *dst, int64_t rows, int32_t n_t, int32_t n_te, bool to_fp32,
                                  cudaStream_t s);
+// lnl_quad.cu (sorted samples, NQ per warp, same extended interleaved layout as lnl_direct_ext)
+size_t lnl_quad_smem_bytes(const QStore &q, bool fp32);
+cudaError_t launch_lnl_quad(const QStore &q, bool fp32, const Batch &b, const Workspace &ws, int n_det, double *lnL_out,
+                            int n_sm, cudaStream_t s, int *n_launch);
 // reduce.cu
 struct ReduceState {             // device, per segment
   double m, s1, s2;

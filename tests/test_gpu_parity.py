@@ -89,7 +89,7 @@ def test_higher_l_harmonics(torch, oracle):
 
 
 # ------------------------------------------------------------------------------------------------ C0, whole config
-KERNELS = [rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_DIRECT, rift.RIFT_KERNEL_GROUPED]
+KERNELS = [rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_DIRECT, rift.RIFT_KERNEL_GROUPED, rift.RIFT_KERNEL_QUAD]
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
@@ -106,6 +106,7 @@ def test_c0_all_samples_both_precisions(torch, oracle, rho, kernel):
         got = lnL.cpu().numpy()
         assert np.array_equal(sh.cpu().numpy()[fr == 0], sh_ref[fr == 0])
         assert ("grouped" in rift.rift_ile_kernel_name(h)) == (kernel == rift.RIFT_KERNEL_GROUPED)
+        assert ("quad" in rift.rift_ile_kernel_name(h)) == (kernel == rift.RIFT_KERNEL_QUAD)
         if prec == rift.RIFT_PREC_FP64:
             assert np.max(rel_err(got, ref)) < TOL_FP64_REL, name
         else:
