@@ -22,6 +22,12 @@ struct rift_ile {
   QStore qse{};
   void *d_Qp = nullptr;            // planar, circularly extended copy for the grouped kernel (NULL if it cannot fit)
   QStore qsp{};
+  TcPlan tc{};                     // tensor-core path (lnl_tc.cu); tc.ok == 0 when the configuration does not fit
+  float *d_Qtc = nullptr;          // A operand: [P][K][nt*128][ka] tf32 words
+  float *tc_blob = nullptr;        // per-chunk workspace of the tensor-core path
+  double *tc_c = nullptr, *tc_quad = nullptr;
+  float2 *tc_part = nullptr;
+  int64_t tc_cap = 0;              // batches the workspace holds
   SortPlan plan{};
   int32_t *d_bucket = nullptr, *d_perm = nullptr;
   uint32_t *d_hist = nullptr;
@@ -143,6 +149,11 @@ void free_handle(rift_ile *h) {
   cudaFree(h->d_Q);
   cudaFree(h->d_Qp);
   cudaFree(h->d_Qe);
+  cudaFree(h->d_Qtc);
+  cudaFree(h->tc_blob);
+  cudaFree(h->tc_c);
+  cudaFree(h->tc_quad);
+  cudaFree(h->tc_part);
   cudaFree(h->d_bucket);
   cudaFree(h->d_perm);
   cudaFree(h->d_hist);
@@ -235,6 +246,102 @@ int32_t next_pow2(int64_t v) {
   int32_t p = 1;
   while (p < v && p < (1 << 30)) p <<= 1;
   return p;
+}
+
+
+// ---- tensor-core path ------------------------------------------------------------------------------------------------
+void make_tc_plan(rift_ile *h, double delta_t) {
+  TcPlan &tp = h->tc;
+  tp = TcPlan{};
+  tp.K = h->K;
+  tp.M = h->M;
+  tp.n_t = h->n_t;
+  tp.nt = (h->n_t + 127) / 128;
+  tp.kh = (2 * h->M + 3) & ~3;
+  tp.ka = (2 * tp.kh + 7) & ~7;
+  tp.kb2 = (tp.kh + 7) & ~7;
+  tp.nch = tp.ka / 4 + tp.kb2 / 4;
+  tp.H = 0;
+  for (int k = 1; k < h->K; ++k) {
+    double d2 = 0;
+    for (int i = 0; i < 3; ++i) {
+      const double d = h->geom.loc[k][i] - h->geom.loc[0][i];
+      d2 += d * d;
+    }
+    const double dm = std::ceil(std::sqrt(d2) / (RIFT_C_LIGHT * delta_t)) + 1.0;
+    if (dm > 1e6) return;
+    tp.dmax[k] = (int)dm;
+    if (tp.dmax[k] > tp.H) tp.H = tp.dmax[k];
+  }
+  tp.pitch = tp.n_t + 2 * tp.H;
+  tp.blob_words = tp.K * tp.nch * 64 + tp.K * 16 + 16;
+  tp.dcol0 = tp.K * tp.nt * tp.ka;
+  const bool fits = h->precision == RIFT_PREC_MIXED && h->n_tau == h->n_t && tp.nt <= 4 && h->M <= 16 &&
+                    tp.K * tp.nt * (tp.ka + RIFT_TC_NB) <= 512 && tp.H < tp.n_t &&
+                    lnl_tc_smem_bytes(tp) <= 227u * 1024u;
+  tp.ok = fits ? 1 : 0;
+}
+
+bool use_tc(const rift_ile *h) {
+  if (!h->tc.ok || h->d_Qtc == nullptr) return false;
+  return h->kernel_variant == RIFT_KERNEL_AUTO || h->kernel_variant == RIFT_KERNEL_TC;
+}
+
+int ensure_tc_workspace(rift_ile *h, int64_t n_batches) {
+  if (n_batches <= h->tc_cap) return RIFT_OK;
+  cudaFree(h->tc_blob);
+  cudaFree(h->tc_c);
+  cudaFree(h->tc_quad);
+  cudaFree(h->tc_part);
+  h->tc_blob = nullptr;
+  h->tc_c = h->tc_quad = nullptr;
+  h->tc_part = nullptr;
+  h->tc_cap = 0;
+  const size_t slots = (size_t)n_batches * RIFT_TC_NB;
+  CU(h, cudaMalloc(&h->tc_blob, (size_t)n_batches * h->tc.blob_words * sizeof(float)));
+  CU(h, cudaMalloc(&h->tc_c, slots * sizeof(double)));
+  CU(h, cudaMalloc(&h->tc_quad, slots * sizeof(double)));
+  CU(h, cudaMalloc(&h->tc_part, slots * 4 * sizeof(float2)));
+  h->tc_cap = n_batches;
+  return RIFT_OK;
+}
+
+// chunks of whole 16-sample batches; per-chunk workspace near 64 MiB so that it stays in the 126 MB L2
+int run_chunks_tc(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *const params[6], double *lnL_out,
+                  int32_t *shift_out, cudaStream_t s) {
+  const int64_t nbps = (n_per_seg + RIFT_TC_NB - 1) / RIFT_TC_NB;
+  const int64_t total = (int64_t)n_seg * nbps;
+  if (total == 0) return RIFT_OK;
+  const size_t per_batch = (size_t)h->tc.blob_words * 4 + (size_t)RIFT_TC_NB * (16 + 32);
+  int64_t cap = (int64_t)((64u << 20) / per_batch);
+  if (cap < 8 * (int64_t)h->n_sm) cap = 8 * (int64_t)h->n_sm;
+  int rc = ensure_tc_workspace(h, total < cap ? total : cap);
+  if (rc != RIFT_OK) return rc;
+  for (int64_t gb0 = 0; gb0 < total; gb0 += cap) {
+    TcChunk c;
+    c.n_per_seg = n_per_seg;
+    c.nbps = nbps;
+    c.gb0 = gb0;
+    c.n_batches = (total - gb0 < cap) ? total - gb0 : cap;
+    c.ids = h->d_ids;
+    c.blob = h->tc_blob;
+    c.scale_c = h->tc_c;
+    c.quad = h->tc_quad;
+    c.part = h->tc_part;
+    {
+      ProfSpan ps(h, 0, s);
+      CU(h, launch_geometry_tc(h->geom, h->d_modes, h->tc, c, params, h->d_U, h->d_V, shift_out, s));
+      ps.end();
+    }
+    ++h->launches;
+    int nl = 0;
+    ProfSpan ps(h, 1, s);
+    CU(h, launch_lnl_tc(h->tc, h->d_Qtc, c, lnL_out, h->n_sm, s, &nl));
+    ps.end();
+    h->launches += nl;
+  }
+  h->kernel_name = "lnl_tc<tf32x3>";
+  return RIFT_OK;
 }
 
 int run_chunks(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *const params[6], double *lnL_out,
@@ -471,6 +578,14 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
         ++h->launches;
       }
     }
+    // A operand of the tensor-core path (tf32 hi | lo pieces), when the configuration fits tensor memory
+    make_tc_plan(h, cfg->delta_t);
+    if (e == cudaSuccess && h->tc.ok) {
+      const size_t words = (size_t)h->P * h->K * h->tc.nt * 128 * h->tc.ka;
+      e = cudaMalloc(&h->d_Qtc, words * sizeof(float));
+      if (e == cudaSuccess) e = launch_convert_q_tc(src, h->d_Qtc, h->tc, h->P, 0);
+      ++h->launches;
+    }
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     cudaFree(tmp);
     if (e != cudaSuccess) return bail(RIFT_ECUDA);
@@ -515,7 +630,8 @@ int rift_ile_destroy(rift_ile_t *h) {
 
 int rift_ile_set_kernel(rift_ile_t *h, int32_t variant) {
   if (!h) return RIFT_EINVAL;
-  if (variant != RIFT_KERNEL_AUTO && variant != RIFT_KERNEL_DIRECT && variant != RIFT_KERNEL_GROUPED && variant != RIFT_KERNEL_QUAD)
+  if (variant != RIFT_KERNEL_AUTO && variant != RIFT_KERNEL_DIRECT && variant != RIFT_KERNEL_GROUPED && variant != RIFT_KERNEL_QUAD &&
+      variant != RIFT_KERNEL_TC)
     return fail(h, RIFT_EINVAL, "unknown kernel variant");
   h->kernel_variant = variant;
   return RIFT_OK;
@@ -534,6 +650,7 @@ int rift_ile_eval_batch(rift_ile_t *h, int32_t n_seg, const int32_t *intrinsic_i
   cudaStream_t s = reinterpret_cast<cudaStream_t>(cuda_stream);
   int rc = upload_ids(h, n_seg, intrinsic_ids, s);
   if (rc != RIFT_OK) return rc;
+  if (use_tc(h)) return run_chunks_tc(h, n_seg, n_per_seg, params, lnL_out, shift_out, s);
   return run_chunks(h, n_seg, n_per_seg, params, lnL_out, shift_out, nullptr, nullptr, nullptr, s);
 }
 

@@ -11,23 +11,16 @@ namespace {
 
 constexpr int GEOM_THREADS = 128;
 
-template <typename CT>
-__global__ void __launch_bounds__(GEOM_THREADS)
-geometry_kernel(DetGeom g, const ModeEntry *__restrict__ modes, Batch b, const double *__restrict__ p_ra,
-                const double *__restrict__ p_dec, const double *__restrict__ p_psi, const double *__restrict__ p_iota,
-                const double *__restrict__ p_phi, const double *__restrict__ p_dist, const double *__restrict__ U,
-                const double *__restrict__ V, Workspace ws, int32_t *__restrict__ shift_out,
-                double *__restrict__ dbg_F, double *__restrict__ dbg_Y, const int32_t *__restrict__ perm) {
-  const int64_t w = (int64_t)blockIdx.x * GEOM_THREADS + threadIdx.x;     // workspace slot (sorted position)
-  if (w >= b.n) return;
-  const int64_t src = perm ? (int64_t)perm[w] : w;                         // chunk-local index of the sample
-  if (ws.orig) ws.orig[w] = (int32_t)src;
-  const int64_t gi = b.g0 + src;                                           // caller's sample index
-  const int32_t point = b.ids[gi / b.n_per_seg];
+// a1-a4 for one sample.  Outputs: shifts s_k, F_k, Y_lm (arrays sized by the caller), c = D_ref/D (NaN for an invalid
+// sample) and the quadratic term q.
+template <int MAXM>
+__device__ __forceinline__ void sample_geometry(const DetGeom &g, const ModeEntry *__restrict__ modes, double ra, double dec,
+                                                double psi, double iota, double phi, double dist, int32_t point,
+                                                const double *__restrict__ U, const double *__restrict__ V,
+                                                int32_t (&shift)[RIFT_MAX_DET], double (&Fre)[RIFT_MAX_DET],
+                                                double (&Fim)[RIFT_MAX_DET], double (&Yre)[MAXM], double (&Yim)[MAXM],
+                                                double &c_out, double &q_out) {
   const int K = g.n_det, M = g.n_modes;
-
-  const double ra = p_ra[gi], dec = p_dec[gi], psi = p_psi[gi], iota = p_iota[gi], phi = p_phi[gi], dist = p_dist[gi];
-
   double sd, cd, sh, ch, sp, cp;
   sincos(dec, &sd, &cd);
   sincos(ra - g.gmst, &sh, &ch);           // ch = cos(ra-gmst) = cos(gha), sh = sin(ra-gmst) = -sin(gha)
@@ -35,43 +28,34 @@ geometry_kernel(DetGeom g, const ModeEntry *__restrict__ modes, Batch b, const d
 
   // ---- a3: delays and integer shifts, every operation individually rounded (no FMA contraction)
   const double nx = __dmul_rn(cd, ch), ny = __dmul_rn(cd, sh), nz = sd;
-  int32_t *my_shift = ws.shift + w * K;
-  for (int k = 0; k < K; ++k) {
-    const double dot = __dadd_rn(__dadd_rn(__dmul_rn(g.loc[k][0], nx), __dmul_rn(g.loc[k][1], ny)),
-                                 __dmul_rn(g.loc[k][2], nz));
-    const double dt = -__ddiv_rn(dot, RIFT_C_LIGHT);
-    const double x = __ddiv_rn(dt, g.delta_t);
-    const int32_t s = (int32_t)floor(__dadd_rn(x, 0.5));
-    my_shift[k] = s;
-    if (shift_out) shift_out[gi * K + k] = s;
+#pragma unroll
+  for (int k = 0; k < RIFT_MAX_DET; ++k) {
+    if (k < K) {
+      const double dot = __dadd_rn(__dadd_rn(__dmul_rn(g.loc[k][0], nx), __dmul_rn(g.loc[k][1], ny)),
+                                   __dmul_rn(g.loc[k][2], nz));
+      const double dt = -__ddiv_rn(dot, RIFT_C_LIGHT);
+      const double x = __ddiv_rn(dt, g.delta_t);
+      shift[k] = (int32_t)floor(__dadd_rn(x, 0.5));
+    }
   }
 
   // ---- a1: antenna factors
   const double sg = -sh, cg = ch;          // sin, cos of the Greenwich hour angle gmst - ra
   const double X[3] = {-cp * sg - sp * cg * sd, -cp * cg + sp * sg * sd, sp * cd};
   const double Yv[3] = {sp * sg - cp * cg * sd, sp * cg + cp * sg * sd, cp * cd};
-  double Fre[RIFT_MAX_DET], Fim[RIFT_MAX_DET];
+  // symmetric 3x3 forms: XX - YY and XY + YX (6 independent entries each)
+  const double pxx[6] = {X[0] * X[0] - Yv[0] * Yv[0], X[1] * X[1] - Yv[1] * Yv[1], X[2] * X[2] - Yv[2] * Yv[2],
+                         X[0] * X[1] - Yv[0] * Yv[1], X[0] * X[2] - Yv[0] * Yv[2], X[1] * X[2] - Yv[1] * Yv[2]};
+  const double pxy[6] = {2.0 * X[0] * Yv[0], 2.0 * X[1] * Yv[1], 2.0 * X[2] * Yv[2], X[0] * Yv[1] + X[1] * Yv[0],
+                         X[0] * Yv[2] + X[2] * Yv[0], X[1] * Yv[2] + X[2] * Yv[1]};
 #pragma unroll
   for (int k = 0; k < RIFT_MAX_DET; ++k) {
     if (k < K) {
       const double *D = g.resp[k];
-      double xdx = 0, ydy = 0, xdy = 0, ydx = 0;
-#pragma unroll
-      for (int i = 0; i < 3; ++i)
-#pragma unroll
-        for (int j = 0; j < 3; ++j) {
-          const double d = D[3 * i + j];
-          xdx += X[i] * d * X[j];
-          ydy += Yv[i] * d * Yv[j];
-          xdy += X[i] * d * Yv[j];
-          ydx += Yv[i] * d * X[j];
-        }
-      Fre[k] = xdx - ydy;
-      Fim[k] = xdy + ydx;
-      if (dbg_F) {
-        dbg_F[(gi * K + k) * 2] = Fre[k];
-        dbg_F[(gi * K + k) * 2 + 1] = Fim[k];
-      }
+      // D need not be exactly symmetric in the caller's array: use D_ij + D_ji for the off-diagonal pairs
+      const double d01 = D[1] + D[3], d02 = D[2] + D[6], d12 = D[5] + D[7];
+      Fre[k] = D[0] * pxx[0] + D[4] * pxx[1] + D[8] * pxx[2] + d01 * pxx[3] + d02 * pxx[4] + d12 * pxx[5];
+      Fim[k] = D[0] * pxy[0] + D[4] * pxy[1] + D[8] * pxy[2] + d01 * pxy[3] + d02 * pxy[4] + d12 * pxy[5];
     }
   }
 
@@ -95,70 +79,222 @@ geometry_kernel(DetGeom g, const ModeEntry *__restrict__ modes, Batch b, const d
       sm[i] = sm[i - 1] * c1 + cm[i - 1] * s1;
     }
   }
-  double Yre[RIFT_MAX_MODES], Yim[RIFT_MAX_MODES];
-  for (int a = 0; a < M; ++a) {
-    const ModeEntry &e = modes[a];
-    double amp = 0.0;
-    for (int t = 0; t < e.n_terms; ++t) amp += e.coef[t] * pc[e.pc[t]] * ps[e.ps[t]];
-    const int am = e.m < 0 ? -e.m : e.m;
-    // e^{i m (-phi)} = cos(m phi) - i sin(m phi)
-    Yre[a] = amp * cm[am];
-    Yim[a] = (e.m < 0) ? amp * sm[am] : -amp * sm[am];
-    if (dbg_Y) {
+#pragma unroll(MAXM <= 16 ? MAXM : 1)
+  for (int a = 0; a < MAXM; ++a) {
+    if (a < M) {
+      const ModeEntry &e = modes[a];
+      double amp = 0.0;
+      for (int t = 0; t < e.n_terms; ++t) amp += e.coef[t] * pc[e.pc[t]] * ps[e.ps[t]];
+      const int am = e.m < 0 ? -e.m : e.m;
+      // e^{i m (-phi)} = cos(m phi) - i sin(m phi)
+      Yre[a] = amp * cm[am];
+      Yim[a] = (e.m < 0) ? amp * sm[am] : -amp * sm[am];
+    }
+  }
+
+  const bool bad = !(dist > 0.0) || isnan(ra) || isnan(dec) || isnan(psi) || isnan(iota) || isnan(phi);
+  const double c = bad ? __longlong_as_double(0x7ff8000000000000LL) : g.d_ref / dist;
+  c_out = c;
+
+  // ---- a4: quadratic term; U Hermitian, V symmetric: diagonal + 2 * strict upper triangle.  The mode-pair products
+  // conj(Y_a) Y_b and Y_a Y_b do not depend on the detector and are formed once.
+  double yuy[RIFT_MAX_DET], yvr[RIFT_MAX_DET], yvi[RIFT_MAX_DET];
+#pragma unroll
+  for (int k = 0; k < RIFT_MAX_DET; ++k) yuy[k] = yvr[k] = yvi[k] = 0.0;
+  const double2 *Up = reinterpret_cast<const double2 *>(U) + (int64_t)point * K * M * M;
+  const double2 *Vp = reinterpret_cast<const double2 *>(V) + (int64_t)point * K * M * M;
+#pragma unroll(MAXM <= 16 ? MAXM : 1)
+  for (int a = 0; a < MAXM; ++a) {
+    if (a < M) {
+      const double ar = Yre[a], ai = Yim[a];
+#pragma unroll(MAXM <= 16 ? MAXM : 1)
+      for (int bb = a; bb < MAXM; ++bb) {
+        if (bb < M) {
+          const double br = Yre[bb], bi = Yim[bb];
+          const double w = (bb == a) ? 1.0 : 2.0;
+          const double cr = w * (ar * br + ai * bi), ci = w * (ar * bi - ai * br);      // conj(Y_a) Y_b
+          const double pr = w * (ar * br - ai * bi), pi = w * (ar * bi + ai * br);      // Y_a Y_b
+#pragma unroll
+          for (int k = 0; k < RIFT_MAX_DET; ++k) {
+            if (k < K) {
+              const double2 u = Up[(k * M + a) * M + bb], v = Vp[(k * M + a) * M + bb];
+              yuy[k] += u.x * cr - u.y * ci;
+              yvr[k] += v.x * pr - v.y * pi;
+              yvi[k] += v.x * pi + v.y * pr;
+            }
+          }
+        }
+      }
+    }
+  }
+  double q = 0.0;
+#pragma unroll
+  for (int k = 0; k < RIFT_MAX_DET; ++k) {
+    if (k < K) {
+      const double f2 = Fre[k] * Fre[k] + Fim[k] * Fim[k];
+      const double f2r = Fre[k] * Fre[k] - Fim[k] * Fim[k], f2i = 2.0 * Fre[k] * Fim[k];
+      q += f2 * yuy[k] + (f2r * yvr[k] - f2i * yvi[k]);
+    }
+  }
+  q_out = 0.25 * c * c * q;
+}
+
+template <typename CT>
+__global__ void __launch_bounds__(GEOM_THREADS)
+geometry_kernel(DetGeom g, const ModeEntry *__restrict__ modes, Batch b, const double *__restrict__ p_ra,
+                const double *__restrict__ p_dec, const double *__restrict__ p_psi, const double *__restrict__ p_iota,
+                const double *__restrict__ p_phi, const double *__restrict__ p_dist, const double *__restrict__ U,
+                const double *__restrict__ V, Workspace ws, int32_t *__restrict__ shift_out,
+                double *__restrict__ dbg_F, double *__restrict__ dbg_Y, const int32_t *__restrict__ perm) {
+  const int64_t w = (int64_t)blockIdx.x * GEOM_THREADS + threadIdx.x;     // workspace slot (sorted position)
+  if (w >= b.n) return;
+  const int64_t src = perm ? (int64_t)perm[w] : w;                         // chunk-local index of the sample
+  if (ws.orig) ws.orig[w] = (int32_t)src;
+  const int64_t gi = b.g0 + src;                                           // caller's sample index
+  const int32_t point = b.ids[gi / b.n_per_seg];
+  const int K = g.n_det, M = g.n_modes;
+
+  int32_t shift[RIFT_MAX_DET];
+  double Fre[RIFT_MAX_DET], Fim[RIFT_MAX_DET], Yre[RIFT_MAX_MODES], Yim[RIFT_MAX_MODES], c, q;
+  sample_geometry<RIFT_MAX_MODES>(g, modes, p_ra[gi], p_dec[gi], p_psi[gi], p_iota[gi], p_phi[gi], p_dist[gi], point, U,
+                                  V, shift, Fre, Fim, Yre, Yim, c, q);
+  int32_t *my_shift = ws.shift + w * K;
+  for (int k = 0; k < K; ++k) {
+    my_shift[k] = shift[k];
+    if (shift_out) shift_out[gi * K + k] = shift[k];
+    if (dbg_F) {
+      dbg_F[(gi * K + k) * 2] = Fre[k];
+      dbg_F[(gi * K + k) * 2 + 1] = Fim[k];
+    }
+  }
+  if (dbg_Y)
+    for (int a = 0; a < M; ++a) {
       dbg_Y[(gi * M + a) * 2] = Yre[a];
       dbg_Y[(gi * M + a) * 2 + 1] = Yim[a];
     }
-  }
-
-  // ---- a5: coefficient vectors B = F_k Y_lm
-  const bool bad = !(dist > 0.0) || isnan(ra) || isnan(dec) || isnan(psi) || isnan(iota) || isnan(phi);
-  const double c = bad ? __longlong_as_double(0x7ff8000000000000LL) : g.d_ref / dist;
   ws.scale_c[w] = c;
-  {
-    CT *out = reinterpret_cast<CT *>(reinterpret_cast<decltype(CT::x) *>(ws.coef) + w * ws.coef_stride);
-    for (int k = 0; k < K; ++k)
-      for (int a = 0; a < M; ++a) {
-        CT v;
-        v.x = Fre[k] * Yre[a] - Fim[k] * Yim[a];
-        v.y = Fre[k] * Yim[a] + Fim[k] * Yre[a];
-        out[k * M + a] = v;
-      }
-  }
-
-  // ---- a4: quadratic term; U Hermitian, V symmetric: diagonal + 2 * strict upper triangle
-  double q = 0.0;
-  for (int k = 0; k < K; ++k) {
-    const double2 *Uk = reinterpret_cast<const double2 *>(U) + ((int64_t)point * K + k) * M * M;
-    const double2 *Vk = reinterpret_cast<const double2 *>(V) + ((int64_t)point * K + k) * M * M;
-    double yuy = 0.0, yvy_re = 0.0, yvy_im = 0.0;
+  ws.quad[w] = q;
+  // ---- a5: coefficient vectors B = F_k Y_lm
+  CT *out = reinterpret_cast<CT *>(reinterpret_cast<decltype(CT::x) *>(ws.coef) + w * ws.coef_stride);
+  for (int k = 0; k < K; ++k)
     for (int a = 0; a < M; ++a) {
-      const double ar = Yre[a], ai = Yim[a];
-      {
-        const double2 u = Uk[a * M + a], v = Vk[a * M + a];
-        yuy += u.x * (ar * ar + ai * ai);
-        const double y2r = ar * ar - ai * ai, y2i = 2.0 * ar * ai;
-        yvy_re += v.x * y2r - v.y * y2i;
-        yvy_im += v.x * y2i + v.y * y2r;
-      }
-      for (int bb = a + 1; bb < M; ++bb) {
-        const double br = Yre[bb], bi = Yim[bb];
-        const double2 u = Uk[a * M + bb], v = Vk[a * M + bb];
-        // conj(Y_a) Y_b and Y_a Y_b
-        const double cr = ar * br + ai * bi, ci = ar * bi - ai * br;
-        const double pr = ar * br - ai * bi, pi = ar * bi + ai * br;
-        yuy += 2.0 * (u.x * cr - u.y * ci);
-        yvy_re += 2.0 * (v.x * pr - v.y * pi);
-        yvy_im += 2.0 * (v.x * pi + v.y * pr);
-      }
+      CT v;
+      v.x = Fre[k] * Yre[a] - Fim[k] * Yim[a];
+      v.y = Fre[k] * Yim[a] + Fim[k] * Yre[a];
+      out[k * M + a] = v;
     }
-    const double f2 = Fre[k] * Fre[k] + Fim[k] * Fim[k];
-    const double f2r = Fre[k] * Fre[k] - Fim[k] * Fim[k], f2i = 2.0 * Fre[k] * Fim[k];
-    q += f2 * yuy + (f2r * yvy_re - f2i * yvy_im);
+}
+
+// round an fp32 value to TF32 (10 explicit mantissa bits), nearest-even
+__device__ __forceinline__ float tf32_rn(float f) {
+  uint32_t u = __float_as_uint(f);
+  u += 0xFFFu + ((u >> 13) & 1u);
+  u &= 0xFFFFE000u;
+  return __uint_as_float(u);
+}
+
+// Tensor-core variant: one thread per batch slot; writes the batch blob described at TcPlan (rift_internal.h).
+template <int MAXM>
+__global__ void __launch_bounds__(GEOM_THREADS)
+geometry_tc_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, TcChunk ch, const double *__restrict__ p_ra,
+                   const double *__restrict__ p_dec, const double *__restrict__ p_psi, const double *__restrict__ p_iota,
+                   const double *__restrict__ p_phi, const double *__restrict__ p_dist, const double *__restrict__ U,
+                   const double *__restrict__ V, int32_t *__restrict__ shift_out) {
+  const int64_t w = (int64_t)blockIdx.x * GEOM_THREADS + threadIdx.x;     // slot = local batch * 16 + n
+  if (w >= ch.n_batches * RIFT_TC_NB) return;
+  const int64_t lb = w / RIFT_TC_NB;
+  const int n = (int)(w % RIFT_TC_NB);
+  const int64_t gb = ch.gb0 + lb;
+  const int64_t seg = gb / ch.nbps;
+  const int64_t i = (gb % ch.nbps) * RIFT_TC_NB + n;
+  const bool valid = i < ch.n_per_seg;
+  const int K = g.n_det, M = g.n_modes;
+  float *blob = ch.blob + lb * tp.blob_words;
+  float4 *chunks = reinterpret_cast<float4 *>(blob);                        // [K][nch][16] float4
+  int32_t *dsh = reinterpret_cast<int32_t *>(blob + K * tp.nch * 64);       // [K][16]
+  float *cl2 = blob + K * tp.nch * 64 + K * 16;                             // [16]
+  const int nc1 = tp.ka >> 2;                                               // chunks of B1
+  if (!valid) {
+    const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int k = 0; k < K; ++k) {
+      for (int c = 0; c < tp.nch; ++c) chunks[(k * tp.nch + c) * 16 + n] = z;
+      dsh[k * 16 + n] = 0;
+    }
+    cl2[n] = 0.f;
+    ch.scale_c[w] = 0.0;
+    ch.quad[w] = 0.0;
+    return;
   }
-  ws.quad[w] = 0.25 * c * c * q;
+  const int64_t gi = seg * ch.n_per_seg + i;
+  const int32_t point = ch.ids[seg];
+  int32_t shift[RIFT_MAX_DET];
+  double Fre[RIFT_MAX_DET], Fim[RIFT_MAX_DET], Yre[MAXM], Yim[MAXM], c, q;
+  sample_geometry<MAXM>(g, modes, p_ra[gi], p_dec[gi], p_psi[gi], p_iota[gi], p_phi[gi], p_dist[gi], point, U, V, shift,
+                        Fre, Fim, Yre, Yim, c, q);
+  ch.scale_c[w] = c;
+  ch.quad[w] = q;
+  cl2[n] = (float)(c * 1.4426950408889634);
+#pragma unroll
+  for (int k = 0; k < RIFT_MAX_DET; ++k) {
+    if (k < K) {
+      if (shift_out) shift_out[gi * K + k] = shift[k];
+      dsh[k * 16 + n] = shift[k] - shift[0];
+      // a5: B = F_k Y_lm split into tf32 hi + lo; kappa = 2a (Re), 2a+1 (Im)
+      float hi[2 * MAXM], lo[2 * MAXM];
+#pragma unroll
+      for (int a = 0; a < MAXM; ++a) {
+        double vr = 0.0, vi = 0.0;
+        if (a < M) {
+          vr = Fre[k] * Yre[a] - Fim[k] * Yim[a];
+          vi = Fre[k] * Yim[a] + Fim[k] * Yre[a];
+        }
+        hi[2 * a] = tf32_rn((float)vr);
+        hi[2 * a + 1] = tf32_rn((float)vi);
+        lo[2 * a] = tf32_rn((float)(vr - (double)hi[2 * a]));
+        lo[2 * a + 1] = tf32_rn((float)(vi - (double)hi[2 * a + 1]));
+      }
+      float4 *dst = chunks + (k * tp.nch) * 16 + n;
+      const int nh = tp.kh >> 2;                                           // chunks of the hi block
+#pragma unroll
+      for (int cc = 0; cc < (2 * MAXM + 3) / 4; ++cc) {
+        if (cc < nh) {
+          float4 vh, vl;
+          vh.x = (4 * cc + 0 < 2 * MAXM) ? hi[4 * cc + 0] : 0.f;
+          vh.y = (4 * cc + 1 < 2 * MAXM) ? hi[4 * cc + 1] : 0.f;
+          vh.z = (4 * cc + 2 < 2 * MAXM) ? hi[4 * cc + 2] : 0.f;
+          vh.w = (4 * cc + 3 < 2 * MAXM) ? hi[4 * cc + 3] : 0.f;
+          vl.x = (4 * cc + 0 < 2 * MAXM) ? lo[4 * cc + 0] : 0.f;
+          vl.y = (4 * cc + 1 < 2 * MAXM) ? lo[4 * cc + 1] : 0.f;
+          vl.z = (4 * cc + 2 < 2 * MAXM) ? lo[4 * cc + 2] : 0.f;
+          vl.w = (4 * cc + 3 < 2 * MAXM) ? lo[4 * cc + 3] : 0.f;
+          dst[cc * 16] = vh;                 // B1, hi block
+          dst[(nh + cc) * 16] = vh;          // B1, lo block of A multiplies hi of B
+          dst[(nc1 + cc) * 16] = vl;         // B2, hi block of A multiplies lo of B
+        }
+      }
+      const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+      for (int cc = 2 * nh; cc < nc1; ++cc) dst[cc * 16] = z;             // padding of B1
+      for (int cc = nc1 + nh; cc < tp.nch; ++cc) dst[cc * 16] = z;        // B2 columns facing A's lo block / padding
+    }
+  }
 }
 
 }  // namespace
+
+cudaError_t launch_geometry_tc(const DetGeom &g, const ModeEntry *modes, const TcPlan &tp, const TcChunk &c,
+                               const double *const params[6], const double *U, const double *V, int32_t *shift_out,
+                               cudaStream_t s) {
+  const int64_t n = c.n_batches * RIFT_TC_NB;
+  if (n <= 0) return cudaSuccess;
+  const unsigned grid = (unsigned)((n + GEOM_THREADS - 1) / GEOM_THREADS);
+  if (tp.M <= 8)
+    geometry_tc_kernel<8><<<grid, GEOM_THREADS, 0, s>>>(g, modes, tp, c, params[0], params[1], params[2], params[3],
+                                                         params[4], params[5], U, V, shift_out);
+  else
+    geometry_tc_kernel<16><<<grid, GEOM_THREADS, 0, s>>>(g, modes, tp, c, params[0], params[1], params[2], params[3],
+                                                          params[4], params[5], U, V, shift_out);
+  return cudaGetLastError();
+}
 
 cudaError_t launch_geometry(const DetGeom &g, const ModeEntry *modes, const Batch &b, const double *const params[6],
                             const double *U, const double *V, bool coef_fp32, const Workspace &ws,

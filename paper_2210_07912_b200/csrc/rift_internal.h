@@ -57,7 +57,32 @@ struct QStore {
 };
 #define RIFT_EXT 416             // 13 slots x 32 lanes: one time block of the fused kernels
 
+// Tensor-core path (lnl_tc.cu): plan of one handle.  Samples are processed in batches of RIFT_TC_NB consecutive samples
+// of one segment; the geometry kernel writes one "blob" per batch: the B operand of the UMMA in its canonical K-major
+// shared-memory layout, [K][nch][16][4] tf32 words (per detector: B1 = [hi | hi] over ka columns, then B2 = [lo | 0] over
+// kb2 columns, in 16-byte chunks of 4 columns), then the relative shifts d_k = s_k - s_0 as int32 [K][16], then
+// c*log2(e) as float [16].
+#define RIFT_TC_NB 16
+struct TcPlan {
+  int32_t ok;                    // 1 if this handle can run the tensor-core kernel
+  int32_t K, M, n_t, nt;         // nt = ceil(n_t / 128) row tiles
+  int32_t kh, ka, kb2, nch;      // hi block width (2M rounded up to 4), A columns (2*kh up to 8), B2 extent (kh up to 8), chunks
+  int32_t H, pitch;              // halo = max_k dmax[k]; exchange-row pitch in floats
+  int32_t blob_words, dcol0;     // 32-bit words per batch blob; first accumulator column in TMEM
+  int32_t dmax[RIFT_MAX_DET];    // bound on |s_k - s_0|
+};
+struct TcChunk {                 // a chunk = global batches [gb0, gb0 + n_batches), batch gb = seg * nbps + b
+  int64_t n_per_seg, nbps, gb0, n_batches;
+  const int32_t *ids;
+  float *blob;                   // [n_batches][blob_words]
+  double *scale_c, *quad;        // [n_batches * 16]
+  float2 *part;                  // [n_batches * 16][4]: per lane-quarter (reference, sum)
+};
+
 // geometry.cu
+cudaError_t launch_geometry_tc(const DetGeom &g, const ModeEntry *modes, const TcPlan &tp, const TcChunk &c,
+                               const double *const params[6], const double *U, const double *V, int32_t *shift_out,
+                               cudaStream_t s);
 cudaError_t launch_geometry(const DetGeom &g, const ModeEntry *modes, const Batch &b, const double *const params[6],
                             const double *U, const double *V, bool coef_fp32, const Workspace &ws,
                             int32_t *shift_out, double *dbg_F, double *dbg_Y, const int32_t *perm, cudaStream_t s);
@@ -85,6 +110,11 @@ cudaError_t launch_convert_q_ext(const double *Q_c128, void *dst, int64_t rows, 
 size_t lnl_quad_smem_bytes(const QStore &q, bool fp32);
 cudaError_t launch_lnl_quad(const QStore &q, bool fp32, const Batch &b, const Workspace &ws, int n_det, double *lnL_out,
                             int n_sm, cudaStream_t s, int *n_launch);
+// lnl_tc.cu (tcgen05 / TMEM contraction, shift applied through a shared-memory exchange)
+size_t lnl_tc_smem_bytes(const TcPlan &tp);
+cudaError_t launch_convert_q_tc(const double *Q_c128, float *dst, const TcPlan &tp, int32_t n_points, cudaStream_t s);
+cudaError_t launch_lnl_tc(const TcPlan &tp, const float *qtc, const TcChunk &c, double *lnL_out, int n_sm,
+                          cudaStream_t s, int *n_launch);
 // reduce.cu
 struct ReduceState {             // device, per segment
   double m, s1, s2;

@@ -89,7 +89,8 @@ def test_higher_l_harmonics(torch, oracle):
 
 
 # ------------------------------------------------------------------------------------------------ C0, whole config
-KERNELS = [rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_DIRECT, rift.RIFT_KERNEL_GROUPED, rift.RIFT_KERNEL_QUAD]
+KERNELS = [rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_DIRECT, rift.RIFT_KERNEL_GROUPED, rift.RIFT_KERNEL_QUAD,
+           rift.RIFT_KERNEL_TC]
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
@@ -107,6 +108,9 @@ def test_c0_all_samples_both_precisions(torch, oracle, rho, kernel):
         assert np.array_equal(sh.cpu().numpy()[fr == 0], sh_ref[fr == 0])
         assert ("grouped" in rift.rift_ile_kernel_name(h)) == (kernel == rift.RIFT_KERNEL_GROUPED)
         assert ("quad" in rift.rift_ile_kernel_name(h)) == (kernel == rift.RIFT_KERNEL_QUAD)
+        # the tensor-core kernel is the default of the mixed mode (and never runs in fp64 mode)
+        assert ("lnl_tc" in rift.rift_ile_kernel_name(h)) == (
+            prec == rift.RIFT_PREC_MIXED and kernel in (rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_TC))
         if prec == rift.RIFT_PREC_FP64:
             assert np.max(rel_err(got, ref)) < TOL_FP64_REL, name
         else:
@@ -178,6 +182,32 @@ def test_edge_sizes_and_invalid_samples(torch, oracle):
     with pytest.raises(rift.RiftError) as e:
         rift.rift_ile_eval_batch(h, [0], 4, p4, None)
     assert e.value.code == rift.RIFT_EINVAL
+    rift.rift_ile_destroy(h)
+
+
+def test_tc_edge_sizes_ragged_batches_and_invalid_samples(torch, oracle):
+    """Tensor-core kernel (mixed mode): sample counts around the 16-sample batch, several short segments in one call,
+    NaN / non-positive distance samples (NaN for that sample only)."""
+    cfg = synth.CONFIGS[1]
+    inp = build(oracle, cfg, n_points=2)
+    h = create(rift, inp, rift.RIFT_PREC_MIXED)
+    for n in (1, 7, 16, 17, 33):
+        ids = [1, 0, 1]
+        params = synth.prior_draw(np.random.default_rng(100 + n), n * len(ids))
+        got = gpu_eval(torch, h, ids, n, params, K=cfg.n_det, kernel=rift.RIFT_KERNEL_TC)[0].cpu().numpy()
+        assert "lnl_tc" in rift.rift_ile_kernel_name(h)
+        ref = np.concatenate([oracle_eval(oracle, inp, ids[s], params[:, s * n:(s + 1) * n])[0] for s in range(len(ids))])
+        assert np.max(np.abs(got - ref)) < TOL_MIXED_LNL, n
+    params = synth.prior_draw(np.random.default_rng(9), 64)
+    params[5, 3] = -10.0
+    params[5, 4] = 0.0
+    params[0, 5] = np.nan
+    params[3, 40] = np.nan
+    got = gpu_eval(torch, h, [0], 64, params, K=cfg.n_det, kernel=rift.RIFT_KERNEL_TC)[0].cpu().numpy()
+    ref = oracle_eval(oracle, inp, 0, params)[0]
+    assert np.array_equal(np.isnan(got), np.isnan(ref)) and np.isnan(got).sum() == 4
+    ok = ~np.isnan(ref)
+    assert np.max(np.abs(got[ok] - ref[ok])) < TOL_MIXED_LNL
     rift.rift_ile_destroy(h)
 
 
