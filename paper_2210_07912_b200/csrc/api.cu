@@ -23,7 +23,8 @@ struct rift_ile {
   void *d_Qp = nullptr;            // planar, circularly extended copy for the grouped kernel (NULL if it cannot fit)
   QStore qsp{};
   TcPlan tc{};                     // tensor-core path (lnl_tc.cu); tc.ok == 0 when the configuration does not fit
-  float *d_Qtc = nullptr;          // A operand: [P][K][nt*128][ka] tf32 words
+  uint32_t *d_Qtc = nullptr;       // A operand: [P][K][nt*128][acols] words of two fp16
+  float *d_qscale = nullptr;       // [P] power-of-two scale of each point's Q in the A operand
   float *tc_blob = nullptr;        // per-chunk workspace of the tensor-core path
   double *tc_c = nullptr, *tc_quad = nullptr;
   float2 *tc_part = nullptr;
@@ -150,6 +151,7 @@ void free_handle(rift_ile *h) {
   cudaFree(h->d_Qp);
   cudaFree(h->d_Qe);
   cudaFree(h->d_Qtc);
+  cudaFree(h->d_qscale);
   cudaFree(h->tc_blob);
   cudaFree(h->tc_c);
   cudaFree(h->tc_quad);
@@ -257,10 +259,9 @@ void make_tc_plan(rift_ile *h, double delta_t) {
   tp.M = h->M;
   tp.n_t = h->n_t;
   tp.nt = (h->n_t + 127) / 128;
-  tp.kh = (2 * h->M + 3) & ~3;
-  tp.ka = (2 * tp.kh + 7) & ~7;
-  tp.kb2 = (tp.kh + 7) & ~7;
-  tp.nch = tp.ka / 4 + tp.kb2 / 4;
+  tp.kp = (6 * h->M + 15) & ~15;
+  tp.nch = tp.kp / 8;
+  tp.acols = tp.kp / 2;
   tp.H = 0;
   for (int k = 1; k < h->K; ++k) {
     double d2 = 0;
@@ -273,11 +274,11 @@ void make_tc_plan(rift_ile *h, double delta_t) {
     tp.dmax[k] = (int)dm;
     if (tp.dmax[k] > tp.H) tp.H = tp.dmax[k];
   }
-  tp.pitch = tp.n_t + 2 * tp.H;
+  tp.pitch = lnl_tc_pitch(tp.n_t, tp.H);
   tp.blob_words = tp.K * tp.nch * 64 + tp.K * 16 + 16;
-  tp.dcol0 = tp.K * tp.nt * tp.ka;
-  const bool fits = h->precision == RIFT_PREC_MIXED && h->n_tau == h->n_t && tp.nt <= 4 && h->M <= 16 &&
-                    tp.K * tp.nt * (tp.ka + RIFT_TC_NB) <= 512 && tp.H < tp.n_t &&
+  tp.dcol0 = tp.K * tp.nt * tp.acols;
+  const bool fits = h->precision == RIFT_PREC_MIXED && h->n_tau == h->n_t && tp.nt <= 4 && h->M <= 8 &&
+                    tp.K * tp.nt * (tp.acols + RIFT_TC_NB) <= 512 && tp.H < tp.n_t && tp.pitch > 0 &&
                     lnl_tc_smem_bytes(tp) <= 227u * 1024u;
   tp.ok = fits ? 1 : 0;
 }
@@ -324,6 +325,7 @@ int run_chunks_tc(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *c
     c.gb0 = gb0;
     c.n_batches = (total - gb0 < cap) ? total - gb0 : cap;
     c.ids = h->d_ids;
+    c.qscale = h->d_qscale;
     c.blob = h->tc_blob;
     c.scale_c = h->tc_c;
     c.quad = h->tc_quad;
@@ -340,7 +342,7 @@ int run_chunks_tc(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *c
     ps.end();
     h->launches += nl;
   }
-  h->kernel_name = "lnl_tc<tf32x3>";
+  h->kernel_name = "lnl_tc<f16x3>";
   return RIFT_OK;
 }
 
@@ -581,10 +583,11 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
     // A operand of the tensor-core path (tf32 hi | lo pieces), when the configuration fits tensor memory
     make_tc_plan(h, cfg->delta_t);
     if (e == cudaSuccess && h->tc.ok) {
-      const size_t words = (size_t)h->P * h->K * h->tc.nt * 128 * h->tc.ka;
-      e = cudaMalloc(&h->d_Qtc, words * sizeof(float));
-      if (e == cudaSuccess) e = launch_convert_q_tc(src, h->d_Qtc, h->tc, h->P, 0);
-      ++h->launches;
+      const size_t words = (size_t)h->P * h->K * h->tc.nt * 128 * h->tc.acols;
+      e = cudaMalloc(&h->d_Qtc, words * sizeof(uint32_t));
+      if (e == cudaSuccess) e = cudaMalloc(&h->d_qscale, sizeof(float) * h->P);
+      if (e == cudaSuccess) e = launch_convert_q_tc(src, h->d_Qtc, h->d_qscale, h->tc, h->P, 0);
+      h->launches += 3;
     }
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     cudaFree(tmp);

@@ -5,6 +5,8 @@
 //   a3 dt_k = -(r_k . n)/c, s_k = floor(dt_k/delta_t + 1/2), pinned operation order   (reading G4; t_k of Eq. (D2))
 //   a4 q = (c^2/4) sum_k [ |F_k|^2 Y^dag U_k Y + Re(F_k^2 Y^T V_k Y) ]               (Eq. (D3))
 //   a5 coefficient vector B_{k,lm} = F_k Y_lm, so that Re sum conj(B) Q = sum (B.re Q.re + B.im Q.im)
+#include <cuda_fp16.h>
+
 #include "rift_internal.h"
 
 namespace {
@@ -185,16 +187,9 @@ geometry_kernel(DetGeom g, const ModeEntry *__restrict__ modes, Batch b, const d
     }
 }
 
-// round an fp32 value to TF32 (10 explicit mantissa bits), nearest-even
-__device__ __forceinline__ float tf32_rn(float f) {
-  uint32_t u = __float_as_uint(f);
-  u += 0xFFFu + ((u >> 13) & 1u);
-  u &= 0xFFFFE000u;
-  return __uint_as_float(u);
-}
-
 // Tensor-core variant: one thread per batch slot; writes the batch blob described at TcPlan (rift_internal.h).
-template <int MAXM>
+// MT = number of modes (compile time, so that the operand chunks are assembled in registers).
+template <int MT>
 __global__ void __launch_bounds__(GEOM_THREADS)
 geometry_tc_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, TcChunk ch, const double *__restrict__ p_ra,
                    const double *__restrict__ p_dec, const double *__restrict__ p_psi, const double *__restrict__ p_iota,
@@ -208,16 +203,18 @@ geometry_tc_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, Tc
   const int64_t seg = gb / ch.nbps;
   const int64_t i = (gb % ch.nbps) * RIFT_TC_NB + n;
   const bool valid = i < ch.n_per_seg;
-  const int K = g.n_det, M = g.n_modes;
+  const int K = g.n_det;
+  constexpr int KP = (6 * MT + 15) & ~15;                                   // contraction length, fp16 elements
+  constexpr int NCH = KP / 8;                                               // 16-byte chunks per detector
   float *blob = ch.blob + lb * tp.blob_words;
-  float4 *chunks = reinterpret_cast<float4 *>(blob);                        // [K][nch][16] float4
-  int32_t *dsh = reinterpret_cast<int32_t *>(blob + K * tp.nch * 64);       // [K][16]
-  float *cl2 = blob + K * tp.nch * 64 + K * 16;                             // [16]
-  const int nc1 = tp.ka >> 2;                                               // chunks of B1
+  uint4 *chunks = reinterpret_cast<uint4 *>(blob);                          // [K][NCH][16] x 8 halfs
+  int32_t *dsh = reinterpret_cast<int32_t *>(blob + K * NCH * 64);          // [K][16]
+  float *cl2 = blob + K * NCH * 64 + K * 16;                                // [16]
   if (!valid) {
-    const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+    const uint4 z = make_uint4(0u, 0u, 0u, 0u);
     for (int k = 0; k < K; ++k) {
-      for (int c = 0; c < tp.nch; ++c) chunks[(k * tp.nch + c) * 16 + n] = z;
+#pragma unroll
+      for (int c = 0; c < NCH; ++c) chunks[(k * NCH + c) * 16 + n] = z;
       dsh[k * 16 + n] = 0;
     }
     cl2[n] = 0.f;
@@ -228,53 +225,44 @@ geometry_tc_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, Tc
   const int64_t gi = seg * ch.n_per_seg + i;
   const int32_t point = ch.ids[seg];
   int32_t shift[RIFT_MAX_DET];
-  double Fre[RIFT_MAX_DET], Fim[RIFT_MAX_DET], Yre[MAXM], Yim[MAXM], c, q;
-  sample_geometry<MAXM>(g, modes, p_ra[gi], p_dec[gi], p_psi[gi], p_iota[gi], p_phi[gi], p_dist[gi], point, U, V, shift,
-                        Fre, Fim, Yre, Yim, c, q);
+  double Fre[RIFT_MAX_DET], Fim[RIFT_MAX_DET], Yre[MT], Yim[MT], c, q;
+  sample_geometry<MT>(g, modes, p_ra[gi], p_dec[gi], p_psi[gi], p_iota[gi], p_phi[gi], p_dist[gi], point, U, V, shift,
+                      Fre, Fim, Yre, Yim, c, q);
   ch.scale_c[w] = c;
   ch.quad[w] = q;
-  cl2[n] = (float)(c * 1.4426950408889634);
+  // exponent scale of the fused kernel: its accumulators carry x * (Q scale of the point) * RIFT_TC_BSCALE
+  cl2[n] = (float)(c * 1.4426950408889634 / ((double)ch.qscale[point] * RIFT_TC_BSCALE));
 #pragma unroll
   for (int k = 0; k < RIFT_MAX_DET; ++k) {
     if (k < K) {
       if (shift_out) shift_out[gi * K + k] = shift[k];
       dsh[k * 16 + n] = shift[k] - shift[0];
-      // a5: B = F_k Y_lm split into tf32 hi + lo; kappa = 2a (Re), 2a+1 (Im)
-      float hi[2 * MAXM], lo[2 * MAXM];
+      // a5: B = F_k Y_lm, scaled, split into fp16 hi + lo; kappa = 2a (Re), 2a+1 (Im).  The contraction index runs over
+      // [hi | hi | lo] facing the A operand's [Q_hi | Q_lo | Q_hi].
+      uint16_t hv[KP];
 #pragma unroll
-      for (int a = 0; a < MAXM; ++a) {
-        double vr = 0.0, vi = 0.0;
-        if (a < M) {
-          vr = Fre[k] * Yre[a] - Fim[k] * Yim[a];
-          vi = Fre[k] * Yim[a] + Fim[k] * Yre[a];
-        }
-        hi[2 * a] = tf32_rn((float)vr);
-        hi[2 * a + 1] = tf32_rn((float)vi);
-        lo[2 * a] = tf32_rn((float)(vr - (double)hi[2 * a]));
-        lo[2 * a + 1] = tf32_rn((float)(vi - (double)hi[2 * a + 1]));
+      for (int a = 0; a < MT; ++a) {
+        const double vr = (Fre[k] * Yre[a] - Fim[k] * Yim[a]) * RIFT_TC_BSCALE;
+        const double vi = (Fre[k] * Yim[a] + Fim[k] * Yre[a]) * RIFT_TC_BSCALE;
+        const __half hr = __double2half(vr), hi = __double2half(vi);
+        const __half lr = __double2half(vr - (double)__half2float(hr)), li = __double2half(vi - (double)__half2float(hi));
+        hv[2 * a] = hv[2 * MT + 2 * a] = __half_as_ushort(hr);
+        hv[2 * a + 1] = hv[2 * MT + 2 * a + 1] = __half_as_ushort(hi);
+        hv[4 * MT + 2 * a] = __half_as_ushort(lr);
+        hv[4 * MT + 2 * a + 1] = __half_as_ushort(li);
       }
-      float4 *dst = chunks + (k * tp.nch) * 16 + n;
-      const int nh = tp.kh >> 2;                                           // chunks of the hi block
 #pragma unroll
-      for (int cc = 0; cc < (2 * MAXM + 3) / 4; ++cc) {
-        if (cc < nh) {
-          float4 vh, vl;
-          vh.x = (4 * cc + 0 < 2 * MAXM) ? hi[4 * cc + 0] : 0.f;
-          vh.y = (4 * cc + 1 < 2 * MAXM) ? hi[4 * cc + 1] : 0.f;
-          vh.z = (4 * cc + 2 < 2 * MAXM) ? hi[4 * cc + 2] : 0.f;
-          vh.w = (4 * cc + 3 < 2 * MAXM) ? hi[4 * cc + 3] : 0.f;
-          vl.x = (4 * cc + 0 < 2 * MAXM) ? lo[4 * cc + 0] : 0.f;
-          vl.y = (4 * cc + 1 < 2 * MAXM) ? lo[4 * cc + 1] : 0.f;
-          vl.z = (4 * cc + 2 < 2 * MAXM) ? lo[4 * cc + 2] : 0.f;
-          vl.w = (4 * cc + 3 < 2 * MAXM) ? lo[4 * cc + 3] : 0.f;
-          dst[cc * 16] = vh;                 // B1, hi block
-          dst[(nh + cc) * 16] = vh;          // B1, lo block of A multiplies hi of B
-          dst[(nc1 + cc) * 16] = vl;         // B2, hi block of A multiplies lo of B
-        }
+      for (int e = 6 * MT; e < KP; ++e) hv[e] = 0;
+      uint4 *dst = chunks + (k * NCH) * 16 + n;
+#pragma unroll
+      for (int cc = 0; cc < NCH; ++cc) {
+        uint4 v;
+        v.x = (uint32_t)hv[8 * cc + 0] | ((uint32_t)hv[8 * cc + 1] << 16);
+        v.y = (uint32_t)hv[8 * cc + 2] | ((uint32_t)hv[8 * cc + 3] << 16);
+        v.z = (uint32_t)hv[8 * cc + 4] | ((uint32_t)hv[8 * cc + 5] << 16);
+        v.w = (uint32_t)hv[8 * cc + 6] | ((uint32_t)hv[8 * cc + 7] << 16);
+        dst[cc * 16] = v;
       }
-      const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-      for (int cc = 2 * nh; cc < nc1; ++cc) dst[cc * 16] = z;             // padding of B1
-      for (int cc = nc1 + nh; cc < tp.nch; ++cc) dst[cc * 16] = z;        // B2 columns facing A's lo block / padding
     }
   }
 }
@@ -287,12 +275,17 @@ cudaError_t launch_geometry_tc(const DetGeom &g, const ModeEntry *modes, const T
   const int64_t n = c.n_batches * RIFT_TC_NB;
   if (n <= 0) return cudaSuccess;
   const unsigned grid = (unsigned)((n + GEOM_THREADS - 1) / GEOM_THREADS);
-  if (tp.M <= 8)
-    geometry_tc_kernel<8><<<grid, GEOM_THREADS, 0, s>>>(g, modes, tp, c, params[0], params[1], params[2], params[3],
-                                                         params[4], params[5], U, V, shift_out);
-  else
-    geometry_tc_kernel<16><<<grid, GEOM_THREADS, 0, s>>>(g, modes, tp, c, params[0], params[1], params[2], params[3],
-                                                          params[4], params[5], U, V, shift_out);
+#define RIFT_GEOM_TC(MT)                                                                                             \
+  case MT:                                                                                                           \
+    geometry_tc_kernel<MT><<<grid, GEOM_THREADS, 0, s>>>(g, modes, tp, c, params[0], params[1], params[2], params[3], \
+                                                          params[4], params[5], U, V, shift_out);                    \
+    break;
+  switch (tp.M) {
+    RIFT_GEOM_TC(1) RIFT_GEOM_TC(2) RIFT_GEOM_TC(3) RIFT_GEOM_TC(4) RIFT_GEOM_TC(5) RIFT_GEOM_TC(6) RIFT_GEOM_TC(7)
+    RIFT_GEOM_TC(8)
+    default: return cudaErrorInvalidValue;
+  }
+#undef RIFT_GEOM_TC
   return cudaGetLastError();
 }
 

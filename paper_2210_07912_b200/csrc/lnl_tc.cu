@@ -4,9 +4,10 @@
 //
 // The contraction over the modes is a GEMM per detector in UNSHIFTED detector time,
 //     P_k[t, n] = sum_kappa Q'_k[t, kappa] B'_k[kappa, n],     t = 0..N_t-1 (rows, M of the UMMA), n = 16 samples (N),
-// with fp32-level accuracy from two TF32 pieces per operand (hi + lo; the lo*lo product is dropped): the A operand
-// Q' = [Q_hi | Q_lo] (ka columns) lives in TENSOR MEMORY for the whole intrinsic point, the B operands
-// B1 = [B_hi | B_hi], B2 = [B_lo | 0] come from shared memory (bulk-copied batch blobs written by the geometry kernel),
+// with fp32-level accuracy from two fp16 pieces per operand (hi + lo, 11 significant bits each, operands pre-scaled by
+// powers of two into the fp16 range; the lo*lo product is dropped; accumulation in fp32): the A operand
+// Q' = [Q_hi | Q_lo | Q_hi] (kp elements) lives in TENSOR MEMORY for the whole intrinsic point, the B operand
+// B' = [B_hi | B_hi | B_lo] comes from shared memory (bulk-copied batch blobs written by the geometry kernel),
 // accumulators P_k (K detectors x nt row tiles x 16 columns) are in TMEM.  In circular mode (N_tau = N_t) the time
 // marginal is invariant under a common rotation, so with t = (j + s_0) mod N_t
 //     x[t] = P_0[t] + sum_{k>=1} P_k[(t + d_k) mod N_t],     d_k = s_k - s_0  (|d_k| <= dmax_k, light travel time),
@@ -17,6 +18,8 @@
 //
 // Warp roles (320 threads, one CTA per SM): warps 0-3 / 4-7 = two epilogue warpgroups (samples 0-7 / 8-15 of each batch;
 // warp w reads TMEM lanes 32 (w%4)..), warp 8 = bulk-copy producer, warp 9 = UMMA issuer (and TMEM allocator).
+#include <cuda_fp16.h>
+
 #include "rift_internal.h"
 #include "tma_utils.cuh"
 
@@ -36,18 +39,18 @@ __device__ __forceinline__ void tc_commit(uint64_t *bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar))
                : "memory");
 }
-// D[tmem] (+)= A[tmem] * B[smem descriptor], kind::tf32, issued by one thread
+// D[tmem] (+)= A[tmem] * B[smem descriptor], kind::f16 (fp16 operands, fp32 accumulate), issued by one thread
 __device__ __forceinline__ void tc_mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc,
                                           uint32_t accumulate) {
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
       "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
       ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
       : "memory");
 }
 // K-major, no swizzle: core matrix = 8 rows x 16 bytes, contiguous (128 B).  LBO = byte distance between the two
-// 16-byte K chunks of one K=8 step, SBO = byte distance between 8-row groups; version 1 (Blackwell).
+// 16-byte K chunks of one K=16 (fp16) step, SBO = byte distance between 8-row groups; version 1 (Blackwell).
 __device__ __forceinline__ uint64_t tc_smem_desc(uint32_t addr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
   return (uint64_t)((addr >> 4) & 0x3FFFu) | ((uint64_t)((lbo_bytes >> 4) & 0x3FFFu) << 16) |
          ((uint64_t)((sbo_bytes >> 4) & 0x3FFFu) << 32) | (1ull << 46);
@@ -71,6 +74,15 @@ __device__ __forceinline__ void tc_st8(uint32_t taddr, const float4 &a, const fl
                "r"(__float_as_uint(b.x)), "r"(__float_as_uint(b.y)), "r"(__float_as_uint(b.z)), "r"(__float_as_uint(b.w))
                : "memory");
 }
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile(
+      "{\n\t.reg .pred P;\n\t"
+      "elect.sync _|P, 0xffffffff;\n\t"
+      "selp.u32 %0, 1, 0, P;\n\t}"
+      : "=r"(pred));
+  return pred != 0;
+}
 __device__ __forceinline__ void named_bar_sync(int id, int n_threads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n_threads) : "memory");
 }
@@ -78,12 +90,52 @@ __device__ __forceinline__ void named_bar_sync(int id, int n_threads) {
 struct TcArgs {
   TcPlan tp;
   TcChunk ch;
-  const float *qtc;              // [P][K][nt*128][ka] tf32 words
+  const uint32_t *qtc;           // [P][K][nt*128][acols] words of two fp16
 };
 
-// instruction descriptor: D fp32, A/B tf32, both K-major, N = 16, M = 128
-constexpr uint32_t TC_IDESC = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(RIFT_TC_NB >> 3) << 17) | ((128u >> 4) << 24);
+// instruction descriptor: D fp32, A/B fp16 (format 0), both K-major, N = 16, M = 128
+constexpr uint32_t TC_IDESC = (1u << 4) | ((uint32_t)(RIFT_TC_NB >> 3) << 17) | ((128u >> 4) << 24);
 
+// mbarrier wait for the roles that idle most of the time (producer, UMMA issuer): long suspend hint
+__device__ __forceinline__ void mbar_wait_idle(uint64_t *bar, uint32_t phase) {
+  uint32_t ok = 0;
+  while (!ok) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(phase), "r"(20000u)
+        : "memory");
+  }
+}
+
+// Reduce 8 per-thread values across the 32 lanes with 9 shuffles: after the call, every lane holds the reduction of
+// value n = 4 b4 + 2 b3 + b2 (b = bits of the lane index).
+template <typename Op>
+__device__ __forceinline__ float treduce8(const float (&v)[8], int lane, Op op) {
+  const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4;
+  float w4[4], w2[2];
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const float send = b4 ? v[j] : v[j + 4], keep = b4 ? v[j + 4] : v[j];
+    w4[j] = op(keep, __shfl_xor_sync(0xffffffffu, send, 16));
+  }
+#pragma unroll
+  for (int j = 0; j < 2; ++j) {
+    const float send = b3 ? w4[j] : w4[j + 2], keep = b3 ? w4[j + 2] : w4[j];
+    w2[j] = op(keep, __shfl_xor_sync(0xffffffffu, send, 8));
+  }
+  const float send = b2 ? w2[0] : w2[1], keep = b2 ? w2[1] : w2[0];
+  float w = op(keep, __shfl_xor_sync(0xffffffffu, send, 4));
+  w = op(w, __shfl_xor_sync(0xffffffffu, w, 2));
+  w = op(w, __shfl_xor_sync(0xffffffffu, w, 1));
+  return w;
+}
+
+// NT = row tiles of 128 (ceil(n_t / 128)); PITCH = floats per exchange row (>= n_t + 2 H), compile-time so that the
+// exchange addresses are one register plus immediates.
+template <int NT, int PITCH>
 __global__ void __launch_bounds__(TC_THREADS, 1) lnl_tc_kernel(const TcArgs args) {
   const TcPlan &tp = args.tp;
   const TcChunk &ch = args.ch;
@@ -96,7 +148,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) lnl_tc_kernel(const TcArgs args
   float *blob_s = reinterpret_cast<float *>(smem_raw + 128);
   float *xb_s = blob_s + TC_STAGES * tp.blob_words;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int K = tp.K, nt = tp.nt, ka = tp.ka;
+  const int K = tp.K, acols = tp.acols;
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < TC_STAGES; ++i) {
@@ -129,13 +181,13 @@ __global__ void __launch_bounds__(TC_THREADS, 1) lnl_tc_kernel(const TcArgs args
     // ---- the A operand of this intrinsic point -> tensor memory (thread = TMEM lane = row of the tile)
     __syncthreads();                       // every role is done with the previous job (all UMMAs have completed)
     if (point != staged_point && warp < 4) {
-      const int rows = nt * 128;
       for (int k = 0; k < K; ++k)
-        for (int i = 0; i < nt; ++i) {
+        for (int i = 0; i < NT; ++i) {
           const int row = 128 * i + 32 * warp + lane;
-          const float4 *src = reinterpret_cast<const float4 *>(args.qtc + (((int64_t)point * K + k) * rows + row) * ka);
-          const uint32_t taddr = tmem_base + ((uint32_t)(32 * warp) << 16) + (uint32_t)((k * nt + i) * ka);
-          for (int c8 = 0; c8 < ka; c8 += 8) {
+          const float4 *src =
+              reinterpret_cast<const float4 *>(args.qtc + (((int64_t)point * K + k) * (NT * 128) + row) * acols);
+          const uint32_t taddr = tmem_base + ((uint32_t)(32 * warp) << 16) + (uint32_t)((k * NT + i) * acols);
+          for (int c8 = 0; c8 < acols; c8 += 8) {
             const float4 a = __ldg(src + (c8 >> 2)), b = __ldg(src + (c8 >> 2) + 1);
             tc_st8(taddr + c8, a, b);
           }
@@ -152,7 +204,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) lnl_tc_kernel(const TcArgs args
       if (lane == 0) {
         for (uint32_t j = 0; j < nb; ++j) {
           const uint32_t g = it + j, stage = g % TC_STAGES, ph = (g / TC_STAGES) & 1u;
-          mbar_wait(bar_empty + stage, ph ^ 1u);
+          mbar_wait_idle(bar_empty + stage, ph ^ 1u);
           const uint32_t bytes = (uint32_t)tp.blob_words * 4u;
           mbar_expect_tx(bar_full + stage, bytes);
           bulk_g2s(blob_s + stage * tp.blob_words, ch.blob + (b0 + j) * tp.blob_words, bytes, bar_full + stage);
@@ -160,24 +212,24 @@ __global__ void __launch_bounds__(TC_THREADS, 1) lnl_tc_kernel(const TcArgs args
       }
       __syncwarp();
     } else if (warp == 9) {
-      // ===== UMMA issuer =====
-      const int n1 = ka >> 3, n2 = tp.kb2 >> 3;                            // K=8 steps of B1, B2
+      // ===== UMMA issuer =====  (K=16 steps outermost: consecutive UMMAs accumulate into different tiles)
+      const int n_steps = tp.kp >> 4;
       for (uint32_t j = 0; j < nb; ++j) {
         const uint32_t g = it + j, stage = g % TC_STAGES, ph = (g / TC_STAGES) & 1u;
-        mbar_wait(bar_full + stage, ph);
-        mbar_wait(bar_tempty, (g & 1u) ^ 1u);
+        mbar_wait_idle(bar_full + stage, ph);
+        mbar_wait_idle(bar_tempty, (g & 1u) ^ 1u);
         tc_fence_after();
-        if (lane == 0) {
-          for (int k = 0; k < K; ++k) {
-            const uint32_t b1 = smem_u32(blob_s + stage * tp.blob_words + k * tp.nch * 64);
-            const uint32_t b2 = b1 + (uint32_t)(ka >> 2) * 256u;
-            for (int i = 0; i < nt; ++i) {
-              const uint32_t d_t = tmem_base + (uint32_t)(tp.dcol0 + (k * nt + i) * RIFT_TC_NB);
-              const uint32_t a_t = tmem_base + (uint32_t)((k * nt + i) * ka);
-              for (int s = 0; s < n1; ++s)
-                tc_mma_ts(d_t, a_t + 8 * s, tc_smem_desc(b1 + 512u * s, 256u, 128u), TC_IDESC, s > 0 ? 1u : 0u);
-              for (int s = 0; s < n2; ++s)
-                tc_mma_ts(d_t, a_t + 8 * s, tc_smem_desc(b2 + 512u * s, 256u, 128u), TC_IDESC, 1u);
+        if (elect_one()) {
+          const uint64_t desc0 = tc_smem_desc(smem_u32(blob_s + stage * tp.blob_words), 256u, 128u);
+          for (int s = 0; s < n_steps; ++s) {
+            for (int k = 0; k < K; ++k) {
+              const uint64_t desc = desc0 + (uint64_t)((k * tp.nch * 256 + s * 512) >> 4);
+#pragma unroll
+              for (int i = 0; i < NT; ++i) {
+                const uint32_t d_t = tmem_base + (uint32_t)(tp.dcol0 + (k * NT + i) * RIFT_TC_NB);
+                const uint32_t a_t = tmem_base + (uint32_t)((k * NT + i) * acols + 8 * s);
+                tc_mma_ts(d_t, a_t, desc, TC_IDESC, s > 0 ? 1u : 0u);
+              }
             }
           }
           tc_commit(bar_tfull);
@@ -189,88 +241,119 @@ __global__ void __launch_bounds__(TC_THREADS, 1) lnl_tc_kernel(const TcArgs args
       const int wg = warp >> 2, q = warp & 3;
       const int T = 32 * q + lane;
       const uint32_t lane_addr = tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)(tp.dcol0 + NH * wg);
-      const int n_t = tp.n_t, H = tp.H, pitch = tp.pitch;
+      const int n_t = tp.n_t, H = tp.H;
+      const float inv_scale = 1.0f / (ch.qscale[point] * (float)RIFT_TC_BSCALE);   // accumulators carry x / inv_scale
+      const bool last_valid = 128 * (NT - 1) + T < n_t;                    // tiles 0..NT-2 are full, the last one ragged
+      const int last_clamp = last_valid ? 0 : (n_t - 1) - (128 * (NT - 1) + T);   // row offset that keeps reads in range
+
+      auto load_tiles = [&](int k, float (&r)[NT][NH]) {
+#pragma unroll
+        for (int i = 0; i < NT; ++i) tc_ld8(lane_addr + (uint32_t)((k * NT + i) * RIFT_TC_NB), r[i]);
+      };
+      auto wait_tiles = [&](float (&r)[NT][NH]) {
+#pragma unroll
+        for (int i = 0; i < NT; ++i) tc_wait_ld8(r[i]);
+      };
+      auto store_tiles = [&](int k, float *xb, const float (&r)[NT][NH]) {
+        const int dm = tp.dmax[k];
+        float *base = xb + (size_t)(k - 1) * NH * PITCH + T + H;
+#pragma unroll
+        for (int i = 0; i < NT; ++i) {
+          const int t = 128 * i + T;
+          if (i < NT - 1 || last_valid) {
+            float *dst = base + 128 * i;
+#pragma unroll
+            for (int n = 0; n < NH; ++n) dst[n * PITCH] = r[i][n];
+            if (t < dm) {
+              float *dh = dst + n_t;
+#pragma unroll
+              for (int n = 0; n < NH; ++n) dh[n * PITCH] = r[i][n];
+            }
+            if (t >= n_t - dm) {
+              float *dl = dst - n_t;
+#pragma unroll
+              for (int n = 0; n < NH; ++n) dl[n * PITCH] = r[i][n];
+            }
+          }
+        }
+      };
+
       for (uint32_t j = 0; j < nb; ++j) {
         const uint32_t g = it + j, stage = g % TC_STAGES, ph = (g / TC_STAGES) & 1u;
         const float *blob = blob_s + stage * tp.blob_words;
-        float *xb = xb_s + (size_t)((wg * 2 + (g & 1u)) * (K - 1)) * NH * pitch;
+        float *xb = xb_s + (size_t)((wg * 2 + (g & 1u)) * (K - 1)) * NH * PITCH;
         mbar_wait(bar_full + stage, ph);
         mbar_wait(bar_tfull, g & 1u);
         tc_fence_after();
 
-        // Phase A: P_k (k >= 1) -> exchange buffer, P_0 -> registers
-        for (int k = 1; k < K; ++k) {
-          const int dm = tp.dmax[k];
-#pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            if (i < nt) {
-              float r[8];
-              tc_ld8(lane_addr + (uint32_t)((k * nt + i) * RIFT_TC_NB), r);
-              tc_wait_ld8(r);
-              const int t = 128 * i + T;
-              if (t < n_t) {
-                float *dst = xb + (size_t)(k - 1) * NH * pitch + t + H;
-#pragma unroll
-                for (int n = 0; n < NH; ++n) dst[n * pitch] = r[n];
-                if (t < dm) {
-#pragma unroll
-                  for (int n = 0; n < NH; ++n) dst[n * pitch + n_t] = r[n];
-                }
-                if (t >= n_t - dm) {
-#pragma unroll
-                  for (int n = 0; n < NH; ++n) dst[n * pitch - n_t] = r[n];
-                }
-              }
-            }
+        // Phase A: P_k (k >= 1) -> exchange buffer, P_0 -> registers; the loads of the next detector are in flight
+        // while the current one is stored
+        float x[NT][NH], ra[NT][NH], rb[NT][NH];
+        if (K > 1) load_tiles(1, ra); else load_tiles(0, x);
+        for (int k = 1; k < K; k += 2) {
+          wait_tiles(ra);
+          if (k + 1 < K) load_tiles(k + 1, rb); else load_tiles(0, x);
+          store_tiles(k, xb, ra);
+          if (k + 1 < K) {
+            wait_tiles(rb);
+            if (k + 2 < K) load_tiles(k + 2, ra); else load_tiles(0, x);
+            store_tiles(k + 1, xb, rb);
           }
         }
-        float x[4][NH];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-          if (i < nt) {
-            tc_ld8(lane_addr + (uint32_t)(i * RIFT_TC_NB), x[i]);
-          } else {
-#pragma unroll
-            for (int n = 0; n < NH; ++n) x[i][n] = 0.f;
-          }
-        }
-#pragma unroll
-        for (int i = 0; i < 4; ++i) tc_wait_ld8(x[i]);
+        wait_tiles(x);
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_tempty);                            // the UMMAs of the next batch may overwrite D
         named_bar_sync(1 + wg, 128);                                       // exchange rows of this warpgroup are complete
 
-        // Phase B: shifted sum over detectors, then per-warp (reference, sum) of the time marginal
-        const int32_t *dsh = reinterpret_cast<const int32_t *>(blob + K * tp.nch * 64);
-        const float *cl2s = blob + K * tp.nch * 64 + K * 16;
-        float2 *part = ch.part + ((b0 + j) * RIFT_TC_NB + NH * wg) * 4 + q;
+        // Phase B: shifted sum over detectors
+        const int32_t *dsh = reinterpret_cast<const int32_t *>(blob + K * tp.nch * 64) + NH * wg;
+        const float *cl2s = blob + K * tp.nch * 64 + K * 16 + NH * wg;
+        for (int k = 1; k < K; ++k) {
+          const int4 d0 = *reinterpret_cast<const int4 *>(dsh + k * 16), d1 = *reinterpret_cast<const int4 *>(dsh + k * 16 + 4);
+          const int d[NH] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
+          const float *base = xb + (size_t)(k - 1) * NH * PITCH + T + H;
+#pragma unroll
+          for (int n = 0; n < NH; ++n) {
+            const float *src = base + d[n] + n * PITCH;
+#pragma unroll
+            for (int i = 0; i < NT - 1; ++i) x[i][n] += src[128 * i];
+            x[NT - 1][n] += src[128 * (NT - 1) + last_clamp];
+          }
+        }
+        // per-warp (reference, sum) of the time marginal for the 8 samples
+        float m[NH];
 #pragma unroll
         for (int n = 0; n < NH; ++n) {
-          for (int k = 1; k < K; ++k) {
-            const int d = dsh[k * 16 + NH * wg + n];
-            const float *src = xb + (size_t)((k - 1) * NH + n) * pitch + T + H + d;
+          if (!last_valid) x[NT - 1][n] = -INFINITY;
+          float mm = x[0][n];
 #pragma unroll
-            for (int i = 0; i < 4; ++i)
-              if (128 * i + T < n_t) x[i][n] += src[128 * i];
-          }
-          float m = -INFINITY;
+          for (int i = 1; i < NT; ++i) mm = fmaxf(mm, x[i][n]);
+          m[n] = mm;
+        }
+        const float mine = treduce8(m, lane, [](float a, float b) { return fmaxf(a, b); });
+        const float4 c0 = *reinterpret_cast<const float4 *>(cl2s), c1 = *reinterpret_cast<const float4 *>(cl2s + 4);
+        const float cl2[NH] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
+        float sums[NH];
 #pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            if (128 * i + T >= n_t) x[i][n] = -INFINITY;
-            m = fmaxf(m, x[i][n]);
-          }
-          m = warp_max(m);
-          const float cl2 = cl2s[NH * wg + n];
-          // reference in log2 units, rounded once: sum_j 2^(x_j cl2 - off) = 2^res sum_j 2^((x_j - m) cl2), res = m cl2 - off
-          const float off = (m == -INFINITY) ? 0.f : m * cl2;
-          const float res = (m == -INFINITY) ? 0.f : fmaf(m, cl2, -off);
+        for (int n = 0; n < NH; ++n) {
+          const float mx = __shfl_sync(0xffffffffu, mine, ((n & 4) << 2) | ((n & 2) << 2) | ((n & 1) << 2));
+          // reference in log2 units, rounded once (the residual is corrected below)
+          const float off = (mx == -INFINITY) ? 0.f : mx * cl2[n];
           float s = 0.f;
 #pragma unroll
-          for (int i = 0; i < 4; ++i) s += fast_exp2(fmaf(x[i][n], cl2, -off));
-#pragma unroll
-          for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-          if (lane == 0) part[n * 4] = make_float2(m, s * fast_exp2(-res));
+          for (int i = 0; i < NT; ++i) s += fast_exp2(fmaf(x[i][n], cl2[n], -off));
+          sums[n] = s;
+        }
+        const float ssum = treduce8(sums, lane, [](float a, float b) { return a + b; });
+        if ((lane & 3) == 0) {
+          const int nsel = lane >> 2;                                      // = 4 b4 + 2 b3 + b2
+          const float cl = cl2s[nsel];
+          // sum_j 2^(x_j cl - off) = 2^res sum_j 2^((x_j - m) cl),  res = m cl - off
+          const float off = (mine == -INFINITY) ? 0.f : mine * cl;
+          const float res = (mine == -INFINITY) ? 0.f : fmaf(mine, cl, -off);
+          ch.part[((b0 + j) * RIFT_TC_NB + NH * wg + nsel) * 4 + q] =
+              make_float2(mine * inv_scale, ssum * fast_exp2(-res));
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_empty + stage);
@@ -308,34 +391,50 @@ __global__ void lnl_tc_finalize_kernel(TcPlan tp, TcChunk ch, double *__restrict
   lnL_out[seg * ch.n_per_seg + i] = c * mm + log(sum) - log((double)tp.n_t) - ch.quad[w];
 }
 
-// Q [P][K][M][n_t] complex128  ->  A operand [P][K][nt*128][ka] tf32 words: columns [0, kh) = hi(Re, Im interleaved),
-// [kh, 2 kh) = lo, zero padding; rows >= n_t are zero.
-__global__ void convert_q_tc_kernel(const double2 *__restrict__ src, float *__restrict__ dst, TcPlan tp, int64_t total) {
+// Per point: max |Re Q|, |Im Q| over detectors, modes, time (bit pattern of the non-negative float, atomicMax)
+__global__ void q_absmax_kernel(const double2 *__restrict__ src, uint32_t *__restrict__ mx, int64_t per_point, int64_t total) {
   for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
-    const int col = (int)(idx % tp.ka);
-    const int64_t r = idx / tp.ka;
+    const double2 v = src[idx];
+    const float a = fmaxf(fabsf((float)v.x), fabsf((float)v.y));
+    if (a > 0.f && a < INFINITY) atomicMax(mx + idx / per_point, __float_as_uint(a));
+  }
+}
+// scale[p] = 2^e with scale * max|Q| in [2^13, 2^14)  (1 when the point is all zero)
+__global__ void q_scale_kernel(const uint32_t *__restrict__ mx, float *__restrict__ scale, int n_points) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= n_points) return;
+  const float a = __uint_as_float(mx[p]);
+  int e = 0;
+  if (a > 0.f) frexpf(a, &e);                                              // a = f 2^e, f in [0.5, 1)
+  scale[p] = (a > 0.f) ? ldexpf(1.0f, 14 - e) : 1.0f;
+}
+
+// Q [P][K][M][n_t] complex128  ->  A operand [P][K][nt*128][acols] words of two fp16: contraction index kappa' over
+// [Q_hi | Q_lo | Q_hi] (each 2M elements, Re/Im interleaved), zero padding up to kp; rows >= n_t are zero.
+__global__ void convert_q_tc_kernel(const double2 *__restrict__ src, uint32_t *__restrict__ dst, const float *__restrict__ scale,
+                                    TcPlan tp, int64_t total) {
+  for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
+    const int col = (int)(idx % tp.acols);
+    const int64_t r = idx / tp.acols;
     const int rows = tp.nt * 128;
     const int t = (int)(r % rows);
     const int64_t pk = r / rows;                                           // point * K + k
-    const int part = col / tp.kh, kap = col % tp.kh;
-    float v = 0.f;
-    if (t < tp.n_t && part < 2 && kap < 2 * tp.M) {
-      const double2 qv = src[(pk * tp.M + (kap >> 1)) * tp.n_t + t];
-      const double x = (kap & 1) ? qv.y : qv.x;
-      uint32_t u = __float_as_uint((float)x);
-      u += 0xFFFu + ((u >> 13) & 1u);
-      u &= 0xFFFFE000u;
-      const float hi = __uint_as_float(u);
-      if (part == 0) {
-        v = hi;
-      } else {
-        uint32_t ul = __float_as_uint((float)(x - (double)hi));
-        ul += 0xFFFu + ((ul >> 13) & 1u);
-        ul &= 0xFFFFE000u;
-        v = __uint_as_float(ul);
+    const double sc = (double)scale[pk / tp.K];
+    uint32_t word = 0;
+    if (t < tp.n_t) {
+      for (int hlf = 0; hlf < 2; ++hlf) {
+        const int kp_i = 2 * col + hlf;
+        const int part = kp_i / (2 * tp.M), kap = kp_i % (2 * tp.M);
+        if (part < 3) {
+          const double2 qv = src[(pk * tp.M + (kap >> 1)) * tp.n_t + t];
+          const double x = ((kap & 1) ? qv.y : qv.x) * sc;
+          const __half hi = __double2half(x);
+          const __half out = (part == 1) ? __double2half(x - (double)__half2float(hi)) : hi;
+          word |= (uint32_t)__half_as_ushort(out) << (16 * hlf);
+        }
       }
     }
-    dst[idx] = v;
+    dst[idx] = word;
   }
 }
 
@@ -345,29 +444,73 @@ size_t lnl_tc_smem_bytes(const TcPlan &tp) {
   return 128 + (size_t)TC_STAGES * tp.blob_words * 4 + (size_t)4 * (tp.K - 1) * NH * tp.pitch * 4;
 }
 
-cudaError_t launch_convert_q_tc(const double *Q_c128, float *dst, const TcPlan &tp, int32_t n_points, cudaStream_t s) {
-  const int64_t total = (int64_t)n_points * tp.K * tp.nt * 128 * tp.ka;
+// exchange-row pitches the kernel is instantiated for; 0 if n_t + 2 H does not fit any
+int lnl_tc_pitch(int n_t, int halo) {
+  const int need = n_t + 2 * halo;
+  const int opts[4] = {256, 512, 640, 768};
+  for (int i = 0; i < 4; ++i)
+    if (need <= opts[i]) return opts[i];
+  return 0;
+}
+
+namespace {
+template <int NT>
+cudaError_t launch_nt(const TcArgs &a, unsigned grid, size_t smem, cudaStream_t s) {
+#define RIFT_TC_CASE(P)                                                                                         \
+  case P: {                                                                                                     \
+    cudaError_t e = cudaFuncSetAttribute(lnl_tc_kernel<NT, P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+    if (e != cudaSuccess) return e;                                                                             \
+    lnl_tc_kernel<NT, P><<<grid, TC_THREADS, smem, s>>>(a);                                                     \
+    return cudaGetLastError();                                                                                  \
+  }
+  switch (a.tp.pitch) {
+    RIFT_TC_CASE(256)
+    RIFT_TC_CASE(512)
+    RIFT_TC_CASE(640)
+    RIFT_TC_CASE(768)
+    default: return cudaErrorInvalidValue;
+  }
+#undef RIFT_TC_CASE
+}
+}  // namespace
+
+cudaError_t launch_convert_q_tc(const double *Q_c128, uint32_t *dst, float *qscale, const TcPlan &tp, int32_t n_points,
+                                cudaStream_t s) {
+  const int64_t total = (int64_t)n_points * tp.K * tp.nt * 128 * tp.acols;
   if (total <= 0) return cudaSuccess;
-  int64_t grid = (total + 255) / 256;
+  const int64_t per_point = (int64_t)tp.K * tp.M * tp.n_t, n_src = per_point * n_points;
+  // qscale doubles as the scratch of the max reduction (bit patterns), then holds the scale
+  cudaError_t e = cudaMemsetAsync(qscale, 0, sizeof(float) * n_points, s);
+  if (e != cudaSuccess) return e;
+  int64_t grid = (n_src + 255) / 256;
   if (grid > 148 * 32) grid = 148 * 32;
-  convert_q_tc_kernel<<<(unsigned)grid, 256, 0, s>>>(reinterpret_cast<const double2 *>(Q_c128), dst, tp, total);
+  q_absmax_kernel<<<(unsigned)grid, 256, 0, s>>>(reinterpret_cast<const double2 *>(Q_c128),
+                                                 reinterpret_cast<uint32_t *>(qscale), per_point, n_src);
+  q_scale_kernel<<<(n_points + 127) / 128, 128, 0, s>>>(reinterpret_cast<const uint32_t *>(qscale), qscale, n_points);
+  grid = (total + 255) / 256;
+  if (grid > 148 * 32) grid = 148 * 32;
+  convert_q_tc_kernel<<<(unsigned)grid, 256, 0, s>>>(reinterpret_cast<const double2 *>(Q_c128), dst, qscale, tp, total);
   return cudaGetLastError();
 }
 
-cudaError_t launch_lnl_tc(const TcPlan &tp, const float *qtc, const TcChunk &c, double *lnL_out, int n_sm,
+cudaError_t launch_lnl_tc(const TcPlan &tp, const uint32_t *qtc, const TcChunk &c, double *lnL_out, int n_sm,
                           cudaStream_t s, int *n_launch) {
   if (c.n_batches <= 0) return cudaSuccess;
   const size_t smem = lnl_tc_smem_bytes(tp);
-  cudaError_t e = cudaFuncSetAttribute(lnl_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return e;
+  cudaError_t e;
   TcArgs a;
   a.tp = tp;
   a.ch = c;
   a.qtc = qtc;
   int64_t grid = n_sm;
   if (grid > c.n_batches) grid = c.n_batches;
-  lnl_tc_kernel<<<(unsigned)grid, TC_THREADS, smem, s>>>(a);
-  e = cudaGetLastError();
+  switch (tp.nt) {
+    case 1: e = launch_nt<1>(a, (unsigned)grid, smem, s); break;
+    case 2: e = launch_nt<2>(a, (unsigned)grid, smem, s); break;
+    case 3: e = launch_nt<3>(a, (unsigned)grid, smem, s); break;
+    case 4: e = launch_nt<4>(a, (unsigned)grid, smem, s); break;
+    default: e = cudaErrorInvalidValue;
+  }
   if (e != cudaSuccess) return e;
   const int64_t n = c.n_batches * RIFT_TC_NB;
   lnl_tc_finalize_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(tp, c, lnL_out);

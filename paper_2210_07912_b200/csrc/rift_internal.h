@@ -59,14 +59,15 @@ struct QStore {
 
 // Tensor-core path (lnl_tc.cu): plan of one handle.  Samples are processed in batches of RIFT_TC_NB consecutive samples
 // of one segment; the geometry kernel writes one "blob" per batch: the B operand of the UMMA in its canonical K-major
-// shared-memory layout, [K][nch][16][4] tf32 words (per detector: B1 = [hi | hi] over ka columns, then B2 = [lo | 0] over
-// kb2 columns, in 16-byte chunks of 4 columns), then the relative shifts d_k = s_k - s_0 as int32 [K][16], then
-// c*log2(e) as float [16].
+// shared-memory layout, [K][nch][16 samples][8 fp16] (per detector the contraction index runs over [B_hi | B_hi | B_lo],
+// kp = 6M rounded up to 16 elements, in 16-byte chunks of 8), then the relative shifts d_k = s_k - s_0 as int32 [K][16],
+// then c*log2(e) / (operand scales) as float [16].
 #define RIFT_TC_NB 16
+#define RIFT_TC_BSCALE 8192.0    // 2^13: scale of the coefficient operand (|F_k Y_lm| < 2) into the fp16 range
 struct TcPlan {
   int32_t ok;                    // 1 if this handle can run the tensor-core kernel
   int32_t K, M, n_t, nt;         // nt = ceil(n_t / 128) row tiles
-  int32_t kh, ka, kb2, nch;      // hi block width (2M rounded up to 4), A columns (2*kh up to 8), B2 extent (kh up to 8), chunks
+  int32_t kp, nch, acols;        // contraction length (fp16 elements), 16-byte chunks per detector, TMEM columns of one A tile
   int32_t H, pitch;              // halo = max_k dmax[k]; exchange-row pitch in floats
   int32_t blob_words, dcol0;     // 32-bit words per batch blob; first accumulator column in TMEM
   int32_t dmax[RIFT_MAX_DET];    // bound on |s_k - s_0|
@@ -74,6 +75,7 @@ struct TcPlan {
 struct TcChunk {                 // a chunk = global batches [gb0, gb0 + n_batches), batch gb = seg * nbps + b
   int64_t n_per_seg, nbps, gb0, n_batches;
   const int32_t *ids;
+  const float *qscale;           // [P] power-of-two scale applied to Q of each point in the A operand
   float *blob;                   // [n_batches][blob_words]
   double *scale_c, *quad;        // [n_batches * 16]
   float2 *part;                  // [n_batches * 16][4]: per lane-quarter (reference, sum)
@@ -112,8 +114,10 @@ cudaError_t launch_lnl_quad(const QStore &q, bool fp32, const Batch &b, const Wo
                             int n_sm, cudaStream_t s, int *n_launch);
 // lnl_tc.cu (tcgen05 / TMEM contraction, shift applied through a shared-memory exchange)
 size_t lnl_tc_smem_bytes(const TcPlan &tp);
-cudaError_t launch_convert_q_tc(const double *Q_c128, float *dst, const TcPlan &tp, int32_t n_points, cudaStream_t s);
-cudaError_t launch_lnl_tc(const TcPlan &tp, const float *qtc, const TcChunk &c, double *lnL_out, int n_sm,
+int lnl_tc_pitch(int n_t, int halo);   // exchange-row pitch (floats) the kernel is instantiated for, 0 = none fits
+cudaError_t launch_convert_q_tc(const double *Q_c128, uint32_t *dst, float *qscale, const TcPlan &tp, int32_t n_points,
+                                cudaStream_t s);
+cudaError_t launch_lnl_tc(const TcPlan &tp, const uint32_t *qtc, const TcChunk &c, double *lnL_out, int n_sm,
                           cudaStream_t s, int *n_launch);
 // reduce.cu
 struct ReduceState {             // device, per segment
