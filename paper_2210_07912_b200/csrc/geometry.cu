@@ -13,15 +13,22 @@ namespace {
 
 constexpr int GEOM_THREADS = 128;
 
+__device__ __forceinline__ double ipow4(double p1, double p2, double p4, double p8, int e) {   // x^e, 0 <= e < 16
+  double r = (e & 1) ? p1 : 1.0;
+  if (e & 2) r *= p2;
+  if (e & 4) r *= p4;
+  if (e & 8) r *= p8;
+  return r;
+}
+
 // a1-a4 for one sample.  Outputs: shifts s_k, F_k, Y_lm (arrays sized by the caller), c = D_ref/D (NaN for an invalid
-// sample) and the quadratic term q.
-template <int MAXM>
+// sample) and the quadratic term q.  `modes` and `Up`/`Vp` (the point's [K][M][M] blocks) may live in shared memory.
+template <int MAXM, int MAXK>
 __device__ __forceinline__ void sample_geometry(const DetGeom &g, const ModeEntry *__restrict__ modes, double ra, double dec,
-                                                double psi, double iota, double phi, double dist, int32_t point,
-                                                const double *__restrict__ U, const double *__restrict__ V,
-                                                int32_t (&shift)[RIFT_MAX_DET], double (&Fre)[RIFT_MAX_DET],
-                                                double (&Fim)[RIFT_MAX_DET], double (&Yre)[MAXM], double (&Yim)[MAXM],
-                                                double &c_out, double &q_out) {
+                                                double psi, double iota, double phi, double dist,
+                                                const double2 *__restrict__ Up, const double2 *__restrict__ Vp,
+                                                int32_t (&shift)[MAXK], double (&Fre)[MAXK], double (&Fim)[MAXK],
+                                                double (&Yre)[MAXM], double (&Yim)[MAXM], double &c_out, double &q_out) {
   const int K = g.n_det, M = g.n_modes;
   double sd, cd, sh, ch, sp, cp;
   sincos(dec, &sd, &cd);
@@ -31,7 +38,7 @@ __device__ __forceinline__ void sample_geometry(const DetGeom &g, const ModeEntr
   // ---- a3: delays and integer shifts, every operation individually rounded (no FMA contraction)
   const double nx = __dmul_rn(cd, ch), ny = __dmul_rn(cd, sh), nz = sd;
 #pragma unroll
-  for (int k = 0; k < RIFT_MAX_DET; ++k) {
+  for (int k = 0; k < MAXK; ++k) {
     if (k < K) {
       const double dot = __dadd_rn(__dadd_rn(__dmul_rn(g.loc[k][0], nx), __dmul_rn(g.loc[k][1], ny)),
                                    __dmul_rn(g.loc[k][2], nz));
@@ -51,7 +58,7 @@ __device__ __forceinline__ void sample_geometry(const DetGeom &g, const ModeEntr
   const double pxy[6] = {2.0 * X[0] * Yv[0], 2.0 * X[1] * Yv[1], 2.0 * X[2] * Yv[2], X[0] * Yv[1] + X[1] * Yv[0],
                          X[0] * Yv[2] + X[2] * Yv[0], X[1] * Yv[2] + X[2] * Yv[1]};
 #pragma unroll
-  for (int k = 0; k < RIFT_MAX_DET; ++k) {
+  for (int k = 0; k < MAXK; ++k) {
     if (k < K) {
       const double *D = g.resp[k];
       // D need not be exactly symmetric in the caller's array: use D_ij + D_ji for the off-diagonal pairs
@@ -61,36 +68,55 @@ __device__ __forceinline__ void sample_geometry(const DetGeom &g, const ModeEntr
     }
   }
 
-  // ---- a2: harmonics.  powers of cos(iota/2), sin(iota/2); e^{-i m phi} by angle addition
-  double pc[17], ps[17], cm[9], sm[9];
+  // ---- a2: harmonics.  The terms of one mode are coef[t] c^(pc0 - 2t) s^(ps0 + 2t) (c, s = cos, sin of iota/2), i.e.
+  // c^pcmin s^psmin times a homogeneous polynomial in c^2, s^2 (Horner); integer powers and e^{-i |m| phi} by binary
+  // powering -- no per-thread tables.
   {
-    double shalf, chalf;
-    sincos(0.5 * iota, &shalf, &chalf);
-    pc[0] = ps[0] = 1.0;
-    const int np = 2 * g.l_max;
-    for (int i = 1; i <= 16; ++i) {
-      pc[i] = (i <= np) ? pc[i - 1] * chalf : 0.0;
-      ps[i] = (i <= np) ? ps[i - 1] * shalf : 0.0;
-    }
-    double s1, c1;
-    sincos(phi, &s1, &c1);
-    cm[0] = 1.0;
-    sm[0] = 0.0;
-    for (int i = 1; i <= 8; ++i) {
-      cm[i] = cm[i - 1] * c1 - sm[i - 1] * s1;
-      sm[i] = sm[i - 1] * c1 + cm[i - 1] * s1;
-    }
-  }
+    double s1, c1, s2h, c2h;
+    sincos(0.5 * iota, &s1, &c1);
+    const double c2 = c1 * c1, c4 = c2 * c2, c8 = c4 * c4;
+    const double s2 = s1 * s1, s4 = s2 * s2, s8 = s4 * s4;
+    sincos(phi, &s2h, &c2h);
+    const double z1r = c2h, z1i = -s2h;                                   // z = e^{-i phi}
+    const double z2r = z1r * z1r - z1i * z1i, z2i = 2.0 * z1r * z1i;
+    const double z4r = z2r * z2r - z2i * z2i, z4i = 2.0 * z2r * z2i;
+    const double z8r = z4r * z4r - z4i * z4i, z8i = 2.0 * z4r * z4i;
 #pragma unroll(MAXM <= 16 ? MAXM : 1)
-  for (int a = 0; a < MAXM; ++a) {
-    if (a < M) {
-      const ModeEntry &e = modes[a];
-      double amp = 0.0;
-      for (int t = 0; t < e.n_terms; ++t) amp += e.coef[t] * pc[e.pc[t]] * ps[e.ps[t]];
-      const int am = e.m < 0 ? -e.m : e.m;
-      // e^{i m (-phi)} = cos(m phi) - i sin(m phi)
-      Yre[a] = amp * cm[am];
-      Yim[a] = (e.m < 0) ? amp * sm[am] : -amp * sm[am];
+    for (int a = 0; a < MAXM; ++a) {
+      if (a < M) {
+        const ModeEntry &e = modes[a];
+        const int n = e.n_terms;
+        double P = e.coef[0], spw = 1.0;
+#pragma unroll
+        for (int t = 1; t < RIFT_MAX_TERMS; ++t) {
+          if (t < n) {
+            spw *= s2;
+            P = P * c2 + e.coef[t] * spw;
+          }
+        }
+        const double amp = P * ipow4(c1, c2, c4, c8, e.pc[n - 1]) * ipow4(s1, s2, s4, s8, e.ps[0]);
+        const int am = e.m < 0 ? -e.m : e.m;
+        double wr = 1.0, wi = 0.0;                                          // z^|m|
+        if (am & 1) wr = z1r, wi = z1i;
+        if (am & 2) {
+          const double t = wr * z2r - wi * z2i;
+          wi = wr * z2i + wi * z2r;
+          wr = t;
+        }
+        if (am & 4) {
+          const double t = wr * z4r - wi * z4i;
+          wi = wr * z4i + wi * z4r;
+          wr = t;
+        }
+        if (am & 8) {
+          const double t = wr * z8r - wi * z8i;
+          wi = wr * z8i + wi * z8r;
+          wr = t;
+        }
+        // e^{i m (-phi)} = z^m (m >= 0) or conj(z^|m|) (m < 0)
+        Yre[a] = amp * wr;
+        Yim[a] = (e.m < 0) ? -amp * wi : amp * wi;
+      }
     }
   }
 
@@ -100,11 +126,9 @@ __device__ __forceinline__ void sample_geometry(const DetGeom &g, const ModeEntr
 
   // ---- a4: quadratic term; U Hermitian, V symmetric: diagonal + 2 * strict upper triangle.  The mode-pair products
   // conj(Y_a) Y_b and Y_a Y_b do not depend on the detector and are formed once.
-  double yuy[RIFT_MAX_DET], yvr[RIFT_MAX_DET], yvi[RIFT_MAX_DET];
+  double yuy[MAXK], yvr[MAXK], yvi[MAXK];
 #pragma unroll
-  for (int k = 0; k < RIFT_MAX_DET; ++k) yuy[k] = yvr[k] = yvi[k] = 0.0;
-  const double2 *Up = reinterpret_cast<const double2 *>(U) + (int64_t)point * K * M * M;
-  const double2 *Vp = reinterpret_cast<const double2 *>(V) + (int64_t)point * K * M * M;
+  for (int k = 0; k < MAXK; ++k) yuy[k] = yvr[k] = yvi[k] = 0.0;
 #pragma unroll(MAXM <= 16 ? MAXM : 1)
   for (int a = 0; a < MAXM; ++a) {
     if (a < M) {
@@ -117,7 +141,7 @@ __device__ __forceinline__ void sample_geometry(const DetGeom &g, const ModeEntr
           const double cr = w * (ar * br + ai * bi), ci = w * (ar * bi - ai * br);      // conj(Y_a) Y_b
           const double pr = w * (ar * br - ai * bi), pi = w * (ar * bi + ai * br);      // Y_a Y_b
 #pragma unroll
-          for (int k = 0; k < RIFT_MAX_DET; ++k) {
+          for (int k = 0; k < MAXK; ++k) {
             if (k < K) {
               const double2 u = Up[(k * M + a) * M + bb], v = Vp[(k * M + a) * M + bb];
               yuy[k] += u.x * cr - u.y * ci;
@@ -131,7 +155,7 @@ __device__ __forceinline__ void sample_geometry(const DetGeom &g, const ModeEntr
   }
   double q = 0.0;
 #pragma unroll
-  for (int k = 0; k < RIFT_MAX_DET; ++k) {
+  for (int k = 0; k < MAXK; ++k) {
     if (k < K) {
       const double f2 = Fre[k] * Fre[k] + Fim[k] * Fim[k];
       const double f2r = Fre[k] * Fre[k] - Fim[k] * Fim[k], f2i = 2.0 * Fre[k] * Fim[k];
@@ -158,8 +182,10 @@ geometry_kernel(DetGeom g, const ModeEntry *__restrict__ modes, Batch b, const d
 
   int32_t shift[RIFT_MAX_DET];
   double Fre[RIFT_MAX_DET], Fim[RIFT_MAX_DET], Yre[RIFT_MAX_MODES], Yim[RIFT_MAX_MODES], c, q;
-  sample_geometry<RIFT_MAX_MODES>(g, modes, p_ra[gi], p_dec[gi], p_psi[gi], p_iota[gi], p_phi[gi], p_dist[gi], point, U,
-                                  V, shift, Fre, Fim, Yre, Yim, c, q);
+  const double2 *Up = reinterpret_cast<const double2 *>(U) + (int64_t)point * K * M * M;
+  const double2 *Vp = reinterpret_cast<const double2 *>(V) + (int64_t)point * K * M * M;
+  sample_geometry<RIFT_MAX_MODES, RIFT_MAX_DET>(g, modes, p_ra[gi], p_dec[gi], p_psi[gi], p_iota[gi], p_phi[gi],
+                                                p_dist[gi], Up, Vp, shift, Fre, Fim, Yre, Yim, c, q);
   int32_t *my_shift = ws.shift + w * K;
   for (int k = 0; k < K; ++k) {
     my_shift[k] = shift[k];
@@ -188,30 +214,50 @@ geometry_kernel(DetGeom g, const ModeEntry *__restrict__ modes, Batch b, const d
 }
 
 // Tensor-core variant: one thread per batch slot; writes the batch blob described at TcPlan (rift_internal.h).
-// MT = number of modes (compile time, so that the operand chunks are assembled in registers).
-template <int MT>
+// MT = number of modes, KT = number of detectors (compile time, so that the operand chunks are assembled in registers
+// and nothing is predicated on k < K).  The mode tables and the U, V blocks of the block's (first) intrinsic point are
+// staged in shared memory.
+template <int MT, int KT>
 __global__ void __launch_bounds__(GEOM_THREADS)
 geometry_tc_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, TcChunk ch, const double *__restrict__ p_ra,
                    const double *__restrict__ p_dec, const double *__restrict__ p_psi, const double *__restrict__ p_iota,
                    const double *__restrict__ p_phi, const double *__restrict__ p_dist, const double *__restrict__ U,
                    const double *__restrict__ V, int32_t *__restrict__ shift_out) {
-  const int64_t w = (int64_t)blockIdx.x * GEOM_THREADS + threadIdx.x;     // slot = local batch * 16 + n
-  if (w >= ch.n_batches * RIFT_TC_NB) return;
+  constexpr int K = KT;
+  constexpr int KP = (6 * MT + 15) & ~15;                                   // contraction length, fp16 elements
+  constexpr int NCH = KP / 8;                                               // 16-byte chunks per detector
+  __shared__ ModeEntry s_modes[MT];
+  __shared__ double2 s_U[KT * MT * MT], s_V[KT * MT * MT];
+  const int64_t n_slots = ch.n_batches * RIFT_TC_NB;
+  const int64_t w0 = (int64_t)blockIdx.x * GEOM_THREADS;                    // first slot of the block
+  const int32_t point0 = ch.ids[(ch.gb0 + w0 / RIFT_TC_NB) / ch.nbps];
+  {
+    const int32_t *src = reinterpret_cast<const int32_t *>(modes);
+    int32_t *dst = reinterpret_cast<int32_t *>(s_modes);
+    for (int i = threadIdx.x; i < (int)(MT * sizeof(ModeEntry) / 4); i += GEOM_THREADS) dst[i] = src[i];
+    const double2 *u = reinterpret_cast<const double2 *>(U) + (int64_t)point0 * K * MT * MT;
+    const double2 *v = reinterpret_cast<const double2 *>(V) + (int64_t)point0 * K * MT * MT;
+    for (int i = threadIdx.x; i < K * MT * MT; i += GEOM_THREADS) {
+      s_U[i] = u[i];
+      s_V[i] = v[i];
+    }
+  }
+  __syncthreads();
+  const int64_t w = w0 + threadIdx.x;                                       // slot = local batch * 16 + n
+  if (w >= n_slots) return;
   const int64_t lb = w / RIFT_TC_NB;
   const int n = (int)(w % RIFT_TC_NB);
   const int64_t gb = ch.gb0 + lb;
   const int64_t seg = gb / ch.nbps;
   const int64_t i = (gb % ch.nbps) * RIFT_TC_NB + n;
   const bool valid = i < ch.n_per_seg;
-  const int K = g.n_det;
-  constexpr int KP = (6 * MT + 15) & ~15;                                   // contraction length, fp16 elements
-  constexpr int NCH = KP / 8;                                               // 16-byte chunks per detector
   float *blob = ch.blob + lb * tp.blob_words;
   uint4 *chunks = reinterpret_cast<uint4 *>(blob);                          // [K][NCH][16] x 8 halfs
   int32_t *dsh = reinterpret_cast<int32_t *>(blob + K * NCH * 64);          // [K][16]
   float *cl2 = blob + K * NCH * 64 + K * 16;                                // [16]
   if (!valid) {
     const uint4 z = make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
     for (int k = 0; k < K; ++k) {
 #pragma unroll
       for (int c = 0; c < NCH; ++c) chunks[(k * NCH + c) * 16 + n] = z;
@@ -224,49 +270,71 @@ geometry_tc_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, Tc
   }
   const int64_t gi = seg * ch.n_per_seg + i;
   const int32_t point = ch.ids[seg];
-  int32_t shift[RIFT_MAX_DET];
-  double Fre[RIFT_MAX_DET], Fim[RIFT_MAX_DET], Yre[MT], Yim[MT], c, q;
-  sample_geometry<MT>(g, modes, p_ra[gi], p_dec[gi], p_psi[gi], p_iota[gi], p_phi[gi], p_dist[gi], point, U, V, shift,
-                      Fre, Fim, Yre, Yim, c, q);
+  const double2 *Up = s_U, *Vp = s_V;
+  if (point != point0) {                                                    // a block that straddles two segments
+    Up = reinterpret_cast<const double2 *>(U) + (int64_t)point * K * MT * MT;
+    Vp = reinterpret_cast<const double2 *>(V) + (int64_t)point * K * MT * MT;
+  }
+  int32_t shift[KT];
+  double Fre[KT], Fim[KT], Yre[MT], Yim[MT], c, q;
+  sample_geometry<MT, KT>(g, s_modes, p_ra[gi], p_dec[gi], p_psi[gi], p_iota[gi], p_phi[gi], p_dist[gi], Up, Vp, shift,
+                          Fre, Fim, Yre, Yim, c, q);
   ch.scale_c[w] = c;
   ch.quad[w] = q;
   // exponent scale of the fused kernel: its accumulators carry x * (Q scale of the point) * RIFT_TC_BSCALE
   cl2[n] = (float)(c * 1.4426950408889634 / ((double)ch.qscale[point] * RIFT_TC_BSCALE));
 #pragma unroll
-  for (int k = 0; k < RIFT_MAX_DET; ++k) {
-    if (k < K) {
-      if (shift_out) shift_out[gi * K + k] = shift[k];
-      dsh[k * 16 + n] = shift[k] - shift[0];
-      // a5: B = F_k Y_lm, scaled, split into fp16 hi + lo; kappa = 2a (Re), 2a+1 (Im).  The contraction index runs over
-      // [hi | hi | lo] facing the A operand's [Q_hi | Q_lo | Q_hi].
-      uint16_t hv[KP];
+  for (int k = 0; k < K; ++k) {
+    if (shift_out) shift_out[gi * K + k] = shift[k];
+    dsh[k * 16 + n] = shift[k] - shift[0];
+    // a5: B = F_k Y_lm, scaled, split into fp16 hi + lo; kappa = 2a (Re), 2a+1 (Im).  The contraction index runs over
+    // [hi | hi | lo] facing the A operand's [Q_hi | Q_lo | Q_hi].
+    uint16_t hv[KP];
 #pragma unroll
-      for (int a = 0; a < MT; ++a) {
-        const double vr = (Fre[k] * Yre[a] - Fim[k] * Yim[a]) * RIFT_TC_BSCALE;
-        const double vi = (Fre[k] * Yim[a] + Fim[k] * Yre[a]) * RIFT_TC_BSCALE;
-        const __half hr = __double2half(vr), hi = __double2half(vi);
-        const __half lr = __double2half(vr - (double)__half2float(hr)), li = __double2half(vi - (double)__half2float(hi));
-        hv[2 * a] = hv[2 * MT + 2 * a] = __half_as_ushort(hr);
-        hv[2 * a + 1] = hv[2 * MT + 2 * a + 1] = __half_as_ushort(hi);
-        hv[4 * MT + 2 * a] = __half_as_ushort(lr);
-        hv[4 * MT + 2 * a + 1] = __half_as_ushort(li);
-      }
+    for (int a = 0; a < MT; ++a) {
+      const double vr = (Fre[k] * Yre[a] - Fim[k] * Yim[a]) * RIFT_TC_BSCALE;
+      const double vi = (Fre[k] * Yim[a] + Fim[k] * Yre[a]) * RIFT_TC_BSCALE;
+      const __half hr = __double2half(vr), hi = __double2half(vi);
+      const __half lr = __double2half(vr - (double)__half2float(hr)), li = __double2half(vi - (double)__half2float(hi));
+      hv[2 * a] = hv[2 * MT + 2 * a] = __half_as_ushort(hr);
+      hv[2 * a + 1] = hv[2 * MT + 2 * a + 1] = __half_as_ushort(hi);
+      hv[4 * MT + 2 * a] = __half_as_ushort(lr);
+      hv[4 * MT + 2 * a + 1] = __half_as_ushort(li);
+    }
 #pragma unroll
-      for (int e = 6 * MT; e < KP; ++e) hv[e] = 0;
-      uint4 *dst = chunks + (k * NCH) * 16 + n;
+    for (int e = 6 * MT; e < KP; ++e) hv[e] = 0;
+    uint4 *dst = chunks + (k * NCH) * 16 + n;
 #pragma unroll
-      for (int cc = 0; cc < NCH; ++cc) {
-        uint4 v;
-        v.x = (uint32_t)hv[8 * cc + 0] | ((uint32_t)hv[8 * cc + 1] << 16);
-        v.y = (uint32_t)hv[8 * cc + 2] | ((uint32_t)hv[8 * cc + 3] << 16);
-        v.z = (uint32_t)hv[8 * cc + 4] | ((uint32_t)hv[8 * cc + 5] << 16);
-        v.w = (uint32_t)hv[8 * cc + 6] | ((uint32_t)hv[8 * cc + 7] << 16);
-        dst[cc * 16] = v;
-      }
+    for (int cc = 0; cc < NCH; ++cc) {
+      uint4 v;
+      v.x = (uint32_t)hv[8 * cc + 0] | ((uint32_t)hv[8 * cc + 1] << 16);
+      v.y = (uint32_t)hv[8 * cc + 2] | ((uint32_t)hv[8 * cc + 3] << 16);
+      v.z = (uint32_t)hv[8 * cc + 4] | ((uint32_t)hv[8 * cc + 5] << 16);
+      v.w = (uint32_t)hv[8 * cc + 6] | ((uint32_t)hv[8 * cc + 7] << 16);
+      dst[cc * 16] = v;
     }
   }
 }
 
+}  // namespace
+
+namespace {
+template <int MT>
+cudaError_t launch_geometry_tc_m(const DetGeom &g, const ModeEntry *modes, const TcPlan &tp, const TcChunk &c,
+                                 const double *const params[6], const double *U, const double *V, int32_t *shift_out,
+                                 unsigned grid, cudaStream_t s) {
+#define RIFT_GEOM_TC(KT)                                                                                                 \
+  case KT:                                                                                                               \
+    geometry_tc_kernel<MT, KT><<<grid, GEOM_THREADS, 0, s>>>(g, modes, tp, c, params[0], params[1], params[2], params[3], \
+                                                              params[4], params[5], U, V, shift_out);                    \
+    break;
+  switch (tp.K) {
+    RIFT_GEOM_TC(1) RIFT_GEOM_TC(2) RIFT_GEOM_TC(3) RIFT_GEOM_TC(4) RIFT_GEOM_TC(5)
+    default: return cudaErrorInvalidValue;
+  }
+#undef RIFT_GEOM_TC
+  return cudaGetLastError();
+}
 }  // namespace
 
 cudaError_t launch_geometry_tc(const DetGeom &g, const ModeEntry *modes, const TcPlan &tp, const TcChunk &c,
@@ -275,18 +343,17 @@ cudaError_t launch_geometry_tc(const DetGeom &g, const ModeEntry *modes, const T
   const int64_t n = c.n_batches * RIFT_TC_NB;
   if (n <= 0) return cudaSuccess;
   const unsigned grid = (unsigned)((n + GEOM_THREADS - 1) / GEOM_THREADS);
-#define RIFT_GEOM_TC(MT)                                                                                             \
-  case MT:                                                                                                           \
-    geometry_tc_kernel<MT><<<grid, GEOM_THREADS, 0, s>>>(g, modes, tp, c, params[0], params[1], params[2], params[3], \
-                                                          params[4], params[5], U, V, shift_out);                    \
-    break;
   switch (tp.M) {
-    RIFT_GEOM_TC(1) RIFT_GEOM_TC(2) RIFT_GEOM_TC(3) RIFT_GEOM_TC(4) RIFT_GEOM_TC(5) RIFT_GEOM_TC(6) RIFT_GEOM_TC(7)
-    RIFT_GEOM_TC(8)
+    case 1: return launch_geometry_tc_m<1>(g, modes, tp, c, params, U, V, shift_out, grid, s);
+    case 2: return launch_geometry_tc_m<2>(g, modes, tp, c, params, U, V, shift_out, grid, s);
+    case 3: return launch_geometry_tc_m<3>(g, modes, tp, c, params, U, V, shift_out, grid, s);
+    case 4: return launch_geometry_tc_m<4>(g, modes, tp, c, params, U, V, shift_out, grid, s);
+    case 5: return launch_geometry_tc_m<5>(g, modes, tp, c, params, U, V, shift_out, grid, s);
+    case 6: return launch_geometry_tc_m<6>(g, modes, tp, c, params, U, V, shift_out, grid, s);
+    case 7: return launch_geometry_tc_m<7>(g, modes, tp, c, params, U, V, shift_out, grid, s);
+    case 8: return launch_geometry_tc_m<8>(g, modes, tp, c, params, U, V, shift_out, grid, s);
     default: return cudaErrorInvalidValue;
   }
-#undef RIFT_GEOM_TC
-  return cudaGetLastError();
 }
 
 cudaError_t launch_geometry(const DetGeom &g, const ModeEntry *modes, const Batch &b, const double *const params[6],
