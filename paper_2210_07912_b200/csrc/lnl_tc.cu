@@ -25,7 +25,7 @@
 
 namespace {
 
-constexpr int TC_THREADS = 320;
+constexpr int TC_THREADS = 384;       // 8 epilogue warps, producer, UMMA issuer, 2 idle warps completing the third warpgroup
 constexpr int TC_STAGES = 3;
 constexpr int NH = RIFT_TC_NB / 2;   // samples per epilogue warpgroup
 
@@ -169,38 +169,49 @@ __global__ void __launch_bounds__(TC_THREADS, 1) lnl_tc_kernel(const TcArgs args
 
   const int64_t b_begin = (ch.n_batches * blockIdx.x) / gridDim.x;
   const int64_t b_end = (ch.n_batches * (blockIdx.x + 1)) / gridDim.x;
-  uint32_t it = 0;                                                        // batches done by this CTA (all roles in step)
-  int staged_point = -1;
 
-  for (int64_t b0 = b_begin; b0 < b_end;) {
-    const int64_t seg = (ch.gb0 + b0) / ch.nbps;
-    const int64_t job_end = min(b_end, (seg + 1) * ch.nbps - ch.gb0);
-    const int point = ch.ids[seg];
-    const uint32_t nb = (uint32_t)(job_end - b0);
-
-    // ---- the A operand of this intrinsic point -> tensor memory (thread = TMEM lane = row of the tile)
-    __syncthreads();                       // every role is done with the previous job (all UMMAs have completed)
-    if (point != staged_point && warp < 4) {
-      for (int k = 0; k < K; ++k)
-        for (int i = 0; i < NT; ++i) {
-          const int row = 128 * i + 32 * warp + lane;
-          const float4 *src =
-              reinterpret_cast<const float4 *>(args.qtc + (((int64_t)point * K + k) * (NT * 128) + row) * acols);
-          const uint32_t taddr = tmem_base + ((uint32_t)(32 * warp) << 16) + (uint32_t)((k * NT + i) * acols);
-          for (int c8 = 0; c8 < acols; c8 += 8) {
-            const float4 a = __ldg(src + (c8 >> 2)), b = __ldg(src + (c8 >> 2) + 1);
-            tc_st8(taddr + c8, a, b);
+  // Jobs = runs of batches of one intrinsic point.  Every role walks the same job list; at a job boundary all warps
+  // meet (all UMMAs of the previous job have completed) and warps 0-3 put the A operand of the new point into tensor
+  // memory (thread = TMEM lane = row of the tile).
+  auto for_each_job = [&](auto &&body) {
+    uint32_t it = 0;                                                      // batches done by this CTA (all roles in step)
+    int staged_point = -1;
+    for (int64_t b0 = b_begin; b0 < b_end;) {
+      const int64_t seg = (ch.gb0 + b0) / ch.nbps;
+      const int64_t job_end = min(b_end, (seg + 1) * ch.nbps - ch.gb0);
+      const int point = ch.ids[seg];
+      const uint32_t nb = (uint32_t)(job_end - b0);
+      __syncthreads();
+      if (point != staged_point && warp < 4) {
+        for (int k = 0; k < K; ++k)
+          for (int i = 0; i < NT; ++i) {
+            const int row = 128 * i + 32 * warp + lane;
+            const float4 *src =
+                reinterpret_cast<const float4 *>(args.qtc + (((int64_t)point * K + k) * (NT * 128) + row) * acols);
+            const uint32_t taddr = tmem_base + ((uint32_t)(32 * warp) << 16) + (uint32_t)((k * NT + i) * acols);
+            for (int c8 = 0; c8 < acols; c8 += 8) {
+              const float4 a = __ldg(src + (c8 >> 2)), b = __ldg(src + (c8 >> 2) + 1);
+              tc_st8(taddr + c8, a, b);
+            }
           }
-        }
-      asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+      }
+      staged_point = point;
+      tc_fence_before();
+      __syncthreads();
+      tc_fence_after();
+      body(point, b0, nb, it);
+      it += nb;
+      b0 = job_end;
     }
-    staged_point = point;
-    tc_fence_before();
-    __syncthreads();
-    tc_fence_after();
+  };
 
+  // Register budget: the service warpgroup (warps 8-11) keeps 40 registers per thread, the epilogue warpgroups take 208.
+  if (warp >= 8) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
     if (warp == 8) {
       // ===== producer: one bulk copy per batch blob =====
+      for_each_job([&](int, int64_t b0, uint32_t nb, uint32_t it) {
       if (lane == 0) {
         for (uint32_t j = 0; j < nb; ++j) {
           const uint32_t g = it + j, stage = g % TC_STAGES, ph = (g / TC_STAGES) & 1u;
@@ -211,9 +222,11 @@ __global__ void __launch_bounds__(TC_THREADS, 1) lnl_tc_kernel(const TcArgs args
         }
       }
       __syncwarp();
+      });
     } else if (warp == 9) {
       // ===== UMMA issuer =====  (K=16 steps outermost: consecutive UMMAs accumulate into different tiles)
       const int n_steps = tp.kp >> 4;
+      for_each_job([&](int, int64_t, uint32_t nb, uint32_t it) {
       for (uint32_t j = 0; j < nb; ++j) {
         const uint32_t g = it + j, stage = g % TC_STAGES, ph = (g / TC_STAGES) & 1u;
         mbar_wait_idle(bar_full + stage, ph);
@@ -236,7 +249,13 @@ __global__ void __launch_bounds__(TC_THREADS, 1) lnl_tc_kernel(const TcArgs args
         }
         __syncwarp();
       }
+      });
     } else {
+      for_each_job([](int, int64_t, uint32_t, uint32_t) {});                // idle warps: job-boundary barriers only
+    }
+  } else {
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 208;");
+    for_each_job([&](int point, int64_t b0, uint32_t nb, uint32_t it) {
       // ===== epilogue warpgroups =====
       const int wg = warp >> 2, q = warp & 3;
       const int T = 32 * q + lane;
@@ -278,37 +297,28 @@ __global__ void __launch_bounds__(TC_THREADS, 1) lnl_tc_kernel(const TcArgs args
         }
       };
 
-      for (uint32_t j = 0; j < nb; ++j) {
-        const uint32_t g = it + j, stage = g % TC_STAGES, ph = (g / TC_STAGES) & 1u;
-        const float *blob = blob_s + stage * tp.blob_words;
+      // Phase A of batch g (after its accumulators are ready): P_k (k >= 1) -> exchange buffer, P_0 -> registers xd; the
+      // loads of the next detector are in flight while the current one is stored.  No spin inside, so that the caller can
+      // fuse it with the reduction of the previous batch in one basic block.
+      auto phase_a = [&](uint32_t g, float (&xd)[NT][NH]) {
         float *xb = xb_s + (size_t)((wg * 2 + (g & 1u)) * (K - 1)) * NH * PITCH;
-        mbar_wait(bar_full + stage, ph);
-        mbar_wait(bar_tfull, g & 1u);
-        tc_fence_after();
-
-        // Phase A: P_k (k >= 1) -> exchange buffer, P_0 -> registers; the loads of the next detector are in flight
-        // while the current one is stored
-        float x[NT][NH], ra[NT][NH], rb[NT][NH];
-        if (K > 1) load_tiles(1, ra); else load_tiles(0, x);
-        for (int k = 1; k < K; k += 2) {
+        float ra[NT][NH];
+        load_tiles(0, xd);                                                 // P_0 stays in registers
+        for (int k = 1; k < K; ++k) {
+          load_tiles(k, ra);
           wait_tiles(ra);
-          if (k + 1 < K) load_tiles(k + 1, rb); else load_tiles(0, x);
           store_tiles(k, xb, ra);
-          if (k + 1 < K) {
-            wait_tiles(rb);
-            if (k + 2 < K) load_tiles(k + 2, ra); else load_tiles(0, x);
-            store_tiles(k + 1, xb, rb);
-          }
         }
-        wait_tiles(x);
+        wait_tiles(xd);
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_tempty);                            // the UMMAs of the next batch may overwrite D
-        named_bar_sync(1 + wg, 128);                                       // exchange rows of this warpgroup are complete
-
-        // Phase B: shifted sum over detectors
+      };
+      // Phase B: shifted sum over detectors
+      auto phase_b = [&](uint32_t g, float (&x)[NT][NH]) {
+        const float *blob = blob_s + (g % TC_STAGES) * tp.blob_words;
+        const float *xb = xb_s + (size_t)((wg * 2 + (g & 1u)) * (K - 1)) * NH * PITCH;
         const int32_t *dsh = reinterpret_cast<const int32_t *>(blob + K * tp.nch * 64) + NH * wg;
-        const float *cl2s = blob + K * tp.nch * 64 + K * 16 + NH * wg;
         for (int k = 1; k < K; ++k) {
           const int4 d0 = *reinterpret_cast<const int4 *>(dsh + k * 16), d1 = *reinterpret_cast<const int4 *>(dsh + k * 16 + 4);
           const int d[NH] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
@@ -321,7 +331,12 @@ __global__ void __launch_bounds__(TC_THREADS, 1) lnl_tc_kernel(const TcArgs args
             x[NT - 1][n] += src[128 * (NT - 1) + last_clamp];
           }
         }
-        // per-warp (reference, sum) of the time marginal for the 8 samples
+      };
+      // per-warp (reference, sum) of the time marginal for the 8 samples of batch g (chunk-local batch index lb)
+      auto reduce = [&](uint32_t g, int64_t lb, float (&x)[NT][NH]) {
+        const uint32_t stage = g % TC_STAGES;
+        const float *blob = blob_s + stage * tp.blob_words;
+        const float *cl2s = blob + K * tp.nch * 64 + K * 16 + NH * wg;
         float m[NH];
 #pragma unroll
         for (int n = 0; n < NH; ++n) {
@@ -352,15 +367,38 @@ __global__ void __launch_bounds__(TC_THREADS, 1) lnl_tc_kernel(const TcArgs args
           // sum_j 2^(x_j cl - off) = 2^res sum_j 2^((x_j - m) cl),  res = m cl - off
           const float off = (mine == -INFINITY) ? 0.f : mine * cl;
           const float res = (mine == -INFINITY) ? 0.f : fmaf(mine, cl, -off);
-          ch.part[((b0 + j) * RIFT_TC_NB + NH * wg + nsel) * 4 + q] =
-              make_float2(mine * inv_scale, ssum * fast_exp2(-res));
+          ch.part[(lb * RIFT_TC_NB + NH * wg + nsel) * 4 + q] = make_float2(mine * inv_scale, ssum * fast_exp2(-res));
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_empty + stage);
+      };
+
+      // Software pipeline over the batches of this job: the reduction of batch g (shuffle / exponential latency chains)
+      // and Phase A of batch g + 1 (tensor-memory loads, shared-memory stores) are issued from one basic block.
+      float x[NT][NH];
+      mbar_wait(bar_tfull, it & 1u);
+      tc_fence_after();
+      phase_a(it, x);
+      for (uint32_t j = 0; j < nb; ++j) {
+        const uint32_t g = it + j;
+        named_bar_sync(1 + wg, 128);                                       // exchange rows of batch g are complete
+        mbar_wait(bar_full + g % TC_STAGES, (g / TC_STAGES) & 1u);         // shifts and exponent scales of batch g
+        phase_b(g, x);
+        if (j + 1 < nb) {
+          mbar_wait(bar_tfull, (g + 1u) & 1u);
+          tc_fence_after();
+          float xn[NT][NH];
+          phase_a(g + 1u, xn);
+          reduce(g, b0 + j, x);
+#pragma unroll
+          for (int i = 0; i < NT; ++i)
+#pragma unroll
+            for (int n = 0; n < NH; ++n) x[i][n] = xn[i][n];
+        } else {
+          reduce(g, b0 + j, x);
+        }
       }
-    }
-    it += nb;
-    b0 = job_end;
+    });
   }
 
   tc_fence_before();
