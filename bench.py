@@ -32,6 +32,9 @@ from paper_2210_07912_b200 import synth  # noqa: E402
 METRIC = "time-marginalized lnL evals/sec"
 UNIT = "evals/s"
 N_SM, FP32_LANES, FP64_LANES = 148, 128, 64        # B200: guide unit counts (B200_PROFILING.md, B300_MICROARCH.md)
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused kernel from the committed `ncu --set full` captures
+# (profiles/), keyed by (kernel, config index); a launch = one chunk of the batch (262144 evaluations for lnl_tc on C1).
+NCU_TRAFFIC_BYTES = {("lnl_tc<f16x3>", 1): 55.03e6, ("lnl_direct_ext<f32>", 1): 58.5e6}
 
 
 def measured_peaks() -> dict:
@@ -192,7 +195,7 @@ def run_ours(args) -> None:
     h = rift.rift_ile_create(loc, resp, cfg.gmst, ml, mm, P, cfg.n_t, cfg.delta_t, cfg.n_t, synth.D_REF_MPC,
                              inp.Q, inp.U, inp.V, precision=prec)
     if args.kernel:
-        rift.rift_ile_set_kernel(h, {"auto": 0, "direct": 1, "grouped": 2, "quad": 3}[args.kernel])
+        rift.rift_ile_set_kernel(h, {"auto": 0, "direct": 1, "grouped": 2, "quad": 3, "tc": 4}[args.kernel])
     ids = list(range(P))
     ps, ws = zip(*[synth.draw_samples(cfg, gids[p], theta_true=inp.theta_true[p]) for p in ids])
     params_np = np.concatenate(ps, axis=1)
@@ -215,14 +218,40 @@ def run_ours(args) -> None:
         return rift.rift_ile_reduce(h, P, N, lnL_d, lnw_d, params_d, synth.HIST_LO, synth.HIST_HI, n_bins, merge=0,
                                     want_hist=True, cuda_stream=stream)
 
+    # End to end through the same public calls, host buffers in and out.  The step is pipelined over groups of
+    # intrinsic points: a copy stream moves group g+1's samples host->device (and group g-1's lnL device->host) while the
+    # compute stream evaluates group g; the reduce runs once over all groups at the end.
+    copy_stream = torch.cuda.Stream()
+    n_groups = min(P, 8)
+    bounds = [(P * i) // n_groups for i in range(n_groups + 1)]
+
     def step_e2e(pd, wd):
-        pd.copy_(params_h, non_blocking=True)
-        if has_w:
-            wd.copy_(lnw_h, non_blocking=True)
-        rift.rift_ile_eval_batch(h, ids, N, pd, lnL_d, None, stream)
+        cur = torch.cuda.current_stream()
+        copy_stream.wait_stream(cur)
+        h2d = []
+        with torch.cuda.stream(copy_stream):
+            for gi in range(n_groups):
+                a, b = bounds[gi] * N, bounds[gi + 1] * N
+                for d in range(6):                       # contiguous pinned rows: plain async 1-D copies
+                    pd[d, a:b].copy_(params_h[d, a:b], non_blocking=True)
+                if has_w:
+                    wd[a:b].copy_(lnw_h[a:b], non_blocking=True)
+                ev = torch.cuda.Event()
+                ev.record(copy_stream)
+                h2d.append(ev)
+        for gi in range(n_groups):
+            a, b = bounds[gi] * N, bounds[gi + 1] * N
+            cur.wait_event(h2d[gi])
+            rift.rift_ile_eval_batch(h, ids[bounds[gi]:bounds[gi + 1]], N, [pd[d, a:b] for d in range(6)], lnL_d[a:b],
+                                     None, stream)
+            done = torch.cuda.Event()
+            done.record(cur)
+            with torch.cuda.stream(copy_stream):
+                copy_stream.wait_event(done)
+                lnL_h[a:b].copy_(lnL_d[a:b], non_blocking=True)
         red = rift.rift_ile_reduce(h, P, N, lnL_d, wd, pd, synth.HIST_LO, synth.HIST_HI, n_bins, merge=0,
                                    want_hist=True, cuda_stream=stream)
-        lnL_h.copy_(lnL_d, non_blocking=True)
+        cur.wait_stream(copy_stream)
         return red
 
     def barrier():
@@ -286,7 +315,13 @@ def run_ours(args) -> None:
                     "d2h_bytes_per_step": int(lnL_h.numel() * 8 + P * (4 + 6 * n_bins) * 8)},
             "gpu_launches": int(launches),
             "roofline": {"bound": "alu", "kernel": rift.rift_ile_kernel_name(h), "achieved": achieved, "peak": peak,
-                         "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                         "unit": "TFLOP/s", "frac": achieved / peak,
+                         "traffic": NCU_TRAFFIC_BYTES.get((rift.rift_ile_kernel_name(h), cfg.index)),
+                         "note": ("algorithmic FP32 flop (4 K M N_tau per evaluation) over the fused kernel's time, against the "
+                                  "FP32 FMA-pipe peak; lnl_tc runs the contraction on the tensor pipe (fp16 hi/lo pieces, fp32 "
+                                  "accumulate), so this is an FMA-pipe-equivalent fraction"
+                                  if "lnl_tc" in rift.rift_ile_kernel_name(h) else
+                                  "algorithmic flop (4 K M N_tau per evaluation) over the fused kernel's time"),
                          "peak_source": f"derived: {N_SM} SM x {FP64_LANES if fp64 else FP32_LANES} lanes x 2 x "
                                         f"{sm_max:.0f} MHz (MEASURED_PEAKS.json sm_max_mhz)",
                          "fma_microbench_tflops": micro, "frac_of_microbench": achieved / micro,
@@ -319,7 +354,7 @@ def main() -> None:
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1)
     ap.add_argument("--precision", default="mixed", choices=["mixed", "fp64"])
-    ap.add_argument("--kernel", default=None, choices=[None, "auto", "direct", "grouped", "quad"])
+    ap.add_argument("--kernel", default=None, choices=[None, "auto", "direct", "grouped", "quad", "tc"])
     ap.add_argument("--points", type=int, default=0, help="override the number of intrinsic points (debug)")
     ap.add_argument("--samples", type=int, default=0, help="override samples per point (debug)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
