@@ -119,6 +119,10 @@ cudaError_t launch_convert_q_tc(const double *Q_c128, uint32_t *dst, float *qsca
                                 cudaStream_t s);
 cudaError_t launch_lnl_tc(const TcPlan &tp, const uint32_t *qtc, const TcChunk &c, double *lnL_out, int n_sm,
                           cudaStream_t s, int *n_launch);
+// lnl_tile.cu (fp64 register-tiled contraction + shared-memory exchange; circular mode, n_t <= 512)
+size_t lnl_tile_smem_bytes(const QStore &q, int K, int pitch);
+cudaError_t launch_lnl_tile(const QStore &q, const Batch &b, const Workspace &ws, int K, int H, int pitch, const int *dmax,
+                            const double *exp_tab, double *lnL_out, int n_sm, cudaStream_t s, int *n_launch);
 // reduce.cu
 struct ReduceState {             // device, per segment
   double m, s1, s2;

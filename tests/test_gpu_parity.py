@@ -90,7 +90,7 @@ def test_higher_l_harmonics(torch, oracle):
 
 # ------------------------------------------------------------------------------------------------ C0, whole config
 KERNELS = [rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_DIRECT, rift.RIFT_KERNEL_GROUPED, rift.RIFT_KERNEL_QUAD,
-           rift.RIFT_KERNEL_TC]
+           rift.RIFT_KERNEL_TC, rift.RIFT_KERNEL_TILE]
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
@@ -111,6 +111,9 @@ def test_c0_all_samples_both_precisions(torch, oracle, rho, kernel):
         # the tensor-core kernel is the default of the mixed mode (and never runs in fp64 mode)
         assert ("lnl_tc" in rift.rift_ile_kernel_name(h)) == (
             prec == rift.RIFT_PREC_MIXED and kernel in (rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_TC))
+        # the register-tiled kernel exists for fp64 only and is opt-in
+        assert ("lnl_tile" in rift.rift_ile_kernel_name(h)) == (
+            prec == rift.RIFT_PREC_FP64 and kernel == rift.RIFT_KERNEL_TILE)
         if prec == rift.RIFT_PREC_FP64:
             assert np.max(rel_err(got, ref)) < TOL_FP64_REL, name
         else:
