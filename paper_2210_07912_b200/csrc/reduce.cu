@@ -97,34 +97,67 @@ reduce_merge_kernel(int64_t n_per_seg, int n_seg, int nbx, int n_bins, int merge
   const double *P = partial + (int64_t)seg * nbx * pstride;
   __shared__ double s_m, s_s1;
   __shared__ int s_nan;
+  __shared__ double s_f[4096];                     // exp(m_b - m) per partial block (nbx <= 4096, reduce_blocks_per_seg)
+  __shared__ double s_red[3][4];
+  __shared__ int s_red_nan[4];
   ReduceState old;
   old.m = -INFINITY;
   old.s1 = old.s2 = 0.0;
   old.n = 0;
   if (merge) old = state[seg];
+  const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
+
+  // pass 1 (all threads): NaN flag and maximum over the stored state and the partial blocks
+  double m = old.m;
+  int nan_seen = isnan(old.m) ? 1 : 0;
+  for (int b = threadIdx.x; b < nbx; b += 128) {
+    if (P[b * pstride + 3] != 0.0) nan_seen = 1;
+    m = fmax(m, P[b * pstride]);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    nan_seen |= __shfl_xor_sync(0xffffffffu, nan_seen, o);
+  }
+  if (lane == 0) {
+    s_red[0][wrp] = m;
+    s_red_nan[wrp] = nan_seen;
+  }
+  __syncthreads();
+  m = fmax(fmax(s_red[0][0], s_red[0][1]), fmax(s_red[0][2], s_red[0][3]));
+  nan_seen = s_red_nan[0] | s_red_nan[1] | s_red_nan[2] | s_red_nan[3];
+  __syncthreads();
+  // pass 2: rescaled sums
+  double s1 = 0.0, s2 = 0.0;
+  const bool live0 = !nan_seen && m > -INFINITY;
+  for (int b = threadIdx.x; b < nbx; b += 128) {
+    const double mb = P[b * pstride];
+    double f = 0.0;
+    if (live0 && mb > -INFINITY) {
+      f = exp(mb - m);
+      s1 += P[b * pstride + 1] * f;
+      s2 += P[b * pstride + 2] * f * f;
+    }
+    s_f[b] = f;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+    s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+  }
+  if (lane == 0) {
+    s_red[1][wrp] = s1;
+    s_red[2][wrp] = s2;
+  }
+  __syncthreads();
 
   if (threadIdx.x == 0) {
-    double m = old.m;
-    int nan_seen = isnan(old.m) ? 1 : 0;
-    for (int b = 0; b < nbx; ++b) {
-      if (P[b * pstride + 3] != 0.0) nan_seen = 1;
-      m = fmax(m, P[b * pstride]);
-    }
-    double s1 = 0.0, s2 = 0.0;
-    if (!nan_seen && m > -INFINITY) {
-      if (old.m > -INFINITY) {
-        const double f = exp(old.m - m);
-        s1 = old.s1 * f;
-        s2 = old.s2 * f * f;
-      }
-      for (int b = 0; b < nbx; ++b) {
-        const double mb = P[b * pstride];
-        if (mb > -INFINITY) {
-          const double f = exp(mb - m);
-          s1 += P[b * pstride + 1] * f;
-          s2 += P[b * pstride + 2] * f * f;
-        }
-      }
+    s1 = (s_red[1][0] + s_red[1][1]) + (s_red[1][2] + s_red[1][3]);
+    s2 = (s_red[2][0] + s_red[2][1]) + (s_red[2][2] + s_red[2][3]);
+    if (live0 && old.m > -INFINITY) {
+      const double f = exp(old.m - m);
+      s1 += old.s1 * f;
+      s2 += old.s2 * f * f;
     }
     const int64_t n = old.n + n_per_seg;
     ReduceState st;
@@ -163,19 +196,20 @@ reduce_merge_kernel(int64_t n_per_seg, int n_seg, int nbx, int n_bins, int merge
   }
   __syncthreads();
   if (state_hist == nullptr) return;
-  const double m = s_m, s1 = s_s1;
-  const bool live = !s_nan && m > -INFINITY;
+  const double mfin = s_m, s1fin = s_s1;
+  const bool live = !s_nan && mfin > -INFINITY;
+  const double f_old = (merge && live && old.m > -INFINITY) ? exp(old.m - mfin) : 0.0;
   for (int i = threadIdx.x; i < 6 * n_bins; i += blockDim.x) {
     double h = 0.0;
     if (live) {
-      if (merge && old.m > -INFINITY) h = state_hist[(int64_t)seg * 6 * n_bins + i] * exp(old.m - m);
+      if (f_old != 0.0) h = state_hist[(int64_t)seg * 6 * n_bins + i] * f_old;
       for (int b = 0; b < nbx; ++b) {
-        const double mb = P[b * pstride];
-        if (mb > -INFINITY) h += P[b * pstride + PARTIAL_HDR + i] * exp(mb - m);
+        const double f = s_f[b];
+        if (f != 0.0) h += P[b * pstride + PARTIAL_HDR + i] * f;
       }
     }
     state_hist[(int64_t)seg * 6 * n_bins + i] = h;
-    if (out_hist) out_hist[(int64_t)seg * 6 * n_bins + i] = (live && s1 > 0.0) ? h / s1 : 0.0;
+    if (out_hist) out_hist[(int64_t)seg * 6 * n_bins + i] = (live && s1fin > 0.0) ? h / s1fin : 0.0;
   }
 }
 
