@@ -438,7 +438,7 @@ __global__ void q_absmax_kernel(const double2 *__restrict__ src, uint32_t *__res
   }
 }
 // scale[p] = 2^e with scale * max|Q| in [2^13, 2^14)  (1 when the point is all zero)
-__global__ void q_scale_kernel(const uint32_t *__restrict__ mx, float *__restrict__ scale, int n_points) {
+__global__ void q_scale_kernel(const uint32_t *mx, float *scale, int n_points) {   // in place: mx aliases scale
   const int p = blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= n_points) return;
   const float a = __uint_as_float(mx[p]);
