@@ -30,6 +30,7 @@ __device__ __forceinline__ void sample_geometry(const DetGeom &g, const ModeEntr
                                                 int32_t (&shift)[MAXK], double (&Fre)[MAXK], double (&Fim)[MAXK],
                                                 double (&Yre)[MAXM], double (&Yim)[MAXM], double &c_out, double &q_out) {
   const int K = g.n_det, M = g.n_modes;
+  const int m_end = (MAXM <= 16) ? MAXM : M;        // unrolled (and predicated on a < M) for small MAXM, runtime bound else
   double sd, cd, sh, ch, sp, cp;
   sincos(dec, &sd, &cd);
   sincos(ra - g.gmst, &sh, &ch);           // ch = cos(ra-gmst) = cos(gha), sh = sin(ra-gmst) = -sin(gha)
@@ -82,7 +83,7 @@ __device__ __forceinline__ void sample_geometry(const DetGeom &g, const ModeEntr
     const double z4r = z2r * z2r - z2i * z2i, z4i = 2.0 * z2r * z2i;
     const double z8r = z4r * z4r - z4i * z4i, z8i = 2.0 * z4r * z4i;
 #pragma unroll(MAXM <= 16 ? MAXM : 1)
-    for (int a = 0; a < MAXM; ++a) {
+    for (int a = 0; a < m_end; ++a) {
       if (a < M) {
         const ModeEntry &e = modes[a];
         const int n = e.n_terms;
@@ -130,11 +131,11 @@ __device__ __forceinline__ void sample_geometry(const DetGeom &g, const ModeEntr
 #pragma unroll
   for (int k = 0; k < MAXK; ++k) yuy[k] = yvr[k] = yvi[k] = 0.0;
 #pragma unroll(MAXM <= 16 ? MAXM : 1)
-  for (int a = 0; a < MAXM; ++a) {
+  for (int a = 0; a < m_end; ++a) {
     if (a < M) {
       const double ar = Yre[a], ai = Yim[a];
 #pragma unroll(MAXM <= 16 ? MAXM : 1)
-      for (int bb = a; bb < MAXM; ++bb) {
+      for (int bb = a; bb < m_end; ++bb) {
         if (bb < M) {
           const double br = Yre[bb], bi = Yim[bb];
           const double w = (bb == a) ? 1.0 : 2.0;
@@ -165,7 +166,8 @@ __device__ __forceinline__ void sample_geometry(const DetGeom &g, const ModeEntr
   q_out = 0.25 * c * c * q;
 }
 
-template <typename CT>
+// CT = coefficient type; MAXM = 8 (mode loops unrolled, Y in registers) or RIFT_MAX_MODES; MAXK = number of detectors.
+template <typename CT, int MAXM, int MAXK>
 __global__ void __launch_bounds__(GEOM_THREADS)
 geometry_kernel(DetGeom g, const ModeEntry *__restrict__ modes, Batch b, const double *__restrict__ p_ra,
                 const double *__restrict__ p_dec, const double *__restrict__ p_psi, const double *__restrict__ p_iota,
@@ -180,12 +182,12 @@ geometry_kernel(DetGeom g, const ModeEntry *__restrict__ modes, Batch b, const d
   const int32_t point = b.ids[gi / b.n_per_seg];
   const int K = g.n_det, M = g.n_modes;
 
-  int32_t shift[RIFT_MAX_DET];
-  double Fre[RIFT_MAX_DET], Fim[RIFT_MAX_DET], Yre[RIFT_MAX_MODES], Yim[RIFT_MAX_MODES], c, q;
+  int32_t shift[MAXK];
+  double Fre[MAXK], Fim[MAXK], Yre[MAXM], Yim[MAXM], c, q;
   const double2 *Up = reinterpret_cast<const double2 *>(U) + (int64_t)point * K * M * M;
   const double2 *Vp = reinterpret_cast<const double2 *>(V) + (int64_t)point * K * M * M;
-  sample_geometry<RIFT_MAX_MODES, RIFT_MAX_DET>(g, modes, p_ra[gi], p_dec[gi], p_psi[gi], p_iota[gi], p_phi[gi],
-                                                p_dist[gi], Up, Vp, shift, Fre, Fim, Yre, Yim, c, q);
+  sample_geometry<MAXM, MAXK>(g, modes, p_ra[gi], p_dec[gi], p_psi[gi], p_iota[gi], p_phi[gi], p_dist[gi], Up, Vp, shift,
+                              Fre, Fim, Yre, Yim, c, q);
   int32_t *my_shift = ws.shift + w * K;
   for (int k = 0; k < K; ++k) {
     my_shift[k] = shift[k];
@@ -356,17 +358,37 @@ cudaError_t launch_geometry_tc(const DetGeom &g, const ModeEntry *modes, const T
   }
 }
 
+namespace {
+template <typename CT, int MAXM>
+cudaError_t launch_geometry_k(const DetGeom &g, const ModeEntry *modes, const Batch &b, const double *const params[6],
+                              const double *U, const double *V, const Workspace &ws, int32_t *shift_out, double *dbg_F,
+                              double *dbg_Y, const int32_t *perm, unsigned grid, cudaStream_t s) {
+#define RIFT_GEOM(KT)                                                                                                   \
+  case KT:                                                                                                              \
+    geometry_kernel<CT, MAXM, KT><<<grid, GEOM_THREADS, 0, s>>>(g, modes, b, params[0], params[1], params[2], params[3], \
+                                                                 params[4], params[5], U, V, ws, shift_out, dbg_F, dbg_Y, \
+                                                                 perm);                                                 \
+    break;
+  switch (g.n_det) {
+    RIFT_GEOM(1) RIFT_GEOM(2) RIFT_GEOM(3) RIFT_GEOM(4) RIFT_GEOM(5) RIFT_GEOM(6) RIFT_GEOM(7) RIFT_GEOM(8)
+    default: return cudaErrorInvalidValue;
+  }
+#undef RIFT_GEOM
+  return cudaGetLastError();
+}
+}  // namespace
+
 cudaError_t launch_geometry(const DetGeom &g, const ModeEntry *modes, const Batch &b, const double *const params[6],
                             const double *U, const double *V, bool coef_fp32, const Workspace &ws,
                             int32_t *shift_out, double *dbg_F, double *dbg_Y, const int32_t *perm, cudaStream_t s) {
   if (b.n <= 0) return cudaSuccess;
-  const int64_t n = b.n;
-  const unsigned grid = (unsigned)((n + GEOM_THREADS - 1) / GEOM_THREADS);
+  const unsigned grid = (unsigned)((b.n + GEOM_THREADS - 1) / GEOM_THREADS);
+  const bool small = g.n_modes <= 8;
   if (coef_fp32)
-    geometry_kernel<float2><<<grid, GEOM_THREADS, 0, s>>>(g, modes, b, params[0], params[1], params[2], params[3],
-                                                           params[4], params[5], U, V, ws, shift_out, dbg_F, dbg_Y, perm);
-  else
-    geometry_kernel<double2><<<grid, GEOM_THREADS, 0, s>>>(g, modes, b, params[0], params[1], params[2], params[3],
-                                                            params[4], params[5], U, V, ws, shift_out, dbg_F, dbg_Y, perm);
-  return cudaGetLastError();
+    return small ? launch_geometry_k<float2, 8>(g, modes, b, params, U, V, ws, shift_out, dbg_F, dbg_Y, perm, grid, s)
+                 : launch_geometry_k<float2, RIFT_MAX_MODES>(g, modes, b, params, U, V, ws, shift_out, dbg_F, dbg_Y, perm,
+                                                             grid, s);
+  return small ? launch_geometry_k<double2, 8>(g, modes, b, params, U, V, ws, shift_out, dbg_F, dbg_Y, perm, grid, s)
+               : launch_geometry_k<double2, RIFT_MAX_MODES>(g, modes, b, params, U, V, ws, shift_out, dbg_F, dbg_Y, perm,
+                                                            grid, s);
 }
