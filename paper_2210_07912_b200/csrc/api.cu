@@ -262,6 +262,8 @@ void make_tc_plan(rift_ile *h, double delta_t) {
   tp.M = h->M;
   tp.n_t = h->n_t;
   tp.nt = (h->n_t + 127) / 128;
+  tp.n_tau = h->n_tau;
+  tp.j0 = (h->n_t - h->n_tau) / 2;
   tp.kp = (6 * h->M + 15) & ~15;
   tp.nch = tp.kp / 8;
   tp.acols = tp.kp / 2;
@@ -280,7 +282,7 @@ void make_tc_plan(rift_ile *h, double delta_t) {
   tp.pitch = lnl_tc_pitch(tp.n_t, tp.H);
   tp.blob_words = tp.K * tp.nch * 64 + tp.K * 16 + 16;
   tp.dcol0 = tp.K * tp.nt * tp.acols;
-  const bool fits = h->precision == RIFT_PREC_MIXED && h->n_tau == h->n_t && tp.nt <= 4 && h->M <= 8 && h->K <= 5 &&
+  const bool fits = h->precision == RIFT_PREC_MIXED && tp.nt <= 4 && h->M <= 8 && h->K <= 5 &&
                     tp.K * tp.nt * (tp.acols + RIFT_TC_NB) <= 512 && tp.H < tp.n_t && tp.pitch > 0 &&
                     lnl_tc_smem_bytes(tp) <= 227u * 1024u;
   tp.ok = fits ? 1 : 0;

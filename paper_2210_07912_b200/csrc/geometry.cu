@@ -288,7 +288,7 @@ geometry_tc_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, Tc
 #pragma unroll
   for (int k = 0; k < K; ++k) {
     if (shift_out) shift_out[gi * K + k] = shift[k];
-    dsh[k * 16 + n] = shift[k] - shift[0];
+    dsh[k * 16 + n] = (k == 0) ? tp.j0 + shift[0] : shift[k] - shift[0];
     // a5: B = F_k Y_lm, scaled, split into fp16 hi + lo; kappa = 2a (Re), 2a+1 (Im).  The contraction index runs over
     // [hi | hi | lo] facing the A operand's [Q_hi | Q_lo | Q_hi].
     uint16_t hv[KP];

@@ -9,7 +9,8 @@
 // Q' = [Q_hi | Q_lo | Q_hi] (kp elements) lives in TENSOR MEMORY for the whole intrinsic point, the B operand
 // B' = [B_hi | B_hi | B_lo] comes from shared memory (bulk-copied batch blobs written by the geometry kernel),
 // accumulators P_k (K detectors x nt row tiles x 16 columns) are in TMEM.  In circular mode (N_tau = N_t) the time
-// marginal is invariant under a common rotation, so with t = (j + s_0) mod N_t
+// marginal is invariant under a common rotation (in guard-band mode, N_tau < N_t, nothing wraps and rows outside the
+// window [j0 + s_0, j0 + s_0 + N_tau) are masked), so with t = (j0 + j + s_0) mod N_t
 //     x[t] = P_0[t] + sum_{k>=1} P_k[(t + d_k) mod N_t],     d_k = s_k - s_0  (|d_k| <= dmax_k, light travel time),
 // and the per-sample shift is applied by a shared-memory exchange: every epilogue thread owns TMEM lane = row t, writes
 // its P_k[t, n] (k >= 1) to Xb[k][n][t + H] (plus wrap-around duplicates inside the halo H) and reads back
@@ -135,7 +136,8 @@ __device__ __forceinline__ float treduce8(const float (&v)[8], int lane, Op op) 
 
 // NT = row tiles of 128 (ceil(n_t / 128)); PITCH = floats per exchange row (>= n_t + 2 H), compile-time so that the
 // exchange addresses are one register plus immediates.
-template <int NT, int PITCH>
+// GUARD = guard-band window (N_tau < N_t): rows outside the window are masked.
+template <int NT, int PITCH, bool GUARD>
 __global__ void __launch_bounds__(TC_THREADS, 1) lnl_tc_kernel(const TcArgs args) {
   const TcPlan &tp = args.tp;
   const TcChunk &ch = args.ch;
@@ -338,6 +340,16 @@ __global__ void __launch_bounds__(TC_THREADS, 1) lnl_tc_kernel(const TcArgs args
         const float *blob = blob_s + stage * tp.blob_words;
         const float *cl2s = blob + K * tp.nch * 64 + K * 16 + NH * wg;
         float m[NH];
+        if constexpr (GUARD) {                // guard-band window: rows outside [j0 + s_0, j0 + s_0 + n_tau) do not count
+          const int32_t *lo = reinterpret_cast<const int32_t *>(blob + K * tp.nch * 64) + NH * wg;
+#pragma unroll
+          for (int n = 0; n < NH; ++n) {
+            const int l0 = lo[n];
+#pragma unroll
+            for (int i = 0; i < NT; ++i)
+              if ((unsigned)(128 * i + T - l0) >= (unsigned)tp.n_tau) x[i][n] = -INFINITY;
+          }
+        }
 #pragma unroll
         for (int n = 0; n < NH; ++n) {
           if (!last_valid) x[NT - 1][n] = -INFINITY;
@@ -426,7 +438,7 @@ __global__ void lnl_tc_finalize_kernel(TcPlan tp, TcChunk ch, double *__restrict
   double sum = 0.0;
   for (int a = 0; a < 4; ++a)
     if (m[a] > -INFINITY) sum += s[a] * exp(c * (m[a] - mm));
-  lnL_out[seg * ch.n_per_seg + i] = c * mm + log(sum) - log((double)tp.n_t) - ch.quad[w];
+  lnL_out[seg * ch.n_per_seg + i] = c * mm + log(sum) - log((double)tp.n_tau) - ch.quad[w];
 }
 
 // Per point: max |Re Q|, |Im Q| over detectors, modes, time (bit pattern of the non-negative float, atomicMax)
@@ -496,9 +508,10 @@ template <int NT>
 cudaError_t launch_nt(const TcArgs &a, unsigned grid, size_t smem, cudaStream_t s) {
 #define RIFT_TC_CASE(P)                                                                                         \
   case P: {                                                                                                     \
-    cudaError_t e = cudaFuncSetAttribute(lnl_tc_kernel<NT, P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+    auto kern = (a.tp.n_tau < a.tp.n_t) ? lnl_tc_kernel<NT, P, true> : lnl_tc_kernel<NT, P, false>;             \
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);         \
     if (e != cudaSuccess) return e;                                                                             \
-    lnl_tc_kernel<NT, P><<<grid, TC_THREADS, smem, s>>>(a);                                                     \
+    kern<<<grid, TC_THREADS, smem, s>>>(a);                                                                     \
     return cudaGetLastError();                                                                                  \
   }
   switch (a.tp.pitch) {

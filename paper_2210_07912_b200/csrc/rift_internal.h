@@ -67,6 +67,7 @@ struct QStore {
 struct TcPlan {
   int32_t ok;                    // 1 if this handle can run the tensor-core kernel
   int32_t K, M, n_t, nt;         // nt = ceil(n_t / 128) row tiles
+  int32_t n_tau, j0;             // marginalisation samples and first window index (n_t - n_tau) / 2; n_tau == n_t: circular
   int32_t kp, nch, acols;        // contraction length (fp16 elements), 16-byte chunks per detector, TMEM columns of one A tile
   int32_t H, pitch;              // halo = max_k dmax[k]; exchange-row pitch in floats
   int32_t blob_words, dcol0;     // 32-bit words per batch blob; first accumulator column in TMEM

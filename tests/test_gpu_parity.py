@@ -225,6 +225,8 @@ def test_guard_band_window(torch, oracle, kernel):
     for prec, tol in ((rift.RIFT_PREC_FP64, None), (rift.RIFT_PREC_MIXED, TOL_MIXED_LNL)):
         h = create(rift, inp, prec, n_tau=n_tau)
         got = gpu_eval(torch, h, [0], 1500, params, K=cfg.n_det, kernel=kernel)[0].cpu().numpy()
+        assert ("lnl_tc" in rift.rift_ile_kernel_name(h)) == (
+            prec == rift.RIFT_PREC_MIXED and kernel in (rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_TC))
         if tol is None:
             assert np.max(rel_err(got, ref)) < TOL_FP64_REL
         else:
