@@ -28,6 +28,7 @@ struct rift_ile {
   float *tc_blob = nullptr;        // per-chunk workspace of the tensor-core path
   double *tc_c = nullptr, *tc_quad = nullptr;
   float2 *tc_part = nullptr;
+  float *tc_xacc = nullptr;        // window sums carried between mode-subset passes (n_sub > 1)
   int64_t tc_cap = 0;              // batches the workspace holds
   double *d_exp_tab = nullptr;     // [64] 2^(j/64) for the fp64 exponential of lnl_tile
   int tile_ok = 0, tile_pitch = 0; // fp64 register-tiled kernel (lnl_tile.cu) usable for this handle
@@ -159,6 +160,7 @@ void free_handle(rift_ile *h) {
   cudaFree(h->tc_c);
   cudaFree(h->tc_quad);
   cudaFree(h->tc_part);
+  cudaFree(h->tc_xacc);
   cudaFree(h->d_bucket);
   cudaFree(h->d_perm);
   cudaFree(h->d_hist);
@@ -264,7 +266,9 @@ void make_tc_plan(rift_ile *h, double delta_t) {
   tp.nt = (h->n_t + 127) / 128;
   tp.n_tau = h->n_tau;
   tp.j0 = (h->n_t - h->n_tau) / 2;
-  tp.kp = (6 * h->M + 15) & ~15;
+  tp.n_sub = (h->M + 7) / 8;                        // mode subsets of at most 8 modes, one pass of lnl_tc each
+  tp.m_sub = (h->M + tp.n_sub - 1) / tp.n_sub;
+  tp.kp = (6 * tp.m_sub + 15) & ~15;
   tp.nch = tp.kp / 8;
   tp.acols = tp.kp / 2;
   tp.H = 0;
@@ -282,7 +286,8 @@ void make_tc_plan(rift_ile *h, double delta_t) {
   tp.pitch = lnl_tc_pitch(tp.n_t, tp.H);
   tp.blob_words = tp.K * tp.nch * 64 + tp.K * 16 + 16;
   tp.dcol0 = tp.K * tp.nt * tp.acols;
-  const bool fits = h->precision == RIFT_PREC_MIXED && tp.nt <= 4 && h->M <= 8 && h->K <= 5 &&
+  const bool fits = h->precision == RIFT_PREC_MIXED && tp.nt <= 4 && h->M <= RIFT_MAX_MODES && h->K <= 5 &&
+                    (tp.n_sub == 1 || h->n_tau == h->n_t) &&
                     tp.K * tp.nt * (tp.acols + RIFT_TC_NB) <= 512 && tp.H < tp.n_t && tp.pitch > 0 &&
                     lnl_tc_smem_bytes(tp) <= 227u * 1024u;
   tp.ok = fits ? 1 : 0;
@@ -302,15 +307,18 @@ int ensure_tc_workspace(rift_ile *h, int64_t n_batches) {
   cudaFree(h->tc_c);
   cudaFree(h->tc_quad);
   cudaFree(h->tc_part);
+  cudaFree(h->tc_xacc);
   h->tc_blob = nullptr;
   h->tc_c = h->tc_quad = nullptr;
   h->tc_part = nullptr;
+  h->tc_xacc = nullptr;
   h->tc_cap = 0;
   const size_t slots = (size_t)n_batches * RIFT_TC_NB;
-  CU(h, cudaMalloc(&h->tc_blob, (size_t)n_batches * h->tc.blob_words * sizeof(float)));
+  CU(h, cudaMalloc(&h->tc_blob, (size_t)h->tc.n_sub * n_batches * h->tc.blob_words * sizeof(float)));
   CU(h, cudaMalloc(&h->tc_c, slots * sizeof(double)));
   CU(h, cudaMalloc(&h->tc_quad, slots * sizeof(double)));
   CU(h, cudaMalloc(&h->tc_part, slots * 4 * sizeof(float2)));
+  if (h->tc.n_sub > 1) CU(h, cudaMalloc(&h->tc_xacc, slots * (size_t)h->tc.nt * 128 * sizeof(float)));
   h->tc_cap = n_batches;
   return RIFT_OK;
 }
@@ -321,7 +329,7 @@ int run_chunks_tc(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *c
   const int64_t nbps = (n_per_seg + RIFT_TC_NB - 1) / RIFT_TC_NB;
   const int64_t total = (int64_t)n_seg * nbps;
   if (total == 0) return RIFT_OK;
-  const size_t per_batch = (size_t)h->tc.blob_words * 4 + (size_t)RIFT_TC_NB * (16 + 32);
+  const size_t per_batch = (size_t)h->tc.n_sub * h->tc.blob_words * 4 + (size_t)RIFT_TC_NB * (16 + 32);
   int64_t cap = (int64_t)((64u << 20) / per_batch);
   if (cap < 8 * (int64_t)h->n_sm) cap = 8 * (int64_t)h->n_sm;
   int rc = ensure_tc_workspace(h, total < cap ? total : cap);
@@ -338,6 +346,7 @@ int run_chunks_tc(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *c
     c.scale_c = h->tc_c;
     c.quad = h->tc_quad;
     c.part = h->tc_part;
+    c.xacc = h->tc_xacc;
     {
       ProfSpan ps(h, 0, s);
       CU(h, launch_geometry_tc(h->geom, h->d_modes, h->tc, c, params, h->d_U, h->d_V, shift_out, s));
@@ -346,11 +355,22 @@ int run_chunks_tc(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *c
     ++h->launches;
     int nl = 0;
     ProfSpan ps(h, 1, s);
-    CU(h, launch_lnl_tc(h->tc, h->d_Qtc, c, lnL_out, h->n_sm, s, &nl));
+    if (h->tc.n_sub == 1) {
+      CU(h, launch_lnl_tc(h->tc, h->d_Qtc, c, RIFT_TC_PASS_SINGLE, lnL_out, h->n_sm, s, &nl));
+    } else {
+      // one pass per mode subset: its own A operand and blobs, window sums handed on through tc_xacc
+      const size_t a_words = (size_t)h->P * h->K * h->tc.nt * 128 * h->tc.acols;
+      for (int sub = 0; sub < h->tc.n_sub; ++sub) {
+        TcChunk cs = c;
+        cs.blob = h->tc_blob + (size_t)sub * c.n_batches * h->tc.blob_words;
+        const int pass = sub == 0 ? RIFT_TC_PASS_FIRST : (sub == h->tc.n_sub - 1 ? RIFT_TC_PASS_LAST : RIFT_TC_PASS_MIDDLE);
+        CU(h, launch_lnl_tc(h->tc, h->d_Qtc + sub * a_words, cs, pass, lnL_out, h->n_sm, s, &nl));
+      }
+    }
     ps.end();
     h->launches += nl;
   }
-  h->kernel_name = "lnl_tc<f16x3>";
+  h->kernel_name = h->tc.n_sub == 1 ? "lnl_tc<f16x3>" : "lnl_tc<f16x3,passes>";
   return RIFT_OK;
 }
 
@@ -595,7 +615,7 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
     // A operand of the tensor-core path (tf32 hi | lo pieces), when the configuration fits tensor memory
     make_tc_plan(h, cfg->delta_t);
     if (e == cudaSuccess && h->tc.ok) {
-      const size_t words = (size_t)h->P * h->K * h->tc.nt * 128 * h->tc.acols;
+      const size_t words = (size_t)h->tc.n_sub * h->P * h->K * h->tc.nt * 128 * h->tc.acols;
       e = cudaMalloc(&h->d_Qtc, words * sizeof(uint32_t));
       if (e == cudaSuccess) e = cudaMalloc(&h->d_qscale, sizeof(float) * h->P);
       if (e == cudaSuccess) e = launch_convert_q_tc(src, h->d_Qtc, h->d_qscale, h->tc, h->P, 0);

@@ -321,6 +321,89 @@ geometry_tc_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, Tc
 }  // namespace
 
 namespace {
+// Tensor-core variant for more than 8 modes: the modes are split into tp.n_sub subsets of tp.m_sub (one pass of lnl_tc each)
+// and every batch gets one blob per subset, [sub][batch][blob_words], each with the subset's coefficient pieces in the
+// UMMA layout followed by the (identical) shifts and exponent scales.  Generic in M: the harmonics live in local memory and
+// the fp16 pieces are stored element by element.
+template <int KT>
+__global__ void __launch_bounds__(GEOM_THREADS)
+geometry_tcx_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, TcChunk ch, const double *__restrict__ p_ra,
+                    const double *__restrict__ p_dec, const double *__restrict__ p_psi, const double *__restrict__ p_iota,
+                    const double *__restrict__ p_phi, const double *__restrict__ p_dist, const double *__restrict__ U,
+                    const double *__restrict__ V, int32_t *__restrict__ shift_out) {
+  constexpr int K = KT;
+  const int M = g.n_modes, ms = tp.m_sub, nch = tp.nch;
+  const int64_t n_slots = ch.n_batches * RIFT_TC_NB;
+  const int64_t w = (int64_t)blockIdx.x * GEOM_THREADS + threadIdx.x;       // slot = local batch * 16 + n
+  if (w >= n_slots) return;
+  const int64_t lb = w / RIFT_TC_NB;
+  const int n = (int)(w % RIFT_TC_NB);
+  const int64_t gb = ch.gb0 + lb;
+  const int64_t seg = gb / ch.nbps;
+  const int64_t i = (gb % ch.nbps) * RIFT_TC_NB + n;
+  const bool valid = i < ch.n_per_seg;
+  const size_t sub_stride = (size_t)ch.n_batches * tp.blob_words;           // floats between the blobs of two subsets
+  float *blob0 = ch.blob + lb * tp.blob_words;
+  if (!valid) {
+    for (int sub = 0; sub < tp.n_sub; ++sub) {
+      float *blob = blob0 + sub * sub_stride;
+      uint4 *chunks = reinterpret_cast<uint4 *>(blob);
+      const uint4 z = make_uint4(0u, 0u, 0u, 0u);
+      for (int k = 0; k < K; ++k) {
+        for (int c = 0; c < nch; ++c) chunks[(k * nch + c) * 16 + n] = z;
+        reinterpret_cast<int32_t *>(blob + K * nch * 64)[k * 16 + n] = 0;
+      }
+      blob[K * nch * 64 + K * 16 + n] = 0.f;
+    }
+    ch.scale_c[w] = 0.0;
+    ch.quad[w] = 0.0;
+    return;
+  }
+  const int64_t gi = seg * ch.n_per_seg + i;
+  const int32_t point = ch.ids[seg];
+  const double2 *Up = reinterpret_cast<const double2 *>(U) + (int64_t)point * K * M * M;
+  const double2 *Vp = reinterpret_cast<const double2 *>(V) + (int64_t)point * K * M * M;
+  int32_t shift[KT];
+  double Fre[KT], Fim[KT], Yre[RIFT_MAX_MODES], Yim[RIFT_MAX_MODES], c, q;
+  sample_geometry<RIFT_MAX_MODES, KT>(g, modes, p_ra[gi], p_dec[gi], p_psi[gi], p_iota[gi], p_phi[gi], p_dist[gi], Up, Vp,
+                                      shift, Fre, Fim, Yre, Yim, c, q);
+  ch.scale_c[w] = c;
+  ch.quad[w] = q;
+  const float cl2v = (float)(c * 1.4426950408889634 / ((double)ch.qscale[point] * RIFT_TC_BSCALE));
+  if (shift_out)
+    for (int k = 0; k < K; ++k) shift_out[gi * K + k] = shift[k];
+  for (int sub = 0; sub < tp.n_sub; ++sub) {
+    float *blob = blob0 + sub * sub_stride;
+    int32_t *dsh = reinterpret_cast<int32_t *>(blob + K * nch * 64);
+    blob[K * nch * 64 + K * 16 + n] = cl2v;
+    for (int k = 0; k < K; ++k) {
+      dsh[k * 16 + n] = (k == 0) ? tp.j0 + shift[0] : shift[k] - shift[0];
+      // element e of the contraction index lives in chunk e / 8 of this sample: halfs [(k nch + e/8) 16 + n] 8 + e % 8
+      uint16_t *hp = reinterpret_cast<uint16_t *>(blob) + ((size_t)(k * nch) * 16 + n) * 8;
+      auto put = [&](int e, uint16_t v) { hp[(size_t)(e >> 3) * 128 + (e & 7)] = v; };
+      for (int al = 0; al < ms; ++al) {
+        const int a = sub * ms + al;
+        double vr = 0.0, vi = 0.0;
+        if (a < M) {
+          vr = (Fre[k] * Yre[a] - Fim[k] * Yim[a]) * RIFT_TC_BSCALE;
+          vi = (Fre[k] * Yim[a] + Fim[k] * Yre[a]) * RIFT_TC_BSCALE;
+        }
+        const __half hr = __double2half(vr), hi = __double2half(vi);
+        const __half lr = __double2half(vr - (double)__half2float(hr)), li = __double2half(vi - (double)__half2float(hi));
+        put(2 * al, __half_as_ushort(hr));
+        put(2 * al + 1, __half_as_ushort(hi));
+        put(2 * ms + 2 * al, __half_as_ushort(hr));
+        put(2 * ms + 2 * al + 1, __half_as_ushort(hi));
+        put(4 * ms + 2 * al, __half_as_ushort(lr));
+        put(4 * ms + 2 * al + 1, __half_as_ushort(li));
+      }
+      for (int e = 6 * ms; e < tp.kp; ++e) put(e, 0);
+    }
+  }
+}
+}  // namespace
+
+namespace {
 template <int MT>
 cudaError_t launch_geometry_tc_m(const DetGeom &g, const ModeEntry *modes, const TcPlan &tp, const TcChunk &c,
                                  const double *const params[6], const double *U, const double *V, int32_t *shift_out,
@@ -345,6 +428,19 @@ cudaError_t launch_geometry_tc(const DetGeom &g, const ModeEntry *modes, const T
   const int64_t n = c.n_batches * RIFT_TC_NB;
   if (n <= 0) return cudaSuccess;
   const unsigned grid = (unsigned)((n + GEOM_THREADS - 1) / GEOM_THREADS);
+  if (tp.n_sub > 1) {
+#define RIFT_GEOM_TCX(KT)                                                                                                \
+  case KT:                                                                                                               \
+    geometry_tcx_kernel<KT><<<grid, GEOM_THREADS, 0, s>>>(g, modes, tp, c, params[0], params[1], params[2], params[3],    \
+                                                           params[4], params[5], U, V, shift_out);                       \
+    break;
+    switch (tp.K) {
+      RIFT_GEOM_TCX(1) RIFT_GEOM_TCX(2) RIFT_GEOM_TCX(3) RIFT_GEOM_TCX(4) RIFT_GEOM_TCX(5)
+      default: return cudaErrorInvalidValue;
+    }
+#undef RIFT_GEOM_TCX
+    return cudaGetLastError();
+  }
   switch (tp.M) {
     case 1: return launch_geometry_tc_m<1>(g, modes, tp, c, params, U, V, shift_out, grid, s);
     case 2: return launch_geometry_tc_m<2>(g, modes, tp, c, params, U, V, shift_out, grid, s);

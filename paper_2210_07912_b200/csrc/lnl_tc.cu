@@ -136,8 +136,10 @@ __device__ __forceinline__ float treduce8(const float (&v)[8], int lane, Op op) 
 
 // NT = row tiles of 128 (ceil(n_t / 128)); PITCH = floats per exchange row (>= n_t + 2 H), compile-time so that the
 // exchange addresses are one register plus immediates.
-// GUARD = guard-band window (N_tau < N_t): rows outside the window are masked.
-template <int NT, int PITCH, bool GUARD>
+// GUARD = guard-band window (N_tau < N_t): rows outside the window are masked.  PASS = RIFT_TC_PASS_*: with the modes split
+// into subsets, every pass but the last writes its window sums x[t, n] to global memory instead of reducing them, every
+// pass but the first adds the sums of the pass before.
+template <int NT, int PITCH, bool GUARD, int PASS>
 __global__ void __launch_bounds__(TC_THREADS, 1) lnl_tc_kernel(const TcArgs args) {
   const TcPlan &tp = args.tp;
   const TcChunk &ch = args.ch;
@@ -317,7 +319,15 @@ __global__ void __launch_bounds__(TC_THREADS, 1) lnl_tc_kernel(const TcArgs args
         if (lane == 0) mbar_arrive(bar_tempty);                            // the UMMAs of the next batch may overwrite D
       };
       // Phase B: shifted sum over detectors
-      auto phase_b = [&](uint32_t g, float (&x)[NT][NH]) {
+      auto phase_b = [&](uint32_t g, int64_t lb, float (&x)[NT][NH]) {
+        float xp[NT][NH];
+        if constexpr (PASS == RIFT_TC_PASS_MIDDLE || PASS == RIFT_TC_PASS_LAST) {   // in flight under the exchange reads
+          const float *src = ch.xacc + ((size_t)(lb * RIFT_TC_NB + NH * wg)) * (NT * 128) + T;
+#pragma unroll
+          for (int n = 0; n < NH; ++n)
+#pragma unroll
+            for (int i = 0; i < NT; ++i) xp[i][n] = __ldcs(src + (size_t)n * (NT * 128) + 128 * i);
+        }
         const float *blob = blob_s + (g % TC_STAGES) * tp.blob_words;
         const float *xb = xb_s + (size_t)((wg * 2 + (g & 1u)) * (K - 1)) * NH * PITCH;
         const int32_t *dsh = reinterpret_cast<const int32_t *>(blob + K * tp.nch * 64) + NH * wg;
@@ -333,9 +343,25 @@ __global__ void __launch_bounds__(TC_THREADS, 1) lnl_tc_kernel(const TcArgs args
             x[NT - 1][n] += src[128 * (NT - 1) + last_clamp];
           }
         }
+        if constexpr (PASS == RIFT_TC_PASS_MIDDLE || PASS == RIFT_TC_PASS_LAST) {
+#pragma unroll
+          for (int n = 0; n < NH; ++n)
+#pragma unroll
+            for (int i = 0; i < NT; ++i) x[i][n] += xp[i][n];
+        }
       };
       // per-warp (reference, sum) of the time marginal for the 8 samples of batch g (chunk-local batch index lb)
       auto reduce = [&](uint32_t g, int64_t lb, float (&x)[NT][NH]) {
+        if constexpr (PASS == RIFT_TC_PASS_FIRST || PASS == RIFT_TC_PASS_MIDDLE) {   // hand the window sums to the next pass
+          float *dst = ch.xacc + ((size_t)(lb * RIFT_TC_NB + NH * wg)) * (NT * 128) + T;
+#pragma unroll
+          for (int n = 0; n < NH; ++n)
+#pragma unroll
+            for (int i = 0; i < NT; ++i) __stcs(dst + (size_t)n * (NT * 128) + 128 * i, x[i][n]);
+          __syncwarp();
+          if (lane == 0) mbar_arrive(bar_empty + g % TC_STAGES);
+          return;
+        }
         const uint32_t stage = g % TC_STAGES;
         const float *blob = blob_s + stage * tp.blob_words;
         const float *cl2s = blob + K * tp.nch * 64 + K * 16 + NH * wg;
@@ -395,7 +421,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) lnl_tc_kernel(const TcArgs args
         const uint32_t g = it + j;
         named_bar_sync(1 + wg, 128);                                       // exchange rows of batch g are complete
         mbar_wait(bar_full + g % TC_STAGES, (g / TC_STAGES) & 1u);         // shifts and exponent scales of batch g
-        phase_b(g, x);
+        phase_b(g, b0 + j, x);
         if (j + 1 < nb) {
           mbar_wait(bar_tfull, (g + 1u) & 1u);
           tc_fence_after();
@@ -462,7 +488,8 @@ __global__ void q_scale_kernel(const uint32_t *mx, float *scale, int n_points) {
 // Q [P][K][M][n_t] complex128  ->  A operand [P][K][nt*128][acols] words of two fp16: contraction index kappa' over
 // [Q_hi | Q_lo | Q_hi] (each 2M elements, Re/Im interleaved), zero padding up to kp; rows >= n_t are zero.
 __global__ void convert_q_tc_kernel(const double2 *__restrict__ src, uint32_t *__restrict__ dst, const float *__restrict__ scale,
-                                    TcPlan tp, int64_t total) {
+                                    TcPlan tp, int sub, int64_t total) {
+  const int ms = tp.m_sub, a0 = sub * tp.m_sub;                            // modes [a0, a0 + ms) of this subset
   for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
     const int col = (int)(idx % tp.acols);
     const int64_t r = idx / tp.acols;
@@ -474,9 +501,10 @@ __global__ void convert_q_tc_kernel(const double2 *__restrict__ src, uint32_t *_
     if (t < tp.n_t) {
       for (int hlf = 0; hlf < 2; ++hlf) {
         const int kp_i = 2 * col + hlf;
-        const int part = kp_i / (2 * tp.M), kap = kp_i % (2 * tp.M);
-        if (part < 3) {
-          const double2 qv = src[(pk * tp.M + (kap >> 1)) * tp.n_t + t];
+        const int part = kp_i / (2 * ms), kap = kp_i % (2 * ms);
+        const int a = a0 + (kap >> 1);
+        if (part < 3 && a < tp.M) {
+          const double2 qv = src[(pk * tp.M + a) * tp.n_t + t];
           const double x = ((kap & 1) ? qv.y : qv.x) * sc;
           const __half hi = __double2half(x);
           const __half out = (part == 1) ? __double2half(x - (double)__half2float(hi)) : hi;
@@ -505,14 +533,23 @@ int lnl_tc_pitch(int n_t, int halo) {
 
 namespace {
 template <int NT>
-cudaError_t launch_nt(const TcArgs &a, unsigned grid, size_t smem, cudaStream_t s) {
-#define RIFT_TC_CASE(P)                                                                                         \
-  case P: {                                                                                                     \
-    auto kern = (a.tp.n_tau < a.tp.n_t) ? lnl_tc_kernel<NT, P, true> : lnl_tc_kernel<NT, P, false>;             \
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);         \
-    if (e != cudaSuccess) return e;                                                                             \
-    kern<<<grid, TC_THREADS, smem, s>>>(a);                                                                     \
-    return cudaGetLastError();                                                                                  \
+cudaError_t launch_nt(const TcArgs &a, int pass, unsigned grid, size_t smem, cudaStream_t s) {
+#define RIFT_TC_CASE(P)                                                                                          \
+  case P: {                                                                                                      \
+    void (*kern)(TcArgs) = nullptr;                                                                              \
+    if (a.tp.n_tau < a.tp.n_t) {                                                                                 \
+      if (pass != RIFT_TC_PASS_SINGLE) return cudaErrorInvalidValue;                                             \
+      kern = lnl_tc_kernel<NT, P, true, RIFT_TC_PASS_SINGLE>;                                                    \
+    } else {                                                                                                     \
+      kern = pass == RIFT_TC_PASS_SINGLE  ? lnl_tc_kernel<NT, P, false, RIFT_TC_PASS_SINGLE>                     \
+             : pass == RIFT_TC_PASS_FIRST ? lnl_tc_kernel<NT, P, false, RIFT_TC_PASS_FIRST>                      \
+             : pass == RIFT_TC_PASS_MIDDLE ? lnl_tc_kernel<NT, P, false, RIFT_TC_PASS_MIDDLE>                    \
+                                           : lnl_tc_kernel<NT, P, false, RIFT_TC_PASS_LAST>;                     \
+    }                                                                                                            \
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);          \
+    if (e != cudaSuccess) return e;                                                                              \
+    kern<<<grid, TC_THREADS, smem, s>>>(a);                                                                      \
+    return cudaGetLastError();                                                                                   \
   }
   switch (a.tp.pitch) {
     RIFT_TC_CASE(256)
@@ -540,11 +577,13 @@ cudaError_t launch_convert_q_tc(const double *Q_c128, uint32_t *dst, float *qsca
   q_scale_kernel<<<(n_points + 127) / 128, 128, 0, s>>>(reinterpret_cast<const uint32_t *>(qscale), qscale, n_points);
   grid = (total + 255) / 256;
   if (grid > 148 * 32) grid = 148 * 32;
-  convert_q_tc_kernel<<<(unsigned)grid, 256, 0, s>>>(reinterpret_cast<const double2 *>(Q_c128), dst, qscale, tp, total);
+  for (int sub = 0; sub < tp.n_sub; ++sub)
+    convert_q_tc_kernel<<<(unsigned)grid, 256, 0, s>>>(reinterpret_cast<const double2 *>(Q_c128), dst + (size_t)sub * total,
+                                                       qscale, tp, sub, total);
   return cudaGetLastError();
 }
 
-cudaError_t launch_lnl_tc(const TcPlan &tp, const uint32_t *qtc, const TcChunk &c, double *lnL_out, int n_sm,
+cudaError_t launch_lnl_tc(const TcPlan &tp, const uint32_t *qtc, const TcChunk &c, int pass, double *lnL_out, int n_sm,
                           cudaStream_t s, int *n_launch) {
   if (c.n_batches <= 0) return cudaSuccess;
   const size_t smem = lnl_tc_smem_bytes(tp);
@@ -556,15 +595,17 @@ cudaError_t launch_lnl_tc(const TcPlan &tp, const uint32_t *qtc, const TcChunk &
   int64_t grid = n_sm;
   if (grid > c.n_batches) grid = c.n_batches;
   switch (tp.nt) {
-    case 1: e = launch_nt<1>(a, (unsigned)grid, smem, s); break;
-    case 2: e = launch_nt<2>(a, (unsigned)grid, smem, s); break;
-    case 3: e = launch_nt<3>(a, (unsigned)grid, smem, s); break;
-    case 4: e = launch_nt<4>(a, (unsigned)grid, smem, s); break;
+    case 1: e = launch_nt<1>(a, pass, (unsigned)grid, smem, s); break;
+    case 2: e = launch_nt<2>(a, pass, (unsigned)grid, smem, s); break;
+    case 3: e = launch_nt<3>(a, pass, (unsigned)grid, smem, s); break;
+    case 4: e = launch_nt<4>(a, pass, (unsigned)grid, smem, s); break;
     default: e = cudaErrorInvalidValue;
   }
   if (e != cudaSuccess) return e;
+  if (n_launch) ++*n_launch;
+  if (pass == RIFT_TC_PASS_FIRST || pass == RIFT_TC_PASS_MIDDLE) return cudaSuccess;   // lnL is assembled after the last pass
   const int64_t n = c.n_batches * RIFT_TC_NB;
   lnl_tc_finalize_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(tp, c, lnL_out);
-  if (n_launch) *n_launch += 2;
+  if (n_launch) ++*n_launch;
   return cudaGetLastError();
 }

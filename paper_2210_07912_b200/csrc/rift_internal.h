@@ -67,6 +67,7 @@ struct QStore {
 struct TcPlan {
   int32_t ok;                    // 1 if this handle can run the tensor-core kernel
   int32_t K, M, n_t, nt;         // nt = ceil(n_t / 128) row tiles
+  int32_t n_sub, m_sub;          // mode subsets (passes) and modes per subset; kp, nch, acols refer to ONE subset
   int32_t n_tau, j0;             // marginalisation samples and first window index (n_t - n_tau) / 2; n_tau == n_t: circular
   int32_t kp, nch, acols;        // contraction length (fp16 elements), 16-byte chunks per detector, TMEM columns of one A tile
   int32_t H, pitch;              // halo = max_k dmax[k]; exchange-row pitch in floats
@@ -80,7 +81,11 @@ struct TcChunk {                 // a chunk = global batches [gb0, gb0 + n_batch
   float *blob;                   // [n_batches][blob_words]
   double *scale_c, *quad;        // [n_batches * 16]
   float2 *part;                  // [n_batches * 16][4]: per lane-quarter (reference, sum)
+  float *xacc;                   // [n_batches * 16][nt * 128]: window sums carried between mode-subset passes (or NULL)
 };
+// Mode-subset passes of lnl_tc (configurations whose A operand does not fit tensor memory whole, e.g. 21 modes): the modes are
+// split into n_sub subsets of m_sub; pass s contracts subset s and adds the window sums of the passes before it.
+enum { RIFT_TC_PASS_SINGLE = 0, RIFT_TC_PASS_FIRST = 1, RIFT_TC_PASS_MIDDLE = 2, RIFT_TC_PASS_LAST = 3 };
 
 // geometry.cu
 cudaError_t launch_geometry_tc(const DetGeom &g, const ModeEntry *modes, const TcPlan &tp, const TcChunk &c,
@@ -117,8 +122,8 @@ cudaError_t launch_lnl_quad(const QStore &q, bool fp32, const Batch &b, const Wo
 size_t lnl_tc_smem_bytes(const TcPlan &tp);
 int lnl_tc_pitch(int n_t, int halo);   // exchange-row pitch (floats) the kernel is instantiated for, 0 = none fits
 cudaError_t launch_convert_q_tc(const double *Q_c128, uint32_t *dst, float *qscale, const TcPlan &tp, int32_t n_points,
-                                cudaStream_t s);
-cudaError_t launch_lnl_tc(const TcPlan &tp, const uint32_t *qtc, const TcChunk &c, double *lnL_out, int n_sm,
+                                cudaStream_t s);   // dst: [n_sub][P][K][nt*128][acols]
+cudaError_t launch_lnl_tc(const TcPlan &tp, const uint32_t *qtc, const TcChunk &c, int pass, double *lnL_out, int n_sm,
                           cudaStream_t s, int *n_launch);
 // lnl_tile.cu (fp64 register-tiled contraction + shared-memory exchange; circular mode, n_t <= 512)
 size_t lnl_tile_smem_bytes(const QStore &q, int K, int pitch);
