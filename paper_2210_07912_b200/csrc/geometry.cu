@@ -323,18 +323,33 @@ geometry_tc_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, Tc
 namespace {
 // Tensor-core variant for more than 8 modes: the modes are split into tp.n_sub subsets of tp.m_sub (one pass of lnl_tc each)
 // and every batch gets one blob per subset, [sub][batch][blob_words], each with the subset's coefficient pieces in the
-// UMMA layout followed by the (identical) shifts and exponent scales.  Generic in M: the harmonics live in local memory and
-// the fp16 pieces are stored element by element.
-template <int KT>
+// UMMA layout followed by the (identical) shifts and exponent scales.  Generic in M (the harmonics live in local memory);
+// MS = modes per subset (compile time, so that the operand chunks are assembled in registers).
+template <int KT, int MS>
 __global__ void __launch_bounds__(GEOM_THREADS)
 geometry_tcx_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, TcChunk ch, const double *__restrict__ p_ra,
                     const double *__restrict__ p_dec, const double *__restrict__ p_psi, const double *__restrict__ p_iota,
                     const double *__restrict__ p_phi, const double *__restrict__ p_dist, const double *__restrict__ U,
-                    const double *__restrict__ V, int32_t *__restrict__ shift_out) {
+                    const double *__restrict__ V, int32_t *__restrict__ shift_out, int stage_uv) {
   constexpr int K = KT;
-  const int M = g.n_modes, ms = tp.m_sub, nch = tp.nch;
+  constexpr int KP = (6 * MS + 15) & ~15, nch = KP / 8;
+  const int M = g.n_modes;
   const int64_t n_slots = ch.n_batches * RIFT_TC_NB;
-  const int64_t w = (int64_t)blockIdx.x * GEOM_THREADS + threadIdx.x;       // slot = local batch * 16 + n
+  // U, V of the block's (first) intrinsic point staged in shared memory when the launch provides room for them
+  extern __shared__ double2 s_uv[];
+  const int64_t w0 = (int64_t)blockIdx.x * GEOM_THREADS;
+  const int32_t point0 = ch.ids[(ch.gb0 + w0 / RIFT_TC_NB) / ch.nbps];
+  const int n_uv = K * M * M;
+  if (stage_uv) {
+    const double2 *u = reinterpret_cast<const double2 *>(U) + (int64_t)point0 * n_uv;
+    const double2 *v = reinterpret_cast<const double2 *>(V) + (int64_t)point0 * n_uv;
+    for (int i = threadIdx.x; i < n_uv; i += GEOM_THREADS) {
+      s_uv[i] = u[i];
+      s_uv[n_uv + i] = v[i];
+    }
+    __syncthreads();
+  }
+  const int64_t w = w0 + threadIdx.x;                                       // slot = local batch * 16 + n
   if (w >= n_slots) return;
   const int64_t lb = w / RIFT_TC_NB;
   const int n = (int)(w % RIFT_TC_NB);
@@ -361,8 +376,12 @@ geometry_tcx_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, T
   }
   const int64_t gi = seg * ch.n_per_seg + i;
   const int32_t point = ch.ids[seg];
-  const double2 *Up = reinterpret_cast<const double2 *>(U) + (int64_t)point * K * M * M;
-  const double2 *Vp = reinterpret_cast<const double2 *>(V) + (int64_t)point * K * M * M;
+  const double2 *Up = reinterpret_cast<const double2 *>(U) + (int64_t)point * n_uv;
+  const double2 *Vp = reinterpret_cast<const double2 *>(V) + (int64_t)point * n_uv;
+  if (stage_uv && point == point0) {
+    Up = s_uv;
+    Vp = s_uv + n_uv;
+  }
   int32_t shift[KT];
   double Fre[KT], Fim[KT], Yre[RIFT_MAX_MODES], Yim[RIFT_MAX_MODES], c, q;
   sample_geometry<RIFT_MAX_MODES, KT>(g, modes, p_ra[gi], p_dec[gi], p_psi[gi], p_iota[gi], p_phi[gi], p_dist[gi], Up, Vp,
@@ -378,11 +397,12 @@ geometry_tcx_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, T
     blob[K * nch * 64 + K * 16 + n] = cl2v;
     for (int k = 0; k < K; ++k) {
       dsh[k * 16 + n] = (k == 0) ? tp.j0 + shift[0] : shift[k] - shift[0];
-      // element e of the contraction index lives in chunk e / 8 of this sample: halfs [(k nch + e/8) 16 + n] 8 + e % 8
-      uint16_t *hp = reinterpret_cast<uint16_t *>(blob) + ((size_t)(k * nch) * 16 + n) * 8;
-      auto put = [&](int e, uint16_t v) { hp[(size_t)(e >> 3) * 128 + (e & 7)] = v; };
-      for (int al = 0; al < ms; ++al) {
-        const int a = sub * ms + al;
+      uint16_t hv[KP];
+#pragma unroll
+      for (int e = 6 * MS; e < KP; ++e) hv[e] = 0;
+#pragma unroll
+      for (int al = 0; al < MS; ++al) {
+        const int a = sub * MS + al;
         double vr = 0.0, vi = 0.0;
         if (a < M) {
           vr = (Fre[k] * Yre[a] - Fim[k] * Yim[a]) * RIFT_TC_BSCALE;
@@ -390,14 +410,21 @@ geometry_tcx_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, T
         }
         const __half hr = __double2half(vr), hi = __double2half(vi);
         const __half lr = __double2half(vr - (double)__half2float(hr)), li = __double2half(vi - (double)__half2float(hi));
-        put(2 * al, __half_as_ushort(hr));
-        put(2 * al + 1, __half_as_ushort(hi));
-        put(2 * ms + 2 * al, __half_as_ushort(hr));
-        put(2 * ms + 2 * al + 1, __half_as_ushort(hi));
-        put(4 * ms + 2 * al, __half_as_ushort(lr));
-        put(4 * ms + 2 * al + 1, __half_as_ushort(li));
+        hv[2 * al] = hv[2 * MS + 2 * al] = __half_as_ushort(hr);
+        hv[2 * al + 1] = hv[2 * MS + 2 * al + 1] = __half_as_ushort(hi);
+        hv[4 * MS + 2 * al] = __half_as_ushort(lr);
+        hv[4 * MS + 2 * al + 1] = __half_as_ushort(li);
       }
-      for (int e = 6 * ms; e < tp.kp; ++e) put(e, 0);
+      uint4 *dst = reinterpret_cast<uint4 *>(blob) + (k * nch) * 16 + n;
+#pragma unroll
+      for (int cc = 0; cc < nch; ++cc) {
+        uint4 v;
+        v.x = (uint32_t)hv[8 * cc + 0] | ((uint32_t)hv[8 * cc + 1] << 16);
+        v.y = (uint32_t)hv[8 * cc + 2] | ((uint32_t)hv[8 * cc + 3] << 16);
+        v.z = (uint32_t)hv[8 * cc + 4] | ((uint32_t)hv[8 * cc + 5] << 16);
+        v.w = (uint32_t)hv[8 * cc + 6] | ((uint32_t)hv[8 * cc + 7] << 16);
+        dst[cc * 16] = v;
+      }
     }
   }
 }
@@ -429,15 +456,32 @@ cudaError_t launch_geometry_tc(const DetGeom &g, const ModeEntry *modes, const T
   if (n <= 0) return cudaSuccess;
   const unsigned grid = (unsigned)((n + GEOM_THREADS - 1) / GEOM_THREADS);
   if (tp.n_sub > 1) {
+    const size_t uv_bytes = (size_t)2 * tp.K * tp.M * tp.M * sizeof(double2);
+    const int stage_uv = uv_bytes <= 96u * 1024u ? 1 : 0;                    // else U, V are read through L1
+    const size_t smem = stage_uv ? uv_bytes : 0;
+#define RIFT_GEOM_TCX_MS(KT, MS)                                                                                         \
+  case MS: {                                                                                                             \
+    auto kern = geometry_tcx_kernel<KT, MS>;                                                                             \
+    if (smem > 48u * 1024u) {                                                                                            \
+      cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                \
+      if (e != cudaSuccess) return e;                                                                                    \
+    }                                                                                                                    \
+    kern<<<grid, GEOM_THREADS, smem, s>>>(g, modes, tp, c, params[0], params[1], params[2], params[3], params[4],        \
+                                          params[5], U, V, shift_out, stage_uv);                                         \
+    break;                                                                                                               \
+  }
 #define RIFT_GEOM_TCX(KT)                                                                                                \
   case KT:                                                                                                               \
-    geometry_tcx_kernel<KT><<<grid, GEOM_THREADS, 0, s>>>(g, modes, tp, c, params[0], params[1], params[2], params[3],    \
-                                                           params[4], params[5], U, V, shift_out);                       \
+    switch (tp.m_sub) {                                                                                                  \
+      RIFT_GEOM_TCX_MS(KT, 5) RIFT_GEOM_TCX_MS(KT, 6) RIFT_GEOM_TCX_MS(KT, 7) RIFT_GEOM_TCX_MS(KT, 8)                    \
+      default: return cudaErrorInvalidValue;                                                                             \
+    }                                                                                                                    \
     break;
     switch (tp.K) {
       RIFT_GEOM_TCX(1) RIFT_GEOM_TCX(2) RIFT_GEOM_TCX(3) RIFT_GEOM_TCX(4) RIFT_GEOM_TCX(5)
       default: return cudaErrorInvalidValue;
     }
+#undef RIFT_GEOM_TCX_MS
 #undef RIFT_GEOM_TCX
     return cudaGetLastError();
   }
