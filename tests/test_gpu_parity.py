@@ -214,6 +214,37 @@ def test_tc_edge_sizes_ragged_batches_and_invalid_samples(torch, oracle):
     rift.rift_ile_destroy(h)
 
 
+_L2 = tuple((2, m) for m in range(-2, 3))
+_L3 = tuple((3, m) for m in range(-3, 4))
+TC_SHAPES = [
+    # detectors, modes, f_s, window -> (row tiles, passes) of the tensor-core kernel
+    (("H1",), _L2[:3], 1024.0, 0.04),                                # K=1, 3 modes, N_t=83: one row tile, no exchange
+    (("H1", "L1"), _L2 + _L3, 4096.0, 0.05),                         # K=2, 12 modes: two passes of 6
+    (("H1", "L1", "V1"), _L2 + _L3[1:5], 2048.0, 0.05),              # K=3, 9 modes, N_t=205: two row tiles, two passes
+    (("H1", "L1", "V1", "S0"), _L2[1:4], 2048.0, 0.08),              # K=4, 3 modes, N_t=329: three row tiles
+    (("H1", "L1", "V1", "S0", "S1"), ((2, 2), (2, -2)), 512.0, 0.2),    # K=5, 2 modes, N_t=205 at 512 Hz (small halo)
+]
+
+
+@pytest.mark.parametrize("shape", range(len(TC_SHAPES)))
+def test_tc_kernel_shapes(torch, oracle, shape):
+    """Detector counts, mode counts (one or several mode-subset passes) and window lengths other than C0-C3's: every
+    (row tiles, pitch, pass) instantiation the plan can pick is compared with the oracle."""
+    dets, modes, f_s, t_w = TC_SHAPES[shape]
+    cfg = synth.with_overrides(synth.CONFIGS[1], detectors=dets, modes=modes, f_s=f_s, t_window=t_w, n_points=2)
+    inp = build(oracle, cfg, n_points=2)
+    n = 333
+    ids = [1, 0]
+    params = np.concatenate([synth.draw_samples(cfg, 40 + s, n)[0] for s in range(len(ids))], axis=1)
+    ref = np.concatenate([oracle_eval(oracle, inp, ids[s], params[:, s * n:(s + 1) * n])[0] for s in range(len(ids))])
+    h = create(rift, inp, rift.RIFT_PREC_MIXED)
+    got, sh, _ = gpu_eval(torch, h, ids, n, params, K=cfg.n_det, kernel=rift.RIFT_KERNEL_TC)
+    assert "lnl_tc" in rift.rift_ile_kernel_name(h), rift.rift_ile_kernel_name(h)
+    assert ("passes" in rift.rift_ile_kernel_name(h)) == (len(modes) > 8)
+    assert np.max(np.abs(got.cpu().numpy() - ref)) < TOL_MIXED_LNL
+    rift.rift_ile_destroy(h)
+
+
 @pytest.mark.parametrize("kernel", KERNELS)
 def test_guard_band_window(torch, oracle, kernel):
     """n_tau < n_t (reading A4): the physical mode in which the circular wrap never triggers."""
