@@ -27,6 +27,8 @@ EXPORTS = ("rift_ile_create", "rift_ile_eval_batch", "rift_ile_reduce", "rift_il
            "rift_ile_launch_count", "rift_ile_kernel_name", "rift_ile_profile", "rift_ile_profile_read",
            "rift_ile_fma_peak", "rift_ile_destroy",
            "rift_ile_strerror", "rift_ile_last_error")
+AC_EXPORTS = ("rift_ac_create", "rift_ac_draw", "rift_ac_update", "rift_ac_get_masses", "rift_ac_ile_ln_weight",
+              "rift_ac_destroy")
 
 
 class RiftError(RuntimeError):
@@ -77,6 +79,19 @@ def lib() -> C.CDLL:
         L.rift_ile_fma_peak.restype = C.c_int
         L.rift_ile_destroy.argtypes = [vp]
         L.rift_ile_destroy.restype = C.c_int
+        # include/rift_ac.h
+        L.rift_ac_create.argtypes = [i32, i32, vp, vp, C.POINTER(vp)]
+        L.rift_ac_create.restype = C.c_int
+        L.rift_ac_draw.argtypes = [vp, i64, C.c_uint64, C.c_uint64, C.POINTER(vp), vp, vp]
+        L.rift_ac_draw.restype = C.c_int
+        L.rift_ac_update.argtypes = [vp, vp, dbl, dbl]
+        L.rift_ac_update.restype = C.c_int
+        L.rift_ac_get_masses.argtypes = [vp, vp]
+        L.rift_ac_get_masses.restype = C.c_int
+        L.rift_ac_ile_ln_weight.argtypes = [i64, C.POINTER(vp), dbl, dbl, vp, vp, vp]
+        L.rift_ac_ile_ln_weight.restype = C.c_int
+        L.rift_ac_destroy.argtypes = [vp]
+        L.rift_ac_destroy.restype = C.c_int
         L.rift_ile_strerror.argtypes = [C.c_int]
         L.rift_ile_strerror.restype = C.c_char_p
         L.rift_ile_last_error.argtypes = [vp]
@@ -215,3 +230,43 @@ def rift_ile_fma_peak(fp64: bool, iters: int = 4096, cuda_stream: int = 0) -> fl
     v = C.c_double()
     _check(lib().rift_ile_fma_peak(int(fp64), int(iters), C.byref(v), int(cuda_stream) or None))
     return float(v.value)
+
+
+# ---------------------------------------------------------------------------------------------- include/rift_ac.h
+def rift_ac_create(n_dim: int, n_bins: int, lo, hi):
+    """Adaptive-cartesian sampler handle (uniform bin masses).  lo, hi: host sequences of length n_dim."""
+    lo_ = np.ascontiguousarray(lo, dtype=np.float64)
+    hi_ = np.ascontiguousarray(hi, dtype=np.float64)
+    if lo_.size != n_dim or hi_.size != n_dim:
+        raise ValueError("lo, hi must have n_dim entries")
+    h = C.c_void_p()
+    _check(lib().rift_ac_create(int(n_dim), int(n_bins), lo_.ctypes.data, hi_.ctypes.data, C.byref(h)))
+    return h
+
+
+def rift_ac_draw(h, n: int, seed: int, offset: int, x, ln_ps, cuda_stream: int = 0) -> None:
+    """x: a [n_dim][n] device tensor (contiguous rows) or a sequence of n_dim device arrays; ln_ps: device [n]."""
+    rows = [x[d] for d in range(x.shape[0])] if hasattr(x, "shape") and not isinstance(x, (list, tuple)) else list(x)
+    ptrs = (C.c_void_p * len(rows))(*[_ptr(r) for r in rows])
+    _check(lib().rift_ac_draw(h, int(n), int(seed), int(offset), ptrs, _ptr(ln_ps), int(cuda_stream) or None))
+
+
+def rift_ac_update(h, hist, floor_mix: float, temper: float = 1.0) -> None:
+    hist_ = np.ascontiguousarray(hist, dtype=np.float64)
+    _check(lib().rift_ac_update(h, hist_.ctypes.data, float(floor_mix), float(temper)))
+
+
+def rift_ac_get_masses(h, n_dim: int, n_bins: int) -> np.ndarray:
+    out = np.empty((n_dim, n_bins), dtype=np.float64)
+    _check(lib().rift_ac_get_masses(h, out.ctypes.data))
+    return out
+
+
+def rift_ac_ile_ln_weight(n: int, params, d_min_mpc: float, d_max_mpc: float, ln_ps, ln_weight,
+                          cuda_stream: int = 0) -> None:
+    _check(lib().rift_ac_ile_ln_weight(int(n), _params6(params), float(d_min_mpc), float(d_max_mpc), _ptr(ln_ps),
+                                       _ptr(ln_weight), int(cuda_stream) or None))
+
+
+def rift_ac_destroy(h) -> None:
+    _check(lib().rift_ac_destroy(h))

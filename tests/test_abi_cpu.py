@@ -22,6 +22,11 @@ def test_library_builds_and_exports_every_declared_symbol():
     L = binding.lib()
     for name in declared:
         assert hasattr(L, name), name
+    header_ac = open(os.path.join(ROOT, "include", "rift_ac.h")).read()
+    declared_ac = set(re.findall(r"\b(rift_ac_[a-z_]+)\s*\(", header_ac))
+    assert declared_ac == set(binding.AC_EXPORTS), declared_ac ^ set(binding.AC_EXPORTS)
+    for name in declared_ac:
+        assert hasattr(L, name), name
 
 
 def test_strerror_and_invalid_arguments_without_gpu():

@@ -1,0 +1,124 @@
+"""Pins of the adaptive-cartesian sampler oracle (oracle/ac_oracle.py; section IV.C.2, :336-358, Eq. (22) :348)
+against what the mathematics fixes: uniformity of the counter-based random numbers, exactness of the inverse-CDF draw,
+the importance-sampling identity E[1/p_s] = volume, the closed form of a Gaussian integral over a box (the paper's own
+integrator test, Fig. 6 :344, is a Gaussian) and the growth of n_eff under adaptation (Eq. (B1), :637)."""
+import math
+
+import numpy as np
+
+from oracle import ac_oracle as ac
+
+
+def test_p13_hash_is_uniform_and_reproducible():
+    u = ac.hash_u01(7, np.arange(400_000))
+    assert u.min() >= 0.0 and u.max() < 1.0
+    assert abs(u.mean() - 0.5) < 4 * math.sqrt(1 / 12 / u.size)
+    assert abs(u.var() - 1 / 12) < 1e-3
+    counts = np.histogram(u, bins=64, range=(0, 1))[0]
+    chi2 = float(((counts - u.size / 64) ** 2 / (u.size / 64)).sum())
+    assert chi2 < 64 + 6 * math.sqrt(2 * 64)                       # chi^2_63: mean 63, sigma 11
+    assert np.array_equal(u[:10], ac.hash_u01(7, np.arange(10)))   # a pure function of (seed, index)
+    assert not np.array_equal(u[:10], ac.hash_u01(8, np.arange(10)))
+    # consecutive indices are not correlated
+    assert abs(np.corrcoef(u[:-1], u[1:])[0, 1]) < 5e-3
+
+
+def test_p14_inverse_cdf_draw_matches_the_histogram():
+    rng = np.random.default_rng(1)
+    n_dim, n_bins, n = 3, 100, 300_000
+    masses = rng.random((n_dim, n_bins)) ** 3 + 1e-3
+    masses /= masses.sum(axis=1, keepdims=True)
+    lo, hi = np.array([-1.0, 0.0, 10.0]), np.array([1.0, 2 * math.pi, 2000.0])
+    x, ln_ps, bins = ac.draw(masses, lo, hi, n, seed=11)
+    w = (hi - lo) / n_bins
+    for d in range(n_dim):
+        assert x[d].min() >= lo[d] and x[d].max() < hi[d]
+        b = np.floor((x[d] - lo[d]) / w[d]).astype(int)
+        assert np.mean(b == bins[d]) > 0.999999                    # x falls in the bin it was drawn for
+        freq = np.bincount(bins[d], minlength=n_bins) / n
+        sig = np.sqrt(masses[d] * (1 - masses[d]) / n)
+        assert np.max(np.abs(freq - masses[d]) / sig) < 5.0
+    # ln p_s is the sum of the ln densities of the drawn bins
+    dens = np.array([masses[d, bins[d]] / w[d] for d in range(n_dim)])
+    assert np.max(np.abs(ln_ps - np.log(dens).sum(axis=0))) < 1e-12
+    # uniform masses reduce to a uniform draw: x = lo + u (hi - lo)
+    xu, lnu, _ = ac.draw(ac.uniform_masses(1, 100), [2.0], [5.0], 1000, seed=3)
+    u = ac.hash_u01(3, np.arange(1000))
+    assert np.max(np.abs(xu[0] - (2.0 + 3.0 * u))) < 1e-12
+    assert np.max(np.abs(lnu + math.log(3.0))) < 1e-12
+
+
+def test_p15_importance_identity_and_update_rule():
+    rng = np.random.default_rng(2)
+    masses = rng.random((2, 50)) + 0.05
+    masses /= masses.sum(axis=1, keepdims=True)
+    lo, hi = np.array([0.0, -3.0]), np.array([4.0, 3.0])
+    x, ln_ps, _ = ac.draw(masses, lo, hi, 400_000, seed=5)
+    w = np.exp(-ln_ps)                                              # integrand 1: E[1/p_s] = volume
+    vol = float(np.prod(hi - lo))
+    assert abs(w.mean() - vol) < 5 * w.std() / math.sqrt(w.size)
+    # update: floor mixing keeps every bin alive, preserves normalisation, temper = 1 and floor = 0 is the identity
+    h = rng.random((2, 50))
+    h[0, :10] = 0.0
+    h /= h.sum(axis=1, keepdims=True)
+    m = ac.update(h, floor=0.1)
+    assert np.allclose(m.sum(axis=1), 1.0, atol=1e-14) and m.min() >= 0.1 / 50 - 1e-18
+    assert np.allclose(ac.update(h, floor=0.0), h, atol=1e-15)
+    t = ac.update(h, floor=0.0, temper=0.5)
+    assert np.allclose(t, np.sqrt(h) / np.sqrt(h).sum(axis=1, keepdims=True), atol=1e-15)
+    assert np.allclose(ac.update(np.zeros((1, 8)), floor=0.3), 1 / 8)          # no information: uniform
+
+
+def _gauss_box_integral(mu, sig, lo, hi):
+    return float(np.prod([0.5 * (math.erf((h - m) / (s * math.sqrt(2))) - math.erf((l - m) / (s * math.sqrt(2))))
+                          for m, s, l, h in zip(mu, sig, lo, hi)]))
+
+
+def test_p16_adaptive_loop_recovers_a_gaussian_integral_and_raises_n_eff():
+    """The paper's integrator test is a three-dimensional Gaussian (Fig. 6, :344); its integral over a box is a product
+    of error functions.  The adaptive loop (draw, weight, histogram, update) must reproduce it within the Monte Carlo
+    error and raise n_eff (Eq. (B1)) well above the value of the uniform first round."""
+    mu, sig = np.array([0.3, -1.0, 2.0]), np.array([0.05, 0.2, 0.1])
+    lo, hi = np.array([-2.0, -4.0, 0.0]), np.array([2.0, 4.0, 4.0])
+    exact = _gauss_box_integral(mu, sig, lo, hi)
+    n_bins, n = 100, 20_000
+    masses = ac.uniform_masses(3, n_bins)
+    neff, est, err = [], [], []
+    for it in range(8):
+        x, ln_ps, bins = ac.draw(masses, lo, hi, n, seed=100, offset=it * n)
+        lnf = (-0.5 * ((x - mu[:, None]) / sig[:, None]) ** 2 - np.log(sig[:, None] * math.sqrt(2 * math.pi))).sum(axis=0)
+        w = np.exp(lnf - ln_ps)
+        est.append(w.mean())
+        err.append(w.std(ddof=1) / math.sqrt(n))
+        neff.append(w.sum() / w.max())
+        hist = np.array([np.bincount(bins[d], weights=w, minlength=n_bins) for d in range(3)])
+        hist /= hist.sum(axis=1, keepdims=True)
+        masses = ac.update(hist, floor=0.1)
+    assert neff[-1] > 20 * neff[0]
+    assert abs(est[-1] - exact) < 5 * err[-1]
+    assert err[-1] < 0.05 * err[0] + 1e-12 or err[-1] < 0.02 * exact
+    # inverse-variance combination of the adapted rounds (Eq. (20)-(21) pool rounds of equal size)
+    pooled = float(np.mean(est[3:]))
+    assert abs(pooled - exact) < 5 * math.sqrt(sum(e * e for e in err[3:])) / len(err[3:])
+
+
+def test_p17_ile_priors_are_normalised():
+    """Reading A18: the six extrinsic priors integrate to one (midpoint quadrature per factor)."""
+    n = 20001
+    mid = lambda a, b: a + (np.arange(n) + 0.5) * (b - a) / n
+    base = np.array([1.0, 0.2, 0.5, 1.0, 2.0, 400.0])
+    def factor(dim, a, b):
+        p = np.tile(base[:, None], (1, n))
+        p[dim] = mid(a, b)
+        ref = np.tile(base[:, None], (1, 1))
+        lp = ac.ln_prior_ile(p, 50.0, 2000.0) - ac.ln_prior_ile(ref, 50.0, 2000.0)[0]
+        return float(np.exp(lp).sum() * (b - a) / n)
+    # each 1-D conditional, normalised by its value at the base point, integrates to 1 / p_dim(base)
+    two_pi = 2 * math.pi
+    assert abs(factor(0, 0, two_pi) - two_pi) < 1e-9
+    assert abs(factor(1, -math.pi / 2, math.pi / 2) - 2 / math.cos(0.2)) < 1e-6
+    assert abs(factor(2, 0, math.pi) - math.pi) < 1e-9
+    assert abs(factor(3, 0, math.pi) - 2 / math.sin(1.0)) < 1e-6
+    assert abs(factor(5, 50.0, 2000.0) - (2000.0 ** 3 - 50.0 ** 3) / (3 * 400.0 ** 2)) < 1e-3
+    out = ac.ln_prior_ile(np.array([[7.0], [0.0], [0.1], [1.0], [1.0], [100.0]]), 50.0, 2000.0)
+    assert out[0] == -np.inf                                        # RA outside [0, 2 pi)
