@@ -173,19 +173,39 @@ geometry_kernel(DetGeom g, const ModeEntry *__restrict__ modes, Batch b, const d
                 const double *__restrict__ p_dec, const double *__restrict__ p_psi, const double *__restrict__ p_iota,
                 const double *__restrict__ p_phi, const double *__restrict__ p_dist, const double *__restrict__ U,
                 const double *__restrict__ V, Workspace ws, int32_t *__restrict__ shift_out,
-                double *__restrict__ dbg_F, double *__restrict__ dbg_Y, const int32_t *__restrict__ perm) {
+                double *__restrict__ dbg_F, double *__restrict__ dbg_Y, const int32_t *__restrict__ perm, int stage_uv) {
+  const int K = g.n_det, M = g.n_modes;
+  // U, V of the intrinsic point of the block's first slot staged in shared memory when the launch provides room
+  extern __shared__ double2 s_uv_g[];
+  const int n_uv = K * M * M;
+  int32_t point0 = -1;
+  if (stage_uv) {
+    const int64_t w0 = (int64_t)blockIdx.x * GEOM_THREADS;
+    const int64_t src0 = perm ? (int64_t)perm[w0] : w0;
+    point0 = b.ids[(b.g0 + src0) / b.n_per_seg];
+    const double2 *u = reinterpret_cast<const double2 *>(U) + (int64_t)point0 * n_uv;
+    const double2 *v = reinterpret_cast<const double2 *>(V) + (int64_t)point0 * n_uv;
+    for (int i = threadIdx.x; i < n_uv; i += GEOM_THREADS) {
+      s_uv_g[i] = u[i];
+      s_uv_g[n_uv + i] = v[i];
+    }
+    __syncthreads();
+  }
   const int64_t w = (int64_t)blockIdx.x * GEOM_THREADS + threadIdx.x;     // workspace slot (sorted position)
   if (w >= b.n) return;
   const int64_t src = perm ? (int64_t)perm[w] : w;                         // chunk-local index of the sample
   if (ws.orig) ws.orig[w] = (int32_t)src;
   const int64_t gi = b.g0 + src;                                           // caller's sample index
   const int32_t point = b.ids[gi / b.n_per_seg];
-  const int K = g.n_det, M = g.n_modes;
 
   int32_t shift[MAXK];
   double Fre[MAXK], Fim[MAXK], Yre[MAXM], Yim[MAXM], c, q;
-  const double2 *Up = reinterpret_cast<const double2 *>(U) + (int64_t)point * K * M * M;
-  const double2 *Vp = reinterpret_cast<const double2 *>(V) + (int64_t)point * K * M * M;
+  const double2 *Up = reinterpret_cast<const double2 *>(U) + (int64_t)point * n_uv;
+  const double2 *Vp = reinterpret_cast<const double2 *>(V) + (int64_t)point * n_uv;
+  if (stage_uv && point == point0) {
+    Up = s_uv_g;
+    Vp = s_uv_g + n_uv;
+  }
   sample_geometry<MAXM, MAXK>(g, modes, p_ra[gi], p_dec[gi], p_psi[gi], p_iota[gi], p_phi[gi], p_dist[gi], Up, Vp, shift,
                               Fre, Fim, Yre, Yim, c, q);
   int32_t *my_shift = ws.shift + w * K;
@@ -503,12 +523,20 @@ template <typename CT, int MAXM>
 cudaError_t launch_geometry_k(const DetGeom &g, const ModeEntry *modes, const Batch &b, const double *const params[6],
                               const double *U, const double *V, const Workspace &ws, int32_t *shift_out, double *dbg_F,
                               double *dbg_Y, const int32_t *perm, unsigned grid, cudaStream_t s) {
+  const size_t uv_bytes = (size_t)2 * g.n_det * g.n_modes * g.n_modes * sizeof(double2);
+  const int stage_uv = (MAXM > 16 && uv_bytes <= 96u * 1024u) ? 1 : 0;      // large mode sets: U, V from shared memory
+  const size_t smem = stage_uv ? uv_bytes : 0;
 #define RIFT_GEOM(KT)                                                                                                   \
-  case KT:                                                                                                              \
-    geometry_kernel<CT, MAXM, KT><<<grid, GEOM_THREADS, 0, s>>>(g, modes, b, params[0], params[1], params[2], params[3], \
-                                                                 params[4], params[5], U, V, ws, shift_out, dbg_F, dbg_Y, \
-                                                                 perm);                                                 \
-    break;
+  case KT: {                                                                                                            \
+    auto kern = geometry_kernel<CT, MAXM, KT>;                                                                          \
+    if (smem > 48u * 1024u) {                                                                                           \
+      cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);               \
+      if (e != cudaSuccess) return e;                                                                                   \
+    }                                                                                                                   \
+    kern<<<grid, GEOM_THREADS, smem, s>>>(g, modes, b, params[0], params[1], params[2], params[3], params[4], params[5], \
+                                          U, V, ws, shift_out, dbg_F, dbg_Y, perm, stage_uv);                           \
+    break;                                                                                                              \
+  }
   switch (g.n_det) {
     RIFT_GEOM(1) RIFT_GEOM(2) RIFT_GEOM(3) RIFT_GEOM(4) RIFT_GEOM(5) RIFT_GEOM(6) RIFT_GEOM(7) RIFT_GEOM(8)
     default: return cudaErrorInvalidValue;
