@@ -323,15 +323,24 @@ int ensure_tc_workspace(rift_ile *h, int64_t n_batches) {
   return RIFT_OK;
 }
 
-// chunks of whole 16-sample batches; per-chunk workspace near 64 MiB so that it stays in the 126 MB L2
+// chunks of whole 16-sample batches.  The per-chunk workspace is 1 GiB by default (RIFT_TC_CHUNK_MIB overrides): measured on
+// C1, every extra launch of the fused kernel costs ~30 us (tensor-memory allocation, A-operand load, pipeline fill, tail),
+// far more than keeping the blobs L2-resident saves (64 MiB chunks: 1.39 ms per step, one chunk: 1.24 ms)
 int run_chunks_tc(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *const params[6], double *lnL_out,
                   int32_t *shift_out, cudaStream_t s) {
   const int64_t nbps = (n_per_seg + RIFT_TC_NB - 1) / RIFT_TC_NB;
   const int64_t total = (int64_t)n_seg * nbps;
   if (total == 0) return RIFT_OK;
   const size_t per_batch = (size_t)h->tc.n_sub * h->tc.blob_words * 4 + (size_t)RIFT_TC_NB * (16 + 32);
-  int64_t cap = (int64_t)((64u << 20) / per_batch);
+  static int chunk_mib = 0;
+  if (chunk_mib == 0) {
+    const char *e = getenv("RIFT_TC_CHUNK_MIB");
+    chunk_mib = (e && atoi(e) > 0) ? atoi(e) : 1024;
+  }
+  int64_t cap = (int64_t)(((size_t)chunk_mib << 20) / per_batch);
   if (cap < 8 * (int64_t)h->n_sm) cap = 8 * (int64_t)h->n_sm;
+  // mode-subset passes stream their window sums through HBM anyway and reload the A operand per launch: larger chunks
+  if (h->tc.n_sub > 1 && cap < 65536) cap = 65536;
   int rc = ensure_tc_workspace(h, total < cap ? total : cap);
   if (rc != RIFT_OK) return rc;
   for (int64_t gb0 = 0; gb0 < total; gb0 += cap) {
