@@ -113,3 +113,37 @@ def test_closed_loop_on_a_synthetic_point(torch, oracle):
     assert abs(pooled["lnZ"][0] - ref["lnZ"][0]) < 5 * sigma + 0.02, (pooled, ref, sigma)
     rift.rift_ac_destroy(s)
     rift.rift_ile_destroy(h)
+
+
+def test_rosenbrock_evidence_of_fig7_on_device(torch, oracle):
+    """Fig. 7 (:356): the AC integrator recovers the evidence of the two-dimensional Rosenbrock likelihood, -5.804
+    (tests/golden/fig7_rosenbrock.txt, reading C3), from 1e6 evaluations in batches of 1e4.  The draws, their densities,
+    the weighted histograms and the pooled evidence (Eq. (20)-(21)) all come from the library; only the integrand is the
+    test's."""
+    import os
+    path = os.path.join(os.path.dirname(__file__), "golden", "fig7_rosenbrock.txt")
+    gold = [ln.split() for ln in open(path) if ln.strip() and not ln.startswith("#")][0]
+    ln_z, n_total, n = float(gold[0]), int(gold[1]), int(gold[2])
+    inp = build(oracle, synth.CONFIGS[0])
+    h_round, h_pool = create(rift, inp, rift.RIFT_PREC_MIXED), create(rift, inp, rift.RIFT_PREC_MIXED)
+    stream = torch.cuda.current_stream().cuda_stream
+    L, nb = 5.0, 100
+    s = rift.rift_ac_create(2, nb, [-L, -L], [L, L])
+    x = torch.empty((2, n), dtype=torch.float64, device="cuda")
+    lps = torch.empty(n, dtype=torch.float64, device="cuda")
+    six = [x[0], x[1], x[0], x[0], x[0], x[0]]                             # reduce histograms six rows; the first two are ours
+    lo6, hi6 = [-L] * 6, [L] * 6
+    for it in range(n_total // n):
+        rift.rift_ac_draw(s, n, seed=78, offset=it * n, x=x, ln_ps=lps, cuda_stream=stream)
+        lnL = -((1.0 - x[0]) ** 2 + 100.0 * (x[1] - x[0] * x[0]) ** 2)
+        lw = -math.log((2 * L) ** 2) - lps
+        one = rift.rift_ile_reduce(h_round, 1, n, lnL, lw, six, lo6, hi6, nb, merge=0, want_hist=True, cuda_stream=stream)
+        pooled = rift.rift_ile_reduce(h_pool, 1, n, lnL, lw, cuda_stream=stream, merge=0 if it == 0 else 1)
+        rift.rift_ac_update(s, one["hist"][0][:2], 0.1, 0.75)
+    rel = float(pooled["rel_err"][0])
+    assert rel < 0.03, pooled
+    assert abs(float(pooled["lnZ"][0]) - ln_z) < 4 * rel + 5e-4, pooled    # the paper prints three decimals
+    assert pooled["n_ess"][0] > 0.5 * float(gold[3]) and pooled["n_eff"][0] > 0.4 * float(gold[4]), pooled
+    rift.rift_ac_destroy(s)
+    rift.rift_ile_destroy(h_round)
+    rift.rift_ile_destroy(h_pool)
