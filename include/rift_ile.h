@@ -45,7 +45,7 @@ enum { RIFT_PREC_FP64 = 0, RIFT_PREC_MIXED = 1 };   /* arithmetic of the window 
 enum { RIFT_Q_C128 = 0, RIFT_Q_C64 = 1 };           /* storage of Q on the device */
 enum { RIFT_MEM_HOST = 0, RIFT_MEM_DEVICE = 1 };    /* where the Q/U/V arrays passed to create live */
 enum { RIFT_KERNEL_AUTO = 0, RIFT_KERNEL_DIRECT = 1, RIFT_KERNEL_GROUPED = 2, RIFT_KERNEL_QUAD = 3, RIFT_KERNEL_TC = 4,
-       RIFT_KERNEL_TILE = 5 };   /* rift_ile_set_kernel */
+       RIFT_KERNEL_TILE = 5, RIFT_KERNEL_TCS = 6 };   /* rift_ile_set_kernel */
 
 #define RIFT_MAX_DET 8
 #define RIFT_MAX_MODES 80

@@ -21,6 +21,7 @@ RIFT_PREC_FP64, RIFT_PREC_MIXED = 0, 1
 RIFT_Q_C128, RIFT_Q_C64 = 0, 1
 RIFT_MEM_HOST, RIFT_MEM_DEVICE = 0, 1
 RIFT_KERNEL_AUTO, RIFT_KERNEL_DIRECT, RIFT_KERNEL_GROUPED, RIFT_KERNEL_QUAD, RIFT_KERNEL_TC, RIFT_KERNEL_TILE = 0, 1, 2, 3, 4, 5
+RIFT_KERNEL_TCS = 6
 RIFT_N_PARAMS = 6
 
 EXPORTS = ("rift_ile_create", "rift_ile_eval_batch", "rift_ile_reduce", "rift_ile_geometry", "rift_ile_set_kernel",

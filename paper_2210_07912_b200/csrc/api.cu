@@ -30,6 +30,9 @@ struct rift_ile {
   float2 *tc_part = nullptr;
   float *tc_xacc = nullptr;        // window sums carried between mode-subset passes (n_sub > 1)
   int64_t tc_cap = 0;              // batches the workspace holds
+  uint16_t *d_Qs = nullptr;        // sorted variant (lnl_tcs.cu): extended detector-1 operand [P][kp/8][as_rows][8] fp16
+  int32_t *tcs_key = nullptr, *tcs_perm = nullptr, *tcs_bkt = nullptr;   // natural-slot keys, sorted-slot permutation, bucket tables
+  int64_t tcs_key_cap = 0, tcs_perm_cap = 0, tcs_bkt_cap = 0;
   double *d_exp_tab = nullptr;     // [64] 2^(j/64) for the fp64 exponential of lnl_tile
   int tile_ok = 0, tile_pitch = 0; // fp64 register-tiled kernel (lnl_tile.cu) usable for this handle
   SortPlan plan{};
@@ -161,6 +164,10 @@ void free_handle(rift_ile *h) {
   cudaFree(h->tc_quad);
   cudaFree(h->tc_part);
   cudaFree(h->tc_xacc);
+  cudaFree(h->d_Qs);
+  cudaFree(h->tcs_key);
+  cudaFree(h->tcs_perm);
+  cudaFree(h->tcs_bkt);
   cudaFree(h->d_bucket);
   cudaFree(h->d_perm);
   cudaFree(h->d_hist);
@@ -257,6 +264,12 @@ int32_t next_pow2(int64_t v) {
 
 
 // ---- tensor-core path ------------------------------------------------------------------------------------------------
+// per-chunk workspace of the tensor-core kernels in MiB (RIFT_TC_CHUNK_MIB, read at every call; default 1024)
+int tc_chunk_mib() {
+  const char *e = getenv("RIFT_TC_CHUNK_MIB");
+  return (e && atoi(e) > 0) ? atoi(e) : 1024;
+}
+
 void make_tc_plan(rift_ile *h, double delta_t) {
   TcPlan &tp = h->tc;
   tp = TcPlan{};
@@ -291,6 +304,20 @@ void make_tc_plan(rift_ile *h, double delta_t) {
                     tp.K * tp.nt * (tp.acols + RIFT_TC_NB) <= 512 && tp.H < tp.n_t && tp.pitch > 0 &&
                     lnl_tc_smem_bytes(tp) <= 227u * 1024u;
   tp.ok = fits ? 1 : 0;
+  // sorted variant: detector 1 fused by the tensor core (lnl_tcs.cu)
+  if (tp.ok && tp.n_sub == 1 && tp.K >= 2) {
+    int hs = 0;
+    for (int k = 2; k < tp.K; ++k) hs = tp.dmax[k] > hs ? tp.dmax[k] : hs;
+    tp.n_bkt = 2 * tp.dmax[1] + 1;
+    tp.as_rows = tp.nt * 128 + 2 * tp.dmax[1];
+    tp.pitch_s = tp.K > 2 ? lnl_tc_pitch(tp.n_t, hs) : 256;
+    tp.blob_words_s = (tp.blob_words + 4 + 31) & ~31;                 // + batch header, stages stay 128-byte aligned
+    tp.dcol0_s = (tp.K - 1) * tp.nt * tp.acols;
+    tp.srt_ok = (tp.pitch_s > 0 && tp.dmax[1] < tp.n_t && (tp.K - 1) * tp.nt * (tp.acols + RIFT_TC_NB) <= 512 &&
+                 tp.as_rows * 16 < (1 << 18) && lnl_tcs_smem_bytes(tp) <= 227u * 1024u)
+                    ? 1
+                    : 0;
+  }
 }
 
 // opt-in (RIFT_KERNEL_TILE): on C1 fp64 it measures 7.1 ms against 6.1 ms of lnl_direct
@@ -298,10 +325,21 @@ bool use_tile(const rift_ile *h) { return h->tile_ok && h->kernel_variant == RIF
 
 bool use_tc(const rift_ile *h) {
   if (!h->tc.ok || h->d_Qtc == nullptr) return false;
-  return h->kernel_variant == RIFT_KERNEL_AUTO || h->kernel_variant == RIFT_KERNEL_TC;
+  return h->kernel_variant == RIFT_KERNEL_AUTO || h->kernel_variant == RIFT_KERNEL_TC || h->kernel_variant == RIFT_KERNEL_TCS;
 }
 
-int ensure_tc_workspace(rift_ile *h, int64_t n_batches) {
+// Sorted variant: worth it when the padding of the shift buckets (about 8 slots per bucket and segment) stays small
+bool use_tcs(const rift_ile *h, int64_t n_per_seg) {
+  if (!h->tc.srt_ok || h->d_Qs == nullptr) return false;
+  if (h->kernel_variant == RIFT_KERNEL_TCS) return true;
+  const char *e = getenv("RIFT_TC_SORT");                                // RIFT_TC_SORT=0: never pick it automatically
+  const bool auto_on = !(e && atoi(e) == 0);
+  return auto_on && h->kernel_variant == RIFT_KERNEL_AUTO && n_per_seg >= 40 * (int64_t)h->tc.n_bkt;
+}
+
+int ensure_tc_workspace(rift_ile *h, int64_t n_batches, int blob_words = 0) {
+  if (blob_words < h->tc.blob_words) blob_words = h->tc.blob_words;
+  if (h->tc.srt_ok && blob_words < h->tc.blob_words_s) blob_words = h->tc.blob_words_s;   // one size for both variants
   if (n_batches <= h->tc_cap) return RIFT_OK;
   cudaFree(h->tc_blob);
   cudaFree(h->tc_c);
@@ -314,7 +352,7 @@ int ensure_tc_workspace(rift_ile *h, int64_t n_batches) {
   h->tc_xacc = nullptr;
   h->tc_cap = 0;
   const size_t slots = (size_t)n_batches * RIFT_TC_NB;
-  CU(h, cudaMalloc(&h->tc_blob, (size_t)h->tc.n_sub * n_batches * h->tc.blob_words * sizeof(float)));
+  CU(h, cudaMalloc(&h->tc_blob, (size_t)h->tc.n_sub * n_batches * blob_words * sizeof(float)));
   CU(h, cudaMalloc(&h->tc_c, slots * sizeof(double)));
   CU(h, cudaMalloc(&h->tc_quad, slots * sizeof(double)));
   CU(h, cudaMalloc(&h->tc_part, slots * 4 * sizeof(float2)));
@@ -332,11 +370,7 @@ int run_chunks_tc(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *c
   const int64_t total = (int64_t)n_seg * nbps;
   if (total == 0) return RIFT_OK;
   const size_t per_batch = (size_t)h->tc.n_sub * h->tc.blob_words * 4 + (size_t)RIFT_TC_NB * (16 + 32);
-  static int chunk_mib = 0;
-  if (chunk_mib == 0) {
-    const char *e = getenv("RIFT_TC_CHUNK_MIB");
-    chunk_mib = (e && atoi(e) > 0) ? atoi(e) : 1024;
-  }
+  const int chunk_mib = tc_chunk_mib();
   int64_t cap = (int64_t)(((size_t)chunk_mib << 20) / per_batch);
   if (cap < 8 * (int64_t)h->n_sm) cap = 8 * (int64_t)h->n_sm;
   // mode-subset passes stream their window sums through HBM anyway and reload the A operand per launch: larger chunks
@@ -344,7 +378,7 @@ int run_chunks_tc(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *c
   int rc = ensure_tc_workspace(h, total < cap ? total : cap);
   if (rc != RIFT_OK) return rc;
   for (int64_t gb0 = 0; gb0 < total; gb0 += cap) {
-    TcChunk c;
+    TcChunk c{};
     c.n_per_seg = n_per_seg;
     c.nbps = nbps;
     c.gb0 = gb0;
@@ -380,6 +414,74 @@ int run_chunks_tc(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *c
     h->launches += nl;
   }
   h->kernel_name = h->tc.n_sub == 1 ? "lnl_tc<f16x3>" : "lnl_tc<f16x3,passes>";
+  return RIFT_OK;
+}
+
+// Sorted tensor-core variant: per chunk, bucket the samples by (segment, d_1), let the geometry kernel write every sample
+// into the next free slot of its bucket, run lnl_tcs over the sorted batches and scatter lnL back.
+int ensure_i32(rift_ile *h, int32_t **p, int64_t *cap, int64_t need) {
+  if (need <= *cap) return RIFT_OK;
+  cudaFree(*p);
+  *p = nullptr;
+  *cap = 0;
+  CU(h, cudaMalloc(p, (size_t)need * sizeof(int32_t)));
+  *cap = need;
+  return RIFT_OK;
+}
+
+int run_chunks_tcs(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *const params[6], double *lnL_out,
+                   int32_t *shift_out, cudaStream_t s) {
+  const TcPlan &tp = h->tc;
+  const int64_t nbps = (n_per_seg + RIFT_TC_NB - 1) / RIFT_TC_NB;
+  const int64_t total = (int64_t)n_seg * nbps;
+  if (total == 0) return RIFT_OK;
+  const size_t per_batch = (size_t)tp.blob_words_s * 4 + (size_t)RIFT_TC_NB * (16 + 32 + 8);
+  const int chunk_mib = tc_chunk_mib();
+  int64_t cap = (int64_t)(((size_t)chunk_mib << 20) / per_batch);
+  if (cap < 8 * (int64_t)h->n_sm) cap = 8 * (int64_t)h->n_sm;
+  const int64_t nb_max = total < cap ? total : cap;
+  int64_t lseg_max = nb_max / nbps + 2;
+  if (lseg_max > n_seg) lseg_max = n_seg;
+  int rc = ensure_tc_workspace(h, nb_max + lseg_max * tp.n_bkt);
+  if (rc == RIFT_OK) rc = ensure_i32(h, &h->tcs_key, &h->tcs_key_cap, 2 * nb_max * RIFT_TC_NB);   // keys, positions
+  if (rc == RIFT_OK) rc = ensure_i32(h, &h->tcs_perm, &h->tcs_perm_cap, (nb_max + lseg_max * tp.n_bkt) * RIFT_TC_NB);
+  if (rc == RIFT_OK) rc = ensure_i32(h, &h->tcs_bkt, &h->tcs_bkt_cap, 2 * lseg_max * tp.n_bkt + lseg_max + 1);
+  if (rc != RIFT_OK) return rc;
+  for (int64_t gb0 = 0; gb0 < total; gb0 += cap) {
+    TcChunk c{};
+    c.n_per_seg = n_per_seg;
+    c.nbps = nbps;
+    c.gb0 = gb0;
+    c.n_batches = (total - gb0 < cap) ? total - gb0 : cap;
+    c.ids = h->d_ids;
+    c.qscale = h->d_qscale;
+    c.blob = h->tc_blob;
+    c.scale_c = h->tc_c;
+    c.quad = h->tc_quad;
+    c.part = h->tc_part;
+    c.n_lseg = (int32_t)((gb0 + c.n_batches - 1) / nbps - gb0 / nbps + 1);
+    c.cap_sorted = c.n_batches + (int64_t)c.n_lseg * tp.n_bkt;
+    const int64_t nbk = (int64_t)c.n_lseg * tp.n_bkt;
+    c.key = h->tcs_key;
+    c.pos = h->tcs_key + c.n_batches * RIFT_TC_NB;
+    c.perm = h->tcs_perm;
+    c.count = h->tcs_bkt;
+    c.base = h->tcs_bkt + nbk;
+    c.seg_begin = h->tcs_bkt + 2 * nbk;
+    int nl = 0;
+    {
+      ProfSpan ps(h, 0, s);
+      CU(h, launch_tcs_buckets(h->geom, tp, c, params, s, &nl));
+      CU(h, launch_geometry_tc(h->geom, h->d_modes, tp, c, params, h->d_U, h->d_V, shift_out, s));
+      ++nl;
+      ps.end();
+    }
+    ProfSpan ps(h, 1, s);
+    CU(h, launch_lnl_tcs(tp, h->d_Qtc, h->d_Qs, c, lnL_out, h->n_sm, s, &nl));
+    ps.end();
+    h->launches += nl;
+  }
+  h->kernel_name = "lnl_tcs<f16x3>";
   return RIFT_OK;
 }
 
@@ -629,6 +731,11 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
       if (e == cudaSuccess) e = cudaMalloc(&h->d_qscale, sizeof(float) * h->P);
       if (e == cudaSuccess) e = launch_convert_q_tc(src, h->d_Qtc, h->d_qscale, h->tc, h->P, 0);
       h->launches += 3;
+      if (e == cudaSuccess && h->tc.srt_ok) {
+        e = cudaMalloc(&h->d_Qs, (size_t)h->P * (h->tc.kp >> 3) * h->tc.as_rows * 8 * sizeof(uint16_t));
+        if (e == cudaSuccess) e = launch_convert_q_tcs(src, h->d_Qs, h->d_qscale, h->tc, h->P, 0);
+        ++h->launches;
+      }
     }
     // fp64 register-tiled kernel: circular window of at most 4 row tiles, Q block + exchange buffers in shared memory
     if (e == cudaSuccess && h->precision == RIFT_PREC_FP64 && h->n_tau == h->n_t && h->n_t <= 512 && h->tc.H < h->n_t &&
@@ -691,7 +798,7 @@ int rift_ile_destroy(rift_ile_t *h) {
 int rift_ile_set_kernel(rift_ile_t *h, int32_t variant) {
   if (!h) return RIFT_EINVAL;
   if (variant != RIFT_KERNEL_AUTO && variant != RIFT_KERNEL_DIRECT && variant != RIFT_KERNEL_GROUPED && variant != RIFT_KERNEL_QUAD &&
-      variant != RIFT_KERNEL_TC && variant != RIFT_KERNEL_TILE)
+      variant != RIFT_KERNEL_TC && variant != RIFT_KERNEL_TILE && variant != RIFT_KERNEL_TCS)
     return fail(h, RIFT_EINVAL, "unknown kernel variant");
   h->kernel_variant = variant;
   return RIFT_OK;
@@ -710,6 +817,7 @@ int rift_ile_eval_batch(rift_ile_t *h, int32_t n_seg, const int32_t *intrinsic_i
   cudaStream_t s = reinterpret_cast<cudaStream_t>(cuda_stream);
   int rc = upload_ids(h, n_seg, intrinsic_ids, s);
   if (rc != RIFT_OK) return rc;
+  if (use_tc(h) && use_tcs(h, n_per_seg)) return run_chunks_tcs(h, n_seg, n_per_seg, params, lnL_out, shift_out, s);
   if (use_tc(h)) return run_chunks_tc(h, n_seg, n_per_seg, params, lnL_out, shift_out, s);
   return run_chunks(h, n_seg, n_per_seg, params, lnL_out, shift_out, nullptr, nullptr, nullptr, s);
 }

@@ -250,9 +250,17 @@ geometry_tc_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, Tc
   constexpr int NCH = KP / 8;                                               // 16-byte chunks per detector
   __shared__ ModeEntry s_modes[MT];
   __shared__ double2 s_U[KT * MT * MT], s_V[KT * MT * MT];
-  const int64_t n_slots = ch.n_batches * RIFT_TC_NB;
+  const bool sorted = ch.key != nullptr;    // sorted variant: slots are the sorted slots, the sample comes through ch.perm
+  const int64_t n_slots = (sorted ? (int64_t)ch.seg_begin[ch.n_lseg] : ch.n_batches) * RIFT_TC_NB;
   const int64_t w0 = (int64_t)blockIdx.x * GEOM_THREADS;                    // first slot of the block
-  const int32_t point0 = ch.ids[(ch.gb0 + w0 / RIFT_TC_NB) / ch.nbps];
+  if (w0 >= n_slots) return;
+  int64_t seg_first = (ch.gb0 + w0 / RIFT_TC_NB) / ch.nbps;                 // segment of the block's first slot
+  if (sorted) {
+    int ls = 0;
+    while (ch.seg_begin[ls + 1] <= w0 / RIFT_TC_NB) ++ls;
+    seg_first = ch.gb0 / ch.nbps + ls;
+  }
+  const int32_t point0 = ch.ids[seg_first];
   {
     const int32_t *src = reinterpret_cast<const int32_t *>(modes);
     int32_t *dst = reinterpret_cast<int32_t *>(s_modes);
@@ -269,11 +277,14 @@ geometry_tc_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, Tc
   if (w >= n_slots) return;
   const int64_t lb = w / RIFT_TC_NB;
   const int n = (int)(w % RIFT_TC_NB);
-  const int64_t gb = ch.gb0 + lb;
+  int64_t wn = w;                                                           // natural slot of the sample
+  if (sorted) wn = ch.perm[w];
+  const int64_t gb = ch.gb0 + wn / RIFT_TC_NB;
   const int64_t seg = gb / ch.nbps;
-  const int64_t i = (gb % ch.nbps) * RIFT_TC_NB + n;
-  const bool valid = i < ch.n_per_seg;
-  float *blob = ch.blob + lb * tp.blob_words;
+  const int64_t i = (gb % ch.nbps) * RIFT_TC_NB + (wn % RIFT_TC_NB);
+  const bool valid = wn >= 0 && i < ch.n_per_seg;
+  const int blob_words = sorted ? tp.blob_words_s : tp.blob_words;
+  float *blob = ch.blob + lb * blob_words;
   uint4 *chunks = reinterpret_cast<uint4 *>(blob);                          // [K][NCH][16] x 8 halfs
   int32_t *dsh = reinterpret_cast<int32_t *>(blob + K * NCH * 64);          // [K][16]
   float *cl2 = blob + K * NCH * 64 + K * 16;                                // [16]
@@ -305,6 +316,10 @@ geometry_tc_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, Tc
   ch.quad[w] = q;
   // exponent scale of the fused kernel: its accumulators carry x * (Q scale of the point) * RIFT_TC_BSCALE
   cl2[n] = (float)(c * 1.4426950408889634 / ((double)ch.qscale[point] * RIFT_TC_BSCALE));
+  if (sorted && n == 0) {                                                   // batch header: the common d_1 (clamped as the key)
+    const int dm = tp.dmax[1], d = shift[KT > 1 ? 1 : 0] - shift[0];
+    reinterpret_cast<int32_t *>(cl2 + 16)[0] = d < -dm ? -dm : (d > dm ? dm : d);
+  }
 #pragma unroll
   for (int k = 0; k < K; ++k) {
     if (shift_out) shift_out[gi * K + k] = shift[k];
@@ -469,10 +484,146 @@ cudaError_t launch_geometry_tc_m(const DetGeom &g, const ModeEntry *modes, const
 }
 }  // namespace
 
+namespace {
+// Sorted tensor-core variant, pass 1: the shift bucket of every natural slot.  The delays are computed with exactly the
+// operations of sample_geometry (a3), so that the bucket's d_1 is the d_1 the geometry kernel will find.
+constexpr int KEY_THREADS = 1024;
+// The bucket counts are formed per block in shared memory (a block touches at most two segments when the sorted variant is
+// used) and added to the global counts with one atomic per non-empty (block, bucket): contended global atomics on a few
+// thousand addresses serialise (measured: 1.6e6 of them on 5440 addresses take 0.13-0.18 ms).  The atomic's return value
+// is the block's offset inside the bucket, so every sample already knows its position in the bucket (ch.pos).
+__global__ void __launch_bounds__(KEY_THREADS)
+tcs_key_kernel(DetGeom g, TcPlan tp, TcChunk ch, const double *__restrict__ p_ra, const double *__restrict__ p_dec,
+               int use_smem) {
+  extern __shared__ int s_hist[];                                            // [2 n_bkt]
+  const int nb2 = 2 * tp.n_bkt;
+  const int64_t w0 = (int64_t)blockIdx.x * KEY_THREADS;
+  const int64_t seg0 = ch.gb0 / ch.nbps;
+  const int lseg0 = (int)((ch.gb0 + w0 / RIFT_TC_NB) / ch.nbps - seg0);
+  if (use_smem) {
+    for (int i = threadIdx.x; i < nb2; i += KEY_THREADS) s_hist[i] = 0;
+    __syncthreads();
+  }
+  const int64_t w = w0 + threadIdx.x;
+  int b = -1;
+  if (w < ch.n_batches * RIFT_TC_NB) {
+    const int64_t gb = ch.gb0 + w / RIFT_TC_NB;
+    const int64_t seg = gb / ch.nbps;
+    const int64_t i = (gb % ch.nbps) * RIFT_TC_NB + (w % RIFT_TC_NB);
+    if (i < ch.n_per_seg) {
+      const int64_t gi = seg * ch.n_per_seg + i;
+      double sd, cd, sh, chh;
+      sincos(p_dec[gi], &sd, &cd);
+      sincos(p_ra[gi] - g.gmst, &sh, &chh);
+      const double nx = __dmul_rn(cd, chh), ny = __dmul_rn(cd, sh), nz = sd;
+      int32_t shift[2];
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {
+        const double dot =
+            __dadd_rn(__dadd_rn(__dmul_rn(g.loc[k][0], nx), __dmul_rn(g.loc[k][1], ny)), __dmul_rn(g.loc[k][2], nz));
+        const double dt = -__ddiv_rn(dot, RIFT_C_LIGHT);
+        const double x = __ddiv_rn(dt, g.delta_t);
+        shift[k] = (int32_t)floor(__dadd_rn(x, 0.5));
+      }
+      const int dm = tp.dmax[1];
+      int d = shift[1] - shift[0];
+      d = d < -dm ? -dm : (d > dm ? dm : d);                                 // only samples with invalid angles can be out of range
+      b = (int)(seg - seg0) * tp.n_bkt + d + dm;
+    }
+  }
+  const int rel = b - lseg0 * tp.n_bkt;
+  const bool loc = use_smem && b >= 0 && rel < nb2;
+  int r = 0;
+  if (loc) r = atomicAdd(&s_hist[rel], 1);
+  else if (b >= 0) r = atomicAdd(ch.count + b, 1);
+  if (use_smem) {
+    __syncthreads();
+    for (int i = threadIdx.x; i < nb2; i += KEY_THREADS) {
+      const int c = s_hist[i];
+      if (c > 0) s_hist[i] = atomicAdd(ch.count + lseg0 * tp.n_bkt + i, c);
+    }
+    __syncthreads();
+  }
+  if (w < ch.n_batches * RIFT_TC_NB) {
+    ch.key[w] = b;
+    if (b >= 0) ch.pos[w] = loc ? s_hist[rel] + r : r;
+  }
+}
+
+// pass 2 (one block): batches per bucket, their exclusive prefix, the first batch of every local segment
+__global__ void __launch_bounds__(1024) tcs_scan_kernel(TcPlan tp, TcChunk ch) {
+  __shared__ int s_warp[32];
+  __shared__ int s_carry;
+  const int n = ch.n_lseg * tp.n_bkt;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (threadIdx.x == 0) s_carry = 0;
+  __syncthreads();
+  for (int i0 = 0; i0 < n; i0 += 1024) {
+    const int i = i0 + threadIdx.x;
+    const int nb = i < n ? (ch.count[i] + RIFT_TC_NB - 1) / RIFT_TC_NB : 0;
+    int v = nb;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int t = __shfl_up_sync(0xffffffffu, v, o);
+      if (lane >= o) v += t;
+    }
+    if (lane == 31) s_warp[warp] = v;
+    __syncthreads();
+    if (warp == 0) {
+      int t = s_warp[lane];
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int u = __shfl_up_sync(0xffffffffu, t, o);
+        if (lane >= o) t += u;
+      }
+      s_warp[lane] = t;
+    }
+    __syncthreads();
+    const int excl = s_carry + (warp ? s_warp[warp - 1] : 0) + v - nb;
+    if (i < n) {
+      ch.base[i] = excl;
+      if (i % tp.n_bkt == 0) ch.seg_begin[i / tp.n_bkt] = excl;
+    }
+    __syncthreads();
+    if (threadIdx.x == 1023) s_carry = excl + nb;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) ch.seg_begin[ch.n_lseg] = s_carry;
+}
+}  // namespace
+
+namespace {
+// pass 3: sorted slot of every sample = first slot of its bucket + position in the bucket; perm was preset to -1 (padding)
+__global__ void __launch_bounds__(256) tcs_fill_kernel(TcChunk ch) {
+  const int64_t w = (int64_t)blockIdx.x * 256 + threadIdx.x;
+  if (w >= ch.n_batches * RIFT_TC_NB) return;
+  const int b = ch.key[w];
+  if (b < 0) return;
+  ch.perm[(int64_t)ch.base[b] * RIFT_TC_NB + ch.pos[w]] = (int32_t)w;
+}
+}  // namespace
+
+cudaError_t launch_tcs_buckets(const DetGeom &g, const TcPlan &tp, const TcChunk &c, const double *const params[6],
+                               cudaStream_t s, int *n_launch) {
+  const int64_t n = c.n_batches * RIFT_TC_NB;
+  if (n <= 0) return cudaSuccess;
+  cudaError_t e = cudaMemsetAsync(c.count, 0, sizeof(int32_t) * (size_t)c.n_lseg * tp.n_bkt, s);
+  if (e != cudaSuccess) return e;
+  const int use_smem = 2 * tp.n_bkt * (int)sizeof(int) <= 32 * 1024 ? 1 : 0;
+  tcs_key_kernel<<<(unsigned)((n + KEY_THREADS - 1) / KEY_THREADS), KEY_THREADS, use_smem ? 2 * tp.n_bkt * sizeof(int) : 0, s>>>(
+      g, tp, c, params[0], params[1], use_smem);
+  tcs_scan_kernel<<<1, 1024, 0, s>>>(tp, c);
+  e = cudaMemsetAsync(c.perm, 0xff, sizeof(int32_t) * (size_t)c.cap_sorted * RIFT_TC_NB, s);
+  if (e != cudaSuccess) return e;
+  tcs_fill_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(c);
+  if (n_launch) *n_launch += 3;
+  return cudaGetLastError();
+}
+
 cudaError_t launch_geometry_tc(const DetGeom &g, const ModeEntry *modes, const TcPlan &tp, const TcChunk &c,
                                const double *const params[6], const double *U, const double *V, int32_t *shift_out,
                                cudaStream_t s) {
-  const int64_t n = c.n_batches * RIFT_TC_NB;
+  const int64_t n = (c.key ? c.cap_sorted : c.n_batches) * RIFT_TC_NB;      // sorted variant: upper bound, trimmed on device
   if (n <= 0) return cudaSuccess;
   const unsigned grid = (unsigned)((n + GEOM_THREADS - 1) / GEOM_THREADS);
   if (tp.n_sub > 1) {

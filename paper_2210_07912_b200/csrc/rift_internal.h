@@ -73,6 +73,11 @@ struct TcPlan {
   int32_t H, pitch;              // halo = max_k dmax[k]; exchange-row pitch in floats
   int32_t blob_words, dcol0;     // 32-bit words per batch blob; first accumulator column in TMEM
   int32_t dmax[RIFT_MAX_DET];    // bound on |s_k - s_0|
+  // sorted variant (lnl_tcs.cu): batches hold samples of ONE relative shift d_1 = s_1 - s_0, so that detector 1 is contracted
+  // from a shared-memory A operand whose rows start at d_1 and accumulates straight onto detector 0; detectors >= 2 keep
+  // the exchange.  n_bkt = 2 dmax[1] + 1 shift buckets per segment; as_rows = rows of the extended detector-1 operand
+  // (row r = time r - dmax[1], wrapped), [kp/8 planes][as_rows][8 fp16]; blob_words_s = blob_words + 4 (batch header: d_1).
+  int32_t srt_ok, n_bkt, as_rows, pitch_s, blob_words_s, dcol0_s;
 };
 struct TcChunk {                 // a chunk = global batches [gb0, gb0 + n_batches), batch gb = seg * nbps + b
   int64_t n_per_seg, nbps, gb0, n_batches;
@@ -82,6 +87,15 @@ struct TcChunk {                 // a chunk = global batches [gb0, gb0 + n_batch
   double *scale_c, *quad;        // [n_batches * 16]
   float2 *part;                  // [n_batches * 16][4]: per lane-quarter (reference, sum)
   float *xacc;                   // [n_batches * 16][nt * 128]: window sums carried between mode-subset passes (or NULL)
+  // sorted variant: key == NULL means natural order.  Natural slot w = (local batch) * 16 + n; sorted slots are assigned
+  // per (local segment, shift bucket) in arrival order, every bucket padded to whole batches.
+  int32_t *key;                  // [n_batches * 16] bucket index (lseg * n_bkt + d_1 + dmax[1]) of a natural slot, -1 = padding
+  int32_t *pos;                  // [n_batches * 16] position of a natural slot inside its bucket
+  int32_t *count, *base;         // [n_lseg * n_bkt] samples per bucket, first sorted batch of the bucket
+  int32_t *seg_begin;            // [n_lseg + 1] first sorted batch of each local segment; seg_begin[n_lseg] = sorted batches
+  int32_t *perm;                 // [cap_sorted * 16] natural slot of a sorted slot, -1 = padding
+  int32_t n_lseg;                // segments touched by this chunk
+  int64_t cap_sorted;            // capacity in sorted batches (n_batches + n_lseg * n_bkt)
 };
 // Mode-subset passes of lnl_tc (configurations whose A operand does not fit tensor memory whole, e.g. 21 modes): the modes are
 // split into n_sub subsets of m_sub; pass s contracts subset s and adds the window sums of the passes before it.
@@ -125,6 +139,14 @@ cudaError_t launch_convert_q_tc(const double *Q_c128, uint32_t *dst, float *qsca
                                 cudaStream_t s);   // dst: [n_sub][P][K][nt*128][acols]
 cudaError_t launch_lnl_tc(const TcPlan &tp, const uint32_t *qtc, const TcChunk &c, int pass, double *lnL_out, int n_sm,
                           cudaStream_t s, int *n_launch);
+// lnl_tcs.cu (sorted variant: detector 1 fused into detector 0 by the tensor core; geometry.cu holds the bucket kernels)
+size_t lnl_tcs_smem_bytes(const TcPlan &tp);
+cudaError_t launch_convert_q_tcs(const double *Q_c128, uint16_t *dst, const float *qscale, const TcPlan &tp,
+                                 int32_t n_points, cudaStream_t s);   // dst: [P][kp/8][as_rows][8] fp16, detector 1
+cudaError_t launch_tcs_buckets(const DetGeom &g, const TcPlan &tp, const TcChunk &c, const double *const params[6],
+                               cudaStream_t s, int *n_launch);        // key, pos, count, base, seg_begin, perm
+cudaError_t launch_lnl_tcs(const TcPlan &tp, const uint32_t *qtc, const uint16_t *qs, const TcChunk &c, double *lnL_out,
+                           int n_sm, cudaStream_t s, int *n_launch);
 // lnl_tile.cu (fp64 register-tiled contraction + shared-memory exchange; circular mode, n_t <= 512)
 size_t lnl_tile_smem_bytes(const QStore &q, int K, int pitch);
 cudaError_t launch_lnl_tile(const QStore &q, const Batch &b, const Workspace &ws, int K, int H, int pitch, const int *dmax,

@@ -90,7 +90,8 @@ def test_higher_l_harmonics(torch, oracle):
 
 # ------------------------------------------------------------------------------------------------ C0, whole config
 KERNELS = [rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_DIRECT, rift.RIFT_KERNEL_GROUPED, rift.RIFT_KERNEL_QUAD,
-           rift.RIFT_KERNEL_TC, rift.RIFT_KERNEL_TILE]
+           rift.RIFT_KERNEL_TC, rift.RIFT_KERNEL_TILE, rift.RIFT_KERNEL_TCS]
+TC_FAMILY = (rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_TC, rift.RIFT_KERNEL_TCS)
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
@@ -110,7 +111,10 @@ def test_c0_all_samples_both_precisions(torch, oracle, rho, kernel):
         assert ("quad" in rift.rift_ile_kernel_name(h)) == (kernel == rift.RIFT_KERNEL_QUAD)
         # the tensor-core kernel is the default of the mixed mode (and never runs in fp64 mode)
         assert ("lnl_tc" in rift.rift_ile_kernel_name(h)) == (
-            prec == rift.RIFT_PREC_MIXED and kernel in (rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_TC))
+            prec == rift.RIFT_PREC_MIXED and kernel in TC_FAMILY)
+        # the shift-sorted variant: on request, or by default when the segments are long enough to fill its buckets
+        if prec == rift.RIFT_PREC_MIXED and kernel == rift.RIFT_KERNEL_TCS:
+            assert "lnl_tcs" in rift.rift_ile_kernel_name(h)
         # the register-tiled kernel exists for fp64 only and is opt-in
         assert ("lnl_tile" in rift.rift_ile_kernel_name(h)) == (
             prec == rift.RIFT_PREC_FP64 and kernel == rift.RIFT_KERNEL_TILE)
@@ -188,7 +192,8 @@ def test_edge_sizes_and_invalid_samples(torch, oracle):
     rift.rift_ile_destroy(h)
 
 
-def test_tc_edge_sizes_ragged_batches_and_invalid_samples(torch, oracle):
+@pytest.mark.parametrize("kernel", [rift.RIFT_KERNEL_TC, rift.RIFT_KERNEL_TCS])
+def test_tc_edge_sizes_ragged_batches_and_invalid_samples(torch, oracle, kernel):
     """Tensor-core kernel (mixed mode): sample counts around the 16-sample batch, several short segments in one call,
     NaN / non-positive distance samples (NaN for that sample only)."""
     cfg = synth.CONFIGS[1]
@@ -197,8 +202,8 @@ def test_tc_edge_sizes_ragged_batches_and_invalid_samples(torch, oracle):
     for n in (1, 7, 16, 17, 33):
         ids = [1, 0, 1]
         params = synth.prior_draw(np.random.default_rng(100 + n), n * len(ids))
-        got = gpu_eval(torch, h, ids, n, params, K=cfg.n_det, kernel=rift.RIFT_KERNEL_TC)[0].cpu().numpy()
-        assert "lnl_tc" in rift.rift_ile_kernel_name(h)
+        got = gpu_eval(torch, h, ids, n, params, K=cfg.n_det, kernel=kernel)[0].cpu().numpy()
+        assert ("lnl_tcs" if kernel == rift.RIFT_KERNEL_TCS else "lnl_tc<") in rift.rift_ile_kernel_name(h)
         ref = np.concatenate([oracle_eval(oracle, inp, ids[s], params[:, s * n:(s + 1) * n])[0] for s in range(len(ids))])
         assert np.max(np.abs(got - ref)) < TOL_MIXED_LNL, n
     params = synth.prior_draw(np.random.default_rng(9), 64)
@@ -206,7 +211,7 @@ def test_tc_edge_sizes_ragged_batches_and_invalid_samples(torch, oracle):
     params[5, 4] = 0.0
     params[0, 5] = np.nan
     params[3, 40] = np.nan
-    got = gpu_eval(torch, h, [0], 64, params, K=cfg.n_det, kernel=rift.RIFT_KERNEL_TC)[0].cpu().numpy()
+    got = gpu_eval(torch, h, [0], 64, params, K=cfg.n_det, kernel=kernel)[0].cpu().numpy()
     ref = oracle_eval(oracle, inp, 0, params)[0]
     assert np.array_equal(np.isnan(got), np.isnan(ref)) and np.isnan(got).sum() == 4
     ok = ~np.isnan(ref)
@@ -226,10 +231,12 @@ TC_SHAPES = [
 ]
 
 
+@pytest.mark.parametrize("kernel", [rift.RIFT_KERNEL_TC, rift.RIFT_KERNEL_TCS])
 @pytest.mark.parametrize("shape", range(len(TC_SHAPES)))
-def test_tc_kernel_shapes(torch, oracle, shape):
+def test_tc_kernel_shapes(torch, oracle, shape, kernel):
     """Detector counts, mode counts (one or several mode-subset passes) and window lengths other than C0-C3's: every
-    (row tiles, pitch, pass) instantiation the plan can pick is compared with the oracle."""
+    (row tiles, pitch, pass) instantiation the plan can pick is compared with the oracle.  The shift-sorted variant exists
+    for two or more detectors and a single pass (K = 2: no exchange left; K = 4, 5: two and three exchanged detectors)."""
     dets, modes, f_s, t_w = TC_SHAPES[shape]
     cfg = synth.with_overrides(synth.CONFIGS[1], detectors=dets, modes=modes, f_s=f_s, t_window=t_w, n_points=2)
     inp = build(oracle, cfg, n_points=2)
@@ -238,10 +245,35 @@ def test_tc_kernel_shapes(torch, oracle, shape):
     params = np.concatenate([synth.draw_samples(cfg, 40 + s, n)[0] for s in range(len(ids))], axis=1)
     ref = np.concatenate([oracle_eval(oracle, inp, ids[s], params[:, s * n:(s + 1) * n])[0] for s in range(len(ids))])
     h = create(rift, inp, rift.RIFT_PREC_MIXED)
-    got, sh, _ = gpu_eval(torch, h, ids, n, params, K=cfg.n_det, kernel=rift.RIFT_KERNEL_TC)
-    assert "lnl_tc" in rift.rift_ile_kernel_name(h), rift.rift_ile_kernel_name(h)
-    assert ("passes" in rift.rift_ile_kernel_name(h)) == (len(modes) > 8)
+    got, sh, _ = gpu_eval(torch, h, ids, n, params, K=cfg.n_det, kernel=kernel)
+    name = rift.rift_ile_kernel_name(h)
+    assert "lnl_tc" in name, name
+    assert ("passes" in name) == (len(modes) > 8)
+    assert ("lnl_tcs" in name) == (kernel == rift.RIFT_KERNEL_TCS and len(dets) >= 2 and len(modes) <= 8), name
     assert np.max(np.abs(got.cpu().numpy() - ref)) < TOL_MIXED_LNL
+    rift.rift_ile_destroy(h)
+
+
+def test_tcs_chunks_across_segments(torch, oracle, monkeypatch):
+    """Shift-sorted variant with a small chunk workspace: chunks that start and end inside segments, several segments
+    per chunk, a ragged last batch in every segment; the default kernel choice picks the variant for segments this long."""
+    cfg = synth.CONFIGS[1]
+    inp = build(oracle, cfg, n_points=3)
+    n, ids = 3533, [2, 0, 1, 1, 0, 2, 0, 1, 2, 0, 1, 2]
+    params = np.concatenate([synth.draw_samples(cfg, 70 + s, n)[0] for s in range(len(ids))], axis=1)
+    h = create(rift, inp, rift.RIFT_PREC_MIXED)
+    monkeypatch.setenv("RIFT_TC_CHUNK_MIB", "1")              # raised to 8 batches per SM = 1184 batches = 5.4 segments
+    got, sh, _ = gpu_eval(torch, h, ids, n, params, K=cfg.n_det)
+    monkeypatch.delenv("RIFT_TC_CHUNK_MIB")
+    assert "lnl_tcs" in rift.rift_ile_kernel_name(h)
+    one, _, _ = gpu_eval(torch, h, ids, n, params, K=cfg.n_det, kernel=rift.RIFT_KERNEL_TC)
+    got, one = got.cpu().numpy(), one.cpu().numpy()
+    assert not np.isnan(got).any()
+    assert np.max(np.abs(got - one)) < TOL_MIXED_LNL          # against the unsorted tensor-core kernel, every sample
+    for s in (0, 5, 11):                                      # against the oracle, a subsample of three segments
+        sel = np.arange(0, n, 7)
+        ref = oracle_eval(oracle, inp, ids[s], params[:, s * n:(s + 1) * n][:, sel])[0]
+        assert np.max(np.abs(got[s * n:(s + 1) * n][sel] - ref)) < TOL_MIXED_LNL, s
     rift.rift_ile_destroy(h)
 
 
@@ -257,7 +289,7 @@ def test_guard_band_window(torch, oracle, kernel):
         h = create(rift, inp, prec, n_tau=n_tau)
         got = gpu_eval(torch, h, [0], 1500, params, K=cfg.n_det, kernel=kernel)[0].cpu().numpy()
         assert ("lnl_tc" in rift.rift_ile_kernel_name(h)) == (
-            prec == rift.RIFT_PREC_MIXED and kernel in (rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_TC))
+            prec == rift.RIFT_PREC_MIXED and kernel in TC_FAMILY)
         if tol is None:
             assert np.max(rel_err(got, ref)) < TOL_FP64_REL
         else:
