@@ -34,7 +34,7 @@ UNIT = "evals/s"
 N_SM, FP32_LANES, FP64_LANES = 148, 128, 64        # B200: guide unit counts (B200_PROFILING.md, B300_MICROARCH.md)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the fused kernel from the committed `ncu --set full` captures
 # (profiles/), keyed by (kernel, config index); a launch of lnl_tc on C1 = the whole step (1.6e6 evaluations).
-NCU_TRAFFIC_BYTES = {("lnl_tc<f16x3>", 1): 379.7e6, ("lnl_direct_ext<f32>", 1): 58.5e6}
+NCU_TRAFFIC_BYTES = {("lnl_tcs<f16x3>", 1): 396.7e6, ("lnl_tc<f16x3>", 1): 379.7e6, ("lnl_direct_ext<f32>", 1): 58.5e6}
 
 
 def measured_peaks() -> dict:

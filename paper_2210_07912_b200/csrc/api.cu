@@ -329,12 +329,14 @@ bool use_tc(const rift_ile *h) {
 }
 
 // Sorted variant: worth it when the padding of the shift buckets (about 8 slots per bucket and segment) stays small
-bool use_tcs(const rift_ile *h, int64_t n_per_seg) {
+bool use_tcs(const rift_ile *h, int32_t n_seg, int64_t n_per_seg) {
   if (!h->tc.srt_ok || h->d_Qs == nullptr) return false;
   if (h->kernel_variant == RIFT_KERNEL_TCS) return true;
   const char *e = getenv("RIFT_TC_SORT");                                // RIFT_TC_SORT=0: never pick it automatically
   const bool auto_on = !(e && atoi(e) == 0);
-  return auto_on && h->kernel_variant == RIFT_KERNEL_AUTO && n_per_seg >= 40 * (int64_t)h->tc.n_bkt;
+  // small calls are launch-bound and the bucketing adds five launches (C0: 0.10 -> 0.125 ms)
+  return auto_on && h->kernel_variant == RIFT_KERNEL_AUTO && n_per_seg >= 40 * (int64_t)h->tc.n_bkt &&
+         (int64_t)n_seg * n_per_seg >= 32768;
 }
 
 int ensure_tc_workspace(rift_ile *h, int64_t n_batches, int blob_words = 0) {
@@ -817,7 +819,7 @@ int rift_ile_eval_batch(rift_ile_t *h, int32_t n_seg, const int32_t *intrinsic_i
   cudaStream_t s = reinterpret_cast<cudaStream_t>(cuda_stream);
   int rc = upload_ids(h, n_seg, intrinsic_ids, s);
   if (rc != RIFT_OK) return rc;
-  if (use_tc(h) && use_tcs(h, n_per_seg)) return run_chunks_tcs(h, n_seg, n_per_seg, params, lnL_out, shift_out, s);
+  if (use_tc(h) && use_tcs(h, n_seg, n_per_seg)) return run_chunks_tcs(h, n_seg, n_per_seg, params, lnL_out, shift_out, s);
   if (use_tc(h)) return run_chunks_tc(h, n_seg, n_per_seg, params, lnL_out, shift_out, s);
   return run_chunks(h, n_seg, n_per_seg, params, lnL_out, shift_out, nullptr, nullptr, nullptr, s);
 }

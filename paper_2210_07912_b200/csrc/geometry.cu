@@ -255,10 +255,14 @@ geometry_tc_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, Tc
   const int64_t w0 = (int64_t)blockIdx.x * GEOM_THREADS;                    // first slot of the block
   if (w0 >= n_slots) return;
   int64_t seg_first = (ch.gb0 + w0 / RIFT_TC_NB) / ch.nbps;                 // segment of the block's first slot
-  if (sorted) {
-    int ls = 0;
-    while (ch.seg_begin[ls + 1] <= w0 / RIFT_TC_NB) ++ls;
-    seg_first = ch.gb0 / ch.nbps + ls;
+  if (sorted) {                                                             // last local segment that begins at or before the batch
+    const int32_t b = (int32_t)(w0 / RIFT_TC_NB);
+    int lo = 0, hi = ch.n_lseg - 1;
+    while (lo < hi) {
+      const int mid = (lo + hi + 1) >> 1;
+      if (ch.seg_begin[mid] <= b) lo = mid; else hi = mid - 1;
+    }
+    seg_first = ch.gb0 / ch.nbps + lo;
   }
   const int32_t point0 = ch.ids[seg_first];
   {
