@@ -42,6 +42,10 @@ int rift_ac_draw(rift_ac_t *h, int64_t n, uint64_t seed, uint64_t offset, double
  * 0 <= floor_mix <= 1, temper > 0. */
 int rift_ac_update(rift_ac_t *h, const double *hist, double floor_mix, double temper);
 
+/* The same with a per-dimension switch: adapt (HOST [n_dim], or NULL = all) != 0 refreshes the dimension, 0 keeps its current
+ * masses -- the "frozen" dimensions of a production run, which adapts the sky for a few rounds and then holds it (:452). */
+int rift_ac_update_dims(rift_ac_t *h, const double *hist, double floor_mix, double temper, const int32_t *adapt);
+
 /* Copy the current bin masses to masses (HOST [n_dim][n_bins]). */
 int rift_ac_get_masses(const rift_ac_t *h, double *masses);
 

@@ -28,8 +28,8 @@ EXPORTS = ("rift_ile_create", "rift_ile_eval_batch", "rift_ile_reduce", "rift_il
            "rift_ile_launch_count", "rift_ile_kernel_name", "rift_ile_profile", "rift_ile_profile_read",
            "rift_ile_fma_peak", "rift_ile_destroy",
            "rift_ile_strerror", "rift_ile_last_error")
-AC_EXPORTS = ("rift_ac_create", "rift_ac_draw", "rift_ac_update", "rift_ac_get_masses", "rift_ac_ile_ln_weight",
-              "rift_ac_destroy")
+AC_EXPORTS = ("rift_ac_create", "rift_ac_draw", "rift_ac_update", "rift_ac_update_dims", "rift_ac_get_masses",
+              "rift_ac_ile_ln_weight", "rift_ac_destroy")
 
 
 class RiftError(RuntimeError):
@@ -87,6 +87,8 @@ def lib() -> C.CDLL:
         L.rift_ac_draw.restype = C.c_int
         L.rift_ac_update.argtypes = [vp, vp, dbl, dbl]
         L.rift_ac_update.restype = C.c_int
+        L.rift_ac_update_dims.argtypes = [vp, vp, dbl, dbl, vp]
+        L.rift_ac_update_dims.restype = C.c_int
         L.rift_ac_get_masses.argtypes = [vp, vp]
         L.rift_ac_get_masses.restype = C.c_int
         L.rift_ac_ile_ln_weight.argtypes = [i64, C.POINTER(vp), dbl, dbl, vp, vp, vp]
@@ -255,6 +257,16 @@ def rift_ac_draw(h, n: int, seed: int, offset: int, x, ln_ps, cuda_stream: int =
 def rift_ac_update(h, hist, floor_mix: float, temper: float = 1.0) -> None:
     hist_ = np.ascontiguousarray(hist, dtype=np.float64)
     _check(lib().rift_ac_update(h, hist_.ctypes.data, float(floor_mix), float(temper)))
+
+
+def rift_ac_update_dims(h, hist, floor_mix: float, temper: float, adapt) -> None:
+    """adapt: one flag per dimension (0 keeps the dimension's current masses), or None for all."""
+    hist_ = np.ascontiguousarray(hist, dtype=np.float64)
+    adapt_ = None if adapt is None else np.ascontiguousarray(adapt, dtype=np.int32)
+    if adapt_ is not None and adapt_.size != hist_.shape[0]:
+        raise ValueError("adapt must have one entry per dimension")
+    _check(lib().rift_ac_update_dims(h, hist_.ctypes.data, float(floor_mix), float(temper),
+                                     None if adapt_ is None else adapt_.ctypes.data))
 
 
 def rift_ac_get_masses(h, n_dim: int, n_bins: int) -> np.ndarray:

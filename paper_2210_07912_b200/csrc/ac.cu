@@ -145,10 +145,15 @@ int rift_ac_draw(rift_ac_t *h, int64_t n, uint64_t seed, uint64_t offset, double
 }
 
 int rift_ac_update(rift_ac_t *h, const double *hist, double floor_mix, double temper) {
+  return rift_ac_update_dims(h, hist, floor_mix, temper, nullptr);
+}
+
+int rift_ac_update_dims(rift_ac_t *h, const double *hist, double floor_mix, double temper, const int32_t *adapt) {
   if (!h || !hist || !(floor_mix >= 0.0 && floor_mix <= 1.0) || !(temper > 0.0)) return RIFT_EINVAL;
   const int nd = h->n_dim, nb = h->n_bins;
   std::vector<double> t(nb);
   for (int d = 0; d < nd; ++d) {
+    if (adapt && !adapt[d]) continue;        // frozen dimension: keeps its masses
     double s = 0.0;
     for (int b = 0; b < nb; ++b) {
       const double v = hist[(size_t)d * nb + b];

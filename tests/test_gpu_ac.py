@@ -147,3 +147,43 @@ def test_rosenbrock_evidence_of_fig7_on_device(torch, oracle):
     rift.rift_ac_destroy(s)
     rift.rift_ile_destroy(h_round)
     rift.rift_ile_destroy(h_pool)
+
+
+def test_round_loop_sky_only_to_n_eff_target_then_frozen(torch, oracle):
+    """The production settings of :452 through paper_2210_07912_b200.ac_loop: rounds until the pooled n_eff reaches 10, only
+    the sky adapted (rift_ac_update_dims), then the same sampler frozen for a second pass, as a worker does for the later
+    points of its batch."""
+    from paper_2210_07912_b200 import ac_loop
+    cfg = synth.with_overrides(synth.CONFIGS[0], rho=6.0)
+    inp = build(oracle, cfg)
+    h = create(rift, inp, rift.RIFT_PREC_MIXED)
+    stream = torch.cuda.current_stream().cuda_stream
+    lo, hi, nb = synth.HIST_LO, synth.HIST_HI, 100
+    n_ref = 2_000_000
+    p_ref = torch.from_numpy(np.ascontiguousarray(synth.prior_draw(np.random.default_rng(123), n_ref))).cuda()
+    lnL = torch.empty(n_ref, dtype=torch.float64, device="cuda")
+    rift.rift_ile_eval_batch(h, [0], n_ref, p_ref, lnL, None, stream)
+    ref = rift.rift_ile_reduce(h, 1, n_ref, lnL, None, cuda_stream=stream)
+
+    s = rift.rift_ac_create(6, nb, lo, hi)
+    kw = dict(lo=lo, hi=hi, n_bins=nb, d_min_mpc=synth.D_MIN_MPC, d_max_mpc=synth.D_MAX_MPC, n_per_round=50_000,
+              n_eff_target=10.0, max_rounds=40, seed=452, cuda_stream=stream)
+    first = ac_loop.integrate(h, s, 0, adapt=ac_loop.SKY_ONLY, **kw)
+    assert first["n_eff"] >= 10.0 and first["rounds"] < 40, first
+    m = rift.rift_ac_get_masses(s, 6, nb)
+    assert np.allclose(m[2:], 1.0 / nb, atol=1e-15)                          # psi, iota, phi, D are not adapted
+    assert first["rounds"] == 1 or np.max(np.abs(m[:2] - 1.0 / nb)) > 1e-3   # the sky is
+    sigma = math.hypot(first["rel_err"], ref["rel_err"][0])
+    assert abs(first["lnZ"] - ref["lnZ"][0]) < 5 * sigma + 0.02, (first, ref)
+
+    frozen = ac_loop.integrate(h, s, 0, frozen=True, offset=first["next_offset"], **kw)
+    assert frozen["n_eff"] >= 10.0 and frozen["rounds"] < 40, frozen
+    assert np.array_equal(rift.rift_ac_get_masses(s, 6, nb), m)              # frozen: the sampler is left alone
+    sigma = math.hypot(frozen["rel_err"], ref["rel_err"][0])
+    assert abs(frozen["lnZ"] - ref["lnZ"][0]) < 5 * sigma + 0.02, (frozen, ref)
+    # equal cost under the prior gives n_eff = ref n_eff * n_evals / n_ref
+    assert frozen["n_eff"] > 1.5 * ref["n_eff"][0] * frozen["n_evals"] / n_ref, (frozen, ref)
+    with pytest.raises(ValueError):
+        rift.rift_ac_update_dims(s, m, 0.1, 1.0, [1, 0])
+    rift.rift_ac_destroy(s)
+    rift.rift_ile_destroy(h)

@@ -256,17 +256,24 @@ def test_tc_kernel_shapes(torch, oracle, shape, kernel):
 
 def test_tcs_chunks_across_segments(torch, oracle, monkeypatch):
     """Shift-sorted variant with a small chunk workspace: chunks that start and end inside segments, several segments
-    per chunk, a ragged last batch in every segment; the default kernel choice picks the variant for segments this long."""
+    per chunk, a ragged last batch in every segment; and the default kernel choice."""
     cfg = synth.CONFIGS[1]
     inp = build(oracle, cfg, n_points=3)
     n, ids = 3533, [2, 0, 1, 1, 0, 2, 0, 1, 2, 0, 1, 2]
     params = np.concatenate([synth.draw_samples(cfg, 70 + s, n)[0] for s in range(len(ids))], axis=1)
     h = create(rift, inp, rift.RIFT_PREC_MIXED)
     monkeypatch.setenv("RIFT_TC_CHUNK_MIB", "1")              # raised to 8 batches per SM = 1184 batches = 5.4 segments
-    got, sh, _ = gpu_eval(torch, h, ids, n, params, K=cfg.n_det)
+    got, sh, _ = gpu_eval(torch, h, ids, n, params, K=cfg.n_det, kernel=rift.RIFT_KERNEL_TCS)
     monkeypatch.delenv("RIFT_TC_CHUNK_MIB")
     assert "lnl_tcs" in rift.rift_ile_kernel_name(h)
     one, _, _ = gpu_eval(torch, h, ids, n, params, K=cfg.n_det, kernel=rift.RIFT_KERNEL_TC)
+    assert "lnl_tc<" in rift.rift_ile_kernel_name(h)
+    # the default choice: the sorted variant for calls of >= 32768 samples in segments of >= 100 samples per shift bucket
+    gpu_eval(torch, h, ids, n, params, K=cfg.n_det, kernel=rift.RIFT_KERNEL_AUTO)
+    assert "lnl_tc<" in rift.rift_ile_kernel_name(h)         # 3533 < 100 * 85
+    big = np.tile(params[:, :n], (1, 12))[:, :4 * 9000]
+    gpu_eval(torch, h, [0, 1, 2, 0], 9000, big, K=cfg.n_det)
+    assert "lnl_tcs" in rift.rift_ile_kernel_name(h)
     got, one = got.cpu().numpy(), one.cpu().numpy()
     assert not np.isnan(got).any()
     assert np.max(np.abs(got - one)) < TOL_MIXED_LNL          # against the unsorted tensor-core kernel, every sample
