@@ -305,7 +305,7 @@ void make_tc_plan(rift_ile *h, double delta_t) {
                     lnl_tc_smem_bytes(tp) <= 227u * 1024u;
   tp.ok = fits ? 1 : 0;
   // sorted variant: detector 1 fused by the tensor core (lnl_tcs.cu)
-  if (tp.ok && tp.n_sub == 1 && tp.K >= 2) {
+  if (tp.ok && tp.K >= 2) {
     int hs = 0;
     for (int k = 2; k < tp.K; ++k) hs = tp.dmax[k] > hs ? tp.dmax[k] : hs;
     tp.n_bkt = 2 * tp.dmax[1] + 1;
@@ -438,10 +438,11 @@ int run_chunks_tcs(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *
   const int64_t nbps = (n_per_seg + RIFT_TC_NB - 1) / RIFT_TC_NB;
   const int64_t total = (int64_t)n_seg * nbps;
   if (total == 0) return RIFT_OK;
-  const size_t per_batch = (size_t)tp.blob_words_s * 4 + (size_t)RIFT_TC_NB * (16 + 32 + 8);
+  const size_t per_batch = (size_t)tp.n_sub * tp.blob_words_s * 4 + (size_t)RIFT_TC_NB * (16 + 32 + 8);
   const int chunk_mib = tc_chunk_mib();
   int64_t cap = (int64_t)(((size_t)chunk_mib << 20) / per_batch);
   if (cap < 8 * (int64_t)h->n_sm) cap = 8 * (int64_t)h->n_sm;
+  if (tp.n_sub > 1 && cap < 65536) cap = 65536;                              // mode-subset passes: as in run_chunks_tc
   const int64_t nb_max = total < cap ? total : cap;
   int64_t lseg_max = nb_max / nbps + 2;
   if (lseg_max > n_seg) lseg_max = n_seg;
@@ -479,12 +480,25 @@ int run_chunks_tcs(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *
       ++nl;
       ps.end();
     }
+    c.xacc = h->tc_xacc;
     ProfSpan ps(h, 1, s);
-    CU(h, launch_lnl_tcs(tp, h->d_Qtc, h->d_Qs, c, lnL_out, h->n_sm, s, &nl));
+    if (tp.n_sub == 1) {
+      CU(h, launch_lnl_tcs(tp, h->d_Qtc, h->d_Qs, c, RIFT_TC_PASS_SINGLE, lnL_out, h->n_sm, s, &nl));
+    } else {
+      // one pass per mode subset: its own A operands and blobs ([sub][cap_sorted][blob_words_s]), window sums through tc_xacc
+      const size_t a_words = (size_t)h->P * h->K * tp.nt * 128 * tp.acols;
+      const size_t as_halfs = (size_t)h->P * (tp.kp >> 3) * tp.as_rows * 8;
+      for (int sub = 0; sub < tp.n_sub; ++sub) {
+        TcChunk cs = c;
+        cs.blob = h->tc_blob + (size_t)sub * c.cap_sorted * tp.blob_words_s;
+        const int pass = sub == 0 ? RIFT_TC_PASS_FIRST : (sub == tp.n_sub - 1 ? RIFT_TC_PASS_LAST : RIFT_TC_PASS_MIDDLE);
+        CU(h, launch_lnl_tcs(tp, h->d_Qtc + sub * a_words, h->d_Qs + sub * as_halfs, cs, pass, lnL_out, h->n_sm, s, &nl));
+      }
+    }
     ps.end();
     h->launches += nl;
   }
-  h->kernel_name = "lnl_tcs<f16x3>";
+  h->kernel_name = tp.n_sub == 1 ? "lnl_tcs<f16x3>" : "lnl_tcs<f16x3,passes>";
   return RIFT_OK;
 }
 
@@ -705,7 +719,7 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
         if (e == cudaSuccess) e = launch_convert_q_ext(src, h->d_Qe, rows, h->n_t, n_te, fp32, 0);
         qe.data = h->d_Qe;
         h->qse = qe;
-        ++h->launches;
+        h->launches += h->tc.n_sub;
       }
     }
     // planar, circularly extended copy for the grouped kernel, if one point's block fits in shared memory
@@ -735,7 +749,7 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
       if (e == cudaSuccess) e = launch_convert_q_tc(src, h->d_Qtc, h->d_qscale, h->tc, h->P, 0);
       h->launches += 3;
       if (e == cudaSuccess && h->tc.srt_ok) {
-        e = cudaMalloc(&h->d_Qs, (size_t)h->P * (h->tc.kp >> 3) * h->tc.as_rows * 8 * sizeof(uint16_t));
+        e = cudaMalloc(&h->d_Qs, (size_t)h->tc.n_sub * h->P * (h->tc.kp >> 3) * h->tc.as_rows * 8 * sizeof(uint16_t));
         if (e == cudaSuccess) e = launch_convert_q_tcs(src, h->d_Qs, h->d_qscale, h->tc, h->P, 0);
         ++h->launches;
       }

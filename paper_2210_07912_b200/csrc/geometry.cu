@@ -373,11 +373,23 @@ geometry_tcx_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, T
   constexpr int K = KT;
   constexpr int KP = (6 * MS + 15) & ~15, nch = KP / 8;
   const int M = g.n_modes;
-  const int64_t n_slots = ch.n_batches * RIFT_TC_NB;
+  const bool sorted = ch.key != nullptr;    // sorted variant: slots are the sorted slots, the sample comes through ch.perm
+  const int64_t n_slots = (sorted ? (int64_t)ch.seg_begin[ch.n_lseg] : ch.n_batches) * RIFT_TC_NB;
   // U, V of the block's (first) intrinsic point staged in shared memory when the launch provides room for them
   extern __shared__ double2 s_uv[];
   const int64_t w0 = (int64_t)blockIdx.x * GEOM_THREADS;
-  const int32_t point0 = ch.ids[(ch.gb0 + w0 / RIFT_TC_NB) / ch.nbps];
+  if (w0 >= n_slots) return;
+  int64_t seg_first = (ch.gb0 + w0 / RIFT_TC_NB) / ch.nbps;
+  if (sorted) {                                                             // last local segment that begins at or before the batch
+    const int32_t b = (int32_t)(w0 / RIFT_TC_NB);
+    int lo = 0, hi = ch.n_lseg - 1;
+    while (lo < hi) {
+      const int mid = (lo + hi + 1) >> 1;
+      if (ch.seg_begin[mid] <= b) lo = mid; else hi = mid - 1;
+    }
+    seg_first = ch.gb0 / ch.nbps + lo;
+  }
+  const int32_t point0 = ch.ids[seg_first];
   const int n_uv = K * M * M;
   if (stage_uv) {
     const double2 *u = reinterpret_cast<const double2 *>(U) + (int64_t)point0 * n_uv;
@@ -392,12 +404,15 @@ geometry_tcx_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, T
   if (w >= n_slots) return;
   const int64_t lb = w / RIFT_TC_NB;
   const int n = (int)(w % RIFT_TC_NB);
-  const int64_t gb = ch.gb0 + lb;
+  int64_t wn = w;                                                           // natural slot of the sample
+  if (sorted) wn = ch.perm[w];
+  const int64_t gb = ch.gb0 + wn / RIFT_TC_NB;
   const int64_t seg = gb / ch.nbps;
-  const int64_t i = (gb % ch.nbps) * RIFT_TC_NB + n;
-  const bool valid = i < ch.n_per_seg;
-  const size_t sub_stride = (size_t)ch.n_batches * tp.blob_words;           // floats between the blobs of two subsets
-  float *blob0 = ch.blob + lb * tp.blob_words;
+  const int64_t i = (gb % ch.nbps) * RIFT_TC_NB + (wn % RIFT_TC_NB);
+  const bool valid = wn >= 0 && i < ch.n_per_seg;
+  const int blob_words = sorted ? tp.blob_words_s : tp.blob_words;
+  const size_t sub_stride = (size_t)(sorted ? ch.cap_sorted : ch.n_batches) * blob_words;   // floats between the blobs of two subsets
+  float *blob0 = ch.blob + lb * blob_words;
   if (!valid) {
     for (int sub = 0; sub < tp.n_sub; ++sub) {
       float *blob = blob0 + sub * sub_stride;
@@ -434,6 +449,10 @@ geometry_tcx_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, T
     float *blob = blob0 + sub * sub_stride;
     int32_t *dsh = reinterpret_cast<int32_t *>(blob + K * nch * 64);
     blob[K * nch * 64 + K * 16 + n] = cl2v;
+    if (sorted && n == 0) {                                                 // batch header: the common d_1 (clamped as the key)
+      const int dm = tp.dmax[1], d = shift[KT > 1 ? 1 : 0] - shift[0];
+      reinterpret_cast<int32_t *>(blob + K * nch * 64 + K * 16 + 16)[0] = d < -dm ? -dm : (d > dm ? dm : d);
+    }
     for (int k = 0; k < K; ++k) {
       dsh[k * 16 + n] = (k == 0) ? tp.j0 + shift[0] : shift[k] - shift[0];
       uint16_t hv[KP];

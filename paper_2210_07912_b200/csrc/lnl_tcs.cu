@@ -28,7 +28,9 @@ struct TcsArgs {
   const uint16_t *qs;            // [P][kp/8][as_rows][8] fp16: extended detector-1 operand
 };
 
-template <int NT, int PITCH, bool GUARD>
+// PASS = RIFT_TC_PASS_* as in lnl_tc.cu: with the modes split into subsets, every pass but the last writes its window sums
+// x[t, n] to global memory instead of reducing them, every pass but the first adds the sums of the pass before.
+template <int NT, int PITCH, bool GUARD, int PASS>
 __global__ void __launch_bounds__(TC_THREADS, 1) lnl_tcs_kernel(const TcsArgs args) {
   const TcPlan &tp = args.tp;
   const TcChunk &ch = args.ch;
@@ -238,7 +240,15 @@ __global__ void __launch_bounds__(TC_THREADS, 1) lnl_tcs_kernel(const TcsArgs ar
         if (lane == 0) mbar_arrive(bar_tempty);                            // the UMMAs of the next batch may overwrite D
       };
       // Phase B: shifted sum over the exchanged detectors
-      auto phase_b = [&](uint32_t g, float (&x)[NT][NH]) {
+      auto phase_b = [&](uint32_t g, int64_t lb, float (&x)[NT][NH]) {
+        float xp[NT][NH];
+        if constexpr (PASS == RIFT_TC_PASS_MIDDLE || PASS == RIFT_TC_PASS_LAST) {   // in flight under the exchange reads
+          const float *src = ch.xacc + ((size_t)(lb * RIFT_TC_NB + NH * wg)) * (NT * 128) + T;
+#pragma unroll
+          for (int n = 0; n < NH; ++n)
+#pragma unroll
+            for (int i = 0; i < NT; ++i) xp[i][n] = __ldcs(src + (size_t)n * (NT * 128) + 128 * i);
+        }
         const float *blob = blob_s + (g % TC_STAGES) * BW;
         const float *xb = xb_s + (size_t)((wg * 2 + (g & 1u)) * (K - 2)) * NH * PITCH;
         const int32_t *dsh = reinterpret_cast<const int32_t *>(blob + K * tp.nch * 64) + NH * wg;
@@ -254,9 +264,25 @@ __global__ void __launch_bounds__(TC_THREADS, 1) lnl_tcs_kernel(const TcsArgs ar
             x[NT - 1][n] += src[128 * (NT - 1) + last_clamp];
           }
         }
+        if constexpr (PASS == RIFT_TC_PASS_MIDDLE || PASS == RIFT_TC_PASS_LAST) {
+#pragma unroll
+          for (int n = 0; n < NH; ++n)
+#pragma unroll
+            for (int i = 0; i < NT; ++i) x[i][n] += xp[i][n];
+        }
       };
       // per-warp (reference, sum) of the time marginal for the 8 samples of batch g (sorted batch index lb)
       auto reduce = [&](uint32_t g, int64_t lb, float (&x)[NT][NH]) {
+        if constexpr (PASS == RIFT_TC_PASS_FIRST || PASS == RIFT_TC_PASS_MIDDLE) {   // hand the window sums to the next pass
+          float *dst = ch.xacc + ((size_t)(lb * RIFT_TC_NB + NH * wg)) * (NT * 128) + T;
+#pragma unroll
+          for (int n = 0; n < NH; ++n)
+#pragma unroll
+            for (int i = 0; i < NT; ++i) __stcs(dst + (size_t)n * (NT * 128) + 128 * i, x[i][n]);
+          __syncwarp();
+          if (lane == 0) mbar_arrive(bar_empty + g % TC_STAGES);
+          return;
+        }
         const uint32_t stage = g % TC_STAGES;
         const float *blob = blob_s + stage * BW;
         const float *cl2s = blob + K * tp.nch * 64 + K * 16 + NH * wg;
@@ -314,7 +340,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) lnl_tcs_kernel(const TcsArgs ar
         const uint32_t g = it + j;
         if (K > 2) named_bar_sync(1 + wg, 128);                            // exchange rows of batch g are complete
         mbar_wait(bar_full + g % TC_STAGES, (g / TC_STAGES) & 1u);         // shifts and exponent scales of batch g
-        phase_b(g, x);
+        phase_b(g, b0 + j, x);
         if (j + 1 < nb) {
           mbar_wait(bar_tfull, (g + 1u) & 1u);
           tc_fence_after();
@@ -364,8 +390,8 @@ __global__ void lnl_tcs_finalize_kernel(TcPlan tp, TcChunk ch, double *__restric
 // Q [P][K][M][n_t] complex128, detector 1  ->  [P][kp/8][as_rows][8] fp16: row r holds time (r - dmax_1) mod n_t for
 // r < n_t + 2 dmax_1 (zero beyond), contraction index kappa' = 8 plane + e over [Q_hi | Q_lo | Q_hi] as in convert_q_tc_kernel.
 __global__ void convert_q_tcs_kernel(const double2 *__restrict__ src, uint16_t *__restrict__ dst, const float *__restrict__ scale,
-                                     TcPlan tp, int64_t total) {
-  const int ms = tp.m_sub, planes = tp.kp >> 3, dm = tp.dmax[1];
+                                     TcPlan tp, int sub, int64_t total) {
+  const int ms = tp.m_sub, planes = tp.kp >> 3, dm = tp.dmax[1], a0 = sub * tp.m_sub;   // modes [a0, a0 + ms) of this subset
   for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
     const int e = (int)(idx & 7);
     const int64_t r64 = idx >> 3;
@@ -374,7 +400,7 @@ __global__ void convert_q_tcs_kernel(const double2 *__restrict__ src, uint16_t *
     const int64_t p = r64 / tp.as_rows / planes;
     const int kp_i = 8 * c + e;
     const int part = kp_i / (2 * ms), kap = kp_i % (2 * ms);
-    const int a = kap >> 1;
+    const int a = a0 + (kap >> 1);
     uint16_t out = 0;
     if (r < tp.n_t + 2 * dm && part < 3 && a < tp.M) {
       int t = (r - dm) % tp.n_t;
@@ -389,10 +415,19 @@ __global__ void convert_q_tcs_kernel(const double2 *__restrict__ src, uint16_t *
 }
 
 template <int NT>
-cudaError_t launch_nt(const TcsArgs &a, unsigned grid, size_t smem, cudaStream_t s) {
+cudaError_t launch_nt(const TcsArgs &a, int pass, unsigned grid, size_t smem, cudaStream_t s) {
 #define RIFT_TCS_CASE(P)                                                                                         \
   case P: {                                                                                                      \
-    void (*kern)(TcsArgs) = a.tp.n_tau < a.tp.n_t ? lnl_tcs_kernel<NT, P, true> : lnl_tcs_kernel<NT, P, false>;   \
+    void (*kern)(TcsArgs) = nullptr;                                                                             \
+    if (a.tp.n_tau < a.tp.n_t) {                                                                                 \
+      if (pass != RIFT_TC_PASS_SINGLE) return cudaErrorInvalidValue;                                             \
+      kern = lnl_tcs_kernel<NT, P, true, RIFT_TC_PASS_SINGLE>;                                                   \
+    } else {                                                                                                     \
+      kern = pass == RIFT_TC_PASS_SINGLE  ? lnl_tcs_kernel<NT, P, false, RIFT_TC_PASS_SINGLE>                    \
+             : pass == RIFT_TC_PASS_FIRST ? lnl_tcs_kernel<NT, P, false, RIFT_TC_PASS_FIRST>                     \
+             : pass == RIFT_TC_PASS_MIDDLE ? lnl_tcs_kernel<NT, P, false, RIFT_TC_PASS_MIDDLE>                   \
+                                           : lnl_tcs_kernel<NT, P, false, RIFT_TC_PASS_LAST>;                    \
+    }                                                                                                            \
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);          \
     if (e != cudaSuccess) return e;                                                                              \
     kern<<<grid, TC_THREADS, smem, s>>>(a);                                                                      \
@@ -417,16 +452,18 @@ size_t lnl_tcs_smem_bytes(const TcPlan &tp) {
 
 cudaError_t launch_convert_q_tcs(const double *Q_c128, uint16_t *dst, const float *qscale, const TcPlan &tp,
                                  int32_t n_points, cudaStream_t s) {
-  const int64_t total = (int64_t)n_points * (tp.kp >> 3) * tp.as_rows * 8;
+  const int64_t total = (int64_t)n_points * (tp.kp >> 3) * tp.as_rows * 8;   // per mode subset
   if (total <= 0) return cudaSuccess;
   int64_t grid = (total + 255) / 256;
   if (grid > 148 * 32) grid = 148 * 32;
-  convert_q_tcs_kernel<<<(unsigned)grid, 256, 0, s>>>(reinterpret_cast<const double2 *>(Q_c128), dst, qscale, tp, total);
+  for (int sub = 0; sub < tp.n_sub; ++sub)
+    convert_q_tcs_kernel<<<(unsigned)grid, 256, 0, s>>>(reinterpret_cast<const double2 *>(Q_c128), dst + (size_t)sub * total,
+                                                        qscale, tp, sub, total);
   return cudaGetLastError();
 }
 
-cudaError_t launch_lnl_tcs(const TcPlan &tp, const uint32_t *qtc, const uint16_t *qs, const TcChunk &c, double *lnL_out,
-                           int n_sm, cudaStream_t s, int *n_launch) {
+cudaError_t launch_lnl_tcs(const TcPlan &tp, const uint32_t *qtc, const uint16_t *qs, const TcChunk &c, int pass,
+                           double *lnL_out, int n_sm, cudaStream_t s, int *n_launch) {
   if (c.n_batches <= 0) return cudaSuccess;
   const size_t smem = lnl_tcs_smem_bytes(tp);
   TcsArgs a;
@@ -438,15 +475,17 @@ cudaError_t launch_lnl_tcs(const TcPlan &tp, const uint32_t *qtc, const uint16_t
   if (grid > c.n_batches) grid = c.n_batches;
   cudaError_t e;
   switch (tp.nt) {
-    case 1: e = launch_nt<1>(a, (unsigned)grid, smem, s); break;
-    case 2: e = launch_nt<2>(a, (unsigned)grid, smem, s); break;
-    case 3: e = launch_nt<3>(a, (unsigned)grid, smem, s); break;
-    case 4: e = launch_nt<4>(a, (unsigned)grid, smem, s); break;
+    case 1: e = launch_nt<1>(a, pass, (unsigned)grid, smem, s); break;
+    case 2: e = launch_nt<2>(a, pass, (unsigned)grid, smem, s); break;
+    case 3: e = launch_nt<3>(a, pass, (unsigned)grid, smem, s); break;
+    case 4: e = launch_nt<4>(a, pass, (unsigned)grid, smem, s); break;
     default: e = cudaErrorInvalidValue;
   }
   if (e != cudaSuccess) return e;
+  if (n_launch) ++*n_launch;
+  if (pass == RIFT_TC_PASS_FIRST || pass == RIFT_TC_PASS_MIDDLE) return cudaSuccess;   // lnL is assembled after the last pass
   const int64_t n = c.cap_sorted * RIFT_TC_NB;
   lnl_tcs_finalize_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(tp, c, lnL_out);
-  if (n_launch) *n_launch += 2;
+  if (n_launch) ++*n_launch;
   return cudaGetLastError();
 }

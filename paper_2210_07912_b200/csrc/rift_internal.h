@@ -142,11 +142,11 @@ cudaError_t launch_lnl_tc(const TcPlan &tp, const uint32_t *qtc, const TcChunk &
 // lnl_tcs.cu (sorted variant: detector 1 fused into detector 0 by the tensor core; geometry.cu holds the bucket kernels)
 size_t lnl_tcs_smem_bytes(const TcPlan &tp);
 cudaError_t launch_convert_q_tcs(const double *Q_c128, uint16_t *dst, const float *qscale, const TcPlan &tp,
-                                 int32_t n_points, cudaStream_t s);   // dst: [P][kp/8][as_rows][8] fp16, detector 1
+                                 int32_t n_points, cudaStream_t s);   // dst: [n_sub][P][kp/8][as_rows][8] fp16, detector 1
 cudaError_t launch_tcs_buckets(const DetGeom &g, const TcPlan &tp, const TcChunk &c, const double *const params[6],
                                cudaStream_t s, int *n_launch);        // key, pos, count, base, seg_begin, perm
-cudaError_t launch_lnl_tcs(const TcPlan &tp, const uint32_t *qtc, const uint16_t *qs, const TcChunk &c, double *lnL_out,
-                           int n_sm, cudaStream_t s, int *n_launch);
+cudaError_t launch_lnl_tcs(const TcPlan &tp, const uint32_t *qtc, const uint16_t *qs, const TcChunk &c, int pass,
+                           double *lnL_out, int n_sm, cudaStream_t s, int *n_launch);
 // lnl_tile.cu (fp64 register-tiled contraction + shared-memory exchange; circular mode, n_t <= 512)
 size_t lnl_tile_smem_bytes(const QStore &q, int K, int pitch);
 cudaError_t launch_lnl_tile(const QStore &q, const Batch &b, const Workspace &ws, int K, int H, int pitch, const int *dmax,

@@ -236,7 +236,7 @@ TC_SHAPES = [
 def test_tc_kernel_shapes(torch, oracle, shape, kernel):
     """Detector counts, mode counts (one or several mode-subset passes) and window lengths other than C0-C3's: every
     (row tiles, pitch, pass) instantiation the plan can pick is compared with the oracle.  The shift-sorted variant exists
-    for two or more detectors and a single pass (K = 2: no exchange left; K = 4, 5: two and three exchanged detectors)."""
+    for two or more detectors (K = 2: no exchange left; K = 4, 5: two and three exchanged detectors), single- and multi-pass."""
     dets, modes, f_s, t_w = TC_SHAPES[shape]
     cfg = synth.with_overrides(synth.CONFIGS[1], detectors=dets, modes=modes, f_s=f_s, t_window=t_w, n_points=2)
     inp = build(oracle, cfg, n_points=2)
@@ -249,7 +249,7 @@ def test_tc_kernel_shapes(torch, oracle, shape, kernel):
     name = rift.rift_ile_kernel_name(h)
     assert "lnl_tc" in name, name
     assert ("passes" in name) == (len(modes) > 8)
-    assert ("lnl_tcs" in name) == (kernel == rift.RIFT_KERNEL_TCS and len(dets) >= 2 and len(modes) <= 8), name
+    assert ("lnl_tcs" in name) == (kernel == rift.RIFT_KERNEL_TCS and len(dets) >= 2), name
     assert np.max(np.abs(got.cpu().numpy() - ref)) < TOL_MIXED_LNL
     rift.rift_ile_destroy(h)
 
