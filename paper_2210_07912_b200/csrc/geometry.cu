@@ -240,7 +240,7 @@ geometry_kernel(DetGeom g, const ModeEntry *__restrict__ modes, Batch b, const d
 // and nothing is predicated on k < K).  The mode tables and the U, V blocks of the block's (first) intrinsic point are
 // staged in shared memory.
 template <int MT, int KT>
-__global__ void __launch_bounds__(GEOM_THREADS)
+__global__ void __launch_bounds__(GEOM_THREADS, 5)
 geometry_tc_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, TcChunk ch, const double *__restrict__ p_ra,
                    const double *__restrict__ p_dec, const double *__restrict__ p_psi, const double *__restrict__ p_iota,
                    const double *__restrict__ p_phi, const double *__restrict__ p_dist, const double *__restrict__ U,
