@@ -113,7 +113,11 @@ int rift_ile_reduce(rift_ile_t *h, int32_t n_seg, int64_t n_per_seg, const doubl
 int rift_ile_geometry(rift_ile_t *h, int32_t intrinsic_id, int64_t n, const double *const params[RIFT_N_PARAMS],
                       void *F, void *Y, int32_t *shift, double *quad, void *cuda_stream);
 
-/* Choose the fused-lnL kernel variant (RIFT_KERNEL_*); AUTO picks per configuration. */
+/* Choose the fused-lnL kernel variant (RIFT_KERNEL_*); AUTO picks per configuration and call size: in mixed precision the
+ * tensor-core kernels (TCS, which buckets the samples by the relative shift of detector 1, for calls of >= 32768 samples in
+ * segments of >= 100 samples per bucket; else TC) when the configuration fits tensor and shared memory, else the direct
+ * kernels; GROUPED, QUAD, TILE are opt-in.  A variant that does not apply to the handle falls back to the AUTO choice.
+ * lnL does not depend on the variant beyond the stated tolerance of the precision mode. */
 int rift_ile_set_kernel(rift_ile_t *h, int32_t variant);
 
 /* Number of kernels launched by this handle since creation (bench.py's gpu_launches), and the name of
