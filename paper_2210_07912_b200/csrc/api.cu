@@ -1,5 +1,6 @@
 // C ABI of librift_ile.so (include/rift_ile.h): handle management, argument validation, chunking, launches.
 // Host logic only -- every step of the hot path runs in the kernels of geometry.cu, lnl_*.cu and reduce.cu.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -17,6 +18,7 @@ struct rift_ile {
   ModeEntry *d_modes = nullptr;
   void *d_Q = nullptr;
   double *d_U = nullptr, *d_V = nullptr;
+  QuadProg qp{};                   // pair program of the quadratic term (M > 8), device tables owned by the handle
   QStore qs{};
   void *d_Qe = nullptr;            // interleaved, circularly extended copy for the direct_ext kernel (NULL if too big)
   QStore qse{};
@@ -172,6 +174,8 @@ void free_handle(rift_ile *h) {
   cudaFree(h->d_perm);
   cudaFree(h->d_hist);
   cudaFree(h->ws.orig);
+  cudaFree(const_cast<uint32_t *>(h->qp.ent_full));
+  cudaFree(const_cast<double2 *>(h->qp.uv));
   cudaFree(h->d_U);
   cudaFree(h->d_V);
   cudaFree(h->ws.coef);
@@ -395,7 +399,7 @@ int run_chunks_tc(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *c
     c.xacc = h->tc_xacc;
     {
       ProfSpan ps(h, 0, s);
-      CU(h, launch_geometry_tc(h->geom, h->d_modes, h->tc, c, params, h->d_U, h->d_V, shift_out, s));
+      CU(h, launch_geometry_tc(h->geom, h->d_modes, h->tc, c, params, h->d_U, h->d_V, h->qp, shift_out, s));
       ps.end();
     }
     ++h->launches;
@@ -476,7 +480,7 @@ int run_chunks_tcs(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *
     {
       ProfSpan ps(h, 0, s);
       CU(h, launch_tcs_buckets(h->geom, tp, c, params, s, &nl));
-      CU(h, launch_geometry_tc(h->geom, h->d_modes, tp, c, params, h->d_U, h->d_V, shift_out, s));
+      CU(h, launch_geometry_tc(h->geom, h->d_modes, tp, c, params, h->d_U, h->d_V, h->qp, shift_out, s));
       ++nl;
       ps.end();
     }
@@ -551,7 +555,7 @@ int run_chunks(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *cons
     }
     {
       ProfSpan ps(h, 0, s);
-      CU(h, launch_geometry(h->geom, h->d_modes, b, params, h->d_U, h->d_V, fp32, ws, shift_out, dbg_F, dbg_Y, perm, s));
+      CU(h, launch_geometry(h->geom, h->d_modes, b, params, h->d_U, h->d_V, h->qp, fp32, ws, shift_out, dbg_F, dbg_Y, perm, s));
       ps.end();
     }
     ++h->launches;
@@ -687,6 +691,49 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
   CUC(cudaMalloc(&h->d_V, uv_bytes));
   CUC(cudaMemcpy(h->d_U, cfg->U, uv_bytes, kind));
   CUC(cudaMemcpy(h->d_V, cfg->V, uv_bytes, kind));
+  if (h->M > 8 && !getenv("RIFT_NO_QUAD_PROG")) {
+    // pair program of the quadratic term (QuadProg, rift_internal.h): entries grouped by matrix and phase exponent
+    const int M = h->M;
+    int n_max = 0;
+    for (int a = 0; a < M; ++a) n_max = std::max(n_max, 2 * std::abs(cfg->mode_m[a]));
+    std::vector<uint32_t> ent;
+    std::vector<int4> bins;
+    auto add_bin = [&](int matrix, int n, int zstep) {
+      const int first = (int)ent.size();
+      for (int a = 0; a < M; ++a)
+        for (int b = a; b < M; ++b) {
+          const int ma = cfg->mode_m[a], mb = cfg->mode_m[b];
+          if (matrix == 0) {
+            if (std::abs(mb - ma) == n) ent.push_back((uint32_t)a | (uint32_t)b << 8 | (mb < ma ? 1u << 17 : 0u));
+          } else if (ma + mb == n) {
+            ent.push_back((uint32_t)a | (uint32_t)b << 8 | 1u << 16);
+          }
+        }
+      bins.push_back(make_int4(first, (int)ent.size(), matrix, zstep));
+    };
+    for (int n = 0; n <= n_max; ++n) add_bin(0, n, n == 0 ? 0 : 1);
+    for (int n = 0; n <= n_max; ++n) add_bin(1, n, n == 0 ? 0 : 1);
+    for (int n = 1; n <= n_max; ++n) add_bin(1, -n, n == 1 ? 2 : 3);
+    if (ent.size() <= RIFT_QP_MAX_ENT && bins.size() <= RIFT_QP_MAX_BINS) {
+      h->qp.n_entries = (int32_t)ent.size();
+      h->qp.n_bins = (int32_t)bins.size();
+      for (size_t e = 0; e < ent.size(); ++e) h->qp.ent[e] = (uint16_t)((ent[e] & 0x7fu) | ((ent[e] >> 8) & 0x7fu) << 7);
+      for (size_t i = 0; i < bins.size(); ++i) {
+        h->qp.bin_begin[i] = (uint16_t)bins[i].x;
+        h->qp.bin_kind[i] = (uint8_t)(bins[i].z | bins[i].w << 1);
+      }
+      h->qp.bin_begin[bins.size()] = (uint16_t)ent.size();
+      uint32_t *d_ent = nullptr;
+      double2 *d_uv = nullptr;
+      CUC(cudaMalloc(&d_ent, ent.size() * sizeof(uint32_t)));
+      h->qp.ent_full = d_ent;
+      CUC(cudaMemcpy(d_ent, ent.data(), ent.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
+      CUC(cudaMalloc(&d_uv, (size_t)h->P * ent.size() * h->K * sizeof(double2)));
+      CUC(launch_build_quad_uv(h->qp, h->d_U, h->d_V, h->P, h->K, h->M, d_uv, 0));
+      CUC(cudaStreamSynchronize(0));
+      h->qp.uv = d_uv;
+    }
+  }
   {
     const bool fp32 = cfg->q_storage == RIFT_Q_C64;
     const int64_t rows = (int64_t)h->P * h->K * h->M;

@@ -23,12 +23,15 @@ __device__ __forceinline__ double ipow4(double p1, double p2, double p4, double 
 
 // a1-a4 for one sample.  Outputs: shifts s_k, F_k, Y_lm (arrays sized by the caller), c = D_ref/D (NaN for an invalid
 // sample) and the quadratic term q.  `modes` and `Up`/`Vp` (the point's [K][M][M] blocks) may live in shared memory.
-template <int MAXM, int MAXK>
+// QUAD = false leaves a4 to quad_prog (below): q_out is 0, the real amplitudes d_a of Y_a = d_a z^{m_a} go to
+// amp_s[a * GEOM_THREADS] (the thread's column of a shared-memory array) and z = e^{-i phi} to z_out[0..1].
+template <int MAXM, int MAXK, bool QUAD = true>
 __device__ __forceinline__ void sample_geometry(const DetGeom &g, const ModeEntry *__restrict__ modes, double ra, double dec,
                                                 double psi, double iota, double phi, double dist,
                                                 const double2 *__restrict__ Up, const double2 *__restrict__ Vp,
                                                 int32_t (&shift)[MAXK], double (&Fre)[MAXK], double (&Fim)[MAXK],
-                                                double (&Yre)[MAXM], double (&Yim)[MAXM], double &c_out, double &q_out) {
+                                                double (&Yre)[MAXM], double (&Yim)[MAXM], double &c_out, double &q_out,
+                                                double *amp_s = nullptr, double *z_out = nullptr) {
   const int K = g.n_det, M = g.n_modes;
   const int m_end = (MAXM <= 16) ? MAXM : M;        // unrolled (and predicated on a < M) for small MAXM, runtime bound else
   double sd, cd, sh, ch, sp, cp;
@@ -79,6 +82,7 @@ __device__ __forceinline__ void sample_geometry(const DetGeom &g, const ModeEntr
     const double s2 = s1 * s1, s4 = s2 * s2, s8 = s4 * s4;
     sincos(phi, &s2h, &c2h);
     const double z1r = c2h, z1i = -s2h;                                   // z = e^{-i phi}
+    if constexpr (!QUAD) z_out[0] = z1r, z_out[1] = z1i;
     const double z2r = z1r * z1r - z1i * z1i, z2i = 2.0 * z1r * z1i;
     const double z4r = z2r * z2r - z2i * z2i, z4i = 2.0 * z2r * z2i;
     const double z8r = z4r * z4r - z4i * z4i, z8i = 2.0 * z4r * z4i;
@@ -117,6 +121,7 @@ __device__ __forceinline__ void sample_geometry(const DetGeom &g, const ModeEntr
         // e^{i m (-phi)} = z^m (m >= 0) or conj(z^|m|) (m < 0)
         Yre[a] = amp * wr;
         Yim[a] = (e.m < 0) ? -amp * wi : amp * wi;
+        if constexpr (!QUAD) amp_s[a * GEOM_THREADS] = amp;
       }
     }
   }
@@ -124,7 +129,9 @@ __device__ __forceinline__ void sample_geometry(const DetGeom &g, const ModeEntr
   const bool bad = !(dist > 0.0) || isnan(ra) || isnan(dec) || isnan(psi) || isnan(iota) || isnan(phi);
   const double c = bad ? __longlong_as_double(0x7ff8000000000000LL) : g.d_ref / dist;
   c_out = c;
-
+  if constexpr (!QUAD) {
+    q_out = 0.0;
+  } else {
   // ---- a4: quadratic term; U Hermitian, V symmetric: diagonal + 2 * strict upper triangle.  The mode-pair products
   // conj(Y_a) Y_b and Y_a Y_b do not depend on the detector and are formed once.
   double yuy[MAXK], yvr[MAXK], yvi[MAXK];
@@ -164,6 +171,104 @@ __device__ __forceinline__ void sample_geometry(const DetGeom &g, const ModeEntr
     }
   }
   q_out = 0.25 * c * c * q;
+  }
+}
+
+// ---- a4 by the pair program (QuadProg, rift_internal.h).  Shared-memory image of one intrinsic point:
+// [n_entries][KT] double2 W | [M][GEOM_THREADS] double amplitudes.  The entry and bin tables are kernel parameters
+// (constant bank, uniform loads): entry e is warp-uniform, so its W is a broadcast read and only the two amplitudes
+// are per-thread.
+struct QuadSmem {
+  size_t uv, amp, total;
+};
+__host__ __device__ inline QuadSmem quad_smem(int n_entries, int K, int M) {
+  QuadSmem L;
+  L.uv = 0;
+  L.amp = (size_t)n_entries * K * sizeof(double2);
+  L.total = L.amp + (size_t)M * GEOM_THREADS * sizeof(double);
+  return L;
+}
+
+__device__ __forceinline__ void quad_stage(const QuadProg &qp, int K, int32_t point, double2 *uv_s) {
+  const double2 *src = qp.uv + (size_t)point * qp.n_entries * K;
+  for (int i = threadIdx.x; i < qp.n_entries * K; i += GEOM_THREADS) uv_s[i] = src[i];
+}
+
+// q / (c^2 / 4) = sum_k |F_k|^2 Y^dag U_k Y + Re(F_k^2 Y^T V_k Y).  `uv` is the point's W block (shared or global memory),
+// `amp` the thread's amplitude column (stride GEOM_THREADS), z = e^{-i phi}.
+template <int KT>
+__device__ __forceinline__ double quad_prog(const QuadProg &qp, const double2 *__restrict__ uv, const double *__restrict__ amp,
+                                            double z1r, double z1i, const double (&Fre)[KT], const double (&Fim)[KT]) {
+  double yuy[KT], yvr[KT], yvi[KT];
+#pragma unroll
+  for (int k = 0; k < KT; ++k) yuy[k] = yvr[k] = yvi[k] = 0.0;
+  double zr = 1.0, zi = 0.0;
+#pragma unroll 1
+  for (int bi = 0; bi < qp.n_bins; ++bi) {
+    const int kind = qp.bin_kind[bi], zstep = kind >> 1;
+    if (zstep == 0) {
+      zr = 1.0, zi = 0.0;
+    } else if (zstep == 2) {
+      zr = z1r, zi = -z1i;
+    } else {
+      const double si = (zstep == 1) ? z1i : -z1i;
+      const double t = zr * z1r - zi * si;
+      zi = zr * si + zi * z1r;
+      zr = t;
+    }
+    double Sr[KT], Si[KT];
+#pragma unroll
+    for (int k = 0; k < KT; ++k) Sr[k] = Si[k] = 0.0;
+    const int e1 = qp.bin_begin[bi + 1];
+#pragma unroll 4
+    for (int e = qp.bin_begin[bi]; e < e1; ++e) {
+      const uint32_t ab = qp.ent[e];
+      const double w = amp[(ab & 0x7fu) * GEOM_THREADS] * amp[(ab >> 7) * GEOM_THREADS];
+      const double2 *u = uv + e * KT;
+#pragma unroll
+      for (int k = 0; k < KT; ++k) {
+        const double2 uk = u[k];
+        Sr[k] = fma(w, uk.x, Sr[k]);
+        Si[k] = fma(w, uk.y, Si[k]);
+      }
+    }
+    if ((kind & 1) == 0) {
+#pragma unroll
+      for (int k = 0; k < KT; ++k) yuy[k] += zr * Sr[k] - zi * Si[k];
+    } else {
+#pragma unroll
+      for (int k = 0; k < KT; ++k) {
+        yvr[k] += zr * Sr[k] - zi * Si[k];
+        yvi[k] += zr * Si[k] + zi * Sr[k];
+      }
+    }
+  }
+  double q = 0.0;
+#pragma unroll
+  for (int k = 0; k < KT; ++k) {
+    const double f2 = Fre[k] * Fre[k] + Fim[k] * Fim[k];
+    const double f2r = Fre[k] * Fre[k] - Fim[k] * Fim[k], f2i = 2.0 * Fre[k] * Fim[k];
+    q += f2 * yuy[k] + (f2r * yvr[k] - f2i * yvi[k]);
+  }
+  return q;
+}
+
+// W of every (point, entry, detector) from the handle's U, V copies ([P][K][M][M] complex128)
+__global__ void build_quad_uv_kernel(const __grid_constant__ QuadProg qp, const double2 *__restrict__ U, const double2 *__restrict__ V, int P, int K,
+                                     int M, double2 *__restrict__ out) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t total = (int64_t)P * qp.n_entries * K;
+  if (i >= total) return;
+  const int k = (int)(i % K);
+  const int e = (int)((i / K) % qp.n_entries);
+  const int64_t p = i / ((int64_t)K * qp.n_entries);
+  const uint32_t w = qp.ent_full[e];
+  const int a = w & 0xffu, b = (w >> 8) & 0xffu;
+  const double2 *src = ((w >> 16) & 1u) ? V : U;
+  double2 v = src[((p * K + k) * M + a) * M + b];
+  if ((w >> 17) & 1u) v.y = -v.y;
+  const double f = (a == b) ? 1.0 : 2.0;
+  out[i] = make_double2(f * v.x, f * v.y);
 }
 
 // CT = coefficient type; MAXM = 8 (mode loops unrolled, Y in registers) or RIFT_MAX_MODES; MAXK = number of detectors.
@@ -364,12 +469,14 @@ namespace {
 // and every batch gets one blob per subset, [sub][batch][blob_words], each with the subset's coefficient pieces in the
 // UMMA layout followed by the (identical) shifts and exponent scales.  Generic in M (the harmonics live in local memory);
 // MS = modes per subset (compile time, so that the operand chunks are assembled in registers).
-template <int KT, int MS>
+// PROG: the quadratic term runs the pair program `qp` (its image of the block's first point in shared memory).
+template <int KT, int MS, bool PROG>
 __global__ void __launch_bounds__(GEOM_THREADS)
 geometry_tcx_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, TcChunk ch, const double *__restrict__ p_ra,
                     const double *__restrict__ p_dec, const double *__restrict__ p_psi, const double *__restrict__ p_iota,
                     const double *__restrict__ p_phi, const double *__restrict__ p_dist, const double *__restrict__ U,
-                    const double *__restrict__ V, int32_t *__restrict__ shift_out, int stage_uv) {
+                    const double *__restrict__ V, const __grid_constant__ QuadProg qp, int32_t *__restrict__ shift_out,
+                    int stage_uv) {
   constexpr int K = KT;
   constexpr int KP = (6 * MS + 15) & ~15, nch = KP / 8;
   const int M = g.n_modes;
@@ -391,7 +498,11 @@ geometry_tcx_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, T
   }
   const int32_t point0 = ch.ids[seg_first];
   const int n_uv = K * M * M;
-  if (stage_uv) {
+  const QuadSmem QL = quad_smem(qp.n_entries, K, M);
+  if (PROG) {
+    quad_stage(qp, K, point0, s_uv);
+    __syncthreads();
+  } else if (stage_uv) {
     const double2 *u = reinterpret_cast<const double2 *>(U) + (int64_t)point0 * n_uv;
     const double2 *v = reinterpret_cast<const double2 *>(V) + (int64_t)point0 * n_uv;
     for (int i = threadIdx.x; i < n_uv; i += GEOM_THREADS) {
@@ -438,8 +549,21 @@ geometry_tcx_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, T
   }
   int32_t shift[KT];
   double Fre[KT], Fim[KT], Yre[RIFT_MAX_MODES], Yim[RIFT_MAX_MODES], c, q;
-  sample_geometry<RIFT_MAX_MODES, KT>(g, modes, p_ra[gi], p_dec[gi], p_psi[gi], p_iota[gi], p_phi[gi], p_dist[gi], Up, Vp,
-                                      shift, Fre, Fim, Yre, Yim, c, q);
+  if (PROG) {
+    unsigned char *sm = reinterpret_cast<unsigned char *>(s_uv);
+    double *amp = reinterpret_cast<double *>(sm + QL.amp) + threadIdx.x;
+    double z[2];
+    sample_geometry<RIFT_MAX_MODES, KT, false>(g, modes, p_ra[gi], p_dec[gi], p_psi[gi], p_iota[gi], p_phi[gi], p_dist[gi],
+                                               nullptr, nullptr, shift, Fre, Fim, Yre, Yim, c, q, amp, z);
+    if (point == point0)                                  // two call sites: shared-memory and global loads of W
+      q = quad_prog<KT>(qp, s_uv, amp, z[0], z[1], Fre, Fim);
+    else
+      q = quad_prog<KT>(qp, qp.uv + (size_t)point * qp.n_entries * K, amp, z[0], z[1], Fre, Fim);
+    q *= 0.25 * c * c;
+  } else {
+    sample_geometry<RIFT_MAX_MODES, KT>(g, modes, p_ra[gi], p_dec[gi], p_psi[gi], p_iota[gi], p_phi[gi], p_dist[gi], Up, Vp,
+                                        shift, Fre, Fim, Yre, Yim, c, q);
+  }
   ch.scale_c[w] = c;
   ch.quad[w] = q;
   const float cl2v = (float)(c * 1.4426950408889634 / ((double)ch.qscale[point] * RIFT_TC_BSCALE));
@@ -644,24 +768,26 @@ cudaError_t launch_tcs_buckets(const DetGeom &g, const TcPlan &tp, const TcChunk
 }
 
 cudaError_t launch_geometry_tc(const DetGeom &g, const ModeEntry *modes, const TcPlan &tp, const TcChunk &c,
-                               const double *const params[6], const double *U, const double *V, int32_t *shift_out,
-                               cudaStream_t s) {
+                               const double *const params[6], const double *U, const double *V, const QuadProg &qp,
+                               int32_t *shift_out, cudaStream_t s) {
   const int64_t n = (c.key ? c.cap_sorted : c.n_batches) * RIFT_TC_NB;      // sorted variant: upper bound, trimmed on device
   if (n <= 0) return cudaSuccess;
   const unsigned grid = (unsigned)((n + GEOM_THREADS - 1) / GEOM_THREADS);
   if (tp.n_sub > 1) {
     const size_t uv_bytes = (size_t)2 * tp.K * tp.M * tp.M * sizeof(double2);
+    const size_t prog_bytes = quad_smem(qp.n_entries, tp.K, tp.M).total;
+    const bool prog = qp.uv != nullptr && prog_bytes <= 96u * 1024u;
     const int stage_uv = uv_bytes <= 96u * 1024u ? 1 : 0;                    // else U, V are read through L1
-    const size_t smem = stage_uv ? uv_bytes : 0;
+    const size_t smem = prog ? prog_bytes : (stage_uv ? uv_bytes : 0);
 #define RIFT_GEOM_TCX_MS(KT, MS)                                                                                         \
   case MS: {                                                                                                             \
-    auto kern = geometry_tcx_kernel<KT, MS>;                                                                             \
+    auto kern = prog ? geometry_tcx_kernel<KT, MS, true> : geometry_tcx_kernel<KT, MS, false>;                           \
     if (smem > 48u * 1024u) {                                                                                            \
       cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                \
       if (e != cudaSuccess) return e;                                                                                    \
     }                                                                                                                    \
     kern<<<grid, GEOM_THREADS, smem, s>>>(g, modes, tp, c, params[0], params[1], params[2], params[3], params[4],        \
-                                          params[5], U, V, shift_out, stage_uv);                                         \
+                                          params[5], U, V, qp, shift_out, stage_uv);                                     \
     break;                                                                                                               \
   }
 #define RIFT_GEOM_TCX(KT)                                                                                                \
@@ -721,8 +847,9 @@ cudaError_t launch_geometry_k(const DetGeom &g, const ModeEntry *modes, const Ba
 }  // namespace
 
 cudaError_t launch_geometry(const DetGeom &g, const ModeEntry *modes, const Batch &b, const double *const params[6],
-                            const double *U, const double *V, bool coef_fp32, const Workspace &ws,
+                            const double *U, const double *V, const QuadProg &qp, bool coef_fp32, const Workspace &ws,
                             int32_t *shift_out, double *dbg_F, double *dbg_Y, const int32_t *perm, cudaStream_t s) {
+  (void)qp;
   if (b.n <= 0) return cudaSuccess;
   const unsigned grid = (unsigned)((b.n + GEOM_THREADS - 1) / GEOM_THREADS);
   const bool small = g.n_modes <= 8;
@@ -733,4 +860,13 @@ cudaError_t launch_geometry(const DetGeom &g, const ModeEntry *modes, const Batc
   return small ? launch_geometry_k<double2, 8>(g, modes, b, params, U, V, ws, shift_out, dbg_F, dbg_Y, perm, grid, s)
                : launch_geometry_k<double2, RIFT_MAX_MODES>(g, modes, b, params, U, V, ws, shift_out, dbg_F, dbg_Y, perm,
                                                             grid, s);
+}
+
+cudaError_t launch_build_quad_uv(const QuadProg &qp, const double *U, const double *V, int32_t P, int32_t K, int32_t M,
+                                 double2 *uv_out, cudaStream_t s) {
+  const int64_t total = (int64_t)P * qp.n_entries * K;
+  if (total <= 0) return cudaSuccess;
+  build_quad_uv_kernel<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(qp, reinterpret_cast<const double2 *>(U),
+                                                                       reinterpret_cast<const double2 *>(V), P, K, M, uv_out);
+  return cudaGetLastError();
 }

@@ -101,13 +101,34 @@ struct TcChunk {                 // a chunk = global batches [gb0, gb0 + n_batch
 // split into n_sub subsets of m_sub; pass s contracts subset s and adds the window sums of the passes before it.
 enum { RIFT_TC_PASS_SINGLE = 0, RIFT_TC_PASS_FIRST = 1, RIFT_TC_PASS_MIDDLE = 2, RIFT_TC_PASS_LAST = 3 };
 
+// Pair program of the quadratic term a4 for mode sets of more than 8 modes (geometry.cu).  With Y_a = d_a(iota) z^{m_a},
+// z = e^{-i phi}, the products conj(Y_a) Y_b = d_a d_b z^{m_b - m_a} and Y_a Y_b = d_a d_b z^{m_a + m_b} share their phase among all
+// mode pairs of equal exponent n, so  Y^dag U_k Y = sum_n Re( z^n S^U_{k,n} ),  Y^T V_k Y = sum_n z^n S^V_{k,n}  with
+// S_{k,n} = sum_{pairs of exponent n} (d_a d_b) W_{k,ab}:  one real weight and 2 K FMAs per (pair, matrix) instead of two complex
+// products and 6 K FMAs.  An entry is one pair a <= b of one matrix; W is U_ab (or conj U_ab when m_b < m_a, exponent
+// |m_b - m_a|) resp. V_ab, times 2 off the diagonal (U Hermitian, V symmetric).  Bins are runs of entries of one (matrix,
+// exponent), ordered U: n = 0, 1, ...; V: n = 0, 1, ..., then n = -1, -2, ... so that z^n is carried by one complex
+// multiplication per bin.
+#define RIFT_QP_MAX_ENT 1024     // mode pairs of both matrices: M (M + 1) <= 1024, i.e. up to 31 modes
+#define RIFT_QP_MAX_BINS 52      // (2 n_max + 1) + n_max + 1 + ... <= 50 for l <= 8
+struct QuadProg {                // passed to the kernels as a __grid_constant__ parameter: the tables are read from the constant bank
+  int32_t n_entries, n_bins;
+  const uint32_t *ent_full;      // device [n_entries]: a | b << 8 | matrix << 16 (0 U, 1 V) | conj << 17 (used to build uv)
+  const double2 *uv;             // device [P][n_entries][K]: W of every entry and detector; NULL = no program
+  uint16_t ent[RIFT_QP_MAX_ENT];             // a | b << 7
+  uint16_t bin_begin[RIFT_QP_MAX_BINS + 1];  // entries of bin i: [bin_begin[i], bin_begin[i + 1])
+  uint8_t bin_kind[RIFT_QP_MAX_BINS];        // matrix | z step << 1  (0 z^0, 1 *= z, 2 conj z, 3 *= conj z)
+};
+
 // geometry.cu
 cudaError_t launch_geometry_tc(const DetGeom &g, const ModeEntry *modes, const TcPlan &tp, const TcChunk &c,
-                               const double *const params[6], const double *U, const double *V, int32_t *shift_out,
-                               cudaStream_t s);
+                               const double *const params[6], const double *U, const double *V, const QuadProg &qp,
+                               int32_t *shift_out, cudaStream_t s);
 cudaError_t launch_geometry(const DetGeom &g, const ModeEntry *modes, const Batch &b, const double *const params[6],
-                            const double *U, const double *V, bool coef_fp32, const Workspace &ws,
+                            const double *U, const double *V, const QuadProg &qp, bool coef_fp32, const Workspace &ws,
                             int32_t *shift_out, double *dbg_F, double *dbg_Y, const int32_t *perm, cudaStream_t s);
+cudaError_t launch_build_quad_uv(const QuadProg &qp, const double *U, const double *V, int32_t P, int32_t K, int32_t M,
+                                 double2 *uv_out, cudaStream_t s);
 // sort.cu
 cudaError_t launch_group_sort(const DetGeom &g, const SortPlan &sp, const Batch &b, const double *const params[6],
                               int32_t *bucket_of, uint32_t *hist, int32_t n_seg_chunk, int32_t *perm, cudaStream_t s,

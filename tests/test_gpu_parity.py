@@ -329,6 +329,37 @@ def test_c2_shape_21_modes(torch, oracle):
         rift.rift_ile_destroy(h)
 
 
+def test_quadratic_term_pair_program(torch, oracle, monkeypatch):
+    """More than 8 modes: the quadratic term a4 (Eq. (D3)) runs the pair program of rift_internal.h (mode pairs grouped by
+    their common phase exponent).  With the same contraction, lnL from the program and from the plain double sum over
+    mode pairs (RIFT_NO_QUAD_PROG) differ by the rounding of q only; both match the oracle.  Mode lists in scrambled order
+    with gaps in m, two segments whose boundary falls inside a thread block (program image of another point)."""
+    modes = ((3, -3), (2, 2), (4, 0), (2, -2), (3, 2), (4, 4), (2, 1), (4, -3), (3, 3), (2, 0), (4, -4))
+    cfg = synth.with_overrides(synth.CONFIGS[1], modes=modes, n_points=2)
+    inp = build(oracle, cfg, n_points=2)
+    n = 333
+    ids = [1, 0]
+    params = np.concatenate([synth.draw_samples(cfg, 70 + s, n)[0] for s in range(len(ids))], axis=1)
+    ref = np.concatenate([oracle_eval(oracle, inp, ids[s], params[:, s * n:(s + 1) * n])[0] for s in range(len(ids))])
+    for prec in (rift.RIFT_PREC_MIXED, rift.RIFT_PREC_FP64):
+        out = []
+        for no_prog in (False, True):
+            if no_prog:
+                monkeypatch.setenv("RIFT_NO_QUAD_PROG", "1")
+            else:
+                monkeypatch.delenv("RIFT_NO_QUAD_PROG", raising=False)
+            h = create(rift, inp, prec)
+            got, _, _ = gpu_eval(torch, h, ids, n, params, K=cfg.n_det)
+            out.append(got.cpu().numpy())
+            rift.rift_ile_destroy(h)
+        monkeypatch.delenv("RIFT_NO_QUAD_PROG", raising=False)
+        assert np.max(rel_err(out[0], out[1])) < 1e-12
+        if prec == rift.RIFT_PREC_FP64:
+            assert np.max(rel_err(out[0], ref)) < TOL_FP64_REL
+        else:
+            assert np.max(np.abs(out[0] - ref)) < TOL_MIXED_LNL
+
+
 def test_c4_shape_long_window(torch, oracle):
     cfg = synth.CONFIGS[4]
     inp = build(oracle, cfg, n_points=1)
