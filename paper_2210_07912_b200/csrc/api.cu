@@ -717,7 +717,7 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
     if (ent.size() <= RIFT_QP_MAX_ENT && bins.size() <= RIFT_QP_MAX_BINS) {
       h->qp.n_entries = (int32_t)ent.size();
       h->qp.n_bins = (int32_t)bins.size();
-      for (size_t e = 0; e < ent.size(); ++e) h->qp.ent[e] = (uint16_t)((ent[e] & 0x7fu) | ((ent[e] >> 8) & 0x7fu) << 7);
+      for (size_t e = 0; e < ent.size(); ++e) h->qp.ent[e] = make_uint2((ent[e] & 0xffu) * RIFT_QP_AMP_STRIDE, ((ent[e] >> 8) & 0xffu) * RIFT_QP_AMP_STRIDE);
       for (size_t i = 0; i < bins.size(); ++i) {
         h->qp.bin_begin[i] = (uint16_t)bins[i].x;
         h->qp.bin_kind[i] = (uint8_t)(bins[i].z | bins[i].w << 1);

@@ -12,6 +12,7 @@
 namespace {
 
 constexpr int GEOM_THREADS = 128;
+static_assert(GEOM_THREADS * sizeof(double) == RIFT_QP_AMP_STRIDE, "amplitude column stride of the pair program");
 
 __device__ __forceinline__ double ipow4(double p1, double p2, double p4, double p8, int e) {   // x^e, 0 <= e < 16
   double r = (e & 1) ? p1 : 1.0;
@@ -222,8 +223,9 @@ __device__ __forceinline__ double quad_prog(const QuadProg &qp, const double2 *_
     const int e1 = qp.bin_begin[bi + 1];
 #pragma unroll 4
     for (int e = qp.bin_begin[bi]; e < e1; ++e) {
-      const uint32_t ab = qp.ent[e];
-      const double w = amp[(ab & 0x7fu) * GEOM_THREADS] * amp[(ab >> 7) * GEOM_THREADS];
+      const uint2 ab = qp.ent[e];
+      const char *ac = reinterpret_cast<const char *>(amp);
+      const double w = *reinterpret_cast<const double *>(ac + ab.x) * *reinterpret_cast<const double *>(ac + ab.y);
       const double2 *u = uv + e * KT;
 #pragma unroll
       for (int k = 0; k < KT; ++k) {
@@ -471,7 +473,7 @@ namespace {
 // MS = modes per subset (compile time, so that the operand chunks are assembled in registers).
 // PROG: the quadratic term runs the pair program `qp` (its image of the block's first point in shared memory).
 template <int KT, int MS, bool PROG>
-__global__ void __launch_bounds__(GEOM_THREADS)
+__global__ void __launch_bounds__(GEOM_THREADS, PROG ? 5 : 1)
 geometry_tcx_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, TcChunk ch, const double *__restrict__ p_ra,
                     const double *__restrict__ p_dec, const double *__restrict__ p_psi, const double *__restrict__ p_iota,
                     const double *__restrict__ p_phi, const double *__restrict__ p_dist, const double *__restrict__ U,

@@ -110,12 +110,13 @@ enum { RIFT_TC_PASS_SINGLE = 0, RIFT_TC_PASS_FIRST = 1, RIFT_TC_PASS_MIDDLE = 2,
 // exponent), ordered U: n = 0, 1, ...; V: n = 0, 1, ..., then n = -1, -2, ... so that z^n is carried by one complex
 // multiplication per bin.
 #define RIFT_QP_MAX_ENT 1024     // mode pairs of both matrices: M (M + 1) <= 1024, i.e. up to 31 modes
+#define RIFT_QP_AMP_STRIDE 1024u  // bytes between d_a and d_{a+1} in a thread's amplitude column (128 threads x 8 bytes)
 #define RIFT_QP_MAX_BINS 52      // (2 n_max + 1) + n_max + 1 + ... <= 50 for l <= 8
 struct QuadProg {                // passed to the kernels as a __grid_constant__ parameter: the tables are read from the constant bank
   int32_t n_entries, n_bins;
   const uint32_t *ent_full;      // device [n_entries]: a | b << 8 | matrix << 16 (0 U, 1 V) | conj << 17 (used to build uv)
   const double2 *uv;             // device [P][n_entries][K]: W of every entry and detector; NULL = no program
-  uint16_t ent[RIFT_QP_MAX_ENT];             // a | b << 7
+  uint2 ent[RIFT_QP_MAX_ENT];                // byte offsets of d_a and d_b in a thread's amplitude column (a * RIFT_QP_AMP_STRIDE)
   uint16_t bin_begin[RIFT_QP_MAX_BINS + 1];  // entries of bin i: [bin_begin[i], bin_begin[i + 1])
   uint8_t bin_kind[RIFT_QP_MAX_BINS];        // matrix | z step << 1  (0 z^0, 1 *= z, 2 conj z, 3 *= conj z)
 };
