@@ -274,19 +274,27 @@ __global__ void build_quad_uv_kernel(const __grid_constant__ QuadProg qp, const 
 }
 
 // CT = coefficient type; MAXM = 8 (mode loops unrolled, Y in registers) or RIFT_MAX_MODES; MAXK = number of detectors.
-template <typename CT, int MAXM, int MAXK>
+// PROG (MAXM > 16 only): the quadratic term runs the pair program `qp`.
+template <typename CT, int MAXM, int MAXK, bool PROG>
 __global__ void __launch_bounds__(GEOM_THREADS)
 geometry_kernel(DetGeom g, const ModeEntry *__restrict__ modes, Batch b, const double *__restrict__ p_ra,
                 const double *__restrict__ p_dec, const double *__restrict__ p_psi, const double *__restrict__ p_iota,
                 const double *__restrict__ p_phi, const double *__restrict__ p_dist, const double *__restrict__ U,
-                const double *__restrict__ V, Workspace ws, int32_t *__restrict__ shift_out,
-                double *__restrict__ dbg_F, double *__restrict__ dbg_Y, const int32_t *__restrict__ perm, int stage_uv) {
+                const double *__restrict__ V, const __grid_constant__ QuadProg qp, Workspace ws,
+                int32_t *__restrict__ shift_out, double *__restrict__ dbg_F, double *__restrict__ dbg_Y,
+                const int32_t *__restrict__ perm, int stage_uv) {
   const int K = g.n_det, M = g.n_modes;
   // U, V of the intrinsic point of the block's first slot staged in shared memory when the launch provides room
   extern __shared__ double2 s_uv_g[];
   const int n_uv = K * M * M;
   int32_t point0 = -1;
-  if (stage_uv) {
+  if (PROG) {
+    const int64_t w0 = (int64_t)blockIdx.x * GEOM_THREADS;
+    const int64_t src0 = perm ? (int64_t)perm[w0] : w0;
+    point0 = b.ids[(b.g0 + src0) / b.n_per_seg];
+    quad_stage(qp, K, point0, s_uv_g);
+    __syncthreads();
+  } else if (stage_uv) {
     const int64_t w0 = (int64_t)blockIdx.x * GEOM_THREADS;
     const int64_t src0 = perm ? (int64_t)perm[w0] : w0;
     point0 = b.ids[(b.g0 + src0) / b.n_per_seg];
@@ -313,8 +321,21 @@ geometry_kernel(DetGeom g, const ModeEntry *__restrict__ modes, Batch b, const d
     Up = s_uv_g;
     Vp = s_uv_g + n_uv;
   }
-  sample_geometry<MAXM, MAXK>(g, modes, p_ra[gi], p_dec[gi], p_psi[gi], p_iota[gi], p_phi[gi], p_dist[gi], Up, Vp, shift,
-                              Fre, Fim, Yre, Yim, c, q);
+  if constexpr (PROG) {
+    double *amp = reinterpret_cast<double *>(reinterpret_cast<unsigned char *>(s_uv_g) + quad_smem(qp.n_entries, K, M).amp) +
+                  threadIdx.x;
+    double z[2];
+    sample_geometry<MAXM, MAXK, false>(g, modes, p_ra[gi], p_dec[gi], p_psi[gi], p_iota[gi], p_phi[gi], p_dist[gi], nullptr,
+                                       nullptr, shift, Fre, Fim, Yre, Yim, c, q, amp, z);
+    if (point == point0)
+      q = quad_prog<MAXK>(qp, s_uv_g, amp, z[0], z[1], Fre, Fim);
+    else
+      q = quad_prog<MAXK>(qp, qp.uv + (size_t)point * qp.n_entries * K, amp, z[0], z[1], Fre, Fim);
+    q *= 0.25 * c * c;
+  } else {
+    sample_geometry<MAXM, MAXK>(g, modes, p_ra[gi], p_dec[gi], p_psi[gi], p_iota[gi], p_phi[gi], p_dist[gi], Up, Vp, shift,
+                                Fre, Fim, Yre, Yim, c, q);
+  }
   int32_t *my_shift = ws.shift + w * K;
   for (int k = 0; k < K; ++k) {
     my_shift[k] = shift[k];
@@ -823,20 +844,23 @@ cudaError_t launch_geometry_tc(const DetGeom &g, const ModeEntry *modes, const T
 namespace {
 template <typename CT, int MAXM>
 cudaError_t launch_geometry_k(const DetGeom &g, const ModeEntry *modes, const Batch &b, const double *const params[6],
-                              const double *U, const double *V, const Workspace &ws, int32_t *shift_out, double *dbg_F,
+                              const double *U, const double *V, const QuadProg &qp, const Workspace &ws, int32_t *shift_out, double *dbg_F,
                               double *dbg_Y, const int32_t *perm, unsigned grid, cudaStream_t s) {
   const size_t uv_bytes = (size_t)2 * g.n_det * g.n_modes * g.n_modes * sizeof(double2);
   const int stage_uv = (MAXM > 16 && uv_bytes <= 96u * 1024u) ? 1 : 0;      // large mode sets: U, V from shared memory
-  const size_t smem = stage_uv ? uv_bytes : 0;
+  const size_t prog_bytes = quad_smem(qp.n_entries, g.n_det, g.n_modes).total;
+  constexpr bool CAN_PROG = MAXM > 16;
+  const bool prog = CAN_PROG && qp.uv != nullptr && prog_bytes <= 96u * 1024u;
+  const size_t smem = prog ? prog_bytes : (stage_uv ? uv_bytes : 0);
 #define RIFT_GEOM(KT)                                                                                                   \
   case KT: {                                                                                                            \
-    auto kern = geometry_kernel<CT, MAXM, KT>;                                                                          \
+    auto kern = prog ? geometry_kernel<CT, MAXM, KT, CAN_PROG> : geometry_kernel<CT, MAXM, KT, false>;                  \
     if (smem > 48u * 1024u) {                                                                                           \
       cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);               \
       if (e != cudaSuccess) return e;                                                                                   \
     }                                                                                                                   \
     kern<<<grid, GEOM_THREADS, smem, s>>>(g, modes, b, params[0], params[1], params[2], params[3], params[4], params[5], \
-                                          U, V, ws, shift_out, dbg_F, dbg_Y, perm, stage_uv);                           \
+                                          U, V, qp, ws, shift_out, dbg_F, dbg_Y, perm, stage_uv);                       \
     break;                                                                                                              \
   }
   switch (g.n_det) {
@@ -851,16 +875,15 @@ cudaError_t launch_geometry_k(const DetGeom &g, const ModeEntry *modes, const Ba
 cudaError_t launch_geometry(const DetGeom &g, const ModeEntry *modes, const Batch &b, const double *const params[6],
                             const double *U, const double *V, const QuadProg &qp, bool coef_fp32, const Workspace &ws,
                             int32_t *shift_out, double *dbg_F, double *dbg_Y, const int32_t *perm, cudaStream_t s) {
-  (void)qp;
   if (b.n <= 0) return cudaSuccess;
   const unsigned grid = (unsigned)((b.n + GEOM_THREADS - 1) / GEOM_THREADS);
   const bool small = g.n_modes <= 8;
   if (coef_fp32)
-    return small ? launch_geometry_k<float2, 8>(g, modes, b, params, U, V, ws, shift_out, dbg_F, dbg_Y, perm, grid, s)
-                 : launch_geometry_k<float2, RIFT_MAX_MODES>(g, modes, b, params, U, V, ws, shift_out, dbg_F, dbg_Y, perm,
+    return small ? launch_geometry_k<float2, 8>(g, modes, b, params, U, V, qp, ws, shift_out, dbg_F, dbg_Y, perm, grid, s)
+                 : launch_geometry_k<float2, RIFT_MAX_MODES>(g, modes, b, params, U, V, qp, ws, shift_out, dbg_F, dbg_Y, perm,
                                                              grid, s);
-  return small ? launch_geometry_k<double2, 8>(g, modes, b, params, U, V, ws, shift_out, dbg_F, dbg_Y, perm, grid, s)
-               : launch_geometry_k<double2, RIFT_MAX_MODES>(g, modes, b, params, U, V, ws, shift_out, dbg_F, dbg_Y, perm,
+  return small ? launch_geometry_k<double2, 8>(g, modes, b, params, U, V, qp, ws, shift_out, dbg_F, dbg_Y, perm, grid, s)
+               : launch_geometry_k<double2, RIFT_MAX_MODES>(g, modes, b, params, U, V, qp, ws, shift_out, dbg_F, dbg_Y, perm,
                                                             grid, s);
 }
 
