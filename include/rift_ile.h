@@ -86,7 +86,10 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out);
  *                            ln[(1/n_tau) sum_j exp(lnL(tau_j))],  tau_j over the window (readings A4, A5).
  *                          dist <= 0 or a NaN parameter gives NaN for that sample only.
  *   shift_out            : DEVICE int32 [n_seg*n_per_seg][n_det] or NULL: s_k = floor(dt_k/delta_t + 1/2) (G4).
- *   cuda_stream          : a cudaStream_t (NULL = legacy default stream).  Asynchronous on that stream. */
+ *   cuda_stream          : a cudaStream_t (NULL = legacy default stream).  Asynchronous on that stream.
+ * Stream capture: the first call of a given size grows the handle's workspace (cudaMalloc) and a new id list is
+ * copied to the device; a repeated call with the same sizes, ids and stream issues kernel launches only and may
+ * be captured into a CUDA graph (the graph then reads params and writes lnL_out / shift_out at replay). */
 int rift_ile_eval_batch(rift_ile_t *h, int32_t n_seg, const int32_t *intrinsic_ids, int64_t n_per_seg,
                         const double *const params[RIFT_N_PARAMS], double *lnL_out, int32_t *shift_out,
                         void *cuda_stream);

@@ -45,6 +45,8 @@ struct rift_ile {
   int64_t ws_cap = 0;
   Workspace ws{};
   int32_t *d_ids = nullptr;
+  std::vector<int32_t> ids_last;   // host copy of the ids d_ids holds, and the stream that uploaded them: an unchanged id list
+  cudaStream_t ids_stream = nullptr;   // is not copied again, so a steady-state eval_batch is kernel launches only (graph capture)
   int64_t ids_cap = 0;
   // reduce state
   ReduceState *d_state = nullptr;
@@ -230,8 +232,15 @@ int upload_ids(rift_ile *h, int32_t n_seg, const int32_t *ids, cudaStream_t s) {
     h->ids_cap = 0;
     CU(h, cudaMalloc(&h->d_ids, (size_t)n_seg * sizeof(int32_t)));
     h->ids_cap = n_seg;
+    h->ids_last.clear();
   }
+  if (h->ids_stream == s && (int32_t)h->ids_last.size() == n_seg &&
+      memcmp(h->ids_last.data(), ids, (size_t)n_seg * sizeof(int32_t)) == 0)
+    return RIFT_OK;
+  h->ids_last.clear();
   CU(h, cudaMemcpyAsync(h->d_ids, ids, (size_t)n_seg * sizeof(int32_t), cudaMemcpyHostToDevice, s));
+  h->ids_last.assign(ids, ids + n_seg);
+  h->ids_stream = s;
   return RIFT_OK;
 }
 

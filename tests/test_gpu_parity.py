@@ -360,6 +360,41 @@ def test_quadratic_term_pair_program(torch, oracle, monkeypatch):
             assert np.max(np.abs(out[0] - ref)) < TOL_MIXED_LNL
 
 
+def test_eval_batch_under_cuda_graph(torch, oracle):
+    """A steady-state eval_batch (workspace grown, id list already on the device) is kernel launches only, so it can be
+    captured into a CUDA graph (bench.py times C0 this way); replays with new sample values in the
+    same buffers match the oracle."""
+    cfg = synth.CONFIGS[0]
+    inp = build(oracle, cfg, n_points=1)
+    n = 1000
+    p1, _ = synth.draw_samples(cfg, 11, n)
+    p2, _ = synth.draw_samples(cfg, 12, n)
+    ref2 = oracle_eval(oracle, inp, 0, p2)[0]
+    for prec, tol in ((rift.RIFT_PREC_FP64, None), (rift.RIFT_PREC_MIXED, TOL_MIXED_LNL)):
+        h = create(rift, inp, prec)
+        params_d = dev(torch, p1)
+        lnL = torch.empty(n, dtype=torch.float64, device="cuda")
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            rift.rift_ile_eval_batch(h, [0], n, params_d, lnL, None, side.cuda_stream)
+        side.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            rift.rift_ile_eval_batch(h, [0], n, params_d, lnL, None, torch.cuda.current_stream().cuda_stream)
+        params_d.copy_(dev(torch, p2))
+        lnL.fill_(float("nan"))
+        g.replay()
+        torch.cuda.synchronize()
+        got = lnL.cpu().numpy()
+        if tol is None:
+            assert np.max(rel_err(got, ref2)) < TOL_FP64_REL
+        else:
+            assert np.max(np.abs(got - ref2)) < tol
+        del g
+        rift.rift_ile_destroy(h)
+
+
 def test_c4_shape_long_window(torch, oracle):
     cfg = synth.CONFIGS[4]
     inp = build(oracle, cfg, n_points=1)
