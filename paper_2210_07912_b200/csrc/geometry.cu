@@ -600,6 +600,13 @@ geometry_tcx_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, T
       const int dm = tp.dmax[1], d = shift[KT > 1 ? 1 : 0] - shift[0];
       reinterpret_cast<int32_t *>(blob + K * nch * 64 + K * 16 + 16)[0] = d < -dm ? -dm : (d > dm ? dm : d);
     }
+    double yr[MS], yi[MS];                                                  // the subset's harmonics, read once for all detectors
+#pragma unroll
+    for (int al = 0; al < MS; ++al) {
+      const int a = sub * MS + al;
+      yr[al] = (a < M) ? Yre[a] * RIFT_TC_BSCALE : 0.0;
+      yi[al] = (a < M) ? Yim[a] * RIFT_TC_BSCALE : 0.0;
+    }
     for (int k = 0; k < K; ++k) {
       dsh[k * 16 + n] = (k == 0) ? tp.j0 + shift[0] : shift[k] - shift[0];
       uint16_t hv[KP];
@@ -607,12 +614,8 @@ geometry_tcx_kernel(DetGeom g, const ModeEntry *__restrict__ modes, TcPlan tp, T
       for (int e = 6 * MS; e < KP; ++e) hv[e] = 0;
 #pragma unroll
       for (int al = 0; al < MS; ++al) {
-        const int a = sub * MS + al;
-        double vr = 0.0, vi = 0.0;
-        if (a < M) {
-          vr = (Fre[k] * Yre[a] - Fim[k] * Yim[a]) * RIFT_TC_BSCALE;
-          vi = (Fre[k] * Yim[a] + Fim[k] * Yre[a]) * RIFT_TC_BSCALE;
-        }
+        const double vr = Fre[k] * yr[al] - Fim[k] * yi[al];
+        const double vi = Fre[k] * yi[al] + Fim[k] * yr[al];
         const __half hr = __double2half(vr), hi = __double2half(vi);
         const __half lr = __double2half(vr - (double)__half2float(hr)), li = __double2half(vi - (double)__half2float(hi));
         hv[2 * al] = hv[2 * MS + 2 * al] = __half_as_ushort(hr);
