@@ -22,6 +22,8 @@ struct rift_ile {
   QStore qs{};
   void *d_Qe = nullptr;            // interleaved, circularly extended copy for the direct_ext kernel (NULL if too big)
   QStore qse{};
+  void *d_Qg = nullptr;            // the same extended layout for configurations whose Q block does NOT fit shared memory:
+  QStore qsg{};                    // lnl_direct reads it from global memory with one address per mode row (no wrap arithmetic)
   void *d_Qp = nullptr;            // planar, circularly extended copy for the grouped kernel (NULL if it cannot fit)
   QStore qsp{};
   TcPlan tc{};                     // tensor-core path (lnl_tc.cu); tc.ok == 0 when the configuration does not fit
@@ -178,6 +180,7 @@ void free_handle(rift_ile *h) {
   cudaFree(h->ws.orig);
   cudaFree(const_cast<uint32_t *>(h->qp.ent_full));
   cudaFree(const_cast<double2 *>(h->qp.uv));
+  cudaFree(h->d_Qg);
   cudaFree(h->d_U);
   cudaFree(h->d_V);
   cudaFree(h->ws.coef);
@@ -587,9 +590,10 @@ int run_chunks(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *cons
         CU(h, launch_lnl_direct_ext(h->qse, fp32, b, ws, h->K, lnL_out, h->n_sm, s, &nl));
         h->kernel_name = fp32 ? "lnl_direct_ext<f32>" : "lnl_direct_ext<f64>";
       } else {
-        CU(h, launch_lnl_direct(h->qs, fp32, in_smem, b, ws, h->K, lnL_out, h->n_sm, s, &nl));
-        h->kernel_name = fp32 ? (in_smem ? "lnl_direct<f32,smem>" : "lnl_direct<f32,global>")
-                              : (in_smem ? "lnl_direct<f64,smem>" : "lnl_direct<f64,global>");
+        const bool ext = !in_smem && h->d_Qg != nullptr;
+        CU(h, launch_lnl_direct(ext ? h->qsg : h->qs, fp32, in_smem, ext, b, ws, h->K, lnL_out, h->n_sm, s, &nl));
+        h->kernel_name = fp32 ? (in_smem ? "lnl_direct<f32,smem>" : (ext ? "lnl_direct<f32,global,ext>" : "lnl_direct<f32,global>"))
+                              : (in_smem ? "lnl_direct<f64,smem>" : (ext ? "lnl_direct<f64,global,ext>" : "lnl_direct<f64,global>"));
       }
       ps.end();
       h->launches += nl;
@@ -764,6 +768,10 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
     // interleaved, circularly extended copy for the direct_ext kernel, if one point's block fits in shared memory
     {
       const int32_t n_te = (h->n_t + RIFT_EXT + 1) & ~1;
+      QStore q0{};                                        // the plain block as lnl_direct would stage it (h->qs is set below)
+      q0.km = h->K * h->M;
+      q0.point_stride_bytes = (int64_t)h->K * h->M * h->n_tp * csz;
+      const bool block_fits = lnl_direct_smem_bytes(q0, fp32, true) <= 227u * 1024u;
       QStore qe{};
       qe.n_t = h->n_t;
       qe.n_tp = n_te;
@@ -776,6 +784,12 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
         qe.data = h->d_Qe;
         h->qse = qe;
         h->launches += h->tc.n_sub;
+      } else if (e == cudaSuccess && !block_fits && !getenv("RIFT_NO_GLOBAL_EXT")) {
+        e = cudaMalloc(&h->d_Qg, (size_t)h->P * qe.point_stride_bytes);
+        if (e == cudaSuccess) e = launch_convert_q_ext(src, h->d_Qg, rows, h->n_t, n_te, fp32, 0);
+        qe.data = h->d_Qg;
+        h->qsg = qe;
+        ++h->launches;
       }
     }
     // planar, circularly extended copy for the grouped kernel, if one point's block fits in shared memory

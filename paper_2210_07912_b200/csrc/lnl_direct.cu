@@ -19,7 +19,7 @@ template <typename Real> struct CplxOf;
 template <> struct CplxOf<float> { typedef float2 type; };
 template <> struct CplxOf<double> { typedef double2 type; };
 
-template <typename Real, bool QSMEM>
+template <typename Real, bool QSMEM, bool EXT>
 __global__ void __launch_bounds__(LNL_THREADS)
 lnl_direct_kernel(QStore q, Batch b, Workspace ws, int K, double *__restrict__ lnL_out) {
   typedef typename CplxOf<Real>::type CT;
@@ -94,14 +94,28 @@ lnl_direct_kernel(QStore q, Batch b, Workspace ws, int K, double *__restrict__ l
             if (jb + lane + 32 * i >= q.n_tau) t = 0;       // masked slot, keep the address in range
             idx[i] = t;
           }
-          for (int m = 0; m < M; ++m) {
-            const CT a = wcoef[k * M + m];
-            const CT *row = Qp + (size_t)(k * M + m) * q.n_tp;
+          if constexpr (EXT) {
+            // extended rows (n_tp >= N_t + 416): the block never wraps, one address per mode row plus immediate offsets
+            const CT *row = Qp + (size_t)(k * M) * q.n_tp + base + lane;
+            for (int m = 0; m < M; ++m, row += q.n_tp) {
+              const CT a = wcoef[k * M + m];
 #pragma unroll
-            for (int i = 0; i < SLOTS; ++i) {
-              const CT v = QSMEM ? row[idx[i]] : __ldg(row + idx[i]);
-              x[i] = fma(a.x, v.x, x[i]);
-              x[i] = fma(a.y, v.y, x[i]);
+              for (int i = 0; i < SLOTS; ++i) {
+                const CT v = __ldg(row + 32 * i);
+                x[i] = fma(a.x, v.x, x[i]);
+                x[i] = fma(a.y, v.y, x[i]);
+              }
+            }
+          } else {
+            for (int m = 0; m < M; ++m) {
+              const CT a = wcoef[k * M + m];
+              const CT *row = Qp + (size_t)(k * M + m) * q.n_tp;
+#pragma unroll
+              for (int i = 0; i < SLOTS; ++i) {
+                const CT v = QSMEM ? row[idx[i]] : __ldg(row + idx[i]);
+                x[i] = fma(a.x, v.x, x[i]);
+                x[i] = fma(a.y, v.y, x[i]);
+              }
             }
           }
         }
@@ -142,10 +156,10 @@ lnl_direct_kernel(QStore q, Batch b, Workspace ws, int K, double *__restrict__ l
   }
 }
 
-template <typename Real, bool QSMEM>
+template <typename Real, bool QSMEM, bool EXT = false>
 cudaError_t launch_t(const QStore &q, const Batch &b, const Workspace &ws, int K, double *lnL_out, int n_sm,
                      size_t smem, cudaStream_t s) {
-  auto kern = lnl_direct_kernel<Real, QSMEM>;
+  auto kern = lnl_direct_kernel<Real, QSMEM, EXT>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   int occ = 0;
@@ -166,11 +180,14 @@ size_t lnl_direct_smem_bytes(const QStore &q, bool fp32, bool q_in_smem) {
   return 128 + (q_in_smem ? (size_t)q.point_stride_bytes : 0) + (size_t)LNL_WARPS * q.km * csz;
 }
 
-cudaError_t launch_lnl_direct(const QStore &q, bool fp32, bool q_in_smem, const Batch &b, const Workspace &ws,
+cudaError_t launch_lnl_direct(const QStore &q, bool fp32, bool q_in_smem, bool q_ext, const Batch &b, const Workspace &ws,
                               int n_det, double *lnL_out, int n_sm, cudaStream_t s, int *n_launch) {
   if (b.n <= 0) return cudaSuccess;
   const size_t smem = lnl_direct_smem_bytes(q, fp32, q_in_smem);
   if (n_launch) ++*n_launch;
+  if (q_ext && !q_in_smem)
+    return fp32 ? launch_t<float, false, true>(q, b, ws, n_det, lnL_out, n_sm, smem, s)
+                : launch_t<double, false, true>(q, b, ws, n_det, lnL_out, n_sm, smem, s);
   if (fp32)
     return q_in_smem ? launch_t<float, true>(q, b, ws, n_det, lnL_out, n_sm, smem, s)
                      : launch_t<float, false>(q, b, ws, n_det, lnL_out, n_sm, smem, s);

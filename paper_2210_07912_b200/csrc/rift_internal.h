@@ -142,7 +142,7 @@ cudaError_t launch_convert_q_planar(const double *Q_c128, void *dst, int64_t row
                                     bool to_fp32, cudaStream_t s);
 // lnl_direct.cu
 size_t lnl_direct_smem_bytes(const QStore &q, bool fp32, bool q_in_smem);
-cudaError_t launch_lnl_direct(const QStore &q, bool fp32, bool q_in_smem, const Batch &b, const Workspace &ws,
+cudaError_t launch_lnl_direct(const QStore &q, bool fp32, bool q_in_smem, bool q_ext, const Batch &b, const Workspace &ws,
                               int n_det, double *lnL_out, int n_sm, cudaStream_t s, int *n_launch);
 // lnl_direct_ext.cu (interleaved layout with a circular extension of RIFT_EXT samples per row)
 size_t lnl_direct_ext_smem_bytes(const QStore &q, bool fp32);
