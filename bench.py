@@ -195,7 +195,7 @@ def run_ours(args) -> None:
     h = rift.rift_ile_create(loc, resp, cfg.gmst, ml, mm, P, cfg.n_t, cfg.delta_t, cfg.n_t, synth.D_REF_MPC,
                              inp.Q, inp.U, inp.V, precision=prec)
     if args.kernel:
-        rift.rift_ile_set_kernel(h, {"auto": 0, "direct": 1, "grouped": 2, "quad": 3, "tc": 4, "tile": 5, "tcs": 6}[args.kernel])
+        rift.rift_ile_set_kernel(h, {"auto": 0, "direct": 1, "tc": 2, "tcs": 3, "mma": 4}[args.kernel])
     ids = list(range(P))
     ps, ws = zip(*[synth.draw_samples(cfg, gids[p], theta_true=inp.theta_true[p]) for p in ids])
     params_np = np.concatenate(ps, axis=1)
@@ -408,7 +408,7 @@ def main() -> None:
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1)
     ap.add_argument("--precision", default="mixed", choices=["mixed", "fp64"])
-    ap.add_argument("--kernel", default=None, choices=[None, "auto", "direct", "grouped", "quad", "tc", "tile", "tcs"])
+    ap.add_argument("--kernel", default=None, choices=[None, "auto", "direct", "tc", "tcs", "mma"])
     ap.add_argument("--points", type=int, default=0, help="override the number of intrinsic points (debug)")
     ap.add_argument("--samples", type=int, default=0, help="override samples per point (debug)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")

@@ -44,8 +44,11 @@ enum {
 enum { RIFT_PREC_FP64 = 0, RIFT_PREC_MIXED = 1 };   /* arithmetic of the window term (reading A17) */
 enum { RIFT_Q_C128 = 0, RIFT_Q_C64 = 1 };           /* storage of Q on the device */
 enum { RIFT_MEM_HOST = 0, RIFT_MEM_DEVICE = 1 };    /* where the Q/U/V arrays passed to create live */
-enum { RIFT_KERNEL_AUTO = 0, RIFT_KERNEL_DIRECT = 1, RIFT_KERNEL_GROUPED = 2, RIFT_KERNEL_QUAD = 3, RIFT_KERNEL_TC = 4,
-       RIFT_KERNEL_TILE = 5, RIFT_KERNEL_TCS = 6 };   /* rift_ile_set_kernel */
+enum { RIFT_KERNEL_AUTO = 0, RIFT_KERNEL_DIRECT = 1, RIFT_KERNEL_TC = 2, RIFT_KERNEL_TCS = 3,
+       RIFT_KERNEL_MMA = 4 };                       /* rift_ile_set_kernel */
+enum { RIFT_OPT_TC_CHUNK_MIB = 1,   /* per-chunk workspace of the tensor-core kernels in MiB (default 1024, >= 1) */
+       RIFT_OPT_TC_SORT = 2,        /* 1 (default): AUTO may pick the shift-sorted tensor-core kernel; 0: never */
+       RIFT_OPT_QUAD_PROG = 3 };    /* 1 (default): quadratic term of > 8 modes by the pair program; 0: plain pair sum */
 
 #define RIFT_MAX_DET 8
 #define RIFT_MAX_MODES 80
@@ -118,10 +121,21 @@ int rift_ile_geometry(rift_ile_t *h, int32_t intrinsic_id, int64_t n, const doub
 
 /* Choose the fused-lnL kernel variant (RIFT_KERNEL_*); AUTO picks per configuration and call size: in mixed precision the
  * tensor-core kernels (TCS, which buckets the samples by the relative shift of detector 1, for calls of >= 32768 samples in
- * segments of >= 100 samples per bucket; else TC) when the configuration fits tensor and shared memory, else the direct
- * kernels; GROUPED, QUAD, TILE are opt-in.  A variant that does not apply to the handle falls back to the AUTO choice.
- * lnL does not depend on the variant beyond the stated tolerance of the precision mode. */
+ * segments of >= 100 samples per bucket; else TC) when the configuration fits tensor and shared memory; in fp64 mode the
+ * FP64 tensor-core kernel (MMA) when the configuration fits; else the direct kernels.  A variant that does not apply to
+ * the handle falls back to the AUTO choice.  lnL does not depend on the variant beyond the stated tolerance of the
+ * precision mode. */
 int rift_ile_set_kernel(rift_ile_t *h, int32_t variant);
+
+/* Tuning options (RIFT_OPT_*), all with defaults; nothing in the library reads the process environment.  Returns
+ * RIFT_EINVAL for an unknown option or a value out of range.  Takes effect from the next eval_batch. */
+int rift_ile_set_option(rift_ile_t *h, int32_t option, int64_t value);
+
+/* Pre-size every per-call workspace for eval_batch calls of up to n_seg segments x n_per_seg samples (and reduce calls of
+ * that shape with n_bins histogram bins, 0 = none), so that those calls allocate nothing (synchronous; cudaMalloc happens
+  * here; a changed reduce shape discards the pooled reduce state).  Without it the first call of a given size grows the
+ * workspace itself. */
+int rift_ile_reserve(rift_ile_t *h, int32_t n_seg, int64_t n_per_seg, int32_t n_bins);
 
 /* Number of kernels launched by this handle since creation (bench.py's gpu_launches), and the name of
  * the fused kernel variant the last eval_batch used. */
@@ -136,9 +150,11 @@ int rift_ile_profile(rift_ile_t *h, int32_t enable);
 int rift_ile_profile_read(rift_ile_t *h, double ms[4], int64_t launches[4]);
 
 /* Dense FMA-pipe microbenchmark (hard part H7): runs `iters` dependent-free FMA per thread over a grid
- * filling the device and returns achieved TFLOP/s in *tflops.  fp64: 0 = FFMA chains, 1 = DFMA chains, 2 = FFMA 7x8
- * register tile (all operands in registers, the operand pattern of the fused kernels). */
-int rift_ile_fma_peak(int32_t fp64, int32_t iters, double *tflops, void *cuda_stream);
+ * filling the device and returns achieved TFLOP/s in *tflops.  mode: 0 = FFMA chains, 1 = DFMA chains, 2 = FFMA 7x8
+ * register tile (all operands in registers, the operand pattern of the fused kernels), 3 / 4 / 5 = FP64 tensor-core
+ * mma.sync m8n8k4 / m16n8k8 / m16n8k16 (8 independent accumulator tiles per warp), 6 = m8n8k4 interleaved with as many
+ * independent DFMA per thread (reports the tensor part: do the two share a pipe?). */
+int rift_ile_fma_peak(int32_t mode, int32_t iters, double *tflops, void *cuda_stream);
 
 int rift_ile_destroy(rift_ile_t *h);
 const char *rift_ile_strerror(int code);

@@ -20,13 +20,13 @@ RIFT_OK, RIFT_EINVAL, RIFT_ENOMEM, RIFT_ECUDA, RIFT_EWINDOW, RIFT_ERANGE, RIFT_E
 RIFT_PREC_FP64, RIFT_PREC_MIXED = 0, 1
 RIFT_Q_C128, RIFT_Q_C64 = 0, 1
 RIFT_MEM_HOST, RIFT_MEM_DEVICE = 0, 1
-RIFT_KERNEL_AUTO, RIFT_KERNEL_DIRECT, RIFT_KERNEL_GROUPED, RIFT_KERNEL_QUAD, RIFT_KERNEL_TC, RIFT_KERNEL_TILE = 0, 1, 2, 3, 4, 5
-RIFT_KERNEL_TCS = 6
+RIFT_KERNEL_AUTO, RIFT_KERNEL_DIRECT, RIFT_KERNEL_TC, RIFT_KERNEL_TCS, RIFT_KERNEL_MMA = 0, 1, 2, 3, 4
+RIFT_OPT_TC_CHUNK_MIB, RIFT_OPT_TC_SORT, RIFT_OPT_QUAD_PROG = 1, 2, 3
 RIFT_N_PARAMS = 6
 
 EXPORTS = ("rift_ile_create", "rift_ile_eval_batch", "rift_ile_reduce", "rift_ile_geometry", "rift_ile_set_kernel",
            "rift_ile_launch_count", "rift_ile_kernel_name", "rift_ile_profile", "rift_ile_profile_read",
-           "rift_ile_fma_peak", "rift_ile_destroy",
+           "rift_ile_fma_peak", "rift_ile_set_option", "rift_ile_reserve", "rift_ile_destroy",
            "rift_ile_strerror", "rift_ile_last_error")
 AC_EXPORTS = ("rift_ac_create", "rift_ac_draw", "rift_ac_update", "rift_ac_update_dims", "rift_ac_get_masses",
               "rift_ac_ile_ln_weight", "rift_ac_destroy")
@@ -68,6 +68,10 @@ def lib() -> C.CDLL:
         L.rift_ile_geometry.restype = C.c_int
         L.rift_ile_set_kernel.argtypes = [vp, i32]
         L.rift_ile_set_kernel.restype = C.c_int
+        L.rift_ile_set_option.argtypes = [vp, i32, i64]
+        L.rift_ile_set_option.restype = C.c_int
+        L.rift_ile_reserve.argtypes = [vp, i32, i64, i32]
+        L.rift_ile_reserve.restype = C.c_int
         L.rift_ile_launch_count.argtypes = [vp]
         L.rift_ile_launch_count.restype = i64
         L.rift_ile_kernel_name.argtypes = [vp]
@@ -209,6 +213,14 @@ def rift_ile_set_kernel(h, variant: int) -> None:
     _check(lib().rift_ile_set_kernel(h, int(variant)), h)
 
 
+def rift_ile_set_option(h, option: int, value: int) -> None:
+    _check(lib().rift_ile_set_option(h, int(option), int(value)), h)
+
+
+def rift_ile_reserve(h, n_seg: int, n_per_seg: int, n_bins: int = 0) -> None:
+    _check(lib().rift_ile_reserve(h, int(n_seg), int(n_per_seg), int(n_bins)), h)
+
+
 def rift_ile_launch_count(h) -> int:
     return int(lib().rift_ile_launch_count(h))
 
@@ -229,9 +241,10 @@ def rift_ile_profile_read(h) -> dict:
     return dict(ms=[float(x) for x in ms], launches=[int(x) for x in nl])
 
 
-def rift_ile_fma_peak(fp64: bool, iters: int = 4096, cuda_stream: int = 0) -> float:
+def rift_ile_fma_peak(mode: int, iters: int = 4096, cuda_stream: int = 0) -> float:
+    """mode: 0 FFMA, 1 DFMA, 2 FFMA register tile, 3/4/5 FP64 mma.sync m8n8k4/m16n8k8/m16n8k16, 6 m8n8k4 + DFMA."""
     v = C.c_double()
-    _check(lib().rift_ile_fma_peak(int(fp64), int(iters), C.byref(v), int(cuda_stream) or None))
+    _check(lib().rift_ile_fma_peak(int(mode), int(iters), C.byref(v), int(cuda_stream) or None))
     return float(v.value)
 
 

@@ -24,8 +24,8 @@ struct rift_ile {
   QStore qse{};
   void *d_Qg = nullptr;            // the same extended layout for configurations whose Q block does NOT fit shared memory:
   QStore qsg{};                    // lnl_direct reads it from global memory with one address per mode row (no wrap arithmetic)
-  void *d_Qp = nullptr;            // planar, circularly extended copy for the grouped kernel (NULL if it cannot fit)
-  QStore qsp{};
+  MmaPlan mma{};                   // fp64 tensor-core path (lnl_mma.cu); mma.ok == 0 when the configuration does not fit
+  void *d_Qm = nullptr;            // its Q operand: [P][K][2 KS][pitch_q] bytes
   TcPlan tc{};                     // tensor-core path (lnl_tc.cu); tc.ok == 0 when the configuration does not fit
   uint32_t *d_Qtc = nullptr;       // A operand: [P][K][nt*128][acols] words of two fp16
   float *d_qscale = nullptr;       // [P] power-of-two scale of each point's Q in the A operand
@@ -37,12 +37,11 @@ struct rift_ile {
   uint16_t *d_Qs = nullptr;        // sorted variant (lnl_tcs.cu): extended detector-1 operand [P][kp/8][as_rows][8] fp16
   int32_t *tcs_key = nullptr, *tcs_perm = nullptr, *tcs_bkt = nullptr;   // natural-slot keys, sorted-slot permutation, bucket tables
   int64_t tcs_key_cap = 0, tcs_perm_cap = 0, tcs_bkt_cap = 0;
-  double *d_exp_tab = nullptr;     // [64] 2^(j/64) for the fp64 exponential of lnl_tile
-  int tile_ok = 0, tile_pitch = 0; // fp64 register-tiled kernel (lnl_tile.cu) usable for this handle
-  SortPlan plan{};
-  int32_t *d_bucket = nullptr, *d_perm = nullptr;
-  uint32_t *d_hist = nullptr;
-  size_t hist_cap = 0;
+  // options (rift_ile_set_option)
+  int64_t opt_tc_chunk_mib = 1024; // per-chunk workspace of the tensor-core kernels
+  int opt_tc_sort = 1;             // AUTO may pick the shift-sorted tensor-core kernel
+  int opt_quad_prog = 1;           // pair program of the quadratic term when M > 8
+  const double2 *qp_uv_saved = nullptr;   // the program's W table while the option is off
   // per-chunk workspace
   int64_t ws_cap = 0;
   Workspace ws{};
@@ -160,11 +159,10 @@ void free_handle(rift_ile *h) {
   }
   cudaFree(h->d_modes);
   cudaFree(h->d_Q);
-  cudaFree(h->d_Qp);
   cudaFree(h->d_Qe);
   cudaFree(h->d_Qtc);
+  cudaFree(h->d_Qm);
   cudaFree(h->d_qscale);
-  cudaFree(h->d_exp_tab);
   cudaFree(h->tc_blob);
   cudaFree(h->tc_c);
   cudaFree(h->tc_quad);
@@ -174,12 +172,8 @@ void free_handle(rift_ile *h) {
   cudaFree(h->tcs_key);
   cudaFree(h->tcs_perm);
   cudaFree(h->tcs_bkt);
-  cudaFree(h->d_bucket);
-  cudaFree(h->d_perm);
-  cudaFree(h->d_hist);
-  cudaFree(h->ws.orig);
   cudaFree(const_cast<uint32_t *>(h->qp.ent_full));
-  cudaFree(const_cast<double2 *>(h->qp.uv));
+  cudaFree(const_cast<double2 *>(h->qp.uv ? h->qp.uv : h->qp_uv_saved));
   cudaFree(h->d_Qg);
   cudaFree(h->d_U);
   cudaFree(h->d_V);
@@ -208,10 +202,6 @@ int ensure_workspace(rift_ile *h, int64_t n) {
   cudaFree(h->ws.scale_c);
   cudaFree(h->ws.quad);
   cudaFree(h->ws.shift);
-  cudaFree(h->ws.orig);
-  cudaFree(h->d_bucket);
-  cudaFree(h->d_perm);
-  h->d_bucket = h->d_perm = nullptr;
   h->ws = Workspace{};
   h->ws_cap = 0;
   CU(h, cudaMalloc(&h->ws.coef, (size_t)n * coef_bytes(h)));
@@ -219,9 +209,6 @@ int ensure_workspace(rift_ile *h, int64_t n) {
   CU(h, cudaMalloc(&h->ws.scale_c, (size_t)n * sizeof(double)));
   CU(h, cudaMalloc(&h->ws.quad, (size_t)n * sizeof(double)));
   CU(h, cudaMalloc(&h->ws.shift, (size_t)n * h->K * sizeof(int32_t)));
-  CU(h, cudaMalloc(&h->ws.orig, (size_t)n * sizeof(int32_t)));
-  CU(h, cudaMalloc(&h->d_bucket, (size_t)n * sizeof(int32_t)));
-  CU(h, cudaMalloc(&h->d_perm, (size_t)n * sizeof(int32_t)));
   h->ws_cap = n;
   return RIFT_OK;
 }
@@ -260,32 +247,8 @@ bool q_fits_smem(const rift_ile *h) {
   return lnl_direct_smem_bytes(h->qs, fp32, true) <= 227u * 1024u;
 }
 
-// AUTO resolves to direct_ext when one point's extended Q block fits in shared memory, else to direct.  The grouped
-// kernel is opt-in (RIFT_KERNEL_GROUPED): on C1 it does not yet beat the direct kernels, profiles/.
-bool use_grouped(const rift_ile *h) {
-  if (h->kernel_variant != RIFT_KERNEL_GROUPED) return false;
-  return h->d_Qp != nullptr;
-}
-bool use_quad(const rift_ile *h) {
-  if (h->kernel_variant != RIFT_KERNEL_QUAD) return false;
-  const bool fp32 = h->precision == RIFT_PREC_MIXED;
-  return h->d_Qe != nullptr && lnl_quad_smem_bytes(h->qse, fp32) <= 227u * 1024u;
-}
-
-int32_t next_pow2(int64_t v) {
-  int32_t p = 1;
-  while (p < v && p < (1 << 30)) p <<= 1;
-  return p;
-}
-
 
 // ---- tensor-core path ------------------------------------------------------------------------------------------------
-// per-chunk workspace of the tensor-core kernels in MiB (RIFT_TC_CHUNK_MIB, read at every call; default 1024)
-int tc_chunk_mib() {
-  const char *e = getenv("RIFT_TC_CHUNK_MIB");
-  return (e && atoi(e) > 0) ? atoi(e) : 1024;
-}
-
 void make_tc_plan(rift_ile *h, double delta_t) {
   TcPlan &tp = h->tc;
   tp = TcPlan{};
@@ -336,12 +299,46 @@ void make_tc_plan(rift_ile *h, double delta_t) {
   }
 }
 
-// opt-in (RIFT_KERNEL_TILE): on C1 fp64 it measures 7.1 ms against 6.1 ms of lnl_direct
-bool use_tile(const rift_ile *h) { return h->tile_ok && h->kernel_variant == RIFT_KERNEL_TILE; }
+// fp64 mode: plan of the DMMA kernel.  Whole Q block of a point resident in shared memory when it fits beside the window
+// buffer of a 16-sample batch, else streamed in (detector, 512-row range, k-step) chunks through a 4- or 3-slot ring.
+void make_mma_plan(rift_ile *h) {
+  MmaPlan &p = h->mma;
+  p = MmaPlan{};
+  if (h->precision != RIFT_PREC_FP64) return;
+  p.K = h->K;
+  p.M = h->M;
+  p.KS = (h->M + 1) / 2;
+  p.n_t = h->n_t;
+  p.n_r = (h->n_t + 7) & ~7;
+  p.n_tau = h->n_tau;
+  p.circular = h->n_tau == h->n_t ? 1 : 0;
+  p.n_x = h->n_tau;
+  p.j0 = (h->n_t - h->n_tau) / 2;
+  p.xp = p.n_x + ((2 - p.n_x) & 7);                   // pitch = 2 (mod 8) doubles: the unshifted store is conflict-free
+  p.pitch_q = p.n_r * 16 + 64;
+  p.point_stride = (int64_t)p.K * 2 * p.KS * p.pitch_q;
+  const int cand[][3] = {{0, 2, 0}, {1, 2, 4}, {1, 2, 3}, {0, 1, 0}, {1, 1, 4}, {1, 1, 3}};   // stream, nt, slots
+  for (const auto &c : cand) {
+    p.stream = c[0];
+    p.nt = c[1];
+    p.slots = c[2];
+    const int tr_max = p.stream ? 480 : 512;              // 32 rows per consumer warp (15 with a producer warp, else 16)
+    p.tr = p.n_r < tr_max ? p.n_r : tr_max;
+    if (!p.stream && p.point_stride >= (1ll << 31)) continue;
+    if (lnl_mma_smem_bytes(p) <= 227u * 1024u) {
+      p.ok = 1;
+      return;
+    }
+  }
+}
+
+bool use_mma(const rift_ile *h) {
+  return h->mma.ok && h->d_Qm != nullptr && h->kernel_variant != RIFT_KERNEL_DIRECT;
+}
 
 bool use_tc(const rift_ile *h) {
   if (!h->tc.ok || h->d_Qtc == nullptr) return false;
-  return h->kernel_variant == RIFT_KERNEL_AUTO || h->kernel_variant == RIFT_KERNEL_TC || h->kernel_variant == RIFT_KERNEL_TCS;
+  return h->kernel_variant != RIFT_KERNEL_DIRECT;              // a variant of the other precision mode = AUTO
 }
 
 // Sorted variant: worth it when the padding of the shift buckets (about 7.5 slots per bucket and segment) stays small:
@@ -349,8 +346,7 @@ bool use_tc(const rift_ile *h) {
 bool use_tcs(const rift_ile *h, int32_t n_seg, int64_t n_per_seg) {
   if (!h->tc.srt_ok || h->d_Qs == nullptr) return false;
   if (h->kernel_variant == RIFT_KERNEL_TCS) return true;
-  const char *e = getenv("RIFT_TC_SORT");                                // RIFT_TC_SORT=0: never pick it automatically
-  const bool auto_on = !(e && atoi(e) == 0);
+  const bool auto_on = h->opt_tc_sort != 0;                              // RIFT_OPT_TC_SORT = 0: never pick it automatically
   // small calls are launch-bound and the bucketing adds five launches (C0: 0.10 -> 0.125 ms)
   return auto_on && h->kernel_variant == RIFT_KERNEL_AUTO && n_per_seg >= 100 * (int64_t)h->tc.n_bkt &&
          (int64_t)n_seg * n_per_seg >= 32768;
@@ -383,18 +379,27 @@ int ensure_tc_workspace(rift_ile *h, int64_t n_batches, int blob_words = 0) {
 // chunks of whole 16-sample batches.  The per-chunk workspace is 1 GiB by default (RIFT_TC_CHUNK_MIB overrides): measured on
 // C1, every extra launch of the fused kernel costs ~30 us (tensor-memory allocation, A-operand load, pipeline fill, tail),
 // far more than keeping the blobs L2-resident saves (64 MiB chunks: 1.39 ms per step, one chunk: 1.24 ms)
+// sizes the workspace of run_chunks_tc for a call shape (also rift_ile_reserve); *cap_out = batches per chunk
+int prepare_tc(rift_ile *h, int32_t n_seg, int64_t n_per_seg, int64_t *cap_out) {
+  const int64_t nbps = (n_per_seg + RIFT_TC_NB - 1) / RIFT_TC_NB;
+  const int64_t total = (int64_t)n_seg * nbps;
+  const size_t per_batch = (size_t)h->tc.n_sub * h->tc.blob_words * 4 + (size_t)RIFT_TC_NB * (16 + 32);
+  const int64_t chunk_mib = h->opt_tc_chunk_mib;
+  int64_t cap = (int64_t)(((size_t)chunk_mib << 20) / per_batch);
+  if (cap < 8 * (int64_t)h->n_sm) cap = 8 * (int64_t)h->n_sm;
+  // mode-subset passes stream their window sums through HBM anyway and reload the A operand per launch: larger chunks
+  if (h->tc.n_sub > 1 && cap < 65536) cap = 65536;
+  *cap_out = cap;
+  return ensure_tc_workspace(h, total < cap ? total : cap);
+}
+
 int run_chunks_tc(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *const params[6], double *lnL_out,
                   int32_t *shift_out, cudaStream_t s) {
   const int64_t nbps = (n_per_seg + RIFT_TC_NB - 1) / RIFT_TC_NB;
   const int64_t total = (int64_t)n_seg * nbps;
   if (total == 0) return RIFT_OK;
-  const size_t per_batch = (size_t)h->tc.n_sub * h->tc.blob_words * 4 + (size_t)RIFT_TC_NB * (16 + 32);
-  const int chunk_mib = tc_chunk_mib();
-  int64_t cap = (int64_t)(((size_t)chunk_mib << 20) / per_batch);
-  if (cap < 8 * (int64_t)h->n_sm) cap = 8 * (int64_t)h->n_sm;
-  // mode-subset passes stream their window sums through HBM anyway and reload the A operand per launch: larger chunks
-  if (h->tc.n_sub > 1 && cap < 65536) cap = 65536;
-  int rc = ensure_tc_workspace(h, total < cap ? total : cap);
+  int64_t cap = 0;
+  int rc = prepare_tc(h, n_seg, n_per_seg, &cap);
   if (rc != RIFT_OK) return rc;
   for (int64_t gb0 = 0; gb0 < total; gb0 += cap) {
     TcChunk c{};
@@ -448,17 +453,16 @@ int ensure_i32(rift_ile *h, int32_t **p, int64_t *cap, int64_t need) {
   return RIFT_OK;
 }
 
-int run_chunks_tcs(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *const params[6], double *lnL_out,
-                   int32_t *shift_out, cudaStream_t s) {
+int prepare_tcs(rift_ile *h, int32_t n_seg, int64_t n_per_seg, int64_t *cap_out) {
   const TcPlan &tp = h->tc;
   const int64_t nbps = (n_per_seg + RIFT_TC_NB - 1) / RIFT_TC_NB;
   const int64_t total = (int64_t)n_seg * nbps;
-  if (total == 0) return RIFT_OK;
   const size_t per_batch = (size_t)tp.n_sub * tp.blob_words_s * 4 + (size_t)RIFT_TC_NB * (16 + 32 + 8);
-  const int chunk_mib = tc_chunk_mib();
+  const int64_t chunk_mib = h->opt_tc_chunk_mib;
   int64_t cap = (int64_t)(((size_t)chunk_mib << 20) / per_batch);
   if (cap < 8 * (int64_t)h->n_sm) cap = 8 * (int64_t)h->n_sm;
   if (tp.n_sub > 1 && cap < 65536) cap = 65536;                              // mode-subset passes: as in run_chunks_tc
+  *cap_out = cap;
   const int64_t nb_max = total < cap ? total : cap;
   int64_t lseg_max = nb_max / nbps + 2;
   if (lseg_max > n_seg) lseg_max = n_seg;
@@ -466,6 +470,17 @@ int run_chunks_tcs(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *
   if (rc == RIFT_OK) rc = ensure_i32(h, &h->tcs_key, &h->tcs_key_cap, 2 * nb_max * RIFT_TC_NB);   // keys, positions
   if (rc == RIFT_OK) rc = ensure_i32(h, &h->tcs_perm, &h->tcs_perm_cap, (nb_max + lseg_max * tp.n_bkt) * RIFT_TC_NB);
   if (rc == RIFT_OK) rc = ensure_i32(h, &h->tcs_bkt, &h->tcs_bkt_cap, 2 * lseg_max * tp.n_bkt + lseg_max + 1);
+  return rc;
+}
+
+int run_chunks_tcs(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *const params[6], double *lnL_out,
+                   int32_t *shift_out, cudaStream_t s) {
+  const TcPlan &tp = h->tc;
+  const int64_t nbps = (n_per_seg + RIFT_TC_NB - 1) / RIFT_TC_NB;
+  const int64_t total = (int64_t)n_seg * nbps;
+  if (total == 0) return RIFT_OK;
+  int64_t cap = 0;
+  int rc = prepare_tcs(h, n_seg, n_per_seg, &cap);
   if (rc != RIFT_OK) return rc;
   for (int64_t gb0 = 0; gb0 < total; gb0 += cap) {
     TcChunk c{};
@@ -518,6 +533,45 @@ int run_chunks_tcs(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *
   return RIFT_OK;
 }
 
+int ensure_reduce_state(rift_ile *h, int32_t n_seg, int32_t nb) {
+  if (h->state_nseg == n_seg && h->state_nbins == nb) return RIFT_OK;
+  cudaFree(h->d_state);
+  cudaFree(h->d_state_hist);
+  h->d_state = nullptr;
+  h->d_state_hist = nullptr;
+  h->state_nseg = 0;
+  h->state_nbins = -1;
+  CU(h, cudaMalloc(&h->d_state, sizeof(ReduceState) * n_seg));
+  if (nb > 0) CU(h, cudaMalloc(&h->d_state_hist, sizeof(double) * (size_t)n_seg * 6 * nb));
+  h->state_nseg = n_seg;
+  h->state_nbins = nb;
+  return RIFT_OK;
+}
+
+int ensure_reduce_buffers(rift_ile *h, int32_t n_seg, int64_t n_per_seg, int32_t nb) {
+  const int32_t bps = reduce_blocks_per_seg(n_per_seg, n_seg);
+  const size_t need_partial = reduce_partial_doubles(n_seg, bps, nb);
+  if (need_partial > h->partial_cap) {
+    cudaFree(h->d_partial);
+    h->d_partial = nullptr;
+    h->partial_cap = 0;
+    CU(h, cudaMalloc(&h->d_partial, need_partial * sizeof(double)));
+    h->partial_cap = need_partial;
+  }
+  const size_t need_out = (size_t)n_seg * (4 + 6 * (size_t)nb);
+  if (need_out > h->out_cap) {
+    cudaFree(h->d_out);
+    if (h->h_out) cudaFreeHost(h->h_out);
+    h->d_out = nullptr;
+    h->h_out = nullptr;
+    h->out_cap = 0;
+    CU(h, cudaMalloc(&h->d_out, need_out * sizeof(double)));
+    CU(h, cudaMallocHost(&h->h_out, need_out * sizeof(double)));
+    h->out_cap = need_out;
+  }
+  return RIFT_OK;
+}
+
 int run_chunks(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *const params[6], double *lnL_out,
                int32_t *shift_out, double *dbg_F, double *dbg_Y, double *dbg_quad, cudaStream_t s) {
   const int64_t total = (int64_t)n_seg * n_per_seg;
@@ -527,8 +581,6 @@ int run_chunks(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *cons
   if (rc != RIFT_OK) return rc;
   const bool fp32 = h->precision == RIFT_PREC_MIXED;
   const bool in_smem = q_fits_smem(h);
-  const bool quad = lnL_out != nullptr && use_quad(h);
-  const bool grouped = lnL_out != nullptr && (use_grouped(h) || quad);      // "grouped": sort the chunk first
   for (int64_t g0 = 0; g0 < total; g0 += cap) {
     Batch b;
     b.n_per_seg = n_per_seg;
@@ -536,38 +588,10 @@ int run_chunks(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *cons
     b.n = (total - g0 < cap) ? total - g0 : cap;
     b.ids = h->d_ids;
     Workspace ws = h->ws;
-    const int32_t *perm = nullptr;
-    if (grouped) {
-      const int32_t n_seg_chunk = (int32_t)((g0 + b.n - 1) / n_per_seg - g0 / n_per_seg + 1);
-      SortPlan sp = h->plan;
-      int32_t nb = sp.n_buckets;
-      const int32_t by_n = next_pow2(n_per_seg);
-      if (nb > by_n) nb = by_n;
-      while ((int64_t)nb * n_seg_chunk > (16ll << 20) && nb > 1) nb >>= 1;
-      if (nb != sp.n_buckets) {
-        sp.exact = 0;
-        sp.n_buckets = nb;
-      }
-      const size_t need = (size_t)nb * n_seg_chunk;
-      if (need > h->hist_cap) {
-        cudaFree(h->d_hist);
-        h->d_hist = nullptr;
-        h->hist_cap = 0;
-        CU(h, cudaMalloc(&h->d_hist, need * sizeof(uint32_t)));
-        h->hist_cap = need;
-      }
-      int nl = 0;
-      ProfSpan ps(h, 3, s);
-      CU(h, launch_group_sort(h->geom, sp, b, params, h->d_bucket, h->d_hist, n_seg_chunk, h->d_perm, s, &nl));
-      ps.end();
-      h->launches += nl;
-      perm = h->d_perm;
-    } else {
-      ws.orig = nullptr;
-    }
+    ws.orig = nullptr;
     {
       ProfSpan ps(h, 0, s);
-      CU(h, launch_geometry(h->geom, h->d_modes, b, params, h->d_U, h->d_V, h->qp, fp32, ws, shift_out, dbg_F, dbg_Y, perm, s));
+      CU(h, launch_geometry(h->geom, h->d_modes, b, params, h->d_U, h->d_V, h->qp, fp32, ws, shift_out, dbg_F, dbg_Y, nullptr, s));
       ps.end();
     }
     ++h->launches;
@@ -575,20 +599,12 @@ int run_chunks(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *cons
     if (lnL_out) {
       int nl = 0;
       ProfSpan ps(h, 1, s);
-      if (quad) {
-        CU(h, launch_lnl_quad(h->qse, fp32, b, ws, h->K, lnL_out, h->n_sm, s, &nl));
-        h->kernel_name = fp32 ? "lnl_quad<f32>" : "lnl_quad<f64>";
-      } else if (grouped) {
-        CU(h, launch_lnl_grouped(h->qsp, fp32, b, ws, h->K, lnL_out, h->n_sm, s, &nl));
-        h->kernel_name = fp32 ? "lnl_grouped<f32>" : "lnl_grouped<f64>";
-      } else if (!fp32 && use_tile(h)) {
-        CU(h, launch_lnl_tile(h->qs, b, ws, h->K, h->tc.H, h->tile_pitch, h->tc.dmax, h->d_exp_tab, lnL_out, h->n_sm, s,
-                              &nl));
-        h->kernel_name = "lnl_tile<f64>";
-      } else if (h->d_Qe != nullptr && fp32 && h->kernel_variant != RIFT_KERNEL_DIRECT) {
-        // (fp64: the extended block leaves room for one CTA per SM only and measures slower than direct)
+      if (!fp32 && use_mma(h)) {
+        CU(h, launch_lnl_mma(h->mma, h->d_Qm, b, ws, lnL_out, h->n_sm, s, &nl));
+        h->kernel_name = h->mma.stream ? "lnl_mma<f64,stream>" : "lnl_mma<f64,resident>";
+      } else if (h->d_Qe != nullptr && fp32) {
         CU(h, launch_lnl_direct_ext(h->qse, fp32, b, ws, h->K, lnL_out, h->n_sm, s, &nl));
-        h->kernel_name = fp32 ? "lnl_direct_ext<f32>" : "lnl_direct_ext<f64>";
+        h->kernel_name = "lnl_direct_ext<f32>";
       } else {
         const bool ext = !in_smem && h->d_Qg != nullptr;
         CU(h, launch_lnl_direct(ext ? h->qsg : h->qs, fp32, in_smem, ext, b, ws, h->K, lnL_out, h->n_sm, s, &nl));
@@ -704,7 +720,7 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
   CUC(cudaMalloc(&h->d_V, uv_bytes));
   CUC(cudaMemcpy(h->d_U, cfg->U, uv_bytes, kind));
   CUC(cudaMemcpy(h->d_V, cfg->V, uv_bytes, kind));
-  if (h->M > 8 && !getenv("RIFT_NO_QUAD_PROG")) {
+  if (h->M > 8) {
     // pair program of the quadratic term (QuadProg, rift_internal.h): entries grouped by matrix and phase exponent
     const int M = h->M;
     int n_max = 0;
@@ -742,9 +758,11 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
       h->qp.ent_full = d_ent;
       CUC(cudaMemcpy(d_ent, ent.data(), ent.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
       CUC(cudaMalloc(&d_uv, (size_t)h->P * ent.size() * h->K * sizeof(double2)));
+      h->qp_uv_saved = d_uv;                                 // owned by the handle from here on (free_handle)
       CUC(launch_build_quad_uv(h->qp, h->d_U, h->d_V, h->P, h->K, h->M, d_uv, 0));
       CUC(cudaStreamSynchronize(0));
       h->qp.uv = d_uv;
+      h->qp_uv_saved = nullptr;
     }
   }
   {
@@ -778,13 +796,13 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
       qe.n_tau = h->n_tau;
       qe.km = h->K * h->M;
       qe.point_stride_bytes = (int64_t)h->K * h->M * n_te * csz;
-      if (e == cudaSuccess && lnl_direct_ext_smem_bytes(qe, fp32) <= 227u * 1024u) {
+      if (e == cudaSuccess && fp32 && lnl_direct_ext_smem_bytes(qe, fp32) <= 227u * 1024u) {   // fp64: measured slower than direct
         e = cudaMalloc(&h->d_Qe, (size_t)h->P * qe.point_stride_bytes);
         if (e == cudaSuccess) e = launch_convert_q_ext(src, h->d_Qe, rows, h->n_t, n_te, fp32, 0);
         qe.data = h->d_Qe;
         h->qse = qe;
-        h->launches += h->tc.n_sub;
-      } else if (e == cudaSuccess && !block_fits && !getenv("RIFT_NO_GLOBAL_EXT")) {
+        ++h->launches;
+      } else if (e == cudaSuccess && !block_fits) {
         e = cudaMalloc(&h->d_Qg, (size_t)h->P * qe.point_stride_bytes);
         if (e == cudaSuccess) e = launch_convert_q_ext(src, h->d_Qg, rows, h->n_t, n_te, fp32, 0);
         qe.data = h->d_Qg;
@@ -792,25 +810,18 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
         ++h->launches;
       }
     }
-    // planar, circularly extended copy for the grouped kernel, if one point's block fits in shared memory
-    {
-      const size_t rsz = fp32 ? 4 : 8;
-      const int32_t n_tpp = (h->n_t + RIFT_EXT + 3) & ~3;
-      QStore qp{};
-      qp.n_t = h->n_t;
-      qp.n_tp = n_tpp;
-      qp.n_tau = h->n_tau;
-      qp.km = h->K * h->M;
-      qp.point_stride_bytes = (int64_t)2 * h->K * h->M * n_tpp * rsz;
-      if (e == cudaSuccess && lnl_grouped_smem_bytes(qp, fp32) <= 227u * 1024u) {
-        e = cudaMalloc(&h->d_Qp, (size_t)h->P * qp.point_stride_bytes);
-        if (e == cudaSuccess) e = launch_convert_q_planar(src, h->d_Qp, rows, h->n_t, n_tpp, fp32, 0);
-        qp.data = h->d_Qp;
-        h->qsp = qp;
+    // Q operand of the fp64 tensor-core kernel.  An allocation failure of this optional layout leaves the variant unavailable.
+    make_mma_plan(h);
+    if (e == cudaSuccess && h->mma.ok) {
+      if (cudaMalloc(&h->d_Qm, (size_t)h->P * h->mma.point_stride) == cudaSuccess) {
+        e = launch_convert_q_mma(src, h->d_Qm, h->mma, h->P, 0);
         ++h->launches;
+      } else {
+        cudaGetLastError();
+        h->d_Qm = nullptr;
       }
     }
-    // A operand of the tensor-core path (tf32 hi | lo pieces), when the configuration fits tensor memory
+    // A operand of the tensor-core path (fp16 hi | lo pieces), when the configuration fits tensor memory
     make_tc_plan(h, cfg->delta_t);
     if (e == cudaSuccess && h->tc.ok) {
       const size_t words = (size_t)h->tc.n_sub * h->P * h->K * h->tc.nt * 128 * h->tc.acols;
@@ -824,22 +835,6 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
         ++h->launches;
       }
     }
-    // fp64 register-tiled kernel: circular window of at most 4 row tiles, Q block + exchange buffers in shared memory
-    if (e == cudaSuccess && h->precision == RIFT_PREC_FP64 && h->n_tau == h->n_t && h->n_t <= 512 && h->tc.H < h->n_t &&
-        8 * h->K * h->M <= 512) {
-      QStore qq{};
-      qq.km = h->K * h->M;
-      qq.point_stride_bytes = (int64_t)h->K * h->M * h->n_tp * 16;
-      const int pitch = (h->n_t + 2 * h->tc.H + 1) & ~1;
-      if (lnl_tile_smem_bytes(qq, h->K, pitch) <= 227u * 1024u) {
-        double tab[64];
-        for (int j = 0; j < 64; ++j) tab[j] = std::exp2(j / 64.0);
-        e = cudaMalloc(&h->d_exp_tab, sizeof(tab));
-        if (e == cudaSuccess) e = cudaMemcpy(h->d_exp_tab, tab, sizeof(tab), cudaMemcpyHostToDevice);
-        h->tile_ok = (e == cudaSuccess);
-        h->tile_pitch = pitch;
-      }
-    }
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     cudaFree(tmp);
     if (e != cudaSuccess) return bail(RIFT_ECUDA);
@@ -850,24 +845,6 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
     h->qs.n_tau = h->n_tau;
     h->qs.km = h->K * h->M;
     h->qs.point_stride_bytes = (int64_t)h->K * h->M * h->n_tp * csz;
-  }
-  {  // grouping plan: ranges of the relative shifts d_k = s_k - s_0
-    SortPlan &sp = h->plan;
-    int64_t prod = 1;
-    for (int k = 0; k < RIFT_MAX_DET; ++k) sp.half[k] = sp.range[k] = 1;
-    for (int k = 1; k < h->K; ++k) {
-      double d2 = 0;
-      for (int i = 0; i < 3; ++i) {
-        const double d = h->geom.loc[k][i] - h->geom.loc[0][i];
-        d2 += d * d;
-      }
-      const int m = (int)std::ceil(std::sqrt(d2) / (RIFT_C_LIGHT * cfg->delta_t)) + 1;
-      sp.half[k] = m;
-      sp.range[k] = 2 * m + 1;
-      if (prod <= (1ll << 40)) prod *= sp.range[k];
-    }
-    sp.exact = prod <= 65536 ? 1 : 0;
-    sp.n_buckets = sp.exact ? next_pow2(prod) : 65536;
   }
 #undef CUC
   (void)rc;
@@ -884,11 +861,60 @@ int rift_ile_destroy(rift_ile_t *h) {
 
 int rift_ile_set_kernel(rift_ile_t *h, int32_t variant) {
   if (!h) return RIFT_EINVAL;
-  if (variant != RIFT_KERNEL_AUTO && variant != RIFT_KERNEL_DIRECT && variant != RIFT_KERNEL_GROUPED && variant != RIFT_KERNEL_QUAD &&
-      variant != RIFT_KERNEL_TC && variant != RIFT_KERNEL_TILE && variant != RIFT_KERNEL_TCS)
+  if (variant != RIFT_KERNEL_AUTO && variant != RIFT_KERNEL_DIRECT && variant != RIFT_KERNEL_TC && variant != RIFT_KERNEL_TCS &&
+      variant != RIFT_KERNEL_MMA)
     return fail(h, RIFT_EINVAL, "unknown kernel variant");
   h->kernel_variant = variant;
   return RIFT_OK;
+}
+
+int rift_ile_set_option(rift_ile_t *h, int32_t option, int64_t value) {
+  if (!h) return RIFT_EINVAL;
+  switch (option) {
+    case RIFT_OPT_TC_CHUNK_MIB:
+      if (value < 1 || value > (1 << 20)) return fail(h, RIFT_EINVAL, "RIFT_OPT_TC_CHUNK_MIB out of range");
+      h->opt_tc_chunk_mib = value;
+      return RIFT_OK;
+    case RIFT_OPT_TC_SORT:
+      h->opt_tc_sort = value != 0;
+      return RIFT_OK;
+    case RIFT_OPT_QUAD_PROG:
+      if ((value != 0) != (h->opt_quad_prog != 0)) {            // the program's W table is kept while the option is off
+        std::swap(h->qp.uv, h->qp_uv_saved);
+        h->opt_quad_prog = value != 0;
+      }
+      return RIFT_OK;
+    default:
+      return fail(h, RIFT_EINVAL, "unknown option");
+  }
+}
+
+int rift_ile_reserve(rift_ile_t *h, int32_t n_seg, int64_t n_per_seg, int32_t n_bins) {
+  if (!h) return RIFT_EINVAL;
+  if (n_seg < 0 || n_seg > 65535 || n_per_seg < 0 || n_bins < 0 || n_bins > 1024) return fail(h, RIFT_EINVAL, "bad size");
+  if (n_seg == 0 || n_per_seg == 0) return RIFT_OK;
+  DeviceGuard g(h->device);
+  if (n_seg > h->ids_cap) {
+    cudaFree(h->d_ids);
+    h->d_ids = nullptr;
+    h->ids_cap = 0;
+    h->ids_last.clear();
+    CU(h, cudaMalloc(&h->d_ids, (size_t)n_seg * sizeof(int32_t)));
+    h->ids_cap = n_seg;
+  }
+  int rc = RIFT_OK;
+  int64_t cap = 0;
+  if (use_tc(h) && use_tcs(h, n_seg, n_per_seg)) {
+    rc = prepare_tcs(h, n_seg, n_per_seg, &cap);
+  } else if (use_tc(h)) {
+    rc = prepare_tc(h, n_seg, n_per_seg, &cap);
+  } else {
+    const int64_t total = (int64_t)n_seg * n_per_seg, c = chunk_samples(h);
+    rc = ensure_workspace(h, total < c ? total : c);
+  }
+  if (rc == RIFT_OK) rc = ensure_reduce_buffers(h, n_seg, n_per_seg, n_bins);
+  if (rc == RIFT_OK) rc = ensure_reduce_state(h, n_seg, n_bins);       // a changed shape discards the pooled reduce state
+  return rc;
 }
 
 int rift_ile_eval_batch(rift_ile_t *h, int32_t n_seg, const int32_t *intrinsic_ids, int64_t n_per_seg,
@@ -945,37 +971,15 @@ int rift_ile_reduce(rift_ile_t *h, int32_t n_seg, int64_t n_per_seg, const doubl
   DeviceGuard g(h->device);
   cudaStream_t s = reinterpret_cast<cudaStream_t>(cuda_stream);
 
-  if (!merge && (h->state_nseg != n_seg || h->state_nbins != nb)) {
-    cudaFree(h->d_state);
-    cudaFree(h->d_state_hist);
-    h->d_state = nullptr;
-    h->d_state_hist = nullptr;
-    h->state_nseg = 0;
-    h->state_nbins = -1;
-    CU(h, cudaMalloc(&h->d_state, sizeof(ReduceState) * n_seg));
-    if (nb > 0) CU(h, cudaMalloc(&h->d_state_hist, sizeof(double) * (size_t)n_seg * 6 * nb));
-    h->state_nseg = n_seg;
-    h->state_nbins = nb;
+  if (!merge) {
+    const int rc = ensure_reduce_state(h, n_seg, nb);
+    if (rc != RIFT_OK) return rc;
   }
   const int32_t bps = reduce_blocks_per_seg(n_per_seg, n_seg);
-  const size_t need_partial = reduce_partial_doubles(n_seg, bps, nb);
-  if (need_partial > h->partial_cap) {
-    cudaFree(h->d_partial);
-    h->d_partial = nullptr;
-    h->partial_cap = 0;
-    CU(h, cudaMalloc(&h->d_partial, need_partial * sizeof(double)));
-    h->partial_cap = need_partial;
-  }
   const size_t need_out = (size_t)n_seg * (4 + 6 * (size_t)nb);
-  if (need_out > h->out_cap) {
-    cudaFree(h->d_out);
-    if (h->h_out) cudaFreeHost(h->h_out);
-    h->d_out = nullptr;
-    h->h_out = nullptr;
-    h->out_cap = 0;
-    CU(h, cudaMalloc(&h->d_out, need_out * sizeof(double)));
-    CU(h, cudaMallocHost(&h->h_out, need_out * sizeof(double)));
-    h->out_cap = need_out;
+  {
+    const int rc = ensure_reduce_buffers(h, n_seg, n_per_seg, nb);
+    if (rc != RIFT_OK) return rc;
   }
   double *d_scalars = h->d_out, *d_hist = h->d_out + 4 * (size_t)n_seg;
   int nl = 0;

@@ -103,6 +103,65 @@ __global__ void __launch_bounds__(256) fma_tile_kernel(int iters, const float *_
   if (s == 123.456f) sink[0] = s;
 }
 
+
+// FP64 tensor-core (DMMA) microbenchmarks: `mma.sync.aligned.m8n8k4.f64` and the larger sm_90+ shapes m16n8k8 / m16n8k16,
+// NACC independent accumulator tiles per warp, all operands in registers.  modes 3, 4, 5 of run_fma_peak; mode 6 interleaves
+// m8n8k4 with as many independent DFMA per thread (do the two share a pipe?).
+__device__ __forceinline__ void dmma884(double (&d)[2], double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
+}
+__device__ __forceinline__ void dmma1688(double (&d)[4], const double (&a)[4], const double (&b)[2]) {
+  asm volatile("mma.sync.aligned.m16n8k8.row.col.f64.f64.f64.f64 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+               : "+d"(d[0]), "+d"(d[1]), "+d"(d[2]), "+d"(d[3])
+               : "d"(a[0]), "d"(a[1]), "d"(a[2]), "d"(a[3]), "d"(b[0]), "d"(b[1]));
+}
+__device__ __forceinline__ void dmma16816(double (&d)[4], const double (&a)[8], const double (&b)[4]) {
+  asm volatile("mma.sync.aligned.m16n8k16.row.col.f64.f64.f64.f64 {%0,%1,%2,%3}, {%4,%5,%6,%7,%8,%9,%10,%11}, {%12,%13,%14,%15}, {%0,%1,%2,%3};"
+               : "+d"(d[0]), "+d"(d[1]), "+d"(d[2]), "+d"(d[3])
+               : "d"(a[0]), "d"(a[1]), "d"(a[2]), "d"(a[3]), "d"(a[4]), "d"(a[5]), "d"(a[6]), "d"(a[7]), "d"(b[0]), "d"(b[1]),
+                 "d"(b[2]), "d"(b[3]));
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(256) dmma_peak_kernel(int iters, const double *__restrict__ src, double *sink) {
+  constexpr int NACC = 8;
+  double a[8], b[4];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) a[i] = src[threadIdx.x + 32 * i];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) b[i] = src[300 + threadIdx.x + 32 * i];
+  double s = 0;
+  if (MODE == 3 || MODE == 6) {
+    double d[NACC][2], f[NACC];
+#pragma unroll
+    for (int t = 0; t < NACC; ++t) d[t][0] = d[t][1] = 0.0, f[t] = a[t & 7];
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+      for (int t = 0; t < NACC; ++t) {
+        dmma884(d[t], a[t & 7], b[t & 3]);
+        if (MODE == 6) f[t] = fma(f[t], 0.999999, 1e-6);
+      }
+    }
+#pragma unroll
+    for (int t = 0; t < NACC; ++t) s += d[t][0] + d[t][1] + (MODE == 6 ? f[t] : 0.0);
+  } else {
+    double d[NACC][4];
+#pragma unroll
+    for (int t = 0; t < NACC; ++t) d[t][0] = d[t][1] = d[t][2] = d[t][3] = 0.0;
+    const double a4[4] = {a[0], a[1], a[2], a[3]}, b2[2] = {b[0], b[1]};
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+      for (int t = 0; t < NACC; ++t) {
+        if (MODE == 4) dmma1688(d[t], a4, b2);
+        else dmma16816(d[t], a, b);
+      }
+    }
+#pragma unroll
+    for (int t = 0; t < NACC; ++t) s += d[t][0] + d[t][1] + d[t][2] + d[t][3];
+  }
+  if (s == 123.456) sink[0] = s;
+}
+
 }  // namespace
 
 cudaError_t launch_convert_q(const double *Q_c128, void *dst, int64_t rows, int32_t n_t, int32_t n_tp, bool to_fp32,
@@ -159,9 +218,9 @@ cudaError_t run_fma_peak(int mode, int iters, double *tflops, cudaStream_t s) {
   void *src = nullptr;
   cudaError_t e = cudaMalloc(&sink, 64);
   if (e != cudaSuccess) return e;
-  e = cudaMalloc(&src, 4096);
+  e = cudaMalloc(&src, 8192);
   if (e != cudaSuccess) return e;
-  cudaMemsetAsync(src, 0, 4096, s);
+  cudaMemsetAsync(src, 0, 8192, s);
   cudaEvent_t t0, t1;
   cudaEventCreate(&t0);
   cudaEventCreate(&t1);
@@ -171,6 +230,14 @@ cudaError_t run_fma_peak(int mode, int iters, double *tflops, cudaStream_t s) {
     cudaEventRecord(t0, s);
     if (mode == 2)
       fma_tile_kernel<<<grid, threads, 0, s>>>(iters, reinterpret_cast<const float *>(src), reinterpret_cast<float *>(sink));
+    else if (mode == 3)
+      dmma_peak_kernel<3><<<grid, threads, 0, s>>>(iters, reinterpret_cast<const double *>(src), reinterpret_cast<double *>(sink));
+    else if (mode == 4)
+      dmma_peak_kernel<4><<<grid, threads, 0, s>>>(iters, reinterpret_cast<const double *>(src), reinterpret_cast<double *>(sink));
+    else if (mode == 5)
+      dmma_peak_kernel<5><<<grid, threads, 0, s>>>(iters, reinterpret_cast<const double *>(src), reinterpret_cast<double *>(sink));
+    else if (mode == 6)
+      dmma_peak_kernel<6><<<grid, threads, 0, s>>>(iters, reinterpret_cast<const double *>(src), reinterpret_cast<double *>(sink));
     else if (fp64)
       fma_peak_kernel<double><<<grid, threads, 0, s>>>(iters, 1.0, reinterpret_cast<double *>(sink));
     else
@@ -187,6 +254,9 @@ cudaError_t run_fma_peak(int mode, int iters, double *tflops, cudaStream_t s) {
   cudaFree(sink);
   cudaFree(src);
   if (e != cudaSuccess) return e;
-  *tflops = 2.0 * (mode == 2 ? 56.0 : 8.0) * (double)iters * grid * threads / (best * 1e-3) / 1e12;
+  // flop per thread and iteration: 8 FMA chains; 56 in the register tile; DMMA: 8 tiles x (m n k / 32 lanes) FMA
+  //   m8n8k4 8, m16n8k8 32, m16n8k16 64 FMA per lane and tile; mode 6 reports the DMMA part only (+ 8 DFMA ride along)
+  const double fma_per_it = mode == 2 ? 56.0 : mode == 3 || mode == 6 ? 64.0 : mode == 4 ? 256.0 : mode == 5 ? 512.0 : 8.0;
+  *tflops = 2.0 * fma_per_it * (double)iters * grid * threads / (best * 1e-3) / 1e12;
   return cudaGetLastError();
 }

@@ -40,16 +40,9 @@ struct Workspace {
   int32_t *orig;                 // [n] chunk-local index of the caller's sample held in this slot (NULL = identity)
 };
 
-// Grouping plan (sort.cu): bucket = exact mixed-radix index of the relative shift tuple, or a hash of it.
-struct SortPlan {
-  int32_t exact, n_buckets;      // n_buckets is a power of two
-  int32_t half[RIFT_MAX_DET];    // d_k + half[k] in [0, range[k])
-  int32_t range[RIFT_MAX_DET];
-};
-
 // Device copy of Q.  Interleaved layout (direct kernel): [P][K*M][n_tp] complex<Real>, n_tp = n_t rounded up to even.
-// Planar extended layout (grouped kernel): [P][2*K*M][n_tp] Real, row 2r = Re, 2r+1 = Im, each row holding the n_t
-// samples followed by a circular repeat of its first RIFT_EXT samples (so base + j never needs a wrap), zero padded.
+// Extended layout (direct_ext): every row is followed by a circular repeat of its first RIFT_EXT samples (so base + j
+// never needs a wrap), zero padded.
 struct QStore {
   const void *data;
   int32_t n_t, n_tp, n_tau, km;
@@ -121,6 +114,19 @@ struct QuadProg {                // passed to the kernels as a __grid_constant__
   uint8_t bin_kind[RIFT_QP_MAX_BINS];        // matrix | z step << 1  (0 z^0, 1 *= z, 2 conj z, 3 *= conj z)
 };
 
+// FP64 tensor-core path (lnl_mma.cu): plan of one handle.  The batch is NB = 8 nt samples; the window buffer holds n_x
+// entries per sample (pitch xp doubles); the Q operand is [P][K][2 KS][pitch_q] bytes (see lnl_mma.cu), resident in shared
+// memory (stream == 0) or streamed in chunks of tr rows x one k-step through `slots` ring slots.
+struct MmaPlan {
+  int32_t ok;
+  int32_t K, M, KS;              // KS = ceil(M / 2) k-steps of 4 real contraction elements (2 modes) per detector
+  int32_t n_t, n_r, n_tau, n_x;  // stored rows, rows padded to 8, marginalisation samples, window entries (n_t if circular)
+  int32_t j0, circular;
+  int32_t nt, xp, tr, stream, slots;
+  int32_t pitch_q;               // bytes per mode row: n_r * 16 + 64
+  int64_t point_stride;          // bytes per intrinsic point
+};
+
 // geometry.cu
 cudaError_t launch_geometry_tc(const DetGeom &g, const ModeEntry *modes, const TcPlan &tp, const TcChunk &c,
                                const double *const params[6], const double *U, const double *V, const QuadProg &qp,
@@ -130,16 +136,6 @@ cudaError_t launch_geometry(const DetGeom &g, const ModeEntry *modes, const Batc
                             int32_t *shift_out, double *dbg_F, double *dbg_Y, const int32_t *perm, cudaStream_t s);
 cudaError_t launch_build_quad_uv(const QuadProg &qp, const double *U, const double *V, int32_t P, int32_t K, int32_t M,
                                  double2 *uv_out, cudaStream_t s);
-// sort.cu
-cudaError_t launch_group_sort(const DetGeom &g, const SortPlan &sp, const Batch &b, const double *const params[6],
-                              int32_t *bucket_of, uint32_t *hist, int32_t n_seg_chunk, int32_t *perm, cudaStream_t s,
-                              int *n_launch);
-// lnl_grouped.cu
-size_t lnl_grouped_smem_bytes(const QStore &q, bool fp32);
-cudaError_t launch_lnl_grouped(const QStore &q, bool fp32, const Batch &b, const Workspace &ws, int n_det,
-                               double *lnL_out, int n_sm, cudaStream_t s, int *n_launch);
-cudaError_t launch_convert_q_planar(const double *Q_c128, void *dst, int64_t rows, int32_t n_t, int32_t n_tp,
-                                    bool to_fp32, cudaStream_t s);
 // lnl_direct.cu
 size_t lnl_direct_smem_bytes(const QStore &q, bool fp32, bool q_in_smem);
 cudaError_t launch_lnl_direct(const QStore &q, bool fp32, bool q_in_smem, bool q_ext, const Batch &b, const Workspace &ws,
@@ -150,10 +146,6 @@ cudaError_t launch_lnl_direct_ext(const QStore &q, bool fp32, const Batch &b, co
                                   double *lnL_out, int n_sm, cudaStream_t s, int *n_launch);
 cudaError_t launch_convert_q_ext(const double *Q_c128, void *dst, int64_t rows, int32_t n_t, int32_t n_te, bool to_fp32,
                                  cudaStream_t s);
-// lnl_quad.cu (sorted samples, NQ per warp, same extended interleaved layout as lnl_direct_ext)
-size_t lnl_quad_smem_bytes(const QStore &q, bool fp32);
-cudaError_t launch_lnl_quad(const QStore &q, bool fp32, const Batch &b, const Workspace &ws, int n_det, double *lnL_out,
-                            int n_sm, cudaStream_t s, int *n_launch);
 // lnl_tc.cu (tcgen05 / TMEM contraction, shift applied through a shared-memory exchange)
 size_t lnl_tc_smem_bytes(const TcPlan &tp);
 int lnl_tc_pitch(int n_t, int halo);   // exchange-row pitch (floats) the kernel is instantiated for, 0 = none fits
@@ -169,10 +161,11 @@ cudaError_t launch_tcs_buckets(const DetGeom &g, const TcPlan &tp, const TcChunk
                                cudaStream_t s, int *n_launch);        // key, pos, count, base, seg_begin, perm
 cudaError_t launch_lnl_tcs(const TcPlan &tp, const uint32_t *qtc, const uint16_t *qs, const TcChunk &c, int pass,
                            double *lnL_out, int n_sm, cudaStream_t s, int *n_launch);
-// lnl_tile.cu (fp64 register-tiled contraction + shared-memory exchange; circular mode, n_t <= 512)
-size_t lnl_tile_smem_bytes(const QStore &q, int K, int pitch);
-cudaError_t launch_lnl_tile(const QStore &q, const Batch &b, const Workspace &ws, int K, int H, int pitch, const int *dmax,
-                            const double *exp_tab, double *lnL_out, int n_sm, cudaStream_t s, int *n_launch);
+// lnl_mma.cu (fp64 mode: DMMA contraction in unshifted detector time, shift applied into a shared-memory window buffer)
+size_t lnl_mma_smem_bytes(const MmaPlan &p);
+cudaError_t launch_convert_q_mma(const double *Q_c128, void *dst, const MmaPlan &p, int32_t n_points, cudaStream_t s);
+cudaError_t launch_lnl_mma(const MmaPlan &p, const void *q, const Batch &b, const Workspace &ws, double *lnL_out, int n_sm,
+                           cudaStream_t s, int *n_launch);
 // reduce.cu
 struct ReduceState {             // device, per segment
   double m, s1, s2;

@@ -89,9 +89,9 @@ def test_higher_l_harmonics(torch, oracle):
 
 
 # ------------------------------------------------------------------------------------------------ C0, whole config
-KERNELS = [rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_DIRECT, rift.RIFT_KERNEL_GROUPED, rift.RIFT_KERNEL_QUAD,
-           rift.RIFT_KERNEL_TC, rift.RIFT_KERNEL_TILE, rift.RIFT_KERNEL_TCS]
-TC_FAMILY = (rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_TC, rift.RIFT_KERNEL_TCS)
+KERNELS = [rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_DIRECT, rift.RIFT_KERNEL_TC, rift.RIFT_KERNEL_TCS, rift.RIFT_KERNEL_MMA]
+TC_FAMILY = (rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_TC, rift.RIFT_KERNEL_TCS, rift.RIFT_KERNEL_MMA)   # MMA: fp64 only, AUTO in mixed
+MMA_FAMILY = (rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_MMA, rift.RIFT_KERNEL_TC, rift.RIFT_KERNEL_TCS)  # TC/TCS: mixed only, AUTO in fp64
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
@@ -107,17 +107,14 @@ def test_c0_all_samples_both_precisions(torch, oracle, rho, kernel):
         lnL, sh, p = gpu_eval(torch, h, [0], cfg.n_samples, params, K=cfg.n_det, kernel=kernel)
         got = lnL.cpu().numpy()
         assert np.array_equal(sh.cpu().numpy()[fr == 0], sh_ref[fr == 0])
-        assert ("grouped" in rift.rift_ile_kernel_name(h)) == (kernel == rift.RIFT_KERNEL_GROUPED)
-        assert ("quad" in rift.rift_ile_kernel_name(h)) == (kernel == rift.RIFT_KERNEL_QUAD)
-        # the tensor-core kernel is the default of the mixed mode (and never runs in fp64 mode)
+        # the tcgen05 kernel is the default of the mixed mode (and never runs in fp64 mode)
         assert ("lnl_tc" in rift.rift_ile_kernel_name(h)) == (
             prec == rift.RIFT_PREC_MIXED and kernel in TC_FAMILY)
         # the shift-sorted variant: on request, or by default when the segments are long enough to fill its buckets
         if prec == rift.RIFT_PREC_MIXED and kernel == rift.RIFT_KERNEL_TCS:
             assert "lnl_tcs" in rift.rift_ile_kernel_name(h)
-        # the register-tiled kernel exists for fp64 only and is opt-in
-        assert ("lnl_tile" in rift.rift_ile_kernel_name(h)) == (
-            prec == rift.RIFT_PREC_FP64 and kernel == rift.RIFT_KERNEL_TILE)
+        # the FP64 tensor-core kernel is the default of the fp64 mode (and never runs in mixed mode)
+        assert ("lnl_mma" in rift.rift_ile_kernel_name(h)) == (prec == rift.RIFT_PREC_FP64 and kernel in MMA_FAMILY)
         if prec == rift.RIFT_PREC_FP64:
             assert np.max(rel_err(got, ref)) < TOL_FP64_REL, name
         else:
@@ -254,7 +251,7 @@ def test_tc_kernel_shapes(torch, oracle, shape, kernel):
     rift.rift_ile_destroy(h)
 
 
-def test_tcs_chunks_across_segments(torch, oracle, monkeypatch):
+def test_tcs_chunks_across_segments(torch, oracle):
     """Shift-sorted variant with a small chunk workspace: chunks that start and end inside segments, several segments
     per chunk, a ragged last batch in every segment; and the default kernel choice."""
     cfg = synth.CONFIGS[1]
@@ -262,9 +259,9 @@ def test_tcs_chunks_across_segments(torch, oracle, monkeypatch):
     n, ids = 3533, [2, 0, 1, 1, 0, 2, 0, 1, 2, 0, 1, 2]
     params = np.concatenate([synth.draw_samples(cfg, 70 + s, n)[0] for s in range(len(ids))], axis=1)
     h = create(rift, inp, rift.RIFT_PREC_MIXED)
-    monkeypatch.setenv("RIFT_TC_CHUNK_MIB", "1")              # raised to 8 batches per SM = 1184 batches = 5.4 segments
+    rift.rift_ile_set_option(h, rift.RIFT_OPT_TC_CHUNK_MIB, 1)   # raised to 8 batches per SM = 1184 batches = 5.4 segments
     got, sh, _ = gpu_eval(torch, h, ids, n, params, K=cfg.n_det, kernel=rift.RIFT_KERNEL_TCS)
-    monkeypatch.delenv("RIFT_TC_CHUNK_MIB")
+    rift.rift_ile_set_option(h, rift.RIFT_OPT_TC_CHUNK_MIB, 1024)
     assert "lnl_tcs" in rift.rift_ile_kernel_name(h)
     one, _, _ = gpu_eval(torch, h, ids, n, params, K=cfg.n_det, kernel=rift.RIFT_KERNEL_TC)
     assert "lnl_tc<" in rift.rift_ile_kernel_name(h)
@@ -274,6 +271,12 @@ def test_tcs_chunks_across_segments(torch, oracle, monkeypatch):
     big = np.tile(params[:, :n], (1, 12))[:, :4 * 9000]
     gpu_eval(torch, h, [0, 1, 2, 0], 9000, big, K=cfg.n_det)
     assert "lnl_tcs" in rift.rift_ile_kernel_name(h)
+    rift.rift_ile_set_option(h, rift.RIFT_OPT_TC_SORT, 0)     # the automatic choice can be switched off
+    gpu_eval(torch, h, [0, 1, 2, 0], 9000, big, K=cfg.n_det)
+    assert "lnl_tc<" in rift.rift_ile_kernel_name(h)
+    with pytest.raises(rift.RiftError) as e:
+        rift.rift_ile_set_option(h, 99, 1)
+    assert e.value.code == rift.RIFT_EINVAL
     got, one = got.cpu().numpy(), one.cpu().numpy()
     assert not np.isnan(got).any()
     assert np.max(np.abs(got - one)) < TOL_MIXED_LNL          # against the unsorted tensor-core kernel, every sample
@@ -329,10 +332,10 @@ def test_c2_shape_21_modes(torch, oracle):
         rift.rift_ile_destroy(h)
 
 
-def test_quadratic_term_pair_program(torch, oracle, monkeypatch):
+def test_quadratic_term_pair_program(torch, oracle):
     """More than 8 modes: the quadratic term a4 (Eq. (D3)) runs the pair program of rift_internal.h (mode pairs grouped by
     their common phase exponent).  With the same contraction, lnL from the program and from the plain double sum over
-    mode pairs (RIFT_NO_QUAD_PROG) differ by the rounding of q only; both match the oracle.  Mode lists in scrambled order
+    mode pairs (RIFT_OPT_QUAD_PROG = 0) differ by the rounding of q only; both match the oracle.  Mode lists in scrambled order
     with gaps in m, two segments whose boundary falls inside a thread block (program image of another point)."""
     modes = ((3, -3), (2, 2), (4, 0), (2, -2), (3, 2), (4, 4), (2, 1), (4, -3), (3, 3), (2, 0), (4, -4))
     cfg = synth.with_overrides(synth.CONFIGS[1], modes=modes, n_points=2)
@@ -343,16 +346,13 @@ def test_quadratic_term_pair_program(torch, oracle, monkeypatch):
     ref = np.concatenate([oracle_eval(oracle, inp, ids[s], params[:, s * n:(s + 1) * n])[0] for s in range(len(ids))])
     for prec in (rift.RIFT_PREC_MIXED, rift.RIFT_PREC_FP64):
         out = []
-        for no_prog in (False, True):
-            if no_prog:
-                monkeypatch.setenv("RIFT_NO_QUAD_PROG", "1")
-            else:
-                monkeypatch.delenv("RIFT_NO_QUAD_PROG", raising=False)
-            h = create(rift, inp, prec)
+        h = create(rift, inp, prec)
+        for no_prog in (False, True, False):
+            rift.rift_ile_set_option(h, rift.RIFT_OPT_QUAD_PROG, 0 if no_prog else 1)
             got, _, _ = gpu_eval(torch, h, ids, n, params, K=cfg.n_det)
             out.append(got.cpu().numpy())
-            rift.rift_ile_destroy(h)
-        monkeypatch.delenv("RIFT_NO_QUAD_PROG", raising=False)
+        rift.rift_ile_destroy(h)
+        assert np.array_equal(out[0], out[2])                 # switching the option back restores the program
         assert np.max(rel_err(out[0], out[1])) < 1e-12
         if prec == rift.RIFT_PREC_FP64:
             assert np.max(rel_err(out[0], ref)) < TOL_FP64_REL
@@ -510,11 +510,6 @@ def _full_size_sampled(torch, oracle, cfg, precisions, n_check_points, stride, l
 def test_c1_full_size(torch, oracle):
     # 16 points x 1e5 samples in ONE eval_batch (bench.py's launch); two whole points and a 1/50 subsample elsewhere
     _full_size_sampled(torch, oracle, synth.CONFIGS[1], (rift.RIFT_PREC_MIXED, rift.RIFT_PREC_FP64), 4, 50, lnz_points=2)
-
-
-def test_c1_full_size_grouped_kernel(torch, oracle):
-    _full_size_sampled(torch, oracle, synth.CONFIGS[1], (rift.RIFT_PREC_MIXED, rift.RIFT_PREC_FP64), 3, 50, lnz_points=1,
-                       kernel=rift.RIFT_KERNEL_GROUPED)
 
 
 @pytest.mark.slow
