@@ -299,37 +299,39 @@ void make_tc_plan(rift_ile *h, double delta_t) {
   }
 }
 
-// fp64 mode: plan of the DMMA kernel.  Whole Q block of a point resident in shared memory when it fits beside the window
-// buffer of a 16-sample batch, else streamed in (detector, 512-row range, k-step) chunks through a 4- or 3-slot ring.
-void make_mma_plan(rift_ile *h) {
+// fp64 mode: plan of the DMMA kernel (windows of up to 512 samples).  Whole Q block of a point resident in shared memory when
+// it fits beside the exchange buffer, else streamed in (detector, k-step) chunks through a 4- or 3-slot ring.
+void make_mma_plan(rift_ile *h, double delta_t) {
   MmaPlan &p = h->mma;
   p = MmaPlan{};
   if (h->precision != RIFT_PREC_FP64) return;
-  p.K = h->K;
-  p.M = h->M;
-  p.KS = (h->M + 1) / 2;
-  p.n_t = h->n_t;
-  p.n_r = (h->n_t + 7) & ~7;
-  p.n_tau = h->n_tau;
-  p.circular = h->n_tau == h->n_t ? 1 : 0;
-  p.n_x = h->n_tau;
-  p.j0 = (h->n_t - h->n_tau) / 2;
-  p.xp = p.n_x + ((2 - p.n_x) & 7);                   // pitch = 2 (mod 8) doubles: the unshifted store is conflict-free
-  p.pitch_q = p.n_r * 16 + 64;
-  p.point_stride = (int64_t)p.K * 2 * p.KS * p.pitch_q;
-  const int cand[][3] = {{0, 2, 0}, {1, 2, 4}, {1, 2, 3}, {0, 1, 0}, {1, 1, 4}, {1, 1, 3}};   // stream, nt, slots
+  int halo = 0;
+  for (int k = 1; k < h->K; ++k) {
+    double d2 = 0;
+    for (int i = 0; i < 3; ++i) {
+      const double d = h->geom.loc[k][i] - h->geom.loc[0][i];
+      d2 += d * d;
+    }
+    const double dm = std::ceil(std::sqrt(d2) / (RIFT_C_LIGHT * delta_t)) + 1.0;
+    if (dm > 1e6) return;
+    if ((int)dm > halo) halo = (int)dm;
+  }
+  const int cand[][2] = {{0, 0}, {1, 4}, {1, 3}};   // stream, slots
   for (const auto &c : cand) {
+    p = MmaPlan{};
+    p.K = h->K;
+    p.M = h->M;
+    p.n_t = h->n_t;
+    p.n_tau = h->n_tau;
+    p.H = halo;
     p.stream = c[0];
-    p.nt = c[1];
-    p.slots = c[2];
-    const int tr_max = p.stream ? 480 : 512;              // 32 rows per consumer warp (15 with a producer warp, else 16)
-    p.tr = p.n_r < tr_max ? p.n_r : tr_max;
-    if (!p.stream && p.point_stride >= (1ll << 31)) continue;
-    if (lnl_mma_smem_bytes(p) <= 227u * 1024u) {
+    p.slots = c[1];
+    if (lnl_mma_finish_plan(p) && lnl_mma_smem_bytes(p) <= 227u * 1024u) {
       p.ok = 1;
       return;
     }
   }
+  p.ok = 0;
 }
 
 bool use_mma(const rift_ile *h) {
@@ -811,7 +813,7 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
       }
     }
     // Q operand of the fp64 tensor-core kernel.  An allocation failure of this optional layout leaves the variant unavailable.
-    make_mma_plan(h);
+    make_mma_plan(h, cfg->delta_t);
     if (e == cudaSuccess && h->mma.ok) {
       if (cudaMalloc(&h->d_Qm, (size_t)h->P * h->mma.point_stride) == cudaSuccess) {
         e = launch_convert_q_mma(src, h->d_Qm, h->mma, h->P, 0);

@@ -4,33 +4,51 @@
 //
 // "Contract in unshifted detector time, then shift": per detector k the window term is the real GEMM
 //     P_k[t, n] = sum_kappa A_k[t, kappa] B_k[kappa, n],   A_k[t, 2m + {0,1}] = {Re, Im} Q_{k,m}[t],  B_k[2m + {0,1}, n] = {Re, Im}(F_k Y_m)_n
-// over ALL stored rows t (M = time, N = samples of the batch, K = 2 x modes), issued as mma.sync.m8n8k4.f64 (DMMA, 256 FMA
-// per instruction and warp: one Q value read from shared memory feeds 8 samples, one coefficient 8 rows -- the direct kernel
-// reads a 16-byte Q value per 2 DFMA and cannot pass 25 % of the pipe).  The per-sample shift is applied when a tile of P_k
-// leaves the registers: x[n][(t - off_{n,k}) mod N_t] (+)= P_k[t, n] in a per-batch window buffer in shared memory (the
-// first detector stores, the others read-modify-write; within one detector every (t, n) owns its target, detectors are
-// separated by a barrier).  The time marginal then runs over the finished windows with lanes over tau.
+// over ALL stored rows t (M = time, N = the 16 samples of a batch, K = 2 x modes), issued as mma.sync.m8n8k4.f64 (DMMA, 256
+// FMA per instruction and warp: one Q value read from shared memory feeds 8 samples, one coefficient 8 rows -- the direct
+// kernel reads a 16-byte Q value per 2 DFMA and cannot pass 25 % of the pipe).  The per-sample shift is applied by an exchange
+// through shared memory, one detector at a time: the tiles of P_k are stored unshifted as rows of 16 samples (128 B, the two
+// 64-byte halves swapped on odd rows: a 16-byte store per thread and tile, conflict-free), with circular copies inside the halo
+// H = max_k |s_k - s_0| so that a reader never wraps; a thread then owns one sample n and the window entries
+// j = JS e + 2 warp + jj (e = 0..NE-1) and adds P_k[j + off_{n,k}][n] into its registers -- half a warp reads 8 samples x 2
+// consecutive rows, conflict-free whatever the shifts are, and the addresses of a thread are one base plus immediates.  The
+// window x never leaves the registers: the time marginal takes a float maximum (any reference >= max - eps serves the
+// log-sum-exp) and the sum of 2^(c log2e (x - m)) with a polynomial exponential, both reduced across warps in shared memory.
 //
 // Q operand: the handle keeps [P][K][M2][pitch] bytes, M2 = 2 ceil(M/2) mode rows per detector (zero rows pad an odd mode
 // count), every row n_r = 8 ceil(N_t/8) complex128 (zero beyond N_t) followed by 64 pad bytes, so that the two mode rows of
 // one k-step sit 64 bytes apart modulo 128 and an A fragment load (8 rows x 2 modes x 16 B) is conflict-free.  Small
 // configurations keep the whole block of the intrinsic point resident in shared memory (one bulk copy per point); larger
-// ones stream (detector, row range, k-step) chunks through a ring filled by a producer warp with cp.async.bulk on mbarriers.
+// ones stream (detector, k-step) chunks through a ring filled by a producer warp with cp.async.bulk on mbarriers.
 #include "rift_internal.h"
 #include "tma_utils.cuh"
 
 namespace {
 
-constexpr int MM_WARPS = 16;                       // warps per CTA: 16 consumers (resident) or 15 consumers + 1 producer (ring),
-                                                   // so that every thread may hold 128 registers
-constexpr int MM_RBW = 4;                          // row blocks (of 8 rows) per warp and row range: a range = 32 rows x consumers
+constexpr int MM_WARPS = 16;                       // warps per CTA
 constexpr int MM_MAX_SLOTS = 8;
+
+// Two shapes of the CTA.  Resident Q block: two independent groups of 8 warps, each with its own batch of 8 samples (one
+// 8-column tile), exchange buffer and named barrier, so that the tensor phase of one group runs under the exchange and
+// exponential phases of the other.  Streamed Q: one group of 15 warps with batches of 16 samples (two tiles per A fragment:
+// half the chunk traffic per sample) and the 16th warp as the bulk-copy producer.
+template <bool STREAM>
+struct MmaShape {
+  static constexpr int NT = STREAM ? 2 : 1;        // 8-sample tiles per batch
+  static constexpr int NBG = 8 * NT;               // samples per batch of a group
+  static constexpr int GROUPS = STREAM ? 1 : 2;
+  static constexpr int GW = STREAM ? 15 : 8;       // warps per group
+  static constexpr int RBW = STREAM ? 4 : 8;       // row blocks (of 8 rows) per warp: wg + GW i
+  static constexpr int GTHR = GW * 32;
+  static constexpr int RB = 64 * NT;               // bytes per exchange row
+  static constexpr int RPW = NT == 2 ? 2 : 4;      // window entries a warp reads per element index e
+  static constexpr int JS = RPW * GW;              // ... a group
+};
 
 __device__ __forceinline__ void mm_arrive(uint64_t *bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-template <int CW>
-__device__ __forceinline__ void mm_bar_consumers() { asm volatile("bar.sync 1, %0;" ::"n"(CW * 32) : "memory"); }
+__device__ __forceinline__ void mm_bar(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
 __device__ __forceinline__ void dmma(double (&d)[2], double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
@@ -38,41 +56,46 @@ __device__ __forceinline__ void dmma(double (&d)[2], double a, double b) {
                : "d"(a), "d"(b));
 }
 
-// 2^y for y <= 0 (NaN propagates): y = n + r, |r| <= 1/2, 2^r by a degree-8 polynomial (interpolation at Chebyshev nodes,
-// relative error 1.1e-12), 2^n through the exponent field.  12 FP64-pipe operations with the argument FMA of the caller.
+// 2^y for y <~ 0 (NaN propagates): y = n + r, |r| <= 1/2, 2^r by a degree-8 polynomial (interpolation at Chebyshev nodes,
+// relative error 1.1e-12), 2^n through the exponent field (n clamped at -1000: 2^-1000 stands in for smaller terms).
+// 12 FP64-pipe operations with the argument FMA of the caller; the coefficients are constant-bank operands.
+__constant__ double MM_EXP2_C[9] = {1.0,
+                                    0x1.62e42fef84cf0p-1,
+                                    0x1.ebfbdff823cedp-3,
+                                    0x1.c6b08dd6fd239p-5,
+                                    0x1.3b2ab7181b784p-7,
+                                    0x1.5d8745a727ee4p-10,
+                                    0x1.4308ac85a5afep-13,
+                                    0x1.00dc4a5363675p-16,
+                                    0x1.63d1363b4014fp-20};
 __device__ __forceinline__ double mm_exp2(double y) {
-  y = fmax(y, -1000.0);
   const double t = y + 6755399441055744.0;                       // 1.5 * 2^52: the low word of t holds rint(y)
-  const int n = __double2loint(t);
+  const int n = max(__double2loint(t), -1000);
   const double r = y - (t - 6755399441055744.0);
-  double p = 0x1.63d1363b4014fp-20;
-  p = fma(p, r, 0x1.00dc4a5363675p-16);
-  p = fma(p, r, 0x1.4308ac85a5afep-13);
-  p = fma(p, r, 0x1.5d8745a727ee4p-10);
-  p = fma(p, r, 0x1.3b2ab7181b784p-7);
-  p = fma(p, r, 0x1.c6b08dd6fd239p-5);
-  p = fma(p, r, 0x1.ebfbdff823cedp-3);
-  p = fma(p, r, 0x1.62e42fef84cf0p-1);
-  p = fma(p, r, 1.0);
+  double p = MM_EXP2_C[8];
+#pragma unroll
+  for (int i = 7; i >= 0; --i) p = fma(p, r, MM_EXP2_C[i]);
   return __hiloint2double(__double2hiint(p) + (n << 20), __double2loint(p));
 }
 
 struct MmaSmem {                                   // byte offsets inside dynamic shared memory
-  uint32_t bars, coef, meta_c, meta_q, meta_off, part, xbuf, q, total;
+  uint32_t bars, grp, grp_stride, coef_bytes, meta, meta_bytes, wmax, psum, xb, q, total;   // coef .. xb: inside a group block
 };
 
 __host__ __device__ inline MmaSmem mma_smem(const MmaPlan &p) {
   MmaSmem L;
-  const uint32_t nb = 8u * p.nt;
+  const uint32_t nbg = p.stream ? 16u : 8u, groups = p.stream ? 1u : 2u, rb = p.stream ? 128u : 64u;
   L.bars = 0;                                                          // full[8], empty[8], resident
-  L.coef = 256;
-  L.meta_c = L.coef + (uint32_t)p.K * p.KS * nb * 4 * 8;               // cs[K][KS][NB][4] doubles
-  L.meta_q = L.meta_c + nb * 8;
-  L.meta_off = L.meta_q + nb * 8;                                      // off[K][NB] int32
-  L.part = (L.meta_off + (uint32_t)p.K * nb * 4 + 15u) & ~15u;         // part[NB][2] double2
-  L.xbuf = L.part + nb * 2 * 16;
-  L.q = (L.xbuf + nb * (uint32_t)p.xp * 8 + 127u) & ~127u;
-  const uint32_t qbytes = p.stream ? (uint32_t)p.slots * 2u * ((uint32_t)p.tr * 16u + 64u)
+  L.grp = 256;
+  L.coef_bytes = (uint32_t)p.K * p.KS * nbg * 4 * 8;                   // cs[K][KS][NBG][4] doubles, two buffers at offset 0
+  L.meta = 2 * L.coef_bytes;
+  L.meta_bytes = 2 * nbg * 8 + (uint32_t)p.K * nbg * 4;                // c[NBG], q[NBG] doubles, off[K][NBG] int32, two buffers
+  L.wmax = (L.meta + 2 * L.meta_bytes + 15u) & ~15u;                   // wmax[2][NBG][16] float
+  L.psum = L.wmax + 2 * nbg * 16 * 4;                                  // psum[2][NBG][16] double
+  L.xb = (L.psum + 2 * nbg * 16 * 8 + 127u) & ~127u;                   // exchange rows
+  L.grp_stride = (L.xb + (uint32_t)p.xb_rows * rb + 127u) & ~127u;
+  L.q = L.grp + groups * L.grp_stride;
+  const uint32_t qbytes = p.stream ? (uint32_t)p.slots * 2u * (uint32_t)p.pitch_q
                                    : (uint32_t)p.K * 2u * p.KS * (uint32_t)p.pitch_q;
   L.total = L.q + qbytes;
   return L;
@@ -80,73 +103,67 @@ __host__ __device__ inline MmaSmem mma_smem(const MmaPlan &p) {
 
 struct MmaArgs {
   MmaPlan p;
+  MmaSmem L;                       // computed on the host: the kernel reads the offsets from the constant bank
   const unsigned char *q;          // [P][K][2 KS][pitch_q]
   Batch b;
   Workspace ws;
   double *lnL_out;
 };
 
-template <int NT, bool STREAM>
+// exchange-buffer byte offset of (row, sample n).  Two tiles: 128-byte rows whose two 64-byte halves swap on odd rows
+template <int NT>
+__device__ __forceinline__ uint32_t xb_off(int row, int n) {
+  return NT == 2 ? (uint32_t)row * 128u + (uint32_t)((n ^ ((row & 1) << 3)) * 8) : (uint32_t)row * 64u + (uint32_t)(n * 8);
+}
+
+template <bool STREAM, int NE, int PFN>
 __global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs A) {
-  constexpr int NB = 8 * NT;
-  constexpr int CW = STREAM ? MM_WARPS - 1 : MM_WARPS;             // consumer warps
+  typedef MmaShape<STREAM> S;
+  constexpr int NT = S::NT, NBG = S::NBG, GW = S::GW, RBW = S::RBW, GTHR = S::GTHR, RB = S::RB, JS = S::JS;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const MmaPlan &P = A.p;
   const Batch &b = A.b;
   const Workspace &ws = A.ws;
-  const MmaSmem L = mma_smem(P);
+  const MmaSmem &L = A.L;
   uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + L.bars);
   uint64_t *empty = full + MM_MAX_SLOTS;
   uint64_t *resbar = empty + MM_MAX_SLOTS;
-  double *cs = reinterpret_cast<double *>(smem_raw + L.coef);
-  double *mc = reinterpret_cast<double *>(smem_raw + L.meta_c);
-  double *mq = reinterpret_cast<double *>(smem_raw + L.meta_q);
-  int *moff = reinterpret_cast<int *>(smem_raw + L.meta_off);
-  double2 *part = reinterpret_cast<double2 *>(smem_raw + L.part);
-  double *xbuf = reinterpret_cast<double *>(smem_raw + L.xbuf);
   unsigned char *qs = smem_raw + L.q;
 
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, tid = threadIdx.x;
-  const int K = P.K, KS = P.KS, n_t = P.n_t, n_r = P.n_r, n_x = P.n_x, xp = P.xp, tr = P.tr;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int K = P.K, KS = P.KS, n_t = P.n_t, n_r = P.n_r, n_x = P.n_x, H = P.H;
   const int m2 = 2 * P.M, km2 = m2 * K;                               // doubles of coefficients per detector / sample
-  const uint32_t slot_bytes = 2u * ((uint32_t)tr * 16u + 64u);
-  const int n_ranges = (n_r + tr - 1) / tr;
+  const uint32_t slot_bytes = 2u * (uint32_t)P.pitch_q;               // one k-step: two consecutive mode rows
 
-  if (tid == 0) {
+  if (threadIdx.x == 0) {
     for (int i = 0; i < MM_MAX_SLOTS; ++i) {
       mbar_init(full + i, 1);
-      mbar_init(empty + i, CW);
+      mbar_init(empty + i, GW);
     }
     mbar_init(resbar, 1);
   }
-  for (int i = tid; i < K * KS * NB * 4; i += blockDim.x) cs[i] = 0.0;  // the pad entries of an odd mode count stay zero
+  for (uint32_t i = threadIdx.x; i < S::GROUPS * L.grp_stride / 8; i += blockDim.x)   // coefficient pads 0, wmax / psum below
+    reinterpret_cast<double *>(smem_raw + L.grp)[i] = 0.0;
   __syncthreads();
 
   const int64_t w_begin = (b.n * blockIdx.x) / gridDim.x;
   const int64_t w_end = (b.n * (blockIdx.x + 1)) / gridDim.x;
 
   // ---------------------------------------------------------------------------------------------- producer warp (ring)
-  if (STREAM && warp == CW) {
+  if (STREAM && warp == GW) {
     if (lane == 0) {
       uint32_t cnt = 0;
       for (int64_t w0 = w_begin; w0 < w_end;) {
         const int64_t seg = (b.g0 + w0) / b.n_per_seg;
         const int64_t run_end = min(w_end, (seg + 1) * b.n_per_seg - b.g0);
         const unsigned char *qp = A.q + (int64_t)b.ids[seg] * P.point_stride;
-        for (int64_t s0 = w0; s0 < run_end; s0 += NB)
+        for (int64_t s0 = w0; s0 < run_end; s0 += NBG)
           for (int k = 0; k < K; ++k)
-            for (int r = 0; r < n_ranges; ++r) {
-              const int r0 = r * tr;
-              const uint32_t rows = (uint32_t)min(tr, n_r - r0);
-              for (int s = 0; s < KS; ++s, ++cnt) {
-                const uint32_t slot = cnt % (uint32_t)P.slots, ph = (cnt / (uint32_t)P.slots) & 1u;
-                mbar_wait(empty + slot, ph ^ 1u);
-                mbar_expect_tx(full + slot, 2u * rows * 16u);
-                const unsigned char *src = qp + (size_t)(k * 2 * KS + 2 * s) * P.pitch_q + (size_t)r0 * 16;
-                unsigned char *dst = qs + slot * slot_bytes;
-                bulk_g2s(dst, src, rows * 16u, full + slot);
-                bulk_g2s(dst + tr * 16 + 64, src + P.pitch_q, rows * 16u, full + slot);
-              }
+            for (int s = 0; s < KS; ++s, ++cnt) {
+              const uint32_t slot = cnt % (uint32_t)P.slots, ph = (cnt / (uint32_t)P.slots) & 1u;
+              mbar_wait(empty + slot, ph ^ 1u);
+              mbar_expect_tx(full + slot, slot_bytes);
+              bulk_g2s(qs + slot * slot_bytes, qp + (size_t)(k * 2 * KS + 2 * s) * P.pitch_q, slot_bytes, full + slot);
             }
         w0 = run_end;
       }
@@ -154,185 +171,265 @@ __global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs
     return;
   }
 
-  // ---------------------------------------------------------------------------------------------- consumer warps
-  const int lr = lane >> 2, lc = lane & 3;                       // fragment coordinates: row (A, C) / column group
-  // byte offset of this lane's A element inside a k-step chunk whose mode rows are `mp` bytes apart
-  const uint32_t mp = STREAM ? (uint32_t)tr * 16u + 64u : (uint32_t)P.pitch_q;
-  const uint32_t a_lane = (uint32_t)(lc >> 1) * mp + (uint32_t)(lc & 1) * 8u;
+  // ---------------------------------------------------------------------------------------------- consumer groups
+  const int g = STREAM ? 0 : warp / GW, wg = warp - g * GW, gtid = threadIdx.x - g * GTHR;
+  const int bar_id = 1 + g;
+  unsigned char *grp = smem_raw + L.grp + g * L.grp_stride;
+  unsigned char *xb = grp + L.xb;
+  float *wmax_all = reinterpret_cast<float *>(grp + L.wmax);
+  double *psum_all = reinterpret_cast<double *>(grp + L.psum);
+  for (int i = gtid; i < 2 * NBG * 16; i += GTHR) wmax_all[i] = -INFINITY;   // slots of absent warps never take part
+  // MMA role: fragment coordinates; row blocks wg + GW i are GW * 128 bytes apart: one base register plus immediates
+  const int lr = lane >> 2, lc = lane & 3;
+  const uint32_t a_base = (uint32_t)(lc >> 1) * (uint32_t)P.pitch_q + (uint32_t)(lc & 1) * 8u + (uint32_t)(8 * wg + lr) * 16u;
+  const int nrb = 8 * wg < n_r ? (n_r - 8 * wg + 8 * GW - 1) / (8 * GW) : 0;   // valid row blocks of this warp (<= RBW)
+  // store role: tile (i, nt) of row t = t0 + 8 GW i goes to st[nt] + i * (8 GW RB); the row parity (hence the swizzle) does
+  // not depend on i
+  const int t0 = 8 * wg + lr;
+  const int row_bias = P.circular ? H : 0;                       // buffer row of stored row t = t + row_bias
+  const uint32_t st0 = xb_off<NT>(t0 + row_bias, 2 * lc), st1 = xb_off<NT>(t0 + row_bias, 8 + 2 * lc);
+  const uint32_t st0h = (NT == 2 && (n_t & 1)) ? st1 : st0, st1h = (NT == 2 && (n_t & 1)) ? st0 : st1;   // halo: parity may flip
+  // exchange-reader role: sample n, window entries j = jb + JS e
+  const int n_mine = NT == 2 ? (((lane >> 4) << 3) | (lane & 7)) : (lane & 7);
+  const int jj = NT == 2 ? ((lane >> 3) & 1) : (lane >> 3), jb = S::RPW * wg + jj;
   const double ln_ntau = log((double)P.n_tau);
+
+  // coefficient items of this thread: element id = gtid + GTHR i of the [NBG][2 K M] block of a batch.  PFN > 0: the next
+  // batch's items wait in registers during a batch; PFN == 0 (many items): they go straight to the other shared-memory
+  // buffer with 8-byte cp.async (zero-filled for the slots past the end of a run)
+  constexpr int PFR = PFN > 0 ? PFN : 1;
+  int pf_src[PFR], pf_dst[PFR];                                  // offset in the workspace row block; cs index | n << 24
+#pragma unroll
+  for (int i = 0; i < PFN; ++i) {
+    const int id = gtid + GTHR * i;
+    pf_src[i] = -1;
+    pf_dst[i] = 0;
+    if (id < NBG * km2) {
+      const int n = id / km2, j = id - n * km2, k = j / m2, kap = j - k * m2;
+      pf_src[i] = n * (int)ws.coef_stride + j;
+      pf_dst[i] = (((k * KS + (kap >> 2)) * NBG + n) * 4 + (kap & 3)) | (n << 24);
+    }
+  }
+  double pf_v[PFR], pf_c = 1.0, pf_q = 0.0;
+  int pf_off = 0;
+  auto prefetch = [&](int64_t s0, int64_t run_end, int dst_buf) {
+    const int nvalid = (int)min((int64_t)NBG, run_end - s0);
+    const double *src = reinterpret_cast<const double *>(ws.coef) + s0 * ws.coef_stride;
+#pragma unroll
+    for (int i = 0; i < PFN; ++i) {
+      pf_v[i] = 0.0;
+      if (pf_src[i] >= 0 && (pf_dst[i] >> 24) < nvalid) pf_v[i] = src[pf_src[i]];
+    }
+    if (PFN == 0) {
+      const uint32_t cs_base = smem_u32(grp + dst_buf * L.coef_bytes);
+      for (int id = gtid; id < NBG * km2; id += GTHR) {
+        const int n = id / km2, j = id - n * km2, k = j / m2, kap = j - k * m2;
+        const uint32_t dst = cs_base + 8u * (uint32_t)(((k * KS + (kap >> 2)) * NBG + n) * 4 + (kap & 3));
+        const double *gp = src + (n < nvalid ? n : 0) * ws.coef_stride + j;
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(dst), "l"(gp), "r"(n < nvalid ? 8 : 0) : "memory");
+      }
+    }
+    pf_c = 1.0, pf_q = 0.0, pf_off = 0;
+    if (gtid < nvalid) {
+      pf_c = ws.scale_c[s0 + gtid];
+      pf_q = ws.quad[s0 + gtid];
+    }
+    if (gtid < NBG * K) {
+      const int k = gtid / NBG, n = gtid - k * NBG;
+      if (n < nvalid) {
+        const int sk = ws.shift[(s0 + n) * K + k];
+        int off = P.circular ? sk - ws.shift[(s0 + n) * K] : P.j0 + sk;
+        // out of range only for a sample with NaN angles (its lnL is NaN anyway)
+        if (off > H) off = H;
+        if (off < (P.circular ? -H : 0)) off = 0;
+        pf_off = off;
+      }
+    }
+  };
+  auto commit = [&](int buf) {
+    double *cs = reinterpret_cast<double *>(grp + buf * L.coef_bytes);
+    unsigned char *meta = grp + L.meta + buf * L.meta_bytes;
+#pragma unroll
+    for (int i = 0; i < PFN; ++i)
+      if (pf_src[i] >= 0) cs[pf_dst[i] & 0xffffff] = pf_v[i];
+    if (PFN == 0) asm volatile("cp.async.wait_all;" ::: "memory");
+    if (gtid < NBG) {
+      reinterpret_cast<double *>(meta)[gtid] = pf_c;
+      reinterpret_cast<double *>(meta)[NBG + gtid] = pf_q;
+    }
+    if (gtid < NBG * K) reinterpret_cast<int *>(meta + 2 * NBG * 8)[gtid] = pf_off;
+  };
+
   uint32_t cnt = 0, res_phase = 0;
   int staged_point = -1;
-
-  for (int64_t w0 = w_begin; w0 < w_end;) {
+  for (int64_t w0 = w_begin; w0 < w_end;) {                      // runs of one segment: every group takes every other batch
     const int64_t seg = (b.g0 + w0) / b.n_per_seg;
     const int64_t run_end = min(w_end, (seg + 1) * b.n_per_seg - b.g0);
     const int point = b.ids[seg];
-    if (!STREAM && point != staged_point) {
-      mm_bar_consumers<CW>();                                        // every warp is done with the previous block
-      if (tid == 0) stage_block(qs, A.q + (int64_t)point * P.point_stride, (uint32_t)P.point_stride, resbar);
+    if (!STREAM && point != staged_point) {                      // both groups are past the previous run
+      if (threadIdx.x == 0) stage_block(qs, A.q + (int64_t)point * P.point_stride, (uint32_t)P.point_stride, resbar);
       mbar_wait(resbar, res_phase);
       res_phase ^= 1u;
       staged_point = point;
     }
+    int64_t s0 = w0 + (int64_t)g * NBG;
+    int buf = 0;
+    if (s0 < run_end) {
+      prefetch(s0, run_end, 0);
+      commit(0);
+    }
+    mm_bar(bar_id, GTHR);
+    for (; s0 < run_end; s0 += S::GROUPS * NBG, buf ^= 1) {
+      const int64_t s_next = s0 + S::GROUPS * NBG;
+      if (s_next < run_end) prefetch(s_next, run_end, buf ^ 1);  // global loads in flight during this batch
+      const double *cs = reinterpret_cast<const double *>(grp + buf * L.coef_bytes);
+      const unsigned char *meta = grp + L.meta + buf * L.meta_bytes;
+      const double *mc = reinterpret_cast<const double *>(meta), *mq = mc + NBG;
+      const int *moff = reinterpret_cast<const int *>(meta + 2 * NBG * 8);
+      float *wmax = wmax_all + buf * NBG * 16;
+      double *psum = psum_all + buf * NBG * 16;
 
-    for (int64_t s0 = w0; s0 < run_end; s0 += NB) {
-      const int nvalid = (int)min((int64_t)NB, run_end - s0);
-      // ---- stage the batch: coefficients as B fragments cs[k][s][n][4], c, q, target offsets
-      for (int e = tid; e < NB * km2; e += CW * 32) {
-        const int n = e / km2, j = e - n * km2, k = j / m2, kap = j - k * m2;
-        const double v = n < nvalid ? reinterpret_cast<const double *>(ws.coef)[(s0 + n) * ws.coef_stride + j] : 0.0;
-        cs[((k * KS + (kap >> 2)) * NB + n) * 4 + (kap & 3)] = v;
-      }
-      if (tid < NB) {
-        mc[tid] = tid < nvalid ? ws.scale_c[s0 + tid] : 1.0;
-        mq[tid] = tid < nvalid ? ws.quad[s0 + tid] : 0.0;
-      }
-      if (tid < NB * K) {
-        const int k = tid / NB, n = tid - k * NB;
-        int off = 0;
-        if (n < nvalid) {
-          const int sk = ws.shift[(s0 + n) * K + k];
-          off = P.circular ? sk - ws.shift[(s0 + n) * K] : P.j0 + sk;
-          if (off <= -n_t || off >= n_t) off = 0;                // only a sample with NaN angles (its lnL is NaN anyway)
-        }
-        moff[tid] = off;
-      }
-      mm_bar_consumers<CW>();
-
+      double x[NE];
       for (int k = 0; k < K; ++k) {
-        int off[NT][2];
+        // ---- P_k tiles of this warp's row blocks
+        double acc[RBW][NT][2];
 #pragma unroll
-        for (int nt = 0; nt < NT; ++nt) {
-          off[nt][0] = moff[k * NB + 8 * nt + 2 * lc];
-          off[nt][1] = moff[k * NB + 8 * nt + 2 * lc + 1];
-        }
-        for (int r = 0; r < n_ranges; ++r) {
-          const int r0 = r * tr;
-          const int rb0 = MM_RBW * warp;                          // first row block of this warp inside the range
-          double acc[MM_RBW][NT][2];
+        for (int i = 0; i < RBW; ++i)
 #pragma unroll
-          for (int i = 0; i < MM_RBW; ++i)
+          for (int nt = 0; nt < NT; ++nt) acc[i][nt][0] = acc[i][nt][1] = 0.0;
+        const unsigned char *chunk = qs + (size_t)(k * 2 * KS) * P.pitch_q;                      // resident layout
+        const double *bs = cs + (size_t)(k * KS) * NBG * 4 + lr * 4 + lc;
+        for (int s = 0; s < KS; ++s, ++cnt, bs += NBG * 4, chunk += slot_bytes) {
+          uint32_t slot = 0;
+          if (STREAM) {
+            slot = cnt % (uint32_t)P.slots;
+            mbar_wait(full + slot, (cnt / (uint32_t)P.slots) & 1u);
+            chunk = qs + slot * slot_bytes;
+          }
+          if (nrb > 0) {
+            double bf[NT];
 #pragma unroll
-            for (int nt = 0; nt < NT; ++nt) acc[i][nt][0] = acc[i][nt][1] = 0.0;
-          const bool active = r0 + 8 * rb0 < n_r;                 // this warp owns rows of the range
-          for (int s = 0; s < KS; ++s, ++cnt) {
-            const unsigned char *chunk;
-            uint32_t slot = 0;
-            if (STREAM) {
-              slot = cnt % (uint32_t)P.slots;
-              mbar_wait(full + slot, (cnt / (uint32_t)P.slots) & 1u);
-              chunk = qs + slot * slot_bytes;
-            } else {
-              chunk = qs + (size_t)(k * 2 * KS + 2 * s) * P.pitch_q + (size_t)r0 * 16;
-            }
-            if (active) {
-              double bf[NT];
+            for (int nt = 0; nt < NT; ++nt) bf[nt] = bs[32 * nt];
+            double af[RBW];
 #pragma unroll
-              for (int nt = 0; nt < NT; ++nt) bf[nt] = cs[((k * KS + s) * NB + 8 * nt + lr) * 4 + lc];
-              double af[MM_RBW];
+            for (int i = 0; i < RBW; ++i)
+              if (i < nrb) af[i] = *reinterpret_cast<const double *>(chunk + a_base + i * (GW * 128));
 #pragma unroll
-              for (int i = 0; i < MM_RBW; ++i) {
-                const int row = 8 * (rb0 + i) + lr;               // rows past n_r of a short last range: clamp (masked below)
-                const int rowc = r0 + row < n_r ? row : 0;
-                af[i] = *reinterpret_cast<const double *>(chunk + a_lane + (uint32_t)rowc * 16u);
-              }
-#pragma unroll
-              for (int i = 0; i < MM_RBW; ++i)
+            for (int i = 0; i < RBW; ++i)
+              if (i < nrb) {
 #pragma unroll
                 for (int nt = 0; nt < NT; ++nt) dmma(acc[i][nt], af[i], bf[nt]);
-            }
-            if (STREAM) {
-              __syncwarp();
-              if (lane == 0) mm_arrive(empty + slot);
-            }
+              }
           }
-          if (active) {
-            // ---- shifted write-out: x[n][(t - off) mod N_t] (+)= P_k[t, n]; all loads first, then all stores
-            uint32_t idx[MM_RBW][NT][2];                              // element of xbuf, ~0 = masked
-            double old[MM_RBW][NT][2];
-#pragma unroll
-            for (int i = 0; i < MM_RBW; ++i) {
-              const int t = r0 + 8 * (rb0 + i) + lr;
-#pragma unroll
-              for (int nt = 0; nt < NT; ++nt)
-#pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                  int u = t - off[nt][e];
-                  bool ok;
-                  if (P.circular) {
-                    u += u < 0 ? n_t : 0;
-                    u -= u >= n_t ? n_t : 0;
-                    ok = t < n_t;
-                  } else {
-                    ok = t < n_t && u >= 0 && u < n_x;
-                  }
-                  idx[i][nt][e] = ok ? (uint32_t)((8 * nt + 2 * lc + e) * xp + u) : 0xffffffffu;
-                  old[i][nt][e] = 0.0;
-                  if (k > 0 && ok) old[i][nt][e] = xbuf[idx[i][nt][e]];
-                }
-            }
-#pragma unroll
-            for (int i = 0; i < MM_RBW; ++i)
-#pragma unroll
-              for (int nt = 0; nt < NT; ++nt)
-#pragma unroll
-                for (int e = 0; e < 2; ++e)
-                  if (idx[i][nt][e] != 0xffffffffu) xbuf[idx[i][nt][e]] = old[i][nt][e] + acc[i][nt][e];
+          if (STREAM) {
+            __syncwarp();
+            if (lane == 0) mm_arrive(empty + slot);
           }
         }
-        mm_bar_consumers<CW>();                                       // detector k is complete in every window
+        mm_bar(bar_id, GTHR);                                    // every reader is done with detector k - 1
+        // ---- unshifted store: row t + row_bias, 16 bytes per tile (samples 8 nt + 2 lc, + 1), circular copies in the halo
+#pragma unroll
+        for (int i = 0; i < RBW; ++i) {
+          const int t = t0 + 8 * GW * i;
+          if (i < nrb && t < n_t) {
+            unsigned char *d = xb + i * (8 * GW * RB);
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) {
+              const double2 v = make_double2(acc[i][nt][0], acc[i][nt][1]);
+              const uint32_t o = nt ? st1 : st0, oh = nt ? st1h : st0h;
+              *reinterpret_cast<double2 *>(d + o) = v;
+              if (P.circular) {
+                if (t < H) *reinterpret_cast<double2 *>(d + n_t * RB + oh) = v;
+                if (t >= n_t - H) *reinterpret_cast<double2 *>(d - n_t * RB + oh) = v;
+              }
+            }
+          }
+        }
+        mm_bar(bar_id, GTHR);                                    // the rows of detector k are complete
+        // ---- shifted read: x_j += P_k[j + off][n]
+        {
+          const unsigned char *src = xb + xb_off<NT>(jb + moff[k * NBG + n_mine] + row_bias, n_mine);
+          if (k == 0) {
+#pragma unroll
+            for (int e = 0; e < NE; ++e) x[e] = *reinterpret_cast<const double *>(src + e * (JS * RB));
+          } else {
+#pragma unroll
+            for (int e = 0; e < NE; ++e) x[e] += *reinterpret_cast<const double *>(src + e * (JS * RB));
+          }
+        }
       }
 
-      // ---- time marginal: portion (sample n, half h) of a window per warp, lanes over tau
-      const int half = (n_x + 1) >> 1;
-      for (int pi = warp; pi < 2 * NB; pi += CW) {
-        const int n = pi >> 1, h = pi & 1;
-        const double *xw = xbuf + n * xp;
-        const int j_lo = h * half, j_hi = min(n_x, j_lo + half);
-        double m = -INFINITY;
-        for (int j = j_lo + lane; j < j_hi; j += 32) m = fmax(m, xw[j]);
-        m = warp_max(m);
-        const double cl2 = mc[n] * 1.4426950408889634;
-        const double mo = -m * cl2;
-        double sum = 0.0;
-        for (int j = j_lo + lane; j < j_hi; j += 32) sum += mm_exp2(fma(xw[j], cl2, mo));
-        sum = warp_sum(sum);
-        if (lane == 0) part[pi] = make_double2(m, sum);
+      // ---- time marginal from the registers
+      float mf = -INFINITY;
+#pragma unroll
+      for (int e = 0; e < NE; ++e)
+        if (jb + JS * e < n_x) mf = fmaxf(mf, __double2float_ru(x[e]));
+      mf = fmaxf(mf, __shfl_xor_sync(0xffffffffu, mf, 8));
+      if (NT == 1) mf = fmaxf(mf, __shfl_xor_sync(0xffffffffu, mf, 16));
+      if (jj == 0) wmax[n_mine * 16 + wg] = mf;
+      mm_bar(bar_id, GTHR);
+      if (s_next < run_end) commit(buf ^ 1);                     // the other buffers were last read two barriers ago
+      {
+        const float4 *wm = reinterpret_cast<const float4 *>(wmax + n_mine * 16);
+        const float4 a0 = wm[0], a1 = wm[1], a2 = wm[2], a3 = wm[3];
+        mf = fmaxf(fmaxf(fmaxf(a0.x, a0.y), fmaxf(a0.z, a0.w)), fmaxf(fmaxf(a1.x, a1.y), fmaxf(a1.z, a1.w)));
+        mf = fmaxf(mf, fmaxf(fmaxf(fmaxf(a2.x, a2.y), fmaxf(a2.z, a2.w)), fmaxf(fmaxf(a3.x, a3.y), fmaxf(a3.z, a3.w))));
       }
-      mm_bar_consumers<CW>();
-      if (tid < nvalid) {
-        const double c = mc[tid];
-        const double2 p0 = part[2 * tid], p1 = part[2 * tid + 1];
-        const double m = fmax(p0.x, p1.x);
-        double sum = 0.0;
-        if (p0.x > -INFINITY) sum += p0.y * exp(c * (p0.x - m));
-        if (p1.x > -INFINITY) sum += p1.y * exp(c * (p1.x - m));
-        A.lnL_out[b.g0 + s0 + tid] = c * m + log(sum) - ln_ntau - mq[tid];
+      const double cl2 = mc[n_mine] * 1.4426950408889634;
+      const double mo = -(double)mf * cl2;
+      double sum = 0.0;
+#pragma unroll
+      for (int e = 0; e < NE; ++e)
+        if (jb + JS * e < n_x) sum += mm_exp2(fma(x[e], cl2, mo));
+      sum += __shfl_xor_sync(0xffffffffu, sum, 8);
+      if (NT == 1) sum += __shfl_xor_sync(0xffffffffu, sum, 16);
+      if (jj == 0) psum[n_mine * 16 + wg] = sum;
+      mm_bar(bar_id, GTHR);
+      if (gtid < (int)min((int64_t)NBG, run_end - s0)) {
+        float m = -INFINITY;
+        double sacc = 0.0;
+#pragma unroll
+        for (int w = 0; w < 16; ++w) {
+          m = fmaxf(m, wmax[gtid * 16 + w]);
+          sacc += psum[gtid * 16 + w];
+        }
+        A.lnL_out[b.g0 + s0 + gtid] = mc[gtid] * (double)m + log(sacc) - ln_ntau - mq[gtid];
       }
-      // the next batch's staging overwrites cs / meta: the combine above read mc, mq, part
-      mm_bar_consumers<CW>();
     }
+    if (!STREAM) mm_bar(3, MM_WARPS * 32);                       // both groups leave the run (and its Q block) together
+    else mm_bar(bar_id, GTHR);
     w0 = run_end;
   }
 }
 
-template <int NT, bool STREAM>
+template <bool STREAM, int NE, int PFN>
 cudaError_t launch_t(const MmaArgs &a, int n_sm, cudaStream_t s) {
-  constexpr int NB = 8 * NT;
-  auto kern = lnl_mma_kernel<NT, STREAM>;
-  const size_t smem = mma_smem(a.p).total;
+  auto kern = lnl_mma_kernel<STREAM, NE, PFN>;
+  const size_t smem = a.L.total;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   int64_t grid = n_sm;
-  const int64_t max_grid = (a.b.n + NB - 1) / NB;
+  const int64_t max_grid = (a.b.n + 15) / 16;
   if (grid > max_grid) grid = max_grid;
   kern<<<(unsigned)grid, MM_WARPS * 32, smem, s>>>(a);
   return cudaGetLastError();
 }
 
+template <bool STREAM, int PFN>
+cudaError_t launch_ne(const MmaArgs &a, int n_sm, cudaStream_t s) {
+  switch (a.p.ne) {
+    case 4: return launch_t<STREAM, 4, PFN>(a, n_sm, s);
+    case 8: return launch_t<STREAM, 8, PFN>(a, n_sm, s);
+    case 13: return launch_t<STREAM, 13, PFN>(a, n_sm, s);
+    case 14: return launch_t<STREAM, 14, PFN>(a, n_sm, s);
+    case 16: return launch_t<STREAM, 16, PFN>(a, n_sm, s);
+    default: return cudaErrorInvalidValue;
+  }
+}
+
 // [rows][n_t] complex128 -> the operand layout described at the top: [P][K][M2][pitch] bytes
 __global__ void convert_q_mma_kernel(const double2 *__restrict__ src, unsigned char *__restrict__ dst, int P, int K, int M,
-                                     int M2, int n_t, int n_r, int pitch) {
+                                     int M2, int n_t, int pitch) {
   const int64_t per_row = pitch / 16;                                       // 16-byte units per row, pad included
   const int64_t total = (int64_t)P * K * M2 * per_row;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
@@ -342,12 +439,40 @@ __global__ void convert_q_mma_kernel(const double2 *__restrict__ src, unsigned c
     const int64_t pk = row / M2;
     double2 v = make_double2(0.0, 0.0);
     if (m < M && t < n_t) v = src[(pk * M + m) * n_t + t];
-    (void)n_r;
     reinterpret_cast<double2 *>(dst)[i] = v;
   }
 }
 
 }  // namespace
+
+// Completes a plan whose K, M, n_t, n_tau, H (circular halo) and stream / slots are set; returns false when the window is too
+// long for the 16 register entries per thread or the row blocks of the CTA.
+bool lnl_mma_finish_plan(MmaPlan &p) {
+  const int gw = p.stream ? MmaShape<true>::GW : MmaShape<false>::GW, js = p.stream ? MmaShape<true>::JS : MmaShape<false>::JS;
+  const int rbw = p.stream ? MmaShape<true>::RBW : MmaShape<false>::RBW, nbg = p.stream ? 16 : 8;
+  p.KS = (p.M + 1) / 2;
+  p.n_r = (p.n_t + 7) & ~7;
+  p.circular = p.n_tau == p.n_t ? 1 : 0;
+  p.n_x = p.n_tau;
+  p.j0 = (p.n_t - p.n_tau) / 2;
+  if (!p.circular) p.H = p.n_t - p.n_tau;                 // guard band: 0 <= off = j0 + s_k <= 2 j0
+  p.pitch_q = p.n_r * 16 + 64;
+  p.point_stride = (int64_t)p.K * 2 * p.KS * p.pitch_q;
+  const int need = (p.n_x + js - 1) / js;
+  static const int nes[] = {4, 8, 13, 14, 16};
+  p.ne = 0;
+  for (int v : nes)
+    if (v >= need) {
+      p.ne = v;
+      break;
+    }
+  const int items = (nbg * 2 * p.K * p.M + gw * 32 - 1) / (gw * 32);
+  p.pfn = (!p.stream && items <= 2) ? 2 : 0;
+  p.xb_rows = p.ne * js + 2 * p.H + 8;
+  if (p.xb_rows < p.n_t + 2 * p.H + 8) p.xb_rows = p.n_t + 2 * p.H + 8;
+  return p.ne != 0 && p.n_r <= 8 * rbw * gw && p.H < p.n_t && p.K * nbg <= gw * 32 &&
+         (p.stream || p.point_stride < (1ll << 20));
+}
 
 size_t lnl_mma_smem_bytes(const MmaPlan &p) { return mma_smem(p).total; }
 
@@ -357,7 +482,7 @@ cudaError_t launch_convert_q_mma(const double *Q_c128, void *dst, const MmaPlan 
   if (grid > 148 * 16) grid = 148 * 16;
   if (grid < 1) grid = 1;
   convert_q_mma_kernel<<<grid, 256, 0, s>>>(reinterpret_cast<const double2 *>(Q_c128), reinterpret_cast<unsigned char *>(dst),
-                                            n_points, p.K, p.M, 2 * p.KS, p.n_t, p.n_r, p.pitch_q);
+                                            n_points, p.K, p.M, 2 * p.KS, p.n_t, p.pitch_q);
   return cudaGetLastError();
 }
 
@@ -366,21 +491,12 @@ cudaError_t launch_lnl_mma(const MmaPlan &p, const void *q, const Batch &b, cons
   if (b.n <= 0) return cudaSuccess;
   MmaArgs a;
   a.p = p;
+  a.L = mma_smem(p);
   a.q = reinterpret_cast<const unsigned char *>(q);
   a.b = b;
   a.ws = ws;
   a.lnL_out = lnL_out;
   if (n_launch) ++*n_launch;
-  if (p.stream) {
-    switch (p.nt) {
-      case 1: return launch_t<1, true>(a, n_sm, s);
-      case 2: return launch_t<2, true>(a, n_sm, s);
-      default: return cudaErrorInvalidValue;
-    }
-  }
-  switch (p.nt) {
-    case 1: return launch_t<1, false>(a, n_sm, s);
-    case 2: return launch_t<2, false>(a, n_sm, s);
-    default: return cudaErrorInvalidValue;
-  }
+  if (p.stream) return launch_ne<true, 0>(a, n_sm, s);
+  return p.pfn == 2 ? launch_ne<false, 2>(a, n_sm, s) : launch_ne<false, 0>(a, n_sm, s);
 }

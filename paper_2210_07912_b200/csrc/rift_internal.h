@@ -114,15 +114,16 @@ struct QuadProg {                // passed to the kernels as a __grid_constant__
   uint8_t bin_kind[RIFT_QP_MAX_BINS];        // matrix | z step << 1  (0 z^0, 1 *= z, 2 conj z, 3 *= conj z)
 };
 
-// FP64 tensor-core path (lnl_mma.cu): plan of one handle.  The batch is NB = 8 nt samples; the window buffer holds n_x
-// entries per sample (pitch xp doubles); the Q operand is [P][K][2 KS][pitch_q] bytes (see lnl_mma.cu), resident in shared
-// memory (stream == 0) or streamed in chunks of tr rows x one k-step through `slots` ring slots.
+// FP64 tensor-core path (lnl_mma.cu): plan of one handle.  Batches of 16 samples; the Q operand is [P][K][2 KS][pitch_q] bytes
+// (see lnl_mma.cu), resident in shared memory (stream == 0) or streamed one (detector, k-step) chunk at a time through
+// `slots` ring slots; the exchange buffer holds xb_rows rows of 16 doubles; a thread keeps `ne` window entries in registers.
 struct MmaPlan {
   int32_t ok;
   int32_t K, M, KS;              // KS = ceil(M / 2) k-steps of 4 real contraction elements (2 modes) per detector
-  int32_t n_t, n_r, n_tau, n_x;  // stored rows, rows padded to 8, marginalisation samples, window entries (n_t if circular)
+  int32_t n_t, n_r, n_tau, n_x;  // stored rows, rows padded to 8, marginalisation samples, window entries
   int32_t j0, circular;
-  int32_t nt, xp, tr, stream, slots;
+  int32_t H;                     // circular: bound on |s_k - s_0| (halo rows); guard band: n_t - n_tau
+  int32_t ne, pfn, xb_rows, stream, slots;
   int32_t pitch_q;               // bytes per mode row: n_r * 16 + 64
   int64_t point_stride;          // bytes per intrinsic point
 };
@@ -162,6 +163,7 @@ cudaError_t launch_tcs_buckets(const DetGeom &g, const TcPlan &tp, const TcChunk
 cudaError_t launch_lnl_tcs(const TcPlan &tp, const uint32_t *qtc, const uint16_t *qs, const TcChunk &c, int pass,
                            double *lnL_out, int n_sm, cudaStream_t s, int *n_launch);
 // lnl_mma.cu (fp64 mode: DMMA contraction in unshifted detector time, shift applied into a shared-memory window buffer)
+bool lnl_mma_finish_plan(MmaPlan &p);
 size_t lnl_mma_smem_bytes(const MmaPlan &p);
 cudaError_t launch_convert_q_mma(const double *Q_c128, void *dst, const MmaPlan &p, int32_t n_points, cudaStream_t s);
 cudaError_t launch_lnl_mma(const MmaPlan &p, const void *q, const Batch &b, const Workspace &ws, double *lnL_out, int n_sm,
