@@ -97,6 +97,20 @@ int rift_ile_eval_batch(rift_ile_t *h, int32_t n_seg, const int32_t *intrinsic_i
                         const double *const params[RIFT_N_PARAMS], double *lnL_out, int32_t *shift_out,
                         void *cuda_stream);
 
+/* The same evaluation from HOST buffers (the call a user with host arrays makes): params are 6 HOST arrays (pinned
+ * memory makes the copies asynchronous), ln_weight a HOST array or NULL, lnL_out a HOST array.  The batch is cut into
+ * n_slices groups of whole segments (0 = 4; at most n_seg): slice g + 1 is uploaded on an internal copy stream and slice
+ * g - 1 read back on a second one while slice g is evaluated on cuda_stream; the device copies live in staging buffers
+ * owned by the handle (grown by cudaMalloc when a call is larger than any before).  Asynchronous: lnL_out is complete
+ * when cuda_stream is (the stream is made to wait for the read-backs).  rift_ile_staged returns the device copies of
+ * the last call (params, ln_weight or NULL, lnL, and the sample count), valid until the next eval_batch_host: pass them
+ * to rift_ile_reduce for the evidence of the same batch without a second upload.  RIFT_ESTATE if nothing was staged. */
+int rift_ile_eval_batch_host(rift_ile_t *h, int32_t n_seg, const int32_t *intrinsic_ids, int64_t n_per_seg,
+                             const double *const params[RIFT_N_PARAMS], const double *ln_weight, double *lnL_out,
+                             int32_t n_slices, void *cuda_stream);
+int rift_ile_staged(rift_ile_t *h, const double *params_dev[RIFT_N_PARAMS], const double **ln_weight_dev,
+                    const double **lnL_dev, int64_t *n);
+
 /* Sample-axis reduce (step a8): per segment, with ln omega_i = lnL_i + ln_weight_i,
  *   lnZ = ln[(1/N) sum omega_i]  (Eq. (3));  n_eff = sum omega / max omega  (B1);
  *   n_ess = (sum omega)^2 / sum omega^2  (B2);  rel_err^2 = (N/n_ess - 1)/(N - 1)  (B3, reading A20);

@@ -26,7 +26,8 @@ RIFT_N_PARAMS = 6
 
 EXPORTS = ("rift_ile_create", "rift_ile_eval_batch", "rift_ile_reduce", "rift_ile_geometry", "rift_ile_set_kernel",
            "rift_ile_launch_count", "rift_ile_kernel_name", "rift_ile_profile", "rift_ile_profile_read",
-           "rift_ile_fma_peak", "rift_ile_set_option", "rift_ile_reserve", "rift_ile_destroy",
+           "rift_ile_fma_peak", "rift_ile_set_option", "rift_ile_reserve", "rift_ile_eval_batch_host",
+           "rift_ile_staged", "rift_ile_destroy",
            "rift_ile_strerror", "rift_ile_last_error")
 AC_EXPORTS = ("rift_ac_create", "rift_ac_draw", "rift_ac_update", "rift_ac_update_dims", "rift_ac_get_masses",
               "rift_ac_ile_ln_weight", "rift_ac_destroy")
@@ -68,6 +69,10 @@ def lib() -> C.CDLL:
         L.rift_ile_geometry.restype = C.c_int
         L.rift_ile_set_kernel.argtypes = [vp, i32]
         L.rift_ile_set_kernel.restype = C.c_int
+        L.rift_ile_eval_batch_host.argtypes = [vp, i32, vp, i64, C.POINTER(vp), vp, vp, i32, vp]
+        L.rift_ile_eval_batch_host.restype = C.c_int
+        L.rift_ile_staged.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(i64)]
+        L.rift_ile_staged.restype = C.c_int
         L.rift_ile_set_option.argtypes = [vp, i32, i64]
         L.rift_ile_set_option.restype = C.c_int
         L.rift_ile_reserve.argtypes = [vp, i32, i64, i32]
@@ -188,6 +193,22 @@ def rift_ile_eval_batch(h, intrinsic_ids: Sequence[int], n_per_seg: int, params,
     ids = np.ascontiguousarray(intrinsic_ids, dtype=np.int32)
     _check(lib().rift_ile_eval_batch(h, int(ids.size), ids.ctypes.data, int(n_per_seg), _params6(params), _ptr(lnL_out),
                                      _ptr(shift_out), int(cuda_stream) or None), h)
+
+
+def rift_ile_eval_batch_host(h, intrinsic_ids: Sequence[int], n_per_seg: int, params, ln_weight, lnL_out,
+                             n_slices: int = 0, cuda_stream: int = 0) -> None:
+    """params: [6][N] HOST array (numpy, or a pinned torch CPU tensor) or six host arrays; lnL_out: HOST array [N]."""
+    ids = np.ascontiguousarray(intrinsic_ids, dtype=np.int32)
+    _check(lib().rift_ile_eval_batch_host(h, int(ids.size), ids.ctypes.data, int(n_per_seg), _params6(params),
+                                          _ptr(ln_weight), _ptr(lnL_out), int(n_slices), int(cuda_stream) or None), h)
+
+
+def rift_ile_staged(h) -> dict:
+    """Device copies left by the last eval_batch_host: dict(params=[6 addresses], ln_weight=address or None, lnL=address, n)."""
+    p = (C.c_void_p * 6)()
+    w, l, n = C.c_void_p(), C.c_void_p(), C.c_int64()
+    _check(lib().rift_ile_staged(h, p, C.byref(w), C.byref(l), C.byref(n)), h)
+    return dict(params=[int(x) for x in p], ln_weight=(int(w.value) if w.value else None), lnL=int(l.value), n=int(n.value))
 
 
 def rift_ile_geometry(h, intrinsic_id: int, n: int, params, F=None, Y=None, shift=None, quad=None,

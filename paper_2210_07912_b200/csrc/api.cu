@@ -57,6 +57,13 @@ struct rift_ile {
   size_t partial_cap = 0;
   double *d_out = nullptr, *h_out = nullptr;
   size_t out_cap = 0;
+  // host-buffer path (rift_ile_eval_batch_host): device staging [7][host_cap] (six parameters, ln weight) + lnL[host_cap],
+  // an upload and a read-back stream, and the events that chain the slices
+  double *d_hp = nullptr, *d_hl = nullptr;
+  int64_t host_cap = 0, host_n = 0;
+  bool host_has_w = false;
+  cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
+  std::vector<cudaEvent_t> host_ev;
   // bookkeeping
   int kernel_variant = RIFT_KERNEL_AUTO;
   const char *kernel_name = "none";
@@ -157,6 +164,11 @@ void free_handle(rift_ile *h) {
     cudaEventDestroy(sp.a);
     cudaEventDestroy(sp.b);
   }
+  for (auto &e : h->host_ev) cudaEventDestroy(e);
+  if (h->s_h2d) cudaStreamDestroy(h->s_h2d);
+  if (h->s_d2h) cudaStreamDestroy(h->s_d2h);
+  cudaFree(h->d_hp);
+  cudaFree(h->d_hl);
   cudaFree(h->d_modes);
   cudaFree(h->d_Q);
   cudaFree(h->d_Qe);
@@ -919,6 +931,15 @@ int rift_ile_reserve(rift_ile_t *h, int32_t n_seg, int64_t n_per_seg, int32_t n_
   return rc;
 }
 
+static int eval_batch_device(rift_ile *h, int32_t n_seg, const int32_t *intrinsic_ids, int64_t n_per_seg,
+                             const double *const params[RIFT_N_PARAMS], double *lnL_out, int32_t *shift_out, cudaStream_t s) {
+  int rc = upload_ids(h, n_seg, intrinsic_ids, s);
+  if (rc != RIFT_OK) return rc;
+  if (use_tc(h) && use_tcs(h, n_seg, n_per_seg)) return run_chunks_tcs(h, n_seg, n_per_seg, params, lnL_out, shift_out, s);
+  if (use_tc(h)) return run_chunks_tc(h, n_seg, n_per_seg, params, lnL_out, shift_out, s);
+  return run_chunks(h, n_seg, n_per_seg, params, lnL_out, shift_out, nullptr, nullptr, nullptr, s);
+}
+
 int rift_ile_eval_batch(rift_ile_t *h, int32_t n_seg, const int32_t *intrinsic_ids, int64_t n_per_seg,
                         const double *const params[RIFT_N_PARAMS], double *lnL_out, int32_t *shift_out,
                         void *cuda_stream) {
@@ -929,12 +950,87 @@ int rift_ile_eval_batch(rift_ile_t *h, int32_t n_seg, const int32_t *intrinsic_i
   for (int d = 0; d < RIFT_N_PARAMS; ++d)
     if (!params[d]) return fail(h, RIFT_EINVAL, "null parameter array");
   DeviceGuard g(h->device);
+  return eval_batch_device(h, n_seg, intrinsic_ids, n_per_seg, params, lnL_out, shift_out,
+                           reinterpret_cast<cudaStream_t>(cuda_stream));
+}
+
+int rift_ile_eval_batch_host(rift_ile_t *h, int32_t n_seg, const int32_t *intrinsic_ids, int64_t n_per_seg,
+                             const double *const params[RIFT_N_PARAMS], const double *ln_weight, double *lnL_out,
+                             int32_t n_slices, void *cuda_stream) {
+  if (!h) return RIFT_EINVAL;
+  if (n_seg < 0 || n_per_seg < 0 || n_slices < 0) return fail(h, RIFT_EINVAL, "negative size");
+  if (n_seg == 0 || n_per_seg == 0) return RIFT_OK;
+  if (!intrinsic_ids || !params || !lnL_out) return fail(h, RIFT_EINVAL, "null pointer");
+  for (int d = 0; d < RIFT_N_PARAMS; ++d)
+    if (!params[d]) return fail(h, RIFT_EINVAL, "null parameter array");
+  for (int32_t i = 0; i < n_seg; ++i)
+    if (intrinsic_ids[i] < 0 || intrinsic_ids[i] >= h->P) return fail(h, RIFT_ERANGE, "intrinsic id outside [0, n_points)");
+  DeviceGuard g(h->device);
   cudaStream_t s = reinterpret_cast<cudaStream_t>(cuda_stream);
-  int rc = upload_ids(h, n_seg, intrinsic_ids, s);
-  if (rc != RIFT_OK) return rc;
-  if (use_tc(h) && use_tcs(h, n_seg, n_per_seg)) return run_chunks_tcs(h, n_seg, n_per_seg, params, lnL_out, shift_out, s);
-  if (use_tc(h)) return run_chunks_tc(h, n_seg, n_per_seg, params, lnL_out, shift_out, s);
-  return run_chunks(h, n_seg, n_per_seg, params, lnL_out, shift_out, nullptr, nullptr, nullptr, s);
+  const int64_t total = (int64_t)n_seg * n_per_seg;
+  if (total > h->host_cap) {
+    if (h->host_cap > 0) CU(h, cudaDeviceSynchronize());         // an earlier call may still read the staging buffers
+    cudaFree(h->d_hp);
+    cudaFree(h->d_hl);
+    h->d_hp = h->d_hl = nullptr;
+    h->host_cap = 0;
+    CU(h, cudaMalloc(&h->d_hp, (size_t)total * 7 * sizeof(double)));
+    CU(h, cudaMalloc(&h->d_hl, (size_t)total * sizeof(double)));
+    h->host_cap = total;
+  }
+  if (!h->s_h2d) CU(h, cudaStreamCreateWithFlags(&h->s_h2d, cudaStreamNonBlocking));
+  if (!h->s_d2h) CU(h, cudaStreamCreateWithFlags(&h->s_d2h, cudaStreamNonBlocking));
+  int G = n_slices > 0 ? n_slices : 4;                           // measured on C1: 2 / 4 / 8 / 16 slices -> 7.1 / 7.7 / 7.3 / 6.2e8 evals/s
+  if (G > n_seg) G = n_seg;
+  while ((int)h->host_ev.size() < 2 * G + 2) {
+    cudaEvent_t e;
+    CU(h, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    h->host_ev.push_back(e);
+  }
+  cudaEvent_t ev_start = h->host_ev[2 * G], ev_end = h->host_ev[2 * G + 1];
+  h->host_n = total;
+  h->host_has_w = ln_weight != nullptr;
+  const int64_t cap = h->host_cap;
+  // uploads: ordered after whatever the caller's stream still does with the staging buffers of the previous call
+  CU(h, cudaEventRecord(ev_start, s));
+  CU(h, cudaStreamWaitEvent(h->s_h2d, ev_start, 0));
+  CU(h, cudaStreamWaitEvent(h->s_d2h, ev_start, 0));
+  for (int gi = 0; gi < G; ++gi) {
+    const int64_t a = (int64_t)((int64_t)n_seg * gi / G) * n_per_seg, b = (int64_t)((int64_t)n_seg * (gi + 1) / G) * n_per_seg;
+    for (int d = 0; d < RIFT_N_PARAMS; ++d)
+      CU(h, cudaMemcpyAsync(h->d_hp + d * cap + a, params[d] + a, (size_t)(b - a) * sizeof(double), cudaMemcpyHostToDevice, h->s_h2d));
+    if (ln_weight)
+      CU(h, cudaMemcpyAsync(h->d_hp + 6 * cap + a, ln_weight + a, (size_t)(b - a) * sizeof(double), cudaMemcpyHostToDevice, h->s_h2d));
+    CU(h, cudaEventRecord(h->host_ev[gi], h->s_h2d));
+  }
+  // evaluation of slice g on the caller's stream while slice g + 1 uploads and slice g - 1 reads back
+  for (int gi = 0; gi < G; ++gi) {
+    const int32_t s0 = (int32_t)((int64_t)n_seg * gi / G), s1 = (int32_t)((int64_t)n_seg * (gi + 1) / G);
+    const int64_t a = (int64_t)s0 * n_per_seg, b = (int64_t)s1 * n_per_seg;
+    const double *p[RIFT_N_PARAMS];
+    for (int d = 0; d < RIFT_N_PARAMS; ++d) p[d] = h->d_hp + d * cap + a;
+    CU(h, cudaStreamWaitEvent(s, h->host_ev[gi], 0));
+    const int rc = eval_batch_device(h, s1 - s0, intrinsic_ids + s0, n_per_seg, p, h->d_hl + a, nullptr, s);
+    if (rc != RIFT_OK) return rc;
+    CU(h, cudaEventRecord(h->host_ev[G + gi], s));
+    CU(h, cudaStreamWaitEvent(h->s_d2h, h->host_ev[G + gi], 0));
+    CU(h, cudaMemcpyAsync(lnL_out + a, h->d_hl + a, (size_t)(b - a) * sizeof(double), cudaMemcpyDeviceToHost, h->s_d2h));
+  }
+  CU(h, cudaEventRecord(ev_end, h->s_d2h));
+  CU(h, cudaStreamWaitEvent(s, ev_end, 0));                      // the caller's stream is complete when lnL_out is
+  return RIFT_OK;
+}
+
+int rift_ile_staged(rift_ile_t *h, const double *params_dev[RIFT_N_PARAMS], const double **ln_weight_dev,
+                    const double **lnL_dev, int64_t *n) {
+  if (!h) return RIFT_EINVAL;
+  if (h->host_n == 0) return fail(h, RIFT_ESTATE, "no rift_ile_eval_batch_host call has staged anything");
+  if (params_dev)
+    for (int d = 0; d < RIFT_N_PARAMS; ++d) params_dev[d] = h->d_hp + d * h->host_cap;
+  if (ln_weight_dev) *ln_weight_dev = h->host_has_w ? h->d_hp + 6 * h->host_cap : nullptr;
+  if (lnL_dev) *lnL_dev = h->d_hl;
+  if (n) *n = h->host_n;
+  return RIFT_OK;
 }
 
 int rift_ile_geometry(rift_ile_t *h, int32_t intrinsic_id, int64_t n, const double *const params[RIFT_N_PARAMS],

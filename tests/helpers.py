@@ -11,10 +11,10 @@ def oracle_geometry_fn(oracle, cfg, loc, resp, ml, mm):
     return lambda th: oracle.geometry_at(th, loc, resp, cfg.gmst, ml, mm, cfg.delta_t)
 
 
-def build(oracle, cfg, n_points=None):
+def build(oracle, cfg, n_points=None, noise=True):
     loc, resp = synth.detector_arrays(cfg)
     ml, mm = synth.mode_arrays(cfg)
-    return synth.build_inputs(cfg, oracle_geometry_fn(oracle, cfg, loc, resp, ml, mm), n_points=n_points)
+    return synth.build_inputs(cfg, oracle_geometry_fn(oracle, cfg, loc, resp, ml, mm), n_points=n_points, noise=noise)
 
 
 def create(binding, inp, precision, n_tau=None, points=None):

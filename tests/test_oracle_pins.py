@@ -56,17 +56,20 @@ def test_p1_higher_closed_forms(oracle):
 
 def test_p1_orthonormal_and_sum_rule(oracle):
     # Gauss-Legendre in cos(theta) x uniform phi: exact for these trigonometric polynomials
+    # (products of two harmonics of l <= 8: degree <= 16 in cos(theta), |m - m'| <= 16 < 24 in phi).  Every l the library
+    # accepts (2 <= l <= 8, include/rift_ile.h) is covered.
     xs, ws = np.polynomial.legendre.leggauss(24)
-    nphi = 24
+    nphi = 36
     phis = TWO_PI * np.arange(nphi) / nphi
-    modes = [(l, m) for l in (2, 3, 4) for m in range(-l, l + 1)]
+    modes = [(l, m) for l in range(2, 9) for m in range(-l, l + 1)]
     vals = np.array([[[oracle.swsh_m2(l, m, math.acos(x), p) for p in phis] for x in xs] for (l, m) in modes])
     gram = np.einsum("atp,btp,t->ab", np.conj(vals), vals, ws) * (TWO_PI / nphi)
     assert np.max(np.abs(gram - np.eye(len(modes)))) < 1e-12
     # sum_m |Y_lm|^2 = (2l+1)/(4 pi) at every angle
-    for l in (2, 3, 4, 5):
-        tot = sum(abs(oracle.swsh_m2(l, m, 1.234, 0.5)) ** 2 for m in range(-l, l + 1))
-        assert abs(tot - (2 * l + 1) / (4 * math.pi)) < 1e-14
+    for l in range(2, 9):
+        for theta in (0.0, 0.3, 1.234, 2.9, math.pi):
+            tot = sum(abs(oracle.swsh_m2(l, m, theta, 0.5)) ** 2 for m in range(-l, l + 1))
+            assert abs(tot - (2 * l + 1) / (4 * math.pi)) < 1e-13
 
 
 def test_p1_face_on_and_reflection(oracle):
@@ -77,7 +80,7 @@ def test_p1_face_on_and_reflection(oracle):
         else:
             assert abs(v) < 1e-15
     rng = np.random.default_rng(3)
-    for l in (2, 3, 4):
+    for l in range(2, 9):
         for m in range(-l, l + 1):
             t, p = rng.uniform(0, math.pi), rng.uniform(0, TWO_PI)
             lhs = oracle.swsh_m2(l, -m, t, p)
