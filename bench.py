@@ -384,3 +384,107 @@ def launch_rate(rift, torch, h, ids, N, data, n_calls=200):
     except Exception as e:                                # reported, not hidden: the graph leg is optional
         out["graph_error"] = str(e)[:200]
     return out
+
+
+def run_ours(args) -> None:
+    import torch
+    import paper_2210_07912_b200 as rift
+    from paper_2210_07912_b200 import build as build_mod
+    from paper_2210_07912_b200 import dist_util
+
+    rank, world, local = dist_util.env_world()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        import torch.distributed as dist
+        dist_util.init("nccl", torch.device("cuda", local))
+    if rank == 0:
+        build_mod.build()
+    dist_util.barrier()
+    rift.lib()
+
+    single = args.config is not None
+    rows_wanted = ([(args.config, args.precision or "mixed")] if single else
+                   [(c, p) for c in (0, 1, 2, 3, 4) for p in ("mixed", "fp64")])
+    headline = rows_wanted[0] if single else HEADLINE
+    peaks = measured_peaks()
+    evidence = roofline_evidence()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
+    sampler = ClockSampler(local) if rank == 0 else None
+    pool = ThreadPoolExecutor(max_workers=max(2, min(16, (os.cpu_count() or 8))))
+    per_config, t_prep = {}, {}
+    for ci in sorted({c for c, _ in rows_wanted}):
+        cfg = synth.CONFIGS[ci]
+        if args.points:
+            cfg = synth.with_overrides(cfg, n_points=args.points)
+        if args.samples:
+            cfg = synth.with_overrides(cfg, n_samples=args.samples)
+        gids = dist_util.shard_points(cfg.n_points, rank, world)     # every rank owns its own intrinsic points
+        t = time.time()
+        data = ConfigData(rift, torch, cfg, gids, pool)
+        t_prep[f"C{ci}"] = round(time.time() - t, 2)
+        for (c, prec) in rows_wanted:
+            if c != ci:
+                continue
+            is_head = (c, prec) == headline
+            row = bench_row(rift, torch, dist_util, data, prec, args.steps if is_head else None,
+                            args.warmup if is_head else 3, flush, sampler, evidence, peaks, world)
+            per_config[f"C{c}/{prec}"] = row
+        del data
+        torch.cuda.empty_cache()
+
+    if rank == 0:
+        head = per_config[f"C{headline[0]}/{headline[1]}"]
+        line = {
+            "metric": METRIC, "value": head["evals_per_s"], "unit": UNIT, "n_gpus": world, "steps": head["steps"],
+            "warmup": head["warmup"], "ms_per_step": head["ms_per_step"], "ms_per_step_best": head["ms_per_step_best"],
+            "ms_per_step_median": head["ms_per_step_median"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": head["dtype"], "data": "synthetic",
+            "config": {"workload": head["workload"], "precision": headline[1], "kernel": head["kernel"],
+                       "l2": "flushed between timed iterations (256 MiB memset)", "parallelism": f"replicas x{world}",
+                       "step": "eval_batch (geometry + fused lnL) + reduce with 6x100-bin histograms",
+                       "rows": "per_config holds all five configs x both precision modes; rows other than the headline are "
+                               "timed over the `steps` they state"},
+            "clocks": head["clocks"], "e2e": head["e2e"], "gpu_launches": head["gpu_launches"],
+            "roofline": head["roofline"], "kernel_ms_per_step": head["kernel_ms_per_step"],
+            "lnZ_point0": head["lnZ_point0"], "n_eff_point0": head["n_eff_point0"],
+            "per_config": per_config, "input_generation_s": t_prep,
+        }
+        if "launch_rate" in head:
+            line["launch_rate"] = head["launch_rate"]
+        if world == 1 and not args.no_cpu:
+            cfgs = sorted({c for c, _ in rows_wanted})
+            base = {c: cpu_baseline(synth.CONFIGS[c], 12.0 if c == headline[0] else 4.0) for c in cfgs}
+            line["cpu_baseline"] = base[headline[0]]
+            for key, row in per_config.items():
+                row["cpu_baseline"] = base[int(key[1])]
+        print(json.dumps(line))
+    if sampler:
+        sampler.stop()
+    pool.shutdown()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=None, help="one config only (default: all five, headline C4 mixed)")
+    ap.add_argument("--precision", default=None, choices=[None, "mixed", "fp64"], help="with --config: the precision mode")
+    ap.add_argument("--points", type=int, default=0, help="override the number of intrinsic points (debug)")
+    ap.add_argument("--samples", type=int, default=0, help="override samples per point (debug)")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
