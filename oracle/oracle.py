@@ -10,18 +10,20 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "rift_oracle.c")
+_SRC_DM = os.path.join(_HERE, "dmarg_oracle.c")
 _LIB = os.path.join(_HERE, "liboracle.so")
 _lib = None
 
 __all__ = ["build", "lib", "num_threads", "antenna", "harmonics", "swsh_m2", "delays", "lnl_core",
-           "logmeanexp", "eval_batch", "ReduceState", "reduce", "geometry_at"]
+           "logmeanexp", "eval_batch", "ReduceState", "reduce", "geometry_at", "dmarg_rule", "dmarg_core",
+           "eval_batch_dmarg"]
 
 
 def build(force: bool = False) -> str:
     """gcc -O2 -ffp-contract=off -fopenmp -> oracle/liboracle.so (rebuilt when the source is newer)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_DM)):
         cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", "-Wall",
-               _SRC, "-o", _LIB, "-lm"]
+               _SRC, _SRC_DM, "-o", _LIB, "-lm"]
         subprocess.run(cmd, check=True)
     return _LIB
 
@@ -63,6 +65,14 @@ def lib():
         L.oracle_reduce_accumulate.restype = None
         L.oracle_reduce_finalize.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp, _dp]
         L.oracle_reduce_finalize.restype = None
+        L.oracle_dmarg_rule.argtypes = [C.c_double, C.c_double, C.c_double, C.c_int, _dp, _dp]
+        L.oracle_dmarg_rule.restype = None
+        L.oracle_dmarg_core.argtypes = [C.c_int, _dp] + [C.c_double] * 5 + [C.c_int]
+        L.oracle_dmarg_core.restype = C.c_double
+        L.oracle_eval_batch_dmarg.argtypes = ([C.c_int, _dp, _dp, C.c_double, C.c_int, _ip, _ip, C.c_int, C.c_int,
+                                               C.c_double, C.c_double, _dp, _dp, _dp, C.c_int64] + [_dp] * 5
+                                              + [C.c_double, C.c_double, C.c_double, C.c_int, _dp, _ip, _bp])
+        L.oracle_eval_batch_dmarg.restype = C.c_int
         _lib = L
     return _lib
 
@@ -214,3 +224,43 @@ def geometry_at(theta, location, response, gmst, mode_l, mode_m, delta_t):
     Y = harmonics(theta[3], theta[4], mode_l, mode_m)[0]
     _dt, sh, _fr = delays(theta[0], theta[1], gmst, location, delta_t)
     return F, Y, sh[0]
+
+
+# ---------------------------------------------------------------------------------------------- dmarg_oracle.c (NEXT-2)
+def dmarg_rule(d_min: float, d_max: float, alpha: float, n_panels: int):
+    """(D[8 n_panels], W[8 n_panels]) of the composite Gauss-Legendre rule in ln D (W includes the prior density)."""
+    D = np.empty(8 * n_panels, dtype=np.float64)
+    W = np.empty(8 * n_panels, dtype=np.float64)
+    lib().oracle_dmarg_rule(float(d_min), float(d_max), float(alpha), int(n_panels), _d(D), _d(W))
+    return D, W
+
+
+def dmarg_core(x, b: float, d_ref: float, d_min: float, d_max: float, alpha: float, n_panels: int) -> float:
+    x = _f64(x)
+    return float(lib().oracle_dmarg_core(int(x.size), _d(x), float(b), float(d_ref), float(d_min), float(d_max),
+                                         float(alpha), int(n_panels)))
+
+
+def eval_batch_dmarg(location, response, gmst: float, mode_l, mode_m, delta_t: float, d_ref_mpc: float, Q, U, V,
+                     params5, d_min: float, d_max: float, n_panels: int, alpha: float = 2.0, n_tau: Optional[int] = None):
+    """Distance-marginalised lnL of all samples of one intrinsic point.  params5: [5][n] (ra, dec, psi, iota, phi_ref).
+    Returns (lnL[n], shift[n][K], fragile[n])."""
+    Q, U, V = _c128(Q), _c128(U), _c128(V)
+    K, M, n_t = Q.shape
+    n_tau = n_t if n_tau is None else int(n_tau)
+    P = [_f64(p) for p in params5[:5]]
+    n = P[0].size
+    r, D = _f64(location).reshape(K, 3), _f64(response).reshape(K, 9)
+    ml = np.ascontiguousarray(mode_l, dtype=np.int32)
+    mm = np.ascontiguousarray(mode_m, dtype=np.int32)
+    lnL = np.empty(n, dtype=np.float64)
+    sh = np.empty((n, K), dtype=np.int32)
+    fr = np.empty(n, dtype=np.uint8)
+    rc = lib().oracle_eval_batch_dmarg(K, _d(r), _d(D), float(gmst), M, ml.ctypes.data_as(_ip), mm.ctypes.data_as(_ip),
+                                       n_t, n_tau, float(delta_t), float(d_ref_mpc), _d(Q.view(np.float64)),
+                                       _d(U.view(np.float64)), _d(V.view(np.float64)), n, *[_d(p) for p in P],
+                                       float(d_min), float(d_max), float(alpha), int(n_panels), _d(lnL),
+                                       sh.ctypes.data_as(_ip), fr.ctypes.data_as(_bp))
+    if rc != 0:
+        raise ValueError("oracle_eval_batch_dmarg: invalid arguments")
+    return lnL, sh, fr
