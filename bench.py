@@ -341,8 +341,41 @@ def bench_row(rift, torch, dist_util, data: ConfigData, precision: str, steps, w
     }
     if evals <= 65536:
         row["launch_rate"] = launch_rate(rift, torch, h, ids, N, data)
+    if cfg.index == 1:                        # NEXT-2: the distance-marginalised evaluation on the same samples (5 parameters)
+        row["dmarg"] = dmarg_row(rift, torch, h, ids, N, data, flush, row)
     rift.rift_ile_destroy(h)
     return row
+
+
+def dmarg_row(rift, torch, h, ids, N, data, flush, row, n_dist=128):
+    """rift_ile_eval_batch_dmarg: evaluations/s, and the sampling efficiency n_ess per
+    evaluation of the 5-D integral against that of the 6-D one on the same intrinsic points."""
+    stream = torch.cuda.current_stream().cuda_stream
+    P = len(ids)
+    lnL = torch.empty_like(data.lnL_d)
+
+    def step():
+        rift.rift_ile_eval_batch_dmarg(h, ids, N, data.params_d, synth.D_MIN_MPC, synth.D_MAX_MPC, n_dist, lnL, None, stream)
+        return rift.rift_ile_reduce(h, P, N, lnL, data.lnw_d, cuda_stream=stream)
+
+    step()
+    torch.cuda.synchronize()
+    ms = []
+    for _ in range(3):
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        red5 = step()
+        b.record()
+        torch.cuda.synchronize()
+        ms.append(a.elapsed_time(b))
+    red6 = rift.rift_ile_reduce(h, P, N, data.lnL_d, data.lnw_d, cuda_stream=stream)
+    t5, t6 = float(np.mean(ms)), row["ms_per_step"]
+    e5, e6 = float(np.median(red5["n_ess"])), float(np.median(red6["n_ess"]))
+    return {"kernel": rift.rift_ile_kernel_name(h), "n_dist": n_dist, "evals_per_s": P * N / (t5 * 1e-3), "ms_per_step": t5,
+            "steps": 3, "cost_ratio_vs_plain": t5 / t6, "median_n_ess_5d": e5, "median_n_ess_6d": e6,
+            "n_ess_gain_at_equal_cost": (e5 / t5) / (e6 / t6) if e6 > 0 else None,
+            "median_lnZ_5d_minus_6d": float(np.median(red5["lnZ"] - red6["lnZ"]))}
 
 
 def launch_rate(rift, torch, h, ids, N, data, n_calls=200):

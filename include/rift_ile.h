@@ -111,6 +111,21 @@ int rift_ile_eval_batch_host(rift_ile_t *h, int32_t n_seg, const int32_t *intrin
 int rift_ile_staged(rift_ile_t *h, const double *params_dev[RIFT_N_PARAMS], const double **ln_weight_dev,
                     const double **lnL_dev, int64_t *n);
 
+/* Distance-marginalised evaluation (SURVEY.md section 8(f) NEXT-2; section IV.C.3, :360-372: "directly marginalize
+ * over distance").  The paper prints no formula; reading D1 of DESIGN.md section 12: with c = D_ref/D, Eq. (D2)-(D3) read
+ * ln L(tau_j, D) = c x_j - c^2 b (the form of Eq. (D5), :780), and
+ *   lnL_out = ln[(1/n_tau) sum_j int_{d_min}^{d_max} p(D) exp(c x_j - c^2 b) dD],  p(D) = 3 D^2/(d_max^3 - d_min^3) (:508),
+ * the integral by a composite 8-point Gauss-Legendre rule in ln D with n_dist nodes (a multiple of 8 in [8, 512]; the
+ * quadrature error in lnL_out is < 1e-5 with 128 nodes up to rho = 12-20 and with 256 nodes up to rho = 30 --
+ * tests/test_dmarg_oracle_pins.py P21, tests/test_gpu_dmarg.py).
+ *   params : HOST array of 5 DEVICE pointers (ra, dec, psi, iota, phi_ref), fp64 [n_seg*n_per_seg]; the sample has no
+ *            distance.  Everything else as rift_ile_eval_batch.  A NaN parameter gives NaN for that sample only.
+ * Runs the direct kernels in either precision mode (the window sums x_j do not depend on D: one contraction, n_dist
+ * exponentials per window entry).  Not capturable on its first call of a new (d_min, d_max, n_dist) or a larger size. */
+int rift_ile_eval_batch_dmarg(rift_ile_t *h, int32_t n_seg, const int32_t *intrinsic_ids, int64_t n_per_seg,
+                              const double *const params[5], double d_min_mpc, double d_max_mpc, int32_t n_dist,
+                              double *lnL_out, int32_t *shift_out, void *cuda_stream);
+
 /* Sample-axis reduce (step a8): per segment, with ln omega_i = lnL_i + ln_weight_i,
  *   lnZ = ln[(1/N) sum omega_i]  (Eq. (3));  n_eff = sum omega / max omega  (B1);
  *   n_ess = (sum omega)^2 / sum omega^2  (B2);  rel_err^2 = (N/n_ess - 1)/(N - 1)  (B3, reading A20);

@@ -27,7 +27,7 @@ RIFT_N_PARAMS = 6
 EXPORTS = ("rift_ile_create", "rift_ile_eval_batch", "rift_ile_reduce", "rift_ile_geometry", "rift_ile_set_kernel",
            "rift_ile_launch_count", "rift_ile_kernel_name", "rift_ile_profile", "rift_ile_profile_read",
            "rift_ile_fma_peak", "rift_ile_set_option", "rift_ile_reserve", "rift_ile_eval_batch_host",
-           "rift_ile_staged", "rift_ile_destroy",
+           "rift_ile_staged", "rift_ile_eval_batch_dmarg", "rift_ile_destroy",
            "rift_ile_strerror", "rift_ile_last_error")
 AC_EXPORTS = ("rift_ac_create", "rift_ac_draw", "rift_ac_update", "rift_ac_update_dims", "rift_ac_get_masses",
               "rift_ac_ile_ln_weight", "rift_ac_destroy")
@@ -71,6 +71,8 @@ def lib() -> C.CDLL:
         L.rift_ile_set_kernel.restype = C.c_int
         L.rift_ile_eval_batch_host.argtypes = [vp, i32, vp, i64, C.POINTER(vp), vp, vp, i32, vp]
         L.rift_ile_eval_batch_host.restype = C.c_int
+        L.rift_ile_eval_batch_dmarg.argtypes = [vp, i32, vp, i64, C.POINTER(vp), dbl, dbl, i32, vp, vp, vp]
+        L.rift_ile_eval_batch_dmarg.restype = C.c_int
         L.rift_ile_staged.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(i64)]
         L.rift_ile_staged.restype = C.c_int
         L.rift_ile_set_option.argtypes = [vp, i32, i64]
@@ -201,6 +203,17 @@ def rift_ile_eval_batch_host(h, intrinsic_ids: Sequence[int], n_per_seg: int, pa
     ids = np.ascontiguousarray(intrinsic_ids, dtype=np.int32)
     _check(lib().rift_ile_eval_batch_host(h, int(ids.size), ids.ctypes.data, int(n_per_seg), _params6(params),
                                           _ptr(ln_weight), _ptr(lnL_out), int(n_slices), int(cuda_stream) or None), h)
+
+
+def rift_ile_eval_batch_dmarg(h, intrinsic_ids: Sequence[int], n_per_seg: int, params5, d_min_mpc: float, d_max_mpc: float,
+                              n_dist: int, lnL_out, shift_out=None, cuda_stream: int = 0) -> None:
+    """params5: a [5][N] (or [6][N]: the distance row is ignored) device tensor or five device arrays."""
+    ids = np.ascontiguousarray(intrinsic_ids, dtype=np.int32)
+    rows = [params5[d] for d in range(5)]
+    ptrs = (C.c_void_p * 5)(*[_ptr(r) for r in rows])
+    _check(lib().rift_ile_eval_batch_dmarg(h, int(ids.size), ids.ctypes.data, int(n_per_seg), ptrs, float(d_min_mpc),
+                                           float(d_max_mpc), int(n_dist), _ptr(lnL_out), _ptr(shift_out),
+                                           int(cuda_stream) or None), h)
 
 
 def rift_ile_staged(h) -> dict:

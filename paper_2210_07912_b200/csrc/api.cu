@@ -64,6 +64,11 @@ struct rift_ile {
   bool host_has_w = false;
   cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
   std::vector<cudaEvent_t> host_ev;
+  // distance marginalisation (rift_ile_eval_batch_dmarg): quadrature nodes c_i = D_ref/D_i, ln W_i; a distance column = D_ref
+  double *d_dm_nodes = nullptr, *d_dm_dist = nullptr;
+  int dm_n = 0;
+  double dm_dmin = 0, dm_dmax = 0;
+  int64_t dm_dist_cap = 0;
   // bookkeeping
   int kernel_variant = RIFT_KERNEL_AUTO;
   const char *kernel_name = "none";
@@ -169,6 +174,8 @@ void free_handle(rift_ile *h) {
   if (h->s_d2h) cudaStreamDestroy(h->s_d2h);
   cudaFree(h->d_hp);
   cudaFree(h->d_hl);
+  cudaFree(h->d_dm_nodes);
+  cudaFree(h->d_dm_dist);
   cudaFree(h->d_modes);
   cudaFree(h->d_Q);
   cudaFree(h->d_Qe);
@@ -587,7 +594,7 @@ int ensure_reduce_buffers(rift_ile *h, int32_t n_seg, int64_t n_per_seg, int32_t
 }
 
 int run_chunks(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *const params[6], double *lnL_out,
-               int32_t *shift_out, double *dbg_F, double *dbg_Y, double *dbg_quad, cudaStream_t s) {
+               int32_t *shift_out, double *dbg_F, double *dbg_Y, double *dbg_quad, cudaStream_t s, int dm_nodes = 0) {
   const int64_t total = (int64_t)n_seg * n_per_seg;
   if (total == 0) return RIFT_OK;
   const int64_t cap = chunk_samples(h);
@@ -613,7 +620,13 @@ int run_chunks(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *cons
     if (lnL_out) {
       int nl = 0;
       ProfSpan ps(h, 1, s);
-      if (!fp32 && use_mma(h)) {
+      if (dm_nodes > 0) {                                   // distance-marginalised variant of the direct kernel
+        const bool fits = lnl_direct_dm_smem_bytes(h->qs, fp32, true, dm_nodes) <= 227u * 1024u;
+        const bool ext = !fits && h->d_Qg != nullptr;
+        CU(h, launch_lnl_direct_dmarg(ext ? h->qsg : h->qs, fp32, fits, ext, b, ws, h->K, dm_nodes, h->d_dm_nodes,
+                                      h->d_dm_nodes + dm_nodes, lnL_out, h->n_sm, s, &nl));
+        h->kernel_name = fp32 ? "lnl_direct_dmarg<f32>" : "lnl_direct_dmarg<f64>";
+      } else if (!fp32 && use_mma(h)) {
         CU(h, launch_lnl_mma(h->mma, h->d_Qm, b, ws, lnL_out, h->n_sm, s, &nl));
         h->kernel_name = h->mma.stream ? "lnl_mma<f64,stream>" : "lnl_mma<f64,resident>";
       } else if (h->d_Qe != nullptr && fp32) {
@@ -1019,6 +1032,63 @@ int rift_ile_eval_batch_host(rift_ile_t *h, int32_t n_seg, const int32_t *intrin
   CU(h, cudaEventRecord(ev_end, h->s_d2h));
   CU(h, cudaStreamWaitEvent(s, ev_end, 0));                      // the caller's stream is complete when lnL_out is
   return RIFT_OK;
+}
+
+int rift_ile_eval_batch_dmarg(rift_ile_t *h, int32_t n_seg, const int32_t *intrinsic_ids, int64_t n_per_seg,
+                              const double *const params[5], double d_min_mpc, double d_max_mpc, int32_t n_dist,
+                              double *lnL_out, int32_t *shift_out, void *cuda_stream) {
+  if (!h) return RIFT_EINVAL;
+  if (n_seg < 0 || n_per_seg < 0) return fail(h, RIFT_EINVAL, "negative size");
+  if (!(d_min_mpc > 0.0) || !(d_max_mpc > d_min_mpc) || !std::isfinite(d_max_mpc)) return fail(h, RIFT_EINVAL, "distance range");
+  if (n_dist < 8 || n_dist > 512 || (n_dist & 7)) return fail(h, RIFT_EINVAL, "n_dist must be a multiple of 8 in [8, 512]");
+  if (n_seg == 0 || n_per_seg == 0) return RIFT_OK;
+  if (!intrinsic_ids || !params || !lnL_out) return fail(h, RIFT_EINVAL, "null pointer");
+  for (int d = 0; d < 5; ++d)
+    if (!params[d]) return fail(h, RIFT_EINVAL, "null parameter array");
+  DeviceGuard g(h->device);
+  cudaStream_t s = reinterpret_cast<cudaStream_t>(cuda_stream);
+  if (h->dm_n != n_dist || h->dm_dmin != d_min_mpc || h->dm_dmax != d_max_mpc) {
+    // composite 8-point Gauss-Legendre rule in u = ln D on n_dist / 8 equal panels: c_i = D_ref / D_i and
+    // ln W_i, W_i = w_i p(D_i) D_i with the d_L^2 prior p(D) = 3 D^2 / (D_max^3 - D_min^3)
+    static const double gx[4] = {0.1834346424956498049, 0.5255324099163289858, 0.7966664774136267396, 0.9602898564975362317};
+    static const double gw[4] = {0.3626837833783619830, 0.3137066458778872873, 0.2223810344533744706, 0.1012285362903762591};
+    std::vector<double> tab(2 * (size_t)n_dist);
+    const int n_panels = n_dist / 8;
+    const double u0 = std::log(d_min_mpc), hp = (std::log(d_max_mpc) - u0) / n_panels;
+    const double ln_norm = std::log(3.0) - std::log(d_max_mpc * d_max_mpc * d_max_mpc - d_min_mpc * d_min_mpc * d_min_mpc);
+    for (int p = 0; p < n_panels; ++p)
+      for (int q = 0; q < 8; ++q) {
+        const double xi = q < 4 ? -gx[3 - q] : gx[q - 4], wi = q < 4 ? gw[3 - q] : gw[q - 4];
+        const double u = u0 + hp * (p + 0.5 * (1.0 + xi));
+        tab[8 * p + q] = h->geom.d_ref / std::exp(u);
+        tab[n_dist + 8 * p + q] = std::log(0.5 * hp * wi) + ln_norm + 3.0 * u;
+      }
+    if (h->dm_n != n_dist) {
+      cudaFree(h->d_dm_nodes);
+      h->d_dm_nodes = nullptr;
+      h->dm_n = 0;
+      CU(h, cudaMalloc(&h->d_dm_nodes, tab.size() * sizeof(double)));
+    }
+    CU(h, cudaStreamSynchronize(s));                             // an earlier call on this stream may still read the table
+    CU(h, cudaMemcpy(h->d_dm_nodes, tab.data(), tab.size() * sizeof(double), cudaMemcpyHostToDevice));
+    h->dm_n = n_dist;
+    h->dm_dmin = d_min_mpc;
+    h->dm_dmax = d_max_mpc;
+  }
+  const int64_t total = (int64_t)n_seg * n_per_seg;
+  if (total > h->dm_dist_cap) {                                  // the geometry kernel runs at D = D_ref: c = 1, q = b
+    cudaFree(h->d_dm_dist);
+    h->d_dm_dist = nullptr;
+    h->dm_dist_cap = 0;
+    CU(h, cudaMalloc(&h->d_dm_dist, (size_t)total * sizeof(double)));
+    h->dm_dist_cap = total;
+    CU(h, launch_fill_f64(h->d_dm_dist, total, h->geom.d_ref, s));
+    ++h->launches;
+  }
+  const double *p6[RIFT_N_PARAMS] = {params[0], params[1], params[2], params[3], params[4], h->d_dm_dist};
+  int rc = upload_ids(h, n_seg, intrinsic_ids, s);
+  if (rc != RIFT_OK) return rc;
+  return run_chunks(h, n_seg, n_per_seg, p6, lnL_out, shift_out, nullptr, nullptr, nullptr, s, n_dist);
 }
 
 int rift_ile_staged(rift_ile_t *h, const double *params_dev[RIFT_N_PARAMS], const double **ln_weight_dev,

@@ -209,6 +209,17 @@ cudaError_t launch_convert_q_planar(const double *Q_c128, void *dst, int64_t row
   return cudaGetLastError();
 }
 
+__global__ void fill_f64_kernel(double *dst, int64_t n, double value) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) dst[i] = value;
+}
+cudaError_t launch_fill_f64(double *dst, int64_t n, double value, cudaStream_t s) {
+  if (n <= 0) return cudaSuccess;
+  int grid = (int)((n + 255) / 256);
+  if (grid > 148 * 8) grid = 148 * 8;
+  fill_f64_kernel<<<grid, 256, 0, s>>>(dst, n, value);
+  return cudaGetLastError();
+}
+
 cudaError_t run_fma_peak(int mode, int iters, double *tflops, cudaStream_t s) {
   const bool fp64 = mode == 1;
   int dev = 0, n_sm = 0;

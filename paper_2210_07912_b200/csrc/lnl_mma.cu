@@ -22,6 +22,7 @@
 // ones stream (detector, k-step) chunks through a ring filled by a producer warp with cp.async.bulk on mbarriers.
 #include "rift_internal.h"
 #include "tma_utils.cuh"
+#include "exp2_poly.cuh"
 
 namespace {
 
@@ -54,28 +55,6 @@ __device__ __forceinline__ void dmma(double (&d)[2], double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                : "+d"(d[0]), "+d"(d[1])
                : "d"(a), "d"(b));
-}
-
-// 2^y for y <~ 0 (NaN propagates): y = n + r, |r| <= 1/2, 2^r by a degree-8 polynomial (interpolation at Chebyshev nodes,
-// relative error 1.1e-12), 2^n through the exponent field (n clamped at -1000: 2^-1000 stands in for smaller terms).
-// 12 FP64-pipe operations with the argument FMA of the caller; the coefficients are constant-bank operands.
-__constant__ double MM_EXP2_C[9] = {1.0,
-                                    0x1.62e42fef84cf0p-1,
-                                    0x1.ebfbdff823cedp-3,
-                                    0x1.c6b08dd6fd239p-5,
-                                    0x1.3b2ab7181b784p-7,
-                                    0x1.5d8745a727ee4p-10,
-                                    0x1.4308ac85a5afep-13,
-                                    0x1.00dc4a5363675p-16,
-                                    0x1.63d1363b4014fp-20};
-__device__ __forceinline__ double mm_exp2(double y) {
-  const double t = y + 6755399441055744.0;                       // 1.5 * 2^52: the low word of t holds rint(y)
-  const int n = max(__double2loint(t), -1000);
-  const double r = y - (t - 6755399441055744.0);
-  double p = MM_EXP2_C[8];
-#pragma unroll
-  for (int i = 7; i >= 0; --i) p = fma(p, r, MM_EXP2_C[i]);
-  return __hiloint2double(__double2hiint(p) + (n << 20), __double2loint(p));
 }
 
 struct MmaSmem {                                   // byte offsets inside dynamic shared memory
@@ -380,7 +359,7 @@ __global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs
       double sum = 0.0;
 #pragma unroll
       for (int e = 0; e < NE; ++e)
-        if (jb + JS * e < n_x) sum += mm_exp2(fma(x[e], cl2, mo));
+        if (jb + JS * e < n_x) sum += poly_exp2(fma(x[e], cl2, mo));
       sum += __shfl_xor_sync(0xffffffffu, sum, 8);
       if (NT == 1) sum += __shfl_xor_sync(0xffffffffu, sum, 16);
       if (jj == 0) psum[n_mine * 16 + wg] = sum;

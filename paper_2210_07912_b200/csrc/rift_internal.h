@@ -141,6 +141,10 @@ cudaError_t launch_build_quad_uv(const QuadProg &qp, const double *U, const doub
 size_t lnl_direct_smem_bytes(const QStore &q, bool fp32, bool q_in_smem);
 cudaError_t launch_lnl_direct(const QStore &q, bool fp32, bool q_in_smem, bool q_ext, const Batch &b, const Workspace &ws,
                               int n_det, double *lnL_out, int n_sm, cudaStream_t s, int *n_launch);
+size_t lnl_direct_dm_smem_bytes(const QStore &q, bool fp32, bool q_in_smem, int n_dist);
+cudaError_t launch_lnl_direct_dmarg(const QStore &q, bool fp32, bool q_in_smem, bool q_ext, const Batch &b,
+                                    const Workspace &ws, int n_det, int n_dist, const double *c_nodes, const double *lnw_nodes,
+                                    double *lnL_out, int n_sm, cudaStream_t s, int *n_launch);   // NEXT-2, distance marginal
 // lnl_direct_ext.cu (interleaved layout with a circular extension of RIFT_EXT samples per row)
 size_t lnl_direct_ext_smem_bytes(const QStore &q, bool fp32);
 cudaError_t launch_lnl_direct_ext(const QStore &q, bool fp32, const Batch &b, const Workspace &ws, int n_det,
@@ -182,4 +186,5 @@ int32_t reduce_blocks_per_seg(int64_t n_per_seg, int32_t n_seg);
 // convert.cu
 cudaError_t launch_convert_q(const double *Q_c128, void *dst, int64_t rows, int32_t n_t, int32_t n_tp, bool to_fp32,
                              cudaStream_t s);
+cudaError_t launch_fill_f64(double *dst, int64_t n, double value, cudaStream_t s);
 cudaError_t run_fma_peak(int mode, int iters, double *tflops, cudaStream_t s);   // 0 fp32, 1 fp64, 2 fp32 register tile
