@@ -45,7 +45,7 @@ enum { RIFT_PREC_FP64 = 0, RIFT_PREC_MIXED = 1 };   /* arithmetic of the window 
 enum { RIFT_Q_C128 = 0, RIFT_Q_C64 = 1 };           /* storage of Q on the device */
 enum { RIFT_MEM_HOST = 0, RIFT_MEM_DEVICE = 1 };    /* where the Q/U/V arrays passed to create live */
 enum { RIFT_KERNEL_AUTO = 0, RIFT_KERNEL_DIRECT = 1, RIFT_KERNEL_TC = 2, RIFT_KERNEL_TCS = 3,
-       RIFT_KERNEL_MMA = 4 };                       /* rift_ile_set_kernel */
+       RIFT_KERNEL_MMA = 4, RIFT_KERNEL_SKY = 5 };  /* rift_ile_set_kernel */
 enum { RIFT_OPT_TC_CHUNK_MIB = 1,   /* per-chunk workspace of the tensor-core kernels in MiB (default 1024, >= 1) */
        RIFT_OPT_TC_SORT = 2,        /* 1 (default): AUTO may pick the shift-sorted tensor-core kernel; 0: never */
        RIFT_OPT_QUAD_PROG = 3 };    /* 1 (default): quadratic term of > 8 modes by the pair program; 0: plain pair sum */
@@ -150,7 +150,8 @@ int rift_ile_geometry(rift_ile_t *h, int32_t intrinsic_id, int64_t n, const doub
 
 /* Choose the fused-lnL kernel variant (RIFT_KERNEL_*); AUTO picks per configuration and call size: in mixed precision the
  * tensor-core kernels (TCS, which buckets the samples by the relative shift of detector 1, for calls of >= 32768 samples in
- * segments of >= 100 samples per bucket; else TC) when the configuration fits tensor and shared memory; in fp64 mode the
+ * segments of >= 100 samples per bucket; else TC) when the configuration fits tensor and shared memory, and for longer
+ * windows SKY (samples bucketed by sky cell, time-tiled tensor-core contraction; segments of >= 256 samples per cell); in fp64 mode the
  * FP64 tensor-core kernel (MMA) when the configuration fits; else the direct kernels.  A variant that does not apply to
  * the handle falls back to the AUTO choice.  lnL does not depend on the variant beyond the stated tolerance of the
  * precision mode. */
@@ -182,7 +183,8 @@ int rift_ile_profile_read(rift_ile_t *h, double ms[4], int64_t launches[4]);
  * filling the device and returns achieved TFLOP/s in *tflops.  mode: 0 = FFMA chains, 1 = DFMA chains, 2 = FFMA 7x8
  * register tile (all operands in registers, the operand pattern of the fused kernels), 3 / 4 / 5 = FP64 tensor-core
  * mma.sync m8n8k4 / m16n8k8 / m16n8k16 (8 independent accumulator tiles per warp), 6 = m8n8k4 interleaved with as many
- * independent DFMA per thread (reports the tensor part: do the two share a pipe?). */
+ * independent DFMA per thread (reports the tensor part: do the two share a pipe?), 7 = mma.sync m16n8k16 fp16 -> fp32
+ * (the legacy tensor path lnl_sky contracts on). */
 int rift_ile_fma_peak(int32_t mode, int32_t iters, double *tflops, void *cuda_stream);
 
 int rift_ile_destroy(rift_ile_t *h);

@@ -20,7 +20,7 @@ RIFT_OK, RIFT_EINVAL, RIFT_ENOMEM, RIFT_ECUDA, RIFT_EWINDOW, RIFT_ERANGE, RIFT_E
 RIFT_PREC_FP64, RIFT_PREC_MIXED = 0, 1
 RIFT_Q_C128, RIFT_Q_C64 = 0, 1
 RIFT_MEM_HOST, RIFT_MEM_DEVICE = 0, 1
-RIFT_KERNEL_AUTO, RIFT_KERNEL_DIRECT, RIFT_KERNEL_TC, RIFT_KERNEL_TCS, RIFT_KERNEL_MMA = 0, 1, 2, 3, 4
+RIFT_KERNEL_AUTO, RIFT_KERNEL_DIRECT, RIFT_KERNEL_TC, RIFT_KERNEL_TCS, RIFT_KERNEL_MMA, RIFT_KERNEL_SKY = 0, 1, 2, 3, 4, 5
 RIFT_OPT_TC_CHUNK_MIB, RIFT_OPT_TC_SORT, RIFT_OPT_QUAD_PROG = 1, 2, 3
 RIFT_N_PARAMS = 6
 

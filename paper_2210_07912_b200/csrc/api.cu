@@ -26,6 +26,14 @@ struct rift_ile {
   QStore qsg{};                    // lnl_direct reads it from global memory with one address per mode row (no wrap arithmetic)
   MmaPlan mma{};                   // fp64 tensor-core path (lnl_mma.cu); mma.ok == 0 when the configuration does not fit
   void *d_Qm = nullptr;            // its Q operand: [P][K][2 KS][pitch_q] bytes
+  SkyPlan sky{};                   // sky-sorted, time-tiled tensor-core path (lnl_sky.cu); sky.ok == 0: does not apply
+  SkyCells sky_cells{};
+  void *d_Qsky = nullptr;          // its Q operand: [P][K][rows_ext][kp] fp16
+  float *d_qscale_sky = nullptr;   // [P]
+  int32_t *sky_buf = nullptr;      // key, pos, count, base, perm, n_batches of a chunk
+  int64_t sky_buf_cap = 0;
+  int32_t *sky_orig = nullptr;     // [slots] chunk-local sample of a sorted slot
+  int64_t sky_orig_cap = 0;
   TcPlan tc{};                     // tensor-core path (lnl_tc.cu); tc.ok == 0 when the configuration does not fit
   uint32_t *d_Qtc = nullptr;       // A operand: [P][K][nt*128][acols] words of two fp16
   float *d_qscale = nullptr;       // [P] power-of-two scale of each point's Q in the A operand
@@ -181,6 +189,10 @@ void free_handle(rift_ile *h) {
   cudaFree(h->d_Qe);
   cudaFree(h->d_Qtc);
   cudaFree(h->d_Qm);
+  cudaFree(h->d_Qsky);
+  cudaFree(h->d_qscale_sky);
+  cudaFree(h->sky_buf);
+  cudaFree(h->sky_orig);
   cudaFree(h->d_qscale);
   cudaFree(h->tc_blob);
   cudaFree(h->tc_c);
@@ -353,12 +365,53 @@ void make_mma_plan(rift_ile *h, double delta_t) {
   p.ok = 0;
 }
 
+// mixed mode, circular window: plan of the sky-sorted kernel (any window length; up to 10 modes for now: one 128-byte
+// operand row per sample of Q)
+void make_sky_plan(rift_ile *h, double delta_t) {
+  SkyPlan &p = h->sky;
+  p = SkyPlan{};
+  if (h->precision != RIFT_PREC_MIXED || h->n_tau != h->n_t || h->K > 8) return;
+  double dmax = 0;
+  for (int k = 1; k < h->K; ++k) {
+    double d2 = 0;
+    for (int i = 0; i < 3; ++i) {
+      const double d = h->geom.loc[k][i] - h->geom.loc[0][i];
+      d2 += d * d;
+    }
+    dmax = std::max(dmax, std::sqrt(d2) / (RIFT_C_LIGHT * delta_t));
+  }
+  if (dmax > 1e5) return;
+  const int dm = (int)std::ceil(dmax) + 1;
+  p.K = h->K;
+  p.M = h->M;
+  p.n_t = h->n_t;
+  p.kp = (6 * h->M + 63) & ~63;
+  p.ks = p.kp / 16;
+  p.rowb = 2 * p.kp;
+  p.R0 = (dm + 7) & ~7;
+  p.n_blocks = (h->n_t + SKY_TBO - 1) / SKY_TBO;
+  p.rows_ext = p.R0 + (p.n_blocks - 1) * SKY_TBO + dm + SKY_TBR + 8;
+  p.point_stride = (int64_t)p.K * p.rows_ext * p.rowb;
+  if (p.ks != 4 && p.ks != 8) return;
+  if (lnl_sky_smem_bytes(p) > 227u * 1024u) return;
+  if (!sky_make_cells(dmax, h->sky_cells)) return;
+  p.ok = 1;
+}
+
+// The sky-sorted kernel pays for its padding (about 32 slots per sky cell and segment): AUTO takes it for segments of at
+// least 256 samples per cell when the tcgen05 kernels do not apply (windows of more than 512 samples: C4).
+bool use_sky(const rift_ile *h, int64_t n_per_seg) {
+  if (!h->sky.ok || h->d_Qsky == nullptr) return false;
+  if (h->kernel_variant == RIFT_KERNEL_SKY) return true;
+  return h->kernel_variant == RIFT_KERNEL_AUTO && !h->tc.ok && n_per_seg >= 256 * (int64_t)h->sky_cells.n_cells;
+}
+
 bool use_mma(const rift_ile *h) {
   return h->mma.ok && h->d_Qm != nullptr && h->kernel_variant != RIFT_KERNEL_DIRECT;
 }
 
 bool use_tc(const rift_ile *h) {
-  if (!h->tc.ok || h->d_Qtc == nullptr) return false;
+  if (!h->tc.ok || h->d_Qtc == nullptr || h->kernel_variant == RIFT_KERNEL_SKY) return false;
   return h->kernel_variant != RIFT_KERNEL_DIRECT;              // a variant of the other precision mode = AUTO
 }
 
@@ -551,6 +604,57 @@ int run_chunks_tcs(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *
     h->launches += nl;
   }
   h->kernel_name = tp.n_sub == 1 ? "lnl_tcs<f16x3>" : "lnl_tcs<f16x3,passes>";
+  return RIFT_OK;
+}
+
+// Sky-sorted path: per chunk (whole segments, up to 2^23 samples) bucket the samples by (segment, sky cell), let the geometry
+// kernel write every sample into its sorted slot (padding slots are null samples), run lnl_sky over the batches of 64 slots.
+int run_chunks_sky(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *const params[6], double *lnL_out,
+                   int32_t *shift_out, cudaStream_t s) {
+  const int64_t total = (int64_t)n_seg * n_per_seg;
+  if (total == 0) return RIFT_OK;
+  const int n_cells = h->sky_cells.n_cells;
+  int64_t cap = (int64_t)1 << 23;
+  if (n_per_seg <= cap) cap = (cap / n_per_seg) * n_per_seg;
+  const int64_t n_max = total < cap ? total : cap;
+  const int64_t lseg_max = n_max / n_per_seg + 2 < n_seg ? n_max / n_per_seg + 2 : n_seg;
+  const int64_t nbk_max = lseg_max * n_cells;
+  const int64_t slots_max = ((n_max + nbk_max * (SKY_NB - 1)) + SKY_NB - 1) / SKY_NB * SKY_NB;
+  int rc = ensure_workspace(h, slots_max);
+  if (rc == RIFT_OK) rc = ensure_i32(h, &h->sky_orig, &h->sky_orig_cap, slots_max);
+  if (rc == RIFT_OK) rc = ensure_i32(h, &h->sky_buf, &h->sky_buf_cap, 2 * n_max + 2 * nbk_max + slots_max + 8);
+  if (rc != RIFT_OK) return rc;
+  for (int64_t g0 = 0; g0 < total; g0 += cap) {
+    Batch b;
+    b.n_per_seg = n_per_seg;
+    b.g0 = g0;
+    b.n = (total - g0 < cap) ? total - g0 : cap;
+    b.ids = h->d_ids;
+    const int n_lseg = (int)((g0 + b.n - 1) / n_per_seg - g0 / n_per_seg + 1);
+    const int64_t nbk = (int64_t)n_lseg * n_cells;
+    const int64_t slots = ((b.n + nbk * (SKY_NB - 1)) + SKY_NB - 1) / SKY_NB * SKY_NB;
+    int32_t *key = h->sky_buf, *pos = key + n_max, *count = pos + n_max, *base = count + nbk_max, *perm = base + nbk_max,
+            *n_batches = perm + slots_max;
+    int nl = 0;
+    Workspace ws = h->ws;
+    ws.orig = h->sky_orig;
+    {
+      ProfSpan ps(h, 0, s);
+      CU(h, launch_sky_sort(h->sky_cells, h->geom.gmst, b, params, n_lseg, key, pos, count, base, perm, slots, n_batches, s, &nl));
+      Batch bs = b;
+      bs.n = slots;                                                // one thread per sorted slot; padding slots return at once
+      CU(h, launch_geometry(h->geom, h->d_modes, bs, params, h->d_U, h->d_V, h->qp, true, ws, shift_out, nullptr, nullptr, perm, s));
+      ++nl;
+      ps.end();
+    }
+    {
+      ProfSpan ps(h, 1, s);
+      CU(h, launch_lnl_sky(h->sky, h->d_Qsky, h->d_qscale_sky, b, ws, n_batches, slots / SKY_NB, lnL_out, h->n_sm, s, &nl));
+      ps.end();
+    }
+    h->launches += nl;
+  }
+  h->kernel_name = "lnl_sky<f16x3>";
   return RIFT_OK;
 }
 
@@ -848,6 +952,19 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
         h->d_Qm = nullptr;
       }
     }
+    // Q operand of the sky-sorted kernel (optional layout: an allocation failure leaves the variant unavailable)
+    make_sky_plan(h, cfg->delta_t);
+    if (e == cudaSuccess && h->sky.ok) {
+      if (cudaMalloc(&h->d_Qsky, (size_t)h->P * h->sky.point_stride) == cudaSuccess &&
+          cudaMalloc(&h->d_qscale_sky, sizeof(float) * h->P) == cudaSuccess) {
+        e = launch_convert_q_sky(src, h->d_Qsky, h->d_qscale_sky, h->sky, h->P, 0);
+        h->launches += 3;
+      } else {
+        cudaGetLastError();
+        cudaFree(h->d_Qsky);
+        h->d_Qsky = nullptr;
+      }
+    }
     // A operand of the tensor-core path (fp16 hi | lo pieces), when the configuration fits tensor memory
     make_tc_plan(h, cfg->delta_t);
     if (e == cudaSuccess && h->tc.ok) {
@@ -889,7 +1006,7 @@ int rift_ile_destroy(rift_ile_t *h) {
 int rift_ile_set_kernel(rift_ile_t *h, int32_t variant) {
   if (!h) return RIFT_EINVAL;
   if (variant != RIFT_KERNEL_AUTO && variant != RIFT_KERNEL_DIRECT && variant != RIFT_KERNEL_TC && variant != RIFT_KERNEL_TCS &&
-      variant != RIFT_KERNEL_MMA)
+      variant != RIFT_KERNEL_MMA && variant != RIFT_KERNEL_SKY)
     return fail(h, RIFT_EINVAL, "unknown kernel variant");
   h->kernel_variant = variant;
   return RIFT_OK;
@@ -948,6 +1065,7 @@ static int eval_batch_device(rift_ile *h, int32_t n_seg, const int32_t *intrinsi
                              const double *const params[RIFT_N_PARAMS], double *lnL_out, int32_t *shift_out, cudaStream_t s) {
   int rc = upload_ids(h, n_seg, intrinsic_ids, s);
   if (rc != RIFT_OK) return rc;
+  if (use_sky(h, n_per_seg)) return run_chunks_sky(h, n_seg, n_per_seg, params, lnL_out, shift_out, s);
   if (use_tc(h) && use_tcs(h, n_seg, n_per_seg)) return run_chunks_tcs(h, n_seg, n_per_seg, params, lnL_out, shift_out, s);
   if (use_tc(h)) return run_chunks_tc(h, n_seg, n_per_seg, params, lnL_out, shift_out, s);
   return run_chunks(h, n_seg, n_per_seg, params, lnL_out, shift_out, nullptr, nullptr, nullptr, s);

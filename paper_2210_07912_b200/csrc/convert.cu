@@ -122,6 +122,29 @@ __device__ __forceinline__ void dmma16816(double (&d)[4], const double (&a)[8], 
                  "d"(b[2]), "d"(b[3]));
 }
 
+// legacy tensor-core path (HMMA): mma.sync m16n8k16, fp16 operands, fp32 accumulate; mode 7 of run_fma_peak
+__global__ void __launch_bounds__(256) hmma_peak_kernel(int iters, const uint32_t *__restrict__ src, float *sink) {
+  uint32_t a[4], b[2];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) a[i] = src[threadIdx.x + 32 * i];
+  b[0] = src[300 + threadIdx.x];
+  b[1] = src[400 + threadIdx.x];
+  float d[8][4];
+#pragma unroll
+  for (int t = 0; t < 8; ++t) d[t][0] = d[t][1] = d[t][2] = d[t][3] = 0.f;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int t = 0; t < 8; ++t)
+      asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                   : "+f"(d[t][0]), "+f"(d[t][1]), "+f"(d[t][2]), "+f"(d[t][3])
+                   : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
+  }
+  float s = 0;
+#pragma unroll
+  for (int t = 0; t < 8; ++t) s += d[t][0] + d[t][1] + d[t][2] + d[t][3];
+  if (s == 123.456f) sink[0] = s;
+}
+
 template <int MODE>
 __global__ void __launch_bounds__(256) dmma_peak_kernel(int iters, const double *__restrict__ src, double *sink) {
   constexpr int NACC = 8;
@@ -247,6 +270,8 @@ cudaError_t run_fma_peak(int mode, int iters, double *tflops, cudaStream_t s) {
       dmma_peak_kernel<4><<<grid, threads, 0, s>>>(iters, reinterpret_cast<const double *>(src), reinterpret_cast<double *>(sink));
     else if (mode == 5)
       dmma_peak_kernel<5><<<grid, threads, 0, s>>>(iters, reinterpret_cast<const double *>(src), reinterpret_cast<double *>(sink));
+    else if (mode == 7)
+      hmma_peak_kernel<<<grid, threads, 0, s>>>(iters, reinterpret_cast<const uint32_t *>(src), reinterpret_cast<float *>(sink));
     else if (mode == 6)
       dmma_peak_kernel<6><<<grid, threads, 0, s>>>(iters, reinterpret_cast<const double *>(src), reinterpret_cast<double *>(sink));
     else if (fp64)
@@ -267,7 +292,7 @@ cudaError_t run_fma_peak(int mode, int iters, double *tflops, cudaStream_t s) {
   if (e != cudaSuccess) return e;
   // flop per thread and iteration: 8 FMA chains; 56 in the register tile; DMMA: 8 tiles x (m n k / 32 lanes) FMA
   //   m8n8k4 8, m16n8k8 32, m16n8k16 64 FMA per lane and tile; mode 6 reports the DMMA part only (+ 8 DFMA ride along)
-  const double fma_per_it = mode == 2 ? 56.0 : mode == 3 || mode == 6 ? 64.0 : mode == 4 ? 256.0 : mode == 5 ? 512.0 : 8.0;
+  const double fma_per_it = mode == 2 ? 56.0 : mode == 3 || mode == 6 ? 64.0 : mode == 4 ? 256.0 : mode == 5 ? 512.0 : mode == 7 ? 8.0 * 64.0 : 8.0;
   *tflops = 2.0 * fma_per_it * (double)iters * grid * threads / (best * 1e-3) / 1e12;
   return cudaGetLastError();
 }

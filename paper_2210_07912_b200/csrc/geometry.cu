@@ -310,6 +310,17 @@ geometry_kernel(DetGeom g, const ModeEntry *__restrict__ modes, Batch b, const d
   if (w >= b.n) return;
   const int64_t src = perm ? (int64_t)perm[w] : w;                         // chunk-local index of the sample
   if (ws.orig) ws.orig[w] = (int32_t)src;
+  if (src < 0) {                                                           // padding slot of a sorted layout: a null sample
+    ws.scale_c[w] = 1.0;
+    ws.quad[w] = 0.0;
+    for (int k = 0; k < K; ++k) ws.shift[w * K + k] = INT32_MAX;           // excluded from the batch's shift bounds
+    CT *out = reinterpret_cast<CT *>(reinterpret_cast<decltype(CT::x) *>(ws.coef) + w * ws.coef_stride);
+    CT z;
+    z.x = 0;
+    z.y = 0;
+    for (int i = 0; i < K * M; ++i) out[i] = z;
+    return;
+  }
   const int64_t gi = b.g0 + src;                                           // caller's sample index
   const int32_t point = b.ids[gi / b.n_per_seg];
 

@@ -2,6 +2,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <cmath>
 
 #include "rift_ile.h"
 
@@ -128,6 +129,26 @@ struct MmaPlan {
   int64_t point_stride;          // bytes per intrinsic point
 };
 
+// Sky-sorted, time-tiled tensor-core path (sky_sort.cu, lnl_sky.cu): mixed precision, windows of any length.
+#define SKY_NB 64                // samples per batch (eight 8-column tiles)
+#define SKY_E 32                 // residual shifts of a batch lie in [0, SKY_E)
+#define SKY_TBO 224              // window entries per time block
+#define SKY_TBR 256              // Q rows per (time block, detector) chunk = SKY_TBO + SKY_E
+#define SKY_MAX_RINGS 512
+struct SkyCells {                // sky cells of the bucketing pass (sky_sort.cu)
+  double delta;                  // ring width (rad)
+  int32_t n_rings, n_cells;
+  int32_t ring_off[SKY_MAX_RINGS + 1];   // first cell of each declination ring
+};
+struct SkyPlan {
+  int32_t ok;
+  int32_t K, M, n_t;
+  int32_t kp, ks, rowb;          // fp16 elements per operand row [Q_hi | Q_lo | Q_hi] (multiple of 64), k-steps of 16, bytes
+  int32_t R0, rows_ext;          // extended row of original row 0; rows per (point, detector): row e holds (e - R0) mod n_t
+  int32_t n_blocks;              // time blocks of SKY_TBO window entries
+  int64_t point_stride;          // bytes per intrinsic point: K * rows_ext * rowb
+};
+
 // geometry.cu
 cudaError_t launch_geometry_tc(const DetGeom &g, const ModeEntry *modes, const TcPlan &tp, const TcChunk &c,
                                const double *const params[6], const double *U, const double *V, const QuadProg &qp,
@@ -172,6 +193,17 @@ size_t lnl_mma_smem_bytes(const MmaPlan &p);
 cudaError_t launch_convert_q_mma(const double *Q_c128, void *dst, const MmaPlan &p, int32_t n_points, cudaStream_t s);
 cudaError_t launch_lnl_mma(const MmaPlan &p, const void *q, const Batch &b, const Workspace &ws, double *lnL_out, int n_sm,
                            cudaStream_t s, int *n_launch);
+// sky_sort.cu / lnl_sky.cu
+bool sky_make_cells(double dmax_samples, SkyCells &c);
+cudaError_t launch_sky_sort(const SkyCells &cells, double gmst, const Batch &b, const double *const params[6], int n_lseg,
+                            int32_t *key, int32_t *pos, int32_t *count, int32_t *base, int32_t *perm, int64_t cap_slots,
+                            int32_t *n_batches, cudaStream_t s, int *n_launch);
+size_t lnl_sky_smem_bytes(const SkyPlan &p);
+cudaError_t launch_convert_q_sky(const double *Q_c128, void *dst, float *qscale, const SkyPlan &p, int32_t n_points,
+                                 cudaStream_t s);
+cudaError_t launch_lnl_sky(const SkyPlan &p, const void *q, const float *qscale, const Batch &b, const Workspace &ws,
+                           const int32_t *n_batches_dev, int64_t max_batches, double *lnL_out, int n_sm, cudaStream_t s,
+                           int *n_launch);
 // reduce.cu
 struct ReduceState {             // device, per segment
   double m, s1, s2;
