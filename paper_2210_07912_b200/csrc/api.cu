@@ -385,14 +385,13 @@ void make_sky_plan(rift_ile *h, double delta_t) {
   p.K = h->K;
   p.M = h->M;
   p.n_t = h->n_t;
-  p.kp = (6 * h->M + 63) & ~63;
+  p.kp = (6 * h->M + 15) & ~15;
   p.ks = p.kp / 16;
   p.rowb = 2 * p.kp;
   p.R0 = (dm + 7) & ~7;
   p.n_blocks = (h->n_t + SKY_TBO - 1) / SKY_TBO;
   p.rows_ext = p.R0 + (p.n_blocks - 1) * SKY_TBO + dm + SKY_TBR + 8;
   p.point_stride = (int64_t)p.K * p.rows_ext * p.rowb;
-  if (p.ks != 4 && p.ks != 8) return;
   if (lnl_sky_smem_bytes(p) > 227u * 1024u) return;
   if (!sky_make_cells(dmax, h->sky_cells)) return;
   p.ok = 1;

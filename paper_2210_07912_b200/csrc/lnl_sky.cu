@@ -6,45 +6,48 @@
 // d_{n,k} = s_k - s_0 = b_k + r_{n,k} with one base b_k per detector and residuals 0 <= r < SKY_E.  Circular window
 // (N_tau = N_t), detector-0 time: x_j = sum_k P_k[(j + b_k + r_{n,k}) mod N_t, n], P_k[t, n] = sum_kappa A_k[t, kappa] B_k[kappa, n].
 // Time is tiled in blocks of 224 window entries.  Per (block, detector) a chunk of 256 consecutive operand rows starting at
-// row  block start + b_k  of the circularly extended fp16 operand [Q_hi | Q_lo | Q_hi] arrives by one bulk copy (three ring
-// slots); 16 warps contract it with the coefficient operand [B_hi | B_hi | B_lo] of the batch (reading B8: fp16 pieces,
-// products exact in the fp32 accumulator) by mma.sync.m16n8k16 -- 4 row tiles x 2 sample tiles per warp, A fragments by
-// ldmatrix from rows whose 16-byte chunks are XOR-swizzled in global memory already; the tiles are stored unshifted into an
-// exchange buffer [256 rows][64 samples] (32-byte groups swizzled by row: conflict-free 8-byte stores); after a barrier
-// every thread adds  P_k[j + r_{n,k}][n]  for its sample n (= lane: one bank per lane whatever the shifts) and its 28 window
-// entries j = 8 e + warp/2 of the block into registers.  After the last detector the block joins the thread's running
-// (max, sum) of 2^(c log2e (x - max)) -- an on-line log-sum-exp, so the window never exists anywhere as a whole.
+// row  block start + b_k  of the circularly extended fp16 operand [Q_hi | Q_lo | Q_hi] (K-major planes of 8 elements) arrives
+// by bulk copies into one of three ring slots; one elected thread contracts it with the coefficient operand
+// [B_hi | B_hi | B_lo] of the batch (reading B8: fp16 pieces, products exact in the fp32 accumulator) by tcgen05.mma, both
+// operands from shared memory, 2 row tiles of 128 x 64 samples x K = 16 per step, accumulators double-buffered in tensor
+// memory so that the tensor core works on chunk i + 1 while the 16 warps drain chunk i: tcgen05.ld (thread = row, 16 samples),
+// unshifted store into an exchange buffer [64 samples][256 rows] (lanes = consecutive rows: conflict-free), barrier, then
+// every warp adds  P_k[j + r_{n,k}][n]  for its 4 samples n and the block's 224 window entries j = lane + 32 e into registers
+// (again lanes = consecutive rows, whatever the shifts).  After the last detector the block joins the lane's running
+// (max, sum) of 2^(c log2e (x - max)) per sample -- an on-line log-sum-exp, so the window never exists anywhere as a whole.
 // Nothing but Q rows, 23 KB of coefficients per batch and one lnL per sample moves through L2 / HBM.
 #include <cuda_fp16.h>
 
-#include "rift_internal.h"
-#include "tma_utils.cuh"
+#include "tc_common.cuh"
 
 namespace {
 
 constexpr int SKY_WARPS = 16, SKY_THREADS = SKY_WARPS * 32, SKY_SLOTS = 3;
-constexpr int SKY_NE = SKY_TBO / 8;                 // window entries per thread and time block
+constexpr int SKY_NE = SKY_TBO / 32;               // window entries per lane, sample and time block
+constexpr int SKY_SPW = SKY_NB / SKY_WARPS;        // samples per warp in the reader role
 constexpr float SKY_BSCALE = 8192.f;               // 2^13: scale of the coefficient operand (|F_k Y_lm| < 2) into the fp16 range
+// instruction descriptor: D fp32, A/B fp16, both K-major, N = 64, M = 128
+constexpr uint32_t SKY_IDESC = (1u << 4) | ((uint32_t)(SKY_NB >> 3) << 17) | ((128u >> 4) << 24);
 
 struct SkySmem {                                   // byte offsets inside dynamic shared memory
-  uint32_t bars, cl2, cval, qval, orig, resid, bk, part, bs, bs_pitch, xb, ring, slot_bytes, total;
+  uint32_t bars, tmem, cl2, cval, qval, orig, resid, bk, bs, bs_det, xb, ring, slot_bytes, total;
 };
 
 __host__ __device__ inline SkySmem sky_smem(const SkyPlan &p) {
   SkySmem L;
-  L.bars = 0;                                                          // full[3]
+  L.bars = 0;                                                          // full[3], tfull[2]
+  L.tmem = 48;
   L.cl2 = 64;                                                          // float [64]
   L.cval = L.cl2 + SKY_NB * 4;                                         // double [64] c = D_ref / D
   L.qval = L.cval + SKY_NB * 8;                                        // double [64] q
   L.orig = L.qval + SKY_NB * 8;                                        // int [64] caller's sample (chunk-local), -1 = padding
   L.resid = L.orig + SKY_NB * 4;                                       // int [K][64] residual shifts
   L.bk = L.resid + (uint32_t)p.K * SKY_NB * 4;                         // int [8] base shifts, [8] = intrinsic point
-  L.part = (L.bk + 64 + 15u) & ~15u;                                   // float2 [8][64] per-warp-pair (max, sum)
-  L.bs = (L.part + 8 * SKY_NB * 8 + 127u) & ~127u;                     // fp16 [K][64][bs_pitch / 2]
-  L.bs_pitch = (uint32_t)p.kp * 2 + 16;                                // + 16 bytes: fragment loads of 8 samples hit 32 banks
-  L.xb = (L.bs + (uint32_t)p.K * SKY_NB * L.bs_pitch + 127u) & ~127u;  // float [256][64]
+  L.bs = (L.bk + 64 + 127u) & ~127u;                                   // fp16 [K][kp/8 planes][64 samples][8]
+  L.bs_det = (uint32_t)(p.kp >> 3) * SKY_NB * 16;
+  L.xb = (L.bs + (uint32_t)p.K * L.bs_det + 127u) & ~127u;             // float [64 samples][256 rows]
   L.ring = L.xb + SKY_TBR * SKY_NB * 4;
-  L.slot_bytes = SKY_TBR * (uint32_t)p.rowb;
+  L.slot_bytes = SKY_TBR * (uint32_t)p.rowb;                           // [kp/8 planes][256 rows][8 fp16]
   L.total = L.ring + SKY_SLOTS * L.slot_bytes;
   return L;
 }
@@ -52,7 +55,7 @@ __host__ __device__ inline SkySmem sky_smem(const SkyPlan &p) {
 struct SkyArgs {
   SkyPlan p;
   SkySmem L;
-  const unsigned char *q;          // [P][K][rows_ext][rowb] fp16, 16-byte chunks swizzled by (row & 7) inside 128-byte segments
+  const unsigned char *q;          // [P][K][kp/8 planes][rows_ext][8] fp16
   const float *qscale;             // [P] power-of-two scale of each point's Q
   Batch b;
   Workspace ws;                    // sorted slots: coef (fp32), scale_c, quad, shift, orig
@@ -60,16 +63,6 @@ struct SkyArgs {
   double *lnL_out;
 };
 
-__device__ __forceinline__ void ldsm_x4(uint32_t addr, uint32_t (&r)[4]) {
-  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];" : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
-}
-__device__ __forceinline__ void hmma(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
-  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
-               : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
-               : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
-}
-
-template <int KS>
 __global__ void __launch_bounds__(SKY_THREADS, 1) lnl_sky_kernel(const SkyArgs A) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const SkyPlan &P = A.p;
@@ -77,40 +70,47 @@ __global__ void __launch_bounds__(SKY_THREADS, 1) lnl_sky_kernel(const SkyArgs A
   const Batch &b = A.b;
   const Workspace &ws = A.ws;
   uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + L.bars);
+  uint64_t *tfull = full + SKY_SLOTS;
+  uint32_t *tmem_ptr_s = reinterpret_cast<uint32_t *>(smem_raw + L.tmem);
   float *cl2_s = reinterpret_cast<float *>(smem_raw + L.cl2);
   double *cval_s = reinterpret_cast<double *>(smem_raw + L.cval);
   double *qval_s = reinterpret_cast<double *>(smem_raw + L.qval);
   int *orig_s = reinterpret_cast<int *>(smem_raw + L.orig);
   int *resid_s = reinterpret_cast<int *>(smem_raw + L.resid);
   int *bk_s = reinterpret_cast<int *>(smem_raw + L.bk);
-  float2 *part_s = reinterpret_cast<float2 *>(smem_raw + L.part);
   unsigned char *bs = smem_raw + L.bs;
-  unsigned char *xb = smem_raw + L.xb;
+  float *xb = reinterpret_cast<float *>(smem_raw + L.xb);
   unsigned char *ring = smem_raw + L.ring;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int K = P.K, n_t = P.n_t, km2 = 2 * P.M * K, m2 = 2 * P.M;
-  if (tid == 0)
+  const int K = P.K, n_t = P.n_t, m2 = 2 * P.M, npl = P.kp >> 3, ks = P.kp >> 4;
+  if (tid == 0) {
     for (int i = 0; i < SKY_SLOTS; ++i) mbar_init(full + i, 1);
+    mbar_init(tfull, 1);
+    mbar_init(tfull + 1, 1);
+  }
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_ptr_s)) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
   __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_ptr_s;
 
-  // MMA role: sample tiles 2 np, 2 np + 1; row tiles rg + 4 i
-  const int g = lane >> 2, t4 = lane & 3, np = warp & 3, rg = warp >> 2;
-  const uint32_t xb_u32 = smem_u32(xb), ring_u32 = smem_u32(ring);
-  // ldmatrix row of this lane inside a 16-row tile, and its 16-byte chunk inside a k-step
-  const int lm_row = (lane & 7) + 8 * ((lane >> 3) & 1), lm_chunk = lane >> 4;
-  // store role: rows 16 rt + g (+ 8), columns 8 nt + 2 t4 (+ 1); the 32-byte groups of a row are XORed with row & 7 = g
-  const uint32_t st0 = (uint32_t)(16 * rg + g) * 256u + (uint32_t)(((2 * np) ^ g) * 32 + t4 * 8);
-  const uint32_t st1 = (uint32_t)(16 * rg + g) * 256u + (uint32_t)(((2 * np + 1) ^ g) * 32 + t4 * 8);
-  // reader role: sample n_mine = 32 (warp & 1) + lane, window entries ph + 8 e of the block
-  const int n_mine = 32 * (warp & 1) + lane, ph = warp >> 1;
+  // drain role: tensor-memory lanes 32 (warp & 3) .. + 31 (rows of a 128-row tile), columns 16 (warp >> 2) .. + 15 (samples)
+  const int q4 = warp & 3, cg = warp >> 2;
+  const uint32_t t_lane = ((uint32_t)(32 * q4)) << 16;
+  float *xst = xb + (size_t)(16 * cg) * SKY_TBR + 32 * q4 + lane;        // + c * 256 (sample) + 128 mt (row tile)
+  // reader role: samples SKY_SPW warp .. + 3, window entries lane + 32 e of the block
   const double ln_ntau = log((double)n_t);
   const int n_chunks = P.n_blocks * K;
+  const uint32_t ring_u32 = smem_u32(ring), bs_u32 = smem_u32(bs);
 
   const int total_batches = *A.n_batches;
   const int bt_begin = (int)(((int64_t)total_batches * blockIdx.x) / gridDim.x);
   const int bt_end = (int)(((int64_t)total_batches * (blockIdx.x + 1)) / gridDim.x);
-  uint32_t cnt = 0;                                              // chunks consumed so far (ring position and phase)
+  uint32_t cnt = 0;                                              // chunks consumed so far (ring slot, buffers, phases)
 
   for (int bt = bt_begin; bt < bt_end; ++bt) {
     const int64_t slot0 = (int64_t)bt * SKY_NB;
@@ -118,8 +118,7 @@ __global__ void __launch_bounds__(SKY_THREADS, 1) lnl_sky_kernel(const SkyArgs A
     if (tid < 8) bk_s[tid] = INT32_MAX;
     __syncthreads();                                             // previous batch fully consumed; bk reset
     if (tid < SKY_NB) {
-      const int o = ws.orig[slot0 + tid];
-      orig_s[tid] = o;
+      orig_s[tid] = ws.orig[slot0 + tid];
       cval_s[tid] = ws.scale_c[slot0 + tid];
       qval_s[tid] = ws.quad[slot0 + tid];
     }
@@ -136,18 +135,25 @@ __global__ void __launch_bounds__(SKY_THREADS, 1) lnl_sky_kernel(const SkyArgs A
         atomicMin(bk_s + k, my_d);
       }
     }
-    // coefficient operand [B_hi | B_hi | B_lo] as fp16 rows of kp elements per (detector, sample)
-    for (int idx = tid; idx < SKY_NB * K * P.kp; idx += SKY_THREADS) {
-      const int kap = idx % P.kp, nk = idx / P.kp, k = nk % K, n = nk / K;
-      __half h = __float2half_rn(0.f);
-      const int region = kap / m2;
-      if (region < 3) {
-        const float v = reinterpret_cast<const float *>(ws.coef)[(slot0 + n) * ws.coef_stride + k * m2 + (kap - region * m2)] * SKY_BSCALE;
-        const __half hi = __float2half_rn(v);
-        h = region < 2 ? hi : __float2half_rn(v - __half2float(hi));
+    // coefficient operand [B_hi | B_hi | B_lo]: K-major planes of 8 elements, [detector][plane][sample][8 fp16]
+    for (int idx = tid; idx < SKY_NB * K * npl; idx += SKY_THREADS) {
+      const int n = idx % SKY_NB, kc = idx / SKY_NB, c = kc % npl, k = kc / npl;
+      const float *src = reinterpret_cast<const float *>(ws.coef) + (slot0 + n) * ws.coef_stride + k * m2;
+      __align__(16) __half hv[8];
+#pragma unroll
+      for (int e = 0; e < 8; ++e) {
+        const int kap = 8 * c + e, region = kap / m2;
+        __half h = __float2half_rn(0.f);
+        if (region < 3) {
+          const float v = src[kap - region * m2] * SKY_BSCALE;
+          const __half hi = __float2half_rn(v);
+          h = region < 2 ? hi : __float2half_rn(v - __half2float(hi));
+        }
+        hv[e] = h;
       }
-      *reinterpret_cast<__half *>(bs + (size_t)(k * SKY_NB + n) * L.bs_pitch + kap * 2) = h;
+      *reinterpret_cast<uint4 *>(bs + (size_t)k * L.bs_det + ((size_t)c * SKY_NB + n) * 16) = *reinterpret_cast<const uint4 *>(hv);
     }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> UMMA operand reads
     __syncthreads();
     const int point = bk_s[8];
     if (tid < SKY_NB * K) {
@@ -157,114 +163,137 @@ __global__ void __launch_bounds__(SKY_THREADS, 1) lnl_sky_kernel(const SkyArgs A
     }
     if (tid < SKY_NB) cl2_s[tid] = (float)(cval_s[tid] * 1.4426950408889634 / ((double)A.qscale[point] * SKY_BSCALE));
     const unsigned char *qpoint = A.q + (int64_t)point * P.point_stride;
-    auto issue = [&](int i, uint32_t c) {                        // chunk i = (block i / K, detector i % K) into ring slot c % 3
+    // chunk i = (block i / K, detector i % K): 256 rows of every plane into ring slot c % 3
+    auto issue_tma = [&](int i, uint32_t c) {
       const int blk = i / K, k = i - blk * K;
       const int bk = bk_s[k] == INT32_MAX ? 0 : bk_s[k];
-      const int64_t row = (int64_t)k * P.rows_ext + P.R0 + blk * SKY_TBO + bk;
+      const int64_t row = P.R0 + blk * SKY_TBO + bk;
       const uint32_t slot = c % SKY_SLOTS;
       mbar_expect_tx(full + slot, L.slot_bytes);
-      bulk_g2s(ring + slot * L.slot_bytes, qpoint + row * P.rowb, L.slot_bytes, full + slot);
+      for (int pl = 0; pl < npl; ++pl)
+        bulk_g2s(ring + slot * L.slot_bytes + pl * (SKY_TBR * 16),
+                 qpoint + (((int64_t)k * npl + pl) * P.rows_ext + row) * 16, SKY_TBR * 16, full + slot);
     };
-    if (tid == 0)
-      for (int i = 0; i < SKY_SLOTS && i < n_chunks; ++i) issue(i, cnt + i);
+    // P_k tiles of chunk i into accumulator buffer c & 1: 2 row tiles x kp / 16 steps
+    auto issue_mma = [&](int i, uint32_t c) {
+      const int k = i % K;
+      const uint32_t slot = c % SKY_SLOTS;
+      mbar_wait(full + slot, (c / SKY_SLOTS) & 1u);
+      tc_fence_after();
+      const uint64_t adesc = tc_smem_desc(ring_u32 + slot * L.slot_bytes, SKY_TBR * 16u, 128u);
+      const uint64_t bdesc = tc_smem_desc(bs_u32 + (uint32_t)k * L.bs_det, SKY_NB * 16u, 128u);
+      for (int s = 0; s < ks; ++s)
+#pragma unroll
+        for (int mt = 0; mt < 2; ++mt)
+          tc_mma_ss(tmem_base + (c & 1u) * 128u + (uint32_t)(mt * SKY_NB),
+                    adesc + (uint64_t)(((uint32_t)(2 * s) * (SKY_TBR * 16u) + (uint32_t)(128 * mt) * 16u) >> 4),
+                    bdesc + (uint64_t)(((uint32_t)(2 * s) * (SKY_NB * 16u)) >> 4), SKY_IDESC, s > 0 ? 1u : 0u);
+      tc_commit(tfull + (c & 1u));
+    };
+    if (warp == 0) {
+      if (elect_one()) {
+        for (int i = 0; i < SKY_SLOTS && i < n_chunks; ++i) issue_tma(i, cnt + i);
+        issue_mma(0, cnt);
+      }
+      __syncwarp();
+    }
     __syncthreads();
 
-    float m_run = -INFINITY, s_run = 0.f;
-    const float cl2n = cl2_s[n_mine];
+    float m_run[SKY_SPW], s_run[SKY_SPW], cl2n[SKY_SPW];
+#pragma unroll
+    for (int sp = 0; sp < SKY_SPW; ++sp) {
+      m_run[sp] = -INFINITY;
+      s_run[sp] = 0.f;
+      cl2n[sp] = cl2_s[SKY_SPW * warp + sp];
+    }
     for (int blk = 0; blk < P.n_blocks; ++blk) {
-      float x[SKY_NE];
+      float x[SKY_SPW][SKY_NE];
       for (int k = 0; k < K; ++k, ++cnt) {
         const int i = blk * K + k;
-        const uint32_t slot = cnt % SKY_SLOTS;
-        // ---- coefficient fragments of this detector for the warp's two sample tiles
-        uint32_t bf[KS][2][2];
-#pragma unroll
-        for (int s = 0; s < KS; ++s)
-#pragma unroll
-          for (int j = 0; j < 2; ++j) {
-            const unsigned char *p = bs + (size_t)(k * SKY_NB + 8 * (2 * np + j) + g) * L.bs_pitch + (16 * s + 2 * t4) * 2;
-            bf[s][j][0] = *reinterpret_cast<const uint32_t *>(p);
-            bf[s][j][1] = *reinterpret_cast<const uint32_t *>(p + 16);
-          }
-        mbar_wait(full + slot, (cnt / SKY_SLOTS) & 1u);
-        // the chunk's first row in the extended operand decides the swizzle of its rows
-        const int bkk = bk_s[k] == INT32_MAX ? 0 : bk_s[k];
-        const int rs = P.R0 + blk * SKY_TBO + bkk;
-        const uint32_t sw = (uint32_t)((rs + lane) & 7);
-        const uint32_t a_base = ring_u32 + slot * L.slot_bytes + (uint32_t)(16 * rg + lm_row) * (uint32_t)P.rowb;
-        float acc[4][2][4];
-#pragma unroll
-        for (int ii = 0; ii < 4; ++ii)
-#pragma unroll
-          for (int j = 0; j < 2; ++j) acc[ii][j][0] = acc[ii][j][1] = acc[ii][j][2] = acc[ii][j][3] = 0.f;
-#pragma unroll
-        for (int s = 0; s < KS; ++s) {
-          const uint32_t c = 2 * s + lm_chunk;
-          const uint32_t coff = (c >> 3) * 128u + (((c & 7u) ^ sw) << 4);
-#pragma unroll
-          for (int ii = 0; ii < 4; ++ii) {
-            uint32_t af[4];
-            ldsm_x4(a_base + (uint32_t)(64 * ii) * (uint32_t)P.rowb + coff, af);
-            hmma(acc[ii][0], af, bf[s][0][0], bf[s][0][1]);
-            hmma(acc[ii][1], af, bf[s][1][0], bf[s][1][1]);
-          }
+        // the tensor core starts on the next chunk (its accumulator buffer was drained before the barriers of chunk i - 1)
+        if (warp == 0 && i + 1 < n_chunks) {
+          if (elect_one()) issue_mma(i + 1, cnt + 1);
+          __syncwarp();
         }
+        // ---- drain chunk i: thread = row, 16 samples per row tile
+        mbar_wait(tfull + (cnt & 1u), (cnt >> 1) & 1u);
+        tc_fence_after();
+        float acc[2][2][8];
+#pragma unroll
+        for (int mt = 0; mt < 2; ++mt) {
+          const uint32_t ta = tmem_base + t_lane + (cnt & 1u) * 128u + (uint32_t)(mt * SKY_NB + 16 * cg);
+          tc_ld8(ta, acc[mt][0]);
+          tc_ld8(ta + 8, acc[mt][1]);
+        }
+#pragma unroll
+        for (int mt = 0; mt < 2; ++mt) {
+          tc_wait_ld8(acc[mt][0]);
+          tc_wait_ld8(acc[mt][1]);
+        }
+        tc_fence_before();
         __syncthreads();                                         // every reader is done with the previous detector's rows
 #pragma unroll
-        for (int ii = 0; ii < 4; ++ii) {
-          unsigned char *d = xb + ii * (64 * 256);
-          *reinterpret_cast<float2 *>(d + st0) = make_float2(acc[ii][0][0], acc[ii][0][1]);
-          *reinterpret_cast<float2 *>(d + st0 + 2048) = make_float2(acc[ii][0][2], acc[ii][0][3]);
-          *reinterpret_cast<float2 *>(d + st1) = make_float2(acc[ii][1][0], acc[ii][1][1]);
-          *reinterpret_cast<float2 *>(d + st1 + 2048) = make_float2(acc[ii][1][2], acc[ii][1][3]);
-        }
+        for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+          for (int h = 0; h < 2; ++h)
+#pragma unroll
+            for (int c = 0; c < 8; ++c) xst[(8 * h + c) * SKY_TBR + 128 * mt] = acc[mt][h][c];
         __syncthreads();                                         // the rows of detector k are complete; chunk i is consumed
-        if (tid == 0 && i + SKY_SLOTS < n_chunks) issue(i + SKY_SLOTS, cnt + SKY_SLOTS);
-        // ---- shifted read: x_j += P_k[j + r][n], lane = sample: one bank per lane
-        {
-          const int row = ph + resid_s[k * SKY_NB + n_mine];
-          const unsigned char *src = xb + (uint32_t)row * 256u + (uint32_t)((((n_mine >> 3) ^ (row & 7)) << 5) + ((n_mine & 7) << 2));
+        tc_fence_after();
+        if (warp == 0 && i + SKY_SLOTS < n_chunks) {
+          if (elect_one()) issue_tma(i + SKY_SLOTS, cnt + SKY_SLOTS);
+          __syncwarp();
+        }
+        // ---- shifted read: x_j += P_k[j + r][n], lanes = consecutive rows
+#pragma unroll
+        for (int sp = 0; sp < SKY_SPW; ++sp) {
+          const int n = SKY_SPW * warp + sp;
+          const float *src = xb + n * SKY_TBR + resid_s[k * SKY_NB + n] + lane;
           if (k == 0) {
 #pragma unroll
-            for (int e = 0; e < SKY_NE; ++e) x[e] = *reinterpret_cast<const float *>(src + e * 2048);
+            for (int e = 0; e < SKY_NE; ++e) x[sp][e] = src[32 * e];
           } else {
 #pragma unroll
-            for (int e = 0; e < SKY_NE; ++e) x[e] += *reinterpret_cast<const float *>(src + e * 2048);
+            for (int e = 0; e < SKY_NE; ++e) x[sp][e] += src[32 * e];
           }
         }
       }
-      // ---- the block joins the running log-sum-exp of this thread
-      const int j0 = blk * SKY_TBO + ph;
-      float bm = -INFINITY;
+      // ---- the block joins the running log-sum-exp of this lane, per sample
+      const int j0 = blk * SKY_TBO + lane;
 #pragma unroll
-      for (int e = 0; e < SKY_NE; ++e)
-        if (j0 + 8 * e < n_t) bm = fmaxf(bm, x[e]);
-      const float m_new = fmaxf(m_run, bm);
-      float s = s_run * fast_exp2((m_run - m_new) * cl2n);
-      if (m_run == -INFINITY) s = 0.f;
+      for (int sp = 0; sp < SKY_SPW; ++sp) {
+        float bm = -INFINITY;
 #pragma unroll
-      for (int e = 0; e < SKY_NE; ++e)
-        if (j0 + 8 * e < n_t) s += fast_exp2((x[e] - m_new) * cl2n);
-      s_run = s;
-      m_run = m_new;
-    }
-    part_s[ph * SKY_NB + n_mine] = make_float2(m_run, s_run);
-    __syncthreads();
-    if (tid < SKY_NB && orig_s[tid] >= 0) {
-      float m = -INFINITY;
+        for (int e = 0; e < SKY_NE; ++e)
+          if (j0 + 32 * e < n_t) bm = fmaxf(bm, x[sp][e]);
+        const float m_new = fmaxf(m_run[sp], bm);
+        float s = m_run[sp] == -INFINITY ? 0.f : s_run[sp] * fast_exp2((m_run[sp] - m_new) * cl2n[sp]);
 #pragma unroll
-      for (int p8 = 0; p8 < 8; ++p8) m = fmaxf(m, part_s[p8 * SKY_NB + tid].x);
-      const float c2 = cl2_s[tid];
-      float s = 0.f;
-#pragma unroll
-      for (int p8 = 0; p8 < 8; ++p8) {
-        const float2 v = part_s[p8 * SKY_NB + tid];
-        if (v.x > -INFINITY) s += v.y * fast_exp2((v.x - m) * c2);
+        for (int e = 0; e < SKY_NE; ++e)
+          if (j0 + 32 * e < n_t) s += fast_exp2((x[sp][e] - m_new) * cl2n[sp]);
+        s_run[sp] = s;
+        m_run[sp] = m_new;
       }
-      const double c = cval_s[tid];
-      const double inv = 1.0 / ((double)A.qscale[point] * SKY_BSCALE);
-      A.lnL_out[b.g0 + orig_s[tid]] = c * ((double)m * inv) + log((double)s) - ln_ntau - qval_s[tid];
     }
+    // ---- per sample: combine the 32 lanes, write lnL
+#pragma unroll
+    for (int sp = 0; sp < SKY_SPW; ++sp) {
+      const int n = SKY_SPW * warp + sp;
+      const float m = warp_max(m_run[sp]);
+      float s = m_run[sp] == -INFINITY ? 0.f : s_run[sp] * fast_exp2((m_run[sp] - m) * cl2n[sp]);
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+      if (lane == 0 && orig_s[n] >= 0) {
+        const double inv = 1.0 / ((double)A.qscale[point] * SKY_BSCALE);
+        A.lnL_out[b.g0 + orig_s[n]] = cval_s[n] * ((double)m * inv) + log((double)s) - ln_ntau - qval_s[n];
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
   }
 }
 
@@ -282,11 +311,16 @@ __global__ void sky_scale_kernel(const uint32_t *__restrict__ mx, float *__restr
 }
 __global__ void convert_q_sky_kernel(const double2 *__restrict__ src, __half *__restrict__ dst, const float *__restrict__ scale,
                                      SkyPlan p, int64_t total) {
+  // dst: [point][detector][plane = kappa / 8][extended row][kappa % 8]
+  const int npl = p.kp >> 3;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
-    const int kap = (int)(i % p.kp);
-    const int64_t rowi = i / p.kp;
-    const int r = (int)(rowi % p.rows_ext);
-    const int64_t pk = rowi / p.rows_ext;                                  // point * K + detector
+    const int e8 = (int)(i & 7);
+    const int64_t ri = i >> 3;
+    const int r = (int)(ri % p.rows_ext);
+    const int64_t pp = ri / p.rows_ext;
+    const int pl = (int)(pp % npl);
+    const int64_t pk = pp / npl;                                          // point * K + detector
+    const int kap = 8 * pl + e8;
     int t = (r - p.R0) % p.n_t;
     if (t < 0) t += p.n_t;
     const int m2 = 2 * p.M, region = kap / m2;
@@ -298,9 +332,7 @@ __global__ void convert_q_sky_kernel(const double2 *__restrict__ src, __half *__
       const __half hi = __float2half_rn(v);
       h = region == 1 ? __float2half_rn(v - __half2float(hi)) : hi;
     }
-    const int c = kap >> 3;
-    const int pos = (c >> 3) * 64 + (((c & 7) ^ (r & 7)) << 3) + (kap & 7);
-    dst[rowi * p.kp + pos] = h;
+    dst[i] = h;
   }
 }
 
@@ -334,12 +366,7 @@ cudaError_t launch_lnl_sky(const SkyPlan &p, const void *q, const float *qscale,
   a.ws = ws;
   a.n_batches = n_batches_dev;
   a.lnL_out = lnL_out;
-  void (*kern)(SkyArgs) = nullptr;
-  switch (p.ks) {
-    case 4: kern = lnl_sky_kernel<4>; break;
-    case 8: kern = lnl_sky_kernel<8>; break;
-    default: return cudaErrorInvalidValue;
-  }
+  void (*kern)(SkyArgs) = lnl_sky_kernel;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)a.L.total);
   if (e != cudaSuccess) return e;
   int64_t grid = n_sm;
