@@ -388,9 +388,9 @@ void make_sky_plan(rift_ile *h, double delta_t) {
   p.kp = (6 * h->M + 15) & ~15;
   p.ks = p.kp / 16;
   p.rowb = 2 * p.kp;
-  p.R0 = (dm + 7) & ~7;
+  p.R0 = ((dm + 7) & ~7) + 8;                       // a chunk starts at the 8-row group holding its first row
   p.n_blocks = (h->n_t + SKY_TBO - 1) / SKY_TBO;
-  p.rows_ext = p.R0 + (p.n_blocks - 1) * SKY_TBO + dm + SKY_TBR + 8;
+  p.rows_ext = (p.R0 + (p.n_blocks - 1) * SKY_TBO + dm + SKY_TBR + 8 + 7) & ~7;
   p.point_stride = (int64_t)p.K * p.rows_ext * p.rowb;
   if (lnl_sky_smem_bytes(p) > 227u * 1024u) return;
   if (!sky_make_cells(dmax, h->sky_cells)) return;

@@ -5,14 +5,15 @@
 // The samples of a chunk arrive bucketed by sky cell (sky_sort.cu): the 64 samples of a batch have relative shifts
 // d_{n,k} = s_k - s_0 = b_k + r_{n,k} with one base b_k per detector and residuals 0 <= r < SKY_E.  Circular window
 // (N_tau = N_t), detector-0 time: x_j = sum_k P_k[(j + b_k + r_{n,k}) mod N_t, n], P_k[t, n] = sum_kappa A_k[t, kappa] B_k[kappa, n].
-// Time is tiled in blocks of 224 window entries.  Per (block, detector) a chunk of 256 consecutive operand rows starting at
-// row  block start + b_k  of the circularly extended fp16 operand [Q_hi | Q_lo | Q_hi] (K-major planes of 8 elements) arrives
-// by bulk copies into one of three ring slots; one elected thread contracts it with the coefficient operand
+// Time is tiled in blocks of 216 window entries.  Per (block, detector) a chunk of 256 consecutive operand rows starting at
+// row  block start + b_k (rounded down to a multiple of 8: the remainder joins the residuals)  of the circularly extended fp16
+// operand [Q_hi | Q_lo | Q_hi] -- stored as groups of 8 rows x K-major planes of 8 elements, so that a chunk is contiguous --
+// arrives by ONE bulk copy into one of three ring slots; one elected thread contracts it with the coefficient operand
 // [B_hi | B_hi | B_lo] of the batch (reading B8: fp16 pieces, products exact in the fp32 accumulator) by tcgen05.mma, both
 // operands from shared memory, 2 row tiles of 128 x 64 samples x K = 16 per step, accumulators double-buffered in tensor
 // memory so that the tensor core works on chunk i + 1 while the 16 warps drain chunk i: tcgen05.ld (thread = row, 16 samples),
 // unshifted store into an exchange buffer [64 samples][256 rows] (lanes = consecutive rows: conflict-free), barrier, then
-// every warp adds  P_k[j + r_{n,k}][n]  for its 4 samples n and the block's 224 window entries j = lane + 32 e into registers
+// every warp adds  P_k[j + r_{n,k}][n]  for its 4 samples n and the block's 216 window entries j = lane + 32 e into registers
 // (again lanes = consecutive rows, whatever the shifts).  After the last detector the block joins the lane's running
 // (max, sum) of 2^(c log2e (x - max)) per sample -- an on-line log-sum-exp, so the window never exists anywhere as a whole.
 // Nothing but Q rows, 23 KB of coefficients per batch and one lnL per sample moves through L2 / HBM.
@@ -23,7 +24,7 @@
 namespace {
 
 constexpr int SKY_WARPS = 16, SKY_THREADS = SKY_WARPS * 32, SKY_SLOTS = 3;
-constexpr int SKY_NE = SKY_TBO / 32;               // window entries per lane, sample and time block
+constexpr int SKY_NE = (SKY_TBO + 31) / 32;        // window entries per lane, sample and time block
 constexpr int SKY_SPW = SKY_NB / SKY_WARPS;        // samples per warp in the reader role
 constexpr float SKY_BSCALE = 8192.f;               // 2^13: scale of the coefficient operand (|F_k Y_lm| < 2) into the fp16 range
 // instruction descriptor: D fp32, A/B fp16, both K-major, N = 64, M = 128
@@ -47,7 +48,7 @@ __host__ __device__ inline SkySmem sky_smem(const SkyPlan &p) {
   L.bs_det = (uint32_t)(p.kp >> 3) * SKY_NB * 16;
   L.xb = (L.bs + (uint32_t)p.K * L.bs_det + 127u) & ~127u;             // float [64 samples][256 rows]
   L.ring = L.xb + SKY_TBR * SKY_NB * 4;
-  L.slot_bytes = SKY_TBR * (uint32_t)p.rowb;                           // [kp/8 planes][256 rows][8 fp16]
+  L.slot_bytes = SKY_TBR * (uint32_t)p.rowb;                           // [32 groups of 8 rows][kp/8 planes][8 rows][8 fp16]
   L.total = L.ring + SKY_SLOTS * L.slot_bytes;
   return L;
 }
@@ -55,7 +56,7 @@ __host__ __device__ inline SkySmem sky_smem(const SkyPlan &p) {
 struct SkyArgs {
   SkyPlan p;
   SkySmem L;
-  const unsigned char *q;          // [P][K][kp/8 planes][rows_ext][8] fp16
+  const unsigned char *q;          // [P][K][rows_ext / 8][kp/8 planes][8 rows][8] fp16
   const float *qscale;             // [P] power-of-two scale of each point's Q
   Batch b;
   Workspace ws;                    // sorted slots: coef (fp32), scale_c, quad, shift, orig
@@ -157,22 +158,22 @@ __global__ void __launch_bounds__(SKY_THREADS, 1) lnl_sky_kernel(const SkyArgs A
     __syncthreads();
     const int point = bk_s[8];
     if (tid < SKY_NB * K) {
-      int r = my_d == INT32_MAX ? 0 : my_d - bk_s[tid / SKY_NB];
+      const int bkk = bk_s[tid / SKY_NB] == INT32_MAX ? 0 : bk_s[tid / SKY_NB];
+      int r = my_d == INT32_MAX ? 0 : my_d - bkk;
       r = r < 0 ? 0 : (r > SKY_E - 1 ? SKY_E - 1 : r);           // out of range only for a sample with NaN angles
-      resid_s[tid] = r;
+      resid_s[tid] = r + (bkk & 7);                              // the chunk starts at the 8-row group holding b_k
     }
     if (tid < SKY_NB) cl2_s[tid] = (float)(cval_s[tid] * 1.4426950408889634 / ((double)A.qscale[point] * SKY_BSCALE));
     const unsigned char *qpoint = A.q + (int64_t)point * P.point_stride;
-    // chunk i = (block i / K, detector i % K): 256 rows of every plane into ring slot c % 3
+    // chunk i = (block i / K, detector i % K): 32 groups of 8 rows (all planes) into ring slot c % 3, one bulk copy
     auto issue_tma = [&](int i, uint32_t c) {
       const int blk = i / K, k = i - blk * K;
       const int bk = bk_s[k] == INT32_MAX ? 0 : bk_s[k];
-      const int64_t row = P.R0 + blk * SKY_TBO + bk;
+      const int64_t grp = (P.R0 + blk * SKY_TBO + (bk & ~7)) >> 3;          // R0, SKY_TBO are multiples of 8; floor for bk < 0
       const uint32_t slot = c % SKY_SLOTS;
       mbar_expect_tx(full + slot, L.slot_bytes);
-      for (int pl = 0; pl < npl; ++pl)
-        bulk_g2s(ring + slot * L.slot_bytes + pl * (SKY_TBR * 16),
-                 qpoint + (((int64_t)k * npl + pl) * P.rows_ext + row) * 16, SKY_TBR * 16, full + slot);
+      bulk_g2s(ring + slot * L.slot_bytes, qpoint + ((int64_t)k * (P.rows_ext >> 3) + grp) * (int64_t)(npl * 128), L.slot_bytes,
+               full + slot);
     };
     // P_k tiles of chunk i into accumulator buffer c & 1: 2 row tiles x kp / 16 steps
     auto issue_mma = [&](int i, uint32_t c) {
@@ -180,18 +181,20 @@ __global__ void __launch_bounds__(SKY_THREADS, 1) lnl_sky_kernel(const SkyArgs A
       const uint32_t slot = c % SKY_SLOTS;
       mbar_wait(full + slot, (c / SKY_SLOTS) & 1u);
       tc_fence_after();
-      const uint64_t adesc = tc_smem_desc(ring_u32 + slot * L.slot_bytes, SKY_TBR * 16u, 128u);
+      // A: planes of one 8-row group are 128 bytes apart (LBO), groups npl * 128 bytes (SBO); B: [plane][sample][16 bytes]
+      const uint64_t adesc = tc_smem_desc(ring_u32 + slot * L.slot_bytes, 128u, (uint32_t)npl * 128u);
       const uint64_t bdesc = tc_smem_desc(bs_u32 + (uint32_t)k * L.bs_det, SKY_NB * 16u, 128u);
-      for (int s = 0; s < ks; ++s)
-#pragma unroll
-        for (int mt = 0; mt < 2; ++mt)
-          tc_mma_ss(tmem_base + (c & 1u) * 128u + (uint32_t)(mt * SKY_NB),
-                    adesc + (uint64_t)(((uint32_t)(2 * s) * (SKY_TBR * 16u) + (uint32_t)(128 * mt) * 16u) >> 4),
-                    bdesc + (uint64_t)(((uint32_t)(2 * s) * (SKY_NB * 16u)) >> 4), SKY_IDESC, s > 0 ? 1u : 0u);
+      const uint32_t d0 = tmem_base + (c & 1u) * 128u;
+      for (int s = 0; s < ks; ++s) {
+        const uint64_t bd = bdesc + (uint64_t)((uint32_t)(2 * s) * (SKY_NB * 16u) >> 4);
+        const uint64_t ad = adesc + (uint64_t)((uint32_t)(2 * s) * 128u >> 4);
+        tc_mma_ss(d0, ad, bd, SKY_IDESC, s > 0 ? 1u : 0u);
+        tc_mma_ss(d0 + SKY_NB, ad + (uint64_t)((16u * (uint32_t)npl * 128u) >> 4), bd, SKY_IDESC, s > 0 ? 1u : 0u);
+      }
       tc_commit(tfull + (c & 1u));
     };
-    if (warp == 0) {
-      if (elect_one()) {
+    if (warp == 0) {                                             // bulk copies and tensor-core instructions come from warp 0 here,
+      if (elect_one()) {                                         // in the loop from two different warps
         for (int i = 0; i < SKY_SLOTS && i < n_chunks; ++i) issue_tma(i, cnt + i);
         issue_mma(0, cnt);
       }
@@ -240,7 +243,7 @@ __global__ void __launch_bounds__(SKY_THREADS, 1) lnl_sky_kernel(const SkyArgs A
             for (int c = 0; c < 8; ++c) xst[(8 * h + c) * SKY_TBR + 128 * mt] = acc[mt][h][c];
         __syncthreads();                                         // the rows of detector k are complete; chunk i is consumed
         tc_fence_after();
-        if (warp == 0 && i + SKY_SLOTS < n_chunks) {
+        if (warp == 5 && i + SKY_SLOTS < n_chunks) {
           if (elect_one()) issue_tma(i + SKY_SLOTS, cnt + SKY_SLOTS);
           __syncwarp();
         }
@@ -260,17 +263,18 @@ __global__ void __launch_bounds__(SKY_THREADS, 1) lnl_sky_kernel(const SkyArgs A
       }
       // ---- the block joins the running log-sum-exp of this lane, per sample
       const int j0 = blk * SKY_TBO + lane;
+      const int j_end = min(n_t, (blk + 1) * SKY_TBO);
 #pragma unroll
       for (int sp = 0; sp < SKY_SPW; ++sp) {
         float bm = -INFINITY;
 #pragma unroll
         for (int e = 0; e < SKY_NE; ++e)
-          if (j0 + 32 * e < n_t) bm = fmaxf(bm, x[sp][e]);
+          if (j0 + 32 * e < j_end) bm = fmaxf(bm, x[sp][e]);
         const float m_new = fmaxf(m_run[sp], bm);
         float s = m_run[sp] == -INFINITY ? 0.f : s_run[sp] * fast_exp2((m_run[sp] - m_new) * cl2n[sp]);
 #pragma unroll
         for (int e = 0; e < SKY_NE; ++e)
-          if (j0 + 32 * e < n_t) s += fast_exp2((x[sp][e] - m_new) * cl2n[sp]);
+          if (j0 + 32 * e < j_end) s += fast_exp2((x[sp][e] - m_new) * cl2n[sp]);
         s_run[sp] = s;
         m_run[sp] = m_new;
       }
@@ -311,15 +315,15 @@ __global__ void sky_scale_kernel(const uint32_t *__restrict__ mx, float *__restr
 }
 __global__ void convert_q_sky_kernel(const double2 *__restrict__ src, __half *__restrict__ dst, const float *__restrict__ scale,
                                      SkyPlan p, int64_t total) {
-  // dst: [point][detector][plane = kappa / 8][extended row][kappa % 8]
+  // dst: [point][detector][group = extended row / 8][plane = kappa / 8][row % 8][kappa % 8]
   const int npl = p.kp >> 3;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
-    const int e8 = (int)(i & 7);
-    const int64_t ri = i >> 3;
-    const int r = (int)(ri % p.rows_ext);
-    const int64_t pp = ri / p.rows_ext;
-    const int pl = (int)(pp % npl);
-    const int64_t pk = pp / npl;                                          // point * K + detector
+    const int e8 = (int)(i & 7), r8 = (int)((i >> 3) & 7);
+    const int64_t gi = i >> 6;
+    const int pl = (int)(gi % npl);
+    const int64_t gg = gi / npl;
+    const int r = (int)(gg % (p.rows_ext >> 3)) * 8 + r8;
+    const int64_t pk = gg / (p.rows_ext >> 3);                             // point * K + detector
     const int kap = 8 * pl + e8;
     int t = (r - p.R0) % p.n_t;
     if (t < 0) t += p.n_t;

@@ -132,8 +132,8 @@ struct MmaPlan {
 // Sky-sorted, time-tiled tensor-core path (sky_sort.cu, lnl_sky.cu): mixed precision, windows of any length.
 #define SKY_NB 64                // samples per batch (eight 8-column tiles)
 #define SKY_E 32                 // residual shifts of a batch lie in [0, SKY_E)
-#define SKY_TBO 224              // window entries per time block
-#define SKY_TBR 256              // Q rows per (time block, detector) chunk = SKY_TBO + SKY_E
+#define SKY_TBO 216              // window entries per time block (a multiple of 8)
+#define SKY_TBR 256              // Q rows per (time block, detector) chunk >= SKY_TBO + SKY_E + 7
 #define SKY_MAX_RINGS 512
 struct SkyCells {                // sky cells of the bucketing pass (sky_sort.cu)
   double delta;                  // ring width (rad)
