@@ -36,8 +36,8 @@ struct SkySmem {                                   // byte offsets inside dynami
 
 __host__ __device__ inline SkySmem sky_smem(const SkyPlan &p) {
   SkySmem L;
-  L.bars = 0;                                                          // full[3], tfull[2]
-  L.tmem = 48;
+  L.bars = 0;                                                          // full[3], tfull[2], tempty[2]
+  L.tmem = 56;
   L.cl2 = 64;                                                          // float [64]
   L.cval = L.cl2 + SKY_NB * 4;                                         // double [64] c = D_ref / D
   L.qval = L.cval + SKY_NB * 8;                                        // double [64] q
@@ -71,7 +71,8 @@ __global__ void __launch_bounds__(SKY_THREADS, 1) lnl_sky_kernel(const SkyArgs A
   const Batch &b = A.b;
   const Workspace &ws = A.ws;
   uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + L.bars);
-  uint64_t *tfull = full + SKY_SLOTS;
+  uint64_t *tfull = full + SKY_SLOTS;                            // accumulators of a chunk ready (tcgen05.commit)
+  uint64_t *tempty = tfull + 2;                                  // accumulator buffer drained by all 16 warps
   uint32_t *tmem_ptr_s = reinterpret_cast<uint32_t *>(smem_raw + L.tmem);
   float *cl2_s = reinterpret_cast<float *>(smem_raw + L.cl2);
   double *cval_s = reinterpret_cast<double *>(smem_raw + L.cval);
@@ -89,6 +90,8 @@ __global__ void __launch_bounds__(SKY_THREADS, 1) lnl_sky_kernel(const SkyArgs A
     for (int i = 0; i < SKY_SLOTS; ++i) mbar_init(full + i, 1);
     mbar_init(tfull, 1);
     mbar_init(tfull + 1, 1);
+    mbar_init(tempty, SKY_WARPS);
+    mbar_init(tempty + 1, SKY_WARPS);
   }
   if (warp == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_ptr_s)) : "memory");
@@ -99,8 +102,11 @@ __global__ void __launch_bounds__(SKY_THREADS, 1) lnl_sky_kernel(const SkyArgs A
   tc_fence_after();
   const uint32_t tmem_base = *tmem_ptr_s;
 
+  // Two groups of 8 warps own the sample halves 0-31 / 32-63 of the batch (their columns of the accumulators, their half of
+  // the exchange buffer) and synchronise among themselves only: one group drains while the other reads.
   // drain role: tensor-memory lanes 32 (warp & 3) .. + 31 (rows of a 128-row tile), columns 16 (warp >> 2) .. + 15 (samples)
-  const int q4 = warp & 3, cg = warp >> 2;
+  const int q4 = warp & 3, cg = warp >> 2, grp = warp >> 3;
+  auto group_bar = [&]() { named_bar_sync(1 + grp, 8 * 32); };
   const uint32_t t_lane = ((uint32_t)(32 * q4)) << 16;
   float *xst = xb + (size_t)(16 * cg) * SKY_TBR + 32 * q4 + lane;        // + c * 256 (sample) + 128 mt (row tile)
   // reader role: samples SKY_SPW warp .. + 3, window entries lane + 32 e of the block
@@ -180,6 +186,7 @@ __global__ void __launch_bounds__(SKY_THREADS, 1) lnl_sky_kernel(const SkyArgs A
       const int k = i % K;
       const uint32_t slot = c % SKY_SLOTS;
       mbar_wait(full + slot, (c / SKY_SLOTS) & 1u);
+      mbar_wait(tempty + (c & 1u), ((c >> 1) & 1u) ^ 1u);         // both groups have drained the chunk before last
       tc_fence_after();
       // A: planes of one 8-row group are 128 bytes apart (LBO), groups npl * 128 bytes (SBO); B: [plane][sample][16 bytes]
       const uint64_t adesc = tc_smem_desc(ring_u32 + slot * L.slot_bytes, 128u, (uint32_t)npl * 128u);
@@ -234,16 +241,18 @@ __global__ void __launch_bounds__(SKY_THREADS, 1) lnl_sky_kernel(const SkyArgs A
           tc_wait_ld8(acc[mt][1]);
         }
         tc_fence_before();
-        __syncthreads();                                         // every reader is done with the previous detector's rows
+        __syncwarp();
+        if (lane == 0) mbar_arrive(tempty + (cnt & 1u));
+        group_bar();                                             // every reader of the group is done with the previous detector
 #pragma unroll
         for (int mt = 0; mt < 2; ++mt)
 #pragma unroll
           for (int h = 0; h < 2; ++h)
 #pragma unroll
             for (int c = 0; c < 8; ++c) xst[(8 * h + c) * SKY_TBR + 128 * mt] = acc[mt][h][c];
-        __syncthreads();                                         // the rows of detector k are complete; chunk i is consumed
+        group_bar();                                             // the group's rows of detector k are complete
         tc_fence_after();
-        if (warp == 5 && i + SKY_SLOTS < n_chunks) {
+        if (warp == 13 && i + SKY_SLOTS < n_chunks) {             // tfull of chunk i was observed: its ring slot is free
           if (elect_one()) issue_tma(i + SKY_SLOTS, cnt + SKY_SLOTS);
           __syncwarp();
         }
