@@ -365,8 +365,8 @@ void make_mma_plan(rift_ile *h, double delta_t) {
   p.ok = 0;
 }
 
-// mixed mode, circular window: plan of the sky-sorted kernel (any window length; up to 10 modes for now: one 128-byte
-// operand row per sample of Q)
+// mixed mode, circular window: plan of the sky-sorted kernel (any window length; the operand row [Q_hi | Q_lo | Q_hi] of
+// 6 M fp16 elements is cut into K pieces of at most 64 elements, one ring slot each)
 void make_sky_plan(rift_ile *h, double delta_t) {
   SkyPlan &p = h->sky;
   p = SkyPlan{};
@@ -385,8 +385,9 @@ void make_sky_plan(rift_ile *h, double delta_t) {
   p.K = h->K;
   p.M = h->M;
   p.n_t = h->n_t;
-  p.kp = (6 * h->M + 15) & ~15;
-  p.ks = p.kp / 16;
+  p.n_pc = (6 * h->M + 63) / 64;
+  p.ppp = 2 * ((6 * h->M + 16 * p.n_pc - 1) / (16 * p.n_pc));
+  p.kp = 8 * p.n_pc * p.ppp;
   p.rowb = 2 * p.kp;
   p.R0 = ((dm + 7) & ~7) + 8;                       // a chunk starts at the 8-row group holding its first row
   p.n_blocks = (h->n_t + SKY_TBO - 1) / SKY_TBO;

@@ -48,7 +48,7 @@ __host__ __device__ inline SkySmem sky_smem(const SkyPlan &p) {
   L.bs_det = (uint32_t)(p.kp >> 3) * SKY_NB * 16;
   L.xb = (L.bs + (uint32_t)p.K * L.bs_det + 127u) & ~127u;             // float [64 samples][256 rows]
   L.ring = L.xb + SKY_TBR * SKY_NB * 4;
-  L.slot_bytes = SKY_TBR * (uint32_t)p.rowb;                           // [32 groups of 8 rows][kp/8 planes][8 rows][8 fp16]
+  L.slot_bytes = SKY_TBR * (uint32_t)p.ppp * 16;                       // one K piece: [32 groups of 8 rows][ppp planes][8 rows][8 fp16]
   L.total = L.ring + SKY_SLOTS * L.slot_bytes;
   return L;
 }
@@ -56,7 +56,7 @@ __host__ __device__ inline SkySmem sky_smem(const SkyPlan &p) {
 struct SkyArgs {
   SkyPlan p;
   SkySmem L;
-  const unsigned char *q;          // [P][K][rows_ext / 8][kp/8 planes][8 rows][8] fp16
+  const unsigned char *q;          // [P][K][n_pc pieces][rows_ext / 8][ppp planes][8 rows][8] fp16
   const float *qscale;             // [P] power-of-two scale of each point's Q
   Batch b;
   Workspace ws;                    // sorted slots: coef (fp32), scale_c, quad, shift, orig
@@ -64,6 +64,8 @@ struct SkyArgs {
   double *lnL_out;
 };
 
+// NPC, PPP: K pieces per chunk and planes per piece at compile time (0: read from the plan)
+template <int NPC, int PPP>
 __global__ void __launch_bounds__(SKY_THREADS, 1) lnl_sky_kernel(const SkyArgs A) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const SkyPlan &P = A.p;
@@ -85,7 +87,8 @@ __global__ void __launch_bounds__(SKY_THREADS, 1) lnl_sky_kernel(const SkyArgs A
   unsigned char *ring = smem_raw + L.ring;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int K = P.K, n_t = P.n_t, m2 = 2 * P.M, npl = P.kp >> 3, ks = P.kp >> 4;
+  const int n_pc = NPC ? NPC : P.n_pc, ppp = PPP ? PPP : P.ppp;
+  const int K = P.K, n_t = P.n_t, m2 = 2 * P.M, npl = n_pc * ppp;
   if (tid == 0) {
     for (int i = 0; i < SKY_SLOTS; ++i) mbar_init(full + i, 1);
     mbar_init(tfull, 1);
@@ -171,38 +174,44 @@ __global__ void __launch_bounds__(SKY_THREADS, 1) lnl_sky_kernel(const SkyArgs A
     }
     if (tid < SKY_NB) cl2_s[tid] = (float)(cval_s[tid] * 1.4426950408889634 / ((double)A.qscale[point] * SKY_BSCALE));
     const unsigned char *qpoint = A.q + (int64_t)point * P.point_stride;
-    // chunk i = (block i / K, detector i % K): 32 groups of 8 rows (all planes) into ring slot c % 3, one bulk copy
-    auto issue_tma = [&](int i, uint32_t c) {
+    // ring entry e = (chunk e / n_pc = (block, detector), K piece e % n_pc): 32 groups of 8 rows x ppp planes, one bulk copy
+    // into ring slot re % 3 (re = the entry's running number)
+    auto issue_tma = [&](int e, uint32_t re) {
+      const int i = e / n_pc, pc = e - i * n_pc;
       const int blk = i / K, k = i - blk * K;
       const int bk = bk_s[k] == INT32_MAX ? 0 : bk_s[k];
       const int64_t grp = (P.R0 + blk * SKY_TBO + (bk & ~7)) >> 3;          // R0, SKY_TBO are multiples of 8; floor for bk < 0
-      const uint32_t slot = c % SKY_SLOTS;
+      const uint32_t slot = re % SKY_SLOTS;
       mbar_expect_tx(full + slot, L.slot_bytes);
-      bulk_g2s(ring + slot * L.slot_bytes, qpoint + ((int64_t)k * (P.rows_ext >> 3) + grp) * (int64_t)(npl * 128), L.slot_bytes,
-               full + slot);
+      bulk_g2s(ring + slot * L.slot_bytes,
+               qpoint + (((int64_t)k * n_pc + pc) * (P.rows_ext >> 3) + grp) * (int64_t)(ppp * 128), L.slot_bytes, full + slot);
     };
     // P_k tiles of chunk i into accumulator buffer c & 1: 2 row tiles x kp / 16 steps
     auto issue_mma = [&](int i, uint32_t c) {
       const int k = i % K;
-      const uint32_t slot = c % SKY_SLOTS;
-      mbar_wait(full + slot, (c / SKY_SLOTS) & 1u);
       mbar_wait(tempty + (c & 1u), ((c >> 1) & 1u) ^ 1u);         // both groups have drained the chunk before last
-      tc_fence_after();
-      // A: planes of one 8-row group are 128 bytes apart (LBO), groups npl * 128 bytes (SBO); B: [plane][sample][16 bytes]
-      const uint64_t adesc = tc_smem_desc(ring_u32 + slot * L.slot_bytes, 128u, (uint32_t)npl * 128u);
-      const uint64_t bdesc = tc_smem_desc(bs_u32 + (uint32_t)k * L.bs_det, SKY_NB * 16u, 128u);
       const uint32_t d0 = tmem_base + (c & 1u) * 128u;
-      for (int s = 0; s < ks; ++s) {
-        const uint64_t bd = bdesc + (uint64_t)((uint32_t)(2 * s) * (SKY_NB * 16u) >> 4);
-        const uint64_t ad = adesc + (uint64_t)((uint32_t)(2 * s) * 128u >> 4);
-        tc_mma_ss(d0, ad, bd, SKY_IDESC, s > 0 ? 1u : 0u);
-        tc_mma_ss(d0 + SKY_NB, ad + (uint64_t)((16u * (uint32_t)npl * 128u) >> 4), bd, SKY_IDESC, s > 0 ? 1u : 0u);
+      for (int pc = 0; pc < n_pc; ++pc) {
+        const uint32_t re = c * (uint32_t)n_pc + (uint32_t)pc, slot = re % SKY_SLOTS;
+        mbar_wait(full + slot, (re / SKY_SLOTS) & 1u);
+        tc_fence_after();
+        // A: planes of one 8-row group are 128 bytes apart (LBO), groups ppp * 128 bytes (SBO); B: [plane][sample][16 bytes]
+        const uint64_t adesc = tc_smem_desc(ring_u32 + slot * L.slot_bytes, 128u, (uint32_t)ppp * 128u);
+        const uint64_t bdesc = tc_smem_desc(bs_u32 + (uint32_t)k * L.bs_det + (uint32_t)(pc * ppp) * (SKY_NB * 16u), SKY_NB * 16u, 128u);
+        for (int s = 0; 2 * s < ppp; ++s) {
+          const uint64_t bd = bdesc + (uint64_t)((uint32_t)(2 * s) * (SKY_NB * 16u) >> 4);
+          const uint64_t ad = adesc + (uint64_t)((uint32_t)(2 * s) * 128u >> 4);
+          const uint32_t accum = (pc > 0 || s > 0) ? 1u : 0u;
+          tc_mma_ss(d0, ad, bd, SKY_IDESC, accum);
+          tc_mma_ss(d0 + SKY_NB, ad + (uint64_t)((16u * (uint32_t)ppp * 128u) >> 4), bd, SKY_IDESC, accum);
+        }
       }
       tc_commit(tfull + (c & 1u));
     };
+    const int n_entries = n_chunks * n_pc;
     if (warp == 0) {                                             // bulk copies and tensor-core instructions come from warp 0 here,
       if (elect_one()) {                                         // in the loop from two different warps
-        for (int i = 0; i < SKY_SLOTS && i < n_chunks; ++i) issue_tma(i, cnt + i);
+        for (int e = 0; e < SKY_SLOTS && e < n_entries; ++e) issue_tma(e, cnt * (uint32_t)n_pc + (uint32_t)e);
         issue_mma(0, cnt);
       }
       __syncwarp();
@@ -252,8 +261,12 @@ __global__ void __launch_bounds__(SKY_THREADS, 1) lnl_sky_kernel(const SkyArgs A
             for (int c = 0; c < 8; ++c) xst[(8 * h + c) * SKY_TBR + 128 * mt] = acc[mt][h][c];
         group_bar();                                             // the group's rows of detector k are complete
         tc_fence_after();
-        if (warp == 13 && i + SKY_SLOTS < n_chunks) {             // tfull of chunk i was observed: its ring slot is free
-          if (elect_one()) issue_tma(i + SKY_SLOTS, cnt + SKY_SLOTS);
+        if (warp == 13) {                                        // tfull of chunk i was observed: its ring slots are free
+          if (elect_one())
+            for (int pc = 0; pc < n_pc; ++pc) {
+              const int e = i * n_pc + pc + SKY_SLOTS;
+              if (e < n_entries) issue_tma(e, cnt * (uint32_t)n_pc + (uint32_t)(pc + SKY_SLOTS));
+            }
           __syncwarp();
         }
         // ---- shifted read: x_j += P_k[j + r][n], lanes = consecutive rows
@@ -324,16 +337,17 @@ __global__ void sky_scale_kernel(const uint32_t *__restrict__ mx, float *__restr
 }
 __global__ void convert_q_sky_kernel(const double2 *__restrict__ src, __half *__restrict__ dst, const float *__restrict__ scale,
                                      SkyPlan p, int64_t total) {
-  // dst: [point][detector][group = extended row / 8][plane = kappa / 8][row % 8][kappa % 8]
-  const int npl = p.kp >> 3;
+  // dst: [point][detector][K piece][group = extended row / 8][plane of the piece][row % 8][kappa % 8]
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
     const int e8 = (int)(i & 7), r8 = (int)((i >> 3) & 7);
     const int64_t gi = i >> 6;
-    const int pl = (int)(gi % npl);
-    const int64_t gg = gi / npl;
+    const int pl = (int)(gi % p.ppp);
+    const int64_t gg = gi / p.ppp;
     const int r = (int)(gg % (p.rows_ext >> 3)) * 8 + r8;
-    const int64_t pk = gg / (p.rows_ext >> 3);                             // point * K + detector
-    const int kap = 8 * pl + e8;
+    const int64_t pp = gg / (p.rows_ext >> 3);
+    const int pc = (int)(pp % p.n_pc);
+    const int64_t pk = pp / p.n_pc;                                        // point * K + detector
+    const int kap = 8 * (pc * p.ppp + pl) + e8;
     int t = (r - p.R0) % p.n_t;
     if (t < 0) t += p.n_t;
     const int m2 = 2 * p.M, region = kap / m2;
@@ -379,7 +393,10 @@ cudaError_t launch_lnl_sky(const SkyPlan &p, const void *q, const float *qscale,
   a.ws = ws;
   a.n_batches = n_batches_dev;
   a.lnL_out = lnL_out;
-  void (*kern)(SkyArgs) = lnl_sky_kernel;
+  void (*kern)(SkyArgs) = lnl_sky_kernel<0, 0>;
+  if (p.n_pc == 1 && p.ppp == 8) kern = lnl_sky_kernel<1, 8>;        // 9-10 modes (C4)
+  else if (p.n_pc == 2 && p.ppp == 8) kern = lnl_sky_kernel<2, 8>;   // 20-21 modes (C2)
+  else if (p.n_pc == 1 && p.ppp == 4) kern = lnl_sky_kernel<1, 4>;   // 5 modes (C1, C3)
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)a.L.total);
   if (e != cudaSuccess) return e;
   int64_t grid = n_sm;

@@ -143,7 +143,8 @@ struct SkyCells {                // sky cells of the bucketing pass (sky_sort.cu
 struct SkyPlan {
   int32_t ok;
   int32_t K, M, n_t;
-  int32_t kp, ks, rowb;          // fp16 elements per operand row [Q_hi | Q_lo | Q_hi] (multiple of 64), k-steps of 16, bytes
+  int32_t kp, rowb;              // fp16 elements per operand row [Q_hi | Q_lo | Q_hi] (padded), bytes per row
+  int32_t n_pc, ppp;             // the row is cut into n_pc K pieces of ppp planes of 8 elements (ppp even, <= 8): kp = 8 n_pc ppp
   int32_t R0, rows_ext;          // extended row of original row 0; rows per (point, detector): row e holds (e - R0) mod n_t
   int32_t n_blocks;              // time blocks of SKY_TBO window entries
   int64_t point_stride;          // bytes per intrinsic point: K * rows_ext * rowb

@@ -254,13 +254,16 @@ def test_tc_kernel_shapes(torch, oracle, shape, kernel):
     rift.rift_ile_destroy(h)
 
 
-@pytest.mark.parametrize("shape", ["c4", "c1", "k1", "k2_512hz"])
+@pytest.mark.parametrize("shape", ["c4", "c1", "c2", "m12", "k1", "k2_512hz"])
 def test_sky_kernel_shapes(torch, oracle, shape):
     """Sky-sorted, time-tiled kernel (mixed mode) on request: the C4 shape (5 detectors, 9 modes, 3277-sample window = 15 time
-    blocks), the C1 shape (two blocks), one detector (no shifts at all), two detectors at 512 Hz (a handful of sky cells);
+    blocks), the C1 shape (two blocks), 21 and 12 modes (operand rows cut into two K pieces), one detector (no shifts at
+    all), two detectors at 512 Hz (a handful of sky cells);
     three segments with repeated intrinsic ids, sample counts far below a cell's batch (mostly padding slots), a NaN sample."""
     cfg = {"c4": synth.with_overrides(synth.CONFIGS[4], n_points=2),
            "c1": synth.with_overrides(synth.CONFIGS[1], n_points=2),
+           "c2": synth.with_overrides(synth.CONFIGS[2], n_points=2),                      # 21 modes: two K pieces per chunk
+           "m12": synth.with_overrides(synth.CONFIGS[1], modes=_L2 + _L3, n_points=2),    # 12 modes: two pieces of 6 planes
            "k1": synth.with_overrides(synth.CONFIGS[1], detectors=("V1",), n_points=2),
            "k2_512hz": synth.with_overrides(synth.CONFIGS[0], f_s=512.0, t_window=0.5, n_points=2)}[shape]
     inp = build(oracle, cfg, n_points=2)
