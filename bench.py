@@ -38,6 +38,7 @@ UNIT = "evals/s"
 HEADLINE = (4, "mixed")                            # the largest single-GPU config of BASELINE.json
 N_SM, FP32_LANES, FP64_LANES = 148, 128, 64        # B200: guide unit counts (B200_PROFILING.md, B300_MICROARCH.md)
 EVIDENCE = os.path.join(ROOT, "profiles", "r2_roofline_evidence.json")
+KERNEL_OVERRIDE = None                             # --kernel (A/B runs of one row): a RIFT_KERNEL_* value
 
 
 def measured_peaks() -> dict:
@@ -238,6 +239,8 @@ def bench_row(rift, torch, dist_util, data: ConfigData, precision: str, steps, w
     ids = list(range(P))
     stream = torch.cuda.current_stream().cuda_stream
     n_bins = 100
+    if KERNEL_OVERRIDE is not None:
+        rift.rift_ile_set_kernel(h, KERNEL_OVERRIDE)
     rift.rift_ile_reserve(h, P, N, n_bins)
 
     def step_resident():
@@ -511,7 +514,12 @@ def main() -> None:
     ap.add_argument("--points", type=int, default=0, help="override the number of intrinsic points (debug)")
     ap.add_argument("--samples", type=int, default=0, help="override samples per point (debug)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--kernel", default=None, choices=[None, "auto", "direct", "tc", "tcs", "mma", "sky"],
+                    help="force a fused-kernel variant (A/B runs with --config)")
     args = ap.parse_args()
+    if args.kernel:
+        global KERNEL_OVERRIDE
+        KERNEL_OVERRIDE = {"auto": 0, "direct": 1, "tc": 2, "tcs": 3, "mma": 4, "sky": 5}[args.kernel]
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)

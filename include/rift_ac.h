@@ -26,7 +26,8 @@ extern "C" {
 
 typedef struct rift_ac rift_ac_t;   /* opaque */
 
-/* n_dim dimensions (1..16) with n_bins bins (1..1024) over [lo[d], hi[d]) (HOST arrays, hi > lo); the bin masses start
+/* n_dim dimensions (1..16) with n_bins bins (1..1024, and 16 n_dim n_bins + 16 n_dim <= 200 KiB: the draw kernel stages the
+ * table in shared memory; else RIFT_EINVAL) over [lo[d], hi[d]) (HOST arrays, hi > lo); the bin masses start
  * uniform. */
 int rift_ac_create(int32_t n_dim, int32_t n_bins, const double *lo, const double *hi, rift_ac_t **out);
 

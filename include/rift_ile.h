@@ -90,9 +90,12 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out);
  *                          dist <= 0 or a NaN parameter gives NaN for that sample only.
  *   shift_out            : DEVICE int32 [n_seg*n_per_seg][n_det] or NULL: s_k = floor(dt_k/delta_t + 1/2) (G4).
  *   cuda_stream          : a cudaStream_t (NULL = legacy default stream).  Asynchronous on that stream.
- * Stream capture: the first call of a given size grows the handle's workspace (cudaMalloc) and a new id list is
- * copied to the device; a repeated call with the same sizes, ids and stream issues kernel launches only and may
- * be captured into a CUDA graph (the graph then reads params and writes lnL_out / shift_out at replay). */
+ * Stream capture: the first call of a given size grows the handle's workspace (cudaMalloc; rift_ile_reserve does it ahead
+ * of time) and a new id list is copied to the device; a repeated call with the same sizes, ids and stream issues kernel
+ * launches only and may be captured into a CUDA graph (the graph then reads params and writes lnL_out / shift_out at
+ * replay).  A captured graph points at the handle's id list and workspaces: it is INVALID after any later call on the
+ * handle with other ids, a larger size, another kernel variant or option, rift_ile_reserve, or rift_ile_destroy -- capture
+ * again after such a call (nothing detects a stale replay). */
 int rift_ile_eval_batch(rift_ile_t *h, int32_t n_seg, const int32_t *intrinsic_ids, int64_t n_per_seg,
                         const double *const params[RIFT_N_PARAMS], double *lnL_out, int32_t *shift_out,
                         void *cuda_stream);

@@ -52,6 +52,9 @@ ac_draw_kernel(int n_dim, int n_bins, const double *__restrict__ tab, double *co
       const int m = (a + b + 1) >> 1;
       if (c[m] <= u) a = m; else b = m - 1;
     }
+    // the masses sum to 1 only up to rounding: a draw past the last positive-mass bin (or into a bin emptied by floor = 0)
+    // steps back to the nearest bin that can be drawn, so that ln p_s stays finite
+    while (a > 0 && !(mass[d * n_bins + a] > 0.0)) --a;
     const double ms = mass[d * n_bins + a];
     const double w = __ddiv_rn(__dsub_rn(hi[d], lo[d]), (double)n_bins);
     double frac = __ddiv_rn(__dsub_rn(u, c[a]), ms);
@@ -104,6 +107,7 @@ extern "C" {
 
 int rift_ac_create(int32_t n_dim, int32_t n_bins, const double *lo, const double *hi, rift_ac_t **out) {
   if (!out || !lo || !hi || n_dim < 1 || n_dim > AC_MAX_DIM || n_bins < 1 || n_bins > 1024) return RIFT_EINVAL;
+  if (((size_t)2 * n_dim * n_bins + 2 * n_dim) * sizeof(double) > 200u * 1024u) return RIFT_EINVAL;   // the draw kernel's table
   for (int d = 0; d < n_dim; ++d)
     if (!(hi[d] > lo[d]) || !std::isfinite(lo[d]) || !std::isfinite(hi[d])) return RIFT_EINVAL;
   rift_ac *h = new (std::nothrow) rift_ac();

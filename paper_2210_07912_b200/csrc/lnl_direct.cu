@@ -178,12 +178,12 @@ lnl_direct_kernel(QStore q, Batch b, Workspace ws, int K, double *__restrict__ l
           const float cl2 = (float)c * 1.4426950408889634f;
           float s = 0.f;
 #pragma unroll
-          for (int i = 0; i < SLOTS; ++i) s += fast_exp2(((float)x[i] - (float)bmax) * cl2);
+          for (int i = 0; i < SLOTS; ++i) s += x[i] == -INFINITY ? 0.f : fast_exp2(((float)x[i] - (float)bmax) * cl2);   // masked slot: 0 even when c = 0
           bsum = (double)s;
         } else {
           double s = 0.0;
 #pragma unroll
-          for (int i = 0; i < SLOTS; ++i) s += exp(c * ((double)x[i] - (double)bmax));
+          for (int i = 0; i < SLOTS; ++i) s += x[i] == -INFINITY ? 0.0 : exp(c * ((double)x[i] - (double)bmax));
           bsum = s;
         }
         bsum = warp_sum(bsum);

@@ -161,14 +161,14 @@ lnl_direct_ext_kernel(QStore q, Batch b, Workspace ws, int K, double *__restrict
           float s0 = 0.f, s1 = 0.f;
 #pragma unroll
           for (int i = 0; i < SLOTS; ++i) {
-            const float e = fast_exp2(fmaf((float)x[i], cl2, -off));
+            const float e = x[i] == -INFINITY ? 0.f : fast_exp2(fmaf((float)x[i], cl2, -off));   // masked slot: 0 even when c = 0
             if (i & 1) s1 += e; else s0 += e;
           }
           bsum = (double)(s0 + s1);
         } else {
           double s = 0.0;
 #pragma unroll
-          for (int i = 0; i < SLOTS; ++i) s += exp(c * ((double)x[i] - (double)bmax));
+          for (int i = 0; i < SLOTS; ++i) s += x[i] == -INFINITY ? 0.0 : exp(c * ((double)x[i] - (double)bmax));
           bsum = s;
         }
         bsum = warp_sum(bsum);

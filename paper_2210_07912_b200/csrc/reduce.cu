@@ -245,6 +245,10 @@ cudaError_t launch_reduce(int32_t n_seg, int64_t n_per_seg, const double *lnL, c
   }
   const int nb = hp ? n_bins : 0;
   const size_t smem = (8 + 6 * (size_t)nb) * sizeof(double);
+  if (smem > 48u * 1024u) {            // 1023-1024 bins: 64 + 48 n_bins bytes pass the default dynamic limit
+    cudaError_t ea = cudaFuncSetAttribute(reduce_partial_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (ea != cudaSuccess) return ea;
+  }
   dim3 grid(blocks_per_seg, n_seg);
   reduce_partial_kernel<<<grid, RED_THREADS, smem, s>>>(n_per_seg, lnL, ln_w, ha, hp ? 1 : 0, nb, partial);
   cudaError_t e = cudaGetLastError();
