@@ -27,6 +27,8 @@ struct rift_ile {
   MmaPlan mma{};                   // fp64 tensor-core path (lnl_mma.cu); mma.ok == 0 when the configuration does not fit
   void *d_Qm = nullptr;            // its Q operand: [P][K][2 KS][pitch_q] bytes
   SkyPlan sky{};                   // sky-sorted, time-tiled tensor-core path (lnl_sky.cu); sky.ok == 0: does not apply
+  Sky64Plan sky64{};               // its fp64 sibling (lnl_sky64.cu)
+  void *d_Qsky64 = nullptr;        // [P][K][rows_ext][kp] doubles
   SkyCells sky_cells{};
   void *d_Qsky = nullptr;          // its Q operand: [P][K][rows_ext][kp] fp16
   float *d_qscale_sky = nullptr;   // [P]
@@ -190,6 +192,7 @@ void free_handle(rift_ile *h) {
   cudaFree(h->d_Qtc);
   cudaFree(h->d_Qm);
   cudaFree(h->d_Qsky);
+  cudaFree(h->d_Qsky64);
   cudaFree(h->d_qscale_sky);
   cudaFree(h->sky_buf);
   cudaFree(h->sky_orig);
@@ -398,9 +401,49 @@ void make_sky_plan(rift_ile *h, double delta_t) {
   p.ok = 1;
 }
 
+// fp64 mode, circular window: plan of lnl_sky64 (windows of any length; up to ~10 modes: three 256-row chunks of fp64 rows)
+void make_sky64_plan(rift_ile *h, double delta_t) {
+  Sky64Plan &p = h->sky64;
+  p = Sky64Plan{};
+  if (h->precision != RIFT_PREC_FP64 || h->n_tau != h->n_t || h->K > 8) return;
+  double dmax = 0;
+  for (int k = 1; k < h->K; ++k) {
+    double d2 = 0;
+    for (int i = 0; i < 3; ++i) {
+      const double d = h->geom.loc[k][i] - h->geom.loc[0][i];
+      d2 += d * d;
+    }
+    dmax = std::max(dmax, std::sqrt(d2) / (RIFT_C_LIGHT * delta_t));
+  }
+  if (dmax > 1e5) return;
+  const int dm = (int)std::ceil(dmax) + 1;
+  p.K = h->K;
+  p.M = h->M;
+  p.n_t = h->n_t;
+  p.kp = (2 * h->M + 3) & ~3;
+  if ((p.kp & 7) == 0) p.kp += 4;                      // rows 32 bytes apart modulo 64: conflict-free fragment loads
+  p.KS = p.kp / 4;
+  p.R0 = dm + 8;
+  p.n_blocks = (h->n_t + 223) / 224;
+  p.rows_ext = p.R0 + (p.n_blocks - 1) * 224 + dm + 256 + 8;
+  p.point_stride = (int64_t)p.K * p.rows_ext * p.kp * 8;
+  for (int slots = 3; slots >= 2; --slots) {
+    p.slots = slots;
+    if (lnl_sky64_smem_bytes(p) <= 227u * 1024u) {
+      p.ok = sky_make_cells(dmax, h->sky_cells) ? 1 : 0;
+      return;
+    }
+  }
+}
+
 // The sky-sorted kernel pays for its padding (about 32 slots per sky cell and segment): AUTO takes it for segments of at
 // least 256 samples per cell when the tcgen05 kernels do not apply (windows of more than 512 samples: C4).
 bool use_sky(const rift_ile *h, int64_t n_per_seg) {
+  if (h->precision == RIFT_PREC_FP64) {
+    if (!h->sky64.ok || h->d_Qsky64 == nullptr) return false;
+    if (h->kernel_variant == RIFT_KERNEL_SKY) return true;
+    return h->kernel_variant == RIFT_KERNEL_AUTO && !h->mma.ok && n_per_seg >= 256 * (int64_t)h->sky_cells.n_cells;
+  }
   if (!h->sky.ok || h->d_Qsky == nullptr) return false;
   if (h->kernel_variant == RIFT_KERNEL_SKY) return true;
   return h->kernel_variant == RIFT_KERNEL_AUTO && !h->tc.ok && n_per_seg >= 256 * (int64_t)h->sky_cells.n_cells;
@@ -643,18 +686,22 @@ int run_chunks_sky(rift_ile *h, int32_t n_seg, int64_t n_per_seg, const double *
       CU(h, launch_sky_sort(h->sky_cells, h->geom.gmst, b, params, n_lseg, key, pos, count, base, perm, slots, n_batches, s, &nl));
       Batch bs = b;
       bs.n = slots;                                                // one thread per sorted slot; padding slots return at once
-      CU(h, launch_geometry(h->geom, h->d_modes, bs, params, h->d_U, h->d_V, h->qp, true, ws, shift_out, nullptr, nullptr, perm, s));
+      CU(h, launch_geometry(h->geom, h->d_modes, bs, params, h->d_U, h->d_V, h->qp, h->precision == RIFT_PREC_MIXED, ws, shift_out,
+                            nullptr, nullptr, perm, s));
       ++nl;
       ps.end();
     }
     {
       ProfSpan ps(h, 1, s);
-      CU(h, launch_lnl_sky(h->sky, h->d_Qsky, h->d_qscale_sky, b, ws, n_batches, slots / SKY_NB, lnL_out, h->n_sm, s, &nl));
+      if (h->precision == RIFT_PREC_MIXED)
+        CU(h, launch_lnl_sky(h->sky, h->d_Qsky, h->d_qscale_sky, b, ws, n_batches, slots / SKY_NB, lnL_out, h->n_sm, s, &nl));
+      else
+        CU(h, launch_lnl_sky64(h->sky64, h->d_Qsky64, b, ws, n_batches, slots / SKY_NB, lnL_out, h->n_sm, s, &nl));
       ps.end();
     }
     h->launches += nl;
   }
-  h->kernel_name = "lnl_sky<f16x3>";
+  h->kernel_name = h->precision == RIFT_PREC_MIXED ? "lnl_sky<f16x3>" : "lnl_sky<f64>";
   return RIFT_OK;
 }
 
@@ -963,6 +1010,16 @@ int rift_ile_create(const rift_ile_config *cfg, rift_ile_t **out) {
         cudaGetLastError();
         cudaFree(h->d_Qsky);
         h->d_Qsky = nullptr;
+      }
+    }
+    make_sky64_plan(h, cfg->delta_t);
+    if (e == cudaSuccess && h->sky64.ok) {
+      if (cudaMalloc(&h->d_Qsky64, (size_t)h->P * h->sky64.point_stride) == cudaSuccess) {
+        e = launch_convert_q_sky64(src, h->d_Qsky64, h->sky64, h->P, 0);
+        ++h->launches;
+      } else {
+        cudaGetLastError();
+        h->d_Qsky64 = nullptr;
       }
     }
     // A operand of the tensor-core path (fp16 hi | lo pieces), when the configuration fits tensor memory

@@ -150,6 +150,13 @@ struct SkyPlan {
   int64_t point_stride;          // bytes per intrinsic point: K * rows_ext * rowb
 };
 
+struct Sky64Plan {               // fp64 sibling (lnl_sky64.cu): operand rows of kp doubles (kp = 4 mod 8), KS = kp / 4 k-steps
+  int32_t ok;
+  int32_t K, M, n_t, kp, KS;
+  int32_t R0, rows_ext, n_blocks, slots;   // blocks of 224 window entries; ring slots of 256 rows
+  int64_t point_stride;          // bytes per intrinsic point: K * rows_ext * kp * 8
+};
+
 // geometry.cu
 cudaError_t launch_geometry_tc(const DetGeom &g, const ModeEntry *modes, const TcPlan &tp, const TcChunk &c,
                                const double *const params[6], const double *U, const double *V, const QuadProg &qp,
@@ -205,6 +212,11 @@ cudaError_t launch_convert_q_sky(const double *Q_c128, void *dst, float *qscale,
 cudaError_t launch_lnl_sky(const SkyPlan &p, const void *q, const float *qscale, const Batch &b, const Workspace &ws,
                            const int32_t *n_batches_dev, int64_t max_batches, double *lnL_out, int n_sm, cudaStream_t s,
                            int *n_launch);
+size_t lnl_sky64_smem_bytes(const Sky64Plan &p);
+cudaError_t launch_convert_q_sky64(const double *Q_c128, void *dst, const Sky64Plan &p, int32_t n_points, cudaStream_t s);
+cudaError_t launch_lnl_sky64(const Sky64Plan &p, const void *q, const Batch &b, const Workspace &ws,
+                             const int32_t *n_batches_dev, int64_t max_batches, double *lnL_out, int n_sm, cudaStream_t s,
+                             int *n_launch);
 // reduce.cu
 struct ReduceState {             // device, per segment
   double m, s1, s2;

@@ -92,8 +92,7 @@ def test_higher_l_harmonics(torch, oracle):
 KERNELS = [rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_DIRECT, rift.RIFT_KERNEL_TC, rift.RIFT_KERNEL_TCS, rift.RIFT_KERNEL_MMA,
            rift.RIFT_KERNEL_SKY]
 TC_FAMILY = (rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_TC, rift.RIFT_KERNEL_TCS, rift.RIFT_KERNEL_MMA)   # MMA: fp64 only, AUTO in mixed
-MMA_FAMILY = (rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_MMA, rift.RIFT_KERNEL_TC, rift.RIFT_KERNEL_TCS,
-              rift.RIFT_KERNEL_SKY)                                                                  # TC/TCS/SKY: mixed only, AUTO in fp64
+MMA_FAMILY = (rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_MMA, rift.RIFT_KERNEL_TC, rift.RIFT_KERNEL_TCS)  # TC/TCS: mixed only, AUTO in fp64
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
@@ -112,7 +111,7 @@ def test_c0_all_samples_both_precisions(torch, oracle, rho, kernel):
         # the tcgen05 kernel is the default of the mixed mode (and never runs in fp64 mode)
         assert ("lnl_tc" in rift.rift_ile_kernel_name(h)) == (
             prec == rift.RIFT_PREC_MIXED and kernel in TC_FAMILY)
-        assert ("lnl_sky" in rift.rift_ile_kernel_name(h)) == (prec == rift.RIFT_PREC_MIXED and kernel == rift.RIFT_KERNEL_SKY)
+        assert ("lnl_sky" in rift.rift_ile_kernel_name(h)) == (kernel == rift.RIFT_KERNEL_SKY)   # both precision modes
         # the shift-sorted variant: on request, or by default when the segments are long enough to fill its buckets
         if prec == rift.RIFT_PREC_MIXED and kernel == rift.RIFT_KERNEL_TCS:
             assert "lnl_tcs" in rift.rift_ile_kernel_name(h)
@@ -272,15 +271,21 @@ def test_sky_kernel_shapes(torch, oracle, shape):
     params[3, 5] = np.nan
     ref = np.concatenate([oracle_eval(oracle, inp, ids[s], params[:, s * n:(s + 1) * n])[0] for s in range(len(ids))])
     sref = np.concatenate([oracle_eval(oracle, inp, ids[s], params[:, s * n:(s + 1) * n])[1] for s in range(len(ids))])
-    h = create(rift, inp, rift.RIFT_PREC_MIXED)
-    got, sh, _ = gpu_eval(torch, h, ids, n, params, K=cfg.n_det, kernel=rift.RIFT_KERNEL_SKY)
-    assert rift.rift_ile_kernel_name(h) == "lnl_sky<f16x3>"
-    got = got.cpu().numpy()
-    assert np.isnan(got[5]) and np.isnan(ref[5]) and np.isnan(got).sum() == 1
     ok = ~np.isnan(ref)
-    assert np.max(np.abs(got[ok] - ref[ok])) < TOL_MIXED_LNL, np.max(np.abs(got[ok] - ref[ok]))
-    assert np.array_equal(sh.cpu().numpy()[ok], sref[ok])
-    rift.rift_ile_destroy(h)
+    for prec in (rift.RIFT_PREC_MIXED, rift.RIFT_PREC_FP64):
+        if prec == rift.RIFT_PREC_FP64 and shape in ("c2", "m12"):
+            continue                                          # fp64 sibling: mode sets whose 256-row chunks fit the ring (M <~ 10)
+        h = create(rift, inp, prec)
+        got, sh, _ = gpu_eval(torch, h, ids, n, params, K=cfg.n_det, kernel=rift.RIFT_KERNEL_SKY)
+        assert rift.rift_ile_kernel_name(h) == ("lnl_sky<f16x3>" if prec == rift.RIFT_PREC_MIXED else "lnl_sky<f64>")
+        got = got.cpu().numpy()
+        assert np.isnan(got[5]) and np.isnan(ref[5]) and np.isnan(got).sum() == 1
+        if prec == rift.RIFT_PREC_MIXED:
+            assert np.max(np.abs(got[ok] - ref[ok])) < TOL_MIXED_LNL, np.max(np.abs(got[ok] - ref[ok]))
+        else:
+            assert np.max(rel_err(got[ok], ref[ok])) < TOL_FP64_REL, np.max(rel_err(got[ok], ref[ok]))
+        assert np.array_equal(sh.cpu().numpy()[ok], sref[ok])
+        rift.rift_ile_destroy(h)
 
 
 def test_tcs_chunks_across_segments(torch, oracle):
@@ -524,7 +529,7 @@ def test_reduce_parity_with_broad_weights(torch, oracle, config):
         rift.rift_ile_destroy(h)
 
 
-@pytest.mark.parametrize("case", ["tc", "tcs", "tcs_passes", "mma_resident", "mma_stream", "sky"])
+@pytest.mark.parametrize("case", ["tc", "tcs", "tcs_passes", "mma_resident", "mma_stream", "sky", "sky64"])
 def test_repeated_calls_are_bit_identical(torch, oracle, case):
     """The warp-specialised kernels hand data between warps through mbarriers, named barriers, tensor memory and shared
     memory; compute-sanitizer is closed on this pool, so the cheap race detector is determinism: 20 calls on the same inputs
@@ -537,7 +542,7 @@ def test_repeated_calls_are_bit_identical(torch, oracle, case):
     mixed = case in ("tc", "tcs", "tcs_passes", "sky")
     h = create(rift, inp, rift.RIFT_PREC_MIXED if mixed else rift.RIFT_PREC_FP64)
     kernel = {"tc": rift.RIFT_KERNEL_TC, "tcs": rift.RIFT_KERNEL_TCS, "tcs_passes": rift.RIFT_KERNEL_TCS,
-              "sky": rift.RIFT_KERNEL_SKY}.get(case, rift.RIFT_KERNEL_MMA)
+              "sky": rift.RIFT_KERNEL_SKY, "sky64": rift.RIFT_KERNEL_SKY}.get(case, rift.RIFT_KERNEL_MMA)
     first = None
     for _ in range(20):
         lnL, _sh, _p = gpu_eval(torch, h, ids, n, params, want_shifts=False, kernel=kernel)
@@ -546,7 +551,8 @@ def test_repeated_calls_are_bit_identical(torch, oracle, case):
             first = g
             name = rift.rift_ile_kernel_name(h)
             want = {"tc": "lnl_tc<f16x3>", "tcs": "lnl_tcs<f16x3>", "tcs_passes": "lnl_tcs<f16x3,passes>",
-                    "mma_resident": "lnl_mma<f64,resident>", "mma_stream": "lnl_mma<f64,stream>", "sky": "lnl_sky<f16x3>"}[case]
+                    "mma_resident": "lnl_mma<f64,resident>", "mma_stream": "lnl_mma<f64,stream>", "sky": "lnl_sky<f16x3>",
+                    "sky64": "lnl_sky<f64>"}[case]
             assert name == want, name
             ref = np.concatenate([oracle_eval(oracle, inp, ids[s], params[:, s * n:(s + 1) * n])[0] for s in range(len(ids))])
             if mixed:
@@ -688,7 +694,7 @@ def test_c3_full_size(torch, oracle):
 def test_c4_full_size(torch, oracle):
     # 8 points x 4e6 samples, mixed and fp64; a 1/60 subsample of four points (2.7e5 samples) ...
     n = _full_size_sampled(torch, oracle, synth.CONFIGS[4], (rift.RIFT_PREC_MIXED, rift.RIFT_PREC_FP64), 4, 60, lnz_points=0,
-                           expect_kernel={rift.RIFT_PREC_MIXED: "lnl_sky", rift.RIFT_PREC_FP64: "lnl_direct<f64"})
+                           expect_kernel={rift.RIFT_PREC_MIXED: "lnl_sky<f16x3>", rift.RIFT_PREC_FP64: "lnl_sky<f64>"})
     assert n >= 100_000
 
 
