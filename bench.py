@@ -200,10 +200,10 @@ class ConfigData:
         th = [synth.true_point(cfg, pid) for pid in gids]
         geo = [gfn(t) for t in th]
         rift.rift_ile_destroy(hboot)
-        synth._dft_matrix(cfg.n_t, cfg.f_s)                  # fill the cache before the worker threads read it
-        self.Q = np.empty((P, K, M, cfg.n_t), dtype=np.complex128)
-        self.U = np.empty((P, K, M, M), dtype=np.complex128)
-        self.V = np.empty((P, K, M, M), dtype=np.complex128)
+        # frequency series of every point on the host (seeded recipe), Q / U / V on the device (rift_ile_precompute, NEXT-3)
+        hs = np.empty((P, K, M, synth.N_FREQ), dtype=np.complex128)
+        ds = np.empty((P, K, synth.N_FREQ), dtype=np.complex128)
+        sp0 = [None]
         self.params_h = torch.empty((6, P * N), dtype=torch.float64).pin_memory()
         self.has_w = cfg.proposal != "prior"
         self.lnw_h = torch.empty(P * N, dtype=torch.float64).pin_memory() if self.has_w else None
@@ -213,14 +213,30 @@ class ConfigData:
         def one(p):                                          # numpy releases the GIL in the heavy parts
             F, Y, shift = geo[p]
             coeff = np.asarray(F).reshape(K, 1) * np.asarray(Y).reshape(1, M)
-            pd = synth.make_point(cfg, gids[p], coeff, shift, synth.D_REF_MPC / th[p][5])
-            self.Q[p], self.U[p], self.V[p] = pd.Q, pd.U, pd.V
+            sp = synth.make_spectra(cfg, gids[p], coeff, shift, synth.D_REF_MPC / th[p][5])
+            hs[p], ds[p] = sp.h, sp.d
+            if p == 0:
+                sp0[0] = sp
             ps, ws = synth.draw_samples(cfg, gids[p], theta_true=th[p])
             pn[:, p * N:(p + 1) * N] = ps
             if wn is not None:
                 wn[p * N:(p + 1) * N] = ws
 
         list(pool.map(one, range(P)))
+        sp = sp0[0]
+        h_d, d_d = torch.from_numpy(hs.view(np.float64)).cuda(), torch.from_numpy(ds.view(np.float64)).cuda()
+        w_d, f_d = torch.from_numpy(sp.w).cuda(), torch.from_numpy(sp.f).cuda()
+        self.Q = torch.empty((P, K, M, cfg.n_t, 2), dtype=torch.float64, device="cuda")
+        self.U = torch.empty((P, K, M, M, 2), dtype=torch.float64, device="cuda")
+        self.V = torch.empty((P, K, M, M, 2), dtype=torch.float64, device="cuda")
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        ev[0].record()
+        rift.rift_ile_precompute(P, K, M, h_d, d_d, w_d, sp.f, f_d, cfg.n_t, cfg.delta_t, self.Q, self.U, self.V,
+                                 torch.cuda.current_stream().cuda_stream)
+        ev[1].record()
+        torch.cuda.synchronize()
+        self.precompute_ms = ev[0].elapsed_time(ev[1])
+        del h_d, d_d, hs, ds
         self.params_d = self.params_h.cuda()
         self.lnw_d = self.lnw_h.cuda() if self.has_w else None
         self.lnL_d = torch.empty(P * N, dtype=torch.float64, device="cuda")
@@ -234,7 +250,7 @@ def bench_row(rift, torch, dist_util, data: ConfigData, precision: str, steps, w
     cfg, P, N, K, M = data.cfg, data.P, data.N, data.cfg.n_det, data.cfg.n_modes
     fp64 = precision == "fp64"
     h = rift.rift_ile_create(data.loc, data.resp, cfg.gmst, data.ml, data.mm, P, cfg.n_t, cfg.delta_t, cfg.n_t,
-                             synth.D_REF_MPC, data.Q, data.U, data.V,
+                             synth.D_REF_MPC, data.Q, data.U, data.V, input_mem=rift.RIFT_MEM_DEVICE,
                              precision=rift.RIFT_PREC_FP64 if fp64 else rift.RIFT_PREC_MIXED)
     ids = list(range(P))
     stream = torch.cuda.current_stream().cuda_stream
@@ -340,6 +356,7 @@ def bench_row(rift, torch, dist_util, data: ConfigData, precision: str, steps, w
                 "h2d_gb_per_s": (data.params_h.numel() * 8 + (data.lnw_h.numel() * 8 if data.has_w else 0)) / (e["ms"] * 1e-3) / 1e9,
                 "path": "rift_ile_eval_batch_host (4 slices: upload / evaluate / read back overlapped) + rift_ile_reduce"},
         "clocks": sampler.window(*r["window"]) if sampler else None,
+        "precompute_ms": data.precompute_ms,      # Q, U, V of all points from their frequency series on the device (NEXT-3)
         "lnZ_point0": float(r["out"]["lnZ"][0]), "n_eff_point0": float(r["out"]["n_eff"][0]),
     }
     if evals <= 65536:

@@ -151,6 +151,20 @@ int rift_ile_reduce(rift_ile_t *h, int32_t n_seg, int64_t n_per_seg, const doubl
 int rift_ile_geometry(rift_ile_t *h, int32_t intrinsic_id, int64_t n, const double *const params[RIFT_N_PARAMS],
                       void *F, void *Y, int32_t *shift, double *quad, void *cuda_stream);
 
+/* The inputs of rift_ile_create from frequency series: the inner products of Eq. (D4a-c)
+ * as weighted sums over a caller-supplied list of frequencies (reading E1: with
+ * weight = 4 df / S_k(f) over f > 0 these are the one-sided products of BASELINE.json configs[0]; with 2 df / S_k(|f|) over
+ * positive and negative f the two-sided Eq. (D4a)):
+ *   Q[p][k][a][j] = sum_n weight[k][n] exp(2 pi i f_n t_j) conj(h[p][k][a][n]) data[p][k][n],  t_j = (j - (n_t-1)/2) delta_t
+ *   U[p][k][a][b] = sum_n weight[k][n] conj(h[p][k][a][n]) h[p][k][b][n];   V[p][k][a][b] = sum_n weight[k][n] h[..a..] h[..b..]
+ * h_modes [P][K][M][n_freq], data [P][K][n_freq] complex128, weight [K][n_freq], freq_hz [n_freq] fp64: DEVICE;
+ * freq_hz_host: the same frequencies on the HOST (to recognise an equally spaced grid); Q [P][K][M][n_t], U, V [P][K][M][M]
+ * complex128: DEVICE outputs, in the layout rift_ile_create takes with input_mem = RIFT_MEM_DEVICE.  No handle; asynchronous
+ * on cuda_stream.  U comes out Hermitian and V symmetric up to rounding (create does not require more). */
+int rift_ile_precompute(int32_t n_points, int32_t n_det, int32_t n_modes, int32_t n_freq, const void *h_modes,
+                        const void *data, const double *weight, const double *freq_hz_host, const double *freq_hz, int32_t n_t,
+                        double delta_t, void *Q, void *U, void *V, void *cuda_stream);
+
 /* Choose the fused-lnL kernel variant (RIFT_KERNEL_*); AUTO picks per configuration and call size: in mixed precision the
  * tensor-core kernels (TCS, which buckets the samples by the relative shift of detector 1, for calls of >= 32768 samples in
  * segments of >= 100 samples per bucket; else TC) when the configuration fits tensor and shared memory, and for longer

@@ -27,7 +27,7 @@ RIFT_N_PARAMS = 6
 EXPORTS = ("rift_ile_create", "rift_ile_eval_batch", "rift_ile_reduce", "rift_ile_geometry", "rift_ile_set_kernel",
            "rift_ile_launch_count", "rift_ile_kernel_name", "rift_ile_profile", "rift_ile_profile_read",
            "rift_ile_fma_peak", "rift_ile_set_option", "rift_ile_reserve", "rift_ile_eval_batch_host",
-           "rift_ile_staged", "rift_ile_eval_batch_dmarg", "rift_ile_destroy",
+           "rift_ile_staged", "rift_ile_eval_batch_dmarg", "rift_ile_precompute", "rift_ile_destroy",
            "rift_ile_strerror", "rift_ile_last_error")
 AC_EXPORTS = ("rift_ac_create", "rift_ac_draw", "rift_ac_update", "rift_ac_update_dims", "rift_ac_get_masses",
               "rift_ac_ile_ln_weight", "rift_ac_destroy")
@@ -73,6 +73,8 @@ def lib() -> C.CDLL:
         L.rift_ile_eval_batch_host.restype = C.c_int
         L.rift_ile_eval_batch_dmarg.argtypes = [vp, i32, vp, i64, C.POINTER(vp), dbl, dbl, i32, vp, vp, vp]
         L.rift_ile_eval_batch_dmarg.restype = C.c_int
+        L.rift_ile_precompute.argtypes = [i32, i32, i32, i32, vp, vp, vp, vp, vp, i32, dbl, vp, vp, vp, vp]
+        L.rift_ile_precompute.restype = C.c_int
         L.rift_ile_staged.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(i64)]
         L.rift_ile_staged.restype = C.c_int
         L.rift_ile_set_option.argtypes = [vp, i32, i64]
@@ -214,6 +216,16 @@ def rift_ile_eval_batch_dmarg(h, intrinsic_ids: Sequence[int], n_per_seg: int, p
     _check(lib().rift_ile_eval_batch_dmarg(h, int(ids.size), ids.ctypes.data, int(n_per_seg), ptrs, float(d_min_mpc),
                                            float(d_max_mpc), int(n_dist), _ptr(lnL_out), _ptr(shift_out),
                                            int(cuda_stream) or None), h)
+
+
+def rift_ile_precompute(n_points: int, n_det: int, n_modes: int, h_modes, data, weight, freq_hz_host, freq_hz, n_t: int,
+                        delta_t: float, Q, U, V, cuda_stream: int = 0) -> None:
+    """Q, U, V (device, complex128) from the frequency series h_modes [P][K][M][NF], data [P][K][NF] (device, complex128),
+    weight [K][NF], freq_hz [NF] (device, fp64); freq_hz_host: the frequencies as a host array."""
+    fh = np.ascontiguousarray(freq_hz_host, dtype=np.float64)
+    _check(lib().rift_ile_precompute(int(n_points), int(n_det), int(n_modes), int(fh.size), _ptr(h_modes), _ptr(data),
+                                     _ptr(weight), fh.ctypes.data, _ptr(freq_hz), int(n_t), float(delta_t), _ptr(Q), _ptr(U),
+                                     _ptr(V), int(cuda_stream) or None))
 
 
 def rift_ile_staged(h) -> dict:

@@ -1343,6 +1343,23 @@ int rift_ile_reduce(rift_ile_t *h, int32_t n_seg, int64_t n_per_seg, const doubl
   return RIFT_OK;
 }
 
+int rift_ile_precompute(int32_t n_points, int32_t n_det, int32_t n_modes, int32_t n_freq, const void *h_modes,
+                        const void *data, const double *weight, const double *freq_hz_host, const double *freq_hz, int32_t n_t,
+                        double delta_t, void *Q, void *U, void *V, void *cuda_stream) {
+  if (n_points < 1 || n_det < 1 || n_det > RIFT_MAX_DET || n_modes < 1 || n_modes > RIFT_MAX_MODES || n_freq < 1 || n_t < 1 ||
+      !(delta_t > 0.0))
+    return RIFT_EINVAL;
+  if (!h_modes || !data || !weight || !freq_hz_host || !freq_hz || !Q || !U || !V) return RIFT_EINVAL;
+  // equally spaced bins (the usual case): one exact phase per run of 32 bins, rotations in between
+  int equal = n_freq > 1 ? 1 : 0;
+  const double df = n_freq > 1 ? (freq_hz_host[n_freq - 1] - freq_hz_host[0]) / (n_freq - 1) : 0.0;
+  for (int32_t n = 0; n < n_freq && equal; ++n)
+    if (std::fabs(freq_hz_host[n] - (freq_hz_host[0] + n * df)) > 1e-12 * std::fmax(1.0, std::fabs(freq_hz_host[n]))) equal = 0;
+  const cudaError_t e = launch_precompute(n_points, n_det, n_modes, n_freq, h_modes, data, weight, freq_hz, equal, df, n_t, delta_t,
+                                          Q, U, V, reinterpret_cast<cudaStream_t>(cuda_stream));
+  return e == cudaSuccess ? RIFT_OK : RIFT_ECUDA;
+}
+
 int rift_ile_profile(rift_ile_t *h, int32_t enable) {
   if (!h) return RIFT_EINVAL;
   h->profiling = enable != 0;

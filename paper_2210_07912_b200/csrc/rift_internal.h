@@ -217,6 +217,10 @@ cudaError_t launch_convert_q_sky64(const double *Q_c128, void *dst, const Sky64P
 cudaError_t launch_lnl_sky64(const Sky64Plan &p, const void *q, const Batch &b, const Workspace &ws,
                              const int32_t *n_batches_dev, int64_t max_batches, double *lnL_out, int n_sm, cudaStream_t s,
                              int *n_launch);
+// precompute.cu (NEXT-3: Q, U, V from frequency series)
+cudaError_t launch_precompute(int32_t P, int32_t K, int32_t M, int32_t n_freq, const void *h, const void *d, const double *w,
+                              const double *f, int equal_spacing, double df, int32_t n_t, double delta_t, void *Q, void *U,
+                              void *V, cudaStream_t s);
 // reduce.cu
 struct ReduceState {             // device, per segment
   double m, s1, s2;

@@ -220,9 +220,20 @@ class PointData:
     scale: float         # the scalar applied to every h_lm (reading A7)
 
 
-def make_point(cfg: Config, point: int, coeff_true: np.ndarray, shift_true: np.ndarray,
-               c_true: float, noise: bool = True) -> PointData:
-    """Build Q, U, V of one intrinsic point by the literal recipe of BASELINE.json configs[0].
+@dataclass
+class Spectra:
+    h: np.ndarray        # [K][M][N_FREQ] complex128: the modes h_lm(f) per detector (reading B1), already scaled (A7)
+    d: np.ndarray        # [K][N_FREQ] complex128: the data of every detector
+    w: np.ndarray        # [K][N_FREQ] float64: inner-product weights 4 df / S(f) (the one-sided recipe of configs[0])
+    f: np.ndarray        # [N_FREQ] Hz
+    rho: float
+    scale: float
+
+
+def make_spectra(cfg: Config, point: int, coeff_true: np.ndarray, shift_true: np.ndarray, c_true: float,
+                 noise: bool = True) -> Spectra:
+    """Frequency series of one intrinsic point by the literal recipe of BASELINE.json configs[0] (the inputs of
+    Eq. (D4a-c)): modes, data, inner-product weights.
 
     coeff_true[k][lm] : complex, the coefficient of h_lm in detector k's data (the caller passes
                         F_k * Y_lm at the true point; this module does not know what it means).
@@ -230,7 +241,7 @@ def make_point(cfg: Config, point: int, coeff_true: np.ndarray, shift_true: np.n
                         exp(-2 pi i f shift/f_s) so that Q_k peaks shift_true[k] samples after t_ref.
     c_true            : D_ref / D_true.
     """
-    K, M, n_t = cfg.n_det, cfg.n_modes, cfg.n_t
+    K, M = cfg.n_det, cfg.n_modes
     coeff_true = np.asarray(coeff_true, dtype=np.complex128).reshape(K, M)
     shift_true = np.asarray(shift_true, dtype=np.int64).reshape(K)
     f, df = freq_grid()
@@ -255,6 +266,19 @@ def make_point(cfg: Config, point: int, coeff_true: np.ndarray, shift_true: np.n
     if noise:
         sig = np.sqrt(S / (4.0 * df))                      # reading A8: Re and Im each N(0, S/(4 df))
         d = d + sig * (rng.standard_normal((K, N_FREQ)) + 1j * rng.standard_normal((K, N_FREQ)))
+    w = np.broadcast_to(4.0 * df / S, (K, N_FREQ)).copy()
+    return Spectra(np.ascontiguousarray(h), np.ascontiguousarray(d), w, f, cfg.rho if rho0 > 0 else 0.0, scale)
+
+
+def make_point(cfg: Config, point: int, coeff_true: np.ndarray, shift_true: np.ndarray,
+               c_true: float, noise: bool = True) -> PointData:
+    """Q, U, V of one intrinsic point from make_spectra's series, on the host (numpy): the generator of the parity tests.
+    (bench.py builds the same arrays on the device with rift_ile_precompute.)"""
+    K, M, n_t = cfg.n_det, cfg.n_modes, cfg.n_t
+    sp = make_spectra(cfg, point, coeff_true, shift_true, c_true, noise)
+    h, d, f = sp.h, sp.d, sp.f
+    df = (F_HIGH_HZ - F_LOW_HZ) / N_FREQ
+    S = psd(cfg.psd, f)
 
     # U = 4 df sum h* h'/S ; V = 4 df sum h h'/S   (configs[0])
     hw = h / S
@@ -268,7 +292,7 @@ def make_point(cfg: Config, point: int, coeff_true: np.ndarray, shift_true: np.n
     W = (np.conj(h) * (d / S)[:, None, :]).reshape(K * M, N_FREQ)
     Q = (4.0 * df) * (W @ E.T)                             # [K*M][N_t]
     return PointData(np.ascontiguousarray(Q.reshape(K, M, n_t)), np.ascontiguousarray(U),
-                     np.ascontiguousarray(V), cfg.rho if rho0 > 0 else 0.0, scale)
+                     np.ascontiguousarray(V), sp.rho, sp.scale)
 
 
 # ----------------------------------------------------------------------------------------------
