@@ -4,22 +4,26 @@
 //
 // "Contract in unshifted detector time, then shift": per detector k the window term is the real GEMM
 //     P_k[t, n] = sum_kappa A_k[t, kappa] B_k[kappa, n],   A_k[t, 2m + {0,1}] = {Re, Im} Q_{k,m}[t],  B_k[2m + {0,1}, n] = {Re, Im}(F_k Y_m)_n
-// over ALL stored rows t (M = time, N = the 16 samples of a batch, K = 2 x modes), issued as mma.sync.m8n8k4.f64 (DMMA, 256
+// over ALL stored rows t (M = time, N = the samples of a batch, K = 2 x modes), issued as mma.sync.m8n8k4.f64 (DMMA, 256
 // FMA per instruction and warp: one Q value read from shared memory feeds 8 samples, one coefficient 8 rows -- the direct
-// kernel reads a 16-byte Q value per 2 DFMA and cannot pass 25 % of the pipe).  The per-sample shift is applied by an exchange
-// through shared memory, one detector at a time: the tiles of P_k are stored unshifted as rows of 16 samples (128 B, the two
-// 64-byte halves swapped on odd rows: a 16-byte store per thread and tile, conflict-free), with circular copies inside the halo
-// H = max_k |s_k - s_0| so that a reader never wraps; a thread then owns one sample n and the window entries
-// j = JS e + 2 warp + jj (e = 0..NE-1) and adds P_k[j + off_{n,k}][n] into its registers -- half a warp reads 8 samples x 2
-// consecutive rows, conflict-free whatever the shifts are, and the addresses of a thread are one base plus immediates.  The
-// window x never leaves the registers: the time marginal takes a float maximum (any reference >= max - eps serves the
-// log-sum-exp) and the sum of 2^(c log2e (x - m)) with a polynomial exponential, both reduced across warps in shared memory.
+// kernel reads a 16-byte Q value per 2 DFMA and cannot pass 25 % of the pipe).  The per-sample shift is applied when the
+// tiles leave the registers: the window X[j][n] of the batch lives in shared memory (rows of NBG samples, pitch NBG * 8 + 8
+// bytes) and the thread holding P_k[t][n] adds it to row j = (t - off_{n,k}) mod N_t -- a plain store for the first detector,
+// a read-modify-write for the others, one group barrier per detector in between (an element is touched by one thread per
+// detector).  The row of tile i of a thread is row_0 + 8 GW i, so the wrap of a circular window is one threshold per sample
+// and detector (tiles below it use one base address, the others a second one, N_t rows apart) and the addresses are a base
+// register plus immediates; rows >= N_t of the operand are zero and add nothing wherever they land.  The tensor phase of
+// detector k + 1 is issued before the barrier that closes detector k.  The time marginal then reads the window back, one
+// sample and NE entries per thread: a float maximum (any reference >= max - eps serves the log-sum-exp) and the sum of
+// 2^(c log2e (x - m)) with a polynomial exponential, both reduced across warps in shared memory.
 //
 // Q operand: the handle keeps [P][K][M2][pitch] bytes, M2 = 2 ceil(M/2) mode rows per detector (zero rows pad an odd mode
 // count), every row n_r = 8 ceil(N_t/8) complex128 (zero beyond N_t) followed by 64 pad bytes, so that the two mode rows of
 // one k-step sit 64 bytes apart modulo 128 and an A fragment load (8 rows x 2 modes x 16 B) is conflict-free.  Small
 // configurations keep the whole block of the intrinsic point resident in shared memory (one bulk copy per point); larger
 // ones stream (detector, k-step) chunks through a ring filled by a producer warp with cp.async.bulk on mbarriers.
+#include <type_traits>
+
 #include "rift_internal.h"
 #include "tma_utils.cuh"
 #include "exp2_poly.cuh"
@@ -41,7 +45,8 @@ struct MmaShape {
   static constexpr int GW = STREAM ? 15 : 8;       // warps per group
   static constexpr int RBW = STREAM ? 4 : 8;       // row blocks (of 8 rows) per warp: wg + GW i
   static constexpr int GTHR = GW * 32;
-  static constexpr int RB = 64 * NT;               // bytes per exchange row
+  static constexpr int XP = 64 * NT + 8;           // bytes per window row (8 pad bytes: 8 consecutive rows, 8 bank pairs)
+  static constexpr int RS = 8 * GW;                // rows between two tiles of a thread
   static constexpr int RPW = NT == 2 ? 2 : 4;      // window entries a warp reads per element index e
   static constexpr int JS = RPW * GW;              // ... a group
 };
@@ -49,6 +54,12 @@ struct MmaShape {
 __device__ __forceinline__ void mm_arrive(uint64_t *bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
+__device__ __forceinline__ double ld_shared_f64(uint32_t a) {
+  double v;
+  asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_shared_f64(uint32_t a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
 __device__ __forceinline__ void mm_bar(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
 __device__ __forceinline__ void dmma(double (&d)[2], double a, double b) {
@@ -63,7 +74,7 @@ struct MmaSmem {                                   // byte offsets inside dynami
 
 __host__ __device__ inline MmaSmem mma_smem(const MmaPlan &p) {
   MmaSmem L;
-  const uint32_t nbg = p.stream ? 16u : 8u, groups = p.stream ? 1u : 2u, rb = p.stream ? 128u : 64u;
+  const uint32_t nbg = p.stream ? 16u : 8u, groups = p.stream ? 1u : 2u, rb = p.stream ? 136u : 72u;
   L.bars = 0;                                                          // full[8], empty[8], resident
   L.grp = 256;
   L.coef_bytes = (uint32_t)p.K * p.KS * nbg * 4 * 8;                   // cs[K][KS][NBG][4] doubles, two buffers at offset 0
@@ -71,13 +82,19 @@ __host__ __device__ inline MmaSmem mma_smem(const MmaPlan &p) {
   L.meta_bytes = 2 * nbg * 8 + (uint32_t)p.K * nbg * 4;                // c[NBG], q[NBG] doubles, off[K][NBG] int32, two buffers
   L.wmax = (L.meta + 2 * L.meta_bytes + 15u) & ~15u;                   // wmax[2][NBG][16] float
   L.psum = L.wmax + 2 * nbg * 16 * 4;                                  // psum[2][NBG][16] double
-  L.xb = (L.psum + 2 * nbg * 16 * 8 + 127u) & ~127u;                   // exchange rows
+  L.xb = (L.psum + 2 * nbg * 16 * 8 + 127u) & ~127u;                   // window rows
   L.grp_stride = (L.xb + (uint32_t)p.xb_rows * rb + 127u) & ~127u;
   L.q = L.grp + groups * L.grp_stride;
   const uint32_t qbytes = p.stream ? (uint32_t)p.slots * 2u * (uint32_t)p.pitch_q
                                    : (uint32_t)p.K * 2u * p.KS * (uint32_t)p.pitch_q;
   L.total = L.q + qbytes;
   return L;
+}
+
+__device__ __forceinline__ float mf_of(const float *wmax, int n, bool wide) {          // maximum of a sample's per-warp slots
+  float m = -INFINITY;
+  for (int w = 0; w < (wide ? 16 : 8); ++w) m = fmaxf(m, wmax[n * 16 + w]);
+  return m;
 }
 
 struct MmaArgs {
@@ -87,18 +104,13 @@ struct MmaArgs {
   Batch b;
   Workspace ws;
   double *lnL_out;
+  double ln_ntau;
 };
-
-// exchange-buffer byte offset of (row, sample n).  Two tiles: 128-byte rows whose two 64-byte halves swap on odd rows
-template <int NT>
-__device__ __forceinline__ uint32_t xb_off(int row, int n) {
-  return NT == 2 ? (uint32_t)row * 128u + (uint32_t)((n ^ ((row & 1) << 3)) * 8) : (uint32_t)row * 64u + (uint32_t)(n * 8);
-}
 
 template <bool STREAM, int NE, int PFN>
 __global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs A) {
   typedef MmaShape<STREAM> S;
-  constexpr int NT = S::NT, NBG = S::NBG, GW = S::GW, RBW = S::RBW, GTHR = S::GTHR, RB = S::RB, JS = S::JS;
+  constexpr int NT = S::NT, NBG = S::NBG, GW = S::GW, RBW = S::RBW, GTHR = S::GTHR, XP = S::XP, RS = S::RS, JS = S::JS;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const MmaPlan &P = A.p;
   const Batch &b = A.b;
@@ -125,12 +137,11 @@ __global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs
     reinterpret_cast<double *>(smem_raw + L.grp)[i] = 0.0;
   __syncthreads();
 
-  const int64_t w_begin = (b.n * blockIdx.x) / gridDim.x;
-  const int64_t w_end = (b.n * (blockIdx.x + 1)) / gridDim.x;
 
   // ---------------------------------------------------------------------------------------------- producer warp (ring)
   if (STREAM && warp == GW) {
     if (lane == 0) {
+      const int64_t w_begin = (b.n * blockIdx.x) / gridDim.x, w_end = (b.n * (blockIdx.x + 1)) / gridDim.x;
       uint32_t cnt = 0;
       for (int64_t w0 = w_begin; w0 < w_end;) {
         const int64_t seg = (b.g0 + w0) / b.n_per_seg;
@@ -154,28 +165,27 @@ __global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs
   const int g = STREAM ? 0 : warp / GW, wg = warp - g * GW, gtid = threadIdx.x - g * GTHR;
   const int bar_id = 1 + g;
   unsigned char *grp = smem_raw + L.grp + g * L.grp_stride;
-  unsigned char *xb = grp + L.xb;
-  float *wmax_all = reinterpret_cast<float *>(grp + L.wmax);
-  double *psum_all = reinterpret_cast<double *>(grp + L.psum);
-  for (int i = gtid; i < 2 * NBG * 16; i += GTHR) wmax_all[i] = -INFINITY;   // slots of absent warps never take part
+  const uint32_t grp_u32 = smem_u32(grp), xb_u32 = grp_u32 + L.xb;
+  for (int i = gtid; i < 2 * NBG * 16; i += GTHR) reinterpret_cast<float *>(grp + L.wmax)[i] = -INFINITY;   // absent warps
   // MMA role: fragment coordinates; row blocks wg + GW i are GW * 128 bytes apart: one base register plus immediates
   const int lr = lane >> 2, lc = lane & 3;
   const uint32_t a_base = (uint32_t)(lc >> 1) * (uint32_t)P.pitch_q + (uint32_t)(lc & 1) * 8u + (uint32_t)(8 * wg + lr) * 16u;
   const int nrb = 8 * wg < n_r ? (n_r - 8 * wg + 8 * GW - 1) / (8 * GW) : 0;   // valid row blocks of this warp (<= RBW)
-  // store role: tile (i, nt) of row t = t0 + 8 GW i goes to st[nt] + i * (8 GW RB); the row parity (hence the swizzle) does
-  // not depend on i
+  // scatter role: the thread holds P_k[t0 + RS i][8 nt + 2 lc + {0, 1}]; window row of stored row t and offset off:
+  // t - off (+- n_t on a circular window), + H on a guard-band window (off >= 0 there, nothing wraps: wrap_bytes 0)
   const int t0 = 8 * wg + lr;
-  const int row_bias = P.circular ? H : 0;                       // buffer row of stored row t = t + row_bias
-  const uint32_t st0 = xb_off<NT>(t0 + row_bias, 2 * lc), st1 = xb_off<NT>(t0 + row_bias, 8 + 2 * lc);
-  const uint32_t st0h = (NT == 2 && (n_t & 1)) ? st1 : st0, st1h = (NT == 2 && (n_t & 1)) ? st0 : st1;   // halo: parity may flip
-  // exchange-reader role: sample n, window entries j = jb + JS e
+  const bool last_ok = t0 + RS * (nrb - 1) < n_t;                // a zero row past n_t would wrap onto another thread's element
+  const int wrap_bytes = P.circular ? n_t * XP : 0;
+  const uint32_t sc_base = xb_u32 + (uint32_t)((t0 + (P.circular ? 0 : H)) * XP + 2 * lc * 8);
+  // window-reader role: sample n, window entries j = jb + JS e, e < nv
   const int n_mine = NT == 2 ? (((lane >> 4) << 3) | (lane & 7)) : (lane & 7);
   const int jj = NT == 2 ? ((lane >> 3) & 1) : (lane >> 3), jb = S::RPW * wg + jj;
-  const double ln_ntau = log((double)P.n_tau);
+  const uint32_t rd_base = xb_u32 + (uint32_t)((jb + (P.circular ? 0 : H)) * XP + n_mine * 8);
+  const int nv = min(NE, max(0, (n_x - jb + JS - 1) / JS));
 
-  // coefficient items of this thread: element id = gtid + GTHR i of the [NBG][2 K M] block of a batch.  PFN > 0: the next
-  // batch's items wait in registers during a batch; PFN == 0 (many items): they go straight to the other shared-memory
-  // buffer with 8-byte cp.async (zero-filled for the slots past the end of a run)
+  // coefficient items of this thread: element id = gtid + GTHR i of the [NBG][2 K M] block of a batch goes to the other
+  // shared-memory buffer with an 8-byte cp.async (zero-filled for the slots past the end of a run).  PFN > 0: the (source,
+  // destination) offsets of the <= PFN items wait in registers; PFN == 0 (many items): recomputed per batch
   constexpr int PFR = PFN > 0 ? PFN : 1;
   int pf_src[PFR], pf_dst[PFR];                                  // offset in the workspace row block; cs index | n << 24
 #pragma unroll
@@ -189,35 +199,38 @@ __global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs
       pf_dst[i] = (((k * KS + (kap >> 2)) * NBG + n) * 4 + (kap & 3)) | (n << 24);
     }
   }
-  double pf_v[PFR], pf_c = 1.0, pf_q = 0.0;
   int pf_off = 0;
-  auto prefetch = [&](int64_t s0, int64_t run_end, int dst_buf) {
-    const int nvalid = (int)min((int64_t)NBG, run_end - s0);
-    const double *src = reinterpret_cast<const double *>(ws.coef) + s0 * ws.coef_stride;
+  auto cp8 = [](uint32_t dst, const void *src, bool ok) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(dst), "l"(src), "r"(ok ? 8 : 0) : "memory");
+  };
+  auto prefetch = [&](int s0, int run_end, int dst_buf) {
+    const int nvalid = min(NBG, run_end - s0);
+    const double *src = reinterpret_cast<const double *>(ws.coef) + (int64_t)s0 * ws.coef_stride;
+    const uint32_t cs_base = grp_u32 + dst_buf * L.coef_bytes;
 #pragma unroll
-    for (int i = 0; i < PFN; ++i) {
-      pf_v[i] = 0.0;
-      if (pf_src[i] >= 0 && (pf_dst[i] >> 24) < nvalid) pf_v[i] = src[pf_src[i]];
-    }
+    for (int i = 0; i < PFN; ++i)
+      if (pf_src[i] >= 0) {
+        const bool ok = (pf_dst[i] >> 24) < nvalid;
+        cp8(cs_base + 8u * (uint32_t)(pf_dst[i] & 0xffffff), src + (ok ? pf_src[i] : 0), ok);
+      }
     if (PFN == 0) {
-      const uint32_t cs_base = smem_u32(grp + dst_buf * L.coef_bytes);
       for (int id = gtid; id < NBG * km2; id += GTHR) {
         const int n = id / km2, j = id - n * km2, k = j / m2, kap = j - k * m2;
-        const uint32_t dst = cs_base + 8u * (uint32_t)(((k * KS + (kap >> 2)) * NBG + n) * 4 + (kap & 3));
-        const double *gp = src + (n < nvalid ? n : 0) * ws.coef_stride + j;
-        asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(dst), "l"(gp), "r"(n < nvalid ? 8 : 0) : "memory");
+        cp8(cs_base + 8u * (uint32_t)(((k * KS + (kap >> 2)) * NBG + n) * 4 + (kap & 3)),
+            src + (n < nvalid ? n : 0) * ws.coef_stride + j, n < nvalid);
       }
     }
-    pf_c = 1.0, pf_q = 0.0, pf_off = 0;
-    if (gtid < nvalid) {
-      pf_c = ws.scale_c[s0 + gtid];
-      pf_q = ws.quad[s0 + gtid];
+    if (gtid < 2 * NBG) {                                        // c[NBG], q[NBG]
+      const int n = gtid & (NBG - 1);
+      const double *mp = (gtid < NBG ? ws.scale_c : ws.quad) + s0 + (n < nvalid ? n : 0);
+      cp8(grp_u32 + L.meta + dst_buf * L.meta_bytes + 8u * gtid, mp, n < nvalid);
     }
+    pf_off = 0;
     if (gtid < NBG * K) {
       const int k = gtid / NBG, n = gtid - k * NBG;
       if (n < nvalid) {
-        const int sk = ws.shift[(s0 + n) * K + k];
-        int off = P.circular ? sk - ws.shift[(s0 + n) * K] : P.j0 + sk;
+        const int sk = ws.shift[(int64_t)(s0 + n) * K + k];
+        int off = P.circular ? sk - ws.shift[(int64_t)(s0 + n) * K] : P.j0 + sk;
         // out of range only for a sample with NaN angles (its lnL is NaN anyway)
         if (off > H) off = H;
         if (off < (P.circular ? -H : 0)) off = 0;
@@ -226,24 +239,16 @@ __global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs
     }
   };
   auto commit = [&](int buf) {
-    double *cs = reinterpret_cast<double *>(grp + buf * L.coef_bytes);
-    unsigned char *meta = grp + L.meta + buf * L.meta_bytes;
-#pragma unroll
-    for (int i = 0; i < PFN; ++i)
-      if (pf_src[i] >= 0) cs[pf_dst[i] & 0xffffff] = pf_v[i];
-    if (PFN == 0) asm volatile("cp.async.wait_all;" ::: "memory");
-    if (gtid < NBG) {
-      reinterpret_cast<double *>(meta)[gtid] = pf_c;
-      reinterpret_cast<double *>(meta)[NBG + gtid] = pf_q;
-    }
-    if (gtid < NBG * K) reinterpret_cast<int *>(meta + 2 * NBG * 8)[gtid] = pf_off;
+    asm volatile("cp.async.wait_all;" ::: "memory");
+    if (gtid < NBG * K) reinterpret_cast<int *>(grp + L.meta + buf * L.meta_bytes + 2 * NBG * 8)[gtid] = pf_off;
   };
 
+  const int w_begin = (int)((b.n * blockIdx.x) / gridDim.x), w_end = (int)((b.n * (blockIdx.x + 1)) / gridDim.x);
   uint32_t cnt = 0, res_phase = 0;
-  int staged_point = -1;
-  for (int64_t w0 = w_begin; w0 < w_end;) {                      // runs of one segment: every group takes every other batch
+  int staged_point = -1, fin_w = 0;
+  for (int w0 = w_begin; w0 < w_end;) {                          // runs of one segment: every group takes every other batch
     const int64_t seg = (b.g0 + w0) / b.n_per_seg;
-    const int64_t run_end = min(w_end, (seg + 1) * b.n_per_seg - b.g0);
+    const int run_end = (int)min((int64_t)w_end, (seg + 1) * b.n_per_seg - b.g0);
     const int point = b.ids[seg];
     if (!STREAM && point != staged_point) {                      // both groups are past the previous run
       if (threadIdx.x == 0) stage_block(qs, A.q + (int64_t)point * P.point_stride, (uint32_t)P.point_stride, resbar);
@@ -251,7 +256,7 @@ __global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs
       res_phase ^= 1u;
       staged_point = point;
     }
-    int64_t s0 = w0 + (int64_t)g * NBG;
+    int s0 = w0 + g * NBG;
     int buf = 0;
     if (s0 < run_end) {
       prefetch(s0, run_end, 0);
@@ -259,121 +264,137 @@ __global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs
     }
     mm_bar(bar_id, GTHR);
     for (; s0 < run_end; s0 += S::GROUPS * NBG, buf ^= 1) {
-      const int64_t s_next = s0 + S::GROUPS * NBG;
-      if (s_next < run_end) prefetch(s_next, run_end, buf ^ 1);  // global loads in flight during this batch
+      const int s_next = s0 + S::GROUPS * NBG;
+      if (s_next < run_end) prefetch(s_next, run_end, buf ^ 1);  // copies in flight during this batch
       const double *cs = reinterpret_cast<const double *>(grp + buf * L.coef_bytes);
       const unsigned char *meta = grp + L.meta + buf * L.meta_bytes;
-      const double *mc = reinterpret_cast<const double *>(meta), *mq = mc + NBG;
       const int *moff = reinterpret_cast<const int *>(meta + 2 * NBG * 8);
-      float *wmax = wmax_all + buf * NBG * 16;
-      double *psum = psum_all + buf * NBG * 16;
 
-      double x[NE];
-      for (int k = 0; k < K; ++k) {
-        // ---- P_k tiles of this warp's row blocks
-        double acc[RBW][NT][2];
-#pragma unroll
-        for (int i = 0; i < RBW; ++i)
-#pragma unroll
-          for (int nt = 0; nt < NT; ++nt) acc[i][nt][0] = acc[i][nt][1] = 0.0;
-        const unsigned char *chunk = qs + (size_t)(k * 2 * KS) * P.pitch_q;                      // resident layout
+      // ---- detectors: tensor phase, then the tiles go to their window rows (store for k = 0, read-modify-write after)
+      auto detector = [&](int k, auto nrb_c) {
+        constexpr int NRB = decltype(nrb_c)::value;              // row blocks of this warp; 0: none (ring bookkeeping only)
+        double acc[NRB > 0 ? NRB : 1][NT][2];
+        const unsigned char *chunk = qs + (size_t)(k * 2 * KS) * P.pitch_q;                        // resident layout
         const double *bs = cs + (size_t)(k * KS) * NBG * 4 + lr * 4 + lc;
-        for (int s = 0; s < KS; ++s, ++cnt, bs += NBG * 4, chunk += slot_bytes) {
+        auto kstep = [&](auto first_c) {                           // the first k-step of a detector clears the accumulators
           uint32_t slot = 0;
           if (STREAM) {
             slot = cnt % (uint32_t)P.slots;
             mbar_wait(full + slot, (cnt / (uint32_t)P.slots) & 1u);
             chunk = qs + slot * slot_bytes;
           }
-          if (nrb > 0) {
-            double bf[NT];
+          if (NRB > 0) {
+            double bf[NT], af[NRB > 0 ? NRB : 1];
 #pragma unroll
             for (int nt = 0; nt < NT; ++nt) bf[nt] = bs[32 * nt];
-            double af[RBW];
 #pragma unroll
-            for (int i = 0; i < RBW; ++i)
-              if (i < nrb) af[i] = *reinterpret_cast<const double *>(chunk + a_base + i * (GW * 128));
+            for (int i = 0; i < NRB; ++i) af[i] = *reinterpret_cast<const double *>(chunk + a_base + i * (GW * 128));
 #pragma unroll
-            for (int i = 0; i < RBW; ++i)
-              if (i < nrb) {
+            for (int i = 0; i < NRB; ++i)
 #pragma unroll
-                for (int nt = 0; nt < NT; ++nt) dmma(acc[i][nt], af[i], bf[nt]);
+              for (int nt = 0; nt < NT; ++nt) {
+                // (a first step written as D = A B + 0 with no read of D raced with the stores of the detector before:
+                // the accumulators are cleared by ordinary moves instead)
+                if (decltype(first_c)::value) acc[i][nt][0] = acc[i][nt][1] = 0.0;
+                dmma(acc[i][nt], af[i], bf[nt]);
               }
           }
           if (STREAM) {
             __syncwarp();
             if (lane == 0) mm_arrive(empty + slot);
           }
-        }
-        mm_bar(bar_id, GTHR);                                    // every reader is done with detector k - 1
-        // ---- unshifted store: row t + row_bias, 16 bytes per tile (samples 8 nt + 2 lc, + 1), circular copies in the halo
+          ++cnt, bs += NBG * 4, chunk += slot_bytes;
+        };
+        kstep(std::true_type());
+        for (int s = 1; s < KS; ++s) kstep(std::false_type());
+        if (k > 0) mm_bar(bar_id, GTHR);                         // detector k - 1 is in the window (k = 0: the batch before is read)
+        if (NRB > 0) {
 #pragma unroll
-        for (int i = 0; i < RBW; ++i) {
-          const int t = t0 + 8 * GW * i;
-          if (i < nrb && t < n_t) {
-            unsigned char *d = xb + i * (8 * GW * RB);
+          for (int nt = 0; nt < NT; ++nt)
 #pragma unroll
-            for (int nt = 0; nt < NT; ++nt) {
-              const double2 v = make_double2(acc[i][nt][0], acc[i][nt][1]);
-              const uint32_t o = nt ? st1 : st0, oh = nt ? st1h : st0h;
-              *reinterpret_cast<double2 *>(d + o) = v;
-              if (P.circular) {
-                if (t < H) *reinterpret_cast<double2 *>(d + n_t * RB + oh) = v;
-                if (t >= n_t - H) *reinterpret_cast<double2 *>(d - n_t * RB + oh) = v;
+            for (int h = 0; h < 2; ++h) {
+              const int off = moff[k * NBG + 8 * nt + 2 * lc + h];
+              const uint32_t base = sc_base + (uint32_t)((8 * nt + h) * 8) - (uint32_t)(off * XP);
+              if (k == 0) {                                      // off = 0 (circular) or the guard-band offset: no wrap
+#pragma unroll
+                for (int i = 0; i < NRB; ++i) st_shared_f64(base + i * (RS * XP), acc[i][nt][h]);
+              } else {
+                // tiles i < thr use b_lo, the others b_lo - wrap: off >= 0 wraps the first rows up, off < 0 the last rows down
+                const int num = (off >= 0 ? off : n_t + off) - t0;
+                const int thr = (max(num, 0) + RS - 1) / RS;
+                const uint32_t b_lo = base + (off >= 0 ? (uint32_t)wrap_bytes : 0u), b_hi = b_lo - (uint32_t)wrap_bytes;
+#pragma unroll
+                for (int i = 0; i < NRB; ++i) {
+                  const uint32_t a = (i < thr ? b_lo : b_hi) + i * (RS * XP);
+                  if (i < NRB - 1 || last_ok) st_shared_f64(a, ld_shared_f64(a) + acc[i][nt][h]);
+                }
               }
             }
-          }
         }
-        mm_bar(bar_id, GTHR);                                    // the rows of detector k are complete
-        // ---- shifted read: x_j += P_k[j + off][n]
-        {
-          const unsigned char *src = xb + xb_off<NT>(jb + moff[k * NBG + n_mine] + row_bias, n_mine);
-          if (k == 0) {
-#pragma unroll
-            for (int e = 0; e < NE; ++e) x[e] = *reinterpret_cast<const double *>(src + e * (JS * RB));
-          } else {
-#pragma unroll
-            for (int e = 0; e < NE; ++e) x[e] += *reinterpret_cast<const double *>(src + e * (JS * RB));
-          }
+      };
+      for (int k = 0; k < K; ++k) {
+        switch (nrb) {
+          case 0: detector(k, std::integral_constant<int, 0>()); break;
+          case 1: detector(k, std::integral_constant<int, 1>()); break;
+          case 2: detector(k, std::integral_constant<int, 2>()); break;
+          case 3: detector(k, std::integral_constant<int, 3>()); break;
+          case 4: detector(k, std::integral_constant<int, 4>()); break;
+          case 5: detector(k, std::integral_constant<int, (RBW > 4 ? 5 : 0)>()); break;
+          case 6: detector(k, std::integral_constant<int, (RBW > 4 ? 6 : 0)>()); break;
+          case 7: detector(k, std::integral_constant<int, (RBW > 4 ? 7 : 0)>()); break;
+          default: detector(k, std::integral_constant<int, (RBW > 4 ? 8 : 0)>()); break;
         }
       }
+      mm_bar(bar_id, GTHR);                                      // the window is complete
 
-      // ---- time marginal from the registers
+      // ---- time marginal: NE window entries of one sample per thread
+      double x[NE];
+#pragma unroll
+      for (int e = 0; e < NE; ++e) x[e] = ld_shared_f64(rd_base + e * (JS * XP));
       float mf = -INFINITY;
 #pragma unroll
       for (int e = 0; e < NE; ++e)
-        if (jb + JS * e < n_x) mf = fmaxf(mf, __double2float_ru(x[e]));
+        if (e < nv) mf = fmaxf(mf, __double2float_ru(x[e]));
       mf = fmaxf(mf, __shfl_xor_sync(0xffffffffu, mf, 8));
       if (NT == 1) mf = fmaxf(mf, __shfl_xor_sync(0xffffffffu, mf, 16));
+      float *wmax = reinterpret_cast<float *>(grp + L.wmax) + buf * NBG * 16;
       if (jj == 0) wmax[n_mine * 16 + wg] = mf;
       mm_bar(bar_id, GTHR);
-      if (s_next < run_end) commit(buf ^ 1);                     // the other buffers were last read two barriers ago
       {
         const float4 *wm = reinterpret_cast<const float4 *>(wmax + n_mine * 16);
-        const float4 a0 = wm[0], a1 = wm[1], a2 = wm[2], a3 = wm[3];
+        const float4 a0 = wm[0], a1 = wm[1];
         mf = fmaxf(fmaxf(fmaxf(a0.x, a0.y), fmaxf(a0.z, a0.w)), fmaxf(fmaxf(a1.x, a1.y), fmaxf(a1.z, a1.w)));
-        mf = fmaxf(mf, fmaxf(fmaxf(fmaxf(a2.x, a2.y), fmaxf(a2.z, a2.w)), fmaxf(fmaxf(a3.x, a3.y), fmaxf(a3.z, a3.w))));
+        if (GW > 8) {
+          const float4 a2 = wm[2], a3 = wm[3];
+          mf = fmaxf(mf, fmaxf(fmaxf(fmaxf(a2.x, a2.y), fmaxf(a2.z, a2.w)), fmaxf(fmaxf(a3.x, a3.y), fmaxf(a3.z, a3.w))));
+        }
       }
-      const double cl2 = mc[n_mine] * 1.4426950408889634;
+      const double cl2 = reinterpret_cast<const double *>(meta)[n_mine] * 1.4426950408889634;
       const double mo = -(double)mf * cl2;
       double sum = 0.0;
 #pragma unroll
       for (int e = 0; e < NE; ++e)
-        if (jb + JS * e < n_x) sum += poly_exp2(fma(x[e], cl2, mo));
+        if (e < nv) sum += poly_exp2(fma(x[e], cl2, mo));
       sum += __shfl_xor_sync(0xffffffffu, sum, 8);
       if (NT == 1) sum += __shfl_xor_sync(0xffffffffu, sum, 16);
+      double *psum = reinterpret_cast<double *>(grp + L.psum) + buf * NBG * 16;
       if (jj == 0) psum[n_mine * 16 + wg] = sum;
+      // the warp that writes this batch's lnL (they take turns) reads c and q before the next batch's copies may land
+      const bool fin = wg == fin_w && lane < min(NBG, run_end - s0);
+      double fc = 0.0, fq = 0.0;
+      if (fin) {
+        fc = reinterpret_cast<const double *>(meta)[lane];
+        fq = reinterpret_cast<const double *>(meta)[NBG + lane];
+      }
+      if (s_next < run_end) commit(buf ^ 1);                     // the other coefficient buffer was last read a batch ago
       mm_bar(bar_id, GTHR);
-      if (gtid < (int)min((int64_t)NBG, run_end - s0)) {
-        float m = -INFINITY;
+      if (fin) {
         double sacc = 0.0;
 #pragma unroll
-        for (int w = 0; w < 16; ++w) {
-          m = fmaxf(m, wmax[gtid * 16 + w]);
-          sacc += psum[gtid * 16 + w];
-        }
-        A.lnL_out[b.g0 + s0 + gtid] = mc[gtid] * (double)m + log(sacc) - ln_ntau - mq[gtid];
+        for (int w = 0; w < (GW > 8 ? 16 : 8); ++w) sacc += psum[lane * 16 + w];
+        A.lnL_out[b.g0 + s0 + lane] = fc * (double)mf_of(wmax, lane, GW > 8) + log(sacc) - A.ln_ntau - fq;
       }
+      fin_w = fin_w + 1 == GW ? 0 : fin_w + 1;
     }
     if (!STREAM) mm_bar(3, MM_WARPS * 32);                       // both groups leave the run (and its Q block) together
     else mm_bar(bar_id, GTHR);
@@ -447,8 +468,7 @@ bool lnl_mma_finish_plan(MmaPlan &p) {
     }
   const int items = (nbg * 2 * p.K * p.M + gw * 32 - 1) / (gw * 32);
   p.pfn = (!p.stream && items <= 2) ? 2 : 0;
-  p.xb_rows = p.ne * js + 2 * p.H + 8;
-  if (p.xb_rows < p.n_t + 2 * p.H + 8) p.xb_rows = p.n_t + 2 * p.H + 8;
+  p.xb_rows = (p.ne * js > p.n_r ? p.ne * js : p.n_r) + (p.circular ? 0 : p.H) + 8;   // window rows (+ guard-band bias)
   return p.ne != 0 && p.n_r <= 8 * rbw * gw && p.H < p.n_t && p.K * nbg <= gw * 32 &&
          (p.stream || p.point_stride < (1ll << 20));
 }
@@ -468,6 +488,7 @@ cudaError_t launch_convert_q_mma(const double *Q_c128, void *dst, const MmaPlan 
 cudaError_t launch_lnl_mma(const MmaPlan &p, const void *q, const Batch &b, const Workspace &ws, double *lnL_out, int n_sm,
                            cudaStream_t s, int *n_launch) {
   if (b.n <= 0) return cudaSuccess;
+  if (b.n > 0x7fffffff) return cudaErrorInvalidValue;             // slots of a chunk are 32-bit inside the kernel
   MmaArgs a;
   a.p = p;
   a.L = mma_smem(p);
@@ -475,6 +496,7 @@ cudaError_t launch_lnl_mma(const MmaPlan &p, const void *q, const Batch &b, cons
   a.b = b;
   a.ws = ws;
   a.lnL_out = lnL_out;
+  a.ln_ntau = log((double)p.n_tau);
   if (n_launch) ++*n_launch;
   if (p.stream) return launch_ne<true, 0>(a, n_sm, s);
   return p.pfn == 2 ? launch_ne<false, 2>(a, n_sm, s) : launch_ne<false, 0>(a, n_sm, s);
