@@ -45,7 +45,7 @@ struct MmaShape {
   static constexpr int GW = STREAM ? 15 : 8;       // warps per group
   static constexpr int RBW = STREAM ? 4 : 8;       // row blocks (of 8 rows) per warp: wg + GW i
   static constexpr int GTHR = GW * 32;
-  static constexpr int XP = 64 * NT + 8;           // bytes per window row (8 pad bytes: 8 consecutive rows, 8 bank pairs)
+  static constexpr int XP = 64 * NT;               // bytes per window row (8-byte slots, swizzled: x_slot)
   static constexpr int RS = 8 * GW;                // rows between two tiles of a thread
   static constexpr int RPW = NT == 2 ? 2 : 4;      // window entries a warp reads per element index e
   static constexpr int JS = RPW * GW;              // ... a group
@@ -68,13 +68,28 @@ __device__ __forceinline__ void dmma(double (&d)[2], double a, double b) {
                : "d"(a), "d"(b));
 }
 
+// 8-byte slot of sample n inside window row r.  A tile column (8 consecutive rows of one sample, any start row) lands on 8
+// different bank pairs, and the four columns of one store / load instruction (samples 2 lc + h) split over both halves of the
+// 16 bank pairs: every scatter instruction is 2 wavefronts whatever the shifts are, and so is a reader's (a few full rows).
+// The slot depends on r mod 8 only: rows 8 apart share it, so tile i of a thread is base + immediate.
+template <int NT>
+__device__ __forceinline__ uint32_t x_slot(int r, int n) {
+  if (NT == 1) return (uint32_t)(n ^ ((r & 7) >> 1));            // bank pair 8 (r & 1) + slot
+  const int low = ((n >> 3) << 2) | (((n >> 2) & 1) << 1) | (n & 1);
+  return (uint32_t)((((n >> 1) & 1) << 3) | (low ^ (r & 7)));      // bank pair = slot
+}
+template <int NT>
+__device__ __forceinline__ uint32_t x_addr(uint32_t xb, int r, int n) {
+  return xb + (uint32_t)(r * (64 * NT)) + 8u * x_slot<NT>(r, n);
+}
+
 struct MmaSmem {                                   // byte offsets inside dynamic shared memory
   uint32_t bars, grp, grp_stride, coef_bytes, meta, meta_bytes, wmax, psum, xb, q, total;   // coef .. xb: inside a group block
 };
 
 __host__ __device__ inline MmaSmem mma_smem(const MmaPlan &p) {
   MmaSmem L;
-  const uint32_t nbg = p.stream ? 16u : 8u, groups = p.stream ? 1u : 2u, rb = p.stream ? 136u : 72u;
+  const uint32_t nbg = p.stream ? 16u : 8u, groups = p.stream ? 1u : 2u, rb = p.stream ? 128u : 64u;
   L.bars = 0;                                                          // full[8], empty[8], resident
   L.grp = 256;
   L.coef_bytes = (uint32_t)p.K * p.KS * nbg * 4 * 8;                   // cs[K][KS][NBG][4] doubles, two buffers at offset 0
@@ -172,15 +187,14 @@ __global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs
   const uint32_t a_base = (uint32_t)(lc >> 1) * (uint32_t)P.pitch_q + (uint32_t)(lc & 1) * 8u + (uint32_t)(8 * wg + lr) * 16u;
   const int nrb = 8 * wg < n_r ? (n_r - 8 * wg + 8 * GW - 1) / (8 * GW) : 0;   // valid row blocks of this warp (<= RBW)
   // scatter role: the thread holds P_k[t0 + RS i][8 nt + 2 lc + {0, 1}]; window row of stored row t and offset off:
-  // t - off (+- n_t on a circular window), + H on a guard-band window (off >= 0 there, nothing wraps: wrap_bytes 0)
+  // t - off (+- n_t on a circular window), + H on a guard-band window (off >= 0 there, nothing wraps: wrap_rows 0)
   const int t0 = 8 * wg + lr;
   const bool last_ok = t0 + RS * (nrb - 1) < n_t;                // a zero row past n_t would wrap onto another thread's element
-  const int wrap_bytes = P.circular ? n_t * XP : 0;
-  const uint32_t sc_base = xb_u32 + (uint32_t)((t0 + (P.circular ? 0 : H)) * XP + 2 * lc * 8);
+  const int wrap_rows = P.circular ? n_t : 0, row_bias = P.circular ? 0 : H;
   // window-reader role: sample n, window entries j = jb + JS e, e < nv
   const int n_mine = NT == 2 ? (((lane >> 4) << 3) | (lane & 7)) : (lane & 7);
   const int jj = NT == 2 ? ((lane >> 3) & 1) : (lane >> 3), jb = S::RPW * wg + jj;
-  const uint32_t rd_base = xb_u32 + (uint32_t)((jb + (P.circular ? 0 : H)) * XP + n_mine * 8);
+  const uint32_t rd_base = x_addr<NT>(xb_u32, jb + row_bias, n_mine);   // JS % 8 == 0: entry e is rd_base + e JS XP
   const int nv = min(NE, max(0, (n_x - jb + JS - 1) / JS));
 
   // coefficient items of this thread: element id = gtid + GTHR i of the [NBG][2 K M] block of a batch goes to the other
@@ -306,30 +320,43 @@ __global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs
           ++cnt, bs += NBG * 4, chunk += slot_bytes;
         };
         kstep(std::true_type());
+#pragma unroll 1
         for (int s = 1; s < KS; ++s) kstep(std::false_type());
         if (k > 0) mm_bar(bar_id, GTHR);                         // detector k - 1 is in the window (k = 0: the batch before is read)
         if (NRB > 0) {
 #pragma unroll
-          for (int nt = 0; nt < NT; ++nt)
+          for (int nt = 0; nt < NT; ++nt) {
+            uint32_t adr[2][NRB > 0 ? NRB : 1];
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
-              const int off = moff[k * NBG + 8 * nt + 2 * lc + h];
-              const uint32_t base = sc_base + (uint32_t)((8 * nt + h) * 8) - (uint32_t)(off * XP);
-              if (k == 0) {                                      // off = 0 (circular) or the guard-band offset: no wrap
+              const int n = 8 * nt + 2 * lc + h, off = moff[k * NBG + n];
+              // k = 0: off = 0 (circular) or the guard-band offset, no wrap.  k > 0: tiles i < thr use row r_lo + RS i, the
+              // others n_t rows less: off >= 0 wraps the first rows up, off < 0 the last rows down
+              const int num = (off >= 0 ? off : n_t + off) - t0;
+              const int thr = k == 0 ? NRB : (max(num, 0) + RS - 1) / RS;
+              const int r_lo = t0 + row_bias - off + (k > 0 && off >= 0 ? wrap_rows : 0);
+              const uint32_t b_lo = x_addr<NT>(xb_u32, r_lo, n), b_hi = x_addr<NT>(xb_u32, r_lo - wrap_rows, n);
 #pragma unroll
-                for (int i = 0; i < NRB; ++i) st_shared_f64(base + i * (RS * XP), acc[i][nt][h]);
-              } else {
-                // tiles i < thr use b_lo, the others b_lo - wrap: off >= 0 wraps the first rows up, off < 0 the last rows down
-                const int num = (off >= 0 ? off : n_t + off) - t0;
-                const int thr = (max(num, 0) + RS - 1) / RS;
-                const uint32_t b_lo = base + (off >= 0 ? (uint32_t)wrap_bytes : 0u), b_hi = b_lo - (uint32_t)wrap_bytes;
-#pragma unroll
-                for (int i = 0; i < NRB; ++i) {
-                  const uint32_t a = (i < thr ? b_lo : b_hi) + i * (RS * XP);
-                  if (i < NRB - 1 || last_ok) st_shared_f64(a, ld_shared_f64(a) + acc[i][nt][h]);
-                }
-              }
+              for (int i = 0; i < NRB; ++i) adr[h][i] = (i < thr ? b_lo : b_hi) + i * (RS * XP);
             }
+            if (k == 0) {
+#pragma unroll
+              for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int i = 0; i < NRB; ++i) st_shared_f64(adr[h][i], acc[i][nt][h]);
+            } else {                                             // all loads of the tile column first: one latency, not NRB
+              double v[2][NRB > 0 ? NRB : 1];
+#pragma unroll
+              for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int i = 0; i < NRB; ++i) v[h][i] = ld_shared_f64(adr[h][i]);
+#pragma unroll
+              for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int i = 0; i < NRB; ++i)
+                  if (i < NRB - 1 || last_ok) st_shared_f64(adr[h][i], v[h][i] + acc[i][nt][h]);
+            }
+          }
         }
       };
       for (int k = 0; k < K; ++k) {
@@ -350,11 +377,11 @@ __global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs
       // ---- time marginal: NE window entries of one sample per thread
       double x[NE];
 #pragma unroll
-      for (int e = 0; e < NE; ++e) x[e] = ld_shared_f64(rd_base + e * (JS * XP));
+      for (int e = 0; e < NE; ++e)
+        x[e] = ld_shared_f64(JS % 8 == 0 ? rd_base + e * (JS * XP) : x_addr<NT>(xb_u32, jb + row_bias + JS * e, n_mine));
       float mf = -INFINITY;
 #pragma unroll
-      for (int e = 0; e < NE; ++e)
-        if (e < nv) mf = fmaxf(mf, __double2float_ru(x[e]));
+      for (int e = 0; e < NE; ++e) mf = fmaxf(mf, e < nv ? __double2float_ru(x[e]) : -INFINITY);
       mf = fmaxf(mf, __shfl_xor_sync(0xffffffffu, mf, 8));
       if (NT == 1) mf = fmaxf(mf, __shfl_xor_sync(0xffffffffu, mf, 16));
       float *wmax = reinterpret_cast<float *>(grp + L.wmax) + buf * NBG * 16;
@@ -373,8 +400,10 @@ __global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs
       const double mo = -(double)mf * cl2;
       double sum = 0.0;
 #pragma unroll
-      for (int e = 0; e < NE; ++e)
-        if (e < nv) sum += poly_exp2(fma(x[e], cl2, mo));
+      for (int e = 0; e < NE; ++e) {                             // no branch: the NE polynomial chains interleave
+        const double pe = poly_exp2(fma(x[e], cl2, mo));
+        sum += e < nv ? pe : 0.0;
+      }
       sum += __shfl_xor_sync(0xffffffffu, sum, 8);
       if (NT == 1) sum += __shfl_xor_sync(0xffffffffu, sum, 16);
       double *psum = reinterpret_cast<double *>(grp + L.psum) + buf * NBG * 16;
