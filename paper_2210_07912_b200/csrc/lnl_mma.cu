@@ -68,15 +68,16 @@ __device__ __forceinline__ void dmma(double (&d)[2], double a, double b) {
                : "d"(a), "d"(b));
 }
 
-// 8-byte slot of sample n inside window row r.  A tile column (8 consecutive rows of one sample, any start row) lands on 8
-// different bank pairs, and the four columns of one store / load instruction (samples 2 lc + h) split over both halves of the
-// 16 bank pairs: every scatter instruction is 2 wavefronts whatever the shifts are, and so is a reader's (a few full rows).
-// The slot depends on r mod 8 only: rows 8 apart share it, so tile i of a thread is base + immediate.
+// 8-byte slot of sample n inside window row r.  Shared memory serves a 64-bit access half a warp at a time: for a scatter
+// instruction that is 4 consecutive rows (any start row, one per sample) of the 4 samples 2 lc + h.  The slot keeps the pair
+// index lc and swaps the rest with the row, so that those 16 accesses land on 16 different bank pairs whatever the shifts
+// are; a reader's half-warp takes whole rows.  The slot depends on r mod 4 only: rows 8 apart share it, so tile i of a
+// thread is base + immediate.
 template <int NT>
 __device__ __forceinline__ uint32_t x_slot(int r, int n) {
-  if (NT == 1) return (uint32_t)(n ^ ((r & 7) >> 1));            // bank pair 8 (r & 1) + slot
-  const int low = ((n >> 3) << 2) | (((n >> 2) & 1) << 1) | (n & 1);
-  return (uint32_t)((((n >> 1) & 1) << 3) | (low ^ (r & 7)));      // bank pair = slot
+  if (NT == 1) return (uint32_t)(n ^ ((r >> 1) & 1));            // bank pair 8 (r & 1) + 2 lc + (h ^ bit 1 of r)
+  const int lc = (n >> 1) & 3, rest = ((n >> 3) << 1) | (n & 1);  // n = 8 nt + 2 lc + h
+  return (uint32_t)(4 * lc + (rest ^ (r & 3)));                   // bank pair = slot
 }
 template <int NT>
 __device__ __forceinline__ uint32_t x_addr(uint32_t xb, int r, int n) {
@@ -192,8 +193,8 @@ __global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs
   const bool last_ok = t0 + RS * (nrb - 1) < n_t;                // a zero row past n_t would wrap onto another thread's element
   const int wrap_rows = P.circular ? n_t : 0, row_bias = P.circular ? 0 : H;
   // window-reader role: sample n, window entries j = jb + JS e, e < nv
-  const int n_mine = NT == 2 ? (((lane >> 4) << 3) | (lane & 7)) : (lane & 7);
-  const int jj = NT == 2 ? ((lane >> 3) & 1) : (lane >> 3), jb = S::RPW * wg + jj;
+  const int n_mine = lane & (NBG - 1);                             // half a warp reads whole rows
+  const int jj = lane / NBG, jb = S::RPW * wg + jj;
   const uint32_t rd_base = x_addr<NT>(xb_u32, jb + row_bias, n_mine);   // JS % 8 == 0: entry e is rd_base + e JS XP
   const int nv = min(NE, max(0, (n_x - jb + JS - 1) / JS));
 
@@ -382,8 +383,8 @@ __global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs
       float mf = -INFINITY;
 #pragma unroll
       for (int e = 0; e < NE; ++e) mf = fmaxf(mf, e < nv ? __double2float_ru(x[e]) : -INFINITY);
-      mf = fmaxf(mf, __shfl_xor_sync(0xffffffffu, mf, 8));
-      if (NT == 1) mf = fmaxf(mf, __shfl_xor_sync(0xffffffffu, mf, 16));
+      if (NT == 1) mf = fmaxf(mf, __shfl_xor_sync(0xffffffffu, mf, 8));
+      mf = fmaxf(mf, __shfl_xor_sync(0xffffffffu, mf, 16));
       float *wmax = reinterpret_cast<float *>(grp + L.wmax) + buf * NBG * 16;
       if (jj == 0) wmax[n_mine * 16 + wg] = mf;
       mm_bar(bar_id, GTHR);
@@ -404,8 +405,8 @@ __global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs
         const double pe = poly_exp2(fma(x[e], cl2, mo));
         sum += e < nv ? pe : 0.0;
       }
-      sum += __shfl_xor_sync(0xffffffffu, sum, 8);
-      if (NT == 1) sum += __shfl_xor_sync(0xffffffffu, sum, 16);
+      if (NT == 1) sum += __shfl_xor_sync(0xffffffffu, sum, 8);
+      sum += __shfl_xor_sync(0xffffffffu, sum, 16);
       double *psum = reinterpret_cast<double *>(grp + L.psum) + buf * NBG * 16;
       if (jj == 0) psum[n_mine * 16 + wg] = sum;
       // the warp that writes this batch's lnL (they take turns) reads c and q before the next batch's copies may land
