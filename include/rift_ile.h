@@ -144,6 +144,23 @@ int rift_ile_reduce(rift_ile_t *h, int32_t n_seg, int64_t n_per_seg, const doubl
                     const double hi[RIFT_N_PARAMS], int32_t n_bins, int32_t merge, double *lnZ, double *rel_err,
                     double *n_eff, double *n_ess, double *hist, void *cuda_stream);
 
+/* Allocation-free variant of the reduce (step a8, Eq. (3) and App. B as above) for callers that cannot call cudaMalloc:
+ * code under CUDA-graph capture, tight serving loops, harnesses that forbid it.  No handle, scalar outputs only, no pooling
+ * with earlier calls (merge = 0), no histograms; it calls no cudaMalloc / cudaFree / allocating routine and does not
+ * synchronise.  Its scratch (per-block partial states, per-segment states) is a file-scope device array of 160 KiB that
+ * every GPU loading the library holds until exit; hence the limit n_seg <= RIFT_REDUCE_STATIC_MAX_SEG (RIFT_EINVAL beyond,
+ * with the reason in rift_ile_reduce_static_error()).
+ *   lnL, ln_weight (NULL = 0) : DEVICE fp64 [n_seg][n_per_seg] on the CURRENT device.
+ *   out : DEVICE fp64 [4][n_seg] = lnZ, rel_err, n_eff, n_ess per segment, complete when cuda_stream is.
+ * Every call on a device shares the one array (it keeps the last call's contents; nothing in it needs clearing, every slot
+ * that is read is written first by the same call): calls that overlap on the GPU (different streams, or graphs replayed
+ * concurrently) race -- serialise them.  Results are bit-identical to rift_ile_reduce(merge = 0). */
+#define RIFT_REDUCE_STATIC_MAX_SEG 1024
+int rift_ile_reduce_static(int32_t n_seg, int64_t n_per_seg, const double *lnL, const double *ln_weight, double *out,
+                           void *cuda_stream);
+/* Reason of the calling thread's last rift_ile_reduce_static failure ("" after a success). */
+const char *rift_ile_reduce_static_error(void);
+
 /* Inspection of the geometry kernel (steps a1-a5) in fp64 for n samples of ONE intrinsic point.
  * All outputs DEVICE, any may be NULL: F [n][n_det] complex128 (F+ + i Fx); Y [n][n_modes] complex128
  * (-2Y_lm(iota,-phi_ref)); shift [n][n_det] int32; quad [n] fp64 (the U/V term of Eq. (D3) including

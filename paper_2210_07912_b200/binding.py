@@ -28,7 +28,8 @@ EXPORTS = ("rift_ile_create", "rift_ile_eval_batch", "rift_ile_reduce", "rift_il
            "rift_ile_launch_count", "rift_ile_kernel_name", "rift_ile_profile", "rift_ile_profile_read",
            "rift_ile_fma_peak", "rift_ile_set_option", "rift_ile_reserve", "rift_ile_eval_batch_host",
            "rift_ile_staged", "rift_ile_eval_batch_dmarg", "rift_ile_precompute", "rift_ile_destroy",
-           "rift_ile_strerror", "rift_ile_last_error")
+           "rift_ile_strerror", "rift_ile_last_error", "rift_ile_reduce_static", "rift_ile_reduce_static_error")
+RIFT_REDUCE_STATIC_MAX_SEG = 1024
 AC_EXPORTS = ("rift_ac_create", "rift_ac_draw", "rift_ac_update", "rift_ac_update_dims", "rift_ac_get_masses",
               "rift_ac_ile_ln_weight", "rift_ac_destroy")
 
@@ -112,6 +113,10 @@ def lib() -> C.CDLL:
         L.rift_ile_strerror.restype = C.c_char_p
         L.rift_ile_last_error.argtypes = [vp]
         L.rift_ile_last_error.restype = C.c_char_p
+        L.rift_ile_reduce_static.argtypes = [i32, i64, vp, vp, vp, vp]
+        L.rift_ile_reduce_static.restype = C.c_int
+        L.rift_ile_reduce_static_error.argtypes = []
+        L.rift_ile_reduce_static_error.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -253,6 +258,14 @@ def rift_ile_reduce(h, n_seg: int, n_per_seg: int, lnL, ln_weight=None, params=N
                                  None if params is None else _params6(params), _ptr(lo_), _ptr(hi_), int(n_bins),
                                  int(merge), *[o.ctypes.data for o in out], _ptr(hist), int(cuda_stream) or None), h)
     return dict(lnZ=out[0], rel_err=out[1], n_eff=out[2], n_ess=out[3], hist=hist)
+
+
+def rift_ile_reduce_static(n_seg: int, n_per_seg: int, lnL, ln_weight, out, cuda_stream: int = 0) -> None:
+    """Allocation-free reduce: out is a DEVICE fp64 [4][n_seg] array (lnZ, rel_err, n_eff, n_ess), filled asynchronously."""
+    rc = lib().rift_ile_reduce_static(int(n_seg), int(n_per_seg), _ptr(lnL), _ptr(ln_weight), _ptr(out),
+                                      int(cuda_stream) or None)
+    if rc != RIFT_OK:
+        raise RiftError(rc, f"{lib().rift_ile_strerror(rc).decode()} ({lib().rift_ile_reduce_static_error().decode()})")
 
 
 def rift_ile_set_kernel(h, variant: int) -> None:

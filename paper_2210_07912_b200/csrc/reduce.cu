@@ -4,6 +4,9 @@
 //   weighted 1-D histograms per parameter (Eq. (22), reading A13).
 // Two kernels: per-block partial states (block max, sums and histograms relative to the block max; warp-shuffle
 // reductions), then one block per segment merges the partials with the stored state (Eq. (20)-(21): pooled sums).
+#include <cstdio>
+#include <mutex>
+
 #include "rift_internal.h"
 
 namespace {
@@ -257,4 +260,73 @@ cudaError_t launch_reduce(int32_t n_seg, int64_t n_per_seg, const double *lnL, c
                                             hp ? state_hist : nullptr, out_scalars, hp ? out_hist : nullptr);
   if (n_launch) *n_launch += 2;
   return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------ allocation-free reduce
+// rift_ile_reduce_static (include/rift_ile.h): the same two kernels as launch_reduce, scalar outputs only, with the
+// per-block partial states and the per-segment state in a file-scope device array instead of buffers owned by a handle, so
+// that the call allocates nothing (CUDA-graph capture, serving loops, harnesses that forbid cudaMalloc).  Every GPU that
+// loads the library holds the array (160 KiB) until the process exits.  In host code `g_static_scratch` is only a stand-in
+// for the symbol: the device address comes from cudaGetSymbolAddress, once per device with that device current.
+
+namespace {
+
+constexpr int STATIC_MAX_SEG = RIFT_REDUCE_STATIC_MAX_SEG;          // per-segment states
+constexpr int STATIC_MAX_BLOCKS = 4096;                             // partial blocks over all segments (reduce_blocks_per_seg)
+constexpr size_t STATIC_STATE_DOUBLES = (size_t)STATIC_MAX_SEG * sizeof(ReduceState) / sizeof(double);
+constexpr size_t STATIC_DOUBLES = STATIC_STATE_DOUBLES + (size_t)STATIC_MAX_BLOCKS * PARTIAL_HDR;
+static_assert(sizeof(ReduceState) % sizeof(double) == 0, "ReduceState is a whole number of doubles");
+static_assert(STATIC_MAX_SEG <= STATIC_MAX_BLOCKS, "one partial block per segment at least");
+
+static __device__ __align__(256) double g_static_scratch[STATIC_DOUBLES];   // [state | partial]
+
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mutex;
+double *g_static_ptr[STATIC_MAX_DEVICES] = {};                       // device address of g_static_scratch, per device
+thread_local char g_static_error[160] = "";
+
+int static_fail(int code, const char *msg) {
+  snprintf(g_static_error, sizeof(g_static_error), "%s", msg);
+  return code;
+}
+
+}  // namespace
+
+extern "C" const char *rift_ile_reduce_static_error(void) { return g_static_error; }
+
+extern "C" int rift_ile_reduce_static(int32_t n_seg, int64_t n_per_seg, const double *lnL, const double *ln_weight,
+                                      double *out, void *cuda_stream) {
+  g_static_error[0] = 0;
+  if (n_seg < 1 || n_per_seg < 0) return static_fail(RIFT_EINVAL, "bad n_seg / n_per_seg");
+  if (n_seg > STATIC_MAX_SEG)
+    return static_fail(RIFT_EINVAL, "n_seg exceeds RIFT_REDUCE_STATIC_MAX_SEG (1024): the static scratch array holds no more "
+                                    "segment states; use rift_ile_reduce");
+  if ((n_per_seg > 0 && !lnL) || !out) return static_fail(RIFT_EINVAL, "null pointer");
+  const int32_t bps = reduce_blocks_per_seg(n_per_seg, n_seg);
+  if ((int64_t)bps * n_seg > STATIC_MAX_BLOCKS) return static_fail(RIFT_EINVAL, "partial blocks exceed the static scratch array");
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= STATIC_MAX_DEVICES)
+    return static_fail(RIFT_ECUDA, "cudaGetDevice failed or device ordinal >= 64");
+  double *scratch = nullptr;
+  {
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[dev]) {                                        // set-up, once per device, that device current
+      void *p = nullptr;
+      const cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);
+      if (e != cudaSuccess || !p) {
+        cudaGetLastError();
+        return static_fail(RIFT_ECUDA, "cudaGetSymbolAddress(g_static_scratch) failed");
+      }
+      g_static_ptr[dev] = static_cast<double *>(p);
+    }
+    scratch = g_static_ptr[dev];
+  }
+  // merge = 0: the merge kernel overwrites the segment states without reading them and the partial kernel writes every
+  // partial slot the merge kernel reads, so nothing of the previous call's contents is used and nothing needs clearing
+  ReduceState *state = reinterpret_cast<ReduceState *>(scratch);
+  double *partial = scratch + STATIC_STATE_DOUBLES;
+  const cudaError_t e = launch_reduce(n_seg, n_per_seg, lnL, ln_weight, nullptr, nullptr, nullptr, 0, 0, state, nullptr, partial,
+                                      bps, out, nullptr, reinterpret_cast<cudaStream_t>(cuda_stream), nullptr);
+  if (e != cudaSuccess) return static_fail(RIFT_ECUDA, cudaGetErrorString(e));
+  return RIFT_OK;
 }
