@@ -161,6 +161,14 @@ int rift_ile_reduce_static(int32_t n_seg, int64_t n_per_seg, const double *lnL, 
 /* Reason of the calling thread's last rift_ile_reduce_static failure ("" after a success). */
 const char *rift_ile_reduce_static_error(void);
 
+/* rho_guess of every intrinsic point, Eq. (D7) read as SURVEY.md A14 (the printed ratio is inverted):
+ *   (2.3 rho_guess)^2 = sum_k sum_lm max_t |Q_{k,lm}(t)|^2 / |U_{k,lm,lm}|   (terms with U_{k,lm,lm} = 0 left out),
+ * the amplitude estimate from which the paper sets the overflow offset O ~ rho_guess^2 / 2 - O(few) (:797) -- this library
+ * works with logarithms throughout and needs no offset; the number is for the caller's sampler settings.  Computed on the
+ * device from the handle's copies of Q (as stored: complex64 storage gives fp32 accuracy) and U.
+ *   rho_guess : HOST [n_points].  Synchronous (allocates and frees a small device buffer). */
+int rift_ile_rho_guess(rift_ile_t *h, double *rho_guess);
+
 /* Inspection of the geometry kernel (steps a1-a5) in fp64 for n samples of ONE intrinsic point.
  * All outputs DEVICE, any may be NULL: F [n][n_det] complex128 (F+ + i Fx); Y [n][n_modes] complex128
  * (-2Y_lm(iota,-phi_ref)); shift [n][n_det] int32; quad [n] fp64 (the U/V term of Eq. (D3) including

@@ -28,7 +28,9 @@ EXPORTS = ("rift_ile_create", "rift_ile_eval_batch", "rift_ile_reduce", "rift_il
            "rift_ile_launch_count", "rift_ile_kernel_name", "rift_ile_profile", "rift_ile_profile_read",
            "rift_ile_fma_peak", "rift_ile_set_option", "rift_ile_reserve", "rift_ile_eval_batch_host",
            "rift_ile_staged", "rift_ile_eval_batch_dmarg", "rift_ile_precompute", "rift_ile_destroy",
-           "rift_ile_strerror", "rift_ile_last_error", "rift_ile_reduce_static", "rift_ile_reduce_static_error")
+           "rift_ile_strerror", "rift_ile_last_error", "rift_ile_reduce_static", "rift_ile_reduce_static_error",
+           "rift_ile_rho_guess")
+SKY_EXPORTS = ("rift_sky_network_frame", "rift_sky_network_to_radec", "rift_sky_radec_to_network")
 RIFT_REDUCE_STATIC_MAX_SEG = 1024
 AC_EXPORTS = ("rift_ac_create", "rift_ac_draw", "rift_ac_update", "rift_ac_update_dims", "rift_ac_get_masses",
               "rift_ac_ile_ln_weight", "rift_ac_destroy")
@@ -113,6 +115,14 @@ def lib() -> C.CDLL:
         L.rift_ile_strerror.restype = C.c_char_p
         L.rift_ile_last_error.argtypes = [vp]
         L.rift_ile_last_error.restype = C.c_char_p
+        L.rift_ile_rho_guess.argtypes = [vp, vp]
+        L.rift_ile_rho_guess.restype = C.c_int
+        L.rift_sky_network_frame.argtypes = [vp, vp, vp]
+        L.rift_sky_network_frame.restype = C.c_int
+        L.rift_sky_network_to_radec.argtypes = [i64, vp, dbl, vp, vp, vp, vp, vp]
+        L.rift_sky_network_to_radec.restype = C.c_int
+        L.rift_sky_radec_to_network.argtypes = [i64, vp, dbl, vp, vp, vp, vp, vp]
+        L.rift_sky_radec_to_network.restype = C.c_int
         L.rift_ile_reduce_static.argtypes = [i32, i64, vp, vp, vp, vp]
         L.rift_ile_reduce_static.restype = C.c_int
         L.rift_ile_reduce_static_error.argtypes = []
@@ -266,6 +276,34 @@ def rift_ile_reduce_static(n_seg: int, n_per_seg: int, lnL, ln_weight, out, cuda
                                       int(cuda_stream) or None)
     if rc != RIFT_OK:
         raise RiftError(rc, f"{lib().rift_ile_strerror(rc).decode()} ({lib().rift_ile_reduce_static_error().decode()})")
+
+
+def rift_ile_rho_guess(h, n_points: int) -> np.ndarray:
+    """rho_guess [n_points] (Eq. (D7), reading A14)."""
+    out = np.empty(int(n_points), dtype=np.float64)
+    _check(lib().rift_ile_rho_guess(h, out.ctypes.data), h)
+    return out
+
+
+def rift_sky_network_frame(loc_a_m, loc_b_m) -> np.ndarray:
+    """R [3][3] (columns x', y', z') of the frame whose pole points from detector a to detector b."""
+    a = np.ascontiguousarray(loc_a_m, dtype=np.float64)
+    b = np.ascontiguousarray(loc_b_m, dtype=np.float64)
+    R = np.empty((3, 3), dtype=np.float64)
+    _check(lib().rift_sky_network_frame(a.ctypes.data, b.ctypes.data, R.ctypes.data))
+    return R
+
+
+def rift_sky_network_to_radec(n: int, R, gmst_rad: float, lam, beta, ra, dec, cuda_stream: int = 0) -> None:
+    R_ = np.ascontiguousarray(R, dtype=np.float64)
+    _check(lib().rift_sky_network_to_radec(int(n), R_.ctypes.data, float(gmst_rad), _ptr(lam), _ptr(beta), _ptr(ra), _ptr(dec),
+                                           int(cuda_stream) or None))
+
+
+def rift_sky_radec_to_network(n: int, R, gmst_rad: float, ra, dec, lam, beta, cuda_stream: int = 0) -> None:
+    R_ = np.ascontiguousarray(R, dtype=np.float64)
+    _check(lib().rift_sky_radec_to_network(int(n), R_.ctypes.data, float(gmst_rad), _ptr(ra), _ptr(dec), _ptr(lam), _ptr(beta),
+                                           int(cuda_stream) or None))
 
 
 def rift_ile_set_kernel(h, variant: int) -> None:

@@ -1360,6 +1360,23 @@ int rift_ile_precompute(int32_t n_points, int32_t n_det, int32_t n_modes, int32_
   return e == cudaSuccess ? RIFT_OK : RIFT_ECUDA;
 }
 
+int rift_ile_rho_guess(rift_ile_t *h, double *rho_guess) {
+  if (!h) return RIFT_EINVAL;
+  if (!rho_guess) return fail(h, RIFT_EINVAL, "null pointer");
+  DeviceGuard g(h->device);
+  double *d_out = nullptr;
+  if (cudaMalloc(&d_out, sizeof(double) * h->P) != cudaSuccess) {
+    cudaGetLastError();
+    return fail(h, RIFT_ENOMEM, "cudaMalloc failed");
+  }
+  cudaError_t e = launch_rho_guess(h->qs, h->q_storage == RIFT_Q_C64, h->d_U, h->P, h->K, h->M, d_out, 0);
+  ++h->launches;
+  if (e == cudaSuccess) e = cudaMemcpy(rho_guess, d_out, sizeof(double) * h->P, cudaMemcpyDeviceToHost);
+  cudaFree(d_out);
+  if (e != cudaSuccess) return fail(h, RIFT_ECUDA, cudaGetErrorString(e));
+  return RIFT_OK;
+}
+
 int rift_ile_profile(rift_ile_t *h, int32_t enable) {
   if (!h) return RIFT_EINVAL;
   h->profiling = enable != 0;

@@ -166,6 +166,9 @@ cudaError_t launch_geometry(const DetGeom &g, const ModeEntry *modes, const Batc
                             int32_t *shift_out, double *dbg_F, double *dbg_Y, const int32_t *perm, cudaStream_t s);
 cudaError_t launch_build_quad_uv(const QuadProg &qp, const double *U, const double *V, int32_t P, int32_t K, int32_t M,
                                  double2 *uv_out, cudaStream_t s);
+// sky_frame.cu
+cudaError_t launch_rho_guess(const QStore &q, bool q_fp32, const double *U, int32_t P, int32_t K, int32_t M, double *out,
+                             cudaStream_t s);
 // lnl_direct.cu
 size_t lnl_direct_smem_bytes(const QStore &q, bool fp32, bool q_in_smem);
 cudaError_t launch_lnl_direct(const QStore &q, bool fp32, bool q_in_smem, bool q_ext, const Batch &b, const Workspace &ws,

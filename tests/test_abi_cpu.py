@@ -27,6 +27,17 @@ def test_library_builds_and_exports_every_declared_symbol():
     assert declared_ac == set(binding.AC_EXPORTS), declared_ac ^ set(binding.AC_EXPORTS)
     for name in declared_ac:
         assert hasattr(L, name), name
+    header_sky = open(os.path.join(ROOT, "include", "rift_sky.h")).read()
+    declared_sky = set(re.findall(r"\b(rift_sky_[a-z_]+)\s*\(", header_sky))
+    assert declared_sky == set(binding.SKY_EXPORTS), declared_sky ^ set(binding.SKY_EXPORTS)
+    for name in declared_sky:
+        assert hasattr(L, name), name
+    # the frame is host arithmetic: checked here against its definition (pole = baseline, right-handed, x' equatorial)
+    R = binding.rift_sky_network_frame([1.0, 2.0, 3.0], [4.0, 0.0, 5.0])
+    z = np.array([3.0, -2.0, 2.0]) / np.sqrt(17.0)
+    assert np.allclose(R[:, 2], z) and np.allclose(R.T @ R, np.eye(3)) and abs(np.linalg.det(R) - 1) < 1e-14 and R[2, 0] == 0.0
+    with pytest.raises(binding.RiftError):
+        binding.rift_sky_network_frame([1.0, 2.0, 3.0], [1.0, 2.0, 3.0])
 
 
 def test_strerror_and_invalid_arguments_without_gpu():
