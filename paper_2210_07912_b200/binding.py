@@ -30,6 +30,9 @@ EXPORTS = ("rift_ile_create", "rift_ile_eval_batch", "rift_ile_reduce", "rift_il
            "rift_ile_staged", "rift_ile_eval_batch_dmarg", "rift_ile_precompute", "rift_ile_destroy",
            "rift_ile_strerror", "rift_ile_last_error", "rift_ile_reduce_static", "rift_ile_reduce_static_error",
            "rift_ile_rho_guess")
+GMM_EXPORTS = ("rift_gmm_create", "rift_gmm_set_model", "rift_gmm_get_model", "rift_gmm_fit", "rift_gmm_draw",
+               "rift_gmm_ln_density", "rift_gmm_box_mass", "rift_gmm_destroy")
+RIFT_GMM_MAX_COMP, RIFT_GMM_MAX_TRIES = 8, 64
 SKY_EXPORTS = ("rift_sky_network_frame", "rift_sky_network_to_radec", "rift_sky_radec_to_network")
 RIFT_REDUCE_STATIC_MAX_SEG = 1024
 AC_EXPORTS = ("rift_ac_create", "rift_ac_draw", "rift_ac_update", "rift_ac_update_dims", "rift_ac_get_masses",
@@ -115,6 +118,16 @@ def lib() -> C.CDLL:
         L.rift_ile_strerror.restype = C.c_char_p
         L.rift_ile_last_error.argtypes = [vp]
         L.rift_ile_last_error.restype = C.c_char_p
+        L.rift_gmm_create.argtypes = [i32, i32, vp, vp, C.POINTER(vp)]
+        L.rift_gmm_set_model.argtypes = [vp, vp, vp, vp, dbl]
+        L.rift_gmm_get_model.argtypes = [vp, vp, vp, vp, C.POINTER(dbl)]
+        L.rift_gmm_fit.argtypes = [vp, i64, C.POINTER(vp), vp, i32, dbl, dbl, i32, C.POINTER(i32), C.POINTER(dbl), vp]
+        L.rift_gmm_draw.argtypes = [vp, i64, C.c_uint64, C.c_uint64, C.POINTER(vp), vp, C.POINTER(i64), vp]
+        L.rift_gmm_ln_density.argtypes = [vp, i64, C.POINTER(vp), vp, vp]
+        L.rift_gmm_box_mass.argtypes = [vp, vp]
+        L.rift_gmm_destroy.argtypes = [vp]
+        for name in GMM_EXPORTS:
+            getattr(L, name).restype = C.c_int
         L.rift_ile_rho_guess.argtypes = [vp, vp]
         L.rift_ile_rho_guess.restype = C.c_int
         L.rift_sky_network_frame.argtypes = [vp, vp, vp]
@@ -276,6 +289,75 @@ def rift_ile_reduce_static(n_seg: int, n_per_seg: int, lnL, ln_weight, out, cuda
                                       int(cuda_stream) or None)
     if rc != RIFT_OK:
         raise RiftError(rc, f"{lib().rift_ile_strerror(rc).decode()} ({lib().rift_ile_reduce_static_error().decode()})")
+
+
+class GmmHandle:
+    """Opaque rift_gmm_t* with the shape needed to marshal arrays."""
+    def __init__(self, ptr, n_dim, n_comp):
+        self.ptr, self.n_dim, self.n_comp = ptr, n_dim, n_comp
+
+
+def _xptrs(g: "GmmHandle", x):
+    if len(x) != g.n_dim:
+        raise ValueError("x must hold one device array per dimension")
+    return (C.c_void_p * g.n_dim)(*[_ptr(v) for v in x])
+
+
+def rift_gmm_create(n_dim: int, n_comp: int, lo, hi) -> GmmHandle:
+    lo_ = np.ascontiguousarray(lo, dtype=np.float64)
+    hi_ = np.ascontiguousarray(hi, dtype=np.float64)
+    if lo_.size != n_dim or hi_.size != n_dim:
+        raise ValueError("lo, hi must have n_dim entries")
+    out = C.c_void_p()
+    _check(lib().rift_gmm_create(int(n_dim), int(n_comp), lo_.ctypes.data, hi_.ctypes.data, C.byref(out)))
+    return GmmHandle(out, int(n_dim), int(n_comp))
+
+
+def rift_gmm_set_model(g: GmmHandle, mu, cov, pi, n_trained: float = 0.0) -> None:
+    mu_ = np.ascontiguousarray(mu, dtype=np.float64).reshape(g.n_comp, g.n_dim)
+    cov_ = np.ascontiguousarray(cov, dtype=np.float64).reshape(g.n_comp, g.n_dim, g.n_dim)
+    pi_ = np.ascontiguousarray(pi, dtype=np.float64).reshape(g.n_comp)
+    _check(lib().rift_gmm_set_model(g.ptr, mu_.ctypes.data, cov_.ctypes.data, pi_.ctypes.data, float(n_trained)))
+
+
+def rift_gmm_get_model(g: GmmHandle):
+    """(mu [K][d], cov [K][d][d], pi [K], n_trained)."""
+    mu = np.empty((g.n_comp, g.n_dim))
+    cov = np.empty((g.n_comp, g.n_dim, g.n_dim))
+    pi = np.empty(g.n_comp)
+    nt = C.c_double()
+    _check(lib().rift_gmm_get_model(g.ptr, mu.ctypes.data, cov.ctypes.data, pi.ctypes.data, C.byref(nt)))
+    return mu, cov, pi, nt.value
+
+
+def rift_gmm_fit(g: GmmHandle, n: int, x, ln_w, n_iter: int, tol: float = 0.0, reg: float = 0.0, merge: int = 0,
+                 cuda_stream: int = 0):
+    """EM on device arrays x (one per dimension) with log-weights ln_w (or None); returns (iterations done, ln L)."""
+    it, ll = C.c_int32(), C.c_double()
+    _check(lib().rift_gmm_fit(g.ptr, int(n), _xptrs(g, x), _ptr(ln_w), int(n_iter), float(tol), float(reg), int(merge),
+                              C.byref(it), C.byref(ll), int(cuda_stream) or None))
+    return it.value, ll.value
+
+
+def rift_gmm_draw(g: GmmHandle, n: int, seed: int, offset: int, x, ln_ps=None, want_failed: bool = False, cuda_stream: int = 0):
+    nf = C.c_int64(0)
+    _check(lib().rift_gmm_draw(g.ptr, int(n), int(seed), int(offset), _xptrs(g, x), _ptr(ln_ps),
+                               C.byref(nf) if want_failed else None, int(cuda_stream) or None))
+    return nf.value if want_failed else None
+
+
+def rift_gmm_ln_density(g: GmmHandle, n: int, x, ln_ps, cuda_stream: int = 0) -> None:
+    _check(lib().rift_gmm_ln_density(g.ptr, int(n), _xptrs(g, x), _ptr(ln_ps), int(cuda_stream) or None))
+
+
+def rift_gmm_box_mass(g: GmmHandle) -> np.ndarray:
+    Z = np.empty(g.n_comp)
+    _check(lib().rift_gmm_box_mass(g.ptr, Z.ctypes.data))
+    return Z
+
+
+def rift_gmm_destroy(g: GmmHandle) -> None:
+    _check(lib().rift_gmm_destroy(g.ptr))
 
 
 def rift_ile_rho_guess(h, n_points: int) -> np.ndarray:

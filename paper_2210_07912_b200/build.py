@@ -21,7 +21,7 @@ INCLUDE = os.path.join(ROOT, "include")
 LIB = os.path.join(HERE, "librift_ile.so")
 OBJ_DIR = os.path.join(HERE, "build")
 SOURCES = ["api.cu", "geometry.cu", "lnl_direct.cu", "lnl_direct_ext.cu", "lnl_tc.cu", "lnl_tcs.cu", "lnl_mma.cu", "lnl_sky.cu", "lnl_sky64.cu", "sky_sort.cu",
-           "reduce.cu", "convert.cu", "precompute.cu", "ac.cu", "sky_frame.cu"]
+           "reduce.cu", "convert.cu", "precompute.cu", "ac.cu", "sky_frame.cu", "gmm.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall", "-I", INCLUDE, "-I", CSRC]
 

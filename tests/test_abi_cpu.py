@@ -32,6 +32,11 @@ def test_library_builds_and_exports_every_declared_symbol():
     assert declared_sky == set(binding.SKY_EXPORTS), declared_sky ^ set(binding.SKY_EXPORTS)
     for name in declared_sky:
         assert hasattr(L, name), name
+    header_gmm = open(os.path.join(ROOT, "include", "rift_gmm.h")).read()
+    declared_gmm = set(re.findall(r"\b(rift_gmm_[a-z_]+)\s*\(", header_gmm))
+    assert declared_gmm == set(binding.GMM_EXPORTS), declared_gmm ^ set(binding.GMM_EXPORTS)
+    for name in declared_gmm:
+        assert hasattr(L, name), name
     # the frame is host arithmetic: checked here against its definition (pole = baseline, right-handed, x' equatorial)
     R = binding.rift_sky_network_frame([1.0, 2.0, 3.0], [4.0, 0.0, 5.0])
     z = np.array([3.0, -2.0, 2.0]) / np.sqrt(17.0)

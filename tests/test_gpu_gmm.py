@@ -1,0 +1,192 @@
+"""GPU parity of the Gaussian-mixture adaptive sampler (include/rift_gmm.h, PAPER.md section
+IV.C.1 and Appendix A) against oracle/gmm_oracle.py on the same seeded inputs: EM iteration by iteration, the online merge, the
+component masses, the density, the truncated draws (same counter-based random numbers), and an adaptive integration loop."""
+import math
+
+import numpy as np
+import pytest
+
+import paper_2210_07912_b200 as rift
+from oracle import gmm_oracle as go
+
+pytestmark = pytest.mark.gpu
+
+TOL_EM = 1e-9                # sums of 1e4-1e5 terms in another order, then divisions (relative, on means / covariances / weights)
+TOL_DRAW = 1e-11             # normcdfinv vs scipy's ndtri through A z + mu (absolute, on O(1) coordinates)
+TOL_LNP = 1e-9               # ln p_s: the component masses Z_k by Gauss-Legendre vs adaptive quadrature
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    assert t.cuda.is_available(), "GPU tests need a CUDA device"
+    rift.lib()
+    return t
+
+
+def _dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _data(rng, n, d):
+    mus = [np.array([-1.0, 0.5])[:d], np.array([1.5, 1.2])[:d], np.array([0.3, -0.8])[:d]]
+    covs = [np.array([[0.4, 0.25], [0.25, 0.3]])[:d, :d], np.array([[0.15, -0.05], [-0.05, 0.5]])[:d, :d], np.eye(2)[:d, :d] * 0.1]
+    k = rng.choice(3, size=n, p=[0.5, 0.3, 0.2])
+    x = np.stack([rng.multivariate_normal(mus[j], covs[j]) for j in k])
+    return x
+
+
+def _init(d):
+    mu0 = np.array([[-0.5, 0.0], [1.0, 1.0], [0.0, -0.5]])[:, :d]
+    cov0 = np.array([np.eye(d) * 0.5] * 3)
+    return mu0, cov0, np.array([0.3, 0.4, 0.3])
+
+
+@pytest.mark.parametrize("d,n,weighted", [(2, 60_001, True), (1, 4_099, True), (2, 777, False)])
+def test_em_matches_oracle_iteration_by_iteration(torch, d, n, weighted):
+    rng = np.random.default_rng(100 + n)
+    x = _data(rng, n, d)
+    ln_w = rng.normal(0.0, 2.0, n) + 700.0 if weighted else None            # a large common offset must not matter
+    if weighted:
+        ln_w[5] = -np.inf
+        ln_w[6] = np.nan                                                     # treated as weight 0
+    lo, hi = x.min(axis=0) - 1.0, x.max(axis=0) + 1.0
+    mu0, cov0, pi0 = _init(d)
+    xs = [_dev(torch, x[:, j]) for j in range(d)]
+    lw = None if ln_w is None else _dev(torch, ln_w)
+    lw_o = np.zeros(n) if ln_w is None else np.where(np.isnan(ln_w), -np.inf, ln_w)
+    for iters, reg in ((1, 0.0), (4, 1e-6), (9, 0.0)):
+        g = rift.rift_gmm_create(d, 3, lo, hi)
+        rift.rift_gmm_set_model(g, mu0, cov0, pi0)
+        it, ll = rift.rift_gmm_fit(g, n, xs, lw, iters, 0.0, reg)
+        mu, cov, pi, nt = rift.rift_gmm_get_model(g)
+        mu_o, cov_o, pi_o, it_o, ll_o = go.fit(x, lw_o, mu0, cov0, pi0, iters, 0.0, reg)
+        assert it == it_o == iters and nt == n
+        assert abs(ll - ll_o) < TOL_EM * max(1.0, abs(ll_o))
+        assert np.max(np.abs(mu - mu_o)) < TOL_EM and np.max(np.abs(cov - cov_o)) < TOL_EM and np.max(np.abs(pi - pi_o)) < TOL_EM
+        rift.rift_gmm_destroy(g)
+    # the tolerance stops both at the same iteration, and repeating the call gives the same bits (fixed reduction order)
+    g = rift.rift_gmm_create(d, 3, lo, hi)
+    rift.rift_gmm_set_model(g, mu0, cov0, pi0)
+    it, ll = rift.rift_gmm_fit(g, n, xs, lw, 300, 1e-7, 0.0)
+    first = rift.rift_gmm_get_model(g)
+    it_o = go.fit(x, lw_o, mu0, cov0, pi0, 300, 1e-7, 0.0)[3]
+    assert it == it_o and 1 < it < 300
+    rift.rift_gmm_set_model(g, mu0, cov0, pi0)
+    rift.rift_gmm_fit(g, n, xs, lw, 300, 1e-7, 0.0)
+    again = rift.rift_gmm_get_model(g)
+    assert all(np.array_equal(a, b) for a, b in zip(first[:3], again[:3]))
+    rift.rift_gmm_destroy(g)
+
+
+def test_online_update_merges_like_the_oracle(torch):
+    rng = np.random.default_rng(7)
+    d, n1, n2 = 2, 20_000, 12_345
+    x1, x2 = _data(rng, n1, d), _data(rng, n2, d) + 0.05
+    lw1, lw2 = rng.normal(0, 1, n1), rng.normal(0, 1, n2)
+    lo, hi = np.array([-6.0, -6.0]), np.array([6.0, 6.0])
+    mu0, cov0, pi0 = _init(d)
+    g = rift.rift_gmm_create(d, 3, lo, hi)
+    rift.rift_gmm_set_model(g, mu0, cov0, pi0)
+    rift.rift_gmm_fit(g, n1, [_dev(torch, x1[:, j]) for j in range(d)], _dev(torch, lw1), 5)
+    rift.rift_gmm_fit(g, n2, [_dev(torch, x2[:, j]) for j in range(d)], _dev(torch, lw2), 5, merge=1)
+    mu, cov, pi, nt = rift.rift_gmm_get_model(g)
+    a = go.fit(x1, lw1, mu0, cov0, pi0, 5)
+    b = go.fit(x2, lw2, a[0], a[1], a[2], 5)                                 # G3: trained from the old model's parameters
+    mu_o, cov_o, pi_o = go.merge(a[0], a[1], a[2], n1, b[0], b[1], b[2], n2)
+    assert nt == n1 + n2 and abs(pi.sum() - 1.0) < 1e-12
+    assert np.max(np.abs(mu - mu_o)) < TOL_EM and np.max(np.abs(cov - cov_o)) < TOL_EM and np.max(np.abs(pi - pi_o)) < TOL_EM
+    # a permuted new model is matched back: set the old model, fit from a permuted start, merge
+    perm = [2, 0, 1]
+    rift.rift_gmm_set_model(g, a[0], a[1], a[2], n1)
+    h2 = rift.rift_gmm_create(d, 3, lo, hi)
+    rift.rift_gmm_set_model(h2, a[0][perm], a[1][perm], a[2][perm], 0)
+    rift.rift_gmm_fit(h2, n2, [_dev(torch, x2[:, j]) for j in range(d)], _dev(torch, lw2), 5)
+    mu_p, cov_p, pi_p, _ = rift.rift_gmm_get_model(h2)
+    assert go.match_components(a[0], a[1], mu_p, cov_p) == perm
+    mo = go.merge(a[0], a[1], a[2], n1, mu_p, cov_p, pi_p, n2)
+    assert np.max(np.abs(mo[0] - mu_o)) < 1e-8                               # the same merged model whatever the order was
+    rift.rift_gmm_destroy(h2)
+    rift.rift_gmm_destroy(g)
+
+
+MODELS = {
+    "2d": (np.array([[0.2, 0.1], [1.2, 0.9], [-0.3, 1.0]]),
+           np.array([[[0.5, 0.35], [0.35, 0.4]], [[0.2, -0.1], [-0.1, 0.3]], [[0.05, 0.0], [0.0, 0.6]]]),
+           np.array([0.5, 0.3, 0.2]), np.array([-0.5, -0.6]), np.array([1.6, 1.4])),
+    "2d_tight": (np.array([[0.0, 0.0], [0.5, 0.45]]),
+                 np.array([[[1.0, 0.99 * 0.5], [0.99 * 0.5, 0.25]], [[0.01, 0.0], [0.0, 0.01]]]),
+                 np.array([0.7, 0.3]), np.array([-1.0, -1.0]), np.array([1.0, 1.0])),
+    "1d": (np.array([[0.5], [2.5]]), np.array([[[0.64]], [[0.09]]]), np.array([0.7, 0.3]), np.array([0.0]), np.array([3.0])),
+}
+
+
+@pytest.mark.parametrize("name", list(MODELS))
+def test_masses_density_and_draws_match_oracle(torch, name):
+    mu, cov, pi, lo, hi = MODELS[name]
+    K, d = mu.shape
+    g = rift.rift_gmm_create(d, K, lo, hi)
+    rift.rift_gmm_set_model(g, mu, cov, pi)
+    Z = rift.rift_gmm_box_mass(g)
+    Z_o = np.array([go.box_mass(mu[k], cov[k], lo, hi) for k in range(K)])
+    assert np.max(np.abs(Z - Z_o) / Z_o) < 1e-9
+    # draws: same counters, same component, same proposal -> the same points up to the inverse normal CDF's rounding
+    n, seed, off = 3000, 12345, 1_000_000_007
+    xs = [torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(d)]
+    lnp = torch.empty(n, dtype=torch.float64, device="cuda")
+    failed = rift.rift_gmm_draw(g, n, seed, off, xs, lnp, want_failed=True)
+    torch.cuda.synchronize()
+    x = np.stack([v.cpu().numpy() for v in xs], axis=1)
+    x_o, failed_o = go.draw(n, seed, off, mu, cov, pi, lo, hi)
+    assert failed == failed_o == 0
+    assert np.all((x >= lo) & (x < hi))
+    diff = np.max(np.abs(x - x_o), axis=1)
+    assert np.mean(diff < TOL_DRAW) > 0.999          # an acceptance within rounding of the domain's edge may differ: none expected
+    assert np.max(diff) < TOL_DRAW
+    lnp_o = go.ln_density(x_o, mu, cov, pi, lo, hi)
+    assert np.max(np.abs(lnp.cpu().numpy() - lnp_o)) < TOL_LNP
+    # the density entry point, inside and outside the domain
+    rng = np.random.default_rng(1)
+    pts = rng.uniform(lo - 0.3, hi + 0.3, size=(5000, d))
+    out = torch.empty(5000, dtype=torch.float64, device="cuda")
+    rift.rift_gmm_ln_density(g, 5000, [_dev(torch, pts[:, j]) for j in range(d)], out)
+    torch.cuda.synchronize()
+    ref = go.ln_density(pts, mu, cov, pi, lo, hi)
+    got = out.cpu().numpy()
+    assert np.array_equal(np.isneginf(got), np.isneginf(ref)) and np.any(np.isneginf(ref))
+    fin = np.isfinite(ref)
+    assert np.max(np.abs(got[fin] - ref[fin])) < TOL_LNP
+    # a second call continues the stream
+    xs2 = [torch.empty(100, dtype=torch.float64, device="cuda") for _ in range(d)]
+    rift.rift_gmm_draw(g, 100, seed, off + 2900, xs2)
+    torch.cuda.synchronize()
+    assert np.array_equal(np.stack([v.cpu().numpy() for v in xs2], axis=1), x[2900:])
+    rift.rift_gmm_destroy(g)
+
+
+def test_adaptive_loop_integrates_a_correlated_gaussian(torch):
+    """The paper's integrator test in miniature (Fig. 6, :332): a narrow, strongly correlated Gaussian 'likelihood' in a wide
+    box.  Draw from p_s, weight by L / p_s, refit (merged online), repeat: the evidence estimate converges to the closed form
+    (the Gaussian's mass inside the box) and the effective sample size grows far beyond that of the uniform start."""
+    lo, hi = np.array([-10.0, -10.0]), np.array([10.0, 10.0])
+    m_true, c_true = np.array([1.0, -2.0]), np.array([[0.04, 0.054], [0.054, 0.09]])          # correlation 0.9
+    exact = go.box_mass(m_true, c_true, lo, hi)
+    g = rift.rift_gmm_create(2, 2, lo, hi)
+    n = 200_000
+    xs = [torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(2)]
+    lnp = torch.empty(n, dtype=torch.float64, device="cuda")
+    prec = torch.from_numpy(np.linalg.inv(c_true)).cuda()
+    ln_norm = -0.5 * math.log(np.linalg.det(c_true)) - math.log(2 * math.pi)
+    ess = []
+    for it in range(6):
+        rift.rift_gmm_draw(g, n, 99, it * n, xs, lnp)
+        d0, d1 = xs[0] - m_true[0], xs[1] - m_true[1]
+        lnL = ln_norm - 0.5 * (prec[0, 0] * d0 * d0 + 2 * prec[0, 1] * d0 * d1 + prec[1, 1] * d1 * d1)
+        lnw = lnL - lnp
+        w = torch.exp(lnw - lnw.max())
+        ess.append(float(w.sum() ** 2 / (w * w).sum()))
+        est = float(torch.exp(lnw).mean())
+        rift.rift_gmm_fit(g, n, xs, lnw, 20, 1e-8, 1e-9, merge=1 if it > 0 else 0)
+    assert ess[0] < 0.01 * n and ess[-1] > 0.5 * n, ess
+    assert abs(est - exact) < 5e-3 * exact, (est, exact)
+    rift.rift_gmm_destroy(g)
