@@ -68,6 +68,11 @@ int rift_gmm_ln_density(rift_gmm_t *h, int64_t n, const double *const *x, double
  * the exact conditional integral over x_2 for n_dim = 2, relative error < 1e-9 for |correlation| <= 0.999). */
 int rift_gmm_box_mass(rift_gmm_t *h, double *Z);
 
+/* out[i] = terms[0][i] + ... + terms[n_terms - 1][i] (left to right), 1 <= n_terms <= 8: the log-density of a sampler made of
+ * several independent groups (sum of the groups' ln p_s), or the log-weight ln omega_i = lnL_i + ln_weight_i that rift_gmm_fit
+ * takes.  terms: HOST array of DEVICE fp64 [n] pointers; out: DEVICE fp64 [n] (may alias a term).  Asynchronous. */
+int rift_gmm_add(int64_t n, int32_t n_terms, const double *const *terms, double *out, void *cuda_stream);
+
 int rift_gmm_destroy(rift_gmm_t *h);
 
 #ifdef __cplusplus

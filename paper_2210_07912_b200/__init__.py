@@ -6,5 +6,6 @@ integrator over the sampler entry points of ``include/rift_ac.h``.
 """
 from . import synth  # noqa: F401
 from . import ac_loop  # noqa: F401
+from . import gmm_loop  # noqa: F401
 from .binding import *  # noqa: F401,F403
 from .binding import lib, RiftError, LIB_PATH, EXPORTS  # noqa: F401

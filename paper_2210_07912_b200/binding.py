@@ -31,7 +31,7 @@ EXPORTS = ("rift_ile_create", "rift_ile_eval_batch", "rift_ile_reduce", "rift_il
            "rift_ile_strerror", "rift_ile_last_error", "rift_ile_reduce_static", "rift_ile_reduce_static_error",
            "rift_ile_rho_guess")
 GMM_EXPORTS = ("rift_gmm_create", "rift_gmm_set_model", "rift_gmm_get_model", "rift_gmm_fit", "rift_gmm_draw",
-               "rift_gmm_ln_density", "rift_gmm_box_mass", "rift_gmm_destroy")
+               "rift_gmm_ln_density", "rift_gmm_box_mass", "rift_gmm_add", "rift_gmm_destroy")
 RIFT_GMM_MAX_COMP, RIFT_GMM_MAX_TRIES = 8, 64
 SKY_EXPORTS = ("rift_sky_network_frame", "rift_sky_network_to_radec", "rift_sky_radec_to_network")
 RIFT_REDUCE_STATIC_MAX_SEG = 1024
@@ -126,6 +126,7 @@ def lib() -> C.CDLL:
         L.rift_gmm_ln_density.argtypes = [vp, i64, C.POINTER(vp), vp, vp]
         L.rift_gmm_box_mass.argtypes = [vp, vp]
         L.rift_gmm_destroy.argtypes = [vp]
+        L.rift_gmm_add.argtypes = [i64, i32, C.POINTER(vp), vp, vp]
         for name in GMM_EXPORTS:
             getattr(L, name).restype = C.c_int
         L.rift_ile_rho_guess.argtypes = [vp, vp]
@@ -354,6 +355,12 @@ def rift_gmm_box_mass(g: GmmHandle) -> np.ndarray:
     Z = np.empty(g.n_comp)
     _check(lib().rift_gmm_box_mass(g.ptr, Z.ctypes.data))
     return Z
+
+
+def rift_gmm_add(n: int, terms, out, cuda_stream: int = 0) -> None:
+    """out = terms[0] + terms[1] + ... on the device."""
+    arr = (C.c_void_p * len(terms))(*[_ptr(t) for t in terms])
+    _check(lib().rift_gmm_add(int(n), len(terms), arr, _ptr(out), int(cuda_stream) or None))
 
 
 def rift_gmm_destroy(g: GmmHandle) -> None:

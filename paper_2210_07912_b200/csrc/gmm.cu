@@ -352,6 +352,17 @@ __global__ void __launch_bounds__(GM_THREADS) gmm_density_kernel(int64_t n, cons
   }
 }
 
+struct SumTerms {
+  const double *t[8];
+};
+__global__ void __launch_bounds__(GM_THREADS) gmm_add_kernel(int64_t n, int n_terms, SumTerms T, double *__restrict__ out) {
+  for (int64_t i = (int64_t)blockIdx.x * GM_THREADS + threadIdx.x; i < n; i += (int64_t)gridDim.x * GM_THREADS) {
+    double v = T.t[0][i];
+    for (int j = 1; j < n_terms; ++j) v += T.t[j][i];
+    out[i] = v;
+  }
+}
+
 inline int gm_grid(int64_t n) {
   int64_t b = (n + GM_THREADS - 1) / GM_THREADS;
   if (b > GM_BLOCKS) b = GM_BLOCKS;
@@ -601,4 +612,18 @@ extern "C" int rift_gmm_box_mass(rift_gmm_t *h, double *Z) {
   ensure_dev(h);
   for (int k = 0; k < h->K; ++k) Z[k] = std::exp(h->dev.lnz[k]);
   return RIFT_OK;
+}
+
+extern "C" int rift_gmm_add(int64_t n, int32_t n_terms, const double *const *terms, double *out, void *cuda_stream) {
+  if (n < 0 || n_terms < 1 || n_terms > 8 || !terms || (n > 0 && !out)) return RIFT_EINVAL;
+  SumTerms T{};
+  for (int j = 0; j < n_terms; ++j) {
+    if (!terms[j]) return RIFT_EINVAL;
+    T.t[j] = terms[j];
+  }
+  if (n == 0) return RIFT_OK;
+  int64_t b = (n + GM_THREADS - 1) / GM_THREADS;
+  if (b > 148 * 8) b = 148 * 8;
+  gmm_add_kernel<<<(int)b, GM_THREADS, 0, reinterpret_cast<cudaStream_t>(cuda_stream)>>>(n, n_terms, T, out);
+  return cudaGetLastError() == cudaSuccess ? RIFT_OK : RIFT_ECUDA;
 }
