@@ -363,6 +363,7 @@ def bench_row(rift, torch, dist_util, data: ConfigData, precision: str, steps, w
         row["launch_rate"] = launch_rate(rift, torch, h, ids, N, data)
     if cfg.index == 1:                        # NEXT-2: the distance-marginalised evaluation on the same samples (5 parameters)
         row["dmarg"] = dmarg_row(rift, torch, h, ids, N, data, flush, row)
+        row["gmm"] = gmm_row(rift, torch, h, data, cfg, row["dmarg"])
     rift.rift_ile_destroy(h)
     return row
 
@@ -396,6 +397,52 @@ def dmarg_row(rift, torch, h, ids, N, data, flush, row, n_dist=128):
             "steps": 3, "cost_ratio_vs_plain": t5 / t6, "median_n_ess_5d": e5, "median_n_ess_6d": e6,
             "n_ess_gain_at_equal_cost": (e5 / t5) / (e6 / t6) if e6 > 0 else None,
             "median_lnZ_5d_minus_6d": float(np.median(red5["lnZ"] - red6["lnZ"]))}
+
+
+def gmm_row(rift, torch, h, data, cfg, dm, n_per_round=200_000, rounds=8, n_dist=128):
+    """the configuration PAPER.md:807 recommends for loud signals on intrinsic point 0 -- GMM
+    sampling (rift_gmm.h) in the rotated network-frame sky (rift_sky.h) with distance marginalisation (gmm_loop.integrate) --
+    timed as a whole (draws, weights, evaluation, reduce, EM refits), with its effective samples per evaluation next to the
+    prior-sampling ones of the dmarg row; plus the sampler kernels alone on 4e6 samples."""
+    from paper_2210_07912_b200 import gmm_loop
+    stream = torch.cuda.current_stream().cuda_stream
+    R = rift.rift_sky_network_frame(data.loc[0], data.loc[1])
+    res = None
+    ms = []
+    for rep in range(2):                      # the first repetition warms up (workspace growth, lazy module load)
+        samplers = gmm_loop.create_samplers(n_comp_sky=3, n_comp_1d=1)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        res = gmm_loop.integrate(h, samplers, 0, R, cfg.gmst, synth.D_MIN_MPC, synth.D_MAX_MPC, n_dist, n_per_round,
+                                 n_eff_target=float("inf"), max_rounds=rounds, seed=11, cuda_stream=stream)
+        b.record()
+        torch.cuda.synchronize()
+        ms.append(a.elapsed_time(b))
+        gmm_loop.destroy_samplers(samplers)
+    n = 4_000_000
+    g = rift.rift_gmm_create(2, 4, [-3.0, -3.0], [3.0, 3.0])
+    xs = [torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(2)]
+    lnp = torch.empty(n, dtype=torch.float64, device="cuda")
+    rift.rift_gmm_draw(g, n, 1, 0, xs, lnp, cuda_stream=stream)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    ev[0].record()
+    for _ in range(10):
+        rift.rift_gmm_draw(g, n, 1, 0, xs, lnp, cuda_stream=stream)
+    ev[1].record()
+    lw = torch.zeros(n, dtype=torch.float64, device="cuda")
+    rift.rift_gmm_fit(g, n, xs, lw, 1, cuda_stream=stream)
+    ev[2].record()
+    it, _ll = rift.rift_gmm_fit(g, n, xs, lw, 10, cuda_stream=stream)
+    ev[3].record()
+    torch.cuda.synchronize()
+    rift.rift_gmm_destroy(g)
+    t_draw, t_em = ev[0].elapsed_time(ev[1]) / 10, ev[2].elapsed_time(ev[3]) / max(it, 1)
+    return {"loop": "gmm_loop.integrate: GMM (sky pair 3 components, iota 1) + network-frame sky + dmarg, point 0",
+            "rounds": res["rounds"], "n_evals": res["n_evals"], "ms_total": ms[-1], "evals_per_s": res["n_evals"] / (ms[-1] * 1e-3),
+            "lnZ": res["lnZ"], "rel_err": res["rel_err"], "n_ess": res["n_ess"], "n_ess_per_eval": res["n_ess"] / res["n_evals"],
+            "n_ess_per_eval_prior_sampling_5d": dm["median_n_ess_5d"] / (data.N),
+            "draw_samples_per_s": n / (t_draw * 1e-3), "em_iteration_samples_per_s": n / (t_em * 1e-3),
+            "draw_ms_4e6": t_draw, "em_iteration_ms_4e6": t_em}
 
 
 def launch_rate(rift, torch, h, ids, N, data, n_calls=200):

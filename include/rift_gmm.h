@@ -54,6 +54,16 @@ int rift_gmm_get_model(const rift_gmm_t *h, double *mu, double *cov, double *pi,
 int rift_gmm_fit(rift_gmm_t *h, int64_t n, const double *const *x, const double *ln_w, int32_t n_iter, double tol, double reg,
                  int32_t merge, int32_t *iters_done, double *loglik, void *cuda_stream);
 
+/* rift_gmm_fit on tempered weights w_n^temper (reading G7; not in the paper, whose sampler is described for weights that
+ * already spread over many samples): temper is the largest value in [0, 1], found by 20 bisection steps from [0, 1], whose
+ * tempered effective sample size (sum_n w_n^temper)^2 / sum_n w_n^(2 temper) is at least ess_min; 1 if the plain weights
+ * already reach it.  A round whose weight sits on a handful of samples (a loud signal seen through a wide proposal) would
+ * otherwise collapse the mixture onto those samples.  The evidence stays unbiased whatever p_s is.  ess_min = 0: rift_gmm_fit.
+ *   temper_used : HOST output (may be NULL). */
+int rift_gmm_fit_tempered(rift_gmm_t *h, int64_t n, const double *const *x, const double *ln_w, double ess_min, int32_t n_iter,
+                          double tol, double reg, int32_t merge, double *temper_used, int32_t *iters_done, double *loglik,
+                          void *cuda_stream);
+
 /* Draw samples index offset .. offset + n - 1 of stream `seed` from p_s and evaluate ln p_s at them.
  *   x : HOST array of n_dim DEVICE pointers, each fp64 [n];  ln_ps : DEVICE fp64 [n] (may be NULL).
  *   n_failed : HOST output or NULL: draws that found no point of the domain in RIFT_GMM_MAX_TRIES proposals (they are set to

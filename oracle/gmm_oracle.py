@@ -23,7 +23,10 @@ Readings:
       never does is set to the domain-clipped mean and counted).  The univariate truncated normals are inverse-CDF draws.
   G6  Random numbers: the counter-based hash of oracle/ac_oracle.py (splitmix64 finaliser of seed + (c + 1) * golden ratio)
       with counter c = (sample * max_tries + try) * 4 + j, j = 0 for the component of try 0, j = 1 + dimension for z_j.
-Pins: tests/test_gmm_oracle_pins.py (P32-P39).
+  G7  Tempering (not in the paper; a safeguard of the adaptive loop): the fit may be run on weights w_n^temper, temper the
+      largest value in [0, 1] found by 20 bisection steps from [0, 1] whose effective sample size (sum w^t)^2 / sum w^(2t)
+      reaches ess_min (1 if the plain weights already do).
+Pins: tests/test_gmm_oracle_pins.py (P32-P40).
 """
 from __future__ import annotations
 
@@ -35,10 +38,31 @@ from scipy import integrate, special
 
 from .ac_oracle import hash_u01
 
-__all__ = ["normalise_ln_weights", "ln_normal", "e_step", "m_step", "fit", "match_components", "merge", "transform", "z_box",
+__all__ = ["tempered_ess", "temper_for_ess", "normalise_ln_weights", "ln_normal", "e_step", "m_step", "fit", "match_components", "merge", "transform", "z_box",
            "box_mass", "draw", "ln_density", "MAX_TRIES"]
 
 MAX_TRIES = 64
+
+
+def tempered_ess(ln_w, beta: float) -> float:
+    ln_w = np.asarray(ln_w, dtype=np.float64)
+    v = ln_w[np.isfinite(ln_w)]
+    w = np.exp(beta * (v - np.max(v)))
+    return float(np.sum(w) ** 2 / np.sum(w * w))
+
+
+def temper_for_ess(ln_w, ess_min: float) -> float:
+    """G7."""
+    if ess_min <= 0 or tempered_ess(ln_w, 1.0) >= ess_min:
+        return 1.0
+    lo, hi = 0.0, 1.0
+    for _ in range(20):
+        mid = 0.5 * (lo + hi)
+        if tempered_ess(ln_w, mid) >= ess_min:
+            lo = mid
+        else:
+            hi = mid
+    return lo
 
 
 def normalise_ln_weights(ln_w) -> np.ndarray:

@@ -30,7 +30,7 @@ EXPORTS = ("rift_ile_create", "rift_ile_eval_batch", "rift_ile_reduce", "rift_il
            "rift_ile_staged", "rift_ile_eval_batch_dmarg", "rift_ile_precompute", "rift_ile_destroy",
            "rift_ile_strerror", "rift_ile_last_error", "rift_ile_reduce_static", "rift_ile_reduce_static_error",
            "rift_ile_rho_guess")
-GMM_EXPORTS = ("rift_gmm_create", "rift_gmm_set_model", "rift_gmm_get_model", "rift_gmm_fit", "rift_gmm_draw",
+GMM_EXPORTS = ("rift_gmm_create", "rift_gmm_set_model", "rift_gmm_get_model", "rift_gmm_fit", "rift_gmm_fit_tempered", "rift_gmm_draw",
                "rift_gmm_ln_density", "rift_gmm_box_mass", "rift_gmm_add", "rift_gmm_destroy")
 RIFT_GMM_MAX_COMP, RIFT_GMM_MAX_TRIES = 8, 64
 SKY_EXPORTS = ("rift_sky_network_frame", "rift_sky_network_to_radec", "rift_sky_radec_to_network")
@@ -122,6 +122,8 @@ def lib() -> C.CDLL:
         L.rift_gmm_set_model.argtypes = [vp, vp, vp, vp, dbl]
         L.rift_gmm_get_model.argtypes = [vp, vp, vp, vp, C.POINTER(dbl)]
         L.rift_gmm_fit.argtypes = [vp, i64, C.POINTER(vp), vp, i32, dbl, dbl, i32, C.POINTER(i32), C.POINTER(dbl), vp]
+        L.rift_gmm_fit_tempered.argtypes = [vp, i64, C.POINTER(vp), vp, dbl, i32, dbl, dbl, i32, C.POINTER(dbl), C.POINTER(i32),
+                                            C.POINTER(dbl), vp]
         L.rift_gmm_draw.argtypes = [vp, i64, C.c_uint64, C.c_uint64, C.POINTER(vp), vp, C.POINTER(i64), vp]
         L.rift_gmm_ln_density.argtypes = [vp, i64, C.POINTER(vp), vp, vp]
         L.rift_gmm_box_mass.argtypes = [vp, vp]
@@ -338,6 +340,15 @@ def rift_gmm_fit(g: GmmHandle, n: int, x, ln_w, n_iter: int, tol: float = 0.0, r
     _check(lib().rift_gmm_fit(g.ptr, int(n), _xptrs(g, x), _ptr(ln_w), int(n_iter), float(tol), float(reg), int(merge),
                               C.byref(it), C.byref(ll), int(cuda_stream) or None))
     return it.value, ll.value
+
+
+def rift_gmm_fit_tempered(g: GmmHandle, n: int, x, ln_w, ess_min: float, n_iter: int, tol: float = 0.0, reg: float = 0.0,
+                          merge: int = 0, cuda_stream: int = 0):
+    """rift_gmm_fit on weights tempered so that their effective sample size reaches ess_min; returns (temper, iterations, ln L)."""
+    it, ll, tp = C.c_int32(), C.c_double(), C.c_double()
+    _check(lib().rift_gmm_fit_tempered(g.ptr, int(n), _xptrs(g, x), _ptr(ln_w), float(ess_min), int(n_iter), float(tol),
+                                       float(reg), int(merge), C.byref(tp), C.byref(it), C.byref(ll), int(cuda_stream) or None))
+    return tp.value, it.value, ll.value
 
 
 def rift_gmm_draw(g: GmmHandle, n: int, seed: int, offset: int, x, ln_ps=None, want_failed: bool = False, cuda_stream: int = 0):

@@ -248,9 +248,36 @@ __global__ void __launch_bounds__(GM_THREADS) gmm_max_kernel(int64_t n, const do
   }
 }
 
+// sum w^beta and sum w^(2 beta), w = exp(ln_w - w_max): the tempered effective sample size (sum)^2 / (sum of squares)
+__global__ void __launch_bounds__(GM_THREADS) gmm_ess_kernel(int64_t n, const double *__restrict__ ln_w, double w_max, double beta,
+                                                             double *__restrict__ partial) {
+  __shared__ double s_w[GM_THREADS / 32][2];
+  double s1 = 0.0, s2 = 0.0;
+  for (int64_t i = (int64_t)blockIdx.x * GM_THREADS + threadIdx.x; i < n; i += (int64_t)gridDim.x * GM_THREADS) {
+    const double v = ln_w[i];
+    if (v == v && v > -INFINITY) {
+      const double w = exp(beta * (v - w_max));
+      s1 += w;
+      s2 += w * w;
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+    s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+  }
+  if ((threadIdx.x & 31) == 0) s_w[threadIdx.x >> 5][0] = s1, s_w[threadIdx.x >> 5][1] = s2;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < GM_THREADS / 32; ++w) s1 += s_w[w][0], s2 += s_w[w][1];
+    partial[2 * blockIdx.x] = s1;
+    partial[2 * blockIdx.x + 1] = s2;
+  }
+}
+
 __global__ void __launch_bounds__(GM_THREADS) gmm_em_kernel(int64_t n, const double *__restrict__ x0p, const double *__restrict__ x1p,
-                                                            const double *__restrict__ ln_w, double w_max, const GmmDev g,
-                                                            double *__restrict__ partial) {
+                                                            const double *__restrict__ ln_w, double w_max, double temper,
+                                                            const GmmDev g, double *__restrict__ partial) {
   __shared__ double s_red[GM_THREADS / 32][GM_ROW];
   double acc[GM_ROW];
 #pragma unroll
@@ -259,7 +286,8 @@ __global__ void __launch_bounds__(GM_THREADS) gmm_em_kernel(int64_t n, const dou
     double w = 1.0;
     if (ln_w) {
       const double v = ln_w[i];
-      w = v == v ? exp(v - w_max) : 0.0;
+      w = v == v ? exp(temper * (v - w_max)) : 0.0;
+      if (v == -INFINITY) w = 0.0;                       // also when temper = 0
     }
     if (w == 0.0) continue;
     const double x0 = x0p[i], x1 = g.d == 2 ? x1p[i] : 0.0;
@@ -512,9 +540,11 @@ void merge_models(int d, int K, const Model &old, double n_old, const Model &nw,
 
 }  // namespace
 
-extern "C" int rift_gmm_fit(rift_gmm_t *h, int64_t n, const double *const *x, const double *ln_w, int32_t n_iter, double tol,
-                            double reg, int32_t merge, int32_t *iters_done, double *loglik, void *cuda_stream) {
-  if (!h || n < 1 || !x || !x[0] || (h->d == 2 && !x[1]) || n_iter < 0 || !(tol >= 0.0) || !(reg >= 0.0)) return RIFT_EINVAL;
+namespace {
+int gmm_fit_impl(rift_gmm_t *h, int64_t n, const double *const *x, const double *ln_w, double ess_min, int32_t n_iter, double tol,
+                 double reg, int32_t merge, double *temper_used, int32_t *iters_done, double *loglik, void *cuda_stream) {
+  if (!h || n < 1 || !x || !x[0] || (h->d == 2 && !x[1]) || n_iter < 0 || !(tol >= 0.0) || !(reg >= 0.0) || !(ess_min >= 0.0))
+    return RIFT_EINVAL;
   GmGuard guard(h->device);
   cudaStream_t s = reinterpret_cast<cudaStream_t>(cuda_stream);
   const int d = h->d, K = h->K, grid = gm_grid(n);
@@ -529,6 +559,34 @@ extern "C" int rift_gmm_fit(rift_gmm_t *h, int64_t n, const double *const *x, co
     for (int b = 0; b < grid; ++b) w_max = std::fmax(w_max, host[b]);
     if (!(w_max > -INFINITY) || !std::isfinite(w_max)) return RIFT_ESTATE;      // every weight is zero (or +inf)
   }
+  // G7: the largest temper in [0, 1] (20 bisection steps) whose tempered effective sample size reaches ess_min
+  double temper = 1.0;
+  if (ln_w && ess_min > 0.0) {
+    auto ess = [&](double beta, double &out) -> bool {
+      gmm_ess_kernel<<<grid, GM_THREADS, 0, s>>>(n, ln_w, w_max, beta, h->d_partial);
+      double part[2 * GM_BLOCKS];
+      if (cudaMemcpyAsync(part, h->d_partial, sizeof(double) * 2 * grid, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+          cudaStreamSynchronize(s) != cudaSuccess)
+        return false;
+      double s1 = 0.0, s2 = 0.0;
+      for (int b = 0; b < grid; ++b) s1 += part[2 * b], s2 += part[2 * b + 1];
+      out = s2 > 0.0 ? s1 * s1 / s2 : 0.0;
+      return true;
+    };
+    double e1;
+    if (!ess(1.0, e1)) return RIFT_ECUDA;
+    if (e1 < ess_min) {
+      double lo_b = 0.0, hi_b = 1.0;
+      for (int step = 0; step < 20; ++step) {
+        const double mid = 0.5 * (lo_b + hi_b);
+        double e;
+        if (!ess(mid, e)) return RIFT_ECUDA;
+        if (e >= ess_min) lo_b = mid;
+        else hi_b = mid;
+      }
+      temper = lo_b;
+    }
+  }
   Model m = h->model;
   double prev = 0.0, ll = -INFINITY;
   bool have_prev = false;
@@ -536,7 +594,7 @@ extern "C" int rift_gmm_fit(rift_gmm_t *h, int64_t n, const double *const *x, co
   while (it < n_iter) {
     GmmDev g;
     derive(d, K, h->lo, h->hi, m, false, g);
-    gmm_em_kernel<<<grid, GM_THREADS, 0, s>>>(n, x[0], d == 2 ? x[1] : nullptr, ln_w, w_max, g, h->d_partial);
+    gmm_em_kernel<<<grid, GM_THREADS, 0, s>>>(n, x[0], d == 2 ? x[1] : nullptr, ln_w, w_max, temper, g, h->d_partial);
     gmm_sum_kernel<<<1, 64, 0, s>>>(grid, h->d_partial, h->d_sums);
     if (cudaGetLastError() != cudaSuccess || cudaMemcpyAsync(host, h->d_sums, sizeof(double) * GM_ROW, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
         cudaStreamSynchronize(s) != cudaSuccess)
@@ -576,7 +634,20 @@ extern "C" int rift_gmm_fit(rift_gmm_t *h, int64_t n, const double *const *x, co
   h->dev_ok = false;
   if (iters_done) *iters_done = it;
   if (loglik) *loglik = ll;
+  if (temper_used) *temper_used = temper;
   return RIFT_OK;
+}
+}  // namespace
+
+extern "C" int rift_gmm_fit(rift_gmm_t *h, int64_t n, const double *const *x, const double *ln_w, int32_t n_iter, double tol,
+                            double reg, int32_t merge, int32_t *iters_done, double *loglik, void *cuda_stream) {
+  return gmm_fit_impl(h, n, x, ln_w, 0.0, n_iter, tol, reg, merge, nullptr, iters_done, loglik, cuda_stream);
+}
+
+extern "C" int rift_gmm_fit_tempered(rift_gmm_t *h, int64_t n, const double *const *x, const double *ln_w, double ess_min,
+                                     int32_t n_iter, double tol, double reg, int32_t merge, double *temper_used,
+                                     int32_t *iters_done, double *loglik, void *cuda_stream) {
+  return gmm_fit_impl(h, n, x, ln_w, ess_min, n_iter, tol, reg, merge, temper_used, iters_done, loglik, cuda_stream);
 }
 
 extern "C" int rift_gmm_draw(rift_gmm_t *h, int64_t n, uint64_t seed, uint64_t offset, double *const *x, double *ln_ps,

@@ -8,8 +8,8 @@ The five extrinsic parameters left after the distance marginal are sampled by in
 what remains of it), and iota, psi, phi_ref by one-dimensional mixtures.  Orchestration only: every round is
     rift_gmm_draw (per group) -> rift_gmm_add (ln p_s) -> rift_ac_ile_ln_weight (ln prior - ln p_s, the prior of (lambda, beta)
     being cos(beta) / 4 pi as for (RA, dec)) -> rift_sky_network_to_radec -> rift_ile_eval_batch_dmarg -> rift_ile_reduce
-    (pooled over rounds, Eq. (20)-(21)) -> rift_gmm_add (ln omega) -> rift_gmm_fit (per adapted group; merged online from the
-    second round, Eq. (A8)-(A11)),
+    (pooled over rounds, Eq. (20)-(21)) -> rift_gmm_add (ln omega) -> rift_gmm_fit_tempered (per adapted group, on weights
+    tempered to an effective sample size of at least `ess_min`, reading G7; merged online from the second round, Eq. (A8)-(A11)),
 all kernels of librift_ile.so on the given stream; the host sees four scalars per round and the mixtures' parameters.
 """
 from __future__ import annotations
@@ -39,7 +39,7 @@ def destroy_samplers(samplers: dict) -> None:
 
 def integrate(h_ile, samplers: dict, point_id: int, R, gmst_rad: float, d_min_mpc: float, d_max_mpc: float, n_dist: int,
               n_per_round: int, n_eff_target: float = 10.0, max_rounds: int = 20, adapt=("sky", "iota"), em_iters: int = 20,
-              em_tol: float = 1e-8, reg: float = 1e-6, seed: int = 0, offset: int = 0, cuda_stream: int = 0) -> dict:
+              em_tol: float = 1e-8, reg: float = 1e-6, ess_min: float = 300.0, seed: int = 0, offset: int = 0, cuda_stream: int = 0) -> dict:
     """Returns dict(lnZ, rel_err, n_eff, n_ess, rounds, n_evals, next_offset) of the pooled rounds; lnZ is the evidence of
     the point marginalised over all six extrinsic parameters.  `samplers` (create_samplers) are refitted in place for the
     groups named in `adapt`; R is rift_sky_network_frame of the two detectors that define the pole."""
@@ -75,7 +75,7 @@ def integrate(h_ile, samplers: dict, point_id: int, R, gmst_rad: float, d_min_mp
         rift.rift_gmm_add(n, [lnL, ln_w], ln_om, cuda_stream)
         for name, rows, _lo, _hi in GROUPS:
             if name in adapt:
-                rift.rift_gmm_fit(samplers[name], n, [x[r] for r in rows], ln_om, em_iters, em_tol, reg,
-                                  merge=1 if rounds > 1 else 0, cuda_stream=cuda_stream)
+                rift.rift_gmm_fit_tempered(samplers[name], n, [x[r] for r in rows], ln_om, ess_min, em_iters, em_tol, reg,
+                                           merge=1 if rounds > 1 else 0, cuda_stream=cuda_stream)
     return dict(lnZ=float(out["lnZ"][0]) - ln_p_dist, rel_err=float(out["rel_err"][0]), n_eff=float(out["n_eff"][0]),
                 n_ess=float(out["n_ess"][0]), rounds=rounds, n_evals=rounds * n, next_offset=offset + rounds * n)

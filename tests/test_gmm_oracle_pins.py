@@ -178,3 +178,19 @@ def test_p39_two_dimensional_draws_and_importance_identity():
     # sample moments of the draws against moments of p_s on the grid
     m_grid = (p[:, None] * grid).sum(axis=0) * 0.005 ** 2
     assert np.max(np.abs(x.mean(axis=0) - m_grid)) < 5 * np.max(x.std(axis=0)) / np.sqrt(len(x))
+
+
+def test_p40_tempering_reaches_the_requested_effective_sample_size():
+    rng = np.random.default_rng(9)
+    ln_w = rng.normal(0.0, 6.0, 20000)                 # a few samples carry all the weight
+    assert go.tempered_ess(ln_w, 1.0) < 50 and abs(go.tempered_ess(ln_w, 0.0) - 20000) < 1e-6
+    ess = [go.tempered_ess(ln_w, b) for b in np.linspace(0, 1, 21)]
+    assert all(a >= b for a, b in zip(ess, ess[1:]))   # monotone: the bisection is well defined
+    for target in (100.0, 1000.0, 15000.0):
+        b = go.temper_for_ess(ln_w, target)
+        assert 0.0 < b < 1.0 and go.tempered_ess(ln_w, b) >= target > go.tempered_ess(ln_w, b + 2.0 ** -19)
+    assert go.temper_for_ess(ln_w, 1.0) == 1.0 and go.temper_for_ess(ln_w, 0.0) == 1.0
+    assert go.temper_for_ess(ln_w, 1e9) == 0.0         # unreachable: all weights equal
+    # the equal-weight closed form: ESS of N(0, s^2) log-weights tempered by b is about n exp(-(b s)^2)
+    b = go.temper_for_ess(ln_w, 20000 * np.exp(-1.0))
+    assert abs(b * 6.0 - 1.0) < 0.05

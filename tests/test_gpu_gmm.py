@@ -79,6 +79,30 @@ def test_em_matches_oracle_iteration_by_iteration(torch, d, n, weighted):
     rift.rift_gmm_destroy(g)
 
 
+def test_tempered_fit_matches_oracle(torch):
+    rng = np.random.default_rng(17)
+    d, n = 2, 50_000
+    x = _data(rng, n, d)
+    ln_w = rng.normal(0.0, 7.0, n) - 300.0
+    ln_w[11] = -np.inf
+    lo, hi = x.min(axis=0) - 1.0, x.max(axis=0) + 1.0
+    mu0, cov0, pi0 = _init(d)
+    xs, lw = [_dev(torch, x[:, j]) for j in range(d)], _dev(torch, ln_w)
+    for ess_min in (500.0, 1.0, 1e9):
+        g = rift.rift_gmm_create(d, 3, lo, hi)
+        rift.rift_gmm_set_model(g, mu0, cov0, pi0)
+        temper, it, ll = rift.rift_gmm_fit_tempered(g, n, xs, lw, ess_min, 5, 0.0, 1e-6)
+        t_o = go.temper_for_ess(ln_w, ess_min)
+        assert temper == t_o, (temper, t_o)                 # the same 20 bisection decisions
+        assert (ess_min == 1.0) == (temper == 1.0) and (ess_min == 1e9) == (temper == 0.0)
+        mu, cov, pi, _nt = rift.rift_gmm_get_model(g)
+        mu_o, cov_o, pi_o, it_o, ll_o = go.fit(x, np.where(np.isfinite(ln_w), t_o * np.where(np.isfinite(ln_w), ln_w, 0.0), -np.inf), mu0, cov0, pi0, 5, 0.0,
+                                                1e-6)
+        assert it == it_o and abs(ll - ll_o) < TOL_EM * max(1.0, abs(ll_o))
+        assert np.max(np.abs(mu - mu_o)) < TOL_EM and np.max(np.abs(cov - cov_o)) < TOL_EM and np.max(np.abs(pi - pi_o)) < TOL_EM
+        rift.rift_gmm_destroy(g)
+
+
 def test_online_update_merges_like_the_oracle(torch):
     rng = np.random.default_rng(7)
     d, n1, n2 = 2, 20_000, 12_345
