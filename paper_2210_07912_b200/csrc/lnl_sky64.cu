@@ -154,30 +154,36 @@ __global__ void __launch_bounds__(S64_THREADS, 1) lnl_sky64_kernel(const S64Args
         s_run[sp] = 0.0;
         cl2n[sp] = cval_s[32 * half + S64_SPW * warp + sp] * 1.4426950408889634;
       }
+      // Software pipeline over the chunks c = (block, detector): the tensor phase of chunk c + 1 is issued between the barrier
+      // that completes the rows of chunk c and the shifted read of those rows, so that the read's shared-memory latency and
+      // the block's exponentials run under the next chunk's DMMAs
+      double acc[2][4][2];
+      auto tensor_phase = [&](int k, uint32_t c) {               // P_k tiles of the chunk in ring slot c % slots
+        const uint32_t slot = c % (uint32_t)slots;
+        mbar_wait(full + slot, (c / (uint32_t)slots) & 1u);
+#pragma unroll
+        for (int rb = 0; rb < 2; ++rb)
+#pragma unroll
+          for (int nt = 0; nt < 4; ++nt) acc[rb][nt][0] = acc[rb][nt][1] = 0.0;
+        const unsigned char *ap = ring + slot * L.slot_bytes + a_off;
+        const double *bp = cs + (size_t)(k * KS) * S64_NB * 4 + g * 4 + t4;
+#pragma unroll 1
+        for (int s = 0; s < KS; ++s, ap += 32, bp += S64_NB * 4) {
+          const double a0 = *reinterpret_cast<const double *>(ap), a1 = *reinterpret_cast<const double *>(ap + 8 * kp * 8);
+#pragma unroll
+          for (int nt = 0; nt < 4; ++nt) {
+            const double bv = bp[32 * nt];
+            dmma64(acc[0][nt], a0, bv);
+            dmma64(acc[1][nt], a1, bv);
+          }
+        }
+      };
+      tensor_phase(0, cnt);
+      double x[S64_SPW][S64_NE];
       for (int blk = 0; blk < P.n_blocks; ++blk) {
-        double x[S64_SPW][S64_NE];
         for (int k = 0; k < K; ++k, ++cnt) {
           const int i = blk * K + k;
-          const uint32_t slot = cnt % (uint32_t)slots;
-          mbar_wait(full + slot, (cnt / (uint32_t)slots) & 1u);
-          // ---- P_k tiles: 2 row blocks x 4 sample tiles
-          double acc[2][4][2];
-#pragma unroll
-          for (int rb = 0; rb < 2; ++rb)
-#pragma unroll
-            for (int nt = 0; nt < 4; ++nt) acc[rb][nt][0] = acc[rb][nt][1] = 0.0;
-          const unsigned char *ap = ring + slot * L.slot_bytes + a_off;
-          const double *bp = cs + (size_t)(k * KS) * S64_NB * 4 + g * 4 + t4;
-          for (int s = 0; s < KS; ++s, ap += 32, bp += S64_NB * 4) {
-            const double a0 = *reinterpret_cast<const double *>(ap), a1 = *reinterpret_cast<const double *>(ap + 8 * kp * 8);
-#pragma unroll
-            for (int nt = 0; nt < 4; ++nt) {
-              const double bv = bp[32 * nt];
-              dmma64(acc[0][nt], a0, bv);
-              dmma64(acc[1][nt], a1, bv);
-            }
-          }
-          __syncthreads();                                       // every reader is done with the previous detector's rows
+          __syncthreads();                                       // every reader is done with the previous chunk's rows
 #pragma unroll
           for (int rb = 0; rb < 2; ++rb)
 #pragma unroll
@@ -185,8 +191,9 @@ __global__ void __launch_bounds__(S64_THREADS, 1) lnl_sky64_kernel(const S64Args
               xst[(8 * nt) * S64_XP + 8 * rb] = acc[rb][nt][0];
               xst[(8 * nt + 1) * S64_XP + 8 * rb] = acc[rb][nt][1];
             }
-          __syncthreads();                                       // the rows of detector k are complete; chunk i is consumed
+          __syncthreads();                                       // the rows of chunk i are complete; its ring slot is free
           if (tid == 0 && i + slots < n_chunks) issue(i + slots, cnt + (uint32_t)slots);
+          if (i + 1 < n_chunks) tensor_phase(k + 1 < K ? k + 1 : 0, cnt + 1u);
           // ---- shifted read: x_j += P_k[j + r][n], lanes = consecutive rows
 #pragma unroll
           for (int sp = 0; sp < S64_SPW; ++sp) {
