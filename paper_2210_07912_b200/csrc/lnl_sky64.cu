@@ -7,11 +7,14 @@
 // A sorted batch of 64 slots (relative shifts d_{n,k} = b_k + r_{n,k}, 0 <= r < SKY_E) is processed as two half batches of 32
 // samples.  Per (block of 224 window entries, detector) a chunk of 256 consecutive rows of the circularly extended operand
 // A_k[t, 2m + {0,1}] = {Re, Im} Q_{k,m}[t] (fp64, rows of kappa_p doubles with kappa_p = 4 (mod 8): conflict-free fragment
-// loads) arrives by one bulk copy into a ring slot; 16 warps contract it with the coefficients B_k[kappa, n] of the half batch
-// -- 2 row blocks of 8 x 4 sample tiles per warp --, store the tiles unshifted into an exchange buffer
-// [32 samples][258 rows] (lanes = rows; sample pairs 32 bytes apart modulo 128), and after a barrier add
+// loads) arrives by one bulk copy into a ring slot.  The CTA is two independent groups of 8 warps, each with 16 samples of the
+// half batch, its own exchange buffer and named barrier: a group contracts the chunk with the coefficients B_k[kappa, n] of its
+// samples -- 4 row blocks of 8 x 2 sample tiles per warp --, stores the tiles unshifted into its exchange buffer
+// [16 samples][258 rows] (lanes = rows; sample pairs 32 bytes apart modulo 128), and after a group barrier adds
 // P_k[j + r_{n,k}][n] for 2 samples per warp and the block's window entries j = lane + 32 e into registers.  After the last
-// detector the block joins the lane's running (float max, fp64 sum of 2^(c log2e (x - max))) per sample.
+// detector the block joins the lane's running (float max, fp64 sum of 2^(c log2e (x - max))) per sample.  The groups drift apart
+// by up to `slots` chunks, so the tensor phase of one runs under the exchange and exponential phases of the other; the group
+// that finishes a chunk last refills its ring slot.
 #include "rift_internal.h"
 #include "tma_utils.cuh"
 #include "exp2_poly.cuh"
@@ -27,7 +30,7 @@ struct S64Smem {
 
 __host__ __device__ inline S64Smem s64_smem(const Sky64Plan &p) {
   S64Smem L;
-  L.bars = 0;                                                          // full[slots]
+  L.bars = 0;                                                          // full[slots] (8 B each), done[slots] ints at +32
   L.cval = 64;                                                         // double [64] c
   L.qval = L.cval + 64 * 8;                                            // double [64] q
   L.orig = L.qval + 64 * 8;                                            // int [64]
@@ -57,6 +60,8 @@ __device__ __forceinline__ void dmma64(double (&d)[2], double a, double b) {
                : "d"(a), "d"(b));
 }
 
+__device__ __forceinline__ void s64_bar(int id) { asm volatile("bar.sync %0, 256;" ::"r"(id) : "memory"); }
+
 __global__ void __launch_bounds__(S64_THREADS, 1) lnl_sky64_kernel(const S64Args A) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const Sky64Plan &P = A.p;
@@ -79,11 +84,16 @@ __global__ void __launch_bounds__(S64_THREADS, 1) lnl_sky64_kernel(const S64Args
     for (int i = 0; i < slots; ++i) mbar_init(full + i, 1);
   __syncthreads();
 
-  // MMA role: fragment coordinates; row blocks 2 warp, 2 warp + 1 of the chunk; all four sample tiles
+  // two groups of 8 warps: group grp takes samples 16 grp .. 16 grp + 15 of the half batch
+  const int grp = warp >> 3, wg = warp & 7, gtid = tid & 255, bar_id = 1 + grp;
+  int *done = reinterpret_cast<int *>(smem_raw + L.bars + 32);   // groups that have consumed the chunk in a ring slot
+  if (tid < 8) done[tid] = 0;
+  // MMA role: fragment coordinates; row blocks 4 wg .. 4 wg + 3 of the chunk; the group's two sample tiles
   const int g = lane >> 2, t4 = lane & 3;
-  const uint32_t a_off = (uint32_t)(16 * warp + g) * (uint32_t)kp * 8u + (uint32_t)t4 * 8u;   // + 8 kp * 8 (second block) + 32 s
-  // store role: rows 16 warp + g (+ 8), samples 8 nt + 2 t4 (+ 1)
-  double *xst = xb + (2 * t4) * S64_XP + 16 * warp + g;
+  const uint32_t a_off = (uint32_t)(32 * wg + g) * (uint32_t)kp * 8u + (uint32_t)t4 * 8u;   // + 8 rb kp * 8 (row block rb) + 32 s
+  // store role: rows 32 wg + g + 8 rb, samples 8 nt + 2 t4 (+ 1) of the group
+  double *xbg = xb + grp * (S64_NB / 2) * S64_XP;
+  double *xst = xbg + (2 * t4) * S64_XP + 32 * wg + g;
   const double ln_ntau = log((double)n_t);
   const int n_chunks = P.n_blocks * K;
 
@@ -152,29 +162,31 @@ __global__ void __launch_bounds__(S64_THREADS, 1) lnl_sky64_kernel(const S64Args
       for (int sp = 0; sp < S64_SPW; ++sp) {
         m_run[sp] = -INFINITY;
         s_run[sp] = 0.0;
-        cl2n[sp] = cval_s[32 * half + S64_SPW * warp + sp] * 1.4426950408889634;
+        cl2n[sp] = cval_s[32 * half + 16 * grp + S64_SPW * wg + sp] * 1.4426950408889634;
       }
       // Software pipeline over the chunks c = (block, detector): the tensor phase of chunk c + 1 is issued between the barrier
       // that completes the rows of chunk c and the shifted read of those rows, so that the read's shared-memory latency and
       // the block's exponentials run under the next chunk's DMMAs
-      double acc[2][4][2];
+      double acc[4][2][2];
       auto tensor_phase = [&](int k, uint32_t c) {               // P_k tiles of the chunk in ring slot c % slots
         const uint32_t slot = c % (uint32_t)slots;
         mbar_wait(full + slot, (c / (uint32_t)slots) & 1u);
 #pragma unroll
-        for (int rb = 0; rb < 2; ++rb)
+        for (int rb = 0; rb < 4; ++rb)
 #pragma unroll
-          for (int nt = 0; nt < 4; ++nt) acc[rb][nt][0] = acc[rb][nt][1] = 0.0;
+          for (int nt = 0; nt < 2; ++nt) acc[rb][nt][0] = acc[rb][nt][1] = 0.0;
         const unsigned char *ap = ring + slot * L.slot_bytes + a_off;
-        const double *bp = cs + (size_t)(k * KS) * S64_NB * 4 + g * 4 + t4;
+        const double *bp = cs + (size_t)(k * KS) * S64_NB * 4 + (16 * grp + g) * 4 + t4;
 #pragma unroll 1
         for (int s = 0; s < KS; ++s, ap += 32, bp += S64_NB * 4) {
-          const double a0 = *reinterpret_cast<const double *>(ap), a1 = *reinterpret_cast<const double *>(ap + 8 * kp * 8);
+          double av[4];
 #pragma unroll
-          for (int nt = 0; nt < 4; ++nt) {
-            const double bv = bp[32 * nt];
-            dmma64(acc[0][nt], a0, bv);
-            dmma64(acc[1][nt], a1, bv);
+          for (int rb = 0; rb < 4; ++rb) av[rb] = *reinterpret_cast<const double *>(ap + rb * (8 * kp * 8));
+          const double b0 = bp[0], b1 = bp[32];
+#pragma unroll
+          for (int rb = 0; rb < 4; ++rb) {
+            dmma64(acc[rb][0], av[rb], b0);
+            dmma64(acc[rb][1], av[rb], b1);
           }
         }
       };
@@ -183,22 +195,30 @@ __global__ void __launch_bounds__(S64_THREADS, 1) lnl_sky64_kernel(const S64Args
       for (int blk = 0; blk < P.n_blocks; ++blk) {
         for (int k = 0; k < K; ++k, ++cnt) {
           const int i = blk * K + k;
-          __syncthreads();                                       // every reader is done with the previous chunk's rows
+          s64_bar(bar_id);                                       // every reader of the group is done with the previous chunk's rows
 #pragma unroll
-          for (int rb = 0; rb < 2; ++rb)
+          for (int rb = 0; rb < 4; ++rb)
 #pragma unroll
-            for (int nt = 0; nt < 4; ++nt) {
+            for (int nt = 0; nt < 2; ++nt) {
               xst[(8 * nt) * S64_XP + 8 * rb] = acc[rb][nt][0];
               xst[(8 * nt + 1) * S64_XP + 8 * rb] = acc[rb][nt][1];
             }
-          __syncthreads();                                       // the rows of chunk i are complete; its ring slot is free
-          if (tid == 0 && i + slots < n_chunks) issue(i + slots, cnt + (uint32_t)slots);
+          s64_bar(bar_id);                                       // the rows of chunk i are complete; the group has consumed it
+          if (gtid == 0) {                                       // the group that consumes the chunk last refills its slot
+            const uint32_t slot = cnt % (uint32_t)slots;
+            __threadfence_block();
+            if (atomicAdd(done + slot, 1) == 1) {
+              done[slot] = 0;
+              __threadfence_block();
+              if (i + slots < n_chunks) issue(i + slots, cnt + (uint32_t)slots);
+            }
+          }
           if (i + 1 < n_chunks) tensor_phase(k + 1 < K ? k + 1 : 0, cnt + 1u);
           // ---- shifted read: x_j += P_k[j + r][n], lanes = consecutive rows
 #pragma unroll
           for (int sp = 0; sp < S64_SPW; ++sp) {
-            const int n = S64_SPW * warp + sp;
-            const double *src = xb + n * S64_XP + resid_s[k * SKY_NB + 32 * half + n] + lane;
+            const int n = S64_SPW * wg + sp;
+            const double *src = xbg + n * S64_XP + resid_s[k * SKY_NB + 32 * half + 16 * grp + n] + lane;
             if (k == 0) {
 #pragma unroll
               for (int e = 0; e < S64_NE; ++e) x[sp][e] = src[32 * e];
@@ -229,7 +249,7 @@ __global__ void __launch_bounds__(S64_THREADS, 1) lnl_sky64_kernel(const S64Args
       // ---- per sample: combine the 32 lanes, write lnL
 #pragma unroll
       for (int sp = 0; sp < S64_SPW; ++sp) {
-        const int n = 32 * half + S64_SPW * warp + sp;
+        const int n = 32 * half + 16 * grp + S64_SPW * wg + sp;
         const float m = warp_max(m_run[sp]);
         double s = m_run[sp] == -INFINITY ? 0.0 : s_run[sp] * poly_exp2(((double)m_run[sp] - (double)m) * cl2n[sp]);
         s = warp_sum(s);
