@@ -350,7 +350,7 @@ void make_mma_plan(rift_ile *h, double delta_t) {
     if (dm > 1e6) return;
     if ((int)dm > halo) halo = (int)dm;
   }
-  const int cand[][2] = {{0, 0}, {1, 4}, {1, 3}};   // stream, slots
+  const int cand[][2] = {{0, 0}, {1, 8}, {1, 6}, {1, 4}, {1, 3}};   // stream, slots (the deepest ring that fits: a refill takes about 4 k-steps)
   for (const auto &c : cand) {
     p = MmaPlan{};
     p.K = h->K;

@@ -158,18 +158,18 @@ __global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs
   if (STREAM && warp == GW) {
     if (lane == 0) {
       const int64_t w_begin = (b.n * blockIdx.x) / gridDim.x, w_end = (b.n * (blockIdx.x + 1)) / gridDim.x;
-      uint32_t cnt = 0;
+      uint32_t slot = 0, ph = 0;                                 // ring position: slot and the parity of its use count
       for (int64_t w0 = w_begin; w0 < w_end;) {
         const int64_t seg = (b.g0 + w0) / b.n_per_seg;
         const int64_t run_end = min(w_end, (seg + 1) * b.n_per_seg - b.g0);
         const unsigned char *qp = A.q + (int64_t)b.ids[seg] * P.point_stride;
         for (int64_t s0 = w0; s0 < run_end; s0 += NBG)
           for (int k = 0; k < K; ++k)
-            for (int s = 0; s < KS; ++s, ++cnt) {
-              const uint32_t slot = cnt % (uint32_t)P.slots, ph = (cnt / (uint32_t)P.slots) & 1u;
+            for (int s = 0; s < KS; ++s) {
               mbar_wait(empty + slot, ph ^ 1u);
               mbar_expect_tx(full + slot, slot_bytes);
               bulk_g2s(qs + slot * slot_bytes, qp + (size_t)(k * 2 * KS + 2 * s) * P.pitch_q, slot_bytes, full + slot);
+              if (++slot == (uint32_t)P.slots) slot = 0, ph ^= 1u;
             }
         w0 = run_end;
       }
@@ -259,7 +259,7 @@ __global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs
   };
 
   const int w_begin = (int)((b.n * blockIdx.x) / gridDim.x), w_end = (int)((b.n * (blockIdx.x + 1)) / gridDim.x);
-  uint32_t cnt = 0, res_phase = 0;
+  uint32_t ring_slot = 0, ring_ph = 0, res_phase = 0;            // ring position of the consumers (as the producer's)
   int staged_point = -1, fin_w = 0;
   for (int w0 = w_begin; w0 < w_end;) {                          // runs of one segment: every group takes every other batch
     const int64_t seg = (b.g0 + w0) / b.n_per_seg;
@@ -292,11 +292,11 @@ __global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs
         const unsigned char *chunk = qs + (size_t)(k * 2 * KS) * P.pitch_q;                        // resident layout
         const double *bs = cs + (size_t)(k * KS) * NBG * 4 + lr * 4 + lc;
         auto kstep = [&](auto first_c) {                           // the first k-step of a detector clears the accumulators
-          uint32_t slot = 0;
+          const uint32_t slot = ring_slot;
           if (STREAM) {
-            slot = cnt % (uint32_t)P.slots;
-            mbar_wait(full + slot, (cnt / (uint32_t)P.slots) & 1u);
+            mbar_wait(full + slot, ring_ph);
             chunk = qs + slot * slot_bytes;
+            if (++ring_slot == (uint32_t)P.slots) ring_slot = 0, ring_ph ^= 1u;
           }
           if (NRB > 0) {
             double bf[NT], af[NRB > 0 ? NRB : 1];
@@ -318,7 +318,7 @@ __global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs
             __syncwarp();
             if (lane == 0) mm_arrive(empty + slot);
           }
-          ++cnt, bs += NBG * 4, chunk += slot_bytes;
+          bs += NBG * 4, chunk += slot_bytes;
         };
         kstep(std::true_type());
 #pragma unroll 1
