@@ -441,6 +441,8 @@ def gmm_row(rift, torch, h, data, cfg, dm, n_per_round=200_000, rounds=8, n_dist
             "rounds": res["rounds"], "n_evals": res["n_evals"], "ms_total": ms[-1], "evals_per_s": res["n_evals"] / (ms[-1] * 1e-3),
             "lnZ": res["lnZ"], "rel_err": res["rel_err"], "n_ess": res["n_ess"], "n_ess_per_eval": res["n_ess"] / res["n_evals"],
             "n_ess_per_eval_prior_sampling_5d": dm["median_n_ess_5d"] / (data.N),
+            "note": ("n_ess of prior sampling is at its floor of 1 (one sample carries the weight of a point's 1e5 draws), so its "
+                     "per-evaluation figure is an upper bound; tests/test_gpu_gmm.py compares at 4e6-1.6e7 prior draws"),
             "draw_samples_per_s": n / (t_draw * 1e-3), "em_iteration_samples_per_s": n / (t_em * 1e-3),
             "draw_ms_4e6": t_draw, "em_iteration_ms_4e6": t_em}
 
