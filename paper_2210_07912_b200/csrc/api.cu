@@ -350,7 +350,9 @@ void make_mma_plan(rift_ile *h, double delta_t) {
     if (dm > 1e6) return;
     if ((int)dm > halo) halo = (int)dm;
   }
-  const int cand[][2] = {{0, 0}, {1, 8}, {1, 6}, {1, 4}, {1, 3}};   // stream, slots (the deepest ring that fits: a refill takes about 4 k-steps)
+  // resident with three or two warp groups (three windows must fit beside the Q block), then streamed with the deepest ring that
+  // fits (a refill takes about as long as 4 k-steps of tensor work)
+  const int cand[][3] = {{0, 0, 3}, {0, 0, 2}, {1, 8, 1}, {1, 6, 1}, {1, 4, 1}, {1, 3, 1}};   // stream, slots, groups
   for (const auto &c : cand) {
     p = MmaPlan{};
     p.K = h->K;
@@ -360,6 +362,7 @@ void make_mma_plan(rift_ile *h, double delta_t) {
     p.H = halo;
     p.stream = c[0];
     p.slots = c[1];
+    p.groups = c[2];
     if (lnl_mma_finish_plan(p) && lnl_mma_smem_bytes(p) <= 227u * 1024u) {
       p.ok = 1;
       return;

@@ -30,18 +30,19 @@
 
 namespace {
 
-constexpr int MM_WARPS = 16;                       // warps per CTA
 constexpr int MM_MAX_SLOTS = 8;
 
-// Two shapes of the CTA.  Resident Q block: two independent groups of 8 warps, each with its own batch of 8 samples (one
+// Two shapes of the CTA.  Resident Q block: two or three independent groups of 8 warps (three when three windows fit beside the Q
+// block: 24 warps of 80 registers; measured +4 % on C1 / C3 over two groups of 128 registers), each with its own batch of 8 samples (one
 // 8-column tile), exchange buffer and named barrier, so that the tensor phase of one group runs under the exchange and
 // exponential phases of the other.  Streamed Q: one group of 15 warps with batches of 16 samples (two tiles per A fragment:
 // half the chunk traffic per sample) and the 16th warp as the bulk-copy producer.
-template <bool STREAM>
+template <bool STREAM, int NG = 2>
 struct MmaShape {
   static constexpr int NT = STREAM ? 2 : 1;        // 8-sample tiles per batch
   static constexpr int NBG = 8 * NT;               // samples per batch of a group
-  static constexpr int GROUPS = STREAM ? 1 : 2;
+  static constexpr int GROUPS = STREAM ? 1 : NG;   // resident: NG = 2 or 3 groups (3: 24 warps of 80 registers, when three windows fit)
+  static constexpr int WARPS = STREAM ? 16 : 8 * NG;
   static constexpr int GW = STREAM ? 15 : 8;       // warps per group
   static constexpr int RBW = STREAM ? 4 : 8;       // row blocks (of 8 rows) per warp: wg + GW i
   static constexpr int GTHR = GW * 32;
@@ -90,7 +91,7 @@ struct MmaSmem {                                   // byte offsets inside dynami
 
 __host__ __device__ inline MmaSmem mma_smem(const MmaPlan &p) {
   MmaSmem L;
-  const uint32_t nbg = p.stream ? 16u : 8u, groups = p.stream ? 1u : 2u, rb = p.stream ? 128u : 64u;
+  const uint32_t nbg = p.stream ? 16u : 8u, groups = p.stream ? 1u : (uint32_t)p.groups, rb = p.stream ? 128u : 64u;
   L.bars = 0;                                                          // full[8], empty[8], resident
   L.grp = 256;
   L.coef_bytes = (uint32_t)p.K * p.KS * nbg * 4 * 8;                   // cs[K][KS][NBG][4] doubles, two buffers at offset 0
@@ -123,9 +124,9 @@ struct MmaArgs {
   double ln_ntau;
 };
 
-template <bool STREAM, int NE, int PFN>
-__global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs A) {
-  typedef MmaShape<STREAM> S;
+template <bool STREAM, int NE, int PFN, int NG>
+__global__ void __launch_bounds__(MmaShape<STREAM, NG>::WARPS * 32, 1) lnl_mma_kernel(const MmaArgs A) {
+  typedef MmaShape<STREAM, NG> S;
   constexpr int NT = S::NT, NBG = S::NBG, GW = S::GW, RBW = S::RBW, GTHR = S::GTHR, XP = S::XP, RS = S::RS, JS = S::JS;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const MmaPlan &P = A.p;
@@ -426,33 +427,33 @@ __global__ void __launch_bounds__(MM_WARPS * 32, 1) lnl_mma_kernel(const MmaArgs
       }
       fin_w = fin_w + 1 == GW ? 0 : fin_w + 1;
     }
-    if (!STREAM) mm_bar(3, MM_WARPS * 32);                       // both groups leave the run (and its Q block) together
+    if (!STREAM) mm_bar(8, S::WARPS * 32);                       // all groups leave the run (and its Q block) together
     else mm_bar(bar_id, GTHR);
     w0 = run_end;
   }
 }
 
-template <bool STREAM, int NE, int PFN>
+template <bool STREAM, int NE, int PFN, int NG>
 cudaError_t launch_t(const MmaArgs &a, int n_sm, cudaStream_t s) {
-  auto kern = lnl_mma_kernel<STREAM, NE, PFN>;
+  auto kern = lnl_mma_kernel<STREAM, NE, PFN, NG>;
   const size_t smem = a.L.total;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   int64_t grid = n_sm;
   const int64_t max_grid = (a.b.n + 15) / 16;
   if (grid > max_grid) grid = max_grid;
-  kern<<<(unsigned)grid, MM_WARPS * 32, smem, s>>>(a);
+  kern<<<(unsigned)grid, MmaShape<STREAM, NG>::WARPS * 32, smem, s>>>(a);
   return cudaGetLastError();
 }
 
-template <bool STREAM, int PFN>
+template <bool STREAM, int PFN, int NG>
 cudaError_t launch_ne(const MmaArgs &a, int n_sm, cudaStream_t s) {
   switch (a.p.ne) {
-    case 4: return launch_t<STREAM, 4, PFN>(a, n_sm, s);
-    case 8: return launch_t<STREAM, 8, PFN>(a, n_sm, s);
-    case 13: return launch_t<STREAM, 13, PFN>(a, n_sm, s);
-    case 14: return launch_t<STREAM, 14, PFN>(a, n_sm, s);
-    case 16: return launch_t<STREAM, 16, PFN>(a, n_sm, s);
+    case 4: return launch_t<STREAM, 4, PFN, NG>(a, n_sm, s);
+    case 8: return launch_t<STREAM, 8, PFN, NG>(a, n_sm, s);
+    case 13: return launch_t<STREAM, 13, PFN, NG>(a, n_sm, s);
+    case 14: return launch_t<STREAM, 14, PFN, NG>(a, n_sm, s);
+    case 16: return launch_t<STREAM, 16, PFN, NG>(a, n_sm, s);
     default: return cudaErrorInvalidValue;
   }
 }
@@ -528,6 +529,7 @@ cudaError_t launch_lnl_mma(const MmaPlan &p, const void *q, const Batch &b, cons
   a.lnL_out = lnL_out;
   a.ln_ntau = log((double)p.n_tau);
   if (n_launch) ++*n_launch;
-  if (p.stream) return launch_ne<true, 0>(a, n_sm, s);
-  return p.pfn == 2 ? launch_ne<false, 2>(a, n_sm, s) : launch_ne<false, 0>(a, n_sm, s);
+  if (p.stream) return launch_ne<true, 0, 2>(a, n_sm, s);
+  if (p.groups == 3) return p.pfn == 2 ? launch_ne<false, 2, 3>(a, n_sm, s) : launch_ne<false, 0, 3>(a, n_sm, s);
+  return p.pfn == 2 ? launch_ne<false, 2, 2>(a, n_sm, s) : launch_ne<false, 0, 2>(a, n_sm, s);
 }

@@ -125,6 +125,7 @@ struct MmaPlan {
   int32_t j0, circular;
   int32_t H;                     // circular: bound on |s_k - s_0| (halo rows); guard band: n_t - n_tau
   int32_t ne, pfn, xb_rows, stream, slots;
+  int32_t groups;                // resident shape: independent 8-warp groups per CTA (2 or 3)
   int32_t pitch_q;               // bytes per mode row: n_r * 16 + 64
   int64_t point_stride;          // bytes per intrinsic point
 };
