@@ -47,7 +47,8 @@ int rift_gmm_get_model(const rift_gmm_t *h, double *mu, double *cov, double *pi,
  *   n_iter   : at most this many M-steps;  tol : stop when |ln L - ln L_prev| < tol (0 = never);  reg : added to the diagonal
  *              of every Sigma_k (Eq. (A5)).
  *   merge    : 0 = the fitted model replaces the handle's (n_trained = n); 1 = it is matched to the handle's model by the
- *              permutation that minimises Eq. (A8) and merged into it by Eq. (A9)-(A11) with N = n_trained, M = n.
+ *              permutation that minimises Eq. (A8) and merged into it by Eq. (A9)-(A11) with N = n_trained, M = n (a model
+ *              trained on 0 samples is replaced).
  *   iters_done, loglik : HOST outputs (may be NULL): M-steps done, ln L of the last E-step.
  * Synchronises cuda_stream once per iteration (the M-step's 50 sums come back to the host).  RIFT_ESTATE if every weight is
  * zero or a covariance stops being positive definite (the handle's model is then unchanged). */
