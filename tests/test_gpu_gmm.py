@@ -246,3 +246,40 @@ def test_gmm_loop_on_the_ile_likelihood_matches_prior_sampling(torch, oracle):
     assert abs(res["lnZ"] - float(ref["lnZ"][0])) < 4.0 * sigma + 0.02, (res, ref)
     # efficiency: effective samples per evaluation at least 5x those of prior sampling
     assert res["n_ess"] / res["n_evals"] > 5.0 * float(ref["n_ess"][0]) / (4 * n_ref), (res, ref)
+
+
+def test_rosenbrock_evidence_of_fig7_with_the_gmm_integrator(torch, oracle):
+    """Fig. 7 (:356) with the GMM integrator: the evidence of the two-dimensional Rosenbrock likelihood, -5.804
+    (tests/golden/fig7_rosenbrock.txt), from 1e6 evaluations in batches of 1e4 -- a curved, strongly correlated ridge, which a
+    correlated mixture follows where a separable sampler cannot.  Draws, densities, EM refits (merged online) and the pooled
+    evidence (Eq. (20)-(21)) come from the library; only the integrand is the test's."""
+    import os
+    from paper_2210_07912_b200 import synth
+    from helpers import build, create
+    path = os.path.join(os.path.dirname(__file__), "golden", "fig7_rosenbrock.txt")
+    gold = [ln.split() for ln in open(path) if ln.strip() and not ln.startswith("#")][0]
+    ln_z, n_total, n = float(gold[0]), int(gold[1]), int(gold[2])
+    inp = build(oracle, synth.CONFIGS[0])
+    h = create(rift, inp, rift.RIFT_PREC_MIXED)                             # only its reduce is used
+    stream = torch.cuda.current_stream().cuda_stream
+    L = 5.0
+    g = rift.rift_gmm_create(2, 6, [-L, -L], [L, L])
+    xs = [torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(2)]
+    lps = torch.empty(n, dtype=torch.float64, device="cuda")
+    lom = torch.empty(n, dtype=torch.float64, device="cuda")
+    pooled = None
+    for it in range(n_total // n):
+        rift.rift_gmm_draw(g, n, 78, it * n, xs, lps, cuda_stream=stream)
+        lnL = -((1.0 - xs[0]) ** 2 + 100.0 * (xs[1] - xs[0] * xs[0]) ** 2)
+        lw = -math.log((2 * L) ** 2) - lps
+        pooled = rift.rift_ile_reduce(h, 1, n, lnL, lw, cuda_stream=stream, merge=0 if it == 0 else 1)
+        rift.rift_gmm_add(n, [lnL, lw], lom, stream)
+        rift.rift_gmm_fit_tempered(g, n, xs, lom, 300.0, 10, 1e-6, 1e-6, merge=1 if it > 0 else 0, cuda_stream=stream)
+    rel = float(pooled["rel_err"][0])
+    assert rel < 0.03, pooled
+    assert abs(float(pooled["lnZ"][0]) - ln_z) < 4 * rel + 5e-4, pooled    # the paper prints three decimals
+    # the correlated mixture follows the curved ridge: two orders of magnitude more effective samples than the separable
+    # histogram sampler of NEXT-1 reaches on the same budget (golden file: the paper's n_ESS ~ 1400 for AC; observed 4.4e5)
+    assert pooled["n_ess"][0] > 100.0 * float(gold[3]), (pooled, gold)
+    rift.rift_gmm_destroy(g)
+    rift.rift_ile_destroy(h)
