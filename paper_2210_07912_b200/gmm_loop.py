@@ -57,7 +57,7 @@ def integrate(h_ile, samplers: dict, point_id: int, R, gmst_rad: float, d_min_mp
     lnL = torch.empty(n, dtype=torch.float64, device="cuda")
     # rift_ac_ile_ln_weight includes ln p(D) of the constant distance row; the marginal already holds the distance prior
     ln_p_dist = math.log(3.0 * d_const ** 2 / (d_max_mpc ** 3 - d_min_mpc ** 3))
-    out, rounds = None, 0
+    out, rounds, n_refit_failures = None, 0, 0
     while rounds < max_rounds:
         for gi, (name, rows, _lo, _hi) in enumerate(GROUPS):
             # every group has its own random-number stream: seed + group index
@@ -75,7 +75,13 @@ def integrate(h_ile, samplers: dict, point_id: int, R, gmst_rad: float, d_min_mp
         rift.rift_gmm_add(n, [lnL, ln_w], ln_om, cuda_stream)
         for name, rows, _lo, _hi in GROUPS:
             if name in adapt:
-                rift.rift_gmm_fit_tempered(samplers[name], n, [x[r] for r in rows], ln_om, ess_min, em_iters, em_tol, reg,
-                                           merge=1 if rounds > 1 else 0, cuda_stream=cuda_stream)
+                try:
+                    rift.rift_gmm_fit_tempered(samplers[name], n, [x[r] for r in rows], ln_om, ess_min, em_iters, em_tol, reg,
+                                               merge=1 if rounds > 1 else 0, cuda_stream=cuda_stream)
+                except rift.RiftError as err:        # an emptied component or a singular covariance: the library left the
+                    if err.code != rift.RIFT_ESTATE:  # group's model unchanged; keep sampling from it
+                        raise
+                    n_refit_failures += 1
     return dict(lnZ=float(out["lnZ"][0]) - ln_p_dist, rel_err=float(out["rel_err"][0]), n_eff=float(out["n_eff"][0]),
-                n_ess=float(out["n_ess"][0]), rounds=rounds, n_evals=rounds * n, next_offset=offset + rounds * n)
+                n_ess=float(out["n_ess"][0]), rounds=rounds, n_evals=rounds * n, next_offset=offset + rounds * n,
+                refit_failures=n_refit_failures)

@@ -283,3 +283,61 @@ def test_rosenbrock_evidence_of_fig7_with_the_gmm_integrator(torch, oracle):
     assert pooled["n_ess"][0] > 100.0 * float(gold[3]), (pooled, gold)
     rift.rift_gmm_destroy(g)
     rift.rift_ile_destroy(h)
+
+
+def test_fig6_correlated_three_dimensional_gaussian_with_pairwise_groups(torch, oracle):
+    """Fig. 6 (:332): weighted samples of a correlated three-dimensional Gaussian likelihood after a fixed number of evaluations;
+    the one-dimensional cumulative distributions they imply are compared with the true ones.  The sampler is a product of a
+    correlated pair (x0, x1) and a single dimension x2 (the pairwise-correlated form: the x2 correlations are left to the
+    weights), refitted every round with the online merge."""
+    from scipy import stats
+    from paper_2210_07912_b200 import synth
+    from helpers import build, create
+    inp = build(oracle, synth.CONFIGS[0])
+    h = create(rift, inp, rift.RIFT_PREC_MIXED)                             # only its reduce is used
+    stream = torch.cuda.current_stream().cuda_stream
+    L, n, rounds = 6.0, 20_000, 20
+    mu = np.array([0.5, -1.0, 1.5])
+    sd = np.array([0.4, 0.7, 0.5])
+    corr = np.array([[1.0, 0.85, 0.3], [0.85, 1.0, 0.2], [0.3, 0.2, 1.0]])
+    cov = corr * np.outer(sd, sd)
+    prec = torch.from_numpy(np.linalg.inv(cov)).cuda()
+    ln_norm = -0.5 * math.log(np.linalg.det(cov)) - 1.5 * math.log(2 * math.pi)
+    g01 = rift.rift_gmm_create(2, 2, [-L, -L], [L, L])
+    g2 = rift.rift_gmm_create(1, 1, [-L], [L])
+    x = torch.empty((3, n), dtype=torch.float64, device="cuda")
+    lp = torch.empty((2, n), dtype=torch.float64, device="cuda")
+    lom = torch.empty(n, dtype=torch.float64, device="cuda")
+    keep_x, keep_w = [], []
+    pooled = None
+    for it in range(rounds):
+        rift.rift_gmm_draw(g01, n, 31, it * n, [x[0], x[1]], lp[0], cuda_stream=stream)
+        rift.rift_gmm_draw(g2, n, 32, it * n, [x[2]], lp[1], cuda_stream=stream)
+        d = x - torch.from_numpy(mu).cuda()[:, None]
+        lnL = ln_norm - 0.5 * torch.einsum("in,ij,jn->n", d, prec, d)
+        lw = -3.0 * math.log(2 * L) - lp[0] - lp[1]
+        pooled = rift.rift_ile_reduce(h, 1, n, lnL, lw, cuda_stream=stream, merge=0 if it == 0 else 1)
+        rift.rift_gmm_add(n, [lnL, lw], lom, stream)
+        for g, rows in ((g01, [x[0], x[1]]), (g2, [x[2]])):
+            rift.rift_gmm_fit_tempered(g, n, rows, lom, 300.0, 10, 1e-6, 1e-6, merge=1 if it > 0 else 0, cuda_stream=stream)
+        if it >= rounds // 2:                                                # the adapted half of the run, as the figure's samples
+            keep_x.append(x.cpu().numpy().copy())
+            keep_w.append(np.exp((lnL + lw).cpu().numpy()))
+    # evidence: the Gaussian's mass in the box (1 to 1e-12) over the prior volume
+    rel = float(pooled["rel_err"][0])
+    assert rel < 0.01 and abs(float(pooled["lnZ"][0]) + 3.0 * math.log(2 * L)) < 4 * rel + 1e-3, pooled
+    assert pooled["n_ess"][0] > 0.03 * rounds * n, pooled      # pooled over ALL rounds: the wide first rounds weigh it down
+    # one-dimensional weighted CDFs against the true marginals
+    X, W = np.concatenate(keep_x, axis=1), np.concatenate(keep_w)
+    for dim in range(3):
+        order = np.argsort(X[dim])
+        cdf = np.cumsum(W[order]) / W.sum()
+        true = stats.norm.cdf(X[dim][order], mu[dim], sd[dim])
+        assert np.max(np.abs(cdf - true)) < 0.01, (dim, np.max(np.abs(cdf - true)))
+    # the pair's mixture has found the correlation
+    m, c, p, _ = rift.rift_gmm_get_model(g01)
+    mix_cov = sum(p[k] * (c[k] + np.outer(m[k], m[k])) for k in range(2)) - np.outer(p @ m, p @ m)
+    assert abs(mix_cov[0, 1] / np.sqrt(mix_cov[0, 0] * mix_cov[1, 1]) - 0.85) < 0.05
+    rift.rift_gmm_destroy(g01)
+    rift.rift_gmm_destroy(g2)
+    rift.rift_ile_destroy(h)
