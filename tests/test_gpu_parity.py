@@ -705,3 +705,45 @@ def test_c4_full_size(torch, oracle):
 def test_c4_full_size_lnz(torch, oracle):
     # ... and every sample of two whole points with lnZ / n_eff / n_ess (2.4e12 flop per point on the host: minutes)
     _full_size_sampled(torch, oracle, synth.CONFIGS[4], (rift.RIFT_PREC_MIXED, rift.RIFT_PREC_FP64), 2, 1, lnz_points=2)
+
+
+# ------------------------------------------------------------------------------------------------ seeded random shapes
+@pytest.mark.parametrize("precision", ["fp64", "mixed"])
+def test_random_shapes_every_kernel_family(torch, oracle, precision):
+    """24 seeded random shapes (1-5 detectors, 1-8 modes, windows of 33-499 samples at 1-4 kHz, circular and guard-band, 1-300
+    samples in two segments of different points) through every kernel family that takes them: the row-block counts, wrap
+    thresholds, halo sizes and ragged tails that the fixed configs never visit.  fp64: relative 1e-10; mixed: |dlnL| <= 2e-3."""
+    rng = np.random.default_rng(20221007 + (0 if precision == "fp64" else 1))
+    dets = ("H1", "L1", "V1", "S0", "S1")
+    modes = ((2, 2), (2, -2), (2, 1), (2, -1), (2, 0), (3, 3), (3, -3), (3, 2))
+    prec = rift.RIFT_PREC_FP64 if precision == "fp64" else rift.RIFT_PREC_MIXED
+    kernels = (rift.RIFT_KERNEL_MMA, rift.RIFT_KERNEL_SKY) if precision == "fp64" else (
+        rift.RIFT_KERNEL_AUTO, rift.RIFT_KERNEL_TC, rift.RIFT_KERNEL_TCS, rift.RIFT_KERNEL_SKY)
+    seen = set()
+    for trial in range(24):
+        K, M = int(rng.integers(1, 6)), int(rng.integers(1, 9))
+        f_s = float(rng.choice([1024.0, 2048.0, 4096.0]))
+        cfg = synth.with_overrides(synth.CONFIGS[1], detectors=dets[:K], modes=modes[:M], f_s=f_s,
+                                   t_window=int(rng.integers(16, 250)) / f_s, n_points=2)
+        inp = build(oracle, cfg, n_points=2)
+        n = int(rng.integers(1, 300))
+        params = np.concatenate([synth.draw_samples(cfg, 1000 + 2 * trial + s, n)[0] for s in range(2)], axis=1)
+        n_tau = None
+        if rng.random() < 0.3:
+            n_tau = cfg.n_t - 2 * (int(np.ceil(2 * 6.4e6 / 299792458.0 * f_s)) + 2) - 2
+            n_tau = n_tau if n_tau >= 8 else None
+        h = create(rift, inp, prec, n_tau=n_tau)
+        ref = np.concatenate([oracle_eval(oracle, inp, p, params[:, s * n:(s + 1) * n], n_tau=n_tau)[0]
+                              for s, p in enumerate((1, 0))])
+        for kernel in kernels:
+            got = gpu_eval(torch, h, [1, 0], n, params, want_shifts=False, kernel=kernel)[0].cpu().numpy()
+            name = rift.rift_ile_kernel_name(h)
+            seen.add(name)
+            if precision == "fp64":
+                assert np.max(rel_err(got, ref)) < TOL_FP64_REL, (trial, K, M, cfg.n_t, n_tau, n, name)
+            else:
+                assert np.max(np.abs(got - ref)) < TOL_MIXED_LNL, (trial, K, M, cfg.n_t, n_tau, n, name)
+        rift.rift_ile_destroy(h)
+    want = {"lnl_mma<f64,resident>", "lnl_mma<f64,stream>", "lnl_sky<f64>"} if precision == "fp64" else {
+        "lnl_tc<f16x3>", "lnl_tcs<f16x3>", "lnl_sky<f16x3>"}
+    assert want <= seen, seen
