@@ -321,13 +321,26 @@ lnl_direct_dm_kernel(QStore q, Batch b, Workspace ws, int K, DmargDev dm, double
             cq[n] = cl2_s[ch + n];
             s[n] = (Real)0;
           }
+          if (sizeof(Real) == 4) {
+            // a slot (32 consecutive window entries, one per lane) whose largest exponent over the chunk's nodes lies below -40
+            // is skipped by the whole warp: every window sum is >= 1 (the maximum entry), so the dropped terms change it by
+            // < N_tau 2^-40 relative.  Near nodes (large c) skip all slots but those around the peak: 1.4x on C1.  (The fp64
+            // kernel keeps all terms: its 13 x 8 independent polynomial chains lose more to the branch than the skip saves)
+            Real cmin = cq[0];
 #pragma unroll
-          for (int i = 0; i < SLOTS; ++i)
+            for (int n = 1; n < 8; ++n) cmin = fmin(cmin, cq[n]);
 #pragma unroll
-            for (int n = 0; n < 8; ++n) {
-              if (sizeof(Real) == 4) s[n] += (Real)fast_exp2((float)x[i] * (float)cq[n]);
-              else s[n] += (Real)(x[i] == -INFINITY ? 0.0 : poly_exp2((double)x[i] * (double)cq[n]));
+            for (int i = 0; i < SLOTS; ++i) {
+              if (!__any_sync(0xffffffffu, x[i] * cmin > (Real)-40)) continue;
+#pragma unroll
+              for (int n = 0; n < 8; ++n) s[n] += (Real)fast_exp2((float)x[i] * (float)cq[n]);
             }
+          } else {
+#pragma unroll
+            for (int i = 0; i < SLOTS; ++i)
+#pragma unroll
+              for (int n = 0; n < 8; ++n) s[n] += (Real)(x[i] == -INFINITY ? 0.0 : poly_exp2((double)x[i] * (double)cq[n]));
+          }
           const Real tot = treduce8r(s, lane, [](Real a, Real c) { return a + c; });
           if ((lane & 3) == 0) S_s[ch + (lane >> 2)] += tot;
         }
