@@ -50,8 +50,10 @@ int rift_gmm_get_model(const rift_gmm_t *h, double *mu, double *cov, double *pi,
  *              permutation that minimises Eq. (A8) and merged into it by Eq. (A9)-(A11) with N = n_trained, M = n (a model
  *              trained on 0 samples is replaced).
  *   iters_done, loglik : HOST outputs (may be NULL): M-steps done, ln L of the last E-step.
- * Synchronises cuda_stream once per iteration (the M-step's 50 sums come back to the host).  RIFT_ESTATE if every weight is
- * zero or a covariance stops being positive definite (the handle's model is then unchanged). */
+ * The whole iteration runs on the device (E-step with the M-step's sums, a fixed-order add, the M-step and its convergence and
+ * validity tests in a one-thread kernel, the model in device memory); the host reads the state back every 8 iterations and once
+ * at the end.  RIFT_ESTATE if every weight is zero, a component empties or a covariance stops being positive definite (the
+ * handle's model is then unchanged). */
 int rift_gmm_fit(rift_gmm_t *h, int64_t n, const double *const *x, const double *ln_w, int32_t n_iter, double tol, double reg,
                  int32_t merge, int32_t *iters_done, double *loglik, void *cuda_stream);
 

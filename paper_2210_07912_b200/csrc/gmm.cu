@@ -2,17 +2,20 @@
 // and Appendix A (:562-625), readings G1-G6 of DESIGN.md section 14.
 //
 // Device work (per sample, embarrassingly parallel, HBM-bound at 8 (n_dim + 1) bytes per sample and pass):
-//   gmm_max_kernel     max of the log-weights (block partials; the host takes the maximum of <= 296 numbers)
+//   gmm_max_kernel     max of the log-weights (block partials; gmm_maxfin_kernel takes their maximum into the fit's state)
+//   gmm_ess_kernel     sum w^t, sum w^2t of reading G7; gmm_ess_step_kernel: one bisection step on the device
 //   gmm_em_kernel      one E-step fused with the sums of the M-step: r_nk = N_k pi_k / sum_j N_j pi_j by log-sum-exp, then per
 //                      component sum w r, sum w r (x - mu_old), sum w r (x - mu_old)(x - mu_old)^T, plus sum w ln P and sum w,
-//                      in registers, reduced by warp shuffles and shared memory to one partial row per block
-//   gmm_sum_kernel     the partial rows added in a fixed order (deterministic) to the 50 numbers the host turns into
-//                      Eq. (A4)-(A6)
+//                      in registers, reduced by warp shuffles and shared memory to one partial row per block; the model is read
+//                      from the fit's device-resident state (EmState)
+//   gmm_sum_kernel     the partial rows added in a fixed order (deterministic)
+//   gmm_mstep_kernel   Eq. (A4)-(A6), the convergence test and the validity checks, one thread (<= 8 components): the next
+//                      E-step's model is written to the device state, no host round trip inside an iteration
 //   gmm_draw_kernel    Eq. (A12)-(A13): component by inverse CDF of pi, box proposal z_j = Phi^-1(Phi(a_j) + u (Phi(b_j) -
 //                      Phi(a_j))), x = mu + A z, retried until x lies in the domain; ln p_s of the accepted point
 //   gmm_density_kernel ln p_s(x) = ln sum_k pi_k N_k(x) / Z_k
-// Host work (n_comp <= 8 numbers of each kind): the M-step's divisions, the 2 x 2 eigen-decomposition, the proposal boxes, the
-// component masses Z_k (Gauss-Legendre), the permutation search of Eq. (A8) and the merge of Eq. (A9)-(A11).
+// Host work (n_comp <= 8 numbers of each kind, once per fit / model change): the 2 x 2 eigen-decomposition, the proposal boxes,
+// the component masses Z_k (Gauss-Legendre), the permutation search of Eq. (A8) and the merge of Eq. (A9)-(A11).
 #include <algorithm>
 #include <cmath>
 #include <cstring>
@@ -196,6 +199,7 @@ struct rift_gmm {
   bool dev_ok = false;
   double *d_partial = nullptr;                     // [GM_BLOCKS][GM_ROW]
   double *d_sums = nullptr;                        // [GM_ROW]
+  void *d_em = nullptr;                            // EmState of a running fit
   unsigned long long *d_fail = nullptr;
 };
 
@@ -231,6 +235,72 @@ __device__ __forceinline__ double gm_log_terms(const GmmDev &g, double x0, doubl
   return m + log(s);
 }
 
+// The model of a running EM fit, kept on the device across iterations (no host round trip per iteration)
+struct EmState {
+  double mu[GM_MAXK][2], cov[GM_MAXK][3], pi[GM_MAXK];   // Eq. (A4)-(A6) of the last M-step
+  double prec[GM_MAXK][3], lnc[GM_MAXK];                 // what the next E-step reads
+  double ll, prev;                                       // ln L of the last E-step, and of the one before the last M-step
+  int it, done, bad;                                     // M-steps done; converged / stopped; an empty component or a bad covariance
+  double w_max, temper;                                  // maximum of the log-weights; the exponent of reading G7
+  double b_lo, b_hi, beta;                               // bisection bracket and the exponent under test
+  int temper_set;
+};
+
+__device__ __forceinline__ void em_derive(int d, int k, EmState &st) {
+  const double a = st.cov[k][0], b = d == 2 ? st.cov[k][1] : 0.0, c = d == 2 ? st.cov[k][2] : 1.0;
+  const double det = a * c - b * b;
+  st.prec[k][0] = c / det, st.prec[k][1] = -b / det, st.prec[k][2] = a / det;
+  st.lnc[k] = (st.pi[k] > 0.0 ? log(st.pi[k]) : -INFINITY) - 0.5 * log(det) - 0.5 * d * 1.8378770664093454836;
+}
+
+// Eq. (A4)-(A6) from the sums about the old means, the convergence test and the validity checks: one thread (<= 8 components)
+__global__ void gmm_mstep_kernel(const double *__restrict__ sums, EmState *__restrict__ stp, int d, int K, double reg, double tol) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  EmState &st = *stp;
+  if (st.done) return;
+  const double W = sums[GM_MAXK * 6 + 1];
+  if (!(W > 0.0)) {
+    st.bad = st.done = 1;
+    return;
+  }
+  const double ll = sums[GM_MAXK * 6] / W;
+  st.ll = ll;
+  if (st.it > 0 && fabs(ll - st.prev) < tol) {
+    st.done = 1;
+    return;
+  }
+  double mu[GM_MAXK][2], cov[GM_MAXK][3], pi[GM_MAXK], psum = 0.0;
+  bool ok = true;
+  for (int k = 0; k < K; ++k) {
+    const double *a = sums + 6 * k;
+    if (!(a[0] > 0.0)) ok = false;                               // an empty component
+    const double e0 = a[1] / a[0], e1 = a[2] / a[0];
+    mu[k][0] = st.mu[k][0] + e0;
+    mu[k][1] = d == 2 ? st.mu[k][1] + e1 : 0.0;
+    cov[k][0] = a[3] / a[0] - e0 * e0 + reg;
+    cov[k][1] = d == 2 ? a[4] / a[0] - e0 * e1 : 0.0;
+    cov[k][2] = d == 2 ? a[5] / a[0] - e1 * e1 + reg : 1.0;
+    pi[k] = a[0] / W;
+    psum += pi[k];
+    const double det = cov[k][0] * cov[k][2] - cov[k][1] * cov[k][1];
+    if (!(pi[k] >= 0.0) || !isfinite(pi[k]) || !isfinite(mu[k][0]) || !isfinite(mu[k][1]) || !(cov[k][0] > 0.0) || !isfinite(cov[k][0]) ||
+        (d == 2 && (!(cov[k][2] > 0.0) || !(det > 0.0) || !isfinite(det))))
+      ok = false;
+  }
+  if (!ok || !(fabs(psum - 1.0) < 1e-9)) {
+    st.bad = st.done = 1;                                        // the model of the last valid M-step stays
+    return;
+  }
+  for (int k = 0; k < K; ++k) {
+    st.mu[k][0] = mu[k][0], st.mu[k][1] = mu[k][1];
+    st.cov[k][0] = cov[k][0], st.cov[k][1] = cov[k][1], st.cov[k][2] = cov[k][2];
+    st.pi[k] = pi[k];
+    em_derive(d, k, st);
+  }
+  st.prev = ll;
+  st.it += 1;
+}
+
 __global__ void __launch_bounds__(GM_THREADS) gmm_max_kernel(int64_t n, const double *__restrict__ ln_w, double *__restrict__ partial) {
   __shared__ double s_w[GM_THREADS / 32];
   double m = -INFINITY;
@@ -248,10 +318,49 @@ __global__ void __launch_bounds__(GM_THREADS) gmm_max_kernel(int64_t n, const do
   }
 }
 
+// maximum of the block maxima; no finite weight at all stops the fit
+__global__ void gmm_maxfin_kernel(int n_blocks, const double *__restrict__ partial, EmState *__restrict__ stp) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  double m = -INFINITY;
+  for (int b = 0; b < n_blocks; ++b) m = fmax(m, partial[b]);
+  stp->w_max = m;
+  if (!(m > -INFINITY) || !isfinite(m)) stp->bad = stp->done = 1;
+}
+
+// one step of reading G7 on the device: step 0 tests temper = 1, steps 1..20 bisect [0, 1]; the exponent under test is
+// stp->beta, the sums of the pass just made are in `partial`
+__global__ void gmm_ess_step_kernel(int n_blocks, const double *__restrict__ partial, EmState *__restrict__ stp, double ess_min,
+                                    int step) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  EmState &st = *stp;
+  if (st.done || st.temper_set) return;
+  double s1 = 0.0, s2 = 0.0;
+  for (int b = 0; b < n_blocks; ++b) s1 += partial[2 * b], s2 += partial[2 * b + 1];
+  const double ess = s2 > 0.0 ? s1 * s1 / s2 : 0.0;
+  if (step == 0) {
+    if (ess >= ess_min) {
+      st.temper = 1.0;
+      st.temper_set = 1;
+    } else {
+      st.b_lo = 0.0, st.b_hi = 1.0, st.beta = 0.5;
+    }
+    return;
+  }
+  if (ess >= ess_min) st.b_lo = st.beta;
+  else st.b_hi = st.beta;
+  st.beta = 0.5 * (st.b_lo + st.b_hi);
+  if (step == 20) {
+    st.temper = st.b_lo;
+    st.temper_set = 1;
+  }
+}
+
 // sum w^beta and sum w^(2 beta), w = exp(ln_w - w_max): the tempered effective sample size (sum)^2 / (sum of squares)
-__global__ void __launch_bounds__(GM_THREADS) gmm_ess_kernel(int64_t n, const double *__restrict__ ln_w, double w_max, double beta,
-                                                             double *__restrict__ partial) {
+__global__ void __launch_bounds__(GM_THREADS) gmm_ess_kernel(int64_t n, const double *__restrict__ ln_w,
+                                                             const EmState *__restrict__ stp, double *__restrict__ partial) {
   __shared__ double s_w[GM_THREADS / 32][2];
+  if (stp->done || stp->temper_set) return;
+  const double w_max = stp->w_max, beta = stp->beta;
   double s1 = 0.0, s2 = 0.0;
   for (int64_t i = (int64_t)blockIdx.x * GM_THREADS + threadIdx.x; i < n; i += (int64_t)gridDim.x * GM_THREADS) {
     const double v = ln_w[i];
@@ -276,9 +385,21 @@ __global__ void __launch_bounds__(GM_THREADS) gmm_ess_kernel(int64_t n, const do
 }
 
 __global__ void __launch_bounds__(GM_THREADS) gmm_em_kernel(int64_t n, const double *__restrict__ x0p, const double *__restrict__ x1p,
-                                                            const double *__restrict__ ln_w, double w_max, double temper,
-                                                            const GmmDev g, double *__restrict__ partial) {
+                                                            const double *__restrict__ ln_w,
+                                                            const EmState *__restrict__ stp, int d, int K,
+                                                            double *__restrict__ partial) {
   __shared__ double s_red[GM_THREADS / 32][GM_ROW];
+  __shared__ GmmDev g;                                           // the fields the E-step reads, from the device-resident model
+  if (stp->done) return;                                         // converged or stopped: the remaining launches are no-ops
+  const double w_max = stp->w_max, temper = stp->temper;
+  if (threadIdx.x == 0) g.d = d, g.K = K;
+  if (threadIdx.x < GM_MAXK) {
+    const int k = threadIdx.x;
+    g.mu[k][0] = stp->mu[k][0], g.mu[k][1] = stp->mu[k][1];
+    g.prec[k][0] = stp->prec[k][0], g.prec[k][1] = stp->prec[k][1], g.prec[k][2] = stp->prec[k][2];
+    g.lnc[k] = stp->lnc[k];
+  }
+  __syncthreads();
   double acc[GM_ROW];
 #pragma unroll
   for (int j = 0; j < GM_ROW; ++j) acc[j] = 0.0;
@@ -435,10 +556,11 @@ extern "C" int rift_gmm_create(int32_t n_dim, int32_t n_comp, const double *lo, 
     h->model.cov[k][0] = s0 * s0, h->model.cov[k][1] = 0.0, h->model.cov[k][2] = s1 * s1;
   }
   if (cudaGetDevice(&h->device) != cudaSuccess || cudaMalloc(&h->d_partial, sizeof(double) * GM_BLOCKS * GM_ROW) != cudaSuccess ||
-      cudaMalloc(&h->d_sums, sizeof(double) * GM_ROW) != cudaSuccess || cudaMalloc(&h->d_fail, sizeof(unsigned long long)) != cudaSuccess) {
+      cudaMalloc(&h->d_sums, sizeof(double) * GM_ROW) != cudaSuccess || cudaMalloc(&h->d_em, 4096) != cudaSuccess || cudaMalloc(&h->d_fail, sizeof(unsigned long long)) != cudaSuccess) {
     cudaGetLastError();
     cudaFree(h->d_partial);
     cudaFree(h->d_sums);
+    cudaFree(h->d_em);
     cudaFree(h->d_fail);
     delete h;
     return RIFT_ENOMEM;
@@ -452,6 +574,7 @@ extern "C" int rift_gmm_destroy(rift_gmm_t *h) {
   GmGuard g(h->device);
   cudaFree(h->d_partial);
   cudaFree(h->d_sums);
+  cudaFree(h->d_em);
   cudaFree(h->d_fail);
   delete h;
   return RIFT_OK;
@@ -548,79 +671,62 @@ int gmm_fit_impl(rift_gmm_t *h, int64_t n, const double *const *x, const double 
   GmGuard guard(h->device);
   cudaStream_t s = reinterpret_cast<cudaStream_t>(cuda_stream);
   const int d = h->d, K = h->K, grid = gm_grid(n);
-  double host[GM_BLOCKS > GM_ROW ? GM_BLOCKS : GM_ROW];
-  double w_max = 0.0;
+  // the model lives on the device for the whole fit: E-step + sums, a fixed-order add, the M-step kernel; the host looks at the
+  // state every 8 iterations (converged / stopped?) and once at the end
+  static_assert(sizeof(EmState) <= 4096, "EmState buffer");
+  EmState st;
+  std::memset(&st, 0, sizeof(st));
+  {
+    GmmDev g;
+    derive(d, K, h->lo, h->hi, h->model, false, g);
+    for (int k = 0; k < K; ++k) {
+      for (int j = 0; j < 2; ++j) st.mu[k][j] = h->model.mu[k][j];
+      for (int j = 0; j < 3; ++j) st.cov[k][j] = h->model.cov[k][j], st.prec[k][j] = g.prec[k][j];
+      st.pi[k] = h->model.pi[k];
+      st.lnc[k] = g.lnc[k];
+    }
+    st.ll = -INFINITY;
+    st.w_max = 0.0, st.temper = 1.0, st.beta = 1.0, st.temper_set = (ln_w && ess_min > 0.0) ? 0 : 1;
+  }
+  EmState *d_st = static_cast<EmState *>(h->d_em);
+  if (cudaMemcpyAsync(d_st, &st, sizeof(st), cudaMemcpyHostToDevice, s) != cudaSuccess) return RIFT_ECUDA;
   if (ln_w) {
     gmm_max_kernel<<<grid, GM_THREADS, 0, s>>>(n, ln_w, h->d_partial);
-    if (cudaMemcpyAsync(host, h->d_partial, sizeof(double) * grid, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
-        cudaStreamSynchronize(s) != cudaSuccess)
-      return RIFT_ECUDA;
-    w_max = -INFINITY;
-    for (int b = 0; b < grid; ++b) w_max = std::fmax(w_max, host[b]);
-    if (!(w_max > -INFINITY) || !std::isfinite(w_max)) return RIFT_ESTATE;      // every weight is zero (or +inf)
-  }
-  // G7: the largest temper in [0, 1] (20 bisection steps) whose tempered effective sample size reaches ess_min
-  double temper = 1.0;
-  if (ln_w && ess_min > 0.0) {
-    auto ess = [&](double beta, double &out) -> bool {
-      gmm_ess_kernel<<<grid, GM_THREADS, 0, s>>>(n, ln_w, w_max, beta, h->d_partial);
-      double part[2 * GM_BLOCKS];
-      if (cudaMemcpyAsync(part, h->d_partial, sizeof(double) * 2 * grid, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
-          cudaStreamSynchronize(s) != cudaSuccess)
-        return false;
-      double s1 = 0.0, s2 = 0.0;
-      for (int b = 0; b < grid; ++b) s1 += part[2 * b], s2 += part[2 * b + 1];
-      out = s2 > 0.0 ? s1 * s1 / s2 : 0.0;
-      return true;
-    };
-    double e1;
-    if (!ess(1.0, e1)) return RIFT_ECUDA;
-    if (e1 < ess_min) {
-      double lo_b = 0.0, hi_b = 1.0;
-      for (int step = 0; step < 20; ++step) {
-        const double mid = 0.5 * (lo_b + hi_b);
-        double e;
-        if (!ess(mid, e)) return RIFT_ECUDA;
-        if (e >= ess_min) lo_b = mid;
-        else hi_b = mid;
+    gmm_maxfin_kernel<<<1, 32, 0, s>>>(grid, h->d_partial, d_st);
+    // G7: the largest temper in [0, 1] (20 bisection steps) whose tempered effective sample size reaches ess_min -- 21 passes
+    // over the log-weights, decided on the device (later passes are no-ops once temper = 1 is accepted)
+    if (ess_min > 0.0)
+      for (int step = 0; step <= 20; ++step) {
+        gmm_ess_kernel<<<grid, GM_THREADS, 0, s>>>(n, ln_w, d_st, h->d_partial);
+        gmm_ess_step_kernel<<<1, 32, 0, s>>>(grid, h->d_partial, d_st, ess_min, step);
       }
-      temper = lo_b;
-    }
   }
-  Model m = h->model;
-  double prev = 0.0, ll = -INFINITY;
-  bool have_prev = false;
-  int it = 0;
-  while (it < n_iter) {
-    GmmDev g;
-    derive(d, K, h->lo, h->hi, m, false, g);
-    gmm_em_kernel<<<grid, GM_THREADS, 0, s>>>(n, x[0], d == 2 ? x[1] : nullptr, ln_w, w_max, temper, g, h->d_partial);
-    gmm_sum_kernel<<<1, 64, 0, s>>>(grid, h->d_partial, h->d_sums);
-    if (cudaGetLastError() != cudaSuccess || cudaMemcpyAsync(host, h->d_sums, sizeof(double) * GM_ROW, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+  for (int it0 = 0; it0 < n_iter && !st.done; it0 += 8) {
+    // n_iter M-steps need n_iter E-steps; a tolerance stop is detected by the E-step after the last M-step it follows
+    const int todo = std::min(8, n_iter - it0);
+    for (int j = 0; j < todo; ++j) {
+      gmm_em_kernel<<<grid, GM_THREADS, 0, s>>>(n, x[0], d == 2 ? x[1] : nullptr, ln_w, d_st, d, K, h->d_partial);
+      gmm_sum_kernel<<<1, 64, 0, s>>>(grid, h->d_partial, h->d_sums);
+      gmm_mstep_kernel<<<1, 32, 0, s>>>(h->d_sums, d_st, d, K, reg, tol);
+    }
+    if (cudaGetLastError() != cudaSuccess || cudaMemcpyAsync(&st, d_st, sizeof(st), cudaMemcpyDeviceToHost, s) != cudaSuccess ||
         cudaStreamSynchronize(s) != cudaSuccess)
       return RIFT_ECUDA;
-    const double W = host[GM_MAXK * 6 + 1];
-    if (!(W > 0.0)) return RIFT_ESTATE;
-    ll = host[GM_MAXK * 6] / W;
-    if (have_prev && std::fabs(ll - prev) < tol) break;
-    Model nm = m;                                          // Eq. (A4)-(A6) from the sums about the old means
-    for (int k = 0; k < K; ++k) {
-      const double *a = host + 6 * k;
-      if (!(a[0] > 0.0)) return RIFT_ESTATE;               // an empty component
-      const double e0 = a[1] / a[0], e1 = a[2] / a[0];
-      nm.mu[k][0] = m.mu[k][0] + e0;
-      nm.mu[k][1] = d == 2 ? m.mu[k][1] + e1 : 0.0;
-      nm.cov[k][0] = a[3] / a[0] - e0 * e0 + reg;
-      nm.cov[k][1] = d == 2 ? a[4] / a[0] - e0 * e1 : 0.0;
-      nm.cov[k][2] = d == 2 ? a[5] / a[0] - e1 * e1 + reg : 1.0;
-      nm.pi[k] = a[0] / W;
-    }
-    if (!model_valid(d, K, nm)) return RIFT_ESTATE;
-    m = nm;
-    prev = ll;
-    have_prev = true;
-    ++it;
   }
+  if (n_iter == 0 && (cudaMemcpyAsync(&st, d_st, sizeof(st), cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+                      cudaStreamSynchronize(s) != cudaSuccess))
+    return RIFT_ECUDA;
+  if (st.bad) return RIFT_ESTATE;                                 // every weight zero, an empty component or a bad covariance
+  const double temper = st.temper;
+  Model m = h->model;
+  for (int k = 0; k < K; ++k) {
+    for (int j = 0; j < 2; ++j) m.mu[k][j] = st.mu[k][j];
+    for (int j = 0; j < 3; ++j) m.cov[k][j] = st.cov[k][j];
+    m.pi[k] = st.pi[k];
+  }
+  if (n_iter > 0 && !model_valid(d, K, m)) return RIFT_ESTATE;
+  const int it = st.it;
+  const double ll = st.ll;
   if (merge && h->n_trained > 0.0) {
     Model out;
     merge_models(d, K, h->model, h->n_trained, m, (double)n, out);
