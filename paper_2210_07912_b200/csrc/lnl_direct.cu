@@ -67,7 +67,7 @@ __device__ __forceinline__ void direct_block(const QStore &q, const typename Cpl
 }
 
 template <typename Real, bool QSMEM, bool EXT>
-__global__ void __launch_bounds__(LNL_THREADS)
+__global__ void __launch_bounds__(LNL_THREADS, 2)
 lnl_direct_kernel(QStore q, Batch b, Workspace ws, int K, double *__restrict__ lnL_out) {
   typedef typename CplxOf<Real>::type CT;
   extern __shared__ __align__(128) unsigned char smem_raw[];
