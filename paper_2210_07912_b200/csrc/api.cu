@@ -352,7 +352,7 @@ void make_mma_plan(rift_ile *h, double delta_t) {
   }
   // resident with three or two warp groups (three windows must fit beside the Q block), then streamed with the deepest ring that
   // fits (a refill takes about as long as 4 k-steps of tensor work)
-  const int cand[][3] = {{0, 0, 3}, {0, 0, 2}, {1, 8, 1}, {1, 6, 1}, {1, 4, 1}, {1, 3, 1}};   // stream, slots, groups
+  const int cand[][3] = {{0, 0, 3}, {0, 0, 2}, {1, 8, 2}, {1, 8, 1}, {1, 6, 1}, {1, 4, 1}, {1, 3, 1}};   // stream, slots, groups
   for (const auto &c : cand) {
     p = MmaPlan{};
     p.K = h->K;

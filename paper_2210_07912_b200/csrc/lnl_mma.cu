@@ -35,16 +35,20 @@ constexpr int MM_MAX_SLOTS = 8;
 // Two shapes of the CTA.  Resident Q block: two or three independent groups of 8 warps (three when three windows fit beside the Q
 // block: 24 warps of 80 registers; measured +4 % on C1 / C3 over two groups of 128 registers), each with its own batch of 8 samples (one
 // 8-column tile), exchange buffer and named barrier, so that the tensor phase of one group runs under the exchange and
-// exponential phases of the other.  Streamed Q: one group of 15 warps with batches of 16 samples (two tiles per A fragment:
-// half the chunk traffic per sample) and the 16th warp as the bulk-copy producer.
+// exponential phases of the other.  Streamed Q: a bulk-copy producer warp feeds a ring of (detector, k-step) chunks to either two
+// groups of 7 warps with batches of 8 samples each (windows up to 448 rows: both groups take every chunk, each for its own batch,
+// and drift apart by up to the ring's depth, so that one group's scatter and exponentials run under the other's tensor phase;
+// C2: 45.3 -> 43.7 ms per 8 points) or one group of 15 warps with batches of 16 samples (two tiles per A fragment).
 template <bool STREAM, int NG = 2>
 struct MmaShape {
-  static constexpr int NT = STREAM ? 2 : 1;        // 8-sample tiles per batch
+  static constexpr int NT = (STREAM && NG == 1) ? 2 : 1;   // 8-sample tiles per batch of a group
   static constexpr int NBG = 8 * NT;               // samples per batch of a group
-  static constexpr int GROUPS = STREAM ? 1 : NG;   // resident: NG = 2 or 3 groups (3: 24 warps of 80 registers, when three windows fit)
+  static constexpr int GROUPS = NG;                // resident: 2 or 3 groups (3: 24 warps of 80 registers, when three windows fit);
+                                                   // streamed: 1 group of 15 warps x 16 samples, or 2 groups of 7 warps x 8 samples that
+                                                   // consume the same ring chunk and drift apart by up to the ring's depth
   static constexpr int WARPS = STREAM ? 16 : 8 * NG;
-  static constexpr int GW = STREAM ? 15 : 8;       // warps per group
-  static constexpr int RBW = STREAM ? 4 : 8;       // row blocks (of 8 rows) per warp: wg + GW i
+  static constexpr int GW = STREAM ? (NG == 1 ? 15 : 7) : 8;   // warps per group
+  static constexpr int RBW = (STREAM && NG == 1) ? 4 : 8;   // row blocks (of 8 rows) per warp: wg + GW i
   static constexpr int GTHR = GW * 32;
   static constexpr int XP = 64 * NT;               // bytes per window row (8-byte slots, swizzled: x_slot)
   static constexpr int RS = 8 * GW;                // rows between two tiles of a thread
@@ -91,7 +95,7 @@ struct MmaSmem {                                   // byte offsets inside dynami
 
 __host__ __device__ inline MmaSmem mma_smem(const MmaPlan &p) {
   MmaSmem L;
-  const uint32_t nbg = p.stream ? 16u : 8u, groups = p.stream ? 1u : (uint32_t)p.groups, rb = p.stream ? 128u : 64u;
+  const uint32_t nbg = (p.stream && p.groups == 1) ? 16u : 8u, groups = (uint32_t)p.groups, rb = nbg * 8u;
   L.bars = 0;                                                          // full[8], empty[8], resident
   L.grp = 256;
   L.coef_bytes = (uint32_t)p.K * p.KS * nbg * 4 * 8;                   // cs[K][KS][NBG][4] doubles, two buffers at offset 0
@@ -146,7 +150,7 @@ __global__ void __launch_bounds__(MmaShape<STREAM, NG>::WARPS * 32, 1) lnl_mma_k
   if (threadIdx.x == 0) {
     for (int i = 0; i < MM_MAX_SLOTS; ++i) {
       mbar_init(full + i, 1);
-      mbar_init(empty + i, GW);
+      mbar_init(empty + i, S::GROUPS * GW);
     }
     mbar_init(resbar, 1);
   }
@@ -156,7 +160,8 @@ __global__ void __launch_bounds__(MmaShape<STREAM, NG>::WARPS * 32, 1) lnl_mma_k
 
 
   // ---------------------------------------------------------------------------------------------- producer warp (ring)
-  if (STREAM && warp == GW) {
+  if (STREAM && warp >= S::GROUPS * GW) {                        // the producer warp; a spare warp (two groups of 7) leaves
+    if (warp > S::GROUPS * GW) return;
     if (lane == 0) {
       const int64_t w_begin = (b.n * blockIdx.x) / gridDim.x, w_end = (b.n * (blockIdx.x + 1)) / gridDim.x;
       uint32_t slot = 0, ph = 0;                                 // ring position: slot and the parity of its use count
@@ -164,7 +169,7 @@ __global__ void __launch_bounds__(MmaShape<STREAM, NG>::WARPS * 32, 1) lnl_mma_k
         const int64_t seg = (b.g0 + w0) / b.n_per_seg;
         const int64_t run_end = min(w_end, (seg + 1) * b.n_per_seg - b.g0);
         const unsigned char *qp = A.q + (int64_t)b.ids[seg] * P.point_stride;
-        for (int64_t s0 = w0; s0 < run_end; s0 += NBG)
+        for (int64_t s0 = w0; s0 < run_end; s0 += S::GROUPS * NBG)   // one pass over the chunks per batch of every group
           for (int k = 0; k < K; ++k)
             for (int s = 0; s < KS; ++s) {
               mbar_wait(empty + slot, ph ^ 1u);
@@ -179,7 +184,7 @@ __global__ void __launch_bounds__(MmaShape<STREAM, NG>::WARPS * 32, 1) lnl_mma_k
   }
 
   // ---------------------------------------------------------------------------------------------- consumer groups
-  const int g = STREAM ? 0 : warp / GW, wg = warp - g * GW, gtid = threadIdx.x - g * GTHR;
+  const int g = warp / GW, wg = warp - g * GW, gtid = threadIdx.x - g * GTHR;
   const int bar_id = 1 + g;
   unsigned char *grp = smem_raw + L.grp + g * L.grp_stride;
   const uint32_t grp_u32 = smem_u32(grp), xb_u32 = grp_u32 + L.xb;
@@ -427,6 +432,18 @@ __global__ void __launch_bounds__(MmaShape<STREAM, NG>::WARPS * 32, 1) lnl_mma_k
       }
       fin_w = fin_w + 1 == GW ? 0 : fin_w + 1;
     }
+    if (STREAM && S::GROUPS > 1) {
+      // a group without a batch in the last pass of the run still takes the pass's chunks off the ring
+      const int n_b = (run_end - w0 + NBG - 1) / NBG, passes = (n_b + S::GROUPS - 1) / S::GROUPS;
+      const int mine = n_b > g ? (n_b - g + S::GROUPS - 1) / S::GROUPS : 0;
+      for (int pass = mine; pass < passes; ++pass)
+        for (int c = 0; c < K * KS; ++c) {
+          mbar_wait(full + ring_slot, ring_ph);
+          __syncwarp();
+          if (lane == 0) mm_arrive(empty + ring_slot);
+          if (++ring_slot == (uint32_t)P.slots) ring_slot = 0, ring_ph ^= 1u;
+        }
+    }
     if (!STREAM) mm_bar(8, S::WARPS * 32);                       // all groups leave the run (and its Q block) together
     else mm_bar(bar_id, GTHR);
     w0 = run_end;
@@ -479,8 +496,8 @@ __global__ void convert_q_mma_kernel(const double2 *__restrict__ src, unsigned c
 // Completes a plan whose K, M, n_t, n_tau, H (circular halo) and stream / slots are set; returns false when the window is too
 // long for the 16 register entries per thread or the row blocks of the CTA.
 bool lnl_mma_finish_plan(MmaPlan &p) {
-  const int gw = p.stream ? MmaShape<true>::GW : MmaShape<false>::GW, js = p.stream ? MmaShape<true>::JS : MmaShape<false>::JS;
-  const int rbw = p.stream ? MmaShape<true>::RBW : MmaShape<false>::RBW, nbg = p.stream ? 16 : 8;
+  const bool wide = p.stream && p.groups == 1;          // one group of 15 warps with batches of 16 samples
+  const int gw = p.stream ? (wide ? 15 : 7) : 8, nbg = wide ? 16 : 8, rbw = wide ? 4 : 8, js = (wide ? 2 : 4) * gw;
   p.KS = (p.M + 1) / 2;
   p.n_r = (p.n_t + 7) & ~7;
   p.circular = p.n_tau == p.n_t ? 1 : 0;
@@ -529,7 +546,7 @@ cudaError_t launch_lnl_mma(const MmaPlan &p, const void *q, const Batch &b, cons
   a.lnL_out = lnL_out;
   a.ln_ntau = log((double)p.n_tau);
   if (n_launch) ++*n_launch;
-  if (p.stream) return launch_ne<true, 0, 2>(a, n_sm, s);
+  if (p.stream) return p.groups == 2 ? launch_ne<true, 0, 2>(a, n_sm, s) : launch_ne<true, 0, 1>(a, n_sm, s);
   if (p.groups == 3) return p.pfn == 2 ? launch_ne<false, 2, 3>(a, n_sm, s) : launch_ne<false, 0, 3>(a, n_sm, s);
   return p.pfn == 2 ? launch_ne<false, 2, 2>(a, n_sm, s) : launch_ne<false, 0, 2>(a, n_sm, s);
 }
