@@ -529,15 +529,19 @@ def test_reduce_parity_with_broad_weights(torch, oracle, config):
         rift.rift_ile_destroy(h)
 
 
-@pytest.mark.parametrize("case", ["tc", "tcs", "tcs_passes", "mma_resident", "mma_resident_two_groups", "mma_stream", "sky", "sky64"])
+@pytest.mark.parametrize("case", ["tc", "tcs", "tcs_passes", "mma_resident", "mma_resident_two_groups", "mma_stream", "mma_stream_one_group", "sky",
+                                  "sky64"])
 def test_repeated_calls_are_bit_identical(torch, oracle, case):
     """The warp-specialised kernels hand data between warps through mbarriers, named barriers, tensor memory and shared
     memory; compute-sanitizer is closed on this pool, so the cheap race detector is determinism: 20 calls on the same inputs
     must return bit-identical lnL (the sorted variant assigns bucket positions by atomics, but no result depends on them)."""
-    modes = {"tcs_passes": _L2 + _L3, "mma_stream": tuple((l, m) for l in (2, 3, 4) for m in range(-l, l + 1))}.get(case, _L2)
+    l234 = tuple((l, m) for l in (2, 3, 4) for m in range(-l, l + 1))
+    modes = {"tcs_passes": _L2 + _L3, "mma_stream": l234, "mma_stream_one_group": l234}.get(case, _L2)
     cfg = synth.with_overrides(synth.CONFIGS[1], modes=modes, n_points=2)
     if case == "mma_resident_two_groups":          # a window of 477 samples: three windows no longer fit beside the Q block
         cfg = synth.with_overrides(cfg, t_window=0.058)
+    if case == "mma_stream_one_group":             # 465 samples = 472 rows > 448: the streamed shape with one group of 15 warps
+        cfg = synth.with_overrides(cfg, t_window=0.0567)
     inp = build(oracle, cfg, n_points=2)
     n, ids = 4099, [1, 0, 1]
     params = np.concatenate([synth.draw_samples(cfg, 90 + s, n)[0] for s in range(len(ids))], axis=1)
@@ -554,7 +558,7 @@ def test_repeated_calls_are_bit_identical(torch, oracle, case):
             name = rift.rift_ile_kernel_name(h)
             want = {"tc": "lnl_tc<f16x3>", "tcs": "lnl_tcs<f16x3>", "tcs_passes": "lnl_tcs<f16x3,passes>",
                     "mma_resident": "lnl_mma<f64,resident>", "mma_resident_two_groups": "lnl_mma<f64,resident>",
-                    "mma_stream": "lnl_mma<f64,stream>", "sky": "lnl_sky<f16x3>",
+                    "mma_stream": "lnl_mma<f64,stream>", "mma_stream_one_group": "lnl_mma<f64,stream>", "sky": "lnl_sky<f16x3>",
                     "sky64": "lnl_sky<f64>"}[case]
             assert name == want, name
             ref = np.concatenate([oracle_eval(oracle, inp, ids[s], params[:, s * n:(s + 1) * n])[0] for s in range(len(ids))])
