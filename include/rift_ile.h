@@ -46,7 +46,7 @@ enum { RIFT_Q_C128 = 0, RIFT_Q_C64 = 1 };           /* storage of Q on the devic
 enum { RIFT_MEM_HOST = 0, RIFT_MEM_DEVICE = 1 };    /* where the Q/U/V arrays passed to create live */
 enum { RIFT_KERNEL_AUTO = 0, RIFT_KERNEL_DIRECT = 1, RIFT_KERNEL_TC = 2, RIFT_KERNEL_TCS = 3,
        RIFT_KERNEL_MMA = 4, RIFT_KERNEL_SKY = 5 };  /* rift_ile_set_kernel */
-enum { RIFT_OPT_TC_CHUNK_MIB = 1,   /* per-chunk workspace of the tensor-core kernels in MiB (default 1024, >= 1) */
+enum { RIFT_OPT_TC_CHUNK_MIB = 1,   /* per-chunk workspace of the tensor-core kernels in MiB (default 4096, >= 1) */
        RIFT_OPT_TC_SORT = 2,        /* 1 (default): AUTO may pick the shift-sorted tensor-core kernel; 0: never */
        RIFT_OPT_QUAD_PROG = 3 };    /* 1 (default): quadratic term of > 8 modes by the pair program; 0: plain pair sum */
 

@@ -48,7 +48,7 @@ struct rift_ile {
   int32_t *tcs_key = nullptr, *tcs_perm = nullptr, *tcs_bkt = nullptr;   // natural-slot keys, sorted-slot permutation, bucket tables
   int64_t tcs_key_cap = 0, tcs_perm_cap = 0, tcs_bkt_cap = 0;
   // options (rift_ile_set_option)
-  int64_t opt_tc_chunk_mib = 1024; // per-chunk workspace of the tensor-core kernels
+  int64_t opt_tc_chunk_mib = 4096; // per-chunk workspace of the tensor-core kernels
   int opt_tc_sort = 1;             // AUTO may pick the shift-sorted tensor-core kernel
   int opt_quad_prog = 1;           // pair program of the quadratic term when M > 8
   const double2 *qp_uv_saved = nullptr;   // the program's W table while the option is off
@@ -496,9 +496,11 @@ int ensure_tc_workspace(rift_ile *h, int64_t n_batches, int blob_words = 0) {
   return RIFT_OK;
 }
 
-// chunks of whole 16-sample batches.  The per-chunk workspace is 1 GiB by default (RIFT_TC_CHUNK_MIB overrides): measured on
-// C1, every extra launch of the fused kernel costs ~30 us (tensor-memory allocation, A-operand load, pipeline fill, tail),
-// far more than keeping the blobs L2-resident saves (64 MiB chunks: 1.39 ms per step, one chunk: 1.24 ms)
+// chunks of whole 16-sample batches.  The per-chunk workspace is at most 4 GiB by default (RIFT_OPT_TC_CHUNK_MIB overrides;
+// a call that needs less allocates less): measured on C1, every extra launch of the fused kernel costs ~30 us (tensor-memory
+// allocation, A-operand load, pipeline fill, tail), far more than keeping the blobs L2-resident saves (64 MiB chunks: 1.39 ms
+// per step, one chunk: 1.24 ms); on C3 (2^24 samples x 6 points) 1 GiB chunks are 103 launches per step and 58.6 ms of lnl_tcs,
+// 4 GiB chunks 26 launches and 57.8 ms, 16 GiB chunks 57.6 ms
 // sizes the workspace of run_chunks_tc for a call shape (also rift_ile_reserve); *cap_out = batches per chunk
 int prepare_tc(rift_ile *h, int32_t n_seg, int64_t n_per_seg, int64_t *cap_out) {
   const int64_t nbps = (n_per_seg + RIFT_TC_NB - 1) / RIFT_TC_NB;

@@ -298,7 +298,7 @@ def test_tcs_chunks_across_segments(torch, oracle):
     h = create(rift, inp, rift.RIFT_PREC_MIXED)
     rift.rift_ile_set_option(h, rift.RIFT_OPT_TC_CHUNK_MIB, 1)   # raised to 8 batches per SM = 1184 batches = 5.4 segments
     got, sh, _ = gpu_eval(torch, h, ids, n, params, K=cfg.n_det, kernel=rift.RIFT_KERNEL_TCS)
-    rift.rift_ile_set_option(h, rift.RIFT_OPT_TC_CHUNK_MIB, 1024)
+    rift.rift_ile_set_option(h, rift.RIFT_OPT_TC_CHUNK_MIB, 4096)
     assert "lnl_tcs" in rift.rift_ile_kernel_name(h)
     one, _, _ = gpu_eval(torch, h, ids, n, params, K=cfg.n_det, kernel=rift.RIFT_KERNEL_TC)
     assert "lnl_tc<" in rift.rift_ile_kernel_name(h)
