@@ -400,7 +400,7 @@ void make_sky_plan(rift_ile *h, double delta_t) {
   p.rows_ext = (p.R0 + (p.n_blocks - 1) * SKY_TBO + dm + SKY_TBR + 8 + 7) & ~7;
   p.point_stride = (int64_t)p.K * p.rows_ext * p.rowb;
   if (lnl_sky_smem_bytes(p) > 227u * 1024u) return;
-  if (!sky_make_cells(dmax, h->sky_cells)) return;
+  if (!sky_make_cells(dmax, SKY_E, h->sky_cells)) return;
   p.ok = 1;
 }
 
@@ -433,7 +433,7 @@ void make_sky64_plan(rift_ile *h, double delta_t) {
   for (int slots = 3; slots >= 2; --slots) {
     p.slots = slots;
     if (lnl_sky64_smem_bytes(p) <= 227u * 1024u) {
-      p.ok = sky_make_cells(dmax, h->sky_cells) ? 1 : 0;
+      p.ok = sky_make_cells(dmax, SKY64_E, h->sky_cells) ? 1 : 0;
       return;
     }
   }

@@ -5,7 +5,8 @@
 // The samples of a chunk arrive bucketed by sky cell (sky_sort.cu): the 64 samples of a batch have relative shifts
 // d_{n,k} = s_k - s_0 = b_k + r_{n,k} with one base b_k per detector and residuals 0 <= r < SKY_E.  Circular window
 // (N_tau = N_t), detector-0 time: x_j = sum_k P_k[(j + b_k + r_{n,k}) mod N_t, n], P_k[t, n] = sum_kappa A_k[t, kappa] B_k[kappa, n].
-// Time is tiled in blocks of 216 window entries.  Per (block, detector) a chunk of 256 consecutive operand rows starting at
+// Time is tiled in blocks of 224 window entries (SKY_TBO = 256 - SKY_E - the 8-row rounding; 15 blocks on C4).
+// Per (block, detector) a chunk of 256 consecutive operand rows starting at
 // row  block start + b_k (rounded down to a multiple of 8: the remainder joins the residuals)  of the circularly extended fp16
 // operand [Q_hi | Q_lo | Q_hi] -- stored as groups of 8 rows x K-major planes of 8 elements, so that a chunk is contiguous --
 // arrives by ONE bulk copy into one of three ring slots; one elected thread contracts it with the coefficient operand
@@ -13,7 +14,7 @@
 // operands from shared memory, 2 row tiles of 128 x 64 samples x K = 16 per step, accumulators double-buffered in tensor
 // memory so that the tensor core works on chunk i + 1 while the 16 warps drain chunk i: tcgen05.ld (thread = row, 16 samples),
 // unshifted store into an exchange buffer [64 samples][256 rows] (lanes = consecutive rows: conflict-free), barrier, then
-// every warp adds  P_k[j + r_{n,k}][n]  for its 4 samples n and the block's 216 window entries j = lane + 32 e into registers
+// every warp adds  P_k[j + r_{n,k}][n]  for its 4 samples n and the block's 224 window entries j = lane + 32 e into registers
 // (again lanes = consecutive rows, whatever the shifts).  After the last detector the block joins the lane's running
 // (max, sum) of 2^(c log2e (x - max)) per sample -- an on-line log-sum-exp, so the window never exists anywhere as a whole.
 // Nothing but Q rows, 23 KB of coefficients per batch and one lnL per sample moves through L2 / HBM.

@@ -4,7 +4,7 @@
 //   a6  x_j = sum_k sum_lm ( B.re Q.re + B.im Q.im ),  B = F_k Y_lm,  Q = Q_{k,lm}[(j0 + s_k + j) mod N_t]   (Eq. (D2))
 //   a7  lnL_tm = c x_max + ln sum_j exp(c (x_j - x_max)) - ln N_tau - q                                   (App. D.2)
 //
-// A sorted batch of 64 slots (relative shifts d_{n,k} = b_k + r_{n,k}, 0 <= r < SKY_E) is processed as two half batches of 32
+// A sorted batch of 64 slots (relative shifts d_{n,k} = b_k + r_{n,k}, 0 <= r < SKY64_E) is processed as two half batches of 32
 // samples.  Per (block of 224 window entries, detector) a chunk of 256 consecutive rows of the circularly extended operand
 // A_k[t, 2m + {0,1}] = {Re, Im} Q_{k,m}[t] (fp64, rows of kappa_p doubles with kappa_p = 4 (mod 8): conflict-free fragment
 // loads) arrives by one bulk copy into a ring slot.  The CTA is two independent groups of 8 warps, each with 16 samples of the
@@ -130,7 +130,7 @@ __global__ void __launch_bounds__(S64_THREADS, 1) lnl_sky64_kernel(const S64Args
     if (tid < SKY_NB * K) {
       const int bkk = bk_s[tid / SKY_NB] == INT32_MAX ? 0 : bk_s[tid / SKY_NB];
       int r = my_d == INT32_MAX ? 0 : my_d - bkk;
-      resid_s[tid] = r < 0 ? 0 : (r > SKY_E - 1 ? SKY_E - 1 : r);   // out of range only for a sample with NaN angles
+      resid_s[tid] = r < 0 ? 0 : (r > SKY64_E - 1 ? SKY64_E - 1 : r);   // out of range only for a sample with NaN angles
     }
     const unsigned char *qpoint = A.q + (int64_t)point * P.point_stride;
     auto issue = [&](int i, uint32_t c) {                        // chunk i = (block i / K, detector i % K) into ring slot c % slots

@@ -132,8 +132,9 @@ struct MmaPlan {
 
 // Sky-sorted, time-tiled tensor-core path (sky_sort.cu, lnl_sky.cu): mixed precision, windows of any length.
 #define SKY_NB 64                // samples per batch (eight 8-column tiles)
-#define SKY_E 32                 // residual shifts of a batch lie in [0, SKY_E)
-#define SKY_TBO 216              // window entries per time block (a multiple of 8)
+#define SKY_E 24                 // mixed mode (lnl_sky): residual shifts of a batch lie in [0, SKY_E)
+#define SKY64_E 32               // fp64 mode (lnl_sky64): its chunks start at any row, so 224 + 32 = 256 rows
+#define SKY_TBO 224              // window entries per time block (a multiple of 8)
 #define SKY_TBR 256              // Q rows per (time block, detector) chunk >= SKY_TBO + SKY_E + 7
 #define SKY_MAX_RINGS 512
 struct SkyCells {                // sky cells of the bucketing pass (sky_sort.cu)
@@ -206,7 +207,7 @@ cudaError_t launch_convert_q_mma(const double *Q_c128, void *dst, const MmaPlan 
 cudaError_t launch_lnl_mma(const MmaPlan &p, const void *q, const Batch &b, const Workspace &ws, double *lnL_out, int n_sm,
                            cudaStream_t s, int *n_launch);
 // sky_sort.cu / lnl_sky.cu
-bool sky_make_cells(double dmax_samples, SkyCells &c);
+bool sky_make_cells(double dmax_samples, int e_max, SkyCells &c);
 cudaError_t launch_sky_sort(const SkyCells &cells, double gmst, const Batch &b, const double *const params[6], int n_lseg,
                             int32_t *key, int32_t *pos, int32_t *count, int32_t *base, int32_t *perm, int64_t cap_slots,
                             int32_t *n_batches, cudaStream_t s, int *n_launch);

@@ -2,10 +2,10 @@
 // Every delay dt_k = -r_k.n/c (step a3) is a Lipschitz function of the source direction n with constant |r_k - r_0|/c for
 // the RELATIVE delay, so samples of one small sky cell have relative shifts d_k = s_k - s_0 within a few samples of one
 // another: a batch of one cell can be contracted by the tensor cores from ONE row range of Q per detector (the batch's
-// smallest shift applied as the row offset) with residual per-sample shifts below SKY_E.  Cells: rings of constant width
+// smallest shift applied as the row offset) with residual per-sample shifts below e_max (SKY_E for lnl_sky, SKY64_E for lnl_sky64).  Cells: rings of constant width
 // delta in declination, each cut into ceil(2 pi cos_max / delta) equal steps of hour angle, so that two directions of a cell
-// are at most sqrt(2) delta apart; delta = (SKY_E - 1) / (sqrt(2) max_k |r_k - r_0| / (c delta_t)) bounds the spread of every
-// d_k inside a cell by SKY_E - 1 (rounding included).
+// are at most sqrt(2) delta apart; delta = (e_max - 1) / (sqrt(2) max_k |r_k - r_0| / (c delta_t)) bounds the spread of every
+// d_k inside a cell by e_max - 1 (rounding included).
 #include "rift_internal.h"
 
 namespace {
@@ -84,9 +84,9 @@ __global__ void __launch_bounds__(256) sky_fill_kernel(int64_t n, const int32_t 
 }  // namespace
 
 // Cells for a bound `dmax` (samples) on |d s_k / d n|: rings and their hour-angle steps.  Returns false if too many rings.
-bool sky_make_cells(double dmax_samples, SkyCells &c) {
+bool sky_make_cells(double dmax_samples, int e_max, SkyCells &c) {
   c = SkyCells{};
-  double delta = (SKY_E - 1) / (1.4142135623730951 * (dmax_samples > 1.0 ? dmax_samples : 1.0));
+  double delta = (e_max - 1) / (1.4142135623730951 * (dmax_samples > 1.0 ? dmax_samples : 1.0));
   if (delta > 0.5) delta = 0.5;
   const int n_rings = (int)std::ceil(3.141592653589793 / delta);
   if (n_rings > SKY_MAX_RINGS) return false;
