@@ -221,6 +221,10 @@ __global__ void __launch_bounds__(SKY_THREADS, 1) lnl_sky_kernel(const SkyArgs A
     }
     __syncthreads();
 
+    // Padding slots sit at the end of a batch (the last batch of a sky cell holds 32 samples on average): a group whose
+    // sample quarter is all padding keeps the barrier protocol of the chunks (tfull / tempty, the ring refills of warp 13)
+    // and skips the drain, the exchange and the log-sum-exp, which leaves the shared-memory pipe to the other groups
+    const bool live = orig_s[16 * grp] >= 0;
     float m_run[SKY_SPW], s_run[SKY_SPW], cl2n[SKY_SPW];
 #pragma unroll
     for (int sp = 0; sp < SKY_SPW; ++sp) {
@@ -241,28 +245,32 @@ __global__ void __launch_bounds__(SKY_THREADS, 1) lnl_sky_kernel(const SkyArgs A
         mbar_wait(tfull + (cnt & 1u), (cnt >> 1) & 1u);
         tc_fence_after();
         float acc[2][2][8];
+        if (live) {
 #pragma unroll
-        for (int mt = 0; mt < 2; ++mt) {
-          const uint32_t ta = tmem_base + t_lane + (cnt & 1u) * 128u + (uint32_t)(mt * SKY_NB + 16 * cg);
-          tc_ld8(ta, acc[mt][0]);
-          tc_ld8(ta + 8, acc[mt][1]);
-        }
+          for (int mt = 0; mt < 2; ++mt) {
+            const uint32_t ta = tmem_base + t_lane + (cnt & 1u) * 128u + (uint32_t)(mt * SKY_NB + 16 * cg);
+            tc_ld8(ta, acc[mt][0]);
+            tc_ld8(ta + 8, acc[mt][1]);
+          }
 #pragma unroll
-        for (int mt = 0; mt < 2; ++mt) {
-          tc_wait_ld8(acc[mt][0]);
-          tc_wait_ld8(acc[mt][1]);
+          for (int mt = 0; mt < 2; ++mt) {
+            tc_wait_ld8(acc[mt][0]);
+            tc_wait_ld8(acc[mt][1]);
+          }
         }
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(tempty + (cnt & 1u));
-        group_bar();                                             // every reader of the group is done with the previous detector
+        if (live) {
+          group_bar();                                           // every reader of the group is done with the previous detector
 #pragma unroll
-        for (int mt = 0; mt < 2; ++mt)
+          for (int mt = 0; mt < 2; ++mt)
 #pragma unroll
-          for (int h = 0; h < 2; ++h)
+            for (int h = 0; h < 2; ++h)
 #pragma unroll
-            for (int c = 0; c < 8; ++c) xst[(8 * h + c) * SKY_TBR + 128 * mt] = acc[mt][h][c];
-        group_bar();                                             // the group's rows of detector k are complete
+              for (int c = 0; c < 8; ++c) xst[(8 * h + c) * SKY_TBR + 128 * mt] = acc[mt][h][c];
+          group_bar();                                           // the group's rows of detector k are complete
+        }
         tc_fence_after();
         if (warp == 13) {                                        // tfull of chunk i was observed: its ring slots are free
           if (elect_one())
@@ -273,6 +281,7 @@ __global__ void __launch_bounds__(SKY_THREADS, 1) lnl_sky_kernel(const SkyArgs A
           __syncwarp();
         }
         // ---- shifted read: x_j += P_k[j + r][n], lanes = consecutive rows
+        if (!live) continue;
 #pragma unroll
         for (int sp = 0; sp < SKY_SPW; ++sp) {
           const int n = SKY_SPW * warp + sp;
@@ -287,6 +296,7 @@ __global__ void __launch_bounds__(SKY_THREADS, 1) lnl_sky_kernel(const SkyArgs A
         }
       }
       // ---- the block joins the running log-sum-exp of this lane, per sample
+      if (!live) continue;
       const int j0 = blk * SKY_TBO + lane;
       const int j_end = min(n_t, (blk + 1) * SKY_TBO);
 #pragma unroll
