@@ -147,6 +147,7 @@ __global__ void __launch_bounds__(S64_THREADS, 1) lnl_sky64_kernel(const S64Args
     for (int half = 0; half < 2; ++half) {
       // ---- coefficients of the half batch as B fragments cs[k][s][n][4] (zero beyond 2 M)
       __syncthreads();                                           // the previous half batch is done with cs, xb and the ring
+      if (half == 1 && orig_s[32] < 0) break;                    // padding sits at the end of a batch: nothing in this half
       for (int idx = tid; idx < K * KS * S64_NB * 4; idx += S64_THREADS) {
         const int e = idx & 3, n = (idx >> 2) % S64_NB, ks = (idx >> 2) / S64_NB, s = ks % KS, k = ks / KS;
         const int kap = 4 * s + e;
@@ -156,6 +157,24 @@ __global__ void __launch_bounds__(S64_THREADS, 1) lnl_sky64_kernel(const S64Args
         for (int i = 0; i < slots && i < n_chunks; ++i) issue(i, cnt + i);
       __syncthreads();
 
+      // A group whose 16 samples are all padding only keeps the ring's bookkeeping: one thread counts the group's consumption
+      // of every chunk once it has landed (and refills the slot if the other group was there first); the FP64 unit is the
+      // other group's meanwhile
+      if (orig_s[32 * half + 16 * grp] < 0) {
+        if (gtid == 0)
+          for (int i = 0; i < n_chunks; ++i) {
+            const uint32_t c = cnt + (uint32_t)i, slot = c % (uint32_t)slots;
+            mbar_wait(full + slot, (c / (uint32_t)slots) & 1u);
+            __threadfence_block();
+            if (atomicAdd(done + slot, 1) == 1) {
+              done[slot] = 0;
+              __threadfence_block();
+              if (i + slots < n_chunks) issue(i + slots, c + (uint32_t)slots);
+            }
+          }
+        cnt += (uint32_t)n_chunks;
+        continue;
+      }
       float m_run[S64_SPW];
       double s_run[S64_SPW], cl2n[S64_SPW];
 #pragma unroll
